@@ -1,0 +1,158 @@
+// A1 polyphase resampler, A5/A6 peak merge + trigger compaction, state reset.
+// Shared by the fp32 and fp16 paths.  See lloid_internal.h for the chunk-local coordinates.
+#include "lloid_internal.h"
+#include "../../include/lloid.h"
+
+namespace lloid {
+
+// ------------------------------------------------------------------------------------------------
+// A1  x^s[j] = sqrt(d) sum_n lp[n] x[d j - n]          (include/lloid.h A1; "downsamples")
+//
+// One CTA produces 256 consecutive outputs of one (rate, detector).  The strain segment it needs,
+// d*256 + 2 K d samples, is read once with coalesced loads and stored de-interleaved by decimation
+// phase, xsm[phi][m] = x[d (jj0 - K + m) + phi], so that in the tap loop thread t reads xsm[phi][t + a]:
+// consecutive threads touch consecutive banks (a stride-d access would be a d-way bank conflict).
+// Taps are pre-scaled by sqrt(d); tap index u = d a + phi.  Output in fp32 and, for the fp16 path, fp16.
+// ------------------------------------------------------------------------------------------------
+constexpr int kResBlock = 256;
+
+__global__ void __launch_bounds__(kResBlock)
+resample_kernel(const RateParams* __restrict__ rates, const float* __restrict__ xw, int xw_pitch,
+                int xw_valid, int k_dn, int c, int want_f16)
+{
+  const RateParams R = rates[blockIdx.z];
+  const int det = blockIdx.y;
+  const int d = R.d;
+  const int jj_lo = R.jj_lo_fixed;
+  const int jj_hi = R.jj_hi_off + c / d;
+  const int jj0 = jj_lo + blockIdx.x * kResBlock;
+  if (jj0 >= jj_hi) return;
+  const float* x = xw + (size_t)det * xw_pitch;
+  const int t = threadIdx.x;
+
+  if (d == 1) {                                   // fp16 copy of the full-rate stream (fp16 path only)
+    const int jj = jj0 + t;
+    if (want_f16 && jj < jj_hi && jj >= 0 && jj < R.xs_len) {
+      const float v = (jj < xw_valid) ? x[jj] : 0.f;
+      R.xs16[(size_t)det * R.xs_len + jj] = __float2half_rn(v);
+    }
+    return;
+  }
+
+  extern __shared__ float xsm[];
+  const int mlen = kResBlock + 2 * k_dn + 1;       // odd row stride: conflict-free transposed stores
+  const int seg = d * (kResBlock + 2 * k_dn) + 1;
+  const int base = d * (jj0 - k_dn);               // xw index of segment element 0
+  for (int i = t; i < seg; i += kResBlock) {
+    const int gi = base + i;
+    const float v = (gi >= 0 && gi < xw_valid) ? x[gi] : 0.f;
+    xsm[(i % d) * mlen + (i / d)] = v;
+  }
+  __syncthreads();
+
+  const float* __restrict__ taps = R.taps;
+  float acc = 0.f;
+  for (int a = 0; a < 2 * k_dn; ++a) {
+    const float* tp = taps + a * d;
+    for (int phi = 0; phi < d; ++phi)
+      acc = fmaf(__ldg(tp + phi), xsm[phi * mlen + t + a], acc);
+  }
+  acc = fmaf(__ldg(taps + 2 * k_dn * d), xsm[t + 2 * k_dn], acc);   // last tap: a = 2K, phi = 0
+
+  const int jj = jj0 + t;
+  if (jj < jj_hi && jj >= 0 && jj < R.xs_len) {
+    const size_t o = (size_t)det * R.xs_len + jj;
+    R.xs32[o] = acc;
+    if (want_f16) R.xs16[o] = __float2half_rn(acc);
+  }
+}
+
+void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
+                     const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
+                     bool want_f16, cudaStream_t st, int64_t* launches)
+{
+  int max_blocks = 0, max_d = 1;
+  bool any = false;
+  for (int r = 0; r < n_rates; ++r) {
+    const RateParams& R = rates_host[r];
+    if (R.d == 1 && !want_f16) continue;
+    any = true;
+    const int span = R.jj_hi_off + c / R.d - R.jj_lo_fixed;
+    const int nb = (span + kResBlock - 1) / kResBlock;
+    if (nb > max_blocks) max_blocks = nb;
+    if (R.d > max_d) max_d = R.d;
+  }
+  if (!any || max_blocks <= 0) return;
+  const size_t smem = sizeof(float) * (size_t)max_d * (kResBlock + 2 * k_dn + 1);
+  static size_t configured = 0;
+  if (smem > 48 * 1024 && smem > configured) {
+    cudaFuncSetAttribute(resample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = smem;
+  }
+  dim3 grid(max_blocks, n_det, n_rates);
+  resample_kernel<<<grid, kResBlock, smem, st>>>(rates_dev, xw, xw_pitch, xw_valid, k_dn, c, want_f16 ? 1 : 0);
+  ++*launches;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A5/A6  merge the per-tile partial maxima into the running in-window maximum of every template,
+// emit a trigger whenever a window completes and |rho| > theta (strict), reset.
+// One thread per (bin, detector, template); tiles are visited in time order so that the first
+// (lowest k) maximum wins ties (R8).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+merge_peaks_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
+                   int tiles_cap, int n_tiles, int c, long long k_a, int W, float theta,
+                   PeakState* __restrict__ state, int n_det, lloid_trigger_t* __restrict__ trig,
+                   long long capacity, unsigned long long* __restrict__ count)
+{
+  const int bd = blockIdx.y;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  const BinParams B = bp[bd];
+  if (p >= B.n_templates) return;
+  PeakState s = state[(size_t)bd * max_templates + p];
+  for (int g = 0; g < n_tiles; ++g) {
+    const Peak pk = partials[((size_t)bd * tiles_cap + g) * max_templates + p];
+    if (pk.q > s.q) { s.q = pk.q; s.re = pk.re; s.im = pk.im; s.k = k_a + pk.kappa; }
+    int kend = (g + 1) * kTimeTile; if (kend > c) kend = c;
+    if (((k_a + kend) % W) == 0) {                  // a peak window [wW, (w+1)W) is complete
+      if (s.q >= 0.f && sqrtf(s.q) > theta) {
+        const unsigned long long idx = atomicAdd(count, 1ull);
+        if ((long long)idx < capacity) {
+          lloid_trigger_t t;
+          t.bin = bd / n_det; t.detector = bd % n_det; t.template_idx = p; t.reserved = 0;
+          t.sample = s.k; t.snr_re = s.re; t.snr_im = s.im;
+          trig[idx] = t;
+        }
+      }
+      s.q = -1.f; s.re = 0.f; s.im = 0.f; s.k = -1;
+    }
+  }
+  state[(size_t)bd * max_templates + p] = s;
+}
+
+void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
+                        int tiles_cap, int n_tiles, int c, int64_t k_a, int W, float theta,
+                        PeakState* state, int n_det, void* triggers, int64_t capacity,
+                        unsigned long long* count, cudaStream_t st, int64_t* launches)
+{
+  dim3 grid((max_templates + 127) / 128, n_bd);
+  merge_peaks_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, tiles_cap, n_tiles, c,
+                                          (long long)k_a, W, theta, state, n_det,
+                                          (lloid_trigger_t*)triggers, (long long)capacity, count);
+  ++*launches;
+}
+
+__global__ void reset_state_kernel(PeakState* s, long long n)
+{
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { PeakState e; e.q = -1.f; e.re = 0.f; e.im = 0.f; e.pad = 0; e.k = -1; s[i] = e; }
+}
+
+void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st)
+{
+  if (n <= 0) return;
+  reset_state_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(state, (long long)n);
+}
+
+}  // namespace lloid

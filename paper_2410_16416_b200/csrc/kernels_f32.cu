@@ -1,0 +1,346 @@
+// fp32 path (LLOID_F32): A2 basis FIR and A3+A4+A5 reconstruction / upsample-accumulate / |rho|^2 /
+// windowed max on the CUDA cores (FFMA).  TF32 tensor MMAs keep a 10-bit mantissa and cannot meet the
+// 1e-3 absolute SNR parity of BASELINE.json's fp32 path, so this path is plain fp32.
+// The fp16 tensor-core path lives in kernels_f16.cu.
+#include "lloid_internal.h"
+
+namespace lloid {
+
+// ------------------------------------------------------------------------------------------------
+// A2  y^s_l[j] = sum_t U^s[l,t] x^s[j - n_s + t]                     ("cross-correlates")
+//
+// CTA tile: 128 low-rate outputs x 32 basis filters, 128 threads, thread tile 8 (time) x 4 (l).
+// The strain window of the tile (128 + n_s samples) is staged once in shared memory; U streams
+// through in 64-tap chunks, transposed to [t][l].  Per 8 taps a thread reads a 16-sample strain
+// window (4 LDS.128) and 8 float4 of U, and issues 256 FMAs: the Toeplitz operand is never
+// materialised anywhere.
+// ------------------------------------------------------------------------------------------------
+constexpr int FIR_TM = 128, FIR_TL = 32, FIR_KC = 64, FIR_US = 36;
+
+__global__ void __launch_bounds__(128)
+fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int c, int zs_len)
+{
+  const SliceParams P = sp[blockIdx.z];
+  const int rows_needed = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+  const int r0 = blockIdx.x * FIR_TM;
+  const int l0 = blockIdx.y * FIR_TL;
+  if (r0 >= rows_needed || l0 >= P.L_pad) return;
+
+  extern __shared__ __align__(16) float smem_f[];
+  float* zs = smem_f;                 // [zs_len]
+  float* Us = smem_f + zs_len;        // [FIR_KC][FIR_US]
+  const RateParams R = rates[P.rate_idx];
+  const float* __restrict__ xs = R.xs32 + (size_t)P.det * R.xs_len;
+  const int tid = threadIdx.x;
+  const int n_taps = P.n_taps;
+  const int jj_start = P.jjY0 + r0 - n_taps;
+  for (int i = tid; i < zs_len; i += 128) {
+    const int idx = jj_start + i;
+    zs[i] = (i < FIR_TM + n_taps && idx >= 0 && idx < R.xs_len) ? xs[idx] : 0.f;
+  }
+
+  const int tl = tid & 7, tj = tid >> 3;
+  float acc[8][4];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) { acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f; }
+
+  const float* __restrict__ U = P.U32;
+  for (int t0 = 0; t0 < n_taps; t0 += FIR_KC) {
+    __syncthreads();
+#pragma unroll 4
+    for (int i = 0; i < (FIR_KC * FIR_TL) / 128; ++i) {
+      const int e = tid + 128 * i;
+      const int ll = e / FIR_KC, tt = e % FIR_KC;
+      const int t = t0 + tt;
+      Us[tt * FIR_US + ll] = (t < n_taps) ? __ldg(U + (size_t)(l0 + ll) * n_taps + t) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll 2
+    for (int tt8 = 0; tt8 < FIR_KC; tt8 += 8) {
+      float zw[16];
+      const float4* zp = reinterpret_cast<const float4*>(zs + tj * 8 + t0 + tt8);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float4 q = zp[v];
+        zw[4 * v] = q.x; zw[4 * v + 1] = q.y; zw[4 * v + 2] = q.z; zw[4 * v + 3] = q.w;
+      }
+#pragma unroll
+      for (int tt = 0; tt < 8; ++tt) {
+        const float4 u = *reinterpret_cast<const float4*>(Us + (tt8 + tt) * FIR_US + tl * 4);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          acc[j][0] = fmaf(zw[j + tt], u.x, acc[j][0]);
+          acc[j][1] = fmaf(zw[j + tt], u.y, acc[j][1]);
+          acc[j][2] = fmaf(zw[j + tt], u.z, acc[j][2]);
+          acc[j][3] = fmaf(zw[j + tt], u.w, acc[j][3]);
+        }
+      }
+    }
+  }
+  float* Y = reinterpret_cast<float*>(P.Y);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int r = r0 + tj * 8 + j;
+    if (r < P.y_rows_cap)
+      *reinterpret_cast<float4*>(Y + (size_t)r * P.L_pad + l0 + tl * 4) =
+          make_float4(acc[j][0], acc[j][1], acc[j][2], acc[j][3]);
+  }
+}
+
+void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
+                    const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches)
+{
+  (void)n_det;
+  int max_rows = 0, max_lt = 0, max_taps = 0;
+  for (int i = 0; i < n_problems; ++i) {
+    const SliceParams& P = sp_host[i];
+    const int rows = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+    if (rows > max_rows) max_rows = rows;
+    if (P.L_pad / FIR_TL > max_lt) max_lt = P.L_pad / FIR_TL;
+    if (P.n_taps > max_taps) max_taps = P.n_taps;
+  }
+  const int zs_len = FIR_TM + ((max_taps + FIR_KC - 1) / FIR_KC) * FIR_KC + 16;
+  const size_t smem = sizeof(float) * ((size_t)zs_len + FIR_KC * FIR_US);
+  static size_t configured = 0;
+  if (smem > 48 * 1024 && smem > configured) {
+    cudaFuncSetAttribute(fir_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = smem;
+  }
+  dim3 grid((max_rows + FIR_TM - 1) / FIR_TM, max_lt, n_problems);
+  fir_f32_kernel<<<grid, 128, smem, st>>>(sp_dev, rates_dev, c, zs_len);
+  ++*launches;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A3 + A4 + A5 fused:  rho^s = R^s y^s at the slice rate, interpolated to f0 and summed over slices
+// in registers, then |rho|^2 and the per-template maximum of the tile.  The dense SNR never leaves
+// the SM (the SNR series is too large to move; here it is not even written to HBM).
+//
+// CTA tile: 64 real rows (32 templates) x 128 f0 samples, 256 threads as 16 (row groups of 4) x
+// 16 (column groups of 8); each thread keeps a 4 x 8 fp32 accumulator of the f0-rate SNR.
+// Per slice: a K-chunked SGEMM R^s[64 x L] * y^s[L x Ks] with Ks = 128 (d = 1, accumulated
+// directly) or 128/d + 16 low-rate samples (d > 1, staged through shared memory and interpolated
+// with the 16-tap polyphase weights w_phi[i] = d lp[d i + phi]).
+// ------------------------------------------------------------------------------------------------
+constexpr int RC_RT = 64, RC_CT = kTimeTile, RC_KC = 32, RC_RS = RC_RT + 4, RC_YS = RC_CT + 4;
+constexpr int RC_KSMAX = RC_CT / 2 + 2 * kKUp;   // 80 low-rate samples at d = 2
+constexpr int RC_RHO_S = RC_KSMAX + 1;
+
+template <int D>
+__device__ __forceinline__ void upsample_acc(float (&acc)[4][8], const float* __restrict__ rho,
+                                             const float* __restrict__ wsm, int ty, int tx)
+{
+  // columns kl = 8 tx + cc;  low-rate local index ml = kl / D, phase phi = kl % D
+  // c[kl] += sum_{i=-8}^{7} wsm[(i+8)*32 + phi] * rho[row][ml + 8 - i]
+  if (D >= 8) {
+    const int ml = (8 * tx) / D;
+    const int phi0 = (8 * tx) % D;
+#pragma unroll
+    for (int i = -kKUp; i < kKUp; ++i) {
+      const float4 w0 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0);
+      const float4 w1 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0 + 4);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        const float v = rho[(4 * ty + r) * RC_RHO_S + ml + kKUp - i];
+        acc[r][0] = fmaf(w0.x, v, acc[r][0]); acc[r][1] = fmaf(w0.y, v, acc[r][1]);
+        acc[r][2] = fmaf(w0.z, v, acc[r][2]); acc[r][3] = fmaf(w0.w, v, acc[r][3]);
+        acc[r][4] = fmaf(w1.x, v, acc[r][4]); acc[r][5] = fmaf(w1.y, v, acc[r][5]);
+        acc[r][6] = fmaf(w1.z, v, acc[r][6]); acc[r][7] = fmaf(w1.w, v, acc[r][7]);
+      }
+    }
+  } else {
+    constexpr int NM = 8 / D;                     // distinct low-rate indices under the 8 columns
+    const int ml0 = (8 * tx) / D;
+#pragma unroll
+    for (int i = -kKUp; i < kKUp; ++i) {
+      float w[D];
+#pragma unroll
+      for (int p = 0; p < D; ++p) w[p] = wsm[(i + kKUp) * 32 + p];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+#pragma unroll
+        for (int m = 0; m < NM; ++m) {
+          const float v = rho[(4 * ty + r) * RC_RHO_S + ml0 + m + kKUp - i];
+#pragma unroll
+          for (int p = 0; p < D; ++p) acc[r][m * D + p] = fmaf(w[p], v, acc[r][m * D + p]);
+        }
+      }
+    }
+  }
+}
+
+template <int NC>
+__device__ __forceinline__ void gemm_lowrate(const float* __restrict__ Rs, const float* __restrict__ Ys,
+                                             float (&tmp)[4][5], int ty, int tx)
+{
+#pragma unroll 8
+  for (int ll = 0; ll < RC_KC; ++ll) {
+    const float4 a = *reinterpret_cast<const float4*>(Rs + ll * RC_RS + 4 * ty);
+#pragma unroll
+    for (int cc = 0; cc < NC; ++cc) {
+      const float b = Ys[ll * RC_YS + tx + 16 * cc];
+      tmp[0][cc] = fmaf(a.x, b, tmp[0][cc]); tmp[1][cc] = fmaf(a.y, b, tmp[1][cc]);
+      tmp[2][cc] = fmaf(a.z, b, tmp[2][cc]); tmp[3][cc] = fmaf(a.w, b, tmp[3][cc]);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict__ bp,
+                 const float* const* __restrict__ upw, Peak* __restrict__ partials, int tiles_cap,
+                 int max_templates, int c, long long k_a, Capture cap)
+{
+  const int bd = blockIdx.z;
+  const BinParams B = bp[bd];
+  const int row0 = blockIdx.y * RC_RT;
+  if (row0 >= 2 * B.n_templates) return;
+  const int g = blockIdx.x;
+  const int kap0 = g * RC_CT;
+
+  extern __shared__ __align__(16) float smem_r[];
+  float* Rs = smem_r;                               // [RC_KC][RC_RS]
+  float* Ys = Rs + RC_KC * RC_RS;                   // [RC_KC][RC_YS]
+  float* rho = Ys + RC_KC * RC_YS;                  // [RC_RT][RC_RHO_S]
+  float* wsm = rho + RC_RT * RC_RHO_S;              // [16][32]
+
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  float acc[4][8];
+#pragma unroll
+  for (int r = 0; r < 4; ++r)
+#pragma unroll
+    for (int cc = 0; cc < 8; ++cc) acc[r][cc] = 0.f;
+
+  for (int s = 0; s < B.n_slices; ++s) {
+    const SliceParams P = sp[B.first_slice + s];
+    const int d = P.d;
+    const int Ks = (d == 1) ? RC_CT : (RC_CT >> P.log2d) + 2 * kKUp;
+    const int r0 = (d == 1) ? kap0 : (kap0 >> P.log2d);
+    const float* __restrict__ R = P.R32;
+    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y);
+    const int Lp = P.L_pad;
+    float tmp[4][5];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int cc = 0; cc < 5; ++cc) tmp[r][cc] = 0.f;
+
+    for (int l0 = 0; l0 < Lp; l0 += RC_KC) {
+      __syncthreads();                               // also: previous slice's upsample has finished
+      if (d > 1 && l0 == 0) {                        // stage this slice's interpolation weights
+        const float* __restrict__ w = upw[P.log2d];  // [16][d]
+        for (int e = tid; e < 16 * d; e += 256) wsm[(e / d) * 32 + (e % d)] = __ldg(w + e);
+      }
+#pragma unroll
+      for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
+        const int e = tid + 256 * i;
+        const int ll = e % RC_KC, row = e / RC_KC;
+        Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
+      }
+      for (int e = tid; e < Ks * RC_KC; e += 256) {
+        const int ll = e % RC_KC, col = e / RC_KC;
+        const int r = r0 + col;
+        Ys[ll * RC_YS + col] = (r < P.y_rows_cap) ? Y[(size_t)r * Lp + l0 + ll] : 0.f;
+      }
+      __syncthreads();
+      if (d == 1) {
+#pragma unroll 8
+        for (int ll = 0; ll < RC_KC; ++ll) {
+          const float4 a = *reinterpret_cast<const float4*>(Rs + ll * RC_RS + 4 * ty);
+          const float4 b0 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx);
+          const float4 b1 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx + 4);
+          const float av[4] = {a.x, a.y, a.z, a.w};
+          const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+          for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 8; ++cc) acc[r][cc] = fmaf(av[r], bv[cc], acc[r][cc]);
+        }
+      } else if (d == 2) gemm_lowrate<5>(Rs, Ys, tmp, ty, tx);
+      else if (d == 4) gemm_lowrate<3>(Rs, Ys, tmp, ty, tx);
+      else gemm_lowrate<2>(Rs, Ys, tmp, ty, tx);
+    }
+    if (d > 1) {
+      const int NC = (d == 2) ? 5 : (d == 4) ? 3 : 2;
+      __syncthreads();                               // previous slice's readers of rho are done
+      for (int cc = 0; cc < NC; ++cc) {
+        const int col = tx + 16 * cc;
+        if (col < Ks) {
+#pragma unroll
+          for (int r = 0; r < 4; ++r) rho[(4 * ty + r) * RC_RHO_S + col] = tmp[r][cc];
+        }
+      }
+      __syncthreads();
+      switch (d) {
+        case 2: upsample_acc<2>(acc, rho, wsm, ty, tx); break;
+        case 4: upsample_acc<4>(acc, rho, wsm, ty, tx); break;
+        case 8: upsample_acc<8>(acc, rho, wsm, ty, tx); break;
+        case 16: upsample_acc<16>(acc, rho, wsm, ty, tx); break;
+        default: upsample_acc<32>(acc, rho, wsm, ty, tx); break;
+      }
+    }
+  }
+
+  // ---- epilogue: |rho|^2, first maximum over the tile's valid columns, one Peak per template
+  const int valid = min(RC_CT, c - kap0);           // ragged last tile of a chunk
+#pragma unroll
+  for (int t = 0; t < 2; ++t) {
+    float bq = -1.f, bre = 0.f, bim = 0.f;
+    int bk = 0x7fffffff;
+#pragma unroll
+    for (int cc = 0; cc < 8; ++cc) {
+      const int kl = 8 * tx + cc;
+      const float re = acc[2 * t][cc], im = acc[2 * t + 1][cc];
+      const float q = re * re + im * im;
+      if (kl < valid && q > bq) { bq = q; bre = re; bim = im; bk = kap0 + kl; }
+    }
+#pragma unroll
+    for (int off = 8; off >= 1; off >>= 1) {
+      const float oq = __shfl_xor_sync(0xffffffffu, bq, off);
+      const float ore = __shfl_xor_sync(0xffffffffu, bre, off);
+      const float oim = __shfl_xor_sync(0xffffffffu, bim, off);
+      const int ok = __shfl_xor_sync(0xffffffffu, bk, off);
+      if (oq > bq || (oq == bq && ok < bk)) { bq = oq; bre = ore; bim = oim; bk = ok; }
+    }
+    const int p = (row0 + 4 * ty) / 2 + t;
+    if (tx == 0 && p < B.n_templates) {
+      Peak pk; pk.q = bq; pk.kappa = bk; pk.re = bre; pk.im = bim;
+      partials[((size_t)bd * tiles_cap + g) * max_templates + p] = pk;
+    }
+  }
+
+  if (cap.snr != nullptr && cap.bd == bd) {         // test-only dense dump from the same accumulators
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int row = row0 + 4 * ty + r;
+      if (row >= cap.rows) continue;
+#pragma unroll
+      for (int cc = 0; cc < 8; ++cc) {
+        const int kl = 8 * tx + cc;
+        const long long k = k_a + kap0 + kl;
+        if (kl < valid && k >= cap.k_begin && k < cap.k_begin + cap.n)
+          cap.snr[(size_t)row * cap.n + (k - cap.k_begin)] = acc[r][cc];
+      }
+    }
+  }
+}
+
+void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
+                      int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap,
+                      cudaStream_t st, int64_t* launches)
+{
+  (void)bp_host;
+  const size_t smem = sizeof(float) * (RC_KC * RC_RS + RC_KC * RC_YS + RC_RT * RC_RHO_S + 16 * 32);
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(recon_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = true;
+  }
+  const int n_tiles = (c + RC_CT - 1) / RC_CT;
+  dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
+  recon_f32_kernel<<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
+                                           c, (long long)k_a, cap);
+  ++*launches;
+}
+
+}  // namespace lloid

@@ -1,0 +1,584 @@
+// Host side of the C ABI in include/lloid.h: bank construction, packing, the chunk scheduler that
+// drives the kernels, history carry (A8), profiling hooks.  No torch types, no CPU fallback.
+#include "../../include/lloid.h"
+#include "lloid_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace lloid;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...)
+{
+  char buf[512];
+  va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CU(call)                                                                              \
+  do { cudaError_t e_ = (call);                                                               \
+       if (e_ != cudaSuccess) return fail(LLOID_ECUDA, "%s failed: %s (%s:%d)", #call,        \
+                                          cudaGetErrorString(e_), __FILE__, __LINE__); } while (0)
+
+inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+// lp_{d,K}[n], n = -K d..K d (index n + K d): Hann-windowed sinc, unit DC gain (include/lloid.h; DESIGN R1).
+// Written independently of oracle/ (no shared code): double precision, evaluated once at finalize.
+std::vector<double> lowpass(int d, int K)
+{
+  const int half = K * d;
+  std::vector<double> lp(2 * half + 1);
+  const double pi = 3.14159265358979323846;
+  double sum = 0.0;
+  for (int n = -half; n <= half; ++n) {
+    const double x = (double)n / d;
+    const double sinc = (n == 0) ? 1.0 : std::sin(pi * x) / (pi * x);
+    const double v = (1.0 / d) * sinc * 0.5 * (1.0 + std::cos(pi * n / (double)half));
+    lp[n + half] = v; sum += v;
+  }
+  for (double& v : lp) v /= sum;
+  return lp;
+}
+
+struct SliceHost { int rate, d, log2d, n_taps, L, L_pad; int64_t end_delay; };
+struct BinHost { int N, S, rows_pad; int64_t M; std::vector<SliceHost> slices; };
+
+}  // namespace
+
+struct lloid_bank {
+  lloid_bank_config_t cfg{};
+  std::vector<BinHost> bins;
+  bool finalized = false;
+  bool f16 = false;
+  int n_bd = 0, max_templates = 0, max_rows_pad = 0, d_max = 1;
+  std::vector<SliceParams> sp_host;
+  std::vector<BinParams> bp_host;
+  std::vector<uint8_t> uploaded;
+  std::vector<RateParams> rates_host;
+  SliceParams* sp_dev = nullptr;
+  BinParams* bp_dev = nullptr;
+  RateParams* rates_dev = nullptr;
+  float* xw = nullptr;
+  float* hist = nullptr;
+  int H = 0, C = 0, xw_pitch = 0, tiles_cap = 0;
+  PeakState* state = nullptr;
+  Peak* partials = nullptr;
+  const float** upw_dev = nullptr;
+  std::vector<void*> owned;
+  int64_t consumed = 0, bytes = 0, last_launches = 0;
+  Capture cap{nullptr, 0, 0, -1, 0};
+  float* stage_strain = nullptr; size_t stage_strain_elems = 0;
+  lloid_trigger_t* stage_trig = nullptr; int64_t stage_trig_cap = 0;
+  unsigned long long* stage_count = nullptr;
+  bool prof = false;
+  std::vector<cudaEvent_t> events; size_t events_used = 0;
+  F16Plan* plan16 = nullptr;
+
+  int slice_index(int bin, int det, int s) const { return bp_host[bin * cfg.n_detectors + det].first_slice + s; }
+};
+
+namespace {
+
+int dev_alloc(lloid_bank* b, void** p, size_t n, bool zero)
+{
+  if (n == 0) n = 16;
+  cudaError_t e = cudaMalloc(p, n);
+  if (e != cudaSuccess) return fail(LLOID_ENOMEM, "cudaMalloc(%zu) failed: %s", n, cudaGetErrorString(e));
+  if (zero) { e = cudaMemset(*p, 0, n); if (e != cudaSuccess) return fail(LLOID_ECUDA, "cudaMemset: %s", cudaGetErrorString(e)); }
+  b->owned.push_back(*p);
+  b->bytes += (int64_t)n;
+  return LLOID_OK;
+}
+
+int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const double* recon,
+                  const float** U32, const float** R32, const __half** U16, const __half** R16)
+{
+  const BinHost& B = b->bins[bin];
+  const SliceHost& S = B.slices[slice];
+  const size_t nu = (size_t)S.L_pad * S.n_taps, nr = (size_t)B.rows_pad * S.L_pad;
+  *U32 = nullptr; *R32 = nullptr; *U16 = nullptr; *R16 = nullptr;
+  if (!b->f16) {
+    std::vector<float> u(nu, 0.f), r(nr, 0.f);
+    for (int l = 0; l < S.L; ++l)
+      for (int t = 0; t < S.n_taps; ++t) u[(size_t)l * S.n_taps + t] = (float)basis[(size_t)l * S.n_taps + t];
+    for (int i = 0; i < 2 * B.N; ++i)
+      for (int l = 0; l < S.L; ++l) r[(size_t)i * S.L_pad + l] = (float)recon[(size_t)i * S.L + l];
+    void *du, *dr;
+    int rc = dev_alloc(b, &du, nu * 4, false); if (rc) return rc;
+    rc = dev_alloc(b, &dr, nr * 4, false); if (rc) return rc;
+    CU(cudaMemcpy(du, u.data(), nu * 4, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(dr, r.data(), nr * 4, cudaMemcpyHostToDevice));
+    *U32 = (const float*)du; *R32 = (const float*)dr;
+  } else {
+    std::vector<__half> u(nu, __float2half(0.f)), r(nr, __float2half(0.f));
+    for (int l = 0; l < S.L; ++l)
+      for (int t = 0; t < S.n_taps; ++t) u[(size_t)l * S.n_taps + t] = __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+    for (int i = 0; i < 2 * B.N; ++i)
+      for (int l = 0; l < S.L; ++l) r[(size_t)i * S.L_pad + l] = __float2half_rn((float)recon[(size_t)i * S.L + l]);
+    void *du, *dr;
+    int rc = dev_alloc(b, &du, nu * 2, false); if (rc) return rc;
+    rc = dev_alloc(b, &dr, nr * 2, false); if (rc) return rc;
+    CU(cudaMemcpy(du, u.data(), nu * 2, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(dr, r.data(), nr * 2, cudaMemcpyHostToDevice));
+    *U16 = (const __half*)du; *R16 = (const __half*)dr;
+  }
+  return LLOID_OK;
+}
+
+int check_ids(const lloid_bank* b, int bin, int det, int slice)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (bin < 0 || bin >= b->cfg.n_bins) return fail(LLOID_EINVAL, "bin %d out of range", bin);
+  if (det < 0 || det >= b->cfg.n_detectors) return fail(LLOID_EINVAL, "detector %d out of range", det);
+  if (slice < 0 || slice >= b->bins[bin].S) return fail(LLOID_EINVAL, "slice %d out of range", slice);
+  return LLOID_OK;
+}
+
+cudaEvent_t next_event(lloid_bank* b, cudaStream_t st)
+{
+  if (b->events_used == b->events.size()) {
+    cudaEvent_t e; cudaEventCreate(&e); b->events.push_back(e);
+  }
+  cudaEvent_t e = b->events[b->events_used++];
+  cudaEventRecord(e, st);
+  return e;
+}
+
+int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int64_t k_a,
+                  lloid_trigger_t* trig, int64_t capacity, unsigned long long* count, cudaStream_t st)
+{
+  const int D = b->cfg.n_detectors;
+  const size_t wp = (size_t)b->xw_pitch * 4;
+  // xw = [history | chunk]; then save the new history (last H samples of [history | chunk])
+  CU(cudaMemcpy2DAsync(b->xw, wp, b->hist, (size_t)b->H * 4, (size_t)b->H * 4, D, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpy2DAsync(b->xw + b->H, wp, strain, (size_t)pitch * 4, (size_t)c * 4, D, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpy2DAsync(b->hist, (size_t)b->H * 4, b->xw + c, wp, (size_t)b->H * 4, D, cudaMemcpyDeviceToDevice, st));
+  if (b->prof) next_event(b, st);
+  launch_resample(b->rates_dev, b->rates_host.data(), (int)b->rates_host.size(), b->xw, b->xw_pitch,
+                  b->H + c, D, b->cfg.k_down, c, b->f16, st, &b->last_launches);
+  if (b->prof) next_event(b, st);
+  const int n_prob = (int)b->sp_host.size();
+  const int n_tiles = (c + kTimeTile - 1) / kTimeTile;
+  if (!b->f16) {
+    launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, c, st, &b->last_launches);
+    if (b->prof) next_event(b, st);
+    launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
+                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st, &b->last_launches);
+  } else {
+    if (launch_fir_f16(b->plan16, b->sp_dev, b->rates_dev, b->rates_host.data(), c, st, &b->last_launches))
+      return fail(LLOID_ECUDA, "fp16 FIR launch failed");
+    if (b->prof) next_event(b, st);
+    if (launch_recon_f16(b->plan16, b->sp_dev, b->bp_dev, b->upw_dev, b->partials, b->tiles_cap, c, k_a,
+                         b->cap, st, &b->last_launches))
+      return fail(LLOID_ECUDA, "fp16 reconstruction launch failed");
+  }
+  if (b->prof) next_event(b, st);
+  launch_merge_peaks(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, n_tiles, c, k_a,
+                     b->cfg.peak_window, b->cfg.snr_threshold, b->state, D, trig, capacity, count, st,
+                     &b->last_launches);
+  if (b->prof) next_event(b, st);
+  CU(cudaGetLastError());
+  return LLOID_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lloid_last_error(void) { return g_err.c_str(); }
+const char* lloid_version(void) { return "lloid-b200 0.1 (sm_100a)"; }
+
+int lloid_check_count(int64_t count, int64_t capacity)
+{
+  if (count > capacity) return fail(LLOID_EOVERFLOW, "trigger buffer overflow: %lld triggers, capacity %lld",
+                                    (long long)count, (long long)capacity);
+  return LLOID_OK;
+}
+
+int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const lloid_bin_desc_t* bins,
+                      const lloid_slice_desc_t* const* slices)
+{
+  if (!out || !cfg || !bins || !slices) return fail(LLOID_EINVAL, "null argument");
+  *out = nullptr;
+  if (cfg->n_bins < 1 || cfg->n_detectors < 1) return fail(LLOID_EINVAL, "n_bins and n_detectors must be >= 1");
+  if (cfg->full_rate_hz < 1) return fail(LLOID_EINVAL, "full_rate_hz must be positive");
+  if (cfg->peak_window < kTimeTile || cfg->peak_window % kTimeTile)
+    return fail(LLOID_EINVAL, "peak_window must be a positive multiple of %d", kTimeTile);
+  if (cfg->k_up != kKUp) return fail(LLOID_EINVAL, "k_up must be %d in this version", kKUp);
+  if (cfg->k_down < 1 || cfg->k_down > 64) return fail(LLOID_EINVAL, "k_down out of range [1, 64]");
+  if (cfg->precision != LLOID_F32 && cfg->precision != LLOID_F16)
+    return fail(LLOID_EINVAL, "precision must be LLOID_F32 or LLOID_F16");
+  if (cfg->max_chunk < 0 || cfg->max_chunk % kTimeTile) return fail(LLOID_EINVAL, "max_chunk must be a multiple of %d", kTimeTile);
+  if (!(cfg->snr_threshold >= 0.f)) return fail(LLOID_EINVAL, "snr_threshold must be >= 0");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(LLOID_ECUDA, "no CUDA device: this library has no CPU fallback");
+  if (cfg->device < 0 || cfg->device >= ndev) return fail(LLOID_ECUDA, "device %d not present", cfg->device);
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, cfg->device));
+  if (prop.major != 10) return fail(LLOID_ECUDA, "device %d is sm_%d%d; this build is sm_100a only", cfg->device, prop.major, prop.minor);
+  CU(cudaSetDevice(cfg->device));
+
+  lloid_bank* b = new (std::nothrow) lloid_bank();
+  if (!b) return fail(LLOID_ENOMEM, "out of host memory");
+  b->cfg = *cfg;
+  b->f16 = cfg->precision == LLOID_F16;
+  b->bins.resize(cfg->n_bins);
+  int first = 0;
+  for (int bi = 0; bi < cfg->n_bins; ++bi) {
+    const lloid_bin_desc_t& bd = bins[bi];
+    BinHost& B = b->bins[bi];
+    if (bd.n_templates < 1 || bd.n_slices < 1 || bd.template_len < 1 || !slices[bi]) {
+      delete b; return fail(LLOID_EINVAL, "bin %d: bad descriptor", bi);
+    }
+    B.N = bd.n_templates; B.S = bd.n_slices; B.M = bd.template_len;
+    B.rows_pad = (int)round_up(2 * B.N, kRowPad);
+    int64_t expect_delay = 0;
+    for (int s = 0; s < B.S; ++s) {
+      const lloid_slice_desc_t& sd = slices[bi][s];
+      SliceHost S;
+      if (sd.rate_hz < 1 || cfg->full_rate_hz % sd.rate_hz) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: rate %d does not divide f0", bi, s, sd.rate_hz); }
+      S.rate = sd.rate_hz; S.d = cfg->full_rate_hz / sd.rate_hz; S.log2d = ilog2(S.d);
+      if ((1 << S.log2d) != S.d || S.d > 32) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: decimation %d is not a power of two <= 32", bi, s, S.d); }
+      if (sd.n_taps < 1 || sd.n_basis < 1 || sd.n_basis > 512) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: n_taps/n_basis out of range", bi, s); }
+      if (sd.end_delay % S.d) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: end_delay not a multiple of d", bi, s); }
+      if (sd.end_delay != expect_delay) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: slices must tile the template back to front (end_delay %lld, expected %lld)", bi, s, (long long)sd.end_delay, (long long)expect_delay); }
+      if (S.d > 1 && sd.end_delay < (int64_t)(cfg->k_down + cfg->k_up) * S.d) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: causality needs end_delay >= (k_down + k_up) * d", bi, s); }
+      S.n_taps = sd.n_taps; S.L = sd.n_basis; S.L_pad = (int)round_up(S.L, kLPad); S.end_delay = sd.end_delay;
+      expect_delay += (int64_t)S.d * S.n_taps;
+      B.slices.push_back(S);
+      b->d_max = std::max(b->d_max, S.d);
+    }
+    if (expect_delay != B.M) { delete b; return fail(LLOID_EINVAL, "bin %d: slices cover %lld samples, template_len is %lld", bi, (long long)expect_delay, (long long)B.M); }
+    b->max_templates = std::max(b->max_templates, B.N);
+    b->max_rows_pad = std::max(b->max_rows_pad, B.rows_pad);
+    for (int det = 0; det < cfg->n_detectors; ++det) {
+      BinParams bp; bp.n_templates = B.N; bp.n_slices = B.S; bp.first_slice = first; bp.rows_pad = B.rows_pad;
+      b->bp_host.push_back(bp);
+      for (int s = 0; s < B.S; ++s) {
+        SliceParams P; memset(&P, 0, sizeof P);
+        const SliceHost& S = B.slices[s];
+        P.d = S.d; P.log2d = S.log2d; P.n_taps = S.n_taps; P.L = S.L; P.L_pad = S.L_pad;
+        P.rows = 2 * B.N; P.rows_pad = B.rows_pad; P.bin = bi; P.det = det; P.slice = s;
+        b->sp_host.push_back(P);
+      }
+      first += B.S;
+    }
+  }
+  b->n_bd = cfg->n_bins * cfg->n_detectors;
+  b->uploaded.assign(b->sp_host.size(), 0);
+  *out = b;
+  return LLOID_OK;
+}
+
+int lloid_bank_upload_slice(lloid_bank_t* b, int32_t bin, int32_t det, int32_t slice, const double* basis,
+                            const double* recon)
+{
+  int rc = check_ids(b, bin, det, slice); if (rc) return rc;
+  if (!basis || !recon) return fail(LLOID_EINVAL, "null array");
+  if (b->finalized) return fail(LLOID_ESTATE, "upload after finalize");
+  CU(cudaSetDevice(b->cfg.device));
+  SliceParams& P = b->sp_host[b->slice_index(bin, det, slice)];
+  rc = upload_arrays(b, bin, slice, basis, recon, &P.U32, &P.R32, &P.U16, &P.R16); if (rc) return rc;
+  b->uploaded[b->slice_index(bin, det, slice)] = 1;
+  return LLOID_OK;
+}
+
+int lloid_bank_upload_slice_shared(lloid_bank_t* b, int32_t bin, int32_t slice, const double* basis,
+                                   const double* recon)
+{
+  int rc = check_ids(b, bin, 0, slice); if (rc) return rc;
+  if (!basis || !recon) return fail(LLOID_EINVAL, "null array");
+  if (b->finalized) return fail(LLOID_ESTATE, "upload after finalize");
+  CU(cudaSetDevice(b->cfg.device));
+  SliceParams& P0 = b->sp_host[b->slice_index(bin, 0, slice)];
+  rc = upload_arrays(b, bin, slice, basis, recon, &P0.U32, &P0.R32, &P0.U16, &P0.R16); if (rc) return rc;
+  for (int det = 0; det < b->cfg.n_detectors; ++det) {
+    SliceParams& P = b->sp_host[b->slice_index(bin, det, slice)];
+    P.U32 = P0.U32; P.R32 = P0.R32; P.U16 = P0.U16; P.R16 = P0.R16;
+    b->uploaded[b->slice_index(bin, det, slice)] = 1;
+  }
+  return LLOID_OK;
+}
+
+int lloid_bank_alias_bin(lloid_bank_t* b, int32_t dst, int32_t src)
+{
+  int rc = check_ids(b, dst, 0, 0); if (rc) return rc;
+  rc = check_ids(b, src, 0, 0); if (rc) return rc;
+  if (b->finalized) return fail(LLOID_ESTATE, "alias after finalize");
+  const BinHost &A = b->bins[dst], &Bs = b->bins[src];
+  if (A.N != Bs.N || A.S != Bs.S || A.M != Bs.M) return fail(LLOID_EINVAL, "alias_bin: geometry differs");
+  for (int s = 0; s < A.S; ++s) {
+    const SliceHost &x = A.slices[s], &y = Bs.slices[s];
+    if (x.d != y.d || x.n_taps != y.n_taps || x.L != y.L || x.end_delay != y.end_delay)
+      return fail(LLOID_EINVAL, "alias_bin: slice %d geometry differs", s);
+    for (int det = 0; det < b->cfg.n_detectors; ++det) {
+      const int is = b->slice_index(src, det, s), id = b->slice_index(dst, det, s);
+      if (!b->uploaded[is]) return fail(LLOID_ESTATE, "alias_bin: source bin %d not uploaded", src);
+      SliceParams& P = b->sp_host[id]; const SliceParams& Q = b->sp_host[is];
+      P.U32 = Q.U32; P.R32 = Q.R32; P.U16 = Q.U16; P.R16 = Q.R16;
+      b->uploaded[id] = 1;
+    }
+  }
+  return LLOID_OK;
+}
+
+int lloid_bank_finalize(lloid_bank_t* b)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (b->finalized) return fail(LLOID_ESTATE, "already finalized");
+  for (size_t i = 0; i < b->uploaded.size(); ++i)
+    if (!b->uploaded[i]) return fail(LLOID_ESTATE, "bin %d detector %d slice %d was never uploaded",
+                                     b->sp_host[i].bin, b->sp_host[i].det, b->sp_host[i].slice);
+  CU(cudaSetDevice(b->cfg.device));
+  const int D = b->cfg.n_detectors, Kd = b->cfg.k_down, Ku = b->cfg.k_up;
+  const size_t esize = b->f16 ? 2 : 4;
+
+  // history length H: enough strain before the chunk for every slice's earliest tap
+  int64_t H = 0;
+  double ybytes_per_sample = 0.0;
+  for (const BinHost& B : b->bins)
+    for (const SliceHost& S : B.slices) {
+      const int64_t need = (S.d == 1) ? S.end_delay + S.n_taps : S.end_delay + (int64_t)S.d * (S.n_taps + Ku + Kd);
+      H = std::max(H, need);
+      ybytes_per_sample += (double)D * S.L_pad * esize / S.d;
+    }
+  H = round_up(H, 256);
+  if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
+  int64_t C = b->cfg.max_chunk;
+  if (C == 0) {
+    const double budget = 96.0 * 1024 * 1024;
+    C = (int64_t)(budget / ybytes_per_sample);
+    C = C / 2048 * 2048;
+    C = std::min<int64_t>(std::max<int64_t>(C, 2048), 65536);
+  }
+  b->H = (int)H; b->C = (int)C;
+  b->xw_pitch = (int)round_up(H + C + 256, 64);
+  b->tiles_cap = (int)(C / kTimeTile) + 1;
+
+  int rc;
+  rc = dev_alloc(b, (void**)&b->xw, (size_t)D * b->xw_pitch * 4, true); if (rc) return rc;
+  rc = dev_alloc(b, (void**)&b->hist, (size_t)D * H * 4, true); if (rc) return rc;
+
+  // rates
+  std::vector<int> ds;
+  for (const BinHost& B : b->bins) for (const SliceHost& S : B.slices) if (std::find(ds.begin(), ds.end(), S.d) == ds.end()) ds.push_back(S.d);
+  std::sort(ds.begin(), ds.end());
+  b->rates_host.resize(ds.size());
+  for (size_t r = 0; r < ds.size(); ++r) {
+    RateParams& R = b->rates_host[r]; memset(&R, 0, sizeof R);
+    R.d = ds[r];
+    R.jj_lo_fixed = INT32_MAX; R.jj_hi_off = INT32_MIN;
+    if (R.d == 1) {
+      R.xs32 = b->xw; R.xs_len = b->xw_pitch;
+    } else {
+      R.xs_len = (int)round_up((H + C) / R.d + 256, 64);
+      rc = dev_alloc(b, (void**)&R.xs32, (size_t)D * R.xs_len * 4, true); if (rc) return rc;
+      std::vector<double> lp = lowpass(R.d, Kd);
+      std::vector<float> taps(lp.size());
+      const double g = std::sqrt((double)R.d);
+      for (size_t u = 0; u < lp.size(); ++u) taps[u] = (float)(g * lp[lp.size() - 1 - u]);
+      float* td; rc = dev_alloc(b, (void**)&td, taps.size() * 4, false); if (rc) return rc;
+      CU(cudaMemcpy(td, taps.data(), taps.size() * 4, cudaMemcpyHostToDevice));
+      R.taps = td;
+    }
+    if (b->f16) { rc = dev_alloc(b, (void**)&R.xs16, (size_t)D * R.xs_len * 2, true); if (rc) return rc; }
+  }
+
+  // per-slice tables: Y buffers, origins, needed resample ranges
+  size_t ybytes = 0;
+  for (SliceParams& P : b->sp_host) {
+    const SliceHost& S = b->bins[P.bin].slices[P.slice];
+    P.rate_idx = (int)(std::find(ds.begin(), ds.end(), S.d) - ds.begin());
+    const int64_t rows = (S.d == 1) ? C : C / S.d + 2 * Ku;
+    P.y_rows_cap = (int)round_up(rows, 128);
+    P.jjY0 = (S.d == 1) ? (int)(H - S.end_delay) : (int)((H - S.end_delay) / S.d - Ku);
+    RateParams& R = b->rates_host[P.rate_idx];
+    R.jj_lo_fixed = std::min(R.jj_lo_fixed, P.jjY0 - S.n_taps);
+    R.jj_hi_off = std::max(R.jj_hi_off, (S.d == 1) ? P.jjY0 : P.jjY0 + 2 * Ku - 1);
+    ybytes += round_up((size_t)P.y_rows_cap * S.L_pad * esize, 256);
+  }
+  char* ybase; rc = dev_alloc(b, (void**)&ybase, ybytes, true); if (rc) return rc;
+  size_t yoff = 0;
+  for (SliceParams& P : b->sp_host) {
+    P.Y = ybase + yoff;
+    yoff += round_up((size_t)P.y_rows_cap * P.L_pad * esize, 256);
+  }
+  for (const RateParams& R : b->rates_host)
+    if (R.jj_lo_fixed < (R.d == 1 ? 0 : Kd)) return fail(LLOID_EINVAL, "internal: history too short for rate d=%d", R.d);
+
+  // interpolation weights  w[(i + K_up) * d + phi] = d * lp_{d,K_up}[d i + phi],  i = -K_up .. K_up - 1
+  std::vector<const float*> upw(kMaxRates, nullptr);
+  for (int d : ds) {
+    if (d == 1) continue;
+    std::vector<double> lp = lowpass(d, Ku);
+    std::vector<float> w((size_t)2 * Ku * d);
+    for (int i = -Ku; i < Ku; ++i)
+      for (int phi = 0; phi < d; ++phi) w[(size_t)(i + Ku) * d + phi] = (float)(d * lp[d * i + phi + Ku * d]);
+    float* wd; rc = dev_alloc(b, (void**)&wd, w.size() * 4, false); if (rc) return rc;
+    CU(cudaMemcpy(wd, w.data(), w.size() * 4, cudaMemcpyHostToDevice));
+    upw[ilog2(d)] = wd;
+  }
+  rc = dev_alloc(b, (void**)&b->upw_dev, kMaxRates * sizeof(float*), false); if (rc) return rc;
+  CU(cudaMemcpy((void*)b->upw_dev, upw.data(), kMaxRates * sizeof(float*), cudaMemcpyHostToDevice));
+
+  rc = dev_alloc(b, (void**)&b->sp_dev, b->sp_host.size() * sizeof(SliceParams), false); if (rc) return rc;
+  CU(cudaMemcpy(b->sp_dev, b->sp_host.data(), b->sp_host.size() * sizeof(SliceParams), cudaMemcpyHostToDevice));
+  rc = dev_alloc(b, (void**)&b->bp_dev, b->bp_host.size() * sizeof(BinParams), false); if (rc) return rc;
+  CU(cudaMemcpy(b->bp_dev, b->bp_host.data(), b->bp_host.size() * sizeof(BinParams), cudaMemcpyHostToDevice));
+  rc = dev_alloc(b, (void**)&b->rates_dev, b->rates_host.size() * sizeof(RateParams), false); if (rc) return rc;
+  CU(cudaMemcpy(b->rates_dev, b->rates_host.data(), b->rates_host.size() * sizeof(RateParams), cudaMemcpyHostToDevice));
+
+  const size_t nstate = (size_t)b->n_bd * b->max_templates;
+  rc = dev_alloc(b, (void**)&b->state, nstate * sizeof(PeakState), false); if (rc) return rc;
+  rc = dev_alloc(b, (void**)&b->partials, nstate * b->tiles_cap * sizeof(Peak), true); if (rc) return rc;
+  rc = dev_alloc(b, (void**)&b->stage_count, 8, true); if (rc) return rc;
+  launch_reset_state(b->state, (int64_t)nstate, 0);
+  CU(cudaDeviceSynchronize());
+
+  if (b->f16) {
+    char err[256] = {0};
+    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, err, sizeof err);
+    if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
+  }
+  b->finalized = true;
+  return LLOID_OK;
+}
+
+int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trigger_t* trig, int64_t capacity,
+                 int64_t* count_dev, void* stream)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (!b->finalized) return fail(LLOID_ESTATE, "filter before finalize");
+  if (!strain_dev || !count_dev || (capacity > 0 && !trig)) return fail(LLOID_EINVAL, "null buffer");
+  if (n <= 0 || n % b->d_max) return fail(LLOID_EINVAL, "n_samples must be a positive multiple of %d", b->d_max);
+  if (capacity < 0) return fail(LLOID_EINVAL, "negative capacity");
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(b->cfg.device));
+  b->last_launches = 0;
+  b->events_used = 0;
+  CU(cudaMemsetAsync(count_dev, 0, 8, st));
+  int64_t k = b->consumed, off = 0, rem = n;
+  while (rem > 0) {
+    int64_t c = std::min<int64_t>(rem, b->C);
+    const int64_t mis = k % kTimeTile;
+    if (mis) c = std::min<int64_t>(c, kTimeTile - mis);     // re-align chunk starts to the tile grid
+    int rc = process_chunk(b, strain_dev + off, n, (int)c, k, trig, capacity, (unsigned long long*)count_dev, st);
+    if (rc) return rc;
+    k += c; off += c; rem -= c;
+  }
+  b->consumed = k;
+  return LLOID_OK;
+}
+
+int lloid_filter_host(lloid_bank_t* b, const float* strain_host, int64_t n, lloid_trigger_t* trig_host,
+                      int64_t capacity, int64_t* count_host, void* stream)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (!b->finalized) return fail(LLOID_ESTATE, "filter before finalize");
+  if (!strain_host || !count_host || (capacity > 0 && !trig_host)) return fail(LLOID_EINVAL, "null buffer");
+  if (n <= 0 || capacity < 0) return fail(LLOID_EINVAL, "bad size");
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(b->cfg.device));
+  const size_t elems = (size_t)b->cfg.n_detectors * n;
+  if (elems > b->stage_strain_elems) {
+    if (b->stage_strain) { cudaFree(b->stage_strain); b->bytes -= (int64_t)b->stage_strain_elems * 4; }
+    cudaError_t e = cudaMalloc((void**)&b->stage_strain, elems * 4);
+    if (e != cudaSuccess) { b->stage_strain = nullptr; b->stage_strain_elems = 0; return fail(LLOID_ENOMEM, "staging alloc failed"); }
+    b->stage_strain_elems = elems; b->bytes += (int64_t)elems * 4;
+  }
+  if (capacity > b->stage_trig_cap) {
+    if (b->stage_trig) { cudaFree(b->stage_trig); b->bytes -= b->stage_trig_cap * 32; }
+    cudaError_t e = cudaMalloc((void**)&b->stage_trig, (size_t)capacity * sizeof(lloid_trigger_t));
+    if (e != cudaSuccess) { b->stage_trig = nullptr; b->stage_trig_cap = 0; return fail(LLOID_ENOMEM, "staging alloc failed"); }
+    b->stage_trig_cap = capacity; b->bytes += capacity * 32;
+  }
+  CU(cudaMemcpyAsync(b->stage_strain, strain_host, elems * 4, cudaMemcpyHostToDevice, st));
+  int rc = lloid_filter(b, b->stage_strain, n, b->stage_trig, capacity, (int64_t*)b->stage_count, stream);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(count_host, b->stage_count, 8, cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  const int64_t got = std::min<int64_t>(*count_host, capacity);
+  if (got > 0) {
+    CU(cudaMemcpyAsync(trig_host, b->stage_trig, (size_t)got * sizeof(lloid_trigger_t), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+  }
+  return lloid_check_count(*count_host, capacity);
+}
+
+int lloid_reset(lloid_bank_t* b, void* stream)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (!b->finalized) return fail(LLOID_ESTATE, "reset before finalize");
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(b->cfg.device));
+  CU(cudaMemsetAsync(b->hist, 0, (size_t)b->cfg.n_detectors * b->H * 4, st));
+  launch_reset_state(b->state, (int64_t)b->n_bd * b->max_templates, st);
+  b->consumed = 0;
+  return LLOID_OK;
+}
+
+int lloid_debug_capture(lloid_bank_t* b, int32_t bin, int32_t det, int64_t k_begin, int64_t n, float* snr_dev)
+{
+  int rc = check_ids(b, bin, det, 0); if (rc) return rc;
+  if (!snr_dev) { b->cap = Capture{nullptr, 0, 0, -1, 0}; return LLOID_OK; }
+  if (n <= 0) return fail(LLOID_EINVAL, "capture length must be positive");
+  b->cap.snr = snr_dev; b->cap.k_begin = k_begin; b->cap.n = n;
+  b->cap.bd = bin * b->cfg.n_detectors + det; b->cap.rows = 2 * b->bins[bin].N;
+  return LLOID_OK;
+}
+
+int64_t lloid_samples_consumed(const lloid_bank_t* b) { return b ? b->consumed : -1; }
+int64_t lloid_chunk_samples(const lloid_bank_t* b) { return b ? b->C : -1; }
+int64_t lloid_last_launch_count(const lloid_bank_t* b) { return b ? b->last_launches : -1; }
+int64_t lloid_device_bytes(const lloid_bank_t* b) { return b ? b->bytes : -1; }
+
+int lloid_set_profiling(lloid_bank_t* b, int32_t enable)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  b->prof = enable != 0; b->events_used = 0;
+  return LLOID_OK;
+}
+
+int lloid_last_stage_ms(lloid_bank_t* b, float* out)
+{
+  if (!b || !out) return fail(LLOID_EINVAL, "null argument");
+  for (int i = 0; i < 5; ++i) out[i] = 0.f;
+  if (!b->prof || b->events_used < 5) return fail(LLOID_ESTATE, "profiling was not enabled for the last call");
+  CU(cudaEventSynchronize(b->events[b->events_used - 1]));
+  for (size_t i = 0; i + 4 < b->events_used; i += 5)
+    for (int s = 0; s < 4; ++s) {
+      float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[i + s], b->events[i + s + 1]));
+      out[s] += ms;
+    }
+  float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[0], b->events[b->events_used - 1]));
+  out[4] = ms;
+  return LLOID_OK;
+}
+
+void lloid_destroy(lloid_bank_t* b)
+{
+  if (!b) return;
+  cudaSetDevice(b->cfg.device);
+  cudaDeviceSynchronize();
+  if (b->plan16) f16_plan_destroy(b->plan16);
+  for (void* p : b->owned) cudaFree(p);
+  if (b->stage_strain) cudaFree(b->stage_strain);
+  if (b->stage_trig) cudaFree(b->stage_trig);
+  for (cudaEvent_t e : b->events) cudaEventDestroy(e);
+  delete b;
+}
+
+}  // extern "C"

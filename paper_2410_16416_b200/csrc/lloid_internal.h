@@ -1,0 +1,95 @@
+// Internal declarations shared by the host API (lloid_api.cu) and the kernels.  Not part of the ABI.
+//
+// Chunk-local coordinates.  lloid_filter walks the caller's buffer in chunks
+// [k_a, k_a + c).  For every detector a work strain buffer xw[H + c] holds the last H samples of
+// history followed by the chunk; xw[i] is absolute sample k_a - H + i.  A rate-d stream is indexed
+// from the same origin: xs_d[jj] is the decimated sample at absolute time k_a - H + d*jj.
+// kappa = k - k_a is the chunk-local output index, 0 <= kappa < c.
+//   slice with d == 1 :  Y row r  <->  kappa = r                      rows [0, c)
+//   slice with d  > 1 :  Y row r  <->  low-rate index floor(kappa/d) = r - K_up   rows [0, c/d + 2 K_up)
+// so that for every slice   c^s[kappa] = sum_{i=-K_up}^{K_up-1} w_phi[i] rho^s[row floor(kappa/d) + K_up - i],
+// phi = kappa mod d, w_phi[i] = d lp_{d,K_up}[d i + phi]   (A4 in include/lloid.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace lloid {
+
+constexpr int kKUp = 8;            // interpolation half-width supported by the kernels
+constexpr int kTimeTile = 128;     // f0 samples per epilogue tile; chunk starts are aligned to it
+constexpr int kMaxRates = 6;       // d in {1,2,4,8,16,32}
+constexpr int kRowPad = 128;       // reconstruction rows padded to a multiple of this
+constexpr int kLPad = 32;          // basis count padded to a multiple of this
+
+struct SliceParams {               // one per (bin, detector, slice); lives in a device table
+  const float*  U32;               // [L_pad][n_taps]            fp32 path
+  const float*  R32;               // [rows_pad][L_pad]          fp32 path
+  const __half* U16;               // [L_pad][n_taps]  K-major   fp16 path (TMA source)
+  const __half* R16;               // [rows_pad][L_pad] K-major  fp16 path (TMA source)
+  void*    Y;                      // chunk-local y^s, row-major [y_rows_cap][L_pad] (fp32 or fp16)
+  int32_t  d, log2d, rate_idx;
+  int32_t  n_taps, L, L_pad;
+  int32_t  rows, rows_pad;         // 2N and its padding
+  int32_t  jjY0;                   // xs index of Y row 0: (H-Delta)/d - K_up (d>1) or H-Delta (d==1)
+  int32_t  y_rows_cap;             // allocated Y rows
+  int32_t  bin, det, slice, pad_;
+};
+
+struct RateParams {                // one per distinct decimation factor
+  const float* taps;               // [2 K_dn d + 1], taps[u] = sqrt(d) lp[K_dn d - u]   (d == 1: unused)
+  float*   xs32;                   // [D][xs_len]  (d == 1: aliases the work strain buffer)
+  __half*  xs16;                   // [D][xs_len]  fp16 path only
+  int32_t  d, xs_len;
+  int32_t  jj_lo_fixed;            // first index needed at a chunk start: constant per bank
+  int32_t  jj_hi_off;              // needed end = jj_hi_off + c/d  (exclusive)
+};
+
+struct BinParams {                 // one per (bin, detector)
+  int32_t n_templates, n_slices, first_slice /* index into SliceParams table */, rows_pad;
+};
+
+struct Peak {                      // 16 bytes: per-tile partial maximum of |rho|^2 for one template
+  float q; int32_t kappa; float re, im;
+};
+
+struct PeakState {                 // running in-window maximum carried across tiles, chunks and calls
+  float q; float re; float im; int32_t pad; int64_t k;
+};
+
+struct Capture {                   // lloid_debug_capture
+  float*  snr; int64_t k_begin, n; int32_t bd; int32_t rows;
+};
+
+// ---- launchers (one translation unit per kernel family) ---------------------------------------
+void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
+                     const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
+                     bool want_f16, cudaStream_t st, int64_t* launches);
+
+void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
+                    const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches);
+
+void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
+                      int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap,
+                      cudaStream_t st, int64_t* launches);
+
+void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
+                        int tiles_cap, int n_tiles, int c, int64_t k_a, int W, float theta,
+                        PeakState* state, int n_det, void* triggers, int64_t capacity,
+                        unsigned long long* count, cudaStream_t st, int64_t* launches);
+
+void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
+
+// fp16 / tcgen05 path (kernels_f16.cu)
+struct F16Plan;                    // opaque host-side plan: tensor maps, work lists
+F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,
+                         int n_det, int chunk_cap, char* err, int errlen);
+void f16_plan_destroy(F16Plan*);
+int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const RateParams* rates_dev, const RateParams* rates_host,
+                    int c, cudaStream_t st, int64_t* launches);
+int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, const BinParams* bp_dev, const float* const* upw_dev,
+                      Peak* partials, int tiles_cap, int c, int64_t k_a, Capture cap, cudaStream_t st,
+                      int64_t* launches);
+
+}  // namespace lloid
