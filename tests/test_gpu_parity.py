@@ -63,7 +63,9 @@ def test_config1_dense_snr_and_triggers(cfg1, precision):
     assert stats["checked"] == 64 * 16 and stats["triggers"] > 0
     inj = w.injections[0]
     hit = trigs[(trigs["template_idx"] == inj.template) & (trigs["sample"] // w.peak_window == inj.end // w.peak_window)]
-    assert len(hit) == 1 and int(hit[0]["sample"]) == inj.end          # recovered at the injected time
+    assert len(hit) == 1 and abs(int(hit[0]["sample"]) - inj.end) <= 2  # recovered at the injected time (noise moves the
+    k_or = int(np.argmax(rho[2 * inj.template] ** 2 + rho[2 * inj.template + 1] ** 2)) # peak by a sample; exact vs oracle)
+    assert int(hit[0]["sample"]) == k_or
     assert stats["exact_index"] >= 0.98 * stats["triggers"]
 
 
@@ -72,7 +74,7 @@ def test_config1c_lossless_bank_recovers_injected_snr(cfg1c, precision):
     w = cfg1c
     trigs, _, _ = pu.run_gpu(w, precision)
     inj = w.injections[0]
-    hit = trigs[(trigs["template_idx"] == inj.template) & (trigs["sample"] == inj.end)]
+    hit = trigs[(trigs["template_idx"] == inj.template) & (np.abs(trigs["sample"] - inj.end) <= 2)]
     assert len(hit) == 1
     amp = float(np.hypot(hit[0]["snr_re"], hit[0]["snr_im"]))
     assert abs(amp - inj.amplitude) < 1.5          # 12 sigma signal + unit noise
@@ -91,7 +93,7 @@ def test_streaming_pieces_equal_one_shot(cfg1, precision):
     w = cfg1
     n = w.n_samples
     one, _, info1 = pu.run_gpu(w, precision)
-    pieces = [2048] * 3 + [4, 60, 1984, 4096, 8, 8192 - 8, 10240]
+    pieces = [2048] * 4 + [4, 60, 1984, 4096, 8, 8192 - 8, 10240]
     assert sum(pieces) == n
     many, _, info2 = pu.run_gpu(w, precision, pieces=pieces)
     assert _as_set(one) == _as_set(many)
@@ -155,6 +157,7 @@ def test_filter_argument_errors(cfg1):
 def test_multi_bin_multi_detector_bank(precision):
     w3 = wl.config3(n_bins=6, n_templates=24, seconds=12, n_detectors=2, n_basis=16)
     assert len({b.template_len for b in w3.bins}) == 3          # all three shape classes present
+    w3.threshold = 3.0                                          # enough noise triggers in 12 s to compare
     tol = pu.TOL[precision]
     k0, k1 = 16384, 16384 + 4096
     for bin_, det in ((0, 1), (3, 0), (5, 1)):
@@ -185,6 +188,6 @@ def test_config2_geometry_excerpt(precision):
     rho = pu.oracle_snr(w, 0, 1, k0, k1)
     assert np.abs(snr - rho).max() <= tol
     stats = pu.check_triggers(trigs, rho, k0, w, 0, 1, tol)
-    hit = trigs[(trigs["detector"] == 1) & (trigs["template_idx"] == inj.template) & (trigs["sample"] == inj.end)]
+    hit = trigs[(trigs["detector"] == 1) & (trigs["template_idx"] == inj.template) & (np.abs(trigs["sample"] - inj.end) <= 2)]
     assert len(hit) == 1
     assert stats["triggers"] > 0
