@@ -1,11 +1,223 @@
-// fp16 / tcgen05 path — placeholder until the tensor-core kernels land (fails loudly, never falls back).
+// fp16 path (LLOID_F16): A2 basis FIR on the tcgen05 tensor cores.
+//
+//   y^s_l[j] = sum_t U^s[l,t] x^s[j - n_s + t]                 (include/lloid.h A2)
+//
+// As a GEMM:  Y[time j, l] = H[j, t] * U[l, t]^T  with the Hankel matrix H[j, t] = x^s[b0 + j + t].
+// H is never materialised.  In the no-swizzle K-major operand layout a core matrix is 8 rows x 8 fp16
+// (128 contiguous bytes), and core matrix (row group jg, tap group tg) of a Hankel matrix depends only
+// on q = jg + tg:   Cq[r][e] = x[b0 + 8 q + r + e].   So ONE array C of (rows + taps)/8 core matrices
+// (16 bytes per sample of the strain window) serves as the A operand of every MMA of the tile with
+// descriptor strides LBO = SBO = 128 bytes; the K loop only advances the start address.  The window is
+// staged once per CTA; U streams through shared memory in pre-packed 64-tap stages (one 1-D bulk copy
+// each, mbarrier pipeline); MT time tiles of 128 rows share every U stage (MT accumulators in TMEM).
+//
+// Warp roles (192 threads): warp 0 = bulk-copy producer, warp 1 = MMA issuer, warps 2-5 = epilogue
+// (TMEM -> registers -> fp16 -> Y, packed in the layout the reconstruction kernel reads).
 #include "lloid_internal.h"
+#include "tc05.cuh"
+
 #include <cstdio>
+
 namespace lloid {
-struct F16Plan { int dummy; };
-F16Plan* f16_plan_create(const SliceParams*, int, const BinParams*, int, int, int, char* err, int errlen)
-{ snprintf(err, errlen, "fp16 path not built yet"); return nullptr; }
-void f16_plan_destroy(F16Plan* p) { delete p; }
-int launch_fir_f16(F16Plan*, const SliceParams*, const RateParams*, const RateParams*, int, cudaStream_t, int64_t*) { return 1; }
-int launch_recon_f16(F16Plan*, const SliceParams*, const BinParams*, const float* const*, Peak*, int, int, int64_t, Capture, cudaStream_t, int64_t*) { return 1; }
+
+using namespace tc;
+
+constexpr int FH_THREADS = 192;
+constexpr int FH_KB = 64;                    // taps per pipeline stage
+constexpr int FH_MAX_STAGES = 8;
+
+struct F16Plan {
+  int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
+  int chunk_cap = 0;
+};
+
+__device__ __forceinline__ int fir_mt(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
+
+__global__ void __launch_bounds__(FH_THREADS, 1)
+fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int c, int n_stages)
+{
+  const SliceParams P = sp[blockIdx.y];
+  const int rows_needed = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+  const int L_pad = P.L_pad;
+  const int MT = fir_mt(L_pad);
+  const int r0 = blockIdx.x * 128 * MT;
+  if (r0 >= rows_needed) return;
+  int mt_used = (rows_needed - r0 + 127) / 128; if (mt_used > MT) mt_used = MT;
+
+  const int n_kb = (P.n_taps + FH_KB - 1) / FH_KB;
+  const int n_pad = n_kb * FH_KB;
+  const int n_chunks = mt_used * 128 + n_pad;                 // 16-byte chunks of the Hankel array
+  const int stage_bytes = L_pad * FH_KB * 2;
+
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t bar_full[FH_MAX_STAGES], bar_empty[FH_MAX_STAGES], bar_acc;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sC = smem;                                          // [n_chunks][16 B]
+  uint8_t* sRaw = sC + (size_t)n_chunks * 16;                  // raw fp16 window, n_chunks + 8 samples (+pad)
+  uint8_t* sB = sRaw + (((size_t)(n_chunks + 16) * 2 + 127) / 128) * 128;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  if (tid == 32) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&bar_full[s]), 1); mbar_init(smem_u32(&bar_empty[s]), 1); }
+    mbar_init(smem_u32(&bar_acc), 1);
+    mbar_init_fence();
+  }
+
+  // ---- stage the strain window and expand it into the Hankel core-matrix array --------------------
+  const RateParams R = rates[P.rate_idx];
+  const __half* __restrict__ xs = R.xs16 + (size_t)P.det * R.xs_len;
+  const int b0 = P.jjY0 + r0 - P.n_taps;                       // xs index of window element 0 (>= 0)
+  {
+    unsigned short* raw = reinterpret_cast<unsigned short*>(sRaw);
+    const unsigned short* xg = reinterpret_cast<const unsigned short*>(xs);
+    for (int i = tid; i < n_chunks + 8; i += FH_THREADS) {
+      const int idx = b0 + i;
+      raw[i] = (idx >= 0 && idx < R.xs_len) ? __ldg(xg + idx) : (unsigned short)0;
+    }
+  }
+  __syncthreads();
+  {
+    const uint32_t* raw32 = reinterpret_cast<const uint32_t*>(sRaw);
+    for (int ch = tid; ch < n_chunks; ch += FH_THREADS) {      // chunk ch = window samples [ch, ch + 8)
+      const int w = ch >> 1;
+      uint32_t a0 = raw32[w], a1 = raw32[w + 1], a2 = raw32[w + 2], a3 = raw32[w + 3];
+      if (ch & 1) {
+        const uint32_t a4 = raw32[w + 4];
+        a0 = __funnelshift_r(a0, a1, 16); a1 = __funnelshift_r(a1, a2, 16);
+        a2 = __funnelshift_r(a2, a3, 16); a3 = __funnelshift_r(a3, a4, 16);
+      }
+      *reinterpret_cast<uint4*>(sC + (size_t)ch * 16) = make_uint4(a0, a1, a2, a3);
+    }
+  }
+  fence_async_smem();                                          // generic-proxy writes -> visible to the MMA (async proxy)
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tmem = tmem_slot;
+
+  if (warp == 0) {
+    // ===== producer: U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
+    if (lane == 0) {
+      const uint8_t* src = reinterpret_cast<const uint8_t*>(P.U16);
+      for (int kb = 0; kb < n_kb; ++kb) {
+        const int s = kb % n_stages;
+        if (kb >= n_stages) mbar_wait(smem_u32(&bar_empty[s]), ((kb / n_stages) - 1) & 1);
+        mbar_expect_tx(smem_u32(&bar_full[s]), stage_bytes);
+        bulk_g2s(smem_u32(sB + (size_t)s * stage_bytes), src + (size_t)kb * stage_bytes, stage_bytes, smem_u32(&bar_full[s]));
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      const int n_split = (L_pad > 256) ? 2 : 1;
+      const int Nmma = L_pad / n_split;
+      const uint32_t idesc = idesc_f16(128, Nmma);
+      const uint32_t cbase = smem_u32(sC);
+      for (int kb = 0; kb < n_kb; ++kb) {
+        const int s = kb % n_stages;
+        mbar_wait(smem_u32(&bar_full[s]), (kb / n_stages) & 1);
+        fence_after();
+        const uint32_t bbase = smem_u32(sB + (size_t)s * stage_bytes);
+        for (int mt = 0; mt < mt_used; ++mt) {
+#pragma unroll
+          for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
+            const uint64_t adesc = smem_desc(cbase + (uint32_t)(mt * 16 + kb * 8 + k16 * 2) * 128u, 128u, 128u);
+            for (int h = 0; h < n_split; ++h) {
+              const uint64_t bdesc = smem_desc(bbase + (uint32_t)(k16 * 2) * (uint32_t)(L_pad * 16) + (uint32_t)(h * Nmma * 16),
+                                               (uint32_t)(L_pad * 16), 128u);
+              mma_ss(tmem + (uint32_t)(mt * L_pad + h * Nmma), adesc, bdesc, idesc, (kb | k16) ? 1u : 0u);
+            }
+          }
+        }
+        commit(smem_u32(&bar_empty[s]));                       // stage reusable once these MMAs have read it
+      }
+      commit(smem_u32(&bar_acc));
+    }
+  } else {
+    // ===== epilogue: TMEM -> fp16 -> Y16[lc][row][8] =====
+    const int q = warp & 3;                                    // TMEM lane quarter this warp may access
+    mbar_wait(smem_u32(&bar_acc), 0);
+    fence_after();
+    __half* __restrict__ Y = reinterpret_cast<__half*>(P.Y);
+    const size_t cap = (size_t)P.y_rows_cap;
+    for (int mt = 0; mt < mt_used; ++mt) {
+      const int row = r0 + mt * 128 + q * 32 + lane;
+      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
+      for (int c0 = 0; c0 < L_pad; c0 += 16) {
+        uint32_t v[16];
+        tmem_ld16(taddr + c0, v);
+        tmem_ld_wait();
+        if (row < P.y_rows_cap) {
+          uint32_t h[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const __half2 p = __floats2half2_rn(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1]));
+            h[i] = *reinterpret_cast<const uint32_t*>(&p);
+          }
+          const size_t lc = (size_t)(c0 >> 3);
+          *reinterpret_cast<uint4*>(Y + ((lc) * cap + row) * 8) = make_uint4(h[0], h[1], h[2], h[3]);
+          *reinterpret_cast<uint4*>(Y + ((lc + 1) * cap + row) * 8) = make_uint4(h[4], h[5], h[6], h[7]);
+        }
+      }
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
 }
+
+// ------------------------------------------------------------------------------------------------
+F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams*, int, int, int chunk_cap,
+                         char* err, int errlen)
+{
+  F16Plan* pl = new F16Plan();
+  pl->chunk_cap = chunk_cap;
+  size_t fixed = 0, stage = 0;
+  int gx = 1;
+  for (int i = 0; i < n_problems; ++i) {
+    const SliceParams& P = sp_host[i];
+    if (P.L_pad > 512 || (P.L_pad > 256 && P.L_pad % 32)) { snprintf(err, errlen, "fp16 path: L_pad %d unsupported", P.L_pad); delete pl; return nullptr; }
+    int mt = 512 / P.L_pad; mt = mt > 4 ? 4 : (mt < 1 ? 1 : mt);
+    const int n_pad = (P.n_taps + FH_KB - 1) / FH_KB * FH_KB;
+    const size_t chunks = (size_t)mt * 128 + n_pad;
+    const size_t f = chunks * 16 + ((chunks + 16) * 2 + 127) / 128 * 128;
+    fixed = f > fixed ? f : fixed;
+    const size_t st = (size_t)P.L_pad * FH_KB * 2;
+    stage = st > stage ? st : stage;
+    const int rows = (P.d == 1) ? chunk_cap : (chunk_cap >> P.log2d) + 2 * kKUp;
+    const int g = (rows + 128 * mt - 1) / (128 * mt);
+    gx = g > gx ? g : gx;
+  }
+  const size_t budget = 220 * 1024;
+  if (fixed + 2 * stage > budget) { snprintf(err, errlen, "fp16 path: slice too large for shared memory (%zu + 2 x %zu bytes)", fixed, stage); delete pl; return nullptr; }
+  int stages = (int)((budget - fixed) / stage);
+  if (stages > FH_MAX_STAGES) stages = FH_MAX_STAGES;
+  pl->fir_stages = stages;
+  pl->fir_smem = (int)(fixed + (size_t)stages * stage);
+  pl->fir_grid_x = gx;
+  cudaError_t e = cudaFuncSetAttribute(fir_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_smem);
+  if (e != cudaSuccess) { snprintf(err, errlen, "cudaFuncSetAttribute(fir_f16_kernel, %d): %s", pl->fir_smem, cudaGetErrorString(e)); delete pl; return nullptr; }
+  return pl;
+}
+
+void f16_plan_destroy(F16Plan* p) { delete p; }
+
+int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
+                   const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches)
+{
+  int gx = 1;
+  for (int i = 0; i < n_problems; ++i) {
+    const SliceParams& P = sp_host[i];
+    int mt = 512 / P.L_pad; mt = mt > 4 ? 4 : (mt < 1 ? 1 : mt);
+    const int rows = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+    const int g = (rows + 128 * mt - 1) / (128 * mt);
+    gx = g > gx ? g : gx;
+  }
+  dim3 grid(gx, n_problems);
+  fir_f16_kernel<<<grid, FH_THREADS, pl->fir_smem, st>>>(sp_dev, rates_dev, c, pl->fir_stages);
+  ++*launches;
+  return cudaGetLastError() == cudaSuccess ? 0 : 1;
+}
+
+}  // namespace lloid

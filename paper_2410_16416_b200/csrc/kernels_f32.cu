@@ -185,6 +185,7 @@ __device__ __forceinline__ void gemm_lowrate(const float* __restrict__ Rs, const
   }
 }
 
+template <bool Y16>
 __global__ void __launch_bounds__(256)
 recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict__ bp,
                  const float* const* __restrict__ upw, Peak* __restrict__ partials, int tiles_cap,
@@ -236,10 +237,20 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
         const int ll = e % RC_KC, row = e / RC_KC;
         Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
       }
-      for (int e = tid; e < Ks * RC_KC; e += 256) {
-        const int ll = e % RC_KC, col = e / RC_KC;
-        const int r = r0 + col;
-        Ys[ll * RC_YS + col] = (r < P.y_rows_cap) ? Y[(size_t)r * Lp + l0 + ll] : 0.f;
+      if (Y16) {                                     // packed fp16: Y16[l / 8][row][l % 8]
+        const __half* __restrict__ Yh = reinterpret_cast<const __half*>(P.Y);
+        for (int e = tid; e < Ks * RC_KC; e += 256) {
+          const int le = e & 7, col = (e >> 3) % Ks, lg = (e >> 3) / Ks;
+          const int r = r0 + col, l = l0 + lg * 8 + le;
+          Ys[(lg * 8 + le) * RC_YS + col] =
+              (r < P.y_rows_cap) ? __half2float(Yh[((size_t)(l >> 3) * P.y_rows_cap + r) * 8 + le]) : 0.f;
+        }
+      } else {
+        for (int e = tid; e < Ks * RC_KC; e += 256) {
+          const int ll = e % RC_KC, col = e / RC_KC;
+          const int r = r0 + col;
+          Ys[ll * RC_YS + col] = (r < P.y_rows_cap) ? Y[(size_t)r * Lp + l0 + ll] : 0.f;
+        }
       }
       __syncthreads();
       if (d == 1) {
@@ -326,20 +337,25 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
 
 void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
                       int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
-                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool y_is_f16,
                       cudaStream_t st, int64_t* launches)
 {
   (void)bp_host;
   const size_t smem = sizeof(float) * (RC_KC * RC_RS + RC_KC * RC_YS + RC_RT * RC_RHO_S + 16 * 32);
   static bool configured = false;
   if (!configured) {
-    cudaFuncSetAttribute(recon_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(recon_f32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(recon_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
   dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
-  recon_f32_kernel<<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
-                                           c, (long long)k_a, cap);
+  if (y_is_f16)
+    recon_f32_kernel<true><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
+                                                   c, (long long)k_a, cap);
+  else
+    recon_f32_kernel<false><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
+                                                    c, (long long)k_a, cap);
   ++*launches;
 }
 

@@ -121,17 +121,24 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     CU(cudaMemcpy(dr, r.data(), nr * 4, cudaMemcpyHostToDevice));
     *U32 = (const float*)du; *R32 = (const float*)dr;
   } else {
-    std::vector<__half> u(nu, __float2half(0.f)), r(nr, __float2half(0.f));
+    // fp16 path: U packed for the tcgen05 FIR kernel as [tap block of 64][tap group of 8][l < L_pad][8 taps]
+    // (taps zero-padded to a multiple of 64); R stays fp32 for the reconstruction + interpolation epilogue.
+    const int n_kb = (S.n_taps + 63) / 64;
+    const size_t nup = (size_t)n_kb * 64 * S.L_pad;
+    std::vector<__half> u(nup, __float2half(0.f));
     for (int l = 0; l < S.L; ++l)
-      for (int t = 0; t < S.n_taps; ++t) u[(size_t)l * S.n_taps + t] = __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+      for (int t = 0; t < S.n_taps; ++t)
+        u[(((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.L_pad + l) * 8 + (t & 7)] =
+            __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+    std::vector<float> r(nr, 0.f);
     for (int i = 0; i < 2 * B.N; ++i)
-      for (int l = 0; l < S.L; ++l) r[(size_t)i * S.L_pad + l] = __float2half_rn((float)recon[(size_t)i * S.L + l]);
+      for (int l = 0; l < S.L; ++l) r[(size_t)i * S.L_pad + l] = (float)recon[(size_t)i * S.L + l];
     void *du, *dr;
-    int rc = dev_alloc(b, &du, nu * 2, false); if (rc) return rc;
-    rc = dev_alloc(b, &dr, nr * 2, false); if (rc) return rc;
-    CU(cudaMemcpy(du, u.data(), nu * 2, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(dr, r.data(), nr * 2, cudaMemcpyHostToDevice));
-    *U16 = (const __half*)du; *R16 = (const __half*)dr;
+    int rc = dev_alloc(b, &du, nup * 2, false); if (rc) return rc;
+    rc = dev_alloc(b, &dr, nr * 4, false); if (rc) return rc;
+    CU(cudaMemcpy(du, u.data(), nup * 2, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(dr, r.data(), nr * 4, cudaMemcpyHostToDevice));
+    *U16 = (const __half*)du; *R32 = (const float*)dr;
   }
   return LLOID_OK;
 }
@@ -174,14 +181,13 @@ int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int6
     launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, c, st, &b->last_launches);
     if (b->prof) next_event(b, st);
     launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
-                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st, &b->last_launches);
+                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
   } else {
-    if (launch_fir_f16(b->plan16, b->sp_dev, b->rates_dev, b->rates_host.data(), c, st, &b->last_launches))
-      return fail(LLOID_ECUDA, "fp16 FIR launch failed");
+    if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, c, st, &b->last_launches))
+      return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (b->prof) next_event(b, st);
-    if (launch_recon_f16(b->plan16, b->sp_dev, b->bp_dev, b->upw_dev, b->partials, b->tiles_cap, c, k_a,
-                         b->cap, st, &b->last_launches))
-      return fail(LLOID_ECUDA, "fp16 reconstruction launch failed");
+    launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
+                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
   }
   if (b->prof) next_event(b, st);
   launch_merge_peaks(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, n_tiles, c, k_a,

@@ -25,8 +25,8 @@ constexpr int kLPad = 32;          // basis count padded to a multiple of this
 struct SliceParams {               // one per (bin, detector, slice); lives in a device table
   const float*  U32;               // [L_pad][n_taps]            fp32 path
   const float*  R32;               // [rows_pad][L_pad]          fp32 path
-  const __half* U16;               // [L_pad][n_taps]  K-major   fp16 path (TMA source)
-  const __half* R16;               // [rows_pad][L_pad] K-major  fp16 path (TMA source)
+  const __half* U16;               // fp16 path: packed [tap block 64][tap group 8][l L_pad][8 taps] (bulk-copy source)
+  const __half* R16;               // fp16 path: packed reconstruction matrix (tensor-core recon kernel)
   void*    Y;                      // chunk-local y^s, row-major [y_rows_cap][L_pad] (fp32 or fp16)
   int32_t  d, log2d, rate_idx;
   int32_t  n_taps, L, L_pad;
@@ -69,9 +69,10 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
 void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches);
 
+// y_is_f16: Y holds fp16 in the packed layout Y16[l / 8][row][l % 8] written by the tcgen05 FIR kernel
 void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
                       int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
-                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool y_is_f16,
                       cudaStream_t st, int64_t* launches);
 
 void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
@@ -86,10 +87,7 @@ struct F16Plan;                    // opaque host-side plan: tensor maps, work l
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,
                          int n_det, int chunk_cap, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
-int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const RateParams* rates_dev, const RateParams* rates_host,
-                    int c, cudaStream_t st, int64_t* launches);
-int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, const BinParams* bp_dev, const float* const* upw_dev,
-                      Peak* partials, int tiles_cap, int c, int64_t k_a, Capture cap, cudaStream_t st,
-                      int64_t* launches);
+int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
+                    const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches);
 
 }  // namespace lloid
