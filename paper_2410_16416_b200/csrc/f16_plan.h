@@ -1,0 +1,38 @@
+// Host-side plan of the fp16 / tcgen05 path, shared by kernels_f16.cu (basis FIR) and
+// kernels_f16_recon.cu (reconstruction + upsample + peaks).  Not part of the ABI.
+#pragma once
+#include "lloid_internal.h"
+
+#include <vector>
+
+namespace lloid {
+
+struct F16Plan {
+  // A2 basis FIR
+  int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
+  int chunk_cap = 0;
+  // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_recon_kernel) + f0-rate kernel (f0_kernel)
+  bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
+  int n_bd = 0, n_lr = 0, n_sm = 148;
+  int low_smem = 0, low_stages = 0, low_units = 0;
+  int f0_smem = 0, f0_stages = 0;
+  int p_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;
+  UpRate up[kNLowRates];
+  std::vector<RateGroup> groups_host;   // [n_bd][n_lr]
+  std::vector<BdPlan> bd_host;          // [n_bd]
+  std::vector<F0Combo> combos_host;     // every (bd, template block)
+  RateGroup* groups_dev = nullptr;
+  BdPlan* bd_dev = nullptr;
+  F0Combo* combos_dev = nullptr;
+  __half* p_dev = nullptr;
+  void* units_dev = nullptr;            // LowUnit[low_units]
+  int units_per_rate[kNLowRates] = {0, 0, 0, 0, 0};
+  std::vector<void*> owned;
+};
+
+// kernels_f16_recon.cu: fills the reconstruction part of the plan (returns false + err on a CUDA failure;
+// an unsupported bank is not an error: tensor_recon stays false).
+bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problems, const BinParams* bp_host,
+                          int n_bd, int chunk_cap, const double* const* up_w, int64_t* bytes, char* err, int errlen);
+
+}  // namespace lloid

@@ -12,8 +12,9 @@
 // each, mbarrier pipeline); MT time tiles of 128 rows share every U stage (MT accumulators in TMEM).
 //
 // Warp roles (192 threads): warp 0 = bulk-copy producer, warp 1 = MMA issuer, warps 2-5 = epilogue
-// (TMEM -> registers -> fp16 -> Y, packed in the layout the reconstruction kernel reads).
-#include "lloid_internal.h"
+// (TMEM -> registers -> fp16 -> Y, packed in the Y16 layout of lloid_internal.h that the reconstruction
+// kernels fetch with 1-D bulk copies as an MMA operand).
+#include "f16_plan.h"
 #include "tc05.cuh"
 
 #include <cstdio>
@@ -25,11 +26,6 @@ using namespace tc;
 constexpr int FH_THREADS = 192;
 constexpr int FH_KB = 64;                    // taps per pipeline stage
 constexpr int FH_MAX_STAGES = 8;
-
-struct F16Plan {
-  int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
-  int chunk_cap = 0;
-};
 
 __device__ __forceinline__ int fir_mt(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
 
@@ -140,9 +136,10 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     mbar_wait(smem_u32(&bar_acc), 0);
     fence_after();
     __half* __restrict__ Y = reinterpret_cast<__half*>(P.Y);
-    const size_t cap = (size_t)P.y_rows_cap;
+    const size_t lgs = (size_t)(L_pad >> 3);
     for (int mt = 0; mt < mt_used; ++mt) {
       const int row = r0 + mt * 128 + q * 32 + lane;
+      __half* __restrict__ Yt = Y + ((size_t)(row >> 7) * lgs * 128 + (row & 127)) * 8;   // Y16[tile][lc][row % 128][8]
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
       for (int c0 = 0; c0 < L_pad; c0 += 16) {
         uint32_t v[16];
@@ -156,8 +153,8 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
             h[i] = *reinterpret_cast<const uint32_t*>(&p);
           }
           const size_t lc = (size_t)(c0 >> 3);
-          *reinterpret_cast<uint4*>(Y + ((lc) * cap + row) * 8) = make_uint4(h[0], h[1], h[2], h[3]);
-          *reinterpret_cast<uint4*>(Y + ((lc + 1) * cap + row) * 8) = make_uint4(h[4], h[5], h[6], h[7]);
+          *reinterpret_cast<uint4*>(Yt + lc * 1024) = make_uint4(h[0], h[1], h[2], h[3]);
+          *reinterpret_cast<uint4*>(Yt + (lc + 1) * 1024) = make_uint4(h[4], h[5], h[6], h[7]);
         }
       }
     }
@@ -168,9 +165,10 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
-F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams*, int, int, int chunk_cap,
-                         char* err, int errlen)
+F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd, int n_det,
+                         int chunk_cap, const double* const* up_w, int64_t* bytes, char* err, int errlen)
 {
+  (void)n_det;
   F16Plan* pl = new F16Plan();
   pl->chunk_cap = chunk_cap;
   size_t fixed = 0, stage = 0;
@@ -198,10 +196,19 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
   pl->fir_grid_x = gx;
   cudaError_t e = cudaFuncSetAttribute(fir_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_smem);
   if (e != cudaSuccess) { snprintf(err, errlen, "cudaFuncSetAttribute(fir_f16_kernel, %d): %s", pl->fir_smem, cudaGetErrorString(e)); delete pl; return nullptr; }
+  if (!f16_plan_build_recon(pl, sp_host, n_problems, bp_host, n_bd, chunk_cap, up_w, bytes, err, errlen)) {
+    f16_plan_destroy(pl);
+    return nullptr;
+  }
   return pl;
 }
 
-void f16_plan_destroy(F16Plan* p) { delete p; }
+void f16_plan_destroy(F16Plan* p)
+{
+  if (!p) return;
+  for (void* q : p->owned) cudaFree(q);
+  delete p;
+}
 
 int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                    const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches)

@@ -1,0 +1,578 @@
+// fp16 path (LLOID_F16): A3 reconstruction, A4 upsample + sum and A5 |rho|^2 / windowed maximum on the
+// tcgen05 tensor cores (include/lloid.h A3-A5; "matrix multiplication of the orthogonal SNR time
+// series with SVD coefficients, and finally up-samples and sums the physical SNR segments").
+//
+// Two kernels per chunk, both with the SAME skeleton (warp 0 = bulk-copy producer, warp 1 = single-thread
+// MMA issuer, warps 2-5 = epilogue; a ring of 8 KB operand stages; two TMEM accumulator buffers of
+// 2 x 128 columns so the epilogue of tile t overlaps the MMAs of tile t + 1):
+//
+//  lowrate_recon_kernel   rho^(d)[i, j] = sum_{slices s at rate d} sum_l R^s[i, l] y^s_l[j]     (d > 1)
+//      A = R^s (stationary in shared memory for the CTA's 128 templates), B = y^s tiles streamed from L2,
+//      D[lane = template, column = low-rate time].  Slices that share a rate are summed BEFORE upsampling
+//      (A4 is linear and its kernel depends only on d).  Output Q16: fp16 at the LOW rate, already in the
+//      core-matrix layout in which the f0 kernel consumes it as an MMA operand.  The dense f0-rate SNR is
+//      never written anywhere.
+//
+//  f0_kernel   rho[i, k] = sum_{d = 1 slices} R^s y^s  +  sum_{d > 1} rho^(d)[i, window(k)] P_d      then A5
+//      The interpolation A4 is itself a tensor-core contraction with the fixed band matrix
+//      P_d[r, kl] = d lp_{d,K_up}[...] (16 non-zeros per column), restricted per 16-row chunk to the output
+//      columns its band touches.  Cosine and sine rows of a template go to two accumulators (columns
+//      [0,128) and [128,256)) of the SAME TMEM lane, so one epilogue thread owns one template: |rho|^2 and
+//      the running maximum over time need no cross-lane traffic at all.
+#include "f16_plan.h"
+#include "tc05.cuh"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+
+namespace lloid {
+
+using namespace tc;
+
+constexpr int RC16_THREADS = 192;
+constexpr int RC16_STAGE = 8192;            // bytes per ring stage: one K = 32 (y) or K = 16 (rho^(d)) operand chunk
+constexpr int RC16_MAX_STAGES = 16;
+constexpr int RC16_SMEM_BUDGET = 220 * 1024;
+
+struct LowUnit { int32_t group, rb; };
+
+struct RingBars {
+  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES], acc_full[2], acc_empty[2], consts;
+};
+
+__device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid)
+{
+  if (warp == 0) tmem_alloc(tmem_slot, 512);
+  if (tid == 32) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&B.full[s]), 1); mbar_init(smem_u32(&B.empty[s]), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 128); }
+    mbar_init(smem_u32(&B.consts), 1);
+    mbar_init_fence();
+  }
+}
+
+__device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, uint32_t bytes, uint32_t bar)
+{
+  for (uint32_t o = 0; o < bytes; o += 32768u) {
+    const uint32_t n = (bytes - o < 32768u) ? bytes - o : 32768u;
+    bulk_g2s(dst + o, src + o, n, bar);
+  }
+}
+
+// one K = 32 chunk of a reconstruction: D[part] (+)= Rsm[l-group lg0 .. lg0 + 3][part] * stage^T, N = 128
+__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t r_smem, int lg0, uint32_t stage, uint32_t idesc,
+                                                bool first)
+{
+#pragma unroll
+  for (int part = 0; part < 2; ++part)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const uint64_t adesc = smem_desc(r_smem + (uint32_t)(((lg0 + 2 * j) * 2 + part) * 2048), 4096u, 128u);
+      const uint64_t bdesc = smem_desc(stage + (uint32_t)(2 * j * 2048), 2048u, 128u);
+      mma_ss(d_tmem + (uint32_t)(part * 128), adesc, bdesc, idesc, (first && j == 0) ? 0u : 1u);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RC16_THREADS, 1)
+lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
+                     const LowUnit* __restrict__ units, int c, int tiles_per_cta, int n_stages)
+{
+  const LowUnit u = units[blockIdx.y];
+  const RateGroup G = groups[u.group];
+  const int rows_needed = (c >> G.log2d) + 2 * kKUp;
+  const int n_tiles = (rows_needed + 127) >> 7;
+  const int t0 = blockIdx.x * tiles_per_cta;
+  if (G.n_slices == 0 || u.rb >= G.n_rb || t0 >= n_tiles) return;
+  const int t1 = min(n_tiles, t0 + tiles_per_cta);
+
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) RingBars bars;
+  __shared__ uint32_t tmem_slot;
+  __shared__ const uint8_t* sY[kMaxGroupSlices];
+  __shared__ const uint8_t* sRsrc[kMaxGroupSlices];
+  __shared__ int sL[kMaxGroupSlices];
+  uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
+  uint8_t* ring = smem + (size_t)G.l_sum * 512;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  ring_setup(bars, &tmem_slot, n_stages, warp, tid);
+  if (tid < G.n_slices) {
+    const SliceParams P = sp[G.slice[tid]];
+    sY[tid] = reinterpret_cast<const uint8_t*>(P.Y);
+    sRsrc[tid] = reinterpret_cast<const uint8_t*>(P.R16) + (size_t)u.rb * P.L_pad * 512;
+    sL[tid] = P.L_pad;
+  }
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tmem = tmem_slot;
+  const int n_slices = G.n_slices;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)G.l_sum * 512u);
+      uint32_t off = 0;
+      for (int i = 0; i < n_slices; ++i) {
+        copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
+        off += (uint32_t)sL[i] * 512u;
+      }
+      int n = 0;
+      for (int t = t0; t < t1; ++t)
+        for (int i = 0; i < n_slices; ++i) {
+          const int lg = sL[i] >> 3;
+          const uint8_t* src = sY[i] + (size_t)t * lg * 2048;
+          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
+            const int s = n % n_stages;
+            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
+            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
+            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)kc * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
+          }
+        }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      mbar_wait(smem_u32(&bars.consts), 0);
+      fence_after();
+      const uint32_t idesc = idesc_f16(128, 128);
+      int n = 0;
+      for (int t = t0, it = 0; t < t1; ++t, ++it) {
+        const int buf = it & 1, use = it >> 1;
+        if (use >= 1) { mbar_wait(smem_u32(&bars.acc_empty[buf]), (use - 1) & 1); fence_after(); }
+        const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
+        bool first = true;
+        int lg0 = 0;
+        for (int i = 0; i < n_slices; ++i) {
+          const int lg = sL[i] >> 3;
+          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
+            const int s = n % n_stages;
+            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+            fence_after();
+            mma_recon_chunk(d_tmem, smem_u32(sR), lg0 + 4 * kc, smem_u32(ring + (size_t)s * RC16_STAGE), idesc, first);
+            first = false;
+            commit(smem_u32(&bars.empty[s]));
+          }
+          lg0 += lg;
+        }
+        commit(smem_u32(&bars.acc_full[buf]));
+      }
+    }
+  } else {
+    const int q = warp & 3;
+    const int pl = q * 32 + lane;
+    __half* __restrict__ Q = G.Q;
+    for (int t = t0, it = 0; t < t1; ++t, ++it) {
+      const int buf = it & 1, use = it >> 1;
+      mbar_wait(smem_u32(&bars.acc_full[buf]), use & 1);
+      fence_after();
+      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
+#pragma unroll 1
+      for (int part = 0; part < 2; ++part)
+#pragma unroll 1
+        for (int c0 = 0; c0 < 128; c0 += 32) {
+          uint32_t v[32];
+          tmem_ld32(taddr + (uint32_t)(part * 128 + c0), v);
+          tmem_ld_wait();
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            uint32_t h[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * g + 2 * e]), __uint_as_float(v[8 * g + 2 * e + 1]));
+              h[e] = *reinterpret_cast<const uint32_t*>(&p2);
+            }
+            const int jg = t * 16 + (c0 >> 3) + g;
+            if (jg < G.q_groups_cap)
+              *reinterpret_cast<uint4*>(Q + ((((size_t)u.rb * G.q_groups_cap + jg) * 2 + part) * 128 + pl) * 8) =
+                  make_uint4(h[0], h[1], h[2], h[3]);
+          }
+        }
+      fence_before();
+      mbar_arrive(smem_u32(&bars.acc_empty[buf]));
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+struct F0Args {
+  const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups; const uint8_t* P;
+  Peak* partials; Capture cap; long long k_a;
+  int n_lr, c, n_tiles, tiles_per_cta, tiles_cap, max_templates, n_stages, p_bytes;
+  UpRate up[kNLowRates];
+};
+
+__global__ void __launch_bounds__(RC16_THREADS, 1)
+f0_kernel(const __grid_constant__ F0Args a)
+{
+  const F0Combo cb = a.combos[blockIdx.y];
+  const BdPlan B = a.bd[cb.bd];
+  const int t0 = blockIdx.x * a.tiles_per_cta;
+  if (t0 >= a.n_tiles) return;
+  const int t1 = min(a.n_tiles, t0 + a.tiles_per_cta);
+
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) RingBars bars;
+  __shared__ uint32_t tmem_slot;
+  __shared__ const uint8_t* sY[kMaxF0Slices];
+  __shared__ const uint8_t* sRsrc[kMaxF0Slices];
+  __shared__ int sL[kMaxF0Slices];
+  __shared__ const uint8_t* sQ[kNLowRates];             // this template block's rho^(d), or null
+  uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
+  uint8_t* sP = smem + (size_t)B.l_sum * 512;           // band matrices
+  uint8_t* ring = sP + a.p_bytes;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int n_stages = a.n_stages;
+  ring_setup(bars, &tmem_slot, n_stages, warp, tid);
+  if (tid < B.n_f0) {
+    const SliceParams P = a.sp[B.f0_slice[tid]];
+    sY[tid] = reinterpret_cast<const uint8_t*>(P.Y);
+    sRsrc[tid] = reinterpret_cast<const uint8_t*>(P.R16) + (size_t)cb.rb * P.L_pad * 512;
+    sL[tid] = P.L_pad;
+  }
+  if (tid >= 64 && tid < 64 + a.n_lr) {
+    const RateGroup G = a.groups[cb.bd * a.n_lr + (tid - 64)];
+    sQ[tid - 64] = (G.n_slices > 0)
+        ? reinterpret_cast<const uint8_t*>(G.Q) + (size_t)cb.rb * G.q_groups_cap * 4096 : nullptr;
+  }
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tmem = tmem_slot;
+  const int n_f0 = B.n_f0, n_lr = a.n_lr;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)B.l_sum * 512u + (uint32_t)a.p_bytes);
+      uint32_t off = 0;
+      for (int i = 0; i < n_f0; ++i) {
+        copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
+        off += (uint32_t)sL[i] * 512u;
+      }
+      copy_pieces(smem_u32(sP), a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
+      int n = 0;
+      for (int t = t0; t < t1; ++t) {
+        for (int i = 0; i < n_f0; ++i) {
+          const int lg = sL[i] >> 3;
+          const uint8_t* src = sY[i] + (size_t)t * lg * 2048;
+          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
+            const int s = n % n_stages;
+            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
+            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
+            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)kc * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
+          }
+        }
+        for (int r = 0; r < n_lr; ++r) {
+          if (sQ[r] == nullptr) continue;
+          const UpRate& U = a.up[r];
+          const int m0 = (t * 128) >> U.log2d, ws = m0 & ~7;
+          const int var = (m0 != ws && U.n_var > 1) ? 1 : 0;
+          const uint8_t* src = sQ[r] + (size_t)(ws >> 3) * 4096;
+          for (int ch = 0; ch < (U.k_win >> 4); ++ch) {
+            if (U.nn[var][ch] == 0) continue;
+            const int s = n % n_stages;
+            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
+            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
+            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)ch * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
+            ++n;
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      mbar_wait(smem_u32(&bars.consts), 0);
+      fence_after();
+      const uint32_t idesc128 = idesc_f16(128, 128);
+      int n = 0;
+      for (int t = t0, it = 0; t < t1; ++t, ++it) {
+        const int buf = it & 1, use = it >> 1;
+        if (use >= 1) { mbar_wait(smem_u32(&bars.acc_empty[buf]), (use - 1) & 1); fence_after(); }
+        const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
+        bool first = true;
+        int lg0 = 0;
+        for (int i = 0; i < n_f0; ++i) {
+          const int lg = sL[i] >> 3;
+          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
+            const int s = n % n_stages;
+            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+            fence_after();
+            mma_recon_chunk(d_tmem, smem_u32(sR), lg0 + 4 * kc, smem_u32(ring + (size_t)s * RC16_STAGE), idesc128, first);
+            first = false;
+            commit(smem_u32(&bars.empty[s]));
+          }
+          lg0 += lg;
+        }
+        for (int r = 0; r < n_lr; ++r) {
+          if (sQ[r] == nullptr) continue;
+          const UpRate& U = a.up[r];
+          const int m0 = (t * 128) >> U.log2d, ws = m0 & ~7;
+          const int var = (m0 != ws && U.n_var > 1) ? 1 : 0;
+          const uint32_t pbase = smem_u32(sP) + (uint32_t)U.p_off[var];
+          for (int ch = 0; ch < (U.k_win >> 4); ++ch) {
+            const int nn = U.nn[var][ch];
+            if (nn == 0) continue;
+            const int n0 = U.n0[var][ch] * 8;
+            const int s = n % n_stages;
+            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+            fence_after();
+            const uint32_t stage = smem_u32(ring + (size_t)s * RC16_STAGE);
+            const uint32_t idesc = idesc_f16(128, nn * 8);
+            const uint64_t bdesc = smem_desc(pbase + (uint32_t)(2 * ch * 2048 + n0 * 16), 2048u, 128u);
+#pragma unroll
+            for (int part = 0; part < 2; ++part) {
+              const uint64_t adesc = smem_desc(stage + (uint32_t)(part * 2048), 4096u, 128u);
+              mma_ss(d_tmem + (uint32_t)(part * 128 + n0), adesc, bdesc, idesc, 1u);
+            }
+            commit(smem_u32(&bars.empty[s]));
+            ++n;
+          }
+        }
+        commit(smem_u32(&bars.acc_full[buf]));
+      }
+    }
+  } else {
+    // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
+    const int q = warp & 3;
+    const int pl = q * 32 + lane;
+    const int p = cb.rb * kTplBlock + pl;
+    const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && 2 * p + 1 < a.cap.rows;
+    for (int t = t0, it = 0; t < t1; ++t, ++it) {
+      const int buf = it & 1, use = it >> 1;
+      mbar_wait(smem_u32(&bars.acc_full[buf]), use & 1);
+      fence_after();
+      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
+      const int kap0 = t * 128;
+      const int valid = min(128, a.c - kap0);
+      float best = -1.f, bre = 0.f, bim = 0.f;
+      int bk = 0;
+#pragma unroll 1
+      for (int c0 = 0; c0 < 128; c0 += 32) {
+        uint32_t re[32], im[32];
+        tmem_ld32(taddr + (uint32_t)c0, re);
+        tmem_ld32(taddr + (uint32_t)(128 + c0), im);
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+          const float qq = fmaf(x, x, y * y);
+          if (c0 + j < valid && qq > best) { best = qq; bk = c0 + j; bre = x; bim = y; }
+        }
+        if (capture) {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const long long k = a.k_a + kap0 + c0 + j;
+            if (c0 + j < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
+              a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(re[j]);
+              a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(im[j]);
+            }
+          }
+        }
+      }
+      fence_before();
+      mbar_arrive(smem_u32(&bars.acc_empty[buf]));
+      if (p < B.n_templates) {
+        Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
+        a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+      }
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side: plan
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+bool plan_alloc(F16Plan* pl, void** p, size_t n, bool zero, int64_t* bytes, char* err, int errlen)
+{
+  if (n == 0) n = 16;
+  cudaError_t e = cudaMalloc(p, n);
+  if (e == cudaSuccess && zero) e = cudaMemset(*p, 0, n);
+  if (e != cudaSuccess) { snprintf(err, errlen, "fp16 plan: device allocation of %zu bytes failed: %s", n, cudaGetErrorString(e)); return false; }
+  pl->owned.push_back(*p);
+  *bytes += (int64_t)n;
+  return true;
+}
+
+}  // namespace
+
+bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problems, const BinParams* bp_host,
+                          int n_bd, int chunk_cap, const double* const* up_w, int64_t* bytes, char* err, int errlen)
+{
+  (void)n_problems;
+  pl->tensor_recon = false;
+  pl->n_bd = n_bd;
+  int dev = 0, n_sm = 148;
+  cudaGetDevice(&dev);
+  if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0) pl->n_sm = n_sm;
+
+  // distinct low rates, ascending d
+  bool have[kMaxRates] = {false, false, false, false, false, false};
+  for (int b = 0; b < n_bd; ++b)
+    for (int s = 0; s < bp_host[b].n_slices; ++s) have[sp_host[bp_host[b].first_slice + s].log2d] = true;
+  int lr_of[kMaxRates];
+  pl->n_lr = 0;
+  for (int l2 = 1; l2 < kMaxRates; ++l2) { lr_of[l2] = -1; if (have[l2]) { lr_of[l2] = pl->n_lr; pl->up[pl->n_lr].log2d = l2; ++pl->n_lr; } }
+
+  bool ok = true;
+  pl->bd_host.assign(n_bd, BdPlan());
+  pl->groups_host.assign((size_t)n_bd * std::max(pl->n_lr, 1), RateGroup());
+  pl->combos_host.clear();
+  pl->l_sum_f0_max = pl->l_sum_low_max = 0;
+  for (int b = 0; b < n_bd && ok; ++b) {
+    BdPlan& B = pl->bd_host[b];
+    memset(&B, 0, sizeof B);
+    B.n_templates = bp_host[b].n_templates;
+    B.n_rb = (B.n_templates + kTplBlock - 1) / kTplBlock;
+    for (int r = 0; r < pl->n_lr; ++r) {
+      RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
+      memset(&G, 0, sizeof G);
+      G.log2d = pl->up[r].log2d; G.n_rb = B.n_rb;
+      G.q_groups_cap = (((chunk_cap >> G.log2d) + 2 * kKUp + 127) / 128) * 16 + 16;
+    }
+    for (int s = 0; s < bp_host[b].n_slices; ++s) {
+      const int idx = bp_host[b].first_slice + s;
+      const SliceParams& P = sp_host[idx];
+      if (P.rows_pad != B.n_rb * 2 * kTplBlock || P.L_pad % 32) { ok = false; break; }
+      if (P.d == 1) {
+        if (B.n_f0 == kMaxF0Slices) { ok = false; break; }
+        B.f0_slice[B.n_f0++] = idx; B.l_sum += P.L_pad;
+      } else {
+        RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + lr_of[P.log2d]];
+        if (G.n_slices == kMaxGroupSlices) { ok = false; break; }
+        G.slice[G.n_slices++] = idx; G.l_sum += P.L_pad;
+      }
+    }
+    if (B.n_f0 == 0) ok = false;
+    pl->l_sum_f0_max = std::max(pl->l_sum_f0_max, B.l_sum);
+    for (int r = 0; r < pl->n_lr; ++r) pl->l_sum_low_max = std::max(pl->l_sum_low_max, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
+    for (int rb = 0; rb < B.n_rb; ++rb) pl->combos_host.push_back(F0Combo{b, rb});
+  }
+  if (!ok) return true;                                   // unsupported geometry: CUDA-core fallback
+
+  // band matrices P_d (A4):  c[kl] = sum_r Q[ws + r] P[r, kl],  ws = (128 t / d) & ~7, mis = 128 t / d - ws,
+  // P[r, kl] = w_phi[i], i = mis + floor(kl / d) + K_up - r in [-K_up, K_up), phi = kl mod d
+  std::vector<__half> pblob;
+  for (int r = 0; r < pl->n_lr; ++r) {
+    UpRate& U = pl->up[r];
+    const int d = 1 << U.log2d;
+    if (!up_w || !up_w[U.log2d]) return true;
+    const double* w = up_w[U.log2d];
+    U.n_var = (128 / d) % 8 ? 2 : 1;
+    const int mis_max = (U.n_var == 2) ? 128 / d : 0;
+    U.k_win = (128 / d + 2 * kKUp + mis_max + 15) / 16 * 16;
+    if (U.k_win / 16 > 8) return true;
+    memset(U.n0, 0, sizeof U.n0); memset(U.nn, 0, sizeof U.nn);
+    U.p_off[1] = 0;
+    for (int v = 0; v < U.n_var; ++v) {
+      const int mis = v * mis_max;
+      U.p_off[v] = (int)(pblob.size() * sizeof(__half));
+      const size_t base = pblob.size();
+      pblob.resize(base + (size_t)U.k_win * 128, __float2half(0.f));
+      std::vector<int> cmin(U.k_win / 16, 1 << 30), cmax(U.k_win / 16, -1);
+      for (int rw = 0; rw < U.k_win; ++rw)
+        for (int kl = 0; kl < 128; ++kl) {
+          const int i = mis + kl / d + kKUp - rw;
+          if (i < -kKUp || i >= kKUp) continue;
+          pblob[base + ((size_t)(rw >> 3) * 128 + kl) * 8 + (rw & 7)] = __float2half_rn((float)w[(size_t)(i + kKUp) * d + kl % d]);
+          cmin[rw >> 4] = std::min(cmin[rw >> 4], kl); cmax[rw >> 4] = std::max(cmax[rw >> 4], kl);
+        }
+      for (int ch = 0; ch < U.k_win / 16; ++ch) {
+        if (cmax[ch] < 0) continue;
+        int n0 = cmin[ch] / 8 * 8;
+        const int nn = (cmax[ch] + 1 - n0 + 15) / 16 * 16;
+        if (n0 + nn > 128) n0 = 128 - nn;
+        U.n0[v][ch] = (uint8_t)(n0 / 8); U.nn[v][ch] = (uint8_t)(nn / 8);
+      }
+    }
+  }
+  pl->p_bytes = (int)(pblob.size() * sizeof(__half));
+
+  // shared-memory budgets (operands stationary: R of the CTA's template block, and P)
+  const int f0_fixed = pl->l_sum_f0_max * 512 + pl->p_bytes;
+  const int low_fixed = pl->l_sum_low_max * 512;
+  pl->f0_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - f0_fixed) / RC16_STAGE);
+  pl->low_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - low_fixed) / RC16_STAGE);
+  if (f0_fixed > RC16_SMEM_BUDGET || low_fixed > RC16_SMEM_BUDGET || pl->f0_stages < 4 || (pl->n_lr > 0 && pl->low_stages < 4)) return true;
+  pl->f0_smem = f0_fixed + pl->f0_stages * RC16_STAGE;
+  pl->low_smem = low_fixed + pl->low_stages * RC16_STAGE;
+
+  // device tables
+  std::vector<LowUnit> units;
+  for (int r = 0; r < pl->n_lr; ++r) pl->units_per_rate[r] = 0;
+  for (int b = 0; b < n_bd; ++b)
+    for (int r = 0; r < pl->n_lr; ++r) {
+      RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
+      if (G.n_slices == 0) continue;
+      void* q = nullptr;
+      if (!plan_alloc(pl, &q, (size_t)G.n_rb * G.q_groups_cap * 4096, true, bytes, err, errlen)) return false;
+      G.Q = (__half*)q;
+      for (int rb = 0; rb < G.n_rb; ++rb) units.push_back(LowUnit{b * pl->n_lr + r, rb});
+      pl->units_per_rate[r] += G.n_rb;
+    }
+  pl->low_units = (int)units.size();
+  auto upload = [&](void** dst, const void* src, size_t n) -> bool {
+    if (!plan_alloc(pl, dst, n, false, bytes, err, errlen)) return false;
+    if (n && cudaMemcpy(*dst, src, n, cudaMemcpyHostToDevice) != cudaSuccess) { snprintf(err, errlen, "fp16 plan: table upload failed"); return false; }
+    return true;
+  };
+  if (!upload((void**)&pl->groups_dev, pl->groups_host.data(), pl->groups_host.size() * sizeof(RateGroup))) return false;
+  if (!upload((void**)&pl->bd_dev, pl->bd_host.data(), pl->bd_host.size() * sizeof(BdPlan))) return false;
+  if (!upload((void**)&pl->combos_dev, pl->combos_host.data(), pl->combos_host.size() * sizeof(F0Combo))) return false;
+  if (!upload((void**)&pl->units_dev, units.data(), units.size() * sizeof(LowUnit))) return false;
+  if (!upload((void**)&pl->p_dev, pblob.data(), pblob.size() * sizeof(__half))) return false;
+
+  cudaError_t e = cudaFuncSetAttribute(f0_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->f0_smem);
+  if (e == cudaSuccess && pl->n_lr > 0)
+    e = cudaFuncSetAttribute(lowrate_recon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->low_smem);
+  if (e != cudaSuccess) { snprintf(err, errlen, "fp16 plan: cudaFuncSetAttribute failed: %s", cudaGetErrorString(e)); return false; }
+  pl->tensor_recon = true;
+  return true;
+}
+
+bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
+
+int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
+                     int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
+{
+  const int target = 2 * pl->n_sm;
+  if (pl->low_units > 0) {
+    long long total = 0; int max_tiles = 1;
+    for (int r = 0; r < pl->n_lr; ++r) {
+      const int tiles = (((c >> pl->up[r].log2d) + 2 * kKUp) + 127) / 128;
+      total += (long long)tiles * pl->units_per_rate[r];
+      max_tiles = std::max(max_tiles, tiles);
+    }
+    const int tpc = (int)std::max<long long>(1, (total + target - 1) / target);
+    dim3 grid((max_tiles + tpc - 1) / tpc, pl->low_units);
+    lowrate_recon_kernel<<<grid, RC16_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
+                                                                  c, tpc, pl->low_stages);
+    ++*launches;
+  }
+  F0Args a;
+  memset(&a, 0, sizeof a);
+  a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;
+  a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
+  a.partials = partials; a.cap = cap; a.k_a = k_a;
+  a.n_lr = pl->n_lr; a.c = c; a.n_tiles = (c + 127) / 128;
+  const int n_combos = (int)pl->combos_host.size();
+  int ranges = (target + n_combos - 1) / n_combos;
+  ranges = std::max(1, std::min(ranges, a.n_tiles));
+  a.tiles_per_cta = (a.n_tiles + ranges - 1) / ranges;
+  a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.n_stages = pl->f0_stages; a.p_bytes = pl->p_bytes;
+  for (int r = 0; r < kNLowRates; ++r) a.up[r] = pl->up[r];
+  dim3 grid((a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta, n_combos);
+  f0_kernel<<<grid, RC16_THREADS, pl->f0_smem, st>>>(a);
+  ++*launches;
+  return cudaGetLastError() == cudaSuccess ? 0 : 1;
+}
+
+}  // namespace lloid

@@ -235,15 +235,20 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
       for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
         const int e = tid + 256 * i;
         const int ll = e % RC_KC, row = e / RC_KC;
-        Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
+        if (Y16) {                                   // packed fp16: R16[p / 128][l / 8][part][p % 128][l % 8]
+          const int i = row0 + row, p = i >> 1, l = l0 + ll;
+          Rs[ll * RC_RS + row] = __half2float(P.R16[((((size_t)(p >> 7) * (Lp >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8 + (l & 7)]);
+        } else {
+          Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
+        }
       }
-      if (Y16) {                                     // packed fp16: Y16[l / 8][row][l % 8]
+      if (Y16) {                                     // packed fp16: Y16[row / 128][l / 8][row % 128][l % 8]
         const __half* __restrict__ Yh = reinterpret_cast<const __half*>(P.Y);
         for (int e = tid; e < Ks * RC_KC; e += 256) {
           const int le = e & 7, col = (e >> 3) % Ks, lg = (e >> 3) / Ks;
           const int r = r0 + col, l = l0 + lg * 8 + le;
           Ys[(lg * 8 + le) * RC_YS + col] =
-              (r < P.y_rows_cap) ? __half2float(Yh[((size_t)(l >> 3) * P.y_rows_cap + r) * 8 + le]) : 0.f;
+              (r < P.y_rows_cap) ? __half2float(Yh[(((size_t)(r >> 7) * (Lp >> 3) + (l >> 3)) * 128 + (r & 127)) * 8 + le]) : 0.f;
         }
       } else {
         for (int e = tid; e < Ks * RC_KC; e += 256) {
@@ -337,7 +342,7 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
 
 void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
                       int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
-                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool y_is_f16,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool packed16,
                       cudaStream_t st, int64_t* launches)
 {
   (void)bp_host;
@@ -350,7 +355,7 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
   }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
   dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
-  if (y_is_f16)
+  if (packed16)
     recon_f32_kernel<true><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
                                                    c, (long long)k_a, cap);
   else

@@ -122,7 +122,8 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     *U32 = (const float*)du; *R32 = (const float*)dr;
   } else {
     // fp16 path: U packed for the tcgen05 FIR kernel as [tap block of 64][tap group of 8][l < L_pad][8 taps]
-    // (taps zero-padded to a multiple of 64); R stays fp32 for the reconstruction + interpolation epilogue.
+    // (taps zero-padded to a multiple of 64); R packed as R16[p / 128][l / 8][part][p % 128][l % 8]
+    // (lloid_internal.h): the reconstruction kernels bulk-copy a template block straight into MMA layout.
     const int n_kb = (S.n_taps + 63) / 64;
     const size_t nup = (size_t)n_kb * 64 * S.L_pad;
     std::vector<__half> u(nup, __float2half(0.f));
@@ -130,15 +131,20 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
       for (int t = 0; t < S.n_taps; ++t)
         u[(((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.L_pad + l) * 8 + (t & 7)] =
             __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
-    std::vector<float> r(nr, 0.f);
-    for (int i = 0; i < 2 * B.N; ++i)
-      for (int l = 0; l < S.L; ++l) r[(size_t)i * S.L_pad + l] = (float)recon[(size_t)i * S.L + l];
+    std::vector<__half> r(nr, __float2half(0.f));
+    const size_t lgs = (size_t)(S.L_pad >> 3);
+    for (int i = 0; i < 2 * B.N; ++i) {
+      const int p = i >> 1, part = i & 1;
+      for (int l = 0; l < S.L; ++l)
+        r[((((size_t)(p >> 7) * lgs + (l >> 3)) * 2 + part) * 128 + (p & 127)) * 8 + (l & 7)] =
+            __float2half_rn((float)recon[(size_t)i * S.L + l]);
+    }
     void *du, *dr;
     int rc = dev_alloc(b, &du, nup * 2, false); if (rc) return rc;
-    rc = dev_alloc(b, &dr, nr * 4, false); if (rc) return rc;
+    rc = dev_alloc(b, &dr, nr * 2, false); if (rc) return rc;
     CU(cudaMemcpy(du, u.data(), nup * 2, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(dr, r.data(), nr * 4, cudaMemcpyHostToDevice));
-    *U16 = (const __half*)du; *R32 = (const float*)dr;
+    CU(cudaMemcpy(dr, r.data(), nr * 2, cudaMemcpyHostToDevice));
+    *U16 = (const __half*)du; *R16 = (const __half*)dr;
   }
   return LLOID_OK;
 }
@@ -186,8 +192,14 @@ int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int6
     if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, c, st, &b->last_launches))
       return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (b->prof) next_event(b, st);
-    launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
-                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
+    if (f16_plan_tensor_recon(b->plan16)) {
+      if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
+                           &b->last_launches))
+        return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    } else {
+      launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
+                       b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
+    }
   }
   if (b->prof) next_event(b, st);
   launch_merge_peaks(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, n_tiles, c, k_a,
@@ -250,7 +262,7 @@ int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const 
       delete b; return fail(LLOID_EINVAL, "bin %d: bad descriptor", bi);
     }
     B.N = bd.n_templates; B.S = bd.n_slices; B.M = bd.template_len;
-    B.rows_pad = (int)round_up(2 * B.N, kRowPad);
+    B.rows_pad = (int)round_up(2 * B.N, b->f16 ? kRowPad16 : kRowPad);
     int64_t expect_delay = 0;
     for (int s = 0; s < B.S; ++s) {
       const lloid_slice_desc_t& sd = slices[bi][s];
@@ -360,12 +372,15 @@ int lloid_bank_finalize(lloid_bank_t* b)
       const int64_t need = (S.d == 1) ? S.end_delay + S.n_taps : S.end_delay + (int64_t)S.d * (S.n_taps + Ku + Kd);
       H = std::max(H, need);
       ybytes_per_sample += (double)D * S.L_pad * esize / S.d;
+      if (b->f16 && S.d > 1) ybytes_per_sample += (double)D * B.rows_pad * 2 / S.d;   // rho^(d) staging (upper bound)
     }
   H = round_up(H, 256);
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
   int64_t C = b->cfg.max_chunk;
   if (C == 0) {
-    const double budget = 96.0 * 1024 * 1024;
+    // keep a chunk's intermediates (y^s, and on the fp16 path the low-rate rho^(d)) within a fraction of
+    // the 126 MB L2: they are written by one kernel and consumed by the next
+    const double budget = (b->f16 ? 72.0 : 96.0) * 1024 * 1024;
     C = (int64_t)(budget / ybytes_per_sample);
     C = C / 2048 * 2048;
     C = std::min<int64_t>(std::max<int64_t>(C, 2048), 65536);
@@ -427,12 +442,18 @@ int lloid_bank_finalize(lloid_bank_t* b)
 
   // interpolation weights  w[(i + K_up) * d + phi] = d * lp_{d,K_up}[d i + phi],  i = -K_up .. K_up - 1
   std::vector<const float*> upw(kMaxRates, nullptr);
+  std::vector<std::vector<double>> upw64(kMaxRates);
   for (int d : ds) {
     if (d == 1) continue;
     std::vector<double> lp = lowpass(d, Ku);
     std::vector<float> w((size_t)2 * Ku * d);
+    std::vector<double>& w64 = upw64[ilog2(d)];
+    w64.resize(w.size());
     for (int i = -Ku; i < Ku; ++i)
-      for (int phi = 0; phi < d; ++phi) w[(size_t)(i + Ku) * d + phi] = (float)(d * lp[d * i + phi + Ku * d]);
+      for (int phi = 0; phi < d; ++phi) {
+        w64[(size_t)(i + Ku) * d + phi] = d * lp[d * i + phi + Ku * d];
+        w[(size_t)(i + Ku) * d + phi] = (float)w64[(size_t)(i + Ku) * d + phi];
+      }
     float* wd; rc = dev_alloc(b, (void**)&wd, w.size() * 4, false); if (rc) return rc;
     CU(cudaMemcpy(wd, w.data(), w.size() * 4, cudaMemcpyHostToDevice));
     upw[ilog2(d)] = wd;
@@ -456,7 +477,10 @@ int lloid_bank_finalize(lloid_bank_t* b)
 
   if (b->f16) {
     char err[256] = {0};
-    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, err, sizeof err);
+    const double* up_w[kMaxRates];
+    for (int l2 = 0; l2 < kMaxRates; ++l2) up_w[l2] = upw64[l2].empty() ? nullptr : upw64[l2].data();
+    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, up_w,
+                                &b->bytes, err, sizeof err);
     if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
   }
   b->finalized = true;

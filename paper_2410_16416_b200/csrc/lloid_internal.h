@@ -19,15 +19,18 @@ namespace lloid {
 constexpr int kKUp = 8;            // interpolation half-width supported by the kernels
 constexpr int kTimeTile = 128;     // f0 samples per epilogue tile; chunk starts are aligned to it
 constexpr int kMaxRates = 6;       // d in {1,2,4,8,16,32}
-constexpr int kRowPad = 128;       // reconstruction rows padded to a multiple of this
+constexpr int kRowPad = 128;       // reconstruction rows padded to a multiple of this (fp32 path)
+constexpr int kRowPad16 = 256;     // fp16 path: 2 x 128 templates per reconstruction CTA
+constexpr int kMaxGroupSlices = 8; // slices of one (bin, detector) that share a rate
+constexpr int kMaxF0Slices = 4;    // full-rate (d == 1) slices of one (bin, detector)
 constexpr int kLPad = 32;          // basis count padded to a multiple of this
 
 struct SliceParams {               // one per (bin, detector, slice); lives in a device table
   const float*  U32;               // [L_pad][n_taps]            fp32 path
   const float*  R32;               // [rows_pad][L_pad]          fp32 path
   const __half* U16;               // fp16 path: packed [tap block 64][tap group 8][l L_pad][8 taps] (bulk-copy source)
-  const __half* R16;               // fp16 path: packed reconstruction matrix (tensor-core recon kernel)
-  void*    Y;                      // chunk-local y^s, row-major [y_rows_cap][L_pad] (fp32 or fp16)
+  const __half* R16;               // fp16 path: packed R16 layout (below)
+  void*    Y;                      // chunk-local y^s: fp32 row-major [y_rows_cap][L_pad], or fp16 packed Y16 (below)
   int32_t  d, log2d, rate_idx;
   int32_t  n_taps, L, L_pad;
   int32_t  rows, rows_pad;         // 2N and its padding
@@ -69,10 +72,11 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
 void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches);
 
-// y_is_f16: Y holds fp16 in the packed layout Y16[l / 8][row][l % 8] written by the tcgen05 FIR kernel
+// packed16: Y and R are the packed fp16 arrays Y16 / R16 of the tcgen05 path (fallback for banks the
+// tensor reconstruction kernels do not cover)
 void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const BinParams* bp_host,
                       int n_bd, int max_rows_pad, const float* const* upw_dev, Peak* partials,
-                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool y_is_f16,
+                      int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool packed16,
                       cudaStream_t st, int64_t* launches);
 
 void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
@@ -82,12 +86,55 @@ void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, co
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
 
-// fp16 / tcgen05 path (kernels_f16.cu)
-struct F16Plan;                    // opaque host-side plan: tensor maps, work lists
+// parallel A5/A6: one thread per (bin, detector, template, peak window touched by the chunk)
+void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
+                          int tiles_cap, int c, int64_t k_a, int W, float theta, PeakState* state,
+                          int n_det, void* triggers, int64_t capacity, unsigned long long* count,
+                          cudaStream_t st, int64_t* launches);
+
+// fp16 / tcgen05 path (kernels_f16.cu: basis FIR; kernels_f16_recon.cu: reconstruction + upsample + peaks)
+//
+// Packed fp16 layouts (all are the tcgen05 no-swizzle K-major canonical layout: a core matrix is 8 rows x
+// 8 fp16 = 128 contiguous bytes, so every operand tile is fetched with plain 1-D bulk copies):
+//   Y16  [time tile of 128 rows][l / 8][row % 128][l % 8]           y^s, written by the FIR kernel
+//   R16  [rb = p / 128][l / 8][part][p % 128][l % 8]                R^s, part 0 = cos rows 2p, 1 = sin rows 2p+1
+//   Q16  [rb][j / 8][part][p % 128][j % 8]                          rho^(d) = sum over the slices at rate d of R^s y^s
+constexpr int kTplBlock = 128;     // complex templates per reconstruction CTA (two M = 128 accumulators: re, im)
+constexpr int kNLowRates = kMaxRates - 1;
+
+struct RateGroup {                 // one per (bin, detector, distinct rate with d > 1)
+  int32_t  n_slices;               // 0: this (bin, detector) has no slice at this rate
+  int32_t  slice[kMaxGroupSlices]; // indices into the SliceParams table
+  int32_t  log2d, q_groups_cap;    // q_groups_cap: allocated groups of 8 low-rate samples per template block
+  int32_t  l_sum, n_rb;            // sum of L_pad over the group's slices; template blocks of 128
+  __half*  Q;
+};
+
+struct BdPlan {                    // one per (bin, detector): what the f0-rate kernel needs
+  int32_t  n_f0;                   // d == 1 slices
+  int32_t  f0_slice[kMaxF0Slices];
+  int32_t  l_sum;                  // sum of L_pad over the d == 1 slices
+  int32_t  n_templates, n_rb;
+};
+
+struct F0Combo { int32_t bd, rb; };   // (bin*detector, template block) handled back to back along time
+
+struct UpRate {                    // one per distinct rate with d > 1 (bank-wide): band matrices of A4
+  int32_t log2d, k_win;            // window length in low-rate samples (multiple of 16)
+  int32_t n_var;                   // 1, or 2 when the window start (multiple of 8 rows) alternates 0 / 4 rows off
+  int32_t p_off[2];                // byte offsets of the variants in the P blob, each [k_win / 8][128][8] fp16
+  uint8_t n0[2][8], nn[2][8];      // per variant and 16-row chunk: first output column / 8 and columns / 8 (0: skip)
+};
+
+struct F16Plan;                    // opaque host-side plan: work lists, band matrices, Q buffers
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,
-                         int n_det, int chunk_cap, char* err, int errlen);
+                         int n_det, int chunk_cap, const double* const* up_w /* [kMaxRates]: w[(i+K_up) d + phi] or null */,
+                         int64_t* bytes, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
+bool f16_plan_tensor_recon(const F16Plan*);   // false: bank outside the tensor reconstruction kernels' limits
 int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches);
+int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
+                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches);
 
 }  // namespace lloid

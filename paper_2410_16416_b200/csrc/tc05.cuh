@@ -78,6 +78,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
                  "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
                : "r"(taddr) : "memory");
 }
+// one 32-bit column of this warp's 32 lanes
+__device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr)
+{
+  uint32_t r;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr) : "memory");
+  return r;
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 // registers -> TMEM, 8 consecutive columns of this warp's 32 lanes
 __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r)
