@@ -95,51 +95,66 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// A5/A6  merge the per-tile partial maxima into the running in-window maximum of every template,
-// emit a trigger whenever a window completes and |rho| > theta (strict), reset.
-// One thread per (bin, detector, template); tiles are visited in time order so that the first
-// (lowest k) maximum wins ties (R8).
+// A5/A6  merge the per-tile partial maxima into the maximum of every peak window [wW, (w+1)W) the chunk
+// touches, emit a trigger for every window the chunk completes with |rho| > theta (strict),
+// and carry the maximum of an unfinished last window to the next chunk / call (A8).
+// One thread per (bin, detector, template, window touched by the chunk); tiles are visited in time order
+// so that the first (lowest k) maximum wins ties (R8).  Chunk starts and W are multiples of the
+// tile length, so a tile never straddles two windows.  The carried state is double-buffered (state_in is
+// the previous chunk's state_out): the thread of the first window reads it, the thread of the last one
+// writes it, and they are different threads whenever the chunk touches more than one window.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
-merge_peaks_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
-                   int tiles_cap, int n_tiles, int c, long long k_a, int W, float theta,
-                   PeakState* __restrict__ state, int n_det, lloid_trigger_t* __restrict__ trig,
-                   long long capacity, unsigned long long* __restrict__ count)
+merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
+                     int tiles_cap, int c, long long k_a, int W, float theta,
+                     const PeakState* __restrict__ state_in, PeakState* __restrict__ state_out, int n_det,
+                     lloid_trigger_t* __restrict__ trig, long long capacity, unsigned long long* __restrict__ count)
 {
   const int bd = blockIdx.y;
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   const BinParams B = bp[bd];
   if (p >= B.n_templates) return;
-  PeakState s = state[(size_t)bd * max_templates + p];
-  for (int g = 0; g < n_tiles; ++g) {
-    const Peak pk = partials[((size_t)bd * tiles_cap + g) * max_templates + p];
+  const long long w_first = k_a / W, w_last = (k_a + c - 1) / W;
+  const long long w = w_first + blockIdx.z;
+  if (w > w_last) return;
+  const long long lo = (w * W > k_a) ? w * W : k_a;
+  const long long hi = ((w + 1) * W < k_a + c) ? (w + 1) * W : k_a + c;
+  PeakState s;
+  if (w * W < k_a) s = state_in[(size_t)bd * max_templates + p];      // window began in an earlier chunk
+  else { s.q = -1.f; s.re = 0.f; s.im = 0.f; s.pad = 0; s.k = -1; }
+  const int g0 = (int)((lo - k_a) / kTimeTile), g1 = (int)((hi - k_a + kTimeTile - 1) / kTimeTile);
+  const Peak* __restrict__ pp = partials + ((size_t)bd * tiles_cap + g0) * max_templates + p;
+#pragma unroll 4
+  for (int g = g0; g < g1; ++g, pp += max_templates) {
+    const Peak pk = *pp;
     if (pk.q > s.q) { s.q = pk.q; s.re = pk.re; s.im = pk.im; s.k = k_a + pk.kappa; }
-    int kend = (g + 1) * kTimeTile; if (kend > c) kend = c;
-    if (((k_a + kend) % W) == 0) {                  // a peak window [wW, (w+1)W) is complete
-      if (s.q >= 0.f && sqrtf(s.q) > theta) {
-        const unsigned long long idx = atomicAdd(count, 1ull);
-        if ((long long)idx < capacity) {
-          lloid_trigger_t t;
-          t.bin = bd / n_det; t.detector = bd % n_det; t.template_idx = p; t.reserved = 0;
-          t.sample = s.k; t.snr_re = s.re; t.snr_im = s.im;
-          trig[idx] = t;
-        }
-      }
-      s.q = -1.f; s.re = 0.f; s.im = 0.f; s.k = -1;
+  }
+  const bool complete = (w + 1) * W <= k_a + c;
+  if (complete && s.q >= 0.f && sqrtf(s.q) > theta) {
+    const unsigned long long idx = atomicAdd(count, 1ull);
+    if ((long long)idx < capacity) {
+      lloid_trigger_t t;
+      t.bin = bd / n_det; t.detector = bd % n_det; t.template_idx = p; t.reserved = 0;
+      t.sample = s.k; t.snr_re = s.re; t.snr_im = s.im;
+      trig[idx] = t;
     }
   }
-  state[(size_t)bd * max_templates + p] = s;
+  if (w == w_last) {
+    if (complete) { s.q = -1.f; s.re = 0.f; s.im = 0.f; s.pad = 0; s.k = -1; }
+    state_out[(size_t)bd * max_templates + p] = s;
+  }
 }
 
-void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                        int tiles_cap, int n_tiles, int c, int64_t k_a, int W, float theta,
-                        PeakState* state, int n_det, void* triggers, int64_t capacity,
-                        unsigned long long* count, cudaStream_t st, int64_t* launches)
+void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
+                          int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
+                          PeakState* state_out, int n_det, void* triggers, int64_t capacity,
+                          unsigned long long* count, cudaStream_t st, int64_t* launches)
 {
-  dim3 grid((max_templates + 127) / 128, n_bd);
-  merge_peaks_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, tiles_cap, n_tiles, c,
-                                          (long long)k_a, W, theta, state, n_det,
-                                          (lloid_trigger_t*)triggers, (long long)capacity, count);
+  const int n_w = (int)((k_a + c - 1) / W - k_a / W) + 1;
+  dim3 grid((max_templates + 127) / 128, n_bd, n_w);
+  merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, tiles_cap, c, (long long)k_a, W,
+                                            theta, state_in, state_out, n_det, (lloid_trigger_t*)triggers,
+                                            (long long)capacity, count);
   ++*launches;
 }
 

@@ -96,11 +96,13 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     // ===== producer: U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
     if (lane == 0) {
       const uint8_t* src = reinterpret_cast<const uint8_t*>(P.U16);
-      for (int kb = 0; kb < n_kb; ++kb) {
-        const int s = kb % n_stages;
-        if (kb >= n_stages) mbar_wait(smem_u32(&bar_empty[s]), ((kb / n_stages) - 1) & 1);
-        mbar_expect_tx(smem_u32(&bar_full[s]), stage_bytes);
-        bulk_g2s(smem_u32(sB + (size_t)s * stage_bytes), src + (size_t)kb * stage_bytes, stage_bytes, smem_u32(&bar_full[s]));
+      const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]), sB_u = smem_u32(sB);
+      int s = 0; uint32_t ph = 0;
+      for (int kb = 0; kb < n_kb; ++kb, src += stage_bytes) {
+        mbar_wait(bempty + 8u * s, ph ^ 1u);
+        mbar_expect_tx(bfull + 8u * s, stage_bytes);
+        bulk_g2s(sB_u + (uint32_t)(s * stage_bytes), src, stage_bytes, bfull + 8u * s);
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
     }
   } else if (warp == 1) {
@@ -109,24 +111,28 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
       const int n_split = (L_pad > 256) ? 2 : 1;
       const int Nmma = L_pad / n_split;
       const uint32_t idesc = idesc_f16(128, Nmma);
-      const uint32_t cbase = smem_u32(sC);
+      const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]);
+      const uint32_t c_lo = desc_lo(smem_u32(sC), 128u);                       // Hankel array: LBO = SBO = 128
+      const uint32_t b_lo0 = desc_lo(smem_u32(sB), (uint32_t)(L_pad * 16));
+      const uint32_t b_step = (uint32_t)(stage_bytes >> 4), b_k16 = (uint32_t)(2 * L_pad);
+      int s = 0; uint32_t ph = 0;
       for (int kb = 0; kb < n_kb; ++kb) {
-        const int s = kb % n_stages;
-        mbar_wait(smem_u32(&bar_full[s]), (kb / n_stages) & 1);
+        mbar_wait(bfull + 8u * s, ph);
         fence_after();
-        const uint32_t bbase = smem_u32(sB + (size_t)s * stage_bytes);
+        const uint32_t b_lo = b_lo0 + (uint32_t)s * b_step;
         for (int mt = 0; mt < mt_used; ++mt) {
+          const uint32_t a_lo = c_lo + (uint32_t)(mt * 16 + kb * 8) * 8u;
+          const uint32_t d_t = tmem + (uint32_t)(mt * L_pad);
 #pragma unroll
           for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
-            const uint64_t adesc = smem_desc(cbase + (uint32_t)(mt * 16 + kb * 8 + k16 * 2) * 128u, 128u, 128u);
-            for (int h = 0; h < n_split; ++h) {
-              const uint64_t bdesc = smem_desc(bbase + (uint32_t)(k16 * 2) * (uint32_t)(L_pad * 16) + (uint32_t)(h * Nmma * 16),
-                                               (uint32_t)(L_pad * 16), 128u);
-              mma_ss(tmem + (uint32_t)(mt * L_pad + h * Nmma), adesc, bdesc, idesc, (kb | k16) ? 1u : 0u);
-            }
+            const uint64_t adesc = desc64(a_lo + (uint32_t)(k16 * 16));
+            for (int h = 0; h < n_split; ++h)
+              mma_ss(d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
+                     (kb | k16) ? 1u : 0u);
           }
         }
-        commit(smem_u32(&bar_empty[s]));                       // stage reusable once these MMAs have read it
+        commit(bempty + 8u * s);                                               // stage reusable once these MMAs have read it
+        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
       commit(smem_u32(&bar_acc));
     }

@@ -19,6 +19,10 @@
 //      columns its band touches.  Cosine and sine rows of a template go to two accumulators (columns
 //      [0,128) and [128,256)) of the SAME TMEM lane, so one epilogue thread owns one template: |rho|^2 and
 //      the running maximum over time need no cross-lane traffic at all.
+//
+// The producer and the MMA issuer are single threads: their per-stage instruction count is what bounds the
+// pipeline once the data is in L2, so both loops are written with incrementing ring / pointer / descriptor
+// state (no division, no 64-bit descriptor rebuild, per-CTA lookup tables in shared memory).
 #include "f16_plan.h"
 #include "tc05.cuh"
 
@@ -41,6 +45,11 @@ struct RingBars {
   uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES], acc_full[2], acc_empty[2], consts;
 };
 
+struct Ring {                               // stage index + phase parity, advanced without division
+  int s; uint32_t ph; int n;
+  __device__ __forceinline__ void advance() { if (++s == n) { s = 0; ph ^= 1u; } }
+};
+
 __device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid)
 {
   if (warp == 0) tmem_alloc(tmem_slot, 512);
@@ -60,18 +69,23 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
   }
 }
 
-// one K = 32 chunk of a reconstruction: D[part] (+)= Rsm[l-group lg0 .. lg0 + 3][part] * stage^T, N = 128
-__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t r_smem, int lg0, uint32_t stage, uint32_t idesc,
-                                                bool first)
+// producer: wait for the stage to be free, then one 8 KB bulk copy into it
+__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src)
 {
-#pragma unroll
-  for (int part = 0; part < 2; ++part)
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      const uint64_t adesc = smem_desc(r_smem + (uint32_t)(((lg0 + 2 * j) * 2 + part) * 2048), 4096u, 128u);
-      const uint64_t bdesc = smem_desc(stage + (uint32_t)(2 * j * 2048), 2048u, 128u);
-      mma_ss(d_tmem + (uint32_t)(part * 128), adesc, bdesc, idesc, (first && j == 0) ? 0u : 1u);
-    }
+  mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
+  mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
+  bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
+  rg.advance();
+}
+
+// one K = 32 chunk of a reconstruction: D[part] (+)= R[l-groups g .. g + 3][part] * stage^T, N = 128.
+// a_lo: descriptor of (group g, part 0) with LBO 4096; b_lo: descriptor of the stage with LBO 2048 (16-byte units)
+__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
+{
+  mma_ss(d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss(d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
+  mma_ss(d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss(d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -109,6 +123,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   fence_after();
   const uint32_t tmem = tmem_slot;
   const int n_slices = G.n_slices;
+  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
 
   if (warp == 0) {
     if (lane == 0) {
@@ -118,17 +133,14 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
         off += (uint32_t)sL[i] * 512u;
       }
-      int n = 0;
+      Ring rg{0, 0u, n_stages};
+      for (int i = 0; i < n_slices; ++i) sY[i] += (size_t)t0 * (sL[i] >> 3) * 2048;   // only this thread reads sY from here on
       for (int t = t0; t < t1; ++t)
         for (int i = 0; i < n_slices; ++i) {
-          const int lg = sL[i] >> 3;
-          const uint8_t* src = sY[i] + (size_t)t * lg * 2048;
-          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
-            const int s = n % n_stages;
-            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
-            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
-            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)kc * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
-          }
+          const int n_kc = sL[i] >> 5;
+          const uint8_t* src = sY[i];
+          for (int kc = 0; kc < n_kc; ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
+          sY[i] = src;                                   // tiles are contiguous in Y16
         }
     }
   } else if (warp == 1) {
@@ -136,24 +148,24 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       mbar_wait(smem_u32(&bars.consts), 0);
       fence_after();
       const uint32_t idesc = idesc_f16(128, 128);
-      int n = 0;
-      for (int t = t0, it = 0; t < t1; ++t, ++it) {
-        const int buf = it & 1, use = it >> 1;
-        if (use >= 1) { mbar_wait(smem_u32(&bars.acc_empty[buf]), (use - 1) & 1); fence_after(); }
+      const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
+      Ring rg{0, 0u, n_stages};
+      uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
+      for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+        fence_after();
         const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
-        bool first = true;
-        int lg0 = 0;
+        uint32_t first = 1u, a_lo = a_base;
         for (int i = 0; i < n_slices; ++i) {
-          const int lg = sL[i] >> 3;
-          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
-            const int s = n % n_stages;
-            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+          const int n_kc = sL[i] >> 5;
+          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
             fence_after();
-            mma_recon_chunk(d_tmem, smem_u32(sR), lg0 + 4 * kc, smem_u32(ring + (size_t)s * RC16_STAGE), idesc, first);
-            first = false;
-            commit(smem_u32(&bars.empty[s]));
+            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
+            first = 0u;
+            commit(bempty + 8u * rg.s);
+            rg.advance();
           }
-          lg0 += lg;
         }
         commit(smem_u32(&bars.acc_full[buf]));
       }
@@ -162,9 +174,9 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     const int q = warp & 3;
     const int pl = q * 32 + lane;
     __half* __restrict__ Q = G.Q;
-    for (int t = t0, it = 0; t < t1; ++t, ++it) {
-      const int buf = it & 1, use = it >> 1;
-      mbar_wait(smem_u32(&bars.acc_full[buf]), use & 1);
+    uint32_t fph = 0u;
+    for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
+      mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
       fence_after();
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
 #pragma unroll 1
@@ -205,6 +217,8 @@ struct F0Args {
   UpRate up[kNLowRates];
 };
 
+struct QItem { uint32_t idesc, b_off, d_off, pad; };    // one 16-row chunk of an interpolation: N, P offset, D column
+
 __global__ void __launch_bounds__(RC16_THREADS, 1)
 f0_kernel(const __grid_constant__ F0Args a)
 {
@@ -221,6 +235,9 @@ f0_kernel(const __grid_constant__ F0Args a)
   __shared__ const uint8_t* sRsrc[kMaxF0Slices];
   __shared__ int sL[kMaxF0Slices];
   __shared__ const uint8_t* sQ[kNLowRates];             // this template block's rho^(d), or null
+  __shared__ int sLog2d[kNLowRates], sNvar[kNLowRates];
+  __shared__ uint32_t sMask[kNLowRates][2];             // active 16-row chunks per variant
+  __shared__ __align__(16) QItem sItem[kNLowRates][2][8];
   uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
   uint8_t* sP = smem + (size_t)B.l_sum * 512;           // band matrices
   uint8_t* ring = sP + a.p_bytes;
@@ -235,15 +252,30 @@ f0_kernel(const __grid_constant__ F0Args a)
     sL[tid] = P.L_pad;
   }
   if (tid >= 64 && tid < 64 + a.n_lr) {
-    const RateGroup G = a.groups[cb.bd * a.n_lr + (tid - 64)];
-    sQ[tid - 64] = (G.n_slices > 0)
-        ? reinterpret_cast<const uint8_t*>(G.Q) + (size_t)cb.rb * G.q_groups_cap * 4096 : nullptr;
+    const int r = tid - 64;
+    const RateGroup G = a.groups[cb.bd * a.n_lr + r];
+    sQ[r] = (G.n_slices > 0) ? reinterpret_cast<const uint8_t*>(G.Q) + (size_t)cb.rb * G.q_groups_cap * 4096 : nullptr;
+    sLog2d[r] = a.up[r].log2d; sNvar[r] = a.up[r].n_var;
+  }
+  if (tid >= 96 && tid < 96 + a.n_lr * 16) {
+    const int r = (tid - 96) >> 4, v = ((tid - 96) >> 3) & 1, ch = (tid - 96) & 7;
+    const UpRate& U = a.up[r];
+    QItem it; it.idesc = 0; it.b_off = 0; it.d_off = 0; it.pad = 0;
+    if (v < U.n_var && ch < (U.k_win >> 4) && U.nn[v][ch]) {
+      it.idesc = idesc_f16(128, U.nn[v][ch] * 8);
+      it.b_off = (uint32_t)((U.p_off[v] + 2 * ch * 2048 + U.n0[v][ch] * 128) >> 4);
+      it.d_off = (uint32_t)U.n0[v][ch] * 8u;
+    }
+    sItem[r][v][ch] = it;
+    const unsigned m = __ballot_sync(__activemask(), it.idesc != 0);   // lanes of one (r, v) are 8 consecutive lanes
+    if (ch == 0) sMask[r][v] = (m >> (lane & 24)) & 0xFFu;
   }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem = tmem_slot;
   const int n_f0 = B.n_f0, n_lr = a.n_lr;
+  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
 
   if (warp == 0) {
     if (lane == 0) {
@@ -254,31 +286,25 @@ f0_kernel(const __grid_constant__ F0Args a)
         off += (uint32_t)sL[i] * 512u;
       }
       copy_pieces(smem_u32(sP), a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
-      int n = 0;
+      Ring rg{0, 0u, n_stages};
+      for (int i = 0; i < n_f0; ++i) sY[i] += (size_t)t0 * (sL[i] >> 3) * 2048;
       for (int t = t0; t < t1; ++t) {
         for (int i = 0; i < n_f0; ++i) {
-          const int lg = sL[i] >> 3;
-          const uint8_t* src = sY[i] + (size_t)t * lg * 2048;
-          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
-            const int s = n % n_stages;
-            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
-            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
-            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)kc * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
-          }
+          const int n_kc = sL[i] >> 5;
+          const uint8_t* src = sY[i];
+          for (int kc = 0; kc < n_kc; ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
+          sY[i] = src;
         }
         for (int r = 0; r < n_lr; ++r) {
-          if (sQ[r] == nullptr) continue;
-          const UpRate& U = a.up[r];
-          const int m0 = (t * 128) >> U.log2d, ws = m0 & ~7;
-          const int var = (m0 != ws && U.n_var > 1) ? 1 : 0;
-          const uint8_t* src = sQ[r] + (size_t)(ws >> 3) * 4096;
-          for (int ch = 0; ch < (U.k_win >> 4); ++ch) {
-            if (U.nn[var][ch] == 0) continue;
-            const int s = n % n_stages;
-            if (n >= n_stages) mbar_wait(smem_u32(&bars.empty[s]), ((n / n_stages) - 1) & 1);
-            mbar_expect_tx(smem_u32(&bars.full[s]), RC16_STAGE);
-            bulk_g2s(smem_u32(ring + (size_t)s * RC16_STAGE), src + (size_t)ch * RC16_STAGE, RC16_STAGE, smem_u32(&bars.full[s]));
-            ++n;
+          const uint8_t* qb = sQ[r];
+          if (qb == nullptr) continue;
+          const int m0 = (t * 128) >> sLog2d[r], ws = m0 & ~7;
+          const int var = (m0 != ws && sNvar[r] > 1) ? 1 : 0;
+          const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
+          uint32_t mask = sMask[r][var];
+          while (mask) {
+            const int ch = __ffs(mask) - 1; mask &= mask - 1;
+            produce(rg, bfull, bempty, ring_u, src + (size_t)ch * RC16_STAGE);
           }
         }
       }
@@ -288,48 +314,42 @@ f0_kernel(const __grid_constant__ F0Args a)
       mbar_wait(smem_u32(&bars.consts), 0);
       fence_after();
       const uint32_t idesc128 = idesc_f16(128, 128);
-      int n = 0;
-      for (int t = t0, it = 0; t < t1; ++t, ++it) {
-        const int buf = it & 1, use = it >> 1;
-        if (use >= 1) { mbar_wait(smem_u32(&bars.acc_empty[buf]), (use - 1) & 1); fence_after(); }
+      const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
+      const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(smem_u32(sP), 2048u);
+      Ring rg{0, 0u, n_stages};
+      uint32_t eph = 3u;
+      for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+        fence_after();
         const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
-        bool first = true;
-        int lg0 = 0;
+        uint32_t first = 1u, a_lo = a_base;
         for (int i = 0; i < n_f0; ++i) {
-          const int lg = sL[i] >> 3;
-          for (int kc = 0; kc < (lg >> 2); ++kc, ++n) {
-            const int s = n % n_stages;
-            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+          const int n_kc = sL[i] >> 5;
+          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
             fence_after();
-            mma_recon_chunk(d_tmem, smem_u32(sR), lg0 + 4 * kc, smem_u32(ring + (size_t)s * RC16_STAGE), idesc128, first);
-            first = false;
-            commit(smem_u32(&bars.empty[s]));
+            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
+            first = 0u;
+            commit(bempty + 8u * rg.s);
+            rg.advance();
           }
-          lg0 += lg;
         }
         for (int r = 0; r < n_lr; ++r) {
           if (sQ[r] == nullptr) continue;
-          const UpRate& U = a.up[r];
-          const int m0 = (t * 128) >> U.log2d, ws = m0 & ~7;
-          const int var = (m0 != ws && U.n_var > 1) ? 1 : 0;
-          const uint32_t pbase = smem_u32(sP) + (uint32_t)U.p_off[var];
-          for (int ch = 0; ch < (U.k_win >> 4); ++ch) {
-            const int nn = U.nn[var][ch];
-            if (nn == 0) continue;
-            const int n0 = U.n0[var][ch] * 8;
-            const int s = n % n_stages;
-            mbar_wait(smem_u32(&bars.full[s]), (n / n_stages) & 1);
+          const int m0 = (t * 128) >> sLog2d[r];
+          const int var = ((m0 & 7) && sNvar[r] > 1) ? 1 : 0;
+          uint32_t mask = sMask[r][var];
+          while (mask) {
+            const int ch = __ffs(mask) - 1; mask &= mask - 1;
+            const uint4 it = *reinterpret_cast<const uint4*>(&sItem[r][var][ch]);   // idesc, b_off, d_off
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
             fence_after();
-            const uint32_t stage = smem_u32(ring + (size_t)s * RC16_STAGE);
-            const uint32_t idesc = idesc_f16(128, nn * 8);
-            const uint64_t bdesc = smem_desc(pbase + (uint32_t)(2 * ch * 2048 + n0 * 16), 2048u, 128u);
-#pragma unroll
-            for (int part = 0; part < 2; ++part) {
-              const uint64_t adesc = smem_desc(stage + (uint32_t)(part * 2048), 4096u, 128u);
-              mma_ss(d_tmem + (uint32_t)(part * 128 + n0), adesc, bdesc, idesc, 1u);
-            }
-            commit(smem_u32(&bars.empty[s]));
-            ++n;
+            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+            const uint64_t bdesc = desc64(p_base + it.y);
+            mma_ss(d_tmem + it.z,        desc64(qa),        bdesc, it.x, 1u);
+            mma_ss(d_tmem + 128u + it.z, desc64(qa + 128u), bdesc, it.x, 1u);
+            commit(bempty + 8u * rg.s);
+            rg.advance();
           }
         }
         commit(smem_u32(&bars.acc_full[buf]));
@@ -341,9 +361,9 @@ f0_kernel(const __grid_constant__ F0Args a)
     const int pl = q * 32 + lane;
     const int p = cb.rb * kTplBlock + pl;
     const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && 2 * p + 1 < a.cap.rows;
-    for (int t = t0, it = 0; t < t1; ++t, ++it) {
-      const int buf = it & 1, use = it >> 1;
-      mbar_wait(smem_u32(&bars.acc_full[buf]), use & 1);
+    uint32_t fph = 0u;
+    for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
+      mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
       fence_after();
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
       const int kap0 = t * 128;
@@ -385,7 +405,6 @@ f0_kernel(const __grid_constant__ F0Args a)
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem, 512);
 }
-
 // ------------------------------------------------------------------------------------------------
 // host side: plan
 // ------------------------------------------------------------------------------------------------

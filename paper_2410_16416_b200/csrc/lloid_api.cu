@@ -72,7 +72,8 @@ struct lloid_bank {
   float* xw = nullptr;
   float* hist = nullptr;
   int H = 0, C = 0, xw_pitch = 0, tiles_cap = 0;
-  PeakState* state = nullptr;
+  PeakState* state = nullptr;            // [2][n_bd][max_templates], double-buffered per chunk
+  int state_cur = 0;
   Peak* partials = nullptr;
   const float** upw_dev = nullptr;
   std::vector<void*> owned;
@@ -182,7 +183,6 @@ int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int6
                   b->H + c, D, b->cfg.k_down, c, b->f16, st, &b->last_launches);
   if (b->prof) next_event(b, st);
   const int n_prob = (int)b->sp_host.size();
-  const int n_tiles = (c + kTimeTile - 1) / kTimeTile;
   if (!b->f16) {
     launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, c, st, &b->last_launches);
     if (b->prof) next_event(b, st);
@@ -202,9 +202,11 @@ int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int6
     }
   }
   if (b->prof) next_event(b, st);
-  launch_merge_peaks(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, n_tiles, c, k_a,
-                     b->cfg.peak_window, b->cfg.snr_threshold, b->state, D, trig, capacity, count, st,
-                     &b->last_launches);
+  const size_t nstate = (size_t)b->n_bd * b->max_templates;
+  launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, c, k_a,
+                       b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
+                       b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
+  b->state_cur ^= 1;
   if (b->prof) next_event(b, st);
   CU(cudaGetLastError());
   return LLOID_OK;
@@ -469,10 +471,10 @@ int lloid_bank_finalize(lloid_bank_t* b)
   CU(cudaMemcpy(b->rates_dev, b->rates_host.data(), b->rates_host.size() * sizeof(RateParams), cudaMemcpyHostToDevice));
 
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
-  rc = dev_alloc(b, (void**)&b->state, nstate * sizeof(PeakState), false); if (rc) return rc;
+  rc = dev_alloc(b, (void**)&b->state, 2 * nstate * sizeof(PeakState), false); if (rc) return rc;
   rc = dev_alloc(b, (void**)&b->partials, nstate * b->tiles_cap * sizeof(Peak), true); if (rc) return rc;
   rc = dev_alloc(b, (void**)&b->stage_count, 8, true); if (rc) return rc;
-  launch_reset_state(b->state, (int64_t)nstate, 0);
+  launch_reset_state(b->state, 2 * (int64_t)nstate, 0);
   CU(cudaDeviceSynchronize());
 
   if (b->f16) {
@@ -555,7 +557,7 @@ int lloid_reset(lloid_bank_t* b, void* stream)
   cudaStream_t st = (cudaStream_t)stream;
   CU(cudaSetDevice(b->cfg.device));
   CU(cudaMemsetAsync(b->hist, 0, (size_t)b->cfg.n_detectors * b->H * 4, st));
-  launch_reset_state(b->state, (int64_t)b->n_bd * b->max_templates, st);
+  launch_reset_state(b->state, 2 * (int64_t)b->n_bd * b->max_templates, st);
   b->consumed = 0;
   return LLOID_OK;
 }

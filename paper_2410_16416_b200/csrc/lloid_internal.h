@@ -79,18 +79,13 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
                       int tiles_cap, int max_templates, int c, int64_t k_a, Capture cap, bool packed16,
                       cudaStream_t st, int64_t* launches);
 
-void launch_merge_peaks(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                        int tiles_cap, int n_tiles, int c, int64_t k_a, int W, float theta,
-                        PeakState* state, int n_det, void* triggers, int64_t capacity,
-                        unsigned long long* count, cudaStream_t st, int64_t* launches);
+// A5/A6: one thread per (bin, detector, template, peak window touched by the chunk); state double-buffered
+void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
+                          int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
+                          PeakState* state_out, int n_det, void* triggers, int64_t capacity,
+                          unsigned long long* count, cudaStream_t st, int64_t* launches);
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
-
-// parallel A5/A6: one thread per (bin, detector, template, peak window touched by the chunk)
-void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                          int tiles_cap, int c, int64_t k_a, int W, float theta, PeakState* state,
-                          int n_det, void* triggers, int64_t capacity, unsigned long long* count,
-                          cudaStream_t st, int64_t* launches);
 
 // fp16 / tcgen05 path (kernels_f16.cu: basis FIR; kernels_f16_recon.cu: reconstruction + upsample + peaks)
 //

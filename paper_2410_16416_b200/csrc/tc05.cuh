@@ -19,6 +19,18 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
          ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | ((uint64_t)1 << 46);
 }
 
+// The same descriptor split in two 32-bit halves for single-thread issue loops: lo = addr >> 4 | (LBO >> 4) << 16,
+// hi = SBO >> 4 | version bit.  Every operand of this library has SBO = 128 bytes; moving an operand (by a
+// multiple of 16 bytes, inside the 256 KB shared window) only adds to lo.
+constexpr uint32_t kDescHi = (128u >> 4) | (1u << 14);
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) { return ((saddr >> 4) & 0x3FFFu) | ((lbo_bytes >> 4) << 16); }
+__device__ __forceinline__ uint64_t desc64(uint32_t lo)
+{
+  uint64_t d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "r"(lo), "r"(kDescHi));
+  return d;
+}
+
 // Instruction descriptor, kind::f16, fp16 A/B (K-major), fp32 D:  c_format[4,6) = 1 (F32), a/b format = 0
 // (F16), a/b major = 0 (K), n_dim[17,23) = N >> 3, m_dim[24,29) = M >> 4.
 __device__ __forceinline__ uint32_t idesc_f16(int M, int N)
