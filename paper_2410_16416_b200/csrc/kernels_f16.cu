@@ -93,36 +93,40 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
   const uint32_t tmem = tmem_slot;
 
   if (warp == 0) {
-    // ===== producer: U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
-    if (lane == 0) {
-      const uint8_t* src = reinterpret_cast<const uint8_t*>(P.U16);
-      const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]), sB_u = smem_u32(sB);
-      int s = 0; uint32_t ph = 0;
-      for (int kb = 0; kb < n_kb; ++kb, src += stage_bytes) {
-        mbar_wait(bempty + 8u * s, ph ^ 1u);
-        mbar_expect_tx(bfull + 8u * s, stage_bytes);
-        bulk_g2s(sB_u + (uint32_t)(s * stage_bytes), src, stage_bytes, bfull + 8u * s);
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
+    // ===== producer (warp-uniform; see tc05.cuh): U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
+    const uint8_t* src = bcast(reinterpret_cast<const uint8_t*>(P.U16));
+    const int n_kb_u = bcast(n_kb);
+    const uint32_t sbytes = (uint32_t)bcast(stage_bytes);
+    const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]), sB_u = bcast(smem_u32(sB));
+    int s = 0; uint32_t ph = 0;
+    for (int kb = 0; kb < n_kb_u; ++kb, src += sbytes) {
+      mbar_wait(bempty + 8u * s, ph ^ 1u);
+      if (elect_one()) {
+        mbar_expect_tx(bfull + 8u * s, sbytes);
+        bulk_g2s(sB_u + (uint32_t)s * sbytes, src, sbytes, bfull + 8u * s);
       }
+      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer =====
-    if (lane == 0) {
-      const int n_split = (L_pad > 256) ? 2 : 1;
-      const int Nmma = L_pad / n_split;
-      const uint32_t idesc = idesc_f16(128, Nmma);
-      const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]);
-      const uint32_t c_lo = desc_lo(smem_u32(sC), 128u);                       // Hankel array: LBO = SBO = 128
-      const uint32_t b_lo0 = desc_lo(smem_u32(sB), (uint32_t)(L_pad * 16));
-      const uint32_t b_step = (uint32_t)(stage_bytes >> 4), b_k16 = (uint32_t)(2 * L_pad);
-      int s = 0; uint32_t ph = 0;
-      for (int kb = 0; kb < n_kb; ++kb) {
-        mbar_wait(bfull + 8u * s, ph);
-        fence_after();
+    // ===== MMA issuer (warp-uniform) =====
+    const int Lp_u = bcast(L_pad), n_kb_u = bcast(n_kb), mt_u = bcast(mt_used);
+    const int n_split = (Lp_u > 256) ? 2 : 1;
+    const int Nmma = Lp_u / n_split;
+    const uint32_t idesc = idesc_f16(128, Nmma);
+    const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]);
+    const uint32_t c_lo = desc_lo(smem_u32(sC), 128u);                         // Hankel array: LBO = SBO = 128
+    const uint32_t b_lo0 = desc_lo(bcast(smem_u32(sB)), (uint32_t)(Lp_u * 16));
+    const uint32_t b_step = (uint32_t)(Lp_u * FH_KB * 2) >> 4, b_k16 = (uint32_t)(2 * Lp_u);
+    const uint32_t tm = bcast(tmem);
+    int s = 0; uint32_t ph = 0;
+    for (int kb = 0; kb < n_kb_u; ++kb) {
+      mbar_wait(bfull + 8u * s, ph);
+      fence_after();
+      if (elect_one()) {
         const uint32_t b_lo = b_lo0 + (uint32_t)s * b_step;
-        for (int mt = 0; mt < mt_used; ++mt) {
+        for (int mt = 0; mt < mt_u; ++mt) {
           const uint32_t a_lo = c_lo + (uint32_t)(mt * 16 + kb * 8) * 8u;
-          const uint32_t d_t = tmem + (uint32_t)(mt * L_pad);
+          const uint32_t d_t = tm + (uint32_t)(mt * Lp_u);
 #pragma unroll
           for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
             const uint64_t adesc = desc64(a_lo + (uint32_t)(k16 * 16));
@@ -132,10 +136,10 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
           }
         }
         commit(bempty + 8u * s);                                               // stage reusable once these MMAs have read it
-        if (++s == n_stages) { s = 0; ph ^= 1u; }
       }
-      commit(smem_u32(&bar_acc));
+      if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
+    if (elect_one()) commit(smem_u32(&bar_acc));
   } else {
     // ===== epilogue: TMEM -> fp16 -> Y16[lc][row][8] =====
     const int q = warp & 3;                                    // TMEM lane quarter this warp may access

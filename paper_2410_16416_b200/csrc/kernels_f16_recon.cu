@@ -69,12 +69,14 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
   }
 }
 
-// producer: wait for the stage to be free, then one 8 KB bulk copy into it
+// producer (whole warp, converged): wait for the stage to be free, then the elected lane issues one 8 KB bulk copy
 __device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src)
 {
   mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
-  mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
-  bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
+  if (elect_one()) {
+    mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
+    bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
+  }
   rg.advance();
 }
 
@@ -126,6 +128,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
 
   if (warp == 0) {
+    // ===== producer (warp-uniform; see tc05.cuh) =====
     if (lane == 0) {
       mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)G.l_sum * 512u);
       uint32_t off = 0;
@@ -133,42 +136,45 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
         off += (uint32_t)sL[i] * 512u;
       }
-      Ring rg{0, 0u, n_stages};
-      for (int i = 0; i < n_slices; ++i) sY[i] += (size_t)t0 * (sL[i] >> 3) * 2048;   // only this thread reads sY from here on
-      for (int t = t0; t < t1; ++t)
-        for (int i = 0; i < n_slices; ++i) {
-          const int n_kc = sL[i] >> 5;
-          const uint8_t* src = sY[i];
-          for (int kc = 0; kc < n_kc; ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
-          sY[i] = src;                                   // tiles are contiguous in Y16
-        }
     }
-  } else if (warp == 1) {
-    if (lane == 0) {
-      mbar_wait(smem_u32(&bars.consts), 0);
-      fence_after();
-      const uint32_t idesc = idesc_f16(128, 128);
-      const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
-      Ring rg{0, 0u, n_stages};
-      uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
-      for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
-        fence_after();
-        const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
-        uint32_t first = 1u, a_lo = a_base;
-        for (int i = 0; i < n_slices; ++i) {
-          const int n_kc = sL[i] >> 5;
-          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
-            fence_after();
-            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
-            first = 0u;
-            commit(bempty + 8u * rg.s);
-            rg.advance();
-          }
-        }
-        commit(smem_u32(&bars.acc_full[buf]));
+    __syncwarp();
+    const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
+    Ring rg{0, 0u, n_stages};
+    for (int t = t0_u; t < t1_u; ++t)
+      for (int i = 0; i < ns_u; ++i) {
+        const int L = bcast(sL[i]);
+        const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;          // tiles are contiguous in Y16
+        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
       }
+  } else if (warp == 1) {
+    // ===== MMA issuer (warp-uniform) =====
+    mbar_wait(smem_u32(&bars.consts), 0);
+    fence_after();
+    const uint32_t idesc = idesc_f16(128, 128);
+    const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
+    const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t tm = bcast(tmem);
+    Ring rg{0, 0u, n_stages};
+    uint32_t eph = 3u;                                    // bit buf: parity to wait for on acc_empty (first use: free)
+    for (int t = t0_u, buf = 0; t < t1_u; ++t, buf ^= 1) {
+      mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+      fence_after();
+      const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
+      uint32_t first = 1u, a_lo = a_base;
+      for (int i = 0; i < ns_u; ++i) {
+        const int n_kc = bcast(sL[i]) >> 5;
+        for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+          mbar_wait(bfull + 8u * rg.s, rg.ph);
+          fence_after();
+          if (elect_one()) {
+            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
+            commit(bempty + 8u * rg.s);
+          }
+          first = 0u;
+          rg.advance();
+        }
+      }
+      if (elect_one()) commit(smem_u32(&bars.acc_full[buf]));
     }
   } else {
     const int q = warp & 3;
@@ -215,9 +221,9 @@ struct F0Args {
   Peak* partials; Capture cap; long long k_a;
   int n_lr, c, n_tiles, tiles_per_cta, tiles_cap, max_templates, n_stages, p_bytes;
   UpRate up[kNLowRates];
+  QItem item[kNLowRates][2][8];                         // per rate, variant, 16-row chunk (kernel parameters: uniform loads)
+  uint32_t mask[kNLowRates][2];                         // active chunks per rate and variant
 };
-
-struct QItem { uint32_t idesc, b_off, d_off, pad; };    // one 16-row chunk of an interpolation: N, P offset, D column
 
 __global__ void __launch_bounds__(RC16_THREADS, 1)
 f0_kernel(const __grid_constant__ F0Args a)
@@ -235,9 +241,6 @@ f0_kernel(const __grid_constant__ F0Args a)
   __shared__ const uint8_t* sRsrc[kMaxF0Slices];
   __shared__ int sL[kMaxF0Slices];
   __shared__ const uint8_t* sQ[kNLowRates];             // this template block's rho^(d), or null
-  __shared__ int sLog2d[kNLowRates], sNvar[kNLowRates];
-  __shared__ uint32_t sMask[kNLowRates][2];             // active 16-row chunks per variant
-  __shared__ __align__(16) QItem sItem[kNLowRates][2][8];
   uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
   uint8_t* sP = smem + (size_t)B.l_sum * 512;           // band matrices
   uint8_t* ring = sP + a.p_bytes;
@@ -255,20 +258,6 @@ f0_kernel(const __grid_constant__ F0Args a)
     const int r = tid - 64;
     const RateGroup G = a.groups[cb.bd * a.n_lr + r];
     sQ[r] = (G.n_slices > 0) ? reinterpret_cast<const uint8_t*>(G.Q) + (size_t)cb.rb * G.q_groups_cap * 4096 : nullptr;
-    sLog2d[r] = a.up[r].log2d; sNvar[r] = a.up[r].n_var;
-  }
-  if (tid >= 96 && tid < 96 + a.n_lr * 16) {
-    const int r = (tid - 96) >> 4, v = ((tid - 96) >> 3) & 1, ch = (tid - 96) & 7;
-    const UpRate& U = a.up[r];
-    QItem it; it.idesc = 0; it.b_off = 0; it.d_off = 0; it.pad = 0;
-    if (v < U.n_var && ch < (U.k_win >> 4) && U.nn[v][ch]) {
-      it.idesc = idesc_f16(128, U.nn[v][ch] * 8);
-      it.b_off = (uint32_t)((U.p_off[v] + 2 * ch * 2048 + U.n0[v][ch] * 128) >> 4);
-      it.d_off = (uint32_t)U.n0[v][ch] * 8u;
-    }
-    sItem[r][v][ch] = it;
-    const unsigned m = __ballot_sync(__activemask(), it.idesc != 0);   // lanes of one (r, v) are 8 consecutive lanes
-    if (ch == 0) sMask[r][v] = (m >> (lane & 24)) & 0xFFu;
   }
   fence_before();
   __syncthreads();
@@ -278,6 +267,7 @@ f0_kernel(const __grid_constant__ F0Args a)
   const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
 
   if (warp == 0) {
+    // ===== producer (warp-uniform; see tc05.cuh) =====
     if (lane == 0) {
       mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)B.l_sum * 512u + (uint32_t)a.p_bytes);
       uint32_t off = 0;
@@ -286,74 +276,81 @@ f0_kernel(const __grid_constant__ F0Args a)
         off += (uint32_t)sL[i] * 512u;
       }
       copy_pieces(smem_u32(sP), a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
-      Ring rg{0, 0u, n_stages};
-      for (int i = 0; i < n_f0; ++i) sY[i] += (size_t)t0 * (sL[i] >> 3) * 2048;
-      for (int t = t0; t < t1; ++t) {
-        for (int i = 0; i < n_f0; ++i) {
-          const int n_kc = sL[i] >> 5;
-          const uint8_t* src = sY[i];
-          for (int kc = 0; kc < n_kc; ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
-          sY[i] = src;
-        }
-        for (int r = 0; r < n_lr; ++r) {
-          const uint8_t* qb = sQ[r];
-          if (qb == nullptr) continue;
-          const int m0 = (t * 128) >> sLog2d[r], ws = m0 & ~7;
-          const int var = (m0 != ws && sNvar[r] > 1) ? 1 : 0;
-          const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
-          uint32_t mask = sMask[r][var];
-          while (mask) {
-            const int ch = __ffs(mask) - 1; mask &= mask - 1;
-            produce(rg, bfull, bempty, ring_u, src + (size_t)ch * RC16_STAGE);
-          }
+    }
+    __syncwarp();
+    const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
+    Ring rg{0, 0u, n_stages};
+    for (int t = t0_u; t < t1_u; ++t) {
+      for (int i = 0; i < nf_u; ++i) {
+        const int L = bcast(sL[i]);
+        const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;
+        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
+      }
+      for (int r = 0; r < n_lr; ++r) {
+        const uint8_t* qb = bcast(sQ[r]);
+        if (qb == nullptr) continue;
+        const int m0 = (t * 128) >> a.up[r].log2d, ws = m0 & ~7;
+        const int var = (m0 != ws && a.up[r].n_var > 1) ? 1 : 0;
+        const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
+        uint32_t mask = a.mask[r][var];
+        while (mask) {
+          const int ch = __ffs(mask) - 1; mask &= mask - 1;
+          produce(rg, bfull, bempty, ring_u, src + (size_t)ch * RC16_STAGE);
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      mbar_wait(smem_u32(&bars.consts), 0);
+    // ===== MMA issuer (warp-uniform) =====
+    mbar_wait(smem_u32(&bars.consts), 0);
+    fence_after();
+    const uint32_t idesc128 = idesc_f16(128, 128);
+    const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
+    const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(smem_u32(sP), 2048u);
+    const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t tm = bcast(tmem);
+    uint32_t have_q = 0u;
+    for (int r = 0; r < n_lr; ++r) have_q |= (bcast(sQ[r]) != nullptr ? 1u : 0u) << r;
+    Ring rg{0, 0u, n_stages};
+    uint32_t eph = 3u;
+    for (int t = t0_u, buf = 0; t < t1_u; ++t, buf ^= 1) {
+      mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
       fence_after();
-      const uint32_t idesc128 = idesc_f16(128, 128);
-      const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
-      const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(smem_u32(sP), 2048u);
-      Ring rg{0, 0u, n_stages};
-      uint32_t eph = 3u;
-      for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
-        fence_after();
-        const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
-        uint32_t first = 1u, a_lo = a_base;
-        for (int i = 0; i < n_f0; ++i) {
-          const int n_kc = sL[i] >> 5;
-          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
-            fence_after();
+      const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
+      uint32_t first = 1u, a_lo = a_base;
+      for (int i = 0; i < nf_u; ++i) {
+        const int n_kc = bcast(sL[i]) >> 5;
+        for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+          mbar_wait(bfull + 8u * rg.s, rg.ph);
+          fence_after();
+          if (elect_one()) {
             mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-            first = 0u;
             commit(bempty + 8u * rg.s);
-            rg.advance();
           }
+          first = 0u;
+          rg.advance();
         }
-        for (int r = 0; r < n_lr; ++r) {
-          if (sQ[r] == nullptr) continue;
-          const int m0 = (t * 128) >> sLog2d[r];
-          const int var = ((m0 & 7) && sNvar[r] > 1) ? 1 : 0;
-          uint32_t mask = sMask[r][var];
-          while (mask) {
-            const int ch = __ffs(mask) - 1; mask &= mask - 1;
-            const uint4 it = *reinterpret_cast<const uint4*>(&sItem[r][var][ch]);   // idesc, b_off, d_off
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
-            fence_after();
-            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
-            const uint64_t bdesc = desc64(p_base + it.y);
-            mma_ss(d_tmem + it.z,        desc64(qa),        bdesc, it.x, 1u);
-            mma_ss(d_tmem + 128u + it.z, desc64(qa + 128u), bdesc, it.x, 1u);
-            commit(bempty + 8u * rg.s);
-            rg.advance();
-          }
-        }
-        commit(smem_u32(&bars.acc_full[buf]));
       }
+      for (int r = 0; r < n_lr; ++r) {
+        if (!((have_q >> r) & 1u)) continue;
+        const int m0 = (t * 128) >> a.up[r].log2d;
+        const int var = ((m0 & 7) && a.up[r].n_var > 1) ? 1 : 0;
+        uint32_t mask = a.mask[r][var];
+        while (mask) {
+          const int ch = __ffs(mask) - 1; mask &= mask - 1;
+          const QItem it = a.item[r][var][ch];
+          mbar_wait(bfull + 8u * rg.s, rg.ph);
+          fence_after();
+          if (elect_one()) {
+            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+            const uint64_t bdesc = desc64(p_base + it.b_off);
+            mma_ss(d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
+            mma_ss(d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
+            commit(bempty + 8u * rg.s);
+          }
+          rg.advance();
+        }
+      }
+      if (elect_one()) commit(smem_u32(&bars.acc_full[buf]));
     }
   } else {
     // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
@@ -588,6 +585,17 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   a.tiles_per_cta = (a.n_tiles + ranges - 1) / ranges;
   a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.n_stages = pl->f0_stages; a.p_bytes = pl->p_bytes;
   for (int r = 0; r < kNLowRates; ++r) a.up[r] = pl->up[r];
+  for (int r = 0; r < pl->n_lr; ++r)
+    for (int v = 0; v < pl->up[r].n_var; ++v)
+      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch) {
+        const UpRate& U = pl->up[r];
+        if (!U.nn[v][ch]) continue;
+        QItem& it = a.item[r][v][ch];
+        it.idesc = (1u << 4) | ((uint32_t)(U.nn[v][ch] * 8 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // idesc_f16(128, N)
+        it.b_off = (uint32_t)((U.p_off[v] + 2 * ch * 2048 + U.n0[v][ch] * 128) >> 4);
+        it.d_off = (uint32_t)U.n0[v][ch] * 8u;
+        a.mask[r][v] |= 1u << ch;
+      }
   dim3 grid((a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta, n_combos);
   f0_kernel<<<grid, RC16_THREADS, pl->f0_smem, st>>>(a);
   ++*launches;

@@ -106,6 +106,28 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r)
 }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
+// ---- warp-uniform single-thread issue -----------------------------------------------------------
+// tcgen05.mma / commit / bulk copies take their operands from UNIFORM registers.  The producer and MMA
+// warps therefore run their loops with all 32 lanes converged and predicate only the issuing instruction
+// on elect_one(): the compiler then keeps descriptors and ring state in the uniform datapath.  (Inside an
+// `if (lane == 0)` region every operand needs an R2UR broadcast loop per instruction, which made the issuing
+// thread -- not the tensor pipe -- the bottleneck.)  Values loaded from memory are made provably uniform
+// with bcast().
+__device__ __forceinline__ bool elect_one()
+{
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ uint32_t bcast(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
+__device__ __forceinline__ int bcast(int v) { return __shfl_sync(0xffffffffu, v, 0); }
+template <typename T> __device__ __forceinline__ const T* bcast(const T* p)
+{
+  const unsigned long long v = reinterpret_cast<unsigned long long>(p);
+  const uint32_t lo = __shfl_sync(0xffffffffu, (uint32_t)v, 0), hi = __shfl_sync(0xffffffffu, (uint32_t)(v >> 32), 0);
+  return reinterpret_cast<const T*>(((unsigned long long)hi << 32) | lo);
+}
+
 // ---- mbarrier ---------------------------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count)
 {
