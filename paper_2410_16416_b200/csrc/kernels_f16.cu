@@ -30,7 +30,7 @@ constexpr int FH_MAX_STAGES = 8;
 __device__ __forceinline__ int fir_mt(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
 
 __global__ void __launch_bounds__(FH_THREADS, 1)
-fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int c, int n_stages)
+fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int o, int c, int n_stages)
 {
   const SliceParams P = sp[blockIdx.y];
   const int rows_needed = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
@@ -63,7 +63,7 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
   // ---- stage the strain window and expand it into the Hankel core-matrix array --------------------
   const RateParams R = rates[P.rate_idx];
   const __half* __restrict__ xs = R.xs16 + (size_t)P.det * R.xs_len;
-  const int b0 = P.jjY0 + r0 - P.n_taps;                       // xs index of window element 0 (>= 0)
+  const int b0 = P.jjY0 + (o >> P.log2d) + r0 - P.n_taps;       // xs index of window element 0 (>= 0)
   {
     unsigned short* raw = reinterpret_cast<unsigned short*>(sRaw);
     const unsigned short* xg = reinterpret_cast<const unsigned short*>(xs);
@@ -221,7 +221,7 @@ void f16_plan_destroy(F16Plan* p)
 }
 
 int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
-                   const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches)
+                   const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches)
 {
   int gx = 1;
   for (int i = 0; i < n_problems; ++i) {
@@ -232,7 +232,7 @@ int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp
     gx = g > gx ? g : gx;
   }
   dim3 grid(gx, n_problems);
-  fir_f16_kernel<<<grid, FH_THREADS, pl->fir_smem, st>>>(sp_dev, rates_dev, c, pl->fir_stages);
+  fir_f16_kernel<<<grid, FH_THREADS, pl->fir_smem, st>>>(sp_dev, rates_dev, o, c, pl->fir_stages);
   ++*launches;
   return cudaGetLastError() == cudaSuccess ? 0 : 1;
 }

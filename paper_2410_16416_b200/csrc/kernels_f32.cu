@@ -18,7 +18,7 @@ namespace lloid {
 constexpr int FIR_TM = 128, FIR_TL = 32, FIR_KC = 64, FIR_US = 36;
 
 __global__ void __launch_bounds__(128)
-fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int c, int zs_len)
+fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int o, int c, int zs_len)
 {
   const SliceParams P = sp[blockIdx.z];
   const int rows_needed = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
@@ -33,7 +33,7 @@ fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
   const float* __restrict__ xs = R.xs32 + (size_t)P.det * R.xs_len;
   const int tid = threadIdx.x;
   const int n_taps = P.n_taps;
-  const int jj_start = P.jjY0 + r0 - n_taps;
+  const int jj_start = P.jjY0 + (o >> P.log2d) + r0 - n_taps;
   for (int i = tid; i < zs_len; i += 128) {
     const int idx = jj_start + i;
     zs[i] = (i < FIR_TM + n_taps && idx >= 0 && idx < R.xs_len) ? xs[idx] : 0.f;
@@ -88,7 +88,7 @@ fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
 }
 
 void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
-                    const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches)
+                    const RateParams* rates_dev, int n_det, int o, int c, cudaStream_t st, int64_t* launches)
 {
   (void)n_det;
   int max_rows = 0, max_lt = 0, max_taps = 0;
@@ -107,7 +107,7 @@ void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n
     configured = smem;
   }
   dim3 grid((max_rows + FIR_TM - 1) / FIR_TM, max_lt, n_problems);
-  fir_f32_kernel<<<grid, 128, smem, st>>>(sp_dev, rates_dev, c, zs_len);
+  fir_f32_kernel<<<grid, 128, smem, st>>>(sp_dev, rates_dev, o, c, zs_len);
   ++*launches;
 }
 

@@ -72,6 +72,7 @@ struct lloid_bank {
   float* xw = nullptr;
   float* hist = nullptr;
   int H = 0, C = 0, xw_pitch = 0, tiles_cap = 0;
+  int S = 0;                             // super-chunk: samples resampled by one A1 launch (multiple of C)
   PeakState* state = nullptr;            // [2][n_bd][max_templates], double-buffered per chunk
   int state_cur = 0;
   Peak* partials = nullptr;
@@ -83,7 +84,7 @@ struct lloid_bank {
   lloid_trigger_t* stage_trig = nullptr; int64_t stage_trig_cap = 0;
   unsigned long long* stage_count = nullptr;
   bool prof = false;
-  std::vector<cudaEvent_t> events; size_t events_used = 0;
+  std::vector<cudaEvent_t> events; std::vector<int> event_tag; size_t events_used = 0;
   F16Plan* plan16 = nullptr;
 
   int slice_index(int bin, int det, int s) const { return bp_host[bin * cfg.n_detectors + det].first_slice + s; }
@@ -159,39 +160,48 @@ int check_ids(const lloid_bank* b, int bin, int det, int slice)
   return LLOID_OK;
 }
 
-cudaEvent_t next_event(lloid_bank* b, cudaStream_t st)
+// profiling: the time between two consecutive events is charged to the stage tag of the later one
+enum { kTagStart = -1, kTagResample = 0, kTagFir = 1, kTagRecon = 2, kTagMerge = 3 };
+void mark(lloid_bank* b, cudaStream_t st, int tag)
 {
+  if (!b->prof) return;
   if (b->events_used == b->events.size()) {
-    cudaEvent_t e; cudaEventCreate(&e); b->events.push_back(e);
+    cudaEvent_t e; cudaEventCreate(&e); b->events.push_back(e); b->event_tag.push_back(tag);
   }
-  cudaEvent_t e = b->events[b->events_used++];
-  cudaEventRecord(e, st);
-  return e;
+  b->event_tag[b->events_used] = tag;
+  cudaEventRecord(b->events[b->events_used++], st);
 }
 
-int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int64_t k_a,
-                  lloid_trigger_t* trig, int64_t capacity, unsigned long long* count, cudaStream_t st)
+// A1 for one super-chunk [k_s, k_s + n_s): xw = [history | strain], new history saved, every rate resampled once.
+int stage_superchunk(lloid_bank* b, const float* strain, int64_t pitch, int n_s, cudaStream_t st)
 {
   const int D = b->cfg.n_detectors;
   const size_t wp = (size_t)b->xw_pitch * 4;
-  // xw = [history | chunk]; then save the new history (last H samples of [history | chunk])
   CU(cudaMemcpy2DAsync(b->xw, wp, b->hist, (size_t)b->H * 4, (size_t)b->H * 4, D, cudaMemcpyDeviceToDevice, st));
-  CU(cudaMemcpy2DAsync(b->xw + b->H, wp, strain, (size_t)pitch * 4, (size_t)c * 4, D, cudaMemcpyDeviceToDevice, st));
-  CU(cudaMemcpy2DAsync(b->hist, (size_t)b->H * 4, b->xw + c, wp, (size_t)b->H * 4, D, cudaMemcpyDeviceToDevice, st));
-  if (b->prof) next_event(b, st);
+  CU(cudaMemcpy2DAsync(b->xw + b->H, wp, strain, (size_t)pitch * 4, (size_t)n_s * 4, D, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpy2DAsync(b->hist, (size_t)b->H * 4, b->xw + n_s, wp, (size_t)b->H * 4, D, cudaMemcpyDeviceToDevice, st));
+  mark(b, st, kTagStart);
   launch_resample(b->rates_dev, b->rates_host.data(), (int)b->rates_host.size(), b->xw, b->xw_pitch,
-                  b->H + c, D, b->cfg.k_down, c, b->f16, st, &b->last_launches);
-  if (b->prof) next_event(b, st);
+                  b->H + n_s, D, b->cfg.k_down, n_s, b->f16, st, &b->last_launches);
+  mark(b, st, kTagResample);
+  return LLOID_OK;
+}
+
+// A2..A6 for one chunk [k_a, k_a + c) that starts `o` samples into the current super-chunk
+int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* trig, int64_t capacity,
+                  unsigned long long* count, cudaStream_t st)
+{
+  const int D = b->cfg.n_detectors;
   const int n_prob = (int)b->sp_host.size();
   if (!b->f16) {
-    launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, c, st, &b->last_launches);
-    if (b->prof) next_event(b, st);
+    launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, o, c, st, &b->last_launches);
+    mark(b, st, kTagFir);
     launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
                      b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
   } else {
-    if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, c, st, &b->last_launches))
+    if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, o, c, st, &b->last_launches))
       return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
-    if (b->prof) next_event(b, st);
+    mark(b, st, kTagFir);
     if (f16_plan_tensor_recon(b->plan16)) {
       if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
                            &b->last_launches))
@@ -201,13 +211,13 @@ int process_chunk(lloid_bank* b, const float* strain, int64_t pitch, int c, int6
                        b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
     }
   }
-  if (b->prof) next_event(b, st);
+  mark(b, st, kTagRecon);
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
   launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, c, k_a,
                        b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
                        b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
   b->state_cur ^= 1;
-  if (b->prof) next_event(b, st);
+  mark(b, st, kTagMerge);
   CU(cudaGetLastError());
   return LLOID_OK;
 }
@@ -380,15 +390,25 @@ int lloid_bank_finalize(lloid_bank_t* b)
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
   int64_t C = b->cfg.max_chunk;
   if (C == 0) {
-    // keep a chunk's intermediates (y^s, and on the fp16 path the low-rate rho^(d)) within a fraction of
-    // the 126 MB L2: they are written by one kernel and consumed by the next
+    // (a) keep a chunk's intermediates (y^s, and on the fp16 path the low-rate rho^(d)) within a fraction of
+    //     the 126 MB L2: they are written by one kernel and consumed by the next;
+    // (b) but give every launch enough (template block x time tile) units to fill the 148 SMs many times over,
+    //     or the per-CTA prologue (operand staging, TMEM allocation) and the launch tail dominate.
     const double budget = (b->f16 ? 72.0 : 96.0) * 1024 * 1024;
-    C = (int64_t)(budget / ybytes_per_sample);
-    C = C / 2048 * 2048;
+    int64_t c_l2 = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
+    int64_t blocks = 0;
+    for (const BinHost& B : b->bins) blocks += (int64_t)D * ((B.N + kTplBlock - 1) / kTplBlock);
+    int64_t c_work = (int64_t)kTimeTile * 148 * 28 / std::max<int64_t>(blocks, 1) / 2048 * 2048;
+    C = std::max(c_l2, c_work);
     C = std::min<int64_t>(std::max<int64_t>(C, 2048), 65536);
   }
   b->H = (int)H; b->C = (int)C;
-  b->xw_pitch = (int)round_up(H + C + 256, 64);
+  // A1 runs once per super-chunk of S samples (not per chunk): the strain is tiny (8 KB/s per detector), so a
+  // long stretch of every rate stays resident and one launch streams it at HBM speed
+  int64_t S = std::max<int64_t>(C, (int64_t)1 << 20);
+  S = S / C * C;
+  b->S = (int)S;
+  b->xw_pitch = (int)round_up(H + S + 256, 64);
   b->tiles_cap = (int)(C / kTimeTile) + 1;
 
   int rc;
@@ -407,7 +427,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
     if (R.d == 1) {
       R.xs32 = b->xw; R.xs_len = b->xw_pitch;
     } else {
-      R.xs_len = (int)round_up((H + C) / R.d + 256, 64);
+      R.xs_len = (int)round_up((H + S) / R.d + 256, 64);
       rc = dev_alloc(b, (void**)&R.xs32, (size_t)D * R.xs_len * 4, true); if (rc) return rc;
       std::vector<double> lp = lowpass(R.d, Kd);
       std::vector<float> taps(lp.size());
@@ -504,12 +524,19 @@ int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trig
   CU(cudaMemsetAsync(count_dev, 0, 8, st));
   int64_t k = b->consumed, off = 0, rem = n;
   while (rem > 0) {
-    int64_t c = std::min<int64_t>(rem, b->C);
-    const int64_t mis = k % kTimeTile;
-    if (mis) c = std::min<int64_t>(c, kTimeTile - mis);     // re-align chunk starts to the tile grid
-    int rc = process_chunk(b, strain_dev + off, n, (int)c, k, trig, capacity, (unsigned long long*)count_dev, st);
+    const int n_s = (int)std::min<int64_t>(rem, b->S);
+    int rc = stage_superchunk(b, strain_dev + off, n, n_s, st);
     if (rc) return rc;
-    k += c; off += c; rem -= c;
+    int o = 0;
+    while (o < n_s) {
+      int64_t c = std::min<int64_t>(n_s - o, b->C);
+      const int64_t mis = (k + o) % kTimeTile;
+      if (mis) c = std::min<int64_t>(c, kTimeTile - mis);   // re-align chunk starts to the tile grid
+      rc = process_chunk(b, o, (int)c, k + o, trig, capacity, (unsigned long long*)count_dev, st);
+      if (rc) return rc;
+      o += (int)c;
+    }
+    k += n_s; off += n_s; rem -= n_s;
   }
   b->consumed = k;
   return LLOID_OK;
@@ -588,13 +615,14 @@ int lloid_last_stage_ms(lloid_bank_t* b, float* out)
 {
   if (!b || !out) return fail(LLOID_EINVAL, "null argument");
   for (int i = 0; i < 5; ++i) out[i] = 0.f;
-  if (!b->prof || b->events_used < 5) return fail(LLOID_ESTATE, "profiling was not enabled for the last call");
+  if (!b->prof || b->events_used < 2) return fail(LLOID_ESTATE, "profiling was not enabled for the last call");
   CU(cudaEventSynchronize(b->events[b->events_used - 1]));
-  for (size_t i = 0; i + 4 < b->events_used; i += 5)
-    for (int s = 0; s < 4; ++s) {
-      float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[i + s], b->events[i + s + 1]));
-      out[s] += ms;
-    }
+  for (size_t i = 1; i < b->events_used; ++i) {
+    const int tag = b->event_tag[i];
+    if (tag < 0) continue;
+    float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[i - 1], b->events[i]));
+    out[tag] += ms;
+  }
   float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[0], b->events[b->events_used - 1]));
   out[4] = ms;
   return LLOID_OK;

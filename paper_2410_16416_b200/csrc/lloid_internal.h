@@ -1,10 +1,12 @@
 // Internal declarations shared by the host API (lloid_api.cu) and the kernels.  Not part of the ABI.
 //
-// Chunk-local coordinates.  lloid_filter walks the caller's buffer in chunks
-// [k_a, k_a + c).  For every detector a work strain buffer xw[H + c] holds the last H samples of
-// history followed by the chunk; xw[i] is absolute sample k_a - H + i.  A rate-d stream is indexed
-// from the same origin: xs_d[jj] is the decimated sample at absolute time k_a - H + d*jj.
-// kappa = k - k_a is the chunk-local output index, 0 <= kappa < c.
+// Coordinates.  lloid_filter walks the caller's buffer in super-chunks [k_s, k_s + n_s)
+// (A1 resamples a whole super-chunk in one launch) and each super-chunk in chunks [k_a, k_a + c),
+// k_a = k_s + o.  For every detector a work strain buffer xw[H + n_s] holds the last H samples of
+// history followed by the super-chunk; xw[i] is absolute sample k_s - H + i.  A rate-d stream is
+// indexed from the same origin: xs_d[jj] is the decimated sample at absolute time k_s - H + d*jj, so
+// a chunk's slice data starts o/d further in.  kappa = k - k_a is the chunk-local output index,
+// 0 <= kappa < c; the Y rows below are chunk-local.
 //   slice with d == 1 :  Y row r  <->  kappa = r                      rows [0, c)
 //   slice with d  > 1 :  Y row r  <->  low-rate index floor(kappa/d) = r - K_up   rows [0, c/d + 2 K_up)
 // so that for every slice   c^s[kappa] = sum_{i=-K_up}^{K_up-1} w_phi[i] rho^s[row floor(kappa/d) + K_up - i],
@@ -34,7 +36,7 @@ struct SliceParams {               // one per (bin, detector, slice); lives in a
   int32_t  d, log2d, rate_idx;
   int32_t  n_taps, L, L_pad;
   int32_t  rows, rows_pad;         // 2N and its padding
-  int32_t  jjY0;                   // xs index of Y row 0: (H-Delta)/d - K_up (d>1) or H-Delta (d==1)
+  int32_t  jjY0;                   // xs index of Y row 0 at o = 0: (H-Delta)/d - K_up (d>1) or H-Delta (d==1)
   int32_t  y_rows_cap;             // allocated Y rows
   int32_t  bin, det, slice, pad_;
 };
@@ -69,8 +71,9 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
                      const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
                      bool want_f16, cudaStream_t st, int64_t* launches);
 
+// o: offset (f0 samples) of the chunk inside the resampled super-chunk; c: chunk length
 void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
-                    const RateParams* rates_dev, int n_det, int c, cudaStream_t st, int64_t* launches);
+                    const RateParams* rates_dev, int n_det, int o, int c, cudaStream_t st, int64_t* launches);
 
 // packed16: Y and R are the packed fp16 arrays Y16 / R16 of the tcgen05 path (fallback for banks the
 // tensor reconstruction kernels do not cover)
@@ -130,7 +133,7 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
 void f16_plan_destroy(F16Plan*);
 bool f16_plan_tensor_recon(const F16Plan*);   // false: bank outside the tensor reconstruction kernels' limits
 int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
-                    const RateParams* rates_dev, int c, cudaStream_t st, int64_t* launches);
+                    const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches);
 int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
                       int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches);
 
