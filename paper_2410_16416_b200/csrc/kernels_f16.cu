@@ -94,6 +94,7 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
 
   if (warp == 0) {
     // ===== producer (warp-uniform; see tc05.cuh): U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
+    const uint32_t lead = elect_u32();
     const uint8_t* src = bcast(reinterpret_cast<const uint8_t*>(P.U16));
     const int n_kb_u = bcast(n_kb);
     const uint32_t sbytes = (uint32_t)bcast(stage_bytes);
@@ -101,14 +102,13 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     int s = 0; uint32_t ph = 0;
     for (int kb = 0; kb < n_kb_u; ++kb, src += sbytes) {
       mbar_wait(bempty + 8u * s, ph ^ 1u);
-      if (elect_one()) {
-        mbar_expect_tx(bfull + 8u * s, sbytes);
-        bulk_g2s(sB_u + (uint32_t)s * sbytes, src, sbytes, bfull + 8u * s);
-      }
+      mbar_expect_tx_e(lead, bfull + 8u * s, sbytes);
+      bulk_g2s_e(lead, sB_u + (uint32_t)s * sbytes, src, sbytes, bfull + 8u * s);
       if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
   } else if (warp == 1) {
     // ===== MMA issuer (warp-uniform) =====
+    const uint32_t lead = elect_u32();
     const int Lp_u = bcast(L_pad), n_kb_u = bcast(n_kb), mt_u = bcast(mt_used);
     const int n_split = (Lp_u > 256) ? 2 : 1;
     const int Nmma = Lp_u / n_split;
@@ -122,7 +122,7 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     for (int kb = 0; kb < n_kb_u; ++kb) {
       mbar_wait(bfull + 8u * s, ph);
       fence_after();
-      if (elect_one()) {
+      {
         const uint32_t b_lo = b_lo0 + (uint32_t)s * b_step;
         for (int mt = 0; mt < mt_u; ++mt) {
           const uint32_t a_lo = c_lo + (uint32_t)(mt * 16 + kb * 8) * 8u;
@@ -131,15 +131,15 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
           for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
             const uint64_t adesc = desc64(a_lo + (uint32_t)(k16 * 16));
             for (int h = 0; h < n_split; ++h)
-              mma_ss(d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
-                     (kb | k16) ? 1u : 0u);
+              mma_ss_e(lead, d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
+                       (kb | k16) ? 1u : 0u);
           }
         }
-        commit(bempty + 8u * s);                                               // stage reusable once these MMAs have read it
+        commit_e(lead, bempty + 8u * s);                                       // stage reusable once these MMAs have read it
       }
       if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
-    if (elect_one()) commit(smem_u32(&bar_acc));
+    commit_e(lead, smem_u32(&bar_acc));
   } else {
     // ===== epilogue: TMEM -> fp16 -> Y16[lc][row][8] =====
     const int q = warp & 3;                                    // TMEM lane quarter this warp may access

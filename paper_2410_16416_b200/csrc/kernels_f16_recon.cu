@@ -69,25 +69,24 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
   }
 }
 
-// producer (whole warp, converged): wait for the stage to be free, then the elected lane issues one 8 KB bulk copy
-__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src)
+// producer (whole warp, converged): wait for the slot to be free, then the elected lane issues one 8 KB bulk copy
+__device__ __forceinline__ void produce(uint32_t lead, Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base,
+                                        const uint8_t* src)
 {
   mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
-  if (elect_one()) {
-    mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
-    bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
-  }
+  mbar_expect_tx_e(lead, bars_full + 8u * rg.s, RC16_STAGE);
+  bulk_g2s_e(lead, ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
   rg.advance();
 }
 
 // one K = 32 chunk of a reconstruction: D[part] (+)= R[l-groups g .. g + 3][part] * stage^T, N = 128.
 // a_lo: descriptor of (group g, part 0) with LBO 4096; b_lo: descriptor of the stage with LBO 2048 (16-byte units)
-__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
+__device__ __forceinline__ void mma_recon_chunk(uint32_t lead, uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
 {
-  mma_ss(d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss(d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
-  mma_ss(d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss(d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
+  mma_ss_e(lead, d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss_e(lead, d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
+  mma_ss_e(lead, d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss_e(lead, d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -139,12 +138,13 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     }
     __syncwarp();
     const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t lead = elect_u32();
     Ring rg{0, 0u, n_stages};
     for (int t = t0_u; t < t1_u; ++t)
       for (int i = 0; i < ns_u; ++i) {
         const int L = bcast(sL[i]);
         const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;          // tiles are contiguous in Y16
-        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
+        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(lead, rg, bfull, bempty, ring_u, src);
       }
   } else if (warp == 1) {
     // ===== MMA issuer (warp-uniform) =====
@@ -153,6 +153,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     const uint32_t idesc = idesc_f16(128, 128);
     const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
     const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t lead = elect_u32();
     const uint32_t tm = bcast(tmem);
     Ring rg{0, 0u, n_stages};
     uint32_t eph = 3u;                                    // bit buf: parity to wait for on acc_empty (first use: free)
@@ -166,15 +167,13 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
           mbar_wait(bfull + 8u * rg.s, rg.ph);
           fence_after();
-          if (elect_one()) {
-            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
-            commit(bempty + 8u * rg.s);
-          }
+          mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
+          commit_e(lead, bempty + 8u * rg.s);
           first = 0u;
           rg.advance();
         }
       }
-      if (elect_one()) commit(smem_u32(&bars.acc_full[buf]));
+      commit_e(lead, smem_u32(&bars.acc_full[buf]));
     }
   } else {
     const int q = warp & 3;
@@ -221,8 +220,8 @@ struct F0Args {
   Peak* partials; Capture cap; long long k_a;
   int n_lr, c, n_tiles, tiles_per_cta, tiles_cap, max_templates, n_stages, p_bytes;
   UpRate up[kNLowRates];
-  QItem item[kNLowRates][2][8];                         // per rate, variant, 16-row chunk (kernel parameters: uniform loads)
-  uint32_t mask[kNLowRates][2];                         // active chunks per rate and variant
+  QItem item[kNLowRates][2][8];                         // per rate and variant: the active 16-row chunks, in order (kernel
+  int32_t n_items[kNLowRates][2];                       // parameters: read with uniform loads); QItem.ch = chunk index
 };
 
 __global__ void __launch_bounds__(RC16_THREADS, 1)
@@ -279,12 +278,13 @@ f0_kernel(const __grid_constant__ F0Args a)
     }
     __syncwarp();
     const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t lead = elect_u32();
     Ring rg{0, 0u, n_stages};
     for (int t = t0_u; t < t1_u; ++t) {
       for (int i = 0; i < nf_u; ++i) {
         const int L = bcast(sL[i]);
         const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;
-        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(rg, bfull, bempty, ring_u, src);
+        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(lead, rg, bfull, bempty, ring_u, src);
       }
       for (int r = 0; r < n_lr; ++r) {
         const uint8_t* qb = bcast(sQ[r]);
@@ -292,11 +292,9 @@ f0_kernel(const __grid_constant__ F0Args a)
         const int m0 = (t * 128) >> a.up[r].log2d, ws = m0 & ~7;
         const int var = (m0 != ws && a.up[r].n_var > 1) ? 1 : 0;
         const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
-        uint32_t mask = a.mask[r][var];
-        while (mask) {
-          const int ch = __ffs(mask) - 1; mask &= mask - 1;
-          produce(rg, bfull, bempty, ring_u, src + (size_t)ch * RC16_STAGE);
-        }
+        const int n_it = a.n_items[r][var];
+        for (int i = 0; i < n_it; ++i)
+          produce(lead, rg, bfull, bempty, ring_u, src + (size_t)a.item[r][var][i].ch * RC16_STAGE);
       }
     }
   } else if (warp == 1) {
@@ -307,6 +305,7 @@ f0_kernel(const __grid_constant__ F0Args a)
     const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
     const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(smem_u32(sP), 2048u);
     const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t lead = elect_u32();
     const uint32_t tm = bcast(tmem);
     uint32_t have_q = 0u;
     for (int r = 0; r < n_lr; ++r) have_q |= (bcast(sQ[r]) != nullptr ? 1u : 0u) << r;
@@ -322,10 +321,8 @@ f0_kernel(const __grid_constant__ F0Args a)
         for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
           mbar_wait(bfull + 8u * rg.s, rg.ph);
           fence_after();
-          if (elect_one()) {
-            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-            commit(bempty + 8u * rg.s);
-          }
+          mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
+          commit_e(lead, bempty + 8u * rg.s);
           first = 0u;
           rg.advance();
         }
@@ -334,23 +331,20 @@ f0_kernel(const __grid_constant__ F0Args a)
         if (!((have_q >> r) & 1u)) continue;
         const int m0 = (t * 128) >> a.up[r].log2d;
         const int var = ((m0 & 7) && a.up[r].n_var > 1) ? 1 : 0;
-        uint32_t mask = a.mask[r][var];
-        while (mask) {
-          const int ch = __ffs(mask) - 1; mask &= mask - 1;
-          const QItem it = a.item[r][var][ch];
+        const int n_it = a.n_items[r][var];
+        for (int i = 0; i < n_it; ++i) {
+          const QItem it = a.item[r][var][i];
           mbar_wait(bfull + 8u * rg.s, rg.ph);
           fence_after();
-          if (elect_one()) {
-            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
-            const uint64_t bdesc = desc64(p_base + it.b_off);
-            mma_ss(d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
-            mma_ss(d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
-            commit(bempty + 8u * rg.s);
-          }
+          const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+          const uint64_t bdesc = desc64(p_base + it.b_off);
+          mma_ss_e(lead, d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
+          mma_ss_e(lead, d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
+          commit_e(lead, bempty + 8u * rg.s);
           rg.advance();
         }
       }
-      if (elect_one()) commit(smem_u32(&bars.acc_full[buf]));
+      commit_e(lead, smem_u32(&bars.acc_full[buf]));
     }
   } else {
     // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
@@ -365,19 +359,30 @@ f0_kernel(const __grid_constant__ F0Args a)
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
       const int kap0 = t * 128;
       const int valid = min(128, a.c - kap0);
-      float best = -1.f, bre = 0.f, bim = 0.f;
-      int bk = 0;
+      // four interleaved running maxima (columns j = m mod 4) break the serial compare/select chain; merged below
+      // with "larger q, then lower k" so that the first maximum of the tile still wins (R8)
+      float bq[4] = {-1.f, -1.f, -1.f, -1.f}, bre4[4] = {0.f, 0.f, 0.f, 0.f}, bim4[4] = {0.f, 0.f, 0.f, 0.f};
+      int bk4[4] = {0, 0, 0, 0};
 #pragma unroll 1
       for (int c0 = 0; c0 < 128; c0 += 32) {
         uint32_t re[32], im[32];
         tmem_ld32(taddr + (uint32_t)c0, re);
         tmem_ld32(taddr + (uint32_t)(128 + c0), im);
         tmem_ld_wait();
+        if (c0 + 32 <= valid) {
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-          const float qq = fmaf(x, x, y * y);
-          if (c0 + j < valid && qq > best) { best = qq; bk = c0 + j; bre = x; bim = y; }
+          for (int j = 0; j < 32; ++j) {
+            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+            const float qq = fmaf(x, x, y * y);
+            if (qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+            const float qq = fmaf(x, x, y * y);
+            if (c0 + j < valid && qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
+          }
         }
         if (capture) {
 #pragma unroll
@@ -390,6 +395,11 @@ f0_kernel(const __grid_constant__ F0Args a)
           }
         }
       }
+      float best = bq[0], bre = bre4[0], bim = bim4[0];
+      int bk = bk4[0];
+#pragma unroll
+      for (int m = 1; m < 4; ++m)
+        if (bq[m] > best || (bq[m] == best && bk4[m] < bk)) { best = bq[m]; bk = bk4[m]; bre = bre4[m]; bim = bim4[m]; }
       fence_before();
       mbar_arrive(smem_u32(&bars.acc_empty[buf]));
       if (p < B.n_templates) {
@@ -590,11 +600,11 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
       for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch) {
         const UpRate& U = pl->up[r];
         if (!U.nn[v][ch]) continue;
-        QItem& it = a.item[r][v][ch];
+        QItem& it = a.item[r][v][a.n_items[r][v]++];
         it.idesc = (1u << 4) | ((uint32_t)(U.nn[v][ch] * 8 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // idesc_f16(128, N)
         it.b_off = (uint32_t)((U.p_off[v] + 2 * ch * 2048 + U.n0[v][ch] * 128) >> 4);
         it.d_off = (uint32_t)U.n0[v][ch] * 8u;
-        a.mask[r][v] |= 1u << ch;
+        it.ch = (uint32_t)ch;
       }
   dim3 grid((a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta, n_combos);
   f0_kernel<<<grid, RC16_THREADS, pl->f0_smem, st>>>(a);

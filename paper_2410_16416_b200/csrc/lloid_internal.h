@@ -124,7 +124,7 @@ struct UpRate {                    // one per distinct rate with d > 1 (bank-wid
   uint8_t n0[2][8], nn[2][8];      // per variant and 16-row chunk: first output column / 8 and columns / 8 (0: skip)
 };
 
-struct QItem { uint32_t idesc, b_off, d_off, pad; };   // one 16-row chunk of an interpolation: MMA N, P offset, D column
+struct QItem { uint32_t idesc, b_off, d_off, ch; };   // one 16-row chunk of an interpolation: MMA N, P offset, D column
 
 struct F16Plan;                    // opaque host-side plan: work lists, band matrices, Q buffers
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,

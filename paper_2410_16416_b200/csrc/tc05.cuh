@@ -52,6 +52,18 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
                "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n"
                :: "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// the same, issued only where lead != 0 (see elect_u32)
+__device__ __forceinline__ void mma_ss_e(uint32_t lead, uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+  asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %5, 0;\n\t"
+               "@q tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+               :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(lead) : "memory");
+}
+__device__ __forceinline__ void commit_e(uint32_t lead, uint32_t mbar)
+{
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t"
+               "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}\n" :: "r"(mbar), "r"(lead) : "memory");
+}
 // mbarrier arrives once all tcgen05 ops issued so far by this thread have completed
 __device__ __forceinline__ void commit(uint32_t mbar)
 {
@@ -119,6 +131,14 @@ __device__ __forceinline__ bool elect_one()
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
   return pred != 0;
 }
+// Branch-free form: `lead` (1 in the elected lane, else 0) guards the issuing instruction INSIDE the asm, so the
+// surrounding loop has no divergent region at all and ptxas keeps ring state and descriptors in uniform registers.
+__device__ __forceinline__ uint32_t elect_u32()
+{
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(pred));
+  return pred;
+}
 __device__ __forceinline__ uint32_t bcast(uint32_t v) { return __shfl_sync(0xffffffffu, v, 0); }
 __device__ __forceinline__ int bcast(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 template <typename T> __device__ __forceinline__ const T* bcast(const T* p)
@@ -147,6 +167,17 @@ __device__ __forceinline__ void mbar_arrive(uint32_t mbar)
 __device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes)
 {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_e(uint32_t lead, uint32_t mbar, uint32_t bytes)
+{
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n\t}\n"
+               :: "r"(mbar), "r"(bytes), "r"(lead) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_e(uint32_t lead, uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t mbar)
+{
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %4, 0;\n\t"
+               "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n\t}\n"
+               :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(mbar), "r"(lead) : "memory");
 }
 // global -> shared bulk copy (bytes multiple of 16, both addresses 16-byte aligned); completes on mbar
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t mbar)
