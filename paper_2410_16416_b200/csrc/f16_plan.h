@@ -25,8 +25,12 @@ struct F16Plan {
   BdPlan* bd_dev = nullptr;
   F0Combo* combos_dev = nullptr;
   __half* p_dev = nullptr;
-  void* units_dev = nullptr;            // LowUnit[low_units]
+  void* units_dev = nullptr;            // LowUnit[low_units], rate-major
   int units_per_rate[kNLowRates] = {0, 0, 0, 0, 0};
+  SchedUnit* low_sched_dev = nullptr;   // [low_units]   cost per tile of every low-rate unit
+  SchedUnit* f0_sched_dev = nullptr;    // [combos]      cost per tile of every f0 unit
+  long long low_wsum[kNLowRates] = {0, 0, 0, 0, 0};
+  long long f0_wsum = 0;
   std::vector<void*> owned;
 };
 

@@ -50,6 +50,43 @@ struct Ring {                               // stage index + phase parity, advan
   __device__ __forceinline__ void advance() { if (++s == n) { s = 0; ph ^= 1u; } }
 };
 
+// ---- static persistent schedule (SchedArgs in lloid_internal.h) ------------------------------------
+struct SchedPos { int u, t; };              // unit index, first tile
+
+__device__ __forceinline__ SchedPos sched_locate(const SchedArgs& s, long long b)
+{
+  SchedPos r;
+  if (b >= s.cls_base[s.n_cls]) { r.u = s.cls_begin[s.n_cls]; r.t = 0; return r; }
+  int c = 0;
+  while (c + 1 < s.n_cls && b >= s.cls_base[c + 1]) ++c;
+  const long long rem = b - s.cls_base[c];
+  const long long nt = s.n_tiles[c];
+  int lo = s.cls_begin[c], hi = s.cls_begin[c + 1] - 1;   // largest u with wprefix[u] * nt <= rem
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if ((long long)s.units[mid].wprefix * nt <= rem) lo = mid; else hi = mid - 1;
+  }
+  const SchedUnit su = s.units[lo];
+  r.u = lo; r.t = (int)((rem - (long long)su.wprefix * nt) / su.w);
+  return r;
+}
+
+// this CTA's range -> rng[0..3] = first unit, first tile, last unit, end tile in the last unit
+__device__ __forceinline__ void sched_range(const SchedArgs& s, int* rng)
+{
+  const long long T = s.cls_base[s.n_cls];
+  const SchedPos a = sched_locate(s, T * (long long)blockIdx.x / (long long)gridDim.x);
+  const SchedPos b = sched_locate(s, T * (long long)(blockIdx.x + 1) / (long long)gridDim.x);
+  rng[0] = a.u; rng[1] = a.t; rng[2] = b.u; rng[3] = b.t;
+}
+
+__device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
+{
+  int c = 0;
+  while (c + 1 < s.n_cls && u >= s.cls_begin[c + 1]) ++c;
+  return c;
+}
+
 __device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid)
 {
   if (warp == 0) tmem_alloc(tmem_slot, 512);
@@ -90,123 +127,177 @@ __device__ __forceinline__ void mma_recon_chunk(uint32_t lead, uint32_t d_tmem, 
 }
 
 // ------------------------------------------------------------------------------------------------
+struct SegLow {                             // per-role copy of the current unit's operand sources
+  const uint8_t* Y[kMaxGroupSlices];
+  const uint8_t* Rsrc[kMaxGroupSlices];
+  int L[kMaxGroupSlices];
+};
+
+__device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __restrict__ sp, const RateGroup& G, int rb, int lane)
+{
+  if (lane < G.n_slices) {
+    const SliceParams* P = sp + G.slice[lane];
+    const int L = P->L_pad;
+    S.Y[lane] = reinterpret_cast<const uint8_t*>(P->Y);
+    S.Rsrc[lane] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 512;
+    S.L[lane] = L;
+  }
+  __syncwarp();
+}
+
+// Persistent: CTA i of gridDim.x runs cost range i of the (rate, unit, tile) sequence (SchedArgs).  At a unit
+// switch the producer first refills the ring with the next unit's y tiles, then waits for the previous unit's
+// last accumulator (all MMAs that read the old R are complete) and only then replaces R: the bubble is one R load.
 __global__ void __launch_bounds__(RC16_THREADS, 1)
 lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
-                     const LowUnit* __restrict__ units, int c, int tiles_per_cta, int n_stages)
+                     const LowUnit* __restrict__ units, const __grid_constant__ SchedArgs sched, int r_bytes, int n_stages)
 {
-  const LowUnit u = units[blockIdx.y];
-  const RateGroup G = groups[u.group];
-  const int rows_needed = (c >> G.log2d) + 2 * kKUp;
-  const int n_tiles = (rows_needed + 127) >> 7;
-  const int t0 = blockIdx.x * tiles_per_cta;
-  if (G.n_slices == 0 || u.rb >= G.n_rb || t0 >= n_tiles) return;
-  const int t1 = min(n_tiles, t0 + tiles_per_cta);
-
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) RingBars bars;
   __shared__ uint32_t tmem_slot;
-  __shared__ const uint8_t* sY[kMaxGroupSlices];
-  __shared__ const uint8_t* sRsrc[kMaxGroupSlices];
-  __shared__ int sL[kMaxGroupSlices];
-  uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
-  uint8_t* ring = smem + (size_t)G.l_sum * 512;
+  __shared__ SegLow seg[2];                             // [0] producer's, [1] MMA issuer's
+  __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) sched_range(sched, s_rng);
+  __syncthreads();
+  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
+  if (u_lo == u_hi && t_lo == t_hi) return;
+
   ring_setup(bars, &tmem_slot, n_stages, warp, tid);
-  if (tid < G.n_slices) {
-    const SliceParams P = sp[G.slice[tid]];
-    sY[tid] = reinterpret_cast<const uint8_t*>(P.Y);
-    sRsrc[tid] = reinterpret_cast<const uint8_t*>(P.R16) + (size_t)u.rb * P.L_pad * 512;
-    sL[tid] = P.L_pad;
-  }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem = tmem_slot;
-  const int n_slices = G.n_slices;
-  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
+  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]);
+  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16
+  const uint32_t ring_u = sR_u + (uint32_t)r_bytes;
 
   if (warp == 0) {
     // ===== producer (warp-uniform; see tc05.cuh) =====
-    if (lane == 0) {
-      mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)G.l_sum * 512u);
-      uint32_t off = 0;
-      for (int i = 0; i < n_slices; ++i) {
-        copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
-        off += (uint32_t)sL[i] * 512u;
-      }
-    }
-    __syncwarp();
-    const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
     const uint32_t lead = elect_u32();
     Ring rg{0, 0u, n_stages};
-    for (int t = t0_u; t < t1_u; ++t)
-      for (int i = 0; i < ns_u; ++i) {
-        const int L = bcast(sL[i]);
-        const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;          // tiles are contiguous in Y16
-        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(lead, rg, bfull, bempty, ring_u, src);
-      }
+    int g = 0, seg_i = 0;                               // tiles / segments done so far by this CTA
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int cls = sched_class(sched, u);
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
+      if (t0 >= t1) continue;
+      const LowUnit un = units[u];
+      const RateGroup G = groups[un.group];
+      seg_low_fill(seg[0], sp, G, un.rb, lane);
+      const int ns_u = bcast(G.n_slices);
+      const uint32_t rbytes_u = (uint32_t)bcast(G.l_sum) * 512u;
+      int countdown = (seg_i == 0) ? 0 : n_stages;      // ring stages to push before R is replaced
+      bool r_done = false;
+      auto load_R = [&]() {
+        if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
+        if (lane == 0) {
+          mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
+          uint32_t off = 0;
+          for (int i = 0; i < ns_u; ++i) {
+            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, smem_u32(&bars.consts));
+            off += (uint32_t)seg[0].L[i] * 512u;
+          }
+        }
+        __syncwarp();
+        r_done = true;
+      };
+      if (countdown == 0) load_R();
+      for (int t = t0; t < t1; ++t)
+        for (int i = 0; i < ns_u; ++i) {
+          const int L = bcast(seg[0].L[i]);
+          const uint8_t* src = bcast(seg[0].Y[i]) + (size_t)t * L * 256;          // tiles are contiguous in Y16
+          for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
+            produce(lead, rg, bfull, bempty, ring_u, src);
+            if (!r_done && --countdown == 0) load_R();
+          }
+        }
+      if (!r_done) load_R();
+      g += t1 - t0; ++seg_i;
+    }
   } else if (warp == 1) {
     // ===== MMA issuer (warp-uniform) =====
-    mbar_wait(smem_u32(&bars.consts), 0);
-    fence_after();
     const uint32_t idesc = idesc_f16(128, 128);
-    const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
-    const int ns_u = bcast(n_slices), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
     const uint32_t lead = elect_u32();
     const uint32_t tm = bcast(tmem);
     Ring rg{0, 0u, n_stages};
-    uint32_t eph = 3u;                                    // bit buf: parity to wait for on acc_empty (first use: free)
-    for (int t = t0_u, buf = 0; t < t1_u; ++t, buf ^= 1) {
-      mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+    uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
+    int buf = 0, seg_i = 0;
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int cls = sched_class(sched, u);
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
+      if (t0 >= t1) continue;
+      const LowUnit un = units[u];
+      const RateGroup G = groups[un.group];
+      seg_low_fill(seg[1], sp, G, un.rb, lane);
+      const int ns_u = bcast(G.n_slices);
+      mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
       fence_after();
-      const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
-      uint32_t first = 1u, a_lo = a_base;
-      for (int i = 0; i < ns_u; ++i) {
-        const int n_kc = bcast(sL[i]) >> 5;
-        for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-          mbar_wait(bfull + 8u * rg.s, rg.ph);
-          fence_after();
-          mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
-          commit_e(lead, bempty + 8u * rg.s);
-          first = 0u;
-          rg.advance();
+      for (int t = t0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+        fence_after();
+        const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
+        uint32_t first = 1u, a_lo = a_base;
+        for (int i = 0; i < ns_u; ++i) {
+          const int n_kc = bcast(seg[1].L[i]) >> 5;
+          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
+            fence_after();
+            mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
+            commit_e(lead, bempty + 8u * rg.s);
+            first = 0u;
+            rg.advance();
+          }
         }
+        commit_e(lead, smem_u32(&bars.acc_full[buf]));
       }
-      commit_e(lead, smem_u32(&bars.acc_full[buf]));
+      ++seg_i;
     }
   } else {
     const int q = warp & 3;
     const int pl = q * 32 + lane;
-    __half* __restrict__ Q = G.Q;
     uint32_t fph = 0u;
-    for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
-      mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
-      fence_after();
-      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
+    int buf = 0;
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int cls = sched_class(sched, u);
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
+      if (t0 >= t1) continue;
+      const LowUnit un = units[u];
+      const RateGroup* Gp = groups + un.group;
+      __half* __restrict__ Q = Gp->Q;
+      const int q_cap = Gp->q_groups_cap;
+      for (int t = t0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
+        fence_after();
+        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
 #pragma unroll 1
-      for (int part = 0; part < 2; ++part)
+        for (int part = 0; part < 2; ++part)
 #pragma unroll 1
-        for (int c0 = 0; c0 < 128; c0 += 32) {
-          uint32_t v[32];
-          tmem_ld32(taddr + (uint32_t)(part * 128 + c0), v);
-          tmem_ld_wait();
+          for (int c0 = 0; c0 < 128; c0 += 32) {
+            uint32_t v[32];
+            tmem_ld32(taddr + (uint32_t)(part * 128 + c0), v);
+            tmem_ld_wait();
 #pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            uint32_t h[4];
+            for (int gq = 0; gq < 4; ++gq) {
+              uint32_t h[4];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * g + 2 * e]), __uint_as_float(v[8 * g + 2 * e + 1]));
-              h[e] = *reinterpret_cast<const uint32_t*>(&p2);
+              for (int e = 0; e < 4; ++e) {
+                const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * gq + 2 * e]), __uint_as_float(v[8 * gq + 2 * e + 1]));
+                h[e] = *reinterpret_cast<const uint32_t*>(&p2);
+              }
+              const int jg = t * 16 + (c0 >> 3) + gq;
+              if (jg < q_cap)
+                *reinterpret_cast<uint4*>(Q + ((((size_t)un.rb * q_cap + jg) * 2 + part) * 128 + pl) * 8) =
+                    make_uint4(h[0], h[1], h[2], h[3]);
             }
-            const int jg = t * 16 + (c0 >> 3) + g;
-            if (jg < G.q_groups_cap)
-              *reinterpret_cast<uint4*>(Q + ((((size_t)u.rb * G.q_groups_cap + jg) * 2 + part) * 128 + pl) * 8) =
-                  make_uint4(h[0], h[1], h[2], h[3]);
           }
-        }
-      fence_before();
-      mbar_arrive(smem_u32(&bars.acc_empty[buf]));
+        fence_before();
+        mbar_arrive(smem_u32(&bars.acc_empty[buf]));
+      }
     }
   }
   fence_before();
@@ -218,193 +309,247 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
 struct F0Args {
   const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups; const uint8_t* P;
   Peak* partials; Capture cap; long long k_a;
-  int n_lr, c, n_tiles, tiles_per_cta, tiles_cap, max_templates, n_stages, p_bytes;
+  int n_lr, c, r_bytes, tiles_cap, max_templates, n_stages, p_bytes;
+  SchedArgs sched;                                      // units = combos, one class
   UpRate up[kNLowRates];
   QItem item[kNLowRates][2][8];                         // per rate and variant: the active 16-row chunks, in order (kernel
   int32_t n_items[kNLowRates][2];                       // parameters: read with uniform loads); QItem.ch = chunk index
 };
 
+struct SegF0 {                                          // per-role copy of the current unit's operand sources
+  const uint8_t* Y[kMaxF0Slices];
+  const uint8_t* Rsrc[kMaxF0Slices];
+  int L[kMaxF0Slices];
+  const uint8_t* Q[kNLowRates];                         // this template block's rho^(d), or null
+};
+
+__device__ __forceinline__ void seg_f0_fill(SegF0& S, const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B, int lane)
+{
+  if (lane < B->n_f0) {
+    const SliceParams* P = a.sp + B->f0_slice[lane];
+    const int L = P->L_pad;
+    S.Y[lane] = reinterpret_cast<const uint8_t*>(P->Y);
+    S.Rsrc[lane] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)cb.rb * L * 512;
+    S.L[lane] = L;
+  }
+  if (lane >= 8 && lane < 8 + a.n_lr) {
+    const int r = lane - 8;
+    const RateGroup* G = a.groups + cb.bd * a.n_lr + r;
+    S.Q[r] = (G->n_slices > 0) ? reinterpret_cast<const uint8_t*>(G->Q) + (size_t)cb.rb * G->q_groups_cap * 4096 : nullptr;
+  }
+  __syncwarp();
+}
+
 __global__ void __launch_bounds__(RC16_THREADS, 1)
 f0_kernel(const __grid_constant__ F0Args a)
 {
-  const F0Combo cb = a.combos[blockIdx.y];
-  const BdPlan B = a.bd[cb.bd];
-  const int t0 = blockIdx.x * a.tiles_per_cta;
-  if (t0 >= a.n_tiles) return;
-  const int t1 = min(a.n_tiles, t0 + a.tiles_per_cta);
-
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) RingBars bars;
   __shared__ uint32_t tmem_slot;
-  __shared__ const uint8_t* sY[kMaxF0Slices];
-  __shared__ const uint8_t* sRsrc[kMaxF0Slices];
-  __shared__ int sL[kMaxF0Slices];
-  __shared__ const uint8_t* sQ[kNLowRates];             // this template block's rho^(d), or null
-  uint8_t* sR = smem;                                   // [l_sum / 8][2][128][8] fp16
-  uint8_t* sP = smem + (size_t)B.l_sum * 512;           // band matrices
-  uint8_t* ring = sP + a.p_bytes;
+  __shared__ SegF0 seg[2];                              // [0] producer's, [1] MMA issuer's
+  __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (tid == 0) sched_range(a.sched, s_rng);
+  __syncthreads();
+  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
+  if (u_lo == u_hi && t_lo == t_hi) return;
+  const int n_tiles = a.sched.n_tiles[0];
+
   const int n_stages = a.n_stages;
   ring_setup(bars, &tmem_slot, n_stages, warp, tid);
-  if (tid < B.n_f0) {
-    const SliceParams P = a.sp[B.f0_slice[tid]];
-    sY[tid] = reinterpret_cast<const uint8_t*>(P.Y);
-    sRsrc[tid] = reinterpret_cast<const uint8_t*>(P.R16) + (size_t)cb.rb * P.L_pad * 512;
-    sL[tid] = P.L_pad;
-  }
-  if (tid >= 64 && tid < 64 + a.n_lr) {
-    const int r = tid - 64;
-    const RateGroup G = a.groups[cb.bd * a.n_lr + r];
-    sQ[r] = (G.n_slices > 0) ? reinterpret_cast<const uint8_t*>(G.Q) + (size_t)cb.rb * G.q_groups_cap * 4096 : nullptr;
-  }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem = tmem_slot;
-  const int n_f0 = B.n_f0, n_lr = a.n_lr;
-  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]), ring_u = smem_u32(ring);
+  const int n_lr = a.n_lr;
+  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]);
+  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16
+  const uint32_t sP_u = sR_u + (uint32_t)a.r_bytes;     // band matrices
+  const uint32_t ring_u = sP_u + (uint32_t)a.p_bytes;
 
   if (warp == 0) {
     // ===== producer (warp-uniform; see tc05.cuh) =====
-    if (lane == 0) {
-      mbar_expect_tx(smem_u32(&bars.consts), (uint32_t)B.l_sum * 512u + (uint32_t)a.p_bytes);
-      uint32_t off = 0;
-      for (int i = 0; i < n_f0; ++i) {
-        copy_pieces(smem_u32(sR) + off, sRsrc[i], (uint32_t)sL[i] * 512u, smem_u32(&bars.consts));
-        off += (uint32_t)sL[i] * 512u;
-      }
-      copy_pieces(smem_u32(sP), a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
-    }
-    __syncwarp();
-    const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
     const uint32_t lead = elect_u32();
     Ring rg{0, 0u, n_stages};
-    for (int t = t0_u; t < t1_u; ++t) {
-      for (int i = 0; i < nf_u; ++i) {
-        const int L = bcast(sL[i]);
-        const uint8_t* src = bcast(sY[i]) + (size_t)t * L * 256;
-        for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) produce(lead, rg, bfull, bempty, ring_u, src);
+    int g = 0, seg_i = 0;
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
+      if (t0 >= t1) continue;
+      const F0Combo cb = a.combos[u];
+      const BdPlan* B = a.bd + cb.bd;
+      seg_f0_fill(seg[0], a, cb, B, lane);
+      const int nf_u = bcast(B->n_f0);
+      const uint32_t rbytes_u = (uint32_t)bcast(B->l_sum) * 512u;
+      int countdown = (seg_i == 0) ? 0 : n_stages;
+      bool r_done = false;
+      auto load_R = [&]() {
+        if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
+        if (lane == 0) {
+          mbar_expect_tx(smem_u32(&bars.consts), rbytes_u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
+          uint32_t off = 0;
+          for (int i = 0; i < nf_u; ++i) {
+            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, smem_u32(&bars.consts));
+            off += (uint32_t)seg[0].L[i] * 512u;
+          }
+          if (seg_i == 0) copy_pieces(sP_u, a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
+        }
+        __syncwarp();
+        r_done = true;
+      };
+      if (countdown == 0) load_R();
+      for (int t = t0; t < t1; ++t) {
+        for (int i = 0; i < nf_u; ++i) {
+          const int L = bcast(seg[0].L[i]);
+          const uint8_t* src = bcast(seg[0].Y[i]) + (size_t)t * L * 256;
+          for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
+            produce(lead, rg, bfull, bempty, ring_u, src);
+            if (!r_done && --countdown == 0) load_R();
+          }
+        }
+        for (int r = 0; r < n_lr; ++r) {
+          const uint8_t* qb = bcast(seg[0].Q[r]);
+          if (qb == nullptr) continue;
+          const int m0 = (t * 128) >> a.up[r].log2d, ws = m0 & ~7;
+          const int var = (m0 != ws && a.up[r].n_var > 1) ? 1 : 0;
+          const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
+          const int n_it = a.n_items[r][var];
+          for (int i = 0; i < n_it; ++i) {
+            produce(lead, rg, bfull, bempty, ring_u, src + (size_t)a.item[r][var][i].ch * RC16_STAGE);
+            if (!r_done && --countdown == 0) load_R();
+          }
+        }
       }
-      for (int r = 0; r < n_lr; ++r) {
-        const uint8_t* qb = bcast(sQ[r]);
-        if (qb == nullptr) continue;
-        const int m0 = (t * 128) >> a.up[r].log2d, ws = m0 & ~7;
-        const int var = (m0 != ws && a.up[r].n_var > 1) ? 1 : 0;
-        const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
-        const int n_it = a.n_items[r][var];
-        for (int i = 0; i < n_it; ++i)
-          produce(lead, rg, bfull, bempty, ring_u, src + (size_t)a.item[r][var][i].ch * RC16_STAGE);
-      }
+      if (!r_done) load_R();
+      g += t1 - t0; ++seg_i;
     }
   } else if (warp == 1) {
     // ===== MMA issuer (warp-uniform) =====
-    mbar_wait(smem_u32(&bars.consts), 0);
-    fence_after();
     const uint32_t idesc128 = idesc_f16(128, 128);
-    const uint32_t a_base = desc_lo(smem_u32(sR), 4096u), b_base = desc_lo(ring_u, 2048u);
-    const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(smem_u32(sP), 2048u);
-    const int nf_u = bcast(n_f0), t0_u = bcast(t0), t1_u = bcast(t1);
+    const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
+    const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(sP_u, 2048u);
     const uint32_t lead = elect_u32();
     const uint32_t tm = bcast(tmem);
-    uint32_t have_q = 0u;
-    for (int r = 0; r < n_lr; ++r) have_q |= (bcast(sQ[r]) != nullptr ? 1u : 0u) << r;
     Ring rg{0, 0u, n_stages};
     uint32_t eph = 3u;
-    for (int t = t0_u, buf = 0; t < t1_u; ++t, buf ^= 1) {
-      mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+    int buf = 0, seg_i = 0;
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
+      if (t0 >= t1) continue;
+      const F0Combo cb = a.combos[u];
+      const BdPlan* B = a.bd + cb.bd;
+      seg_f0_fill(seg[1], a, cb, B, lane);
+      const int nf_u = bcast(B->n_f0);
+      uint32_t have_q = 0u;
+      for (int r = 0; r < n_lr; ++r) have_q |= (bcast(seg[1].Q[r]) != nullptr ? 1u : 0u) << r;
+      mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
       fence_after();
-      const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
-      uint32_t first = 1u, a_lo = a_base;
-      for (int i = 0; i < nf_u; ++i) {
-        const int n_kc = bcast(sL[i]) >> 5;
-        for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-          mbar_wait(bfull + 8u * rg.s, rg.ph);
-          fence_after();
-          mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-          commit_e(lead, bempty + 8u * rg.s);
-          first = 0u;
-          rg.advance();
+      for (int t = t0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+        fence_after();
+        const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
+        uint32_t first = 1u, a_lo = a_base;
+        for (int i = 0; i < nf_u; ++i) {
+          const int n_kc = bcast(seg[1].L[i]) >> 5;
+          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
+            fence_after();
+            mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
+            commit_e(lead, bempty + 8u * rg.s);
+            first = 0u;
+            rg.advance();
+          }
         }
-      }
-      for (int r = 0; r < n_lr; ++r) {
-        if (!((have_q >> r) & 1u)) continue;
-        const int m0 = (t * 128) >> a.up[r].log2d;
-        const int var = ((m0 & 7) && a.up[r].n_var > 1) ? 1 : 0;
-        const int n_it = a.n_items[r][var];
-        for (int i = 0; i < n_it; ++i) {
-          const QItem it = a.item[r][var][i];
-          mbar_wait(bfull + 8u * rg.s, rg.ph);
-          fence_after();
-          const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
-          const uint64_t bdesc = desc64(p_base + it.b_off);
-          mma_ss_e(lead, d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
-          mma_ss_e(lead, d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
-          commit_e(lead, bempty + 8u * rg.s);
-          rg.advance();
+        for (int r = 0; r < n_lr; ++r) {
+          if (!((have_q >> r) & 1u)) continue;
+          const int m0 = (t * 128) >> a.up[r].log2d;
+          const int var = ((m0 & 7) && a.up[r].n_var > 1) ? 1 : 0;
+          const int n_it = a.n_items[r][var];
+          for (int i = 0; i < n_it; ++i) {
+            const QItem it = a.item[r][var][i];
+            mbar_wait(bfull + 8u * rg.s, rg.ph);
+            fence_after();
+            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+            const uint64_t bdesc = desc64(p_base + it.b_off);
+            mma_ss_e(lead, d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
+            mma_ss_e(lead, d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
+            commit_e(lead, bempty + 8u * rg.s);
+            rg.advance();
+          }
         }
+        commit_e(lead, smem_u32(&bars.acc_full[buf]));
       }
-      commit_e(lead, smem_u32(&bars.acc_full[buf]));
+      ++seg_i;
     }
   } else {
     // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
     const int q = warp & 3;
     const int pl = q * 32 + lane;
-    const int p = cb.rb * kTplBlock + pl;
-    const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && 2 * p + 1 < a.cap.rows;
     uint32_t fph = 0u;
-    for (int t = t0, buf = 0; t < t1; ++t, buf ^= 1) {
-      mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
-      fence_after();
-      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
-      const int kap0 = t * 128;
-      const int valid = min(128, a.c - kap0);
-      // four interleaved running maxima (columns j = m mod 4) break the serial compare/select chain; merged below
-      // with "larger q, then lower k" so that the first maximum of the tile still wins (R8)
-      float bq[4] = {-1.f, -1.f, -1.f, -1.f}, bre4[4] = {0.f, 0.f, 0.f, 0.f}, bim4[4] = {0.f, 0.f, 0.f, 0.f};
-      int bk4[4] = {0, 0, 0, 0};
-#pragma unroll 1
-      for (int c0 = 0; c0 < 128; c0 += 32) {
-        uint32_t re[32], im[32];
-        tmem_ld32(taddr + (uint32_t)c0, re);
-        tmem_ld32(taddr + (uint32_t)(128 + c0), im);
-        tmem_ld_wait();
-        if (c0 + 32 <= valid) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-            const float qq = fmaf(x, x, y * y);
-            if (qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
+    int buf = 0;
+    for (int u = u_lo; u <= u_hi; ++u) {
+      if (u == u_hi && t_hi == 0) break;
+      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
+      if (t0 >= t1) continue;
+      const F0Combo cb = a.combos[u];
+      const int n_templates = a.bd[cb.bd].n_templates;
+      const int p = cb.rb * kTplBlock + pl;
+      const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && 2 * p + 1 < a.cap.rows;
+      for (int t = t0; t < t1; ++t, buf ^= 1) {
+        mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
+        fence_after();
+        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
+        const int kap0 = t * 128;
+        const int valid = min(128, a.c - kap0);
+        // four interleaved running maxima (columns j = m mod 4) break the serial compare/select chain; merged below
+        // with "larger q, then lower k" so that the first maximum of the tile still wins (R8)
+        float bq[4] = {-1.f, -1.f, -1.f, -1.f}, bre4[4] = {0.f, 0.f, 0.f, 0.f}, bim4[4] = {0.f, 0.f, 0.f, 0.f};
+        int bk4[4] = {0, 0, 0, 0};
+  #pragma unroll 1
+        for (int c0 = 0; c0 < 128; c0 += 32) {
+          uint32_t re[32], im[32];
+          tmem_ld32(taddr + (uint32_t)c0, re);
+          tmem_ld32(taddr + (uint32_t)(128 + c0), im);
+          tmem_ld_wait();
+          if (c0 + 32 <= valid) {
+  #pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+              const float qq = fmaf(x, x, y * y);
+              if (qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
+            }
+          } else {
+  #pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
+              const float qq = fmaf(x, x, y * y);
+              if (c0 + j < valid && qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
+            }
           }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-            const float qq = fmaf(x, x, y * y);
-            if (c0 + j < valid && qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
-          }
-        }
-        if (capture) {
-#pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const long long k = a.k_a + kap0 + c0 + j;
-            if (c0 + j < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
-              a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(re[j]);
-              a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(im[j]);
+          if (capture) {
+  #pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const long long k = a.k_a + kap0 + c0 + j;
+              if (c0 + j < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
+                a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(re[j]);
+                a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(im[j]);
+              }
             }
           }
         }
-      }
-      float best = bq[0], bre = bre4[0], bim = bim4[0];
-      int bk = bk4[0];
-#pragma unroll
-      for (int m = 1; m < 4; ++m)
-        if (bq[m] > best || (bq[m] == best && bk4[m] < bk)) { best = bq[m]; bk = bk4[m]; bre = bre4[m]; bim = bim4[m]; }
-      fence_before();
-      mbar_arrive(smem_u32(&bars.acc_empty[buf]));
-      if (p < B.n_templates) {
-        Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
-        a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+        float best = bq[0], bre = bre4[0], bim = bim4[0];
+        int bk = bk4[0];
+  #pragma unroll
+        for (int m = 1; m < 4; ++m)
+          if (bq[m] > best || (bq[m] == best && bk4[m] < bk)) { best = bq[m]; bk = bk4[m]; bre = bre4[m]; bim = bim4[m]; }
+        fence_before();
+        mbar_arrive(smem_u32(&bars.acc_empty[buf]));
+        if (p < n_templates) {
+          Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
+          a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+        }
       }
     }
   }
@@ -532,18 +677,36 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   pl->low_smem = low_fixed + pl->low_stages * RC16_STAGE;
 
   // device tables
-  std::vector<LowUnit> units;
-  for (int r = 0; r < pl->n_lr; ++r) pl->units_per_rate[r] = 0;
-  for (int b = 0; b < n_bd; ++b)
-    for (int r = 0; r < pl->n_lr; ++r) {
+  std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
+  std::vector<SchedUnit> low_sched;
+  for (int r = 0; r < pl->n_lr; ++r) {
+    pl->units_per_rate[r] = 0; pl->low_wsum[r] = 0;
+    for (int b = 0; b < n_bd; ++b) {
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
       if (G.n_slices == 0) continue;
       void* q = nullptr;
       if (!plan_alloc(pl, &q, (size_t)G.n_rb * G.q_groups_cap * 4096, true, bytes, err, errlen)) return false;
       G.Q = (__half*)q;
-      for (int rb = 0; rb < G.n_rb; ++rb) units.push_back(LowUnit{b * pl->n_lr + r, rb});
+      for (int rb = 0; rb < G.n_rb; ++rb) {
+        units.push_back(LowUnit{b * pl->n_lr + r, rb});
+        low_sched.push_back(SchedUnit{G.l_sum / 32, (int32_t)pl->low_wsum[r]});
+        pl->low_wsum[r] += G.l_sum / 32;
+      }
       pl->units_per_rate[r] += G.n_rb;
     }
+  }
+  // f0 units = combos; cost per tile = ring stages: y chunks of the d == 1 slices + interpolation chunks
+  std::vector<SchedUnit> f0_sched;
+  pl->f0_wsum = 0;
+  for (const F0Combo& cb : pl->combos_host) {
+    int w = pl->bd_host[cb.bd].l_sum / 32;
+    for (int r = 0; r < pl->n_lr; ++r) {
+      if (pl->groups_host[(size_t)cb.bd * pl->n_lr + r].n_slices == 0) continue;
+      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch) w += pl->up[r].nn[0][ch] ? 1 : 0;
+    }
+    f0_sched.push_back(SchedUnit{w, (int32_t)pl->f0_wsum});
+    pl->f0_wsum += w;
+  }
   pl->low_units = (int)units.size();
   auto upload = [&](void** dst, const void* src, size_t n) -> bool {
     if (!plan_alloc(pl, dst, n, false, bytes, err, errlen)) return false;
@@ -555,6 +718,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   if (!upload((void**)&pl->combos_dev, pl->combos_host.data(), pl->combos_host.size() * sizeof(F0Combo))) return false;
   if (!upload((void**)&pl->units_dev, units.data(), units.size() * sizeof(LowUnit))) return false;
   if (!upload((void**)&pl->p_dev, pblob.data(), pblob.size() * sizeof(__half))) return false;
+  if (!upload((void**)&pl->low_sched_dev, low_sched.data(), low_sched.size() * sizeof(SchedUnit))) return false;
+  if (!upload((void**)&pl->f0_sched_dev, f0_sched.data(), f0_sched.size() * sizeof(SchedUnit))) return false;
 
   cudaError_t e = cudaFuncSetAttribute(f0_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->f0_smem);
   if (e == cudaSuccess && pl->n_lr > 0)
@@ -569,18 +734,20 @@ bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
 int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
 {
-  const int target = 2 * pl->n_sm;
   if (pl->low_units > 0) {
-    long long total = 0; int max_tiles = 1;
+    SchedArgs sc;
+    memset(&sc, 0, sizeof sc);
+    sc.units = pl->low_sched_dev; sc.n_cls = pl->n_lr;
+    long long tiles_total = 0;
     for (int r = 0; r < pl->n_lr; ++r) {
-      const int tiles = (((c >> pl->up[r].log2d) + 2 * kKUp) + 127) / 128;
-      total += (long long)tiles * pl->units_per_rate[r];
-      max_tiles = std::max(max_tiles, tiles);
+      sc.cls_begin[r + 1] = sc.cls_begin[r] + pl->units_per_rate[r];
+      sc.n_tiles[r] = (((c >> pl->up[r].log2d) + 2 * kKUp) + 127) / 128;
+      sc.cls_base[r + 1] = sc.cls_base[r] + pl->low_wsum[r] * sc.n_tiles[r];
+      tiles_total += (long long)sc.n_tiles[r] * pl->units_per_rate[r];
     }
-    const int tpc = (int)std::max<long long>(1, (total + target - 1) / target);
-    dim3 grid((max_tiles + tpc - 1) / tpc, pl->low_units);
+    const int grid = (int)std::min<long long>(pl->n_sm, tiles_total);
     lowrate_recon_kernel<<<grid, RC16_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
-                                                                  c, tpc, pl->low_stages);
+                                                                  sc, pl->l_sum_low_max * 512, pl->low_stages);
     ++*launches;
   }
   F0Args a;
@@ -588,11 +755,15 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;
   a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
   a.partials = partials; a.cap = cap; a.k_a = k_a;
-  a.n_lr = pl->n_lr; a.c = c; a.n_tiles = (c + 127) / 128;
+  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 512;
   const int n_combos = (int)pl->combos_host.size();
-  int ranges = (target + n_combos - 1) / n_combos;
-  ranges = std::max(1, std::min(ranges, a.n_tiles));
-  a.tiles_per_cta = (a.n_tiles + ranges - 1) / ranges;
+  const int n_tiles = (c + 127) / 128;
+  a.sched.units = pl->f0_sched_dev; a.sched.n_cls = 1;
+  a.sched.cls_begin[1] = n_combos; a.sched.n_tiles[0] = n_tiles;
+  a.sched.cls_base[1] = pl->f0_wsum * n_tiles;
+  // one CTA per SM; when the units fit, a whole number of CTAs per unit so that no CTA has to swap R mid-way
+  int grid = (n_combos <= pl->n_sm) ? n_combos * (pl->n_sm / n_combos) : pl->n_sm;
+  grid = (int)std::min<long long>(grid, (long long)n_combos * n_tiles);
   a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.n_stages = pl->f0_stages; a.p_bytes = pl->p_bytes;
   for (int r = 0; r < kNLowRates; ++r) a.up[r] = pl->up[r];
   for (int r = 0; r < pl->n_lr; ++r)
@@ -606,7 +777,6 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
         it.d_off = (uint32_t)U.n0[v][ch] * 8u;
         it.ch = (uint32_t)ch;
       }
-  dim3 grid((a.n_tiles + a.tiles_per_cta - 1) / a.tiles_per_cta, n_combos);
   f0_kernel<<<grid, RC16_THREADS, pl->f0_smem, st>>>(a);
   ++*launches;
   return cudaGetLastError() == cudaSuccess ? 0 : 1;

@@ -124,7 +124,21 @@ struct UpRate {                    // one per distinct rate with d > 1 (bank-wid
   uint8_t n0[2][8], nn[2][8];      // per variant and 16-row chunk: first output column / 8 and columns / 8 (0: skip)
 };
 
-struct QItem { uint32_t idesc, b_off, d_off, ch; };   // one 16-row chunk of an interpolation: MMA N, P offset, D column
+struct QItem { uint32_t idesc, b_off, d_off, ch; };
+
+// Static schedule of a persistent tensor kernel (A7).  Work = units x time tiles; a unit is one stationary
+// operand set (f0 kernel: one (bin, detector, template block); low-rate kernel: the same per rate).  Units are
+// stored class-major (class = rate: every unit of a class has the same number of time tiles in a chunk) with a
+// cost w per tile (ring stages).  CTA i of G takes the cost range [T i / G, T (i + 1) / G) of the flattened
+// (class, unit, tile) sequence, so every SM gets the same tensor work whatever the bank geometry.
+struct SchedUnit { int32_t w, wprefix; };   // wprefix: sum of w over the earlier units of the same class
+struct SchedArgs {
+  const SchedUnit* units;
+  int32_t   n_cls;
+  int32_t   cls_begin[kNLowRates + 1];      // unit index range of class c: [cls_begin[c], cls_begin[c + 1])
+  int32_t   n_tiles[kNLowRates];            // time tiles per unit of class c for this chunk
+  long long cls_base[kNLowRates + 1];       // cost before class c; cls_base[n_cls] = total
+};   // one 16-row chunk of an interpolation: MMA N, P offset, D column
 
 struct F16Plan;                    // opaque host-side plan: work lists, band matrices, Q buffers
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,
