@@ -118,7 +118,7 @@ def oracle_sample(w, seconds: float):
     b = w.bins[0]
     W = w.peak_window
     k0 = ((b.template_len + W - 1) // W + 1) * W
-    k1 = min(w.n_samples, k0 + int(round(seconds * w.f0)) // W * W)
+    k1 = min(w.n_samples, k0 + max(1, int(round(seconds * w.f0)) // W) * W)
     x = w.strain[0].astype(np.float64)
     t0 = time.perf_counter()
     rho = oc.snr_series(x, b.slices, b.basis, b.recon, k0, k1, w.k_down, w.k_up)
@@ -246,7 +246,8 @@ def run_ours(args):
         ach = dom[1] / (dom[2] * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom[0], "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
                     "traffic": None, "peak_source": "derived: 148 SM x 128 FFMA/clk x 2 x 1.965 GHz"}
-    roofline["stage_ms"] = {"resample": stage[0], "fir": stage[1], "recon_epilogue": stage[2], "merge_compact": stage[3], "total": stage[4]}
+    roofline["stage_ms"] = {"resample": stage[0], "fir": stage[1], "recon_epilogue": stage[2], "merge_compact": stage[3], "total": stage[4],
+                            "recon_lowrate_part": stage[5]}
 
     # ---- end to end: pinned host strain in, triggers out ---------------------------------------
     strain_pin = torch.from_numpy(w.strain).pin_memory()

@@ -169,11 +169,12 @@ int64_t lloid_last_launch_count(const lloid_bank_t *bank);
 int64_t lloid_device_bytes(const lloid_bank_t *bank);
 
 /* Time (ms, CUDA events on the call's stream) spent by the last lloid_filter call in each stage:
- * out_ms[0..4] = resample, basis FIR, reconstruction+epilogue, peak merge/compaction, whole call.
+ * out_ms[0..5] = resample, basis FIR, reconstruction+epilogue (both kernels of the fp16 path), peak
+ * merge/compaction, whole call, and the low-rate reconstruction kernel's share of [2] (fp16 path; else 0).
  * Only recorded when enabled with lloid_set_profiling(bank, 1) (which makes lloid_filter record
  * events; reading them synchronises on the last event).  Used by bench.py for the roofline leg. */
 int lloid_set_profiling(lloid_bank_t *bank, int32_t enable);
-int lloid_last_stage_ms(lloid_bank_t *bank, float *out_ms /* host, float[5] */);
+int lloid_last_stage_ms(lloid_bank_t *bank, float *out_ms /* host, float[6] */);
 
 void lloid_destroy(lloid_bank_t *bank);
 const char *lloid_last_error(void);

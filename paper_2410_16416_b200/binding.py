@@ -191,7 +191,7 @@ def lloid_set_profiling(bank, enable: bool) -> None:
 
 
 def lloid_last_stage_ms(bank) -> np.ndarray:
-    out = (C.c_float * 5)()
+    out = (C.c_float * 6)()
     _check(lib().lloid_last_stage_ms(bank, out))
     return np.array(list(out), dtype=np.float64)
 

@@ -106,24 +106,28 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
   }
 }
 
-// producer (whole warp, converged): wait for the slot to be free, then the elected lane issues one 8 KB bulk copy
-__device__ __forceinline__ void produce(uint32_t lead, Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base,
-                                        const uint8_t* src)
+// The producer and the MMA issuer each run as ONE elected thread inside `if (elect_one())`: ptxas recognises the
+// elect.sync-guarded region as single-threaded and keeps the whole loop (ring state, descriptors, barrier
+// addresses) in uniform registers -- about 25 SASS instructions per 4-MMA stage, no R2UR at all.  (A per-lane
+// predicate on the issuing instruction instead costs an ELECT + R2UR.BROADCAST waterfall per MMA: measured
+// ~450 issue cycles per stage, which bounded both kernels.)
+// producer: wait for the slot to be free, then one 8 KB bulk copy
+__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src)
 {
   mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
-  mbar_expect_tx_e(lead, bars_full + 8u * rg.s, RC16_STAGE);
-  bulk_g2s_e(lead, ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
+  mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
+  bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
   rg.advance();
 }
 
 // one K = 32 chunk of a reconstruction: D[part] (+)= R[l-groups g .. g + 3][part] * stage^T, N = 128.
 // a_lo: descriptor of (group g, part 0) with LBO 4096; b_lo: descriptor of the stage with LBO 2048 (16-byte units)
-__device__ __forceinline__ void mma_recon_chunk(uint32_t lead, uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
+__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
 {
-  mma_ss_e(lead, d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss_e(lead, d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
-  mma_ss_e(lead, d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss_e(lead, d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
+  mma_ss(d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss(d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
+  mma_ss(d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
+  mma_ss(d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -133,16 +137,15 @@ struct SegLow {                             // per-role copy of the current unit
   int L[kMaxGroupSlices];
 };
 
-__device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __restrict__ sp, const RateGroup& G, int rb, int lane)
+__device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __restrict__ sp, const RateGroup* __restrict__ G, int rb)
 {
-  if (lane < G.n_slices) {
-    const SliceParams* P = sp + G.slice[lane];
+  for (int i = 0; i < G->n_slices; ++i) {               // one thread
+    const SliceParams* P = sp + G->slice[i];
     const int L = P->L_pad;
-    S.Y[lane] = reinterpret_cast<const uint8_t*>(P->Y);
-    S.Rsrc[lane] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 512;
-    S.L[lane] = L;
+    S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
+    S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 512;
+    S.L[i] = L;
   }
-  __syncwarp();
 }
 
 // Persistent: CTA i of gridDim.x runs cost range i of the (rate, unit, tile) sequence (SchedArgs).  At a unit
@@ -174,8 +177,8 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   const uint32_t ring_u = sR_u + (uint32_t)r_bytes;
 
   if (warp == 0) {
-    // ===== producer (warp-uniform; see tc05.cuh) =====
-    const uint32_t lead = elect_u32();
+    // ===== producer: one elected thread =====
+    if (elect_one()) {
     Ring rg{0, 0u, n_stages};
     int g = 0, seg_i = 0;                               // tiles / segments done so far by this CTA
     for (int u = u_lo; u <= u_hi; ++u) {
@@ -184,15 +187,15 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
       if (t0 >= t1) continue;
       const LowUnit un = units[u];
-      const RateGroup G = groups[un.group];
-      seg_low_fill(seg[0], sp, G, un.rb, lane);
-      const int ns_u = bcast(G.n_slices);
-      const uint32_t rbytes_u = (uint32_t)bcast(G.l_sum) * 512u;
+      const RateGroup* G = groups + un.group;
+      seg_low_fill(seg[0], sp, G, un.rb);
+      const int ns_u = G->n_slices;
+      const uint32_t rbytes_u = (uint32_t)G->l_sum * 512u;
       int countdown = (seg_i == 0) ? 0 : n_stages;      // ring stages to push before R is replaced
       bool r_done = false;
       auto load_R = [&]() {
         if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
-        if (lane == 0) {
+        {
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
           uint32_t off = 0;
           for (int i = 0; i < ns_u; ++i) {
@@ -200,28 +203,28 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
             off += (uint32_t)seg[0].L[i] * 512u;
           }
         }
-        __syncwarp();
         r_done = true;
       };
       if (countdown == 0) load_R();
       for (int t = t0; t < t1; ++t)
         for (int i = 0; i < ns_u; ++i) {
-          const int L = bcast(seg[0].L[i]);
-          const uint8_t* src = bcast(seg[0].Y[i]) + (size_t)t * L * 256;          // tiles are contiguous in Y16
+          const int L = seg[0].L[i];
+          const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;          // tiles are contiguous in Y16
           for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-            produce(lead, rg, bfull, bempty, ring_u, src);
+            produce(rg, bfull, bempty, ring_u, src);
             if (!r_done && --countdown == 0) load_R();
           }
         }
       if (!r_done) load_R();
       g += t1 - t0; ++seg_i;
     }
+    }
   } else if (warp == 1) {
-    // ===== MMA issuer (warp-uniform) =====
+    // ===== MMA issuer: one elected thread =====
+    if (elect_one()) {
     const uint32_t idesc = idesc_f16(128, 128);
     const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
-    const uint32_t lead = elect_u32();
-    const uint32_t tm = bcast(tmem);
+    const uint32_t tm = tmem;
     Ring rg{0, 0u, n_stages};
     uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
     int buf = 0, seg_i = 0;
@@ -231,9 +234,9 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
       if (t0 >= t1) continue;
       const LowUnit un = units[u];
-      const RateGroup G = groups[un.group];
-      seg_low_fill(seg[1], sp, G, un.rb, lane);
-      const int ns_u = bcast(G.n_slices);
+      const RateGroup* G = groups + un.group;
+      seg_low_fill(seg[1], sp, G, un.rb);
+      const int ns_u = G->n_slices;
       mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
       fence_after();
       for (int t = t0; t < t1; ++t, buf ^= 1) {
@@ -242,19 +245,20 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
         uint32_t first = 1u, a_lo = a_base;
         for (int i = 0; i < ns_u; ++i) {
-          const int n_kc = bcast(seg[1].L[i]) >> 5;
+          const int n_kc = seg[1].L[i] >> 5;
           for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
             mbar_wait(bfull + 8u * rg.s, rg.ph);
             fence_after();
-            mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
-            commit_e(lead, bempty + 8u * rg.s);
+            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
+            commit(bempty + 8u * rg.s);
             first = 0u;
             rg.advance();
           }
         }
-        commit_e(lead, smem_u32(&bars.acc_full[buf]));
+        commit(smem_u32(&bars.acc_full[buf]));
       }
       ++seg_i;
+    }
     }
   } else {
     const int q = warp & 3;
@@ -323,22 +327,27 @@ struct SegF0 {                                          // per-role copy of the 
   const uint8_t* Q[kNLowRates];                         // this template block's rho^(d), or null
 };
 
-__device__ __forceinline__ void seg_f0_fill(SegF0& S, const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B, int lane)
+__device__ __forceinline__ void seg_f0_fill(SegF0& S, const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B)
 {
-  if (lane < B->n_f0) {
-    const SliceParams* P = a.sp + B->f0_slice[lane];
+  for (int i = 0; i < B->n_f0; ++i) {                   // one thread
+    const SliceParams* P = a.sp + B->f0_slice[i];
     const int L = P->L_pad;
-    S.Y[lane] = reinterpret_cast<const uint8_t*>(P->Y);
-    S.Rsrc[lane] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)cb.rb * L * 512;
-    S.L[lane] = L;
+    S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
+    S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)cb.rb * L * 512;
+    S.L[i] = L;
   }
-  if (lane >= 8 && lane < 8 + a.n_lr) {
-    const int r = lane - 8;
+  for (int r = 0; r < a.n_lr; ++r) {
     const RateGroup* G = a.groups + cb.bd * a.n_lr + r;
     S.Q[r] = (G->n_slices > 0) ? reinterpret_cast<const uint8_t*>(G->Q) + (size_t)cb.rb * G->q_groups_cap * 4096 : nullptr;
   }
-  __syncwarp();
 }
+
+// Per-unit tables of the interpolation work of one tile, so that the per-chunk code of both single-thread loops
+// is a table read plus the issuing instructions.  v = t & 1 selects the band-matrix variant of the rates whose
+// window start alternates (d = 32); the chunks of a (rate, variant) are consecutive.
+struct ItTab { uint32_t idesc, b_lo, d_off, pad; };                                  // MMA issuer: one per chunk
+struct PrTab { const uint8_t* q; int32_t log2d, ch0[2], n[2]; int32_t pad; };           // producer: one per rate present
+constexpr int kMaxTileItems = kNLowRates * 8;
 
 __global__ void __launch_bounds__(RC16_THREADS, 1)
 f0_kernel(const __grid_constant__ F0Args a)
@@ -347,6 +356,8 @@ f0_kernel(const __grid_constant__ F0Args a)
   __shared__ __align__(8) RingBars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ SegF0 seg[2];                              // [0] producer's, [1] MMA issuer's
+  __shared__ __align__(16) ItTab s_it[2][kMaxTileItems];
+  __shared__ PrTab s_pr[kNLowRates];
   __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -369,8 +380,8 @@ f0_kernel(const __grid_constant__ F0Args a)
   const uint32_t ring_u = sP_u + (uint32_t)a.p_bytes;
 
   if (warp == 0) {
-    // ===== producer (warp-uniform; see tc05.cuh) =====
-    const uint32_t lead = elect_u32();
+    // ===== producer: one elected thread =====
+    if (elect_one()) {
     Ring rg{0, 0u, n_stages};
     int g = 0, seg_i = 0;
     for (int u = u_lo; u <= u_hi; ++u) {
@@ -379,14 +390,26 @@ f0_kernel(const __grid_constant__ F0Args a)
       if (t0 >= t1) continue;
       const F0Combo cb = a.combos[u];
       const BdPlan* B = a.bd + cb.bd;
-      seg_f0_fill(seg[0], a, cb, B, lane);
-      const int nf_u = bcast(B->n_f0);
-      const uint32_t rbytes_u = (uint32_t)bcast(B->l_sum) * 512u;
+      seg_f0_fill(seg[0], a, cb, B);
+      const int nf_u = B->n_f0;
+      const uint32_t rbytes_u = (uint32_t)B->l_sum * 512u;
+      int npr = 0;
+      for (int r = 0; r < n_lr; ++r) {
+        if (seg[0].Q[r] == nullptr) continue;
+        PrTab e;
+        e.q = seg[0].Q[r]; e.log2d = a.up[r].log2d; e.pad = 0;
+        for (int v = 0; v < 2; ++v) {
+          const int vv = a.up[r].n_var > 1 ? v : 0;
+          e.n[v] = a.n_items[r][vv];
+          e.ch0[v] = e.n[v] > 0 ? (int)a.item[r][vv][0].ch : 0;
+        }
+        s_pr[npr++] = e;
+      }
       int countdown = (seg_i == 0) ? 0 : n_stages;
       bool r_done = false;
       auto load_R = [&]() {
         if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
-        if (lane == 0) {
+        {
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
           uint32_t off = 0;
           for (int i = 0; i < nf_u; ++i) {
@@ -395,28 +418,26 @@ f0_kernel(const __grid_constant__ F0Args a)
           }
           if (seg_i == 0) copy_pieces(sP_u, a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
         }
-        __syncwarp();
         r_done = true;
       };
       if (countdown == 0) load_R();
       for (int t = t0; t < t1; ++t) {
         for (int i = 0; i < nf_u; ++i) {
-          const int L = bcast(seg[0].L[i]);
-          const uint8_t* src = bcast(seg[0].Y[i]) + (size_t)t * L * 256;
+          const int L = seg[0].L[i];
+          const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;
           for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-            produce(lead, rg, bfull, bempty, ring_u, src);
+            produce(rg, bfull, bempty, ring_u, src);
             if (!r_done && --countdown == 0) load_R();
           }
         }
-        for (int r = 0; r < n_lr; ++r) {
-          const uint8_t* qb = bcast(seg[0].Q[r]);
-          if (qb == nullptr) continue;
-          const int m0 = (t * 128) >> a.up[r].log2d, ws = m0 & ~7;
-          const int var = (m0 != ws && a.up[r].n_var > 1) ? 1 : 0;
-          const uint8_t* src = qb + (size_t)(ws >> 3) * 4096;
-          const int n_it = a.n_items[r][var];
-          for (int i = 0; i < n_it; ++i) {
-            produce(lead, rg, bfull, bempty, ring_u, src + (size_t)a.item[r][var][i].ch * RC16_STAGE);
+        const int v = t & 1;
+        for (int j = 0; j < npr; ++j) {
+          const PrTab* e = &s_pr[j];
+          const int ws = ((t * 128) >> e->log2d) & ~7;
+          const uint8_t* src = e->q + (size_t)(ws >> 3) * 4096 + (size_t)e->ch0[v] * RC16_STAGE;
+          const int n_it = e->n[v];
+          for (int i = 0; i < n_it; ++i, src += RC16_STAGE) {
+            produce(rg, bfull, bempty, ring_u, src);
             if (!r_done && --countdown == 0) load_R();
           }
         }
@@ -424,13 +445,14 @@ f0_kernel(const __grid_constant__ F0Args a)
       if (!r_done) load_R();
       g += t1 - t0; ++seg_i;
     }
+    }
   } else if (warp == 1) {
-    // ===== MMA issuer (warp-uniform) =====
+    // ===== MMA issuer: one elected thread =====
+    if (elect_one()) {
     const uint32_t idesc128 = idesc_f16(128, 128);
     const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
     const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(sP_u, 2048u);
-    const uint32_t lead = elect_u32();
-    const uint32_t tm = bcast(tmem);
+    const uint32_t tm = tmem;
     Ring rg{0, 0u, n_stages};
     uint32_t eph = 3u;
     int buf = 0, seg_i = 0;
@@ -440,10 +462,19 @@ f0_kernel(const __grid_constant__ F0Args a)
       if (t0 >= t1) continue;
       const F0Combo cb = a.combos[u];
       const BdPlan* B = a.bd + cb.bd;
-      seg_f0_fill(seg[1], a, cb, B, lane);
-      const int nf_u = bcast(B->n_f0);
-      uint32_t have_q = 0u;
-      for (int r = 0; r < n_lr; ++r) have_q |= (bcast(seg[1].Q[r]) != nullptr ? 1u : 0u) << r;
+      seg_f0_fill(seg[1], a, cb, B);
+      const int nf_u = B->n_f0;
+      int nit[2] = {0, 0};
+      for (int v = 0; v < 2; ++v)
+        for (int r = 0; r < n_lr; ++r) {
+          if (seg[1].Q[r] == nullptr) continue;
+          const int vv = a.up[r].n_var > 1 ? v : 0;
+          for (int i = 0; i < a.n_items[r][vv]; ++i) {
+            const QItem it = a.item[r][vv][i];
+            ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.d_off = it.d_off; e.pad = 0;
+            s_it[v][nit[v]++] = e;
+          }
+        }
       mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
       fence_after();
       for (int t = t0; t < t1; ++t, buf ^= 1) {
@@ -452,36 +483,33 @@ f0_kernel(const __grid_constant__ F0Args a)
         const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
         uint32_t first = 1u, a_lo = a_base;
         for (int i = 0; i < nf_u; ++i) {
-          const int n_kc = bcast(seg[1].L[i]) >> 5;
+          const int n_kc = seg[1].L[i] >> 5;
           for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
             mbar_wait(bfull + 8u * rg.s, rg.ph);
             fence_after();
-            mma_recon_chunk(lead, d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-            commit_e(lead, bempty + 8u * rg.s);
+            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
+            commit(bempty + 8u * rg.s);
             first = 0u;
             rg.advance();
           }
         }
-        for (int r = 0; r < n_lr; ++r) {
-          if (!((have_q >> r) & 1u)) continue;
-          const int m0 = (t * 128) >> a.up[r].log2d;
-          const int var = ((m0 & 7) && a.up[r].n_var > 1) ? 1 : 0;
-          const int n_it = a.n_items[r][var];
-          for (int i = 0; i < n_it; ++i) {
-            const QItem it = a.item[r][var][i];
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
-            fence_after();
-            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
-            const uint64_t bdesc = desc64(p_base + it.b_off);
-            mma_ss_e(lead, d_tmem + it.d_off,        desc64(qa),        bdesc, it.idesc, 1u);
-            mma_ss_e(lead, d_tmem + 128u + it.d_off, desc64(qa + 128u), bdesc, it.idesc, 1u);
-            commit_e(lead, bempty + 8u * rg.s);
-            rg.advance();
-          }
+        const ItTab* tab = s_it[t & 1];
+        const int n_it = nit[t & 1];
+        for (int k = 0; k < n_it; ++k) {
+          const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, d_off
+          mbar_wait(bfull + 8u * rg.s, rg.ph);
+          fence_after();
+          const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+          const uint64_t bdesc = desc64(e.y);
+          mma_ss(d_tmem + e.z,        desc64(qa),        bdesc, e.x, 1u);
+          mma_ss(d_tmem + 128u + e.z, desc64(qa + 128u), bdesc, e.x, 1u);
+          commit(bempty + 8u * rg.s);
+          rg.advance();
         }
-        commit_e(lead, smem_u32(&bars.acc_full[buf]));
+        commit(smem_u32(&bars.acc_full[buf]));
       }
       ++seg_i;
+    }
     }
   } else {
     // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
@@ -666,6 +694,13 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
   }
   pl->p_bytes = (int)(pblob.size() * sizeof(__half));
+  for (int r = 0; r < pl->n_lr; ++r)                       // the kernels rely on: active chunks of a variant are consecutive,
+    for (int v = 0; v < pl->up[r].n_var; ++v) {            // and only a window start that alternates with t has two variants
+      int first = -1, last = -1, cnt = 0;
+      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch)
+        if (pl->up[r].nn[v][ch]) { if (first < 0) first = ch; last = ch; ++cnt; }
+      if (cnt == 0 || last - first + 1 != cnt) return true;
+    }
 
   // shared-memory budgets (operands stationary: R of the CTA's template block, and P)
   const int f0_fixed = pl->l_sum_f0_max * 512 + pl->p_bytes;
@@ -732,7 +767,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
 
 int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
-                     int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
+                     int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
 {
   if (pl->low_units > 0) {
     SchedArgs sc;
@@ -750,6 +785,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
                                                                   sc, pl->l_sum_low_max * 512, pl->low_stages);
     ++*launches;
   }
+  if (after_lowrate) cudaEventRecord(after_lowrate, st);
   F0Args a;
   memset(&a, 0, sizeof a);
   a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;

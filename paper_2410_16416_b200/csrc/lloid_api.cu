@@ -161,15 +161,19 @@ int check_ids(const lloid_bank* b, int bin, int det, int slice)
 }
 
 // profiling: the time between two consecutive events is charged to the stage tag of the later one
-enum { kTagStart = -1, kTagResample = 0, kTagFir = 1, kTagRecon = 2, kTagMerge = 3 };
-void mark(lloid_bank* b, cudaStream_t st, int tag)
+enum { kTagStart = -1, kTagResample = 0, kTagFir = 1, kTagRecon = 2, kTagMerge = 3, kTagLowRecon = 5 };
+cudaEvent_t grab(lloid_bank* b, int tag)          // next event of the list, tagged; the caller records it
 {
-  if (!b->prof) return;
+  if (!b->prof) return nullptr;
   if (b->events_used == b->events.size()) {
     cudaEvent_t e; cudaEventCreate(&e); b->events.push_back(e); b->event_tag.push_back(tag);
   }
   b->event_tag[b->events_used] = tag;
-  cudaEventRecord(b->events[b->events_used++], st);
+  return b->events[b->events_used++];
+}
+void mark(lloid_bank* b, cudaStream_t st, int tag)
+{
+  if (cudaEvent_t e = grab(b, tag)) cudaEventRecord(e, st);
 }
 
 // A1 for one super-chunk [k_s, k_s + n_s): xw = [history | strain], new history saved, every rate resampled once.
@@ -204,7 +208,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     mark(b, st, kTagFir);
     if (f16_plan_tensor_recon(b->plan16)) {
       if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
-                           &b->last_launches))
+                           &b->last_launches, grab(b, kTagLowRecon)))
         return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     } else {
       launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
@@ -614,7 +618,7 @@ int lloid_set_profiling(lloid_bank_t* b, int32_t enable)
 int lloid_last_stage_ms(lloid_bank_t* b, float* out)
 {
   if (!b || !out) return fail(LLOID_EINVAL, "null argument");
-  for (int i = 0; i < 5; ++i) out[i] = 0.f;
+  for (int i = 0; i < 6; ++i) out[i] = 0.f;
   if (!b->prof || b->events_used < 2) return fail(LLOID_ESTATE, "profiling was not enabled for the last call");
   CU(cudaEventSynchronize(b->events[b->events_used - 1]));
   for (size_t i = 1; i < b->events_used; ++i) {
@@ -625,6 +629,7 @@ int lloid_last_stage_ms(lloid_bank_t* b, float* out)
   }
   float ms = 0.f; CU(cudaEventElapsedTime(&ms, b->events[0], b->events[b->events_used - 1]));
   out[4] = ms;
+  out[2] += out[5];                               // [5] (low-rate reconstruction kernel) is a part of [2]
   return LLOID_OK;
 }
 

@@ -149,6 +149,7 @@ bool f16_plan_tensor_recon(const F16Plan*);   // false: bank outside the tensor 
 int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches);
 int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
-                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches);
+                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches,
+                      cudaEvent_t after_lowrate /* recorded between the two kernels when non-null */);
 
 }  // namespace lloid
