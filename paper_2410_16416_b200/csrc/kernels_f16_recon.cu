@@ -29,6 +29,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 
 namespace lloid {
 
@@ -42,7 +43,7 @@ constexpr int RC16_SMEM_BUDGET = 220 * 1024;
 struct LowUnit { int32_t group, rb; };
 
 struct RingBars {
-  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES], acc_full[2], acc_empty[2], consts;
+  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES], acc_full[2], acc_empty[2], consts, unit_done;
 };
 
 struct Ring {                               // stage index + phase parity, advanced without division
@@ -94,6 +95,7 @@ __device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int
     for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&B.full[s]), 1); mbar_init(smem_u32(&B.empty[s]), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 128); }
     mbar_init(smem_u32(&B.consts), 1);
+    mbar_init(smem_u32(&B.unit_done), 1);
     mbar_init_fence();
   }
 }
@@ -194,7 +196,9 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       int countdown = (seg_i == 0) ? 0 : n_stages;      // ring stages to push before R is replaced
       bool r_done = false;
       auto load_R = [&]() {
-        if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
+        // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
+        // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
+        if (seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(seg_i - 1) & 1u);
         {
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
           uint32_t off = 0;
@@ -257,6 +261,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         }
         commit(smem_u32(&bars.acc_full[buf]));
       }
+      commit(smem_u32(&bars.unit_done));
       ++seg_i;
     }
     }
@@ -408,7 +413,9 @@ f0_kernel(const __grid_constant__ F0Args a)
       int countdown = (seg_i == 0) ? 0 : n_stages;
       bool r_done = false;
       auto load_R = [&]() {
-        if (seg_i > 0) { const int gl = g - 1; mbar_wait(smem_u32(&bars.acc_full[gl & 1]), (uint32_t)(gl >> 1) & 1u); }
+        // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
+        // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
+        if (seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(seg_i - 1) & 1u);
         {
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
           uint32_t off = 0;
@@ -508,6 +515,7 @@ f0_kernel(const __grid_constant__ F0Args a)
         }
         commit(smem_u32(&bars.acc_full[buf]));
       }
+      commit(smem_u32(&bars.unit_done));
       ++seg_i;
     }
     }
@@ -786,6 +794,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     ++*launches;
   }
   if (after_lowrate) cudaEventRecord(after_lowrate, st);
+  if (getenv("LLOID_DEBUG_SYNC") && cudaStreamSynchronize(st) != cudaSuccess) { fprintf(stderr, "lloid: lowrate_recon_kernel faulted\n"); return 1; }
   F0Args a;
   memset(&a, 0, sizeof a);
   a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;

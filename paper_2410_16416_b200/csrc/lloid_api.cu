@@ -8,6 +8,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -191,6 +192,17 @@ int stage_superchunk(lloid_bank* b, const float* strain, int64_t pitch, int n_s,
   return LLOID_OK;
 }
 
+// LLOID_DEBUG_SYNC=1 in the environment: synchronise after every kernel of a chunk and name the one that faulted
+// (debugging aid only; lloid_filter is then no longer asynchronous).
+int debug_sync(const char* what, int64_t k_a, cudaStream_t st)
+{
+  static const bool on = getenv("LLOID_DEBUG_SYNC") != nullptr;
+  if (!on) return LLOID_OK;
+  const cudaError_t e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(LLOID_ECUDA, "%s faulted in the chunk starting at sample %lld: %s", what, (long long)k_a, cudaGetErrorString(e));
+  return LLOID_OK;
+}
+
 // A2..A6 for one chunk [k_a, k_a + c) that starts `o` samples into the current super-chunk
 int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* trig, int64_t capacity,
                   unsigned long long* count, cudaStream_t st)
@@ -206,6 +218,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, o, c, st, &b->last_launches))
       return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     mark(b, st, kTagFir);
+    if (int rc = debug_sync("fir_f16_kernel", k_a, st)) return rc;
     if (f16_plan_tensor_recon(b->plan16)) {
       if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
                            &b->last_launches, grab(b, kTagLowRecon)))
@@ -216,12 +229,14 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     }
   }
   mark(b, st, kTagRecon);
+  if (int rc = debug_sync("reconstruction kernels", k_a, st)) return rc;
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
   launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, c, k_a,
                        b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
                        b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
   b->state_cur ^= 1;
   mark(b, st, kTagMerge);
+  if (int rc = debug_sync("merge_windows_kernel", k_a, st)) return rc;
   CU(cudaGetLastError());
   return LLOID_OK;
 }

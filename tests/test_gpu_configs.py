@@ -1,0 +1,114 @@
+"""GPU-vs-oracle parity at BASELINE.json's sizes and shapes, through the C ABI, in the launch configuration
+bench.py times (automatic chunking, whole strain in one lloid_filter call).  The oracle cannot run a full config,
+so outputs are SAMPLED: the dense SNR of one peak window around an injection (all templates, one detector) is
+compared element by element, the triggers of that window go through the comparison rule of tests/parity_util.py,
+and properties that hold at any size are checked on everything else (one trigger per (bin, detector, template,
+window) at most, every injection recovered in every detector at its injected time, replicated bins identical).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2410_16416_b200 import binding as lb          # noqa: E402
+from paper_2410_16416_b200 import workloads as wl        # noqa: E402
+import parity_util as pu                                 # noqa: E402
+
+PRECISIONS = [pytest.param(lb.LLOID_F32, id="fp32"), pytest.param(lb.LLOID_F16, id="fp16")]
+
+
+def _unique_keys(trigs, W):
+    keys = np.stack([trigs["bin"].astype(np.int64), trigs["detector"].astype(np.int64),
+                     trigs["template_idx"].astype(np.int64), trigs["sample"] // W], axis=1)
+    return len(np.unique(keys, axis=0)) == len(keys)
+
+
+@pytest.fixture(scope="module")
+def cfg2_full():
+    return wl.config2()          # 1000 templates, 8 slices, L = 150, 2 detectors x 4096 s, 20 injections
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config2_full_size_sampled(cfg2_full, precision):
+    w = cfg2_full
+    W, tol = w.peak_window, pu.TOL[precision]
+    inj = w.injections[13]
+    det = 1
+    k0 = (inj.end // W) * W                       # the peak window that holds injection 13
+    trigs, snr, info = pu.run_gpu(w, precision, capture=(0, det, k0, W))
+    assert info["consumed"] == w.n_samples and info["counts"][0] == len(trigs)
+    rho = pu.oracle_snr(w, 0, det, k0, k0 + W)
+    assert not np.isnan(snr).any()
+    err = np.abs(snr - rho)
+    assert err.max() <= tol, f"dense SNR error {err.max():.3e} > {tol}"
+    stats = pu.check_triggers(trigs, rho, k0, w, 0, det, tol)
+    assert stats["checked"] == 1000 and stats["triggers"] > 0
+    # properties at full size
+    assert _unique_keys(trigs, W)
+    amp = np.hypot(trigs["snr_re"], trigs["snr_im"])
+    assert (amp > w.threshold).all() and np.isfinite(amp).all()
+    assert trigs["sample"].min() >= 0 and trigs["sample"].max() < w.n_samples
+    for i in w.injections:                        # every injection, both detectors, at its injected time
+        for d in range(w.n_detectors):
+            hit = trigs[(trigs["detector"] == d) & (trigs["template_idx"] == i.template) & (np.abs(trigs["sample"] - i.end) <= 2)]
+            assert len(hit) == 1, f"injection p={i.template} e={i.end} det={d} not recovered"
+            a = float(np.hypot(hit[0]["snr_re"], hit[0]["snr_im"]))
+            assert abs(a - i.amplitude) < 4.5, (a, i.amplitude)   # retained power >= 0.9 (R14) and unit noise
+    # noise trigger rate: chi^2_2 tail over ~2000 independent samples per window (0.1 - 0.5)
+    rate = len(trigs) / (1000 * w.n_detectors * (w.n_samples // W))
+    assert 0.05 < rate < 0.6, rate
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config3_hundred_bins_batched(precision):
+    """BASELINE config 3 shape: 100 bins x 500 templates x 2 detectors, 3 slices 2048/512/128 Hz, L = 64, three
+    template-length classes; shortened to 40 s of strain (cost is linear in duration)."""
+    w = wl.config3(n_bins=100, n_templates=500, seconds=40, n_detectors=2, n_basis=64)
+    tol = pu.TOL[precision]
+    W = w.peak_window
+    bin_, det = 57, 1                              # 4 s class
+    k0 = 10 * W
+    trigs, snr, info = pu.run_gpu(w, precision, capture=(bin_, det, k0, 2 * W))
+    rho = pu.oracle_snr(w, bin_, det, k0, k0 + 2 * W)
+    assert np.abs(snr - rho).max() <= tol
+    pu.check_triggers(trigs, rho, k0, w, bin_, det, tol)
+    assert _unique_keys(trigs, W)
+    assert set(np.unique(trigs["bin"])) == set(range(100)) and set(np.unique(trigs["detector"])) == {0, 1}
+    # bins of one shape class share their arrays (the paper replicates one bank): identical triggers
+    strip = lambda t: sorted((int(x["detector"]), int(x["template_idx"]), int(x["sample"]), float(x["snr_re"])) for x in t)
+    assert w.bins[34] is w.bins[57]
+    assert strip(trigs[trigs["bin"] == 34]) == strip(trigs[trigs["bin"] == 57])
+    assert strip(trigs[trigs["bin"] == 0]) != strip(trigs[trigs["bin"] == 57])
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config4_geometry_heterogeneous_L(precision):
+    """BASELINE config 4 shape: 6 slices 2048..64 Hz, M = 64 s, L(b, s) = 100 + ((37 b + 61 s) mod 201) in
+    [100, 300], 3 detectors; reduced to 5 bins x 160 templates x 100 s."""
+    w = wl.config4(n_bins=5, n_templates=160, seconds=100, n_detectors=3, n_distinct=2)
+    Ls = sorted({s.n_basis for b in w.bins for s in b.slices})
+    assert Ls[0] >= 100 and Ls[-1] > 256, Ls       # spans the L_pad <= 256 and > 256 code paths
+    tol = pu.TOL[precision]
+    W = w.peak_window
+    k0 = 66 * W                                    # past the 64 s start-up transient
+    for bin_, det in ((3, 2), (0, 0)):
+        trigs, snr, info = pu.run_gpu(w, precision, capture=(bin_, det, k0, W))
+        rho = pu.oracle_snr(w, bin_, det, k0, k0 + W)
+        assert np.abs(snr - rho).max() <= tol
+        pu.check_triggers(trigs, rho, k0, w, bin_, det, tol)
+    assert _unique_keys(trigs, W)
+
+
+def _as_set(trigs):
+    return sorted((int(t["bin"]), int(t["detector"]), int(t["template_idx"]), int(t["sample"]),
+                   float(t["snr_re"]), float(t["snr_im"])) for t in trigs)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config5_one_second_buffers_equal_one_shot(precision):
+    """BASELINE config 5: the config-3 bank fed 1 s buffers with history carried (A8).  12 bins, 24 s."""
+    w = wl.config3(n_bins=12, n_templates=500, seconds=24, n_detectors=2, n_basis=64)
+    one, _, _ = pu.run_gpu(w, precision)
+    many, _, info = pu.run_gpu(w, precision, pieces=[w.f0] * 24)
+    assert info["consumed"] == w.n_samples and len(info["counts"]) == 24
+    assert _as_set(one) == _as_set(many) and len(one) > 0
