@@ -15,7 +15,7 @@ struct F16Plan {
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
-  int f0_smem = 0, f0_stages = 0;
+  int f0_smem = 0, f0_stages = 0, f0_r_bufs = 1;
   int p_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;
   UpRate up[kNLowRates];
   std::vector<RateGroup> groups_host;   // [n_bd][n_lr]

@@ -318,7 +318,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
 struct F0Args {
   const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups; const uint8_t* P;
   Peak* partials; Capture cap; long long k_a;
-  int n_lr, c, r_bytes, tiles_cap, max_templates, n_stages, p_bytes;
+  int n_lr, c, r_bytes, r_bufs, tiles_cap, max_templates, nsy, nsq, p_bytes;
   SchedArgs sched;                                      // units = combos, one class
   UpRate up[kNLowRates];
   QItem item[kNLowRates][2][8];                         // per rate and variant: the active 16-row chunks, in order (kernel
@@ -347,22 +347,59 @@ __device__ __forceinline__ void seg_f0_fill(SegF0& S, const F0Args& a, const F0C
   }
 }
 
-// Per-unit tables of the interpolation work of one tile, so that the per-chunk code of both single-thread loops
+// Per-unit tables of the interpolation work of one tile, so that the per-chunk code of the single-thread loops
 // is a table read plus the issuing instructions.  v = t & 1 selects the band-matrix variant of the rates whose
 // window start alternates (d = 32); the chunks of a (rate, variant) are consecutive.
 struct ItTab { uint32_t idesc, b_lo, d_off, pad; };                                  // MMA issuer: one per chunk
 struct PrTab { const uint8_t* q; int32_t log2d, ch0[2], n[2]; int32_t pad; };           // producer: one per rate present
 constexpr int kMaxTileItems = kNLowRates * 8;
 
-__global__ void __launch_bounds__(RC16_THREADS, 1)
+// f0_kernel roles.  A single thread sustains one instruction every ~7 cycles, so one producer and one issuer
+// thread cannot feed 19 eight-KB stages per 2600-cycle tile; the work is split over five single-thread roles
+// over two rings (y tiles: PY -> IY; window chunks: PQ0 / PQ1 alternate -> IQ).  Each ring has ONE consumer, so its
+// slots are released in order and a producer can never run two laps ahead of a slot (which would alias the
+// barrier's phase parity):
+//   warp 0  PY   bulk copies of the y tiles of the d = 1 slices; owns R and P (stationary operands)
+//   warp 6,7 PQ  bulk copies of the rho^(d) window chunks, even / odd chunk of the tile
+//   warp 1  IY   MMAs of the d = 1 slices into accumulator buf = tile parity, then commit -> ybar[buf]
+//   warp 8  IQ   waits ybar[buf] (the y part is COMPLETE: orders its accumulating MMAs after IY's zeroing one),
+//                interpolation MMAs, commit -> acc_full[buf]
+//   warps 2-5    epilogue (one thread = one template)
+// While IQ works on tile t, IY already fills the other accumulator with tile t + 1.
+constexpr int F0_THREADS = 288;
+
+struct F0Bars {
+  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES];      // y ring: slots [0, nsy); chunk ring: slots [nsy, nsy + nsq)
+  uint64_t acc_full[2], acc_empty[2], ybar[2], consts[2], unit_done[2];
+};
+
+#define FOR_SEGMENTS(u, t0, t1)                                                                   \
+  for (int u = u_lo; u <= u_hi; ++u)                                                              \
+    if (u == u_hi && t_hi == 0) break;                                                            \
+    else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles; t0 >= t1) continue; \
+    else
+
+// stages of one tile of this unit: y chunks, interpolation chunks per variant
+__device__ __forceinline__ void f0_unit_counts(const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B, int& ny, int (&nit)[2])
+{
+  ny = B->l_sum >> 5;
+  nit[0] = nit[1] = 0;
+  for (int r = 0; r < a.n_lr; ++r) {
+    if (a.groups[cb.bd * a.n_lr + r].n_slices == 0) continue;
+    nit[0] += a.n_items[r][0];
+    nit[1] += a.n_items[r][a.up[r].n_var > 1 ? 1 : 0];
+  }
+}
+
+__global__ void __launch_bounds__(F0_THREADS, 1)
 f0_kernel(const __grid_constant__ F0Args a)
 {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) RingBars bars;
+  __shared__ __align__(8) F0Bars bars;
   __shared__ uint32_t tmem_slot;
-  __shared__ SegF0 seg[2];                              // [0] producer's, [1] MMA issuer's
+  __shared__ SegF0 seg[2];                              // [0] PY's, [1] IY's
   __shared__ __align__(16) ItTab s_it[2][kMaxTileItems];
-  __shared__ PrTab s_pr[kNLowRates];
+  __shared__ PrTab s_pr[2][kNLowRates];
   __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -372,163 +409,200 @@ f0_kernel(const __grid_constant__ F0Args a)
   if (u_lo == u_hi && t_lo == t_hi) return;
   const int n_tiles = a.sched.n_tiles[0];
 
-  const int n_stages = a.n_stages;
-  ring_setup(bars, &tmem_slot, n_stages, warp, tid);
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  if (tid == 32) {
+    for (int s = 0; s < RC16_MAX_STAGES; ++s) { mbar_init(smem_u32(&bars.full[s]), 1); mbar_init(smem_u32(&bars.empty[s]), 1); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(smem_u32(&bars.acc_full[b]), 1); mbar_init(smem_u32(&bars.acc_empty[b]), 128);
+      mbar_init(smem_u32(&bars.ybar[b]), 1); mbar_init(smem_u32(&bars.consts[b]), 1); mbar_init(smem_u32(&bars.unit_done[b]), 1);
+    }
+    mbar_init_fence();
+  }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem = tmem_slot;
   const int n_lr = a.n_lr;
+  const int nsy = a.nsy, nsq = a.nsq;
+  const int r_bufs = a.r_bufs;
   const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]);
-  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16
-  const uint32_t sP_u = sR_u + (uint32_t)a.r_bytes;     // band matrices
+  const uint32_t qfull = bfull + 8u * nsy, qempty = bempty + 8u * nsy;
+  const uint32_t sR_u = smem_u32(smem);                 // r_bufs x [l_sum / 8][2][128][8] fp16
+  const uint32_t sP_u = sR_u + (uint32_t)(a.r_bytes * r_bufs);   // band matrices
   const uint32_t ring_u = sP_u + (uint32_t)a.p_bytes;
+  const uint32_t qring_u = ring_u + (uint32_t)nsy * RC16_STAGE;
 
   if (warp == 0) {
-    // ===== producer: one elected thread =====
+    // ===== PY: y tiles of the d = 1 slices, R and P =====
     if (elect_one()) {
-    Ring rg{0, 0u, n_stages};
-    int g = 0, seg_i = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
-      if (t0 >= t1) continue;
-      const F0Combo cb = a.combos[u];
-      const BdPlan* B = a.bd + cb.bd;
-      seg_f0_fill(seg[0], a, cb, B);
-      const int nf_u = B->n_f0;
-      const uint32_t rbytes_u = (uint32_t)B->l_sum * 512u;
-      int npr = 0;
-      for (int r = 0; r < n_lr; ++r) {
-        if (seg[0].Q[r] == nullptr) continue;
-        PrTab e;
-        e.q = seg[0].Q[r]; e.log2d = a.up[r].log2d; e.pad = 0;
-        for (int v = 0; v < 2; ++v) {
-          const int vv = a.up[r].n_var > 1 ? v : 0;
-          e.n[v] = a.n_items[r][vv];
-          e.ch0[v] = e.n[v] > 0 ? (int)a.item[r][vv][0].ch : 0;
-        }
-        s_pr[npr++] = e;
-      }
-      int countdown = (seg_i == 0) ? 0 : n_stages;
-      bool r_done = false;
-      auto load_R = [&]() {
-        // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
-        // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
-        if (seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(seg_i - 1) & 1u);
-        {
-          mbar_expect_tx(smem_u32(&bars.consts), rbytes_u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
-          uint32_t off = 0;
+      int seg_i = 0;
+      Ring rg{0, 0u, nsy};
+      FOR_SEGMENTS(u, t0, t1) {
+        const F0Combo cb = a.combos[u];
+        const BdPlan* B = a.bd + cb.bd;
+        seg_f0_fill(seg[0], a, cb, B);
+        const int nf_u = B->n_f0;
+        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
+        // R (and P, once) go out after `pre` y stages of the unit's first tile are in flight: the ring refills while
+        // the previous unit drains, and the switch costs one R load.  pre <= ring size, or IY (which waits for R) could
+        // never free the slot PY is waiting for.
+        int pre = (seg_i == 0) ? 0 : min(nsy, B->l_sum >> 5);
+        bool need_R = true;
+        auto load_R = [&]() {
+          // this R buffer's previous unit is complete (per-buffer barrier: never more than one phase away)
+          if (use > 0) mbar_wait(smem_u32(&bars.unit_done[rb_i]), (uint32_t)(use - 1) & 1u);
+          const uint32_t cb_u = smem_u32(&bars.consts[rb_i]);
+          mbar_expect_tx(cb_u, (uint32_t)B->l_sum * 512u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
+          uint32_t off = (uint32_t)(rb_i * a.r_bytes);
           for (int i = 0; i < nf_u; ++i) {
-            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, smem_u32(&bars.consts));
+            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, cb_u);
             off += (uint32_t)seg[0].L[i] * 512u;
           }
-          if (seg_i == 0) copy_pieces(sP_u, a.P, (uint32_t)a.p_bytes, smem_u32(&bars.consts));
-        }
-        r_done = true;
-      };
-      if (countdown == 0) load_R();
-      for (int t = t0; t < t1; ++t) {
-        for (int i = 0; i < nf_u; ++i) {
-          const int L = seg[0].L[i];
-          const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;
-          for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-            produce(rg, bfull, bempty, ring_u, src);
-            if (!r_done && --countdown == 0) load_R();
+          if (seg_i == 0) copy_pieces(sP_u, a.P, (uint32_t)a.p_bytes, cb_u);
+          need_R = false;
+        };
+        if (pre == 0) load_R();
+        for (int t = t0; t < t1; ++t)
+          for (int i = 0; i < nf_u; ++i) {
+            const int L = seg[0].L[i];
+            const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;      // tiles are contiguous in Y16
+            for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
+              produce(rg, bfull, bempty, ring_u, src);
+              if (need_R && --pre == 0) load_R();
+            }
           }
+        ++seg_i;
+      }
+    }
+  } else if (warp == 6 || warp == 7) {
+    // ===== PQ: rho^(d) window chunks, even (warp 6) / odd (warp 7) chunk of the tile =====
+    if (elect_one()) {
+      const int pq = warp - 6;
+      PrTab* tab = s_pr[pq];
+      Ring rg{0, 0u, nsq};
+      int own = pq == 0;                                 // the ring's stages alternate between the two PQ threads
+      FOR_SEGMENTS(u, t0, t1) {
+        const F0Combo cb = a.combos[u];
+        int npr = 0;
+        for (int r = 0; r < n_lr; ++r) {
+          const RateGroup* G = a.groups + cb.bd * n_lr + r;
+          if (G->n_slices == 0) continue;
+          PrTab e;
+          e.q = reinterpret_cast<const uint8_t*>(G->Q) + (size_t)cb.rb * G->q_groups_cap * 4096;
+          e.log2d = a.up[r].log2d; e.pad = 0;
+          for (int v = 0; v < 2; ++v) {
+            const int vv = a.up[r].n_var > 1 ? v : 0;
+            e.n[v] = a.n_items[r][vv];
+            e.ch0[v] = e.n[v] > 0 ? (int)a.item[r][vv][0].ch : 0;
+          }
+          tab[npr++] = e;
         }
-        const int v = t & 1;
-        for (int j = 0; j < npr; ++j) {
-          const PrTab* e = &s_pr[j];
-          const int ws = ((t * 128) >> e->log2d) & ~7;
-          const uint8_t* src = e->q + (size_t)(ws >> 3) * 4096 + (size_t)e->ch0[v] * RC16_STAGE;
-          const int n_it = e->n[v];
-          for (int i = 0; i < n_it; ++i, src += RC16_STAGE) {
-            produce(rg, bfull, bempty, ring_u, src);
-            if (!r_done && --countdown == 0) load_R();
+        for (int t = t0; t < t1; ++t) {
+          const int v = t & 1;
+          for (int j = 0; j < npr; ++j) {
+            const PrTab* e = &tab[j];
+            const int ws = ((t * 128) >> e->log2d) & ~7;
+            const uint8_t* src = e->q + (size_t)(ws >> 3) * 4096 + (size_t)e->ch0[v] * RC16_STAGE;
+            const int n_it = e->n[v];
+            for (int i = 0; i < n_it; ++i, src += RC16_STAGE, own ^= 1) {
+              if (own) produce(rg, qfull, qempty, qring_u, src); else rg.advance();
+            }
           }
         }
       }
-      if (!r_done) load_R();
-      g += t1 - t0; ++seg_i;
-    }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: one elected thread =====
+    // ===== IY: MMAs of the d = 1 slices =====
     if (elect_one()) {
-    const uint32_t idesc128 = idesc_f16(128, 128);
-    const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
-    const uint32_t qa_base = desc_lo(ring_u, 4096u), p_base = desc_lo(sP_u, 2048u);
-    const uint32_t tm = tmem;
-    Ring rg{0, 0u, n_stages};
-    uint32_t eph = 3u;
-    int buf = 0, seg_i = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
-      if (t0 >= t1) continue;
-      const F0Combo cb = a.combos[u];
-      const BdPlan* B = a.bd + cb.bd;
-      seg_f0_fill(seg[1], a, cb, B);
-      const int nf_u = B->n_f0;
-      int nit[2] = {0, 0};
-      for (int v = 0; v < 2; ++v)
-        for (int r = 0; r < n_lr; ++r) {
-          if (seg[1].Q[r] == nullptr) continue;
-          const int vv = a.up[r].n_var > 1 ? v : 0;
-          for (int i = 0; i < a.n_items[r][vv]; ++i) {
-            const QItem it = a.item[r][vv][i];
-            ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.d_off = it.d_off; e.pad = 0;
-            s_it[v][nit[v]++] = e;
-          }
-        }
-      mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
-      fence_after();
-      for (int t = t0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+      const uint32_t idesc128 = idesc_f16(128, 128);
+      const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
+      uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
+      int seg_i = 0, buf = 0;
+      Ring rg{0, 0u, nsy};
+      FOR_SEGMENTS(u, t0, t1) {
+        const F0Combo cb = a.combos[u];
+        const BdPlan* B = a.bd + cb.bd;
+        seg_f0_fill(seg[1], a, cb, B);
+        const int nf_u = B->n_f0;
+        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
+        mbar_wait(smem_u32(&bars.consts[rb_i]), (uint32_t)use & 1u);
         fence_after();
-        const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
-        uint32_t first = 1u, a_lo = a_base;
-        for (int i = 0; i < nf_u; ++i) {
-          const int n_kc = seg[1].L[i] >> 5;
-          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
+        const uint32_t a_seg = a_base + (uint32_t)((rb_i * a.r_bytes) >> 4);
+        for (int t = t0; t < t1; ++t, buf ^= 1) {
+          mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+          fence_after();
+          const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
+          uint32_t first = 1u, a_lo = a_seg;
+          for (int i = 0; i < nf_u; ++i) {
+            const int n_kc = seg[1].L[i] >> 5;
+            for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
+              mbar_wait(bfull + 8u * rg.s, rg.ph);
+              fence_after();
+              mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
+              commit(bempty + 8u * rg.s);
+              first = 0u;
+              rg.advance();
+            }
+          }
+          commit(smem_u32(&bars.ybar[buf]));
+        }
+        ++seg_i;
+      }
+    }
+  } else if (warp == 8) {
+    // ===== IQ: interpolation MMAs (A4), after the tile's y part is complete =====
+    if (elect_one()) {
+      const uint32_t qa_base = desc_lo(qring_u, 4096u), p_base = desc_lo(sP_u, 2048u);
+      uint32_t yph = 0u;
+      int seg_i = 0, buf = 0;
+      Ring rg{0, 0u, nsq};
+      FOR_SEGMENTS(u, t0, t1) {
+        const F0Combo cb = a.combos[u];
+        const BdPlan* B = a.bd + cb.bd;
+        int nit[2] = {0, 0};
+        for (int v = 0; v < 2; ++v)
+          for (int r = 0; r < n_lr; ++r) {
+            if (a.groups[cb.bd * n_lr + r].n_slices == 0) continue;
+            const int vv = a.up[r].n_var > 1 ? v : 0;
+            for (int i = 0; i < a.n_items[r][vv]; ++i) {
+              const QItem it = a.item[r][vv][i];
+              ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.d_off = it.d_off; e.pad = 0;
+              s_it[v][nit[v]++] = e;
+            }
+          }
+        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
+        if (seg_i == 0) { mbar_wait(smem_u32(&bars.consts[0]), 0u); fence_after(); }   // P has landed (loaded once, with the first R)
+        for (int t = t0; t < t1; ++t, buf ^= 1) {
+          mbar_wait(smem_u32(&bars.ybar[buf]), (yph >> buf) & 1u); yph ^= 1u << buf;
+          fence_after();
+          const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
+          const ItTab* tab = s_it[t & 1];
+          const int n_it = nit[t & 1];
+          for (int k = 0; k < n_it; ++k) {
+            const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, d_off
+            mbar_wait(qfull + 8u * rg.s, rg.ph);
             fence_after();
-            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-            commit(bempty + 8u * rg.s);
-            first = 0u;
+            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
+            const uint64_t bdesc = desc64(e.y);
+            mma_ss(d_tmem + e.z,        desc64(qa),        bdesc, e.x, 1u);
+            mma_ss(d_tmem + 128u + e.z, desc64(qa + 128u), bdesc, e.x, 1u);
+            commit(qempty + 8u * rg.s);
             rg.advance();
           }
+          commit(smem_u32(&bars.acc_full[buf]));
         }
-        const ItTab* tab = s_it[t & 1];
-        const int n_it = nit[t & 1];
-        for (int k = 0; k < n_it; ++k) {
-          const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, d_off
-          mbar_wait(bfull + 8u * rg.s, rg.ph);
-          fence_after();
-          const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
-          const uint64_t bdesc = desc64(e.y);
-          mma_ss(d_tmem + e.z,        desc64(qa),        bdesc, e.x, 1u);
-          mma_ss(d_tmem + 128u + e.z, desc64(qa + 128u), bdesc, e.x, 1u);
-          commit(bempty + 8u * rg.s);
-          rg.advance();
-        }
-        commit(smem_u32(&bars.acc_full[buf]));
+        commit(smem_u32(&bars.unit_done[rb_i]));
+        (void)use;
+        ++seg_i;
       }
-      commit(smem_u32(&bars.unit_done));
-      ++seg_i;
     }
-    }
-  } else {
+  } else if (warp >= 2 && warp <= 5) {
     // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
     const int q = warp & 3;
     const int pl = q * 32 + lane;
     uint32_t fph = 0u;
     int buf = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles;
-      if (t0 >= t1) continue;
+    FOR_SEGMENTS(u, t0, t1) {
       const F0Combo cb = a.combos[u];
       const int n_templates = a.bd[cb.bd].n_templates;
       const int p = cb.rb * kTplBlock + pl;
@@ -711,9 +785,12 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
 
   // shared-memory budgets (operands stationary: R of the CTA's template block, and P)
-  const int f0_fixed = pl->l_sum_f0_max * 512 + pl->p_bytes;
+  // R double-buffered (no bubble at a unit switch) when that still leaves >= 8 ring stages
+  pl->f0_r_bufs = (RC16_SMEM_BUDGET - 2 * pl->l_sum_f0_max * 512 - pl->p_bytes) / RC16_STAGE >= 8 ? 2 : 1;
+  const int f0_fixed = pl->f0_r_bufs * pl->l_sum_f0_max * 512 + pl->p_bytes;
   const int low_fixed = pl->l_sum_low_max * 512;
   pl->f0_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - f0_fixed) / RC16_STAGE);
+
   pl->low_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - low_fixed) / RC16_STAGE);
   if (f0_fixed > RC16_SMEM_BUDGET || low_fixed > RC16_SMEM_BUDGET || pl->f0_stages < 4 || (pl->n_lr > 0 && pl->low_stages < 4)) return true;
   pl->f0_smem = f0_fixed + pl->f0_stages * RC16_STAGE;
@@ -809,7 +886,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   // one CTA per SM; when the units fit, a whole number of CTAs per unit so that no CTA has to swap R mid-way
   int grid = (n_combos <= pl->n_sm) ? n_combos * (pl->n_sm / n_combos) : pl->n_sm;
   grid = (int)std::min<long long>(grid, (long long)n_combos * n_tiles);
-  a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.n_stages = pl->f0_stages; a.p_bytes = pl->p_bytes;
+  a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.nsy = std::max(2, pl->f0_stages / 3); a.nsq = pl->f0_stages - a.nsy; a.r_bufs = pl->f0_r_bufs; a.p_bytes = pl->p_bytes;
   for (int r = 0; r < kNLowRates; ++r) a.up[r] = pl->up[r];
   for (int r = 0; r < pl->n_lr; ++r)
     for (int v = 0; v < pl->up[r].n_var; ++v)
@@ -822,9 +899,11 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
         it.d_off = (uint32_t)U.n0[v][ch] * 8u;
         it.ch = (uint32_t)ch;
       }
-  f0_kernel<<<grid, RC16_THREADS, pl->f0_smem, st>>>(a);
+  f0_kernel<<<grid, F0_THREADS, pl->f0_smem, st>>>(a);
   ++*launches;
-  return cudaGetLastError() == cudaSuccess ? 0 : 1;
+  const cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) fprintf(stderr, "lloid: f0_kernel launch (grid %d, %d threads, %d B shared, %zu B params): %s\n", grid, F0_THREADS, pl->f0_smem, sizeof a, cudaGetErrorString(e));
+  return e == cudaSuccess ? 0 : 1;
 }
 
 }  // namespace lloid

@@ -409,17 +409,13 @@ int lloid_bank_finalize(lloid_bank_t* b)
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
   int64_t C = b->cfg.max_chunk;
   if (C == 0) {
-    // (a) keep a chunk's intermediates (y^s, and on the fp16 path the low-rate rho^(d)) within a fraction of
-    //     the 126 MB L2: they are written by one kernel and consumed by the next;
-    // (b) but give every launch enough (template block x time tile) units to fill the 148 SMs many times over,
-    //     or the per-CTA prologue (operand staging, TMEM allocation) and the launch tail dominate.
-    const double budget = (b->f16 ? 72.0 : 96.0) * 1024 * 1024;
-    int64_t c_l2 = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
-    int64_t blocks = 0;
-    for (const BinHost& B : b->bins) blocks += (int64_t)D * ((B.N + kTplBlock - 1) / kTplBlock);
-    int64_t c_work = (int64_t)kTimeTile * 148 * 28 / std::max<int64_t>(blocks, 1) / 2048 * 2048;
-    C = std::max(c_l2, c_work);
-    C = std::min<int64_t>(std::max<int64_t>(C, 2048), 65536);
+    // Every chunk costs four kernel boundaries (launch gap, prologue with TMEM allocation and the stationary
+    // operands, pipeline fill and drain: ~60 us in total, measured), so chunks are made LONG: up to 2^17 samples,
+    // bounded by 4 GiB of chunk-local intermediates (y^s, and on the fp16 path the low-rate rho^(d)).  Keeping the
+    // intermediates L2-resident with short chunks was measured slower on every config.
+    const double budget = 4.0 * 1024 * 1024 * 1024;
+    C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
+    C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
   }
   b->H = (int)H; b->C = (int)C;
   // A1 runs once per super-chunk of S samples (not per chunk): the strain is tiny (8 KB/s per detector), so a
