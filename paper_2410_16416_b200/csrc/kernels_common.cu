@@ -1,6 +1,7 @@
 // A1 polyphase resampler, A5/A6 peak merge + trigger compaction, state reset.
 // Shared by the fp32 and fp16 paths.  See lloid_internal.h for the chunk-local coordinates.
 #include "lloid_internal.h"
+#include <algorithm>
 #include "../../include/lloid.h"
 
 namespace lloid {
@@ -67,6 +68,89 @@ resample_kernel(const RateParams* __restrict__ rates, const float* __restrict__ 
   }
 }
 
+// Register-tiled variant (K_dn even): one thread produces 4 consecutive outputs with a sliding window of the
+// strain in registers, so one shared-memory load and one (broadcast) tap load feed 4 FMAs.  The segment is stored
+// xs4[phi][m & 3][m >> 2] (decimation phase, then the residue of the low-rate index): thread t reads quotient
+// t + const of one residue row -- consecutive banks -- for every window element.  Taps are staged per phase,
+// tp[phi][a] = taps[a d + phi].  128 threads x 4 = 512 outputs per CTA.
+constexpr int kRes4Threads = 128, kRes4Out = 4 * kRes4Threads;
+
+__global__ void __launch_bounds__(kRes4Threads)
+resample4_kernel(const RateParams* __restrict__ rates, const float* __restrict__ xw, int xw_pitch,
+                 int xw_valid, int k_dn, int c, int want_f16)
+{
+  const RateParams R = rates[blockIdx.z];
+  const int det = blockIdx.y;
+  const int d = R.d;
+  const int jj_lo = R.jj_lo_fixed;
+  const int jj_hi = R.jj_hi_off + c / d;
+  const int jj0 = jj_lo + blockIdx.x * kRes4Out;
+  if (jj0 >= jj_hi) return;
+  const float* x = xw + (size_t)det * xw_pitch;
+  const int t = threadIdx.x;
+
+  if (d == 1) {                                   // fp16 copy of the full-rate stream (fp16 path only)
+    if (want_f16)
+      for (int i = t; i < kRes4Out; i += kRes4Threads) {
+        const int jj = jj0 + i;
+        if (jj < jj_hi && jj >= 0 && jj < R.xs_len) R.xs16[(size_t)det * R.xs_len + jj] = __float2half_rn(jj < xw_valid ? x[jj] : 0.f);
+      }
+    return;
+  }
+
+  extern __shared__ float xsm[];
+  const int K2 = 2 * k_dn;
+  const int Q = (kRes4Out + K2) / 4 + 1;          // quotients per residue row
+  float* xs4 = xsm;                               // [d][4][Q]
+  float* tp = xsm + (size_t)d * 4 * Q;            // [d][K2], then the last tap
+  const int seg = d * (kRes4Out + K2) + 1;
+  const int base = d * (jj0 - k_dn);              // xw index of segment element 0
+  for (int i = t; i < seg; i += kRes4Threads) {
+    const int gi = base + i;
+    const float v = (gi >= 0 && gi < xw_valid) ? x[gi] : 0.f;
+    const int m = i / d, phi = i - m * d;
+    xs4[(phi * 4 + (m & 3)) * Q + (m >> 2)] = v;
+  }
+  for (int i = t; i < K2 * d + 1; i += kRes4Threads) {
+    const int a = i / d, phi = i - a * d;
+    tp[(a == K2) ? d * K2 : phi * K2 + a] = __ldg(R.taps + i);
+  }
+  __syncthreads();
+
+  float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+  for (int phi = 0; phi < d; ++phi) {
+    const float* __restrict__ xb = xs4 + (size_t)phi * 4 * Q + t;
+    const float* __restrict__ tb = tp + phi * K2;
+    float w0 = xb[0], w1 = xb[Q], w2 = xb[2 * Q], w3 = xb[3 * Q];
+#pragma unroll 4
+    for (int a4 = 0; a4 < K2; a4 += 4) {
+      const int qn = (a4 >> 2) + 1;
+      const float4 tv = *reinterpret_cast<const float4*>(tb + a4);
+      const float n0 = xb[qn], n1 = xb[Q + qn], n2 = xb[2 * Q + qn], n3 = xb[3 * Q + qn];
+      a0 = fmaf(tv.x, w0, a0); a1 = fmaf(tv.x, w1, a1); a2 = fmaf(tv.x, w2, a2); a3 = fmaf(tv.x, w3, a3);
+      a0 = fmaf(tv.y, w1, a0); a1 = fmaf(tv.y, w2, a1); a2 = fmaf(tv.y, w3, a2); a3 = fmaf(tv.y, n0, a3);
+      a0 = fmaf(tv.z, w2, a0); a1 = fmaf(tv.z, w3, a1); a2 = fmaf(tv.z, n0, a2); a3 = fmaf(tv.z, n1, a3);
+      a0 = fmaf(tv.w, w3, a0); a1 = fmaf(tv.w, n0, a1); a2 = fmaf(tv.w, n1, a2); a3 = fmaf(tv.w, n2, a3);
+      w0 = n0; w1 = n1; w2 = n2; w3 = n3;
+    }
+  }
+  {                                               // last tap: a = 2K, phi = 0; after the loop w_i = x[m = 4t + i + 2K] of phase d-1,
+    const float tl = tp[d * K2];                  // so re-read phase 0
+    const float* __restrict__ xb = xs4 + t + (K2 >> 2);
+    a0 = fmaf(tl, xb[0], a0); a1 = fmaf(tl, xb[Q], a1); a2 = fmaf(tl, xb[2 * Q], a2); a3 = fmaf(tl, xb[3 * Q], a3);
+  }
+  const float acc[4] = {a0, a1, a2, a3};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int jj = jj0 + 4 * t + i;
+    if (jj < jj_hi && jj >= 0 && jj < R.xs_len) {
+      const size_t o = (size_t)det * R.xs_len + jj;
+      R.xs32[o] = acc[i];
+      if (want_f16) R.xs16[o] = __float2half_rn(acc[i]);
+    }
+  }
+}
+
 void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
                      const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
                      bool want_f16, cudaStream_t st, int64_t* launches)
@@ -88,6 +172,26 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
   if (smem > 48 * 1024 && smem > configured) {
     cudaFuncSetAttribute(resample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = smem;
+  }
+  if (k_dn % 2 == 0) {                              // register-tiled kernel: 512 outputs per CTA
+    int blocks4 = 0;
+    for (int r = 0; r < n_rates; ++r) {
+      const RateParams& R = rates_host[r];
+      if (R.d == 1 && !want_f16) continue;
+      const int span = R.jj_hi_off + c / R.d - R.jj_lo_fixed;
+      blocks4 = std::max(blocks4, (span + kRes4Out - 1) / kRes4Out);
+    }
+    const int Q = (kRes4Out + 2 * k_dn) / 4 + 1;
+    const size_t smem4 = sizeof(float) * ((size_t)max_d * 4 * Q + (size_t)max_d * 2 * k_dn + 4);
+    static size_t configured4 = 0;
+    if (smem4 > 48 * 1024 && smem4 > configured4) {
+      cudaFuncSetAttribute(resample4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
+      configured4 = smem4;
+    }
+    dim3 grid4(blocks4, n_det, n_rates);
+    resample4_kernel<<<grid4, kRes4Threads, smem4, st>>>(rates_dev, xw, xw_pitch, xw_valid, k_dn, c, want_f16 ? 1 : 0);
+    ++*launches;
+    return;
   }
   dim3 grid(max_blocks, n_det, n_rates);
   resample_kernel<<<grid, kResBlock, smem, st>>>(rates_dev, xw, xw_pitch, xw_valid, k_dn, c, want_f16 ? 1 : 0);
