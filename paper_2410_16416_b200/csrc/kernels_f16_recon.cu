@@ -153,14 +153,16 @@ __device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __res
 // Persistent: CTA i of gridDim.x runs cost range i of the (rate, unit, tile) sequence (SchedArgs).  At a unit
 // switch the producer first refills the ring with the next unit's y tiles, then waits for the previous unit's
 // last accumulator (all MMAs that read the old R are complete) and only then replaces R: the bubble is one R load.
-__global__ void __launch_bounds__(RC16_THREADS, 1)
+constexpr int LOW_THREADS = 224;             // warps: 0 producer A (+R), 1 MMA issuer, 2-5 epilogue, 6 producer B
+
+__global__ void __launch_bounds__(LOW_THREADS, 1)
 lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
                      const LowUnit* __restrict__ units, const __grid_constant__ SchedArgs sched, int r_bytes, int n_stages)
 {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) RingBars bars;
   __shared__ uint32_t tmem_slot;
-  __shared__ SegLow seg[2];                             // [0] producer's, [1] MMA issuer's
+  __shared__ SegLow seg[3];                             // [0], [2] the producers', [1] MMA issuer's
   __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -178,11 +180,15 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16
   const uint32_t ring_u = sR_u + (uint32_t)r_bytes;
 
-  if (warp == 0) {
-    // ===== producer: one elected thread =====
+  if (warp == 0 || warp == 6) {
+    // ===== producers: two elected threads fill alternate stages of the ring (one thread sustains ~1 instruction per
+    // 7 cycles: a single producer is slower than the MMAs it feeds); warp 0 also owns R =====
     if (elect_one()) {
+    const int pr = warp == 0 ? 0 : 1;
+    SegLow& sg = seg[2 * pr];
     Ring rg{0, 0u, n_stages};
-    int g = 0, seg_i = 0;                               // tiles / segments done so far by this CTA
+    int own = pr == 0;
+    int seg_i = 0;                                      // segments done so far by this CTA
     for (int u = u_lo; u <= u_hi; ++u) {
       if (u == u_hi && t_hi == 0) break;
       const int cls = sched_class(sched, u);
@@ -190,11 +196,11 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       if (t0 >= t1) continue;
       const LowUnit un = units[u];
       const RateGroup* G = groups + un.group;
-      seg_low_fill(seg[0], sp, G, un.rb);
+      seg_low_fill(sg, sp, G, un.rb);
       const int ns_u = G->n_slices;
       const uint32_t rbytes_u = (uint32_t)G->l_sum * 512u;
       int countdown = (seg_i == 0) ? 0 : n_stages;      // ring stages to push before R is replaced
-      bool r_done = false;
+      bool r_done = pr != 0;
       auto load_R = [&]() {
         // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
         // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
@@ -203,24 +209,25 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
           uint32_t off = 0;
           for (int i = 0; i < ns_u; ++i) {
-            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, smem_u32(&bars.consts));
-            off += (uint32_t)seg[0].L[i] * 512u;
+            copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.L[i] * 512u, smem_u32(&bars.consts));
+            off += (uint32_t)sg.L[i] * 512u;
           }
         }
         r_done = true;
       };
-      if (countdown == 0) load_R();
+      if (!r_done && countdown == 0) load_R();
       for (int t = t0; t < t1; ++t)
         for (int i = 0; i < ns_u; ++i) {
-          const int L = seg[0].L[i];
-          const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;          // tiles are contiguous in Y16
+          const int L = sg.L[i];
+          const uint8_t* src = sg.Y[i] + (size_t)t * L * 256;          // tiles are contiguous in Y16
           for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-            produce(rg, bfull, bempty, ring_u, src);
+            if (own) produce(rg, bfull, bempty, ring_u, src); else rg.advance();
+            own ^= 1;
             if (!r_done && --countdown == 0) load_R();
           }
         }
       if (!r_done) load_R();
-      g += t1 - t0; ++seg_i;
+      ++seg_i;
     }
     }
   } else if (warp == 1) {
@@ -866,7 +873,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
       tiles_total += (long long)sc.n_tiles[r] * pl->units_per_rate[r];
     }
     const int grid = (int)std::min<long long>(pl->n_sm, tiles_total);
-    lowrate_recon_kernel<<<grid, RC16_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
+    lowrate_recon_kernel<<<grid, LOW_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
                                                                   sc, pl->l_sum_low_max * 512, pl->low_stages);
     ++*launches;
   }

@@ -179,6 +179,12 @@ __device__ __forceinline__ void bulk_g2s_e(uint32_t lead, uint32_t dst_smem, con
                "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n\t}\n"
                :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(mbar), "r"(lead) : "memory");
 }
+// pull a contiguous global range (16-byte aligned, multiple of 16 bytes) into L2 ahead of its bulk copy: the copy
+// then sees L2-hit latency, so the HBM requests in flight are no longer bounded by the shared-memory ring
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes)
+{
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" :: "l"(src), "r"(bytes) : "memory");
+}
 // global -> shared bulk copy (bytes multiple of 16, both addresses 16-byte aligned); completes on mbar
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t mbar)
 {
