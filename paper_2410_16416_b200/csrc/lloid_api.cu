@@ -413,9 +413,11 @@ int lloid_bank_finalize(lloid_bank_t* b)
     // operands, pipeline fill and drain: ~60 us in total, measured), so chunks are made LONG: up to 2^17 samples,
     // bounded by 4 GiB of chunk-local intermediates (y^s, and on the fp16 path the low-rate rho^(d)).  Keeping the
     // intermediates L2-resident with short chunks was measured slower on every config.
-    const double budget = 4.0 * 1024 * 1024 * 1024;
+    // The fp32 path is different: its reconstruction kernel re-reads every y tile once per 64-row block, so there the
+    // chunk is sized to keep y^s in L2 (96 MB), as measured best (2.3 s vs 3.0 s per config-2 step).
+    const double budget = b->f16 ? 4.0 * 1024 * 1024 * 1024 : 96.0 * 1024 * 1024;
     C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
-    C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
+    C = std::min<int64_t>(std::max<int64_t>(C, 2048), b->f16 ? 131072 : 65536);
   }
   b->H = (int)H; b->C = (int)C;
   // A1 runs once per super-chunk of S samples (not per chunk): the strain is tiny (8 KB/s per detector), so a
