@@ -88,12 +88,12 @@ __device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
   return c;
 }
 
-__device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid)
+__device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid, int n_epilogue_threads)
 {
   if (warp == 0) tmem_alloc(tmem_slot, 512);
   if (tid == 32) {
     for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&B.full[s]), 1); mbar_init(smem_u32(&B.empty[s]), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 128); }
+    for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), n_epilogue_threads); }
     mbar_init(smem_u32(&B.consts), 1);
     mbar_init(smem_u32(&B.unit_done), 1);
     mbar_init_fence();
@@ -153,7 +153,8 @@ __device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __res
 // Persistent: CTA i of gridDim.x runs cost range i of the (rate, unit, tile) sequence (SchedArgs).  At a unit
 // switch the producer first refills the ring with the next unit's y tiles, then waits for the previous unit's
 // last accumulator (all MMAs that read the old R are complete) and only then replaces R: the bubble is one R load.
-constexpr int LOW_THREADS = 224;             // warps: 0 producer A (+R), 1 MMA issuer, 2-5 epilogue, 6 producer B
+constexpr int LOW_THREADS = 352;             // warps: 0 producer A (+R), 1 MMA issuer, 2-5 epilogue (cos rows), 6 producer B,
+                                             // 7-10 epilogue (sin rows): the TMEM -> fp16 -> rho^(d) pass was the slowest stage
 
 __global__ void __launch_bounds__(LOW_THREADS, 1)
 lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
@@ -171,7 +172,7 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
   if (u_lo == u_hi && t_lo == t_hi) return;
 
-  ring_setup(bars, &tmem_slot, n_stages, warp, tid);
+  ring_setup(bars, &tmem_slot, n_stages, warp, tid, 256);
   fence_before();
   __syncthreads();
   fence_after();
@@ -273,8 +274,10 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     }
     }
   } else {
+    // ===== epilogue: warps 2-5 convert the cosine accumulator, warps 7-10 the sine one (lane quarter = warp % 4) =====
     const int q = warp & 3;
     const int pl = q * 32 + lane;
+    const int part = warp >= 7 ? 1 : 0;
     uint32_t fph = 0u;
     int buf = 0;
     for (int u = u_lo; u <= u_hi; ++u) {
@@ -290,8 +293,6 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
         mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
         fence_after();
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
-#pragma unroll 1
-        for (int part = 0; part < 2; ++part)
 #pragma unroll 1
           for (int c0 = 0; c0 < 128; c0 += 32) {
             uint32_t v[32];
