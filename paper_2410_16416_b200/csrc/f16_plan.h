@@ -11,6 +11,12 @@ struct F16Plan {
   // A2 basis FIR
   int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
   int chunk_cap = 0;
+  // persistent FIR (fir_f16_pers_kernel): unit lists per chunk length ([0]: the full chunk, [1]: the last one used)
+  bool fir_pers = false;
+  int fir_n_sm = 148, fir_hk_bytes = 0, fir_stage_cap = 0, fir_pers_stages = 0, fir_pers_smem = 0;
+  std::vector<int2> fir_list_host[2];
+  void* fir_list_dev[2] = {nullptr, nullptr};
+  int fir_list_c[2] = {-1, -1}, fir_list_n[2] = {0, 0};
   // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_recon_kernel) + f0-rate kernel (f0_kernel)
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
   int n_bd = 0, n_lr = 0, n_sm = 148;

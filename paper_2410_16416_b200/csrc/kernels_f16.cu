@@ -17,7 +17,9 @@
 #include "f16_plan.h"
 #include "tc05.cuh"
 
+#include <algorithm>
 #include <cstdio>
+#include <vector>
 
 namespace lloid {
 
@@ -27,7 +29,8 @@ constexpr int FH_THREADS = 192;
 constexpr int FH_KB = 64;                    // taps per pipeline stage
 constexpr int FH_MAX_STAGES = 8;
 
-__device__ __forceinline__ int fir_mt(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
+__host__ __device__ __forceinline__ int fir_mt(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
+static inline int fir_mt_host(int L_pad) { int mt = 512 / L_pad; return mt > 4 ? 4 : (mt < 1 ? 1 : mt); }
 
 __global__ void __launch_bounds__(FH_THREADS, 1)
 fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int o, int c, int n_stages)
@@ -93,31 +96,34 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
   const uint32_t tmem = tmem_slot;
 
   if (warp == 0) {
-    // ===== producer (warp-uniform; see tc05.cuh): U stages, pre-packed [kb][tap group 8][l L_pad][8 taps] =====
-    const uint32_t lead = elect_u32();
-    const uint8_t* src = bcast(reinterpret_cast<const uint8_t*>(P.U16));
-    const int n_kb_u = bcast(n_kb);
-    const uint32_t sbytes = (uint32_t)bcast(stage_bytes);
-    const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]), sB_u = bcast(smem_u32(sB));
+    // ===== producer: one elected thread (ptxas keeps an elect.sync-guarded loop in uniform registers; a per-lane
+    // predicate on the issuing instruction costs an R2UR waterfall per instruction): U stages, pre-packed
+    // [kb][tap group 8][l L_pad][8 taps] =====
+    if (elect_one()) {
+    const uint8_t* src = reinterpret_cast<const uint8_t*>(P.U16);
+    const int n_kb_u = n_kb;
+    const uint32_t sbytes = (uint32_t)stage_bytes;
+    const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]), sB_u = smem_u32(sB);
     int s = 0; uint32_t ph = 0;
     for (int kb = 0; kb < n_kb_u; ++kb, src += sbytes) {
       mbar_wait(bempty + 8u * s, ph ^ 1u);
-      mbar_expect_tx_e(lead, bfull + 8u * s, sbytes);
-      bulk_g2s_e(lead, sB_u + (uint32_t)s * sbytes, src, sbytes, bfull + 8u * s);
+      mbar_expect_tx(bfull + 8u * s, sbytes);
+      bulk_g2s(sB_u + (uint32_t)s * sbytes, src, sbytes, bfull + 8u * s);
       if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
+    }
   } else if (warp == 1) {
-    // ===== MMA issuer (warp-uniform) =====
-    const uint32_t lead = elect_u32();
-    const int Lp_u = bcast(L_pad), n_kb_u = bcast(n_kb), mt_u = bcast(mt_used);
+    // ===== MMA issuer: one elected thread =====
+    if (elect_one()) {
+    const int Lp_u = L_pad, n_kb_u = n_kb, mt_u = mt_used;
     const int n_split = (Lp_u > 256) ? 2 : 1;
     const int Nmma = Lp_u / n_split;
     const uint32_t idesc = idesc_f16(128, Nmma);
     const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]);
     const uint32_t c_lo = desc_lo(smem_u32(sC), 128u);                         // Hankel array: LBO = SBO = 128
-    const uint32_t b_lo0 = desc_lo(bcast(smem_u32(sB)), (uint32_t)(Lp_u * 16));
+    const uint32_t b_lo0 = desc_lo(smem_u32(sB), (uint32_t)(Lp_u * 16));
     const uint32_t b_step = (uint32_t)(Lp_u * FH_KB * 2) >> 4, b_k16 = (uint32_t)(2 * Lp_u);
-    const uint32_t tm = bcast(tmem);
+    const uint32_t tm = tmem;
     int s = 0; uint32_t ph = 0;
     for (int kb = 0; kb < n_kb_u; ++kb) {
       mbar_wait(bfull + 8u * s, ph);
@@ -131,15 +137,16 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
           for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
             const uint64_t adesc = desc64(a_lo + (uint32_t)(k16 * 16));
             for (int h = 0; h < n_split; ++h)
-              mma_ss_e(lead, d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
+              mma_ss(d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
                        (kb | k16) ? 1u : 0u);
           }
         }
-        commit_e(lead, bempty + 8u * s);                                       // stage reusable once these MMAs have read it
+        commit(bempty + 8u * s);                                       // stage reusable once these MMAs have read it
       }
       if (++s == n_stages) { s = 0; ph ^= 1u; }
     }
-    commit_e(lead, smem_u32(&bar_acc));
+    commit(smem_u32(&bar_acc));
+    }
   } else {
     // ===== epilogue: TMEM -> fp16 -> Y16[lc][row][8] =====
     const int q = warp & 3;                                    // TMEM lane quarter this warp may access
@@ -167,6 +174,209 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
           *reinterpret_cast<uint4*>(Yt + (lc + 1) * 1024) = make_uint4(h[4], h[5], h[6], h[7]);
         }
       }
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Persistent variant: one CTA per SM walks the (slice problem, block of MT time tiles) units
+// list[blockIdx.x], list[blockIdx.x + gridDim.x], ...: the host sorts the units by descending cost and deals them in
+// serpentine order, so the SMs finish within ~5 % of each other and neighbours in the list (same slice) share U in L2.
+// What the one-unit-per-CTA kernel serialises is overlapped here:
+//   warps 6-9  stage the strain window of the NEXT unit and expand it into the second Hankel buffer,
+//   warp 0     keeps the U ring full across unit boundaries,
+//   warp 1     issues the MMAs (one elected thread),
+//   warps 2-5  drain the accumulators of the previous unit (TMEM -> fp16 -> Y16); only this drain is still exposed,
+//              because MT x L_pad accumulator columns leave no room for a second set.
+// TMEM, the barriers and the ring are set up once per launch instead of once per unit.
+constexpr int FP_THREADS = 320;
+
+struct FirUnit {                   // what every role derives from the unit index
+  int valid, p, r0, mt_used, n_kb, n_chunks, L_pad, b0;
+};
+
+__device__ __forceinline__ FirUnit fir_unit(const SliceParams* __restrict__ sp, const int2* __restrict__ list, int u, int o, int c)
+{
+  FirUnit U;
+  const int2 e = list[u];                // (problem, block of MT time tiles), dealt to the CTAs by descending cost
+  U.p = e.x;
+  const SliceParams* P = sp + U.p;
+  const int d = P->d, log2d = P->log2d, n_taps = P->n_taps;
+  U.L_pad = P->L_pad;
+  const int rows_needed = (d == 1) ? c : (c >> log2d) + 2 * kKUp;
+  const int MT = fir_mt(U.L_pad);
+  U.r0 = e.y * 128 * MT;
+  U.valid = U.r0 < rows_needed;
+  int m = (rows_needed - U.r0 + 127) / 128; U.mt_used = m > MT ? MT : m;
+  U.n_kb = (n_taps + FH_KB - 1) / FH_KB;
+  U.n_chunks = U.mt_used * 128 + U.n_kb * FH_KB;
+  U.b0 = P->jjY0 + (o >> log2d) + U.r0 - n_taps;
+  return U;
+}
+
+__global__ void __launch_bounds__(FP_THREADS, 1)
+fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int o, int c, int n_stages,
+                    const int2* __restrict__ list, int n_units, int hk_bytes, int stage_cap)
+{
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) uint64_t bar_full[FH_MAX_STAGES], bar_empty[FH_MAX_STAGES], hk_full[2], hk_empty[2], acc_full, acc_empty;
+  __shared__ uint32_t tmem_slot;
+  // [2] x { Hankel array (n_chunks x 16 B) | raw fp16 window }, then the U ring
+  uint8_t* sB = smem + 2 * (size_t)hk_bytes;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  if (warp == 0) tmem_alloc(&tmem_slot, 512);
+  if (tid == 32) {
+    for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&bar_full[s]), 1); mbar_init(smem_u32(&bar_empty[s]), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&hk_full[b]), 128); mbar_init(smem_u32(&hk_empty[b]), 1); }
+    mbar_init(smem_u32(&acc_full), 1); mbar_init(smem_u32(&acc_empty), 128);
+    mbar_init_fence();
+  }
+  fence_before();
+  __syncthreads();
+  fence_after();
+  const uint32_t tmem = tmem_slot;
+  const uint32_t bfull = smem_u32(&bar_full[0]), bempty = smem_u32(&bar_empty[0]);
+
+  if (warp >= 6) {
+    // ===== stagers (128 threads): strain window -> raw fp16 -> Hankel core-matrix array, double-buffered =====
+    const int st = tid - 192;
+    int k = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const FirUnit U = fir_unit(sp, list, u, o, c);
+      if (!U.valid) continue;
+      const int b = k & 1;
+      uint8_t* sC = smem + (size_t)b * hk_bytes;
+      uint8_t* sRaw = sC + (size_t)U.n_chunks * 16;
+      if (k >= 2) mbar_wait(smem_u32(&hk_empty[b]), (uint32_t)((k >> 1) - 1) & 1u);     // MMAs that read this buffer are complete
+      const SliceParams* P = sp + U.p;
+      const RateParams* R = rates + P->rate_idx;
+      const int xs_len = R->xs_len;
+      const unsigned short* xg = reinterpret_cast<const unsigned short*>(R->xs16 + (size_t)P->det * xs_len);
+      unsigned short* raw = reinterpret_cast<unsigned short*>(sRaw);
+      for (int i = st; i < U.n_chunks + 8; i += 128) {
+        const int idx = U.b0 + i;
+        raw[i] = (idx >= 0 && idx < xs_len) ? __ldg(xg + idx) : (unsigned short)0;
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      const uint32_t* raw32 = reinterpret_cast<const uint32_t*>(sRaw);
+      for (int ch = st; ch < U.n_chunks; ch += 128) {            // chunk ch = window samples [ch, ch + 8)
+        const int w = ch >> 1;
+        uint32_t a0 = raw32[w], a1 = raw32[w + 1], a2 = raw32[w + 2], a3 = raw32[w + 3];
+        if (ch & 1) {
+          const uint32_t a4 = raw32[w + 4];
+          a0 = __funnelshift_r(a0, a1, 16); a1 = __funnelshift_r(a1, a2, 16);
+          a2 = __funnelshift_r(a2, a3, 16); a3 = __funnelshift_r(a3, a4, 16);
+        }
+        *reinterpret_cast<uint4*>(sC + (size_t)ch * 16) = make_uint4(a0, a1, a2, a3);
+      }
+      fence_async_smem();                                        // generic-proxy writes -> visible to the MMAs (async proxy)
+      mbar_arrive(smem_u32(&hk_full[b]));
+      asm volatile("bar.sync 1, 128;" ::: "memory");             // raw of this buffer may be overwritten two units later only
+      ++k;
+    }
+  } else if (warp == 0) {
+    // ===== producer: one elected thread; the U ring runs on across unit boundaries =====
+    if (elect_one()) {
+      const uint32_t sB_u = smem_u32(sB);
+      int s = 0; uint32_t ph = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const FirUnit U = fir_unit(sp, list, u, o, c);
+        if (!U.valid) continue;
+        const uint8_t* src = reinterpret_cast<const uint8_t*>(sp[U.p].U16);
+        const uint32_t sbytes = (uint32_t)(U.L_pad * FH_KB * 2);
+        for (int kb = 0; kb < U.n_kb; ++kb, src += sbytes) {
+          mbar_wait(bempty + 8u * s, ph ^ 1u);
+          mbar_expect_tx(bfull + 8u * s, sbytes);
+          bulk_g2s(sB_u + (uint32_t)s * (uint32_t)stage_cap, src, sbytes, bfull + 8u * s);
+          if (++s == n_stages) { s = 0; ph ^= 1u; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer: one elected thread =====
+    if (elect_one()) {
+      int s = 0; uint32_t ph = 0;
+      int k = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const FirUnit U = fir_unit(sp, list, u, o, c);
+        if (!U.valid) continue;
+        const int b = k & 1;
+        const int Lp = U.L_pad;
+        const int n_split = (Lp > 256) ? 2 : 1;
+        const int Nmma = Lp / n_split;
+        const uint32_t idesc = idesc_f16(128, Nmma);
+        const uint32_t c_lo = desc_lo(smem_u32(smem + (size_t)b * hk_bytes), 128u);      // Hankel array: LBO = SBO = 128
+        const uint32_t b_lo0 = desc_lo(smem_u32(sB), (uint32_t)(Lp * 16));
+        const uint32_t b_step = (uint32_t)stage_cap >> 4, b_k16 = (uint32_t)(2 * Lp);
+        mbar_wait(smem_u32(&hk_full[b]), (uint32_t)(k >> 1) & 1u);                       // this unit's Hankel array is built
+        if (k >= 1) mbar_wait(smem_u32(&acc_empty), (uint32_t)(k - 1) & 1u);             // the previous unit's accumulators are drained
+        fence_after();
+        for (int kb = 0; kb < U.n_kb; ++kb) {
+          mbar_wait(bfull + 8u * s, ph);
+          fence_after();
+          const uint32_t b_lo = b_lo0 + (uint32_t)s * b_step;
+          for (int mt = 0; mt < U.mt_used; ++mt) {
+            const uint32_t a_lo = c_lo + (uint32_t)(mt * 16 + kb * 8) * 8u;
+            const uint32_t d_t = tmem + (uint32_t)(mt * Lp);
+#pragma unroll
+            for (int k16 = 0; k16 < FH_KB / 16; ++k16) {
+              const uint64_t adesc = desc64(a_lo + (uint32_t)(k16 * 16));
+              for (int h = 0; h < n_split; ++h)
+                mma_ss(d_t + (uint32_t)(h * Nmma), adesc, desc64(b_lo + (uint32_t)k16 * b_k16 + (uint32_t)(h * Nmma)), idesc,
+                       (kb | k16) ? 1u : 0u);
+            }
+          }
+          commit(bempty + 8u * s);                                 // stage reusable once these MMAs have read it
+          if (++s == n_stages) { s = 0; ph ^= 1u; }
+        }
+        commit(smem_u32(&hk_empty[b]));                            // Hankel buffer reusable once every MMA of the unit is complete
+        commit(smem_u32(&acc_full));
+        ++k;
+      }
+    }
+  } else {
+    // ===== epilogue (warps 2-5): TMEM -> fp16 -> Y16[lc][row][8] =====
+    const int q = warp & 3;                                        // TMEM lane quarter this warp may access
+    int k = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const FirUnit U = fir_unit(sp, list, u, o, c);
+      if (!U.valid) continue;
+      const SliceParams* P = sp + U.p;
+      __half* __restrict__ Y = reinterpret_cast<__half*>(P->Y);
+      const int y_rows_cap = P->y_rows_cap;
+      const int L_pad = U.L_pad;
+      const size_t lgs = (size_t)(L_pad >> 3);
+      mbar_wait(smem_u32(&acc_full), (uint32_t)k & 1u);
+      fence_after();
+      for (int mt = 0; mt < U.mt_used; ++mt) {
+        const int row = U.r0 + mt * 128 + q * 32 + lane;
+        __half* __restrict__ Yt = Y + ((size_t)(row >> 7) * lgs * 128 + (row & 127)) * 8;   // Y16[tile][lc][row % 128][8]
+        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
+        for (int c0 = 0; c0 < L_pad; c0 += 32) {
+          uint32_t v[32];
+          tmem_ld32(taddr + c0, v);
+          tmem_ld_wait();
+          if (row < y_rows_cap) {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+              uint32_t h[4];
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * g + 2 * i]), __uint_as_float(v[8 * g + 2 * i + 1]));
+                h[i] = *reinterpret_cast<const uint32_t*>(&p2);
+              }
+              *reinterpret_cast<uint4*>(Yt + ((size_t)(c0 >> 3) + g) * 1024) = make_uint4(h[0], h[1], h[2], h[3]);
+            }
+          }
+        }
+      }
+      fence_before();
+      mbar_arrive(smem_u32(&acc_empty));
+      ++k;
     }
   }
   fence_before();
@@ -204,6 +414,31 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
   pl->fir_stages = stages;
   pl->fir_smem = (int)(fixed + (size_t)stages * stage);
   pl->fir_grid_x = gx;
+  // persistent variant: two Hankel buffers + at least 3 ring stages
+  pl->fir_pers = false;
+  if (2 * fixed + 3 * stage <= budget) {
+    int dev = 0, n_sm = 148;
+    cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) n_sm = 148;
+    pl->fir_n_sm = n_sm;
+    pl->fir_hk_bytes = (int)fixed; pl->fir_stage_cap = (int)stage;
+    pl->fir_pers_stages = std::min<int>(FH_MAX_STAGES, (int)((budget - 2 * fixed) / stage));
+    pl->fir_pers_smem = (int)(2 * fixed + (size_t)pl->fir_pers_stages * stage);
+    size_t cap_units = 0;
+    for (int i = 0; i < n_problems; ++i) {
+      const SliceParams& P = sp_host[i];
+      const int mt = fir_mt_host(P.L_pad);
+      const int rows = (P.d == 1) ? chunk_cap : (chunk_cap >> P.log2d) + 2 * kKUp;
+      cap_units += (size_t)(rows + 128 * mt - 1) / (128 * mt);
+    }
+    bool ok = cudaFuncSetAttribute(fir_f16_pers_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_pers_smem) == cudaSuccess;
+    for (int k = 0; k < 2 && ok; ++k) {
+      void* d = nullptr;
+      ok = cudaMalloc(&d, (cap_units + 1) * sizeof(int2)) == cudaSuccess;
+      if (ok) { pl->owned.push_back(d); pl->fir_list_dev[k] = d; pl->fir_list_c[k] = -1; *bytes += (int64_t)((cap_units + 1) * sizeof(int2)); }
+    }
+    pl->fir_pers = ok;
+  }
   cudaError_t e = cudaFuncSetAttribute(fir_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_smem);
   if (e != cudaSuccess) { snprintf(err, errlen, "cudaFuncSetAttribute(fir_f16_kernel, %d): %s", pl->fir_smem, cudaGetErrorString(e)); delete pl; return nullptr; }
   if (!f16_plan_build_recon(pl, sp_host, n_problems, bp_host, n_bd, chunk_cap, up_w, bytes, err, errlen)) {
@@ -220,9 +455,50 @@ void f16_plan_destroy(F16Plan* p)
   delete p;
 }
 
+// units of one chunk length: sorted by descending cost (taps x tiles), dealt to the CTAs in serpentine order
+static int fir_build_list(F16Plan* pl, const SliceParams* sp_host, int n_problems, int c, int slot, cudaStream_t st)
+{
+  struct Ent { long long cost; int p, r; };
+  std::vector<Ent> ents;
+  for (int i = 0; i < n_problems; ++i) {
+    const SliceParams& P = sp_host[i];
+    const int mt = fir_mt_host(P.L_pad);
+    const int rows = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+    const int nb = (rows + 128 * mt - 1) / (128 * mt);
+    const int n_kb = (P.n_taps + FH_KB - 1) / FH_KB;
+    for (int r = 0; r < nb; ++r) {
+      const int used = std::min(mt, (rows - r * 128 * mt + 127) / 128);
+      ents.push_back(Ent{(long long)n_kb * used * P.L_pad + 40LL * P.L_pad, i, r});
+    }
+  }
+  std::stable_sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) { return a.cost > b.cost; });
+  const int G = std::min<int>(pl->fir_n_sm, (int)ents.size());
+  std::vector<int2>& L = pl->fir_list_host[slot];
+  L.resize(ents.size());
+  const size_t full = ents.size() / G * G;                  // complete rounds are mirrored on odd rounds, the last partial one is not
+  for (size_t i = 0; i < ents.size(); ++i) {
+    const size_t round = i / G, j = i % G;
+    const size_t pos = (i < full && (round & 1)) ? round * G + (G - 1 - j) : i;
+    L[pos] = make_int2(ents[i].p, ents[i].r);
+  }
+  pl->fir_list_c[slot] = c; pl->fir_list_n[slot] = (int)ents.size();
+  return cudaMemcpyAsync(pl->fir_list_dev[slot], L.data(), L.size() * sizeof(int2), cudaMemcpyHostToDevice, st) == cudaSuccess ? 0 : 1;
+}
+
 int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                    const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches)
 {
+  if (pl->fir_pers) {
+    int slot = (c == pl->chunk_cap) ? 0 : 1;
+    if (pl->fir_list_c[slot] != c && fir_build_list(pl, sp_host, n_problems, c, slot, st)) return 1;
+    const int n_units = pl->fir_list_n[slot];
+    const int grid = std::min(pl->fir_n_sm, n_units);
+    fir_f16_pers_kernel<<<grid, FP_THREADS, pl->fir_pers_smem, st>>>(sp_dev, rates_dev, o, c, pl->fir_pers_stages,
+                                                                    (const int2*)pl->fir_list_dev[slot], n_units, pl->fir_hk_bytes,
+                                                                    pl->fir_stage_cap);
+    ++*launches;
+    return cudaGetLastError() == cudaSuccess ? 0 : 1;
+  }
   int gx = 1;
   for (int i = 0; i < n_problems; ++i) {
     const SliceParams& P = sp_host[i];
