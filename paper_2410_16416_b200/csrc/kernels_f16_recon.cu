@@ -2,15 +2,16 @@
 // tcgen05 tensor cores (include/lloid.h A3-A5; "matrix multiplication of the orthogonal SNR time
 // series with SVD coefficients, and finally up-samples and sums the physical SNR segments").
 //
-// Two kernels per chunk, both with the SAME skeleton (warp 0 = bulk-copy producer, warp 1 = single-thread
-// MMA issuer, warps 2-5 = epilogue; a ring of 8 KB operand stages; two TMEM accumulator buffers of
-// 2 x 128 columns so the epilogue of tile t overlaps the MMAs of tile t + 1):
+// Two persistent kernels per chunk (one CTA per SM, static cost-balanced (unit, tile) ranges: SchedArgs), built from
+// the same pieces: single-thread producer / MMA-issuer roles inside `if (elect_one())`, rings of 8 KB operand stages
+// filled by 1-D bulk copies, two TMEM accumulator buffers of 2 x 128 columns so the epilogue of tile t overlaps the
+// MMAs of tile t + 1:
 //
 //  lowrate_recon_kernel   rho^(d)[i, j] = sum_{slices s at rate d} sum_l R^s[i, l] y^s_l[j]     (d > 1)
-//      A = R^s (stationary in shared memory for the CTA's 128 templates), B = y^s tiles streamed from L2,
-//      D[lane = template, column = low-rate time].  Slices that share a rate are summed BEFORE upsampling
-//      (A4 is linear and its kernel depends only on d).  Output Q16: fp16 at the LOW rate, already in the
-//      core-matrix layout in which the f0 kernel consumes it as an MMA operand.  The dense f0-rate SNR is
+//      A = R^s (stationary in shared memory for the CTA's 128 templates), B = y^s tiles streamed by two alternating
+//      producer threads, D[lane = template, column = low-rate time].  Slices that share a rate are summed BEFORE
+//      upsampling (A4 is linear and its kernel depends only on d).  Output Q16: fp16 at the LOW rate, already in
+//      the core-matrix layout in which the f0 kernel consumes it as an MMA operand.  The dense f0-rate SNR is
 //      never written anywhere.
 //
 //  f0_kernel   rho[i, k] = sum_{d = 1 slices} R^s y^s  +  sum_{d > 1} rho^(d)[i, window(k)] P_d      then A5
@@ -18,11 +19,12 @@
 //      P_d[r, kl] = d lp_{d,K_up}[...] (16 non-zeros per column), restricted per 16-row chunk to the output
 //      columns its band touches.  Cosine and sine rows of a template go to two accumulators (columns
 //      [0,128) and [128,256)) of the SAME TMEM lane, so one epilogue thread owns one template: |rho|^2 and
-//      the running maximum over time need no cross-lane traffic at all.
+//      the running maximum over time need no cross-lane traffic at all.  Five single-thread roles on two rings
+//      (see the comment above f0_kernel).
 //
-// The producer and the MMA issuer are single threads: their per-stage instruction count is what bounds the
-// pipeline once the data is in L2, so both loops are written with incrementing ring / pointer / descriptor
-// state (no division, no 64-bit descriptor rebuild, per-CTA lookup tables in shared memory).
+// A single thread retires about one instruction per 7 cycles: per-stage instruction counts of the role loops are
+// what bounds the pipeline once the data is there, so the loops carry incrementing ring / pointer / descriptor
+// state (no division, no 64-bit descriptor rebuild) and read per-unit tables from shared memory.
 #include "f16_plan.h"
 #include "tc05.cuh"
 
@@ -35,7 +37,6 @@ namespace lloid {
 
 using namespace tc;
 
-constexpr int RC16_THREADS = 192;
 constexpr int RC16_STAGE = 8192;            // bytes per ring stage: one K = 32 (y) or K = 16 (rho^(d)) operand chunk
 constexpr int RC16_MAX_STAGES = 16;
 constexpr int RC16_SMEM_BUDGET = 220 * 1024;
