@@ -191,3 +191,48 @@ def test_config2_geometry_excerpt(precision):
     hit = trigs[(trigs["detector"] == 1) & (trigs["template_idx"] == inj.template) & (np.abs(trigs["sample"] - inj.end) <= 2)]
     assert len(hit) == 1
     assert stats["triggers"] > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases: other decimation half-widths (odd K_dn runs the generic resampler), degenerate banks,
+# minimal buffers, count-only calls
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("precision", PRECISIONS)
+@pytest.mark.parametrize("k_down", [7, 8, 24])
+def test_other_decimation_half_widths(k_down, precision):
+    w = wl.toy(n_templates=6, M=4096, spans=((2048, 0.0, 0.25), (512, 0.25, 1.0), (128, 1.0, 2.0)), seconds=6.0,
+               n_basis=[10, 12, 9], f_low=25.0, mc=(1.2, 1.3))
+    w.k_down = k_down
+    w.peak_window = 512
+    _, _, _, _, stats = _dense_check(w, precision, 0, w.n_samples)
+    assert stats["checked"] == 6 * (w.n_samples // 512)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_single_template_single_basis_vector(precision):
+    w = wl.toy(n_templates=1, M=512, spans=((2048, 0.0, 0.125), (1024, 0.125, 0.25)), seconds=2.0, n_basis=[1, 1], f_low=40.0)
+    w.peak_window = 256
+    w.threshold = 1.0
+    _, _, _, info, stats = _dense_check(w, precision, 0, w.n_samples)
+    assert stats["checked"] == w.n_samples // 256 and stats["triggers"] > 0
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_minimal_buffers_and_count_only_calls(cfg1, precision):
+    """Buffers of exactly the largest decimation factor (4 samples here) for a stretch of the stream, and a call
+    with capacity 0 / no trigger buffer: the count is still exact and overflow is reported by lloid_check_count."""
+    import torch
+    w = cfg1
+    n = w.n_samples
+    one, _, _ = pu.run_gpu(w, precision)
+    pieces = [8192] + [4] * 64 + [n - 8192 - 256]
+    many, _, info = pu.run_gpu(w, precision, pieces=pieces)
+    assert _as_set(one) == _as_set(many) and info["consumed"] == n
+    bank = lb.Bank(w, precision)
+    strain = torch.from_numpy(w.strain).cuda()
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    lb.lloid_filter(bank.handle, strain.data_ptr(), n, 0, 0, cnt.data_ptr())
+    torch.cuda.synchronize()
+    assert int(cnt.item()) == len(one)
+    assert lb.lloid_check_count(int(cnt.item()), 0) == lb.LLOID_EOVERFLOW
+    bank.close()
