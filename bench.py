@@ -70,7 +70,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -89,9 +89,17 @@ class ClockSampler:
             except Exception:
                 self.proc.kill()
 
+    def mark_begin(self):
+        self.i0 = len(self.rows)
+
+    def mark_end(self):
+        time.sleep(0.06)                       # let the sample that covers the end of the region arrive
+        self.i1 = len(self.rows)
+
     def summary(self):
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        rows = self.rows[getattr(self, "i0", 0):getattr(self, "i1", len(self.rows))] or self.rows
+        for r in rows:
             try:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except Exception:
@@ -201,13 +209,13 @@ def run_ours(args):
         bank.filter(strain_dev, trig_dev, cnt_dev, stream)
 
     # ---- device-resident throughput -----------------------------------------------------------
-    for _ in range(args.warmup):
-        step_device()
-    barrier()
     launches = 0
     times = []
-    with ClockSampler(local) as clocks:
+    with ClockSampler(local) as clocks:          # started before the warm-up: nvidia-smi needs a moment to come up
+        for _ in range(args.warmup):
+            step_device()
         barrier()
+        clocks.mark_begin()
         for _ in range(args.steps):
             flush.zero_()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -218,6 +226,7 @@ def run_ours(args):
             times.append(e0.elapsed_time(e1))
             launches += lb.lloid_last_launch_count(bank.handle)
         barrier()
+        clocks.mark_end()
     n_trig = int(cnt_dev.item())
     t_dev = torch.tensor([sum(times)], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -372,7 +381,7 @@ def run_stream(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--precision", default="f16", choices=["f16", "f32"])
