@@ -273,6 +273,9 @@ def run_ours(args):
         # A1 resampler against HBM: bytes = read x (4 B) + write every rate stream (fp32 + fp16) per f0 sample
         rates = sorted({s.d for b in w.bins for s in b.slices})
         res_bytes = samples * (4.0 + sum((6.0 / d) if d > 1 else 2.0 for d in rates))
+        merge_bytes = (n / 128.0) * n_templates * D * 16.0          # one 16-byte partial peak per template and 128-sample tile
+        roofline["merge_hbm"] = {"achieved": merge_bytes / (stage[3] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                                 "frac": merge_bytes / (stage[3] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[3]}
         roofline["resample_hbm"] = {"achieved": res_bytes / (stage[0] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
                                     "frac": res_bytes / (stage[0] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[0]}
     else:

@@ -228,10 +228,15 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
   else { s.q = -1.f; s.re = 0.f; s.im = 0.f; s.pad = 0; s.k = -1; }
   const int g0 = (int)((lo - k_a) / kTimeTile), g1 = (int)((hi - k_a + kTimeTile - 1) / kTimeTile);
   const Peak* __restrict__ pp = partials + ((size_t)bd * tiles_cap + g0) * max_templates + p;
-#pragma unroll 4
-  for (int g = g0; g < g1; ++g, pp += max_templates) {
-    const Peak pk = *pp;
-    if (pk.q > s.q) { s.q = pk.q; s.re = pk.re; s.im = pk.im; s.k = k_a + pk.kappa; }
+  for (int g = g0; g < g1; g += 8) {               // 8 independent 16-byte loads in flight per thread, then the ordered compare
+    float4 v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      v[i] = (g + i < g1) ? __ldcs(reinterpret_cast<const float4*>(pp + (size_t)i * max_templates)) : make_float4(-2.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)                     // Peak = {q, kappa, re, im}
+      if (v[i].x > s.q) { s.q = v[i].x; s.re = v[i].z; s.im = v[i].w; s.k = k_a + __float_as_int(v[i].y); }
+    pp += (size_t)8 * max_templates;
   }
   const bool complete = (w + 1) * W <= k_a + c;
   if (complete && s.q >= 0.f && sqrtf(s.q) > theta) {
