@@ -4,6 +4,8 @@
 // The fp16 tensor-core path lives in kernels_f16.cu.
 #include "lloid_internal.h"
 
+#include <algorithm>
+
 namespace lloid {
 
 // ------------------------------------------------------------------------------------------------
@@ -361,6 +363,235 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
   else
     recon_f32_kernel<false><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, partials, tiles_cap, max_templates,
                                                     c, (long long)k_a, cap);
+  ++*launches;
+}
+
+// ------------------------------------------------------------------------------------------------
+// A3 at the low rates, once per chunk:  Q[i, r] = sum_{slices s of the group} sum_l R^s[i, l] Y^s[r, l]
+// (Y row r <-> low-rate index r - K_up, lloid_internal.h).  Plain register-tiled SGEMM "NT": CTA tile 128 rows x 128
+// low-rate columns, 256 threads, 8 x 8 per thread, K chunks of 16 staged transposed in shared memory.  The fused
+// f0 kernel used to recompute these products for every 128-sample tile with its 2 K_up halo (8x redundant at d = 32).
+// ------------------------------------------------------------------------------------------------
+constexpr int LG_T = 128, LG_K = 16, LG_S = LG_T + 4;
+
+__global__ void __launch_bounds__(256)
+lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __restrict__ groups, int c)
+{
+  const Q32Group G = groups[blockIdx.z];
+  if (G.n_slices == 0) return;
+  const int cols_needed = (c >> G.log2d) + 2 * kKUp;
+  const int j0 = blockIdx.x * LG_T, row0 = blockIdx.y * LG_T;
+  if (j0 >= cols_needed || row0 >= G.rows_pad) return;
+
+  __shared__ __align__(16) float As[LG_K][LG_S], Bs[LG_K][LG_S];
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  const int lr = tid >> 1, lk = (tid & 1) * 8;          // this thread stages row lr, k = lk .. lk + 7 of both tiles
+  float acc[8][8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i)
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+
+  for (int s = 0; s < G.n_slices; ++s) {
+    const SliceParams P = sp[G.slice[s]];
+    const float* __restrict__ R = P.R32 + (size_t)(row0 + lr) * P.L_pad + lk;
+    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)(j0 + lr) * P.L_pad + lk;
+    const bool y_ok = j0 + lr < P.y_rows_cap;
+    for (int l0 = 0; l0 < P.L_pad; l0 += LG_K) {
+      const float4 a0 = __ldg(reinterpret_cast<const float4*>(R + l0)), a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + 4));
+      float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+      if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0); b1 = *reinterpret_cast<const float4*>(Y + l0 + 4); }
+      __syncthreads();
+      As[lk + 0][lr] = a0.x; As[lk + 1][lr] = a0.y; As[lk + 2][lr] = a0.z; As[lk + 3][lr] = a0.w;
+      As[lk + 4][lr] = a1.x; As[lk + 5][lr] = a1.y; As[lk + 6][lr] = a1.z; As[lk + 7][lr] = a1.w;
+      Bs[lk + 0][lr] = b0.x; Bs[lk + 1][lr] = b0.y; Bs[lk + 2][lr] = b0.z; Bs[lk + 3][lr] = b0.w;
+      Bs[lk + 4][lr] = b1.x; Bs[lk + 5][lr] = b1.y; Bs[lk + 6][lr] = b1.z; Bs[lk + 7][lr] = b1.w;
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < LG_K; ++k) {
+        const float4 av0 = *reinterpret_cast<const float4*>(&As[k][ty * 8]), av1 = *reinterpret_cast<const float4*>(&As[k][ty * 8 + 4]);
+        const float4 bv0 = *reinterpret_cast<const float4*>(&Bs[k][tx * 8]), bv1 = *reinterpret_cast<const float4*>(&Bs[k][tx * 8 + 4]);
+        const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
+        const float b[8] = {bv0.x, bv0.y, bv0.z, bv0.w, bv1.x, bv1.y, bv1.z, bv1.w};
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    float* q = G.Q + (size_t)(row0 + ty * 8 + i) * G.q_cols + j0 + tx * 8;
+    *reinterpret_cast<float4*>(q) = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
+    *reinterpret_cast<float4*>(q + 4) = make_float4(acc[i][4], acc[i][5], acc[i][6], acc[i][7]);
+  }
+}
+
+void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_dev, const Q32Group* groups_host, int n_groups,
+                             int max_rows_pad, int c, cudaStream_t st, int64_t* launches)
+{
+  int max_cols = 0;
+  for (int g = 0; g < n_groups; ++g)
+    if (groups_host[g].n_slices) max_cols = std::max(max_cols, (c >> groups_host[g].log2d) + 2 * kKUp);
+  if (max_cols == 0) return;
+  dim3 grid((max_cols + LG_T - 1) / LG_T, (max_rows_pad + LG_T - 1) / LG_T, n_groups);
+  lowrate_gemm_f32_kernel<<<grid, 256, 0, st>>>(sp_dev, groups_dev, c);
+  ++*launches;
+}
+
+// ------------------------------------------------------------------------------------------------
+// fp32 path, second kernel: A3 of the d = 1 slices + A4 + A5 fused as in recon_f32_kernel, but the low-rate
+// rho^(d) come precomputed from lowrate_gemm_f32_kernel: per rate the CTA stages a [64 rows x (128/d + 2 K_up)]
+// window of Q and interpolates it into its register accumulators.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict__ bp,
+                   const float* const* __restrict__ upw, const Q32Group* __restrict__ groups,
+                   Peak* __restrict__ partials, int tiles_cap, int max_templates, int c, long long k_a, Capture cap)
+{
+  const int bd = blockIdx.z;
+  const BinParams B = bp[bd];
+  const int row0 = blockIdx.y * RC_RT;
+  if (row0 >= 2 * B.n_templates) return;
+  const int g = blockIdx.x;
+  const int kap0 = g * RC_CT;
+
+  extern __shared__ __align__(16) float smem_r[];
+  float* Rs = smem_r;                               // [RC_KC][RC_RS]
+  float* Ys = Rs + RC_KC * RC_RS;                   // [RC_KC][RC_YS]
+  float* rho = Ys + RC_KC * RC_YS;                  // [RC_RT][RC_RHO_S]
+  float* wsm = rho + RC_RT * RC_RHO_S;              // [16][32]
+
+  const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+  float acc[4][8];
+#pragma unroll
+  for (int r = 0; r < 4; ++r)
+#pragma unroll
+    for (int cc = 0; cc < 8; ++cc) acc[r][cc] = 0.f;
+
+  // ---- d = 1 slices: K-chunked SGEMM straight into the accumulators
+  for (int s = 0; s < B.n_slices; ++s) {
+    const SliceParams P = sp[B.first_slice + s];
+    if (P.d != 1) continue;
+    const float* __restrict__ R = P.R32;
+    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y);
+    const int Lp = P.L_pad;
+    for (int l0 = 0; l0 < Lp; l0 += RC_KC) {
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
+        const int e = tid + 256 * i;
+        const int ll = e % RC_KC, row = e / RC_KC;
+        Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
+      }
+      for (int e = tid; e < RC_CT * RC_KC; e += 256) {
+        const int ll = e % RC_KC, col = e / RC_KC;
+        const int r = kap0 + col;
+        Ys[ll * RC_YS + col] = (r < P.y_rows_cap) ? Y[(size_t)r * Lp + l0 + ll] : 0.f;
+      }
+      __syncthreads();
+#pragma unroll 8
+      for (int ll = 0; ll < RC_KC; ++ll) {
+        const float4 a = *reinterpret_cast<const float4*>(Rs + ll * RC_RS + 4 * ty);
+        const float4 b0 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx);
+        const float4 b1 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx + 4);
+        const float av[4] = {a.x, a.y, a.z, a.w};
+        const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int cc = 0; cc < 8; ++cc) acc[r][cc] = fmaf(av[r], bv[cc], acc[r][cc]);
+      }
+    }
+  }
+
+  // ---- low rates: window of the precomputed rho^(d), interpolated (A4)
+  for (int l2 = 1; l2 < kMaxRates; ++l2) {
+    const Q32Group* G = groups + (size_t)bd * kNLowRates + (l2 - 1);
+    if (G->n_slices == 0) continue;
+    const int d = 1 << l2;
+    const int Ks = (RC_CT >> l2) + 2 * kKUp;
+    const int r0 = kap0 >> l2;
+    const float* __restrict__ Q = G->Q;
+    const int qc = G->q_cols;
+    __syncthreads();                                 // previous readers of rho / wsm are done
+    {
+      const float* __restrict__ w = upw[l2];         // [16][d]
+      for (int e = tid; e < 16 * d; e += 256) wsm[(e / d) * 32 + (e % d)] = __ldg(w + e);
+    }
+    for (int e = tid; e < RC_RT * Ks; e += 256) {
+      const int col = e % Ks, row = e / Ks;
+      rho[row * RC_RHO_S + col] = (r0 + col < qc) ? Q[(size_t)(row0 + row) * qc + r0 + col] : 0.f;
+    }
+    __syncthreads();
+    switch (d) {
+      case 2: upsample_acc<2>(acc, rho, wsm, ty, tx); break;
+      case 4: upsample_acc<4>(acc, rho, wsm, ty, tx); break;
+      case 8: upsample_acc<8>(acc, rho, wsm, ty, tx); break;
+      case 16: upsample_acc<16>(acc, rho, wsm, ty, tx); break;
+      default: upsample_acc<32>(acc, rho, wsm, ty, tx); break;
+    }
+  }
+
+  // ---- epilogue: |rho|^2, first maximum over the tile's valid columns, one Peak per template
+  const int valid = min(RC_CT, c - kap0);           // ragged last tile of a chunk
+#pragma unroll
+  for (int t = 0; t < 2; ++t) {
+    float bq = -1.f, bre = 0.f, bim = 0.f;
+    int bk = 0x7fffffff;
+#pragma unroll
+    for (int cc = 0; cc < 8; ++cc) {
+      const int kl = 8 * tx + cc;
+      const float re = acc[2 * t][cc], im = acc[2 * t + 1][cc];
+      const float q = re * re + im * im;
+      if (kl < valid && q > bq) { bq = q; bre = re; bim = im; bk = kap0 + kl; }
+    }
+#pragma unroll
+    for (int off = 8; off >= 1; off >>= 1) {
+      const float oq = __shfl_xor_sync(0xffffffffu, bq, off);
+      const float ore = __shfl_xor_sync(0xffffffffu, bre, off);
+      const float oim = __shfl_xor_sync(0xffffffffu, bim, off);
+      const int ok = __shfl_xor_sync(0xffffffffu, bk, off);
+      if (oq > bq || (oq == bq && ok < bk)) { bq = oq; bre = ore; bim = oim; bk = ok; }
+    }
+    const int p = (row0 + 4 * ty) / 2 + t;
+    if (tx == 0 && p < B.n_templates) {
+      Peak pk; pk.q = bq; pk.kappa = bk; pk.re = bre; pk.im = bim;
+      partials[((size_t)bd * tiles_cap + g) * max_templates + p] = pk;
+    }
+  }
+
+  if (cap.snr != nullptr && cap.bd == bd) {         // test-only dense dump from the same accumulators
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int row = row0 + 4 * ty + r;
+      if (row >= cap.rows) continue;
+#pragma unroll
+      for (int cc = 0; cc < 8; ++cc) {
+        const int kl = 8 * tx + cc;
+        const long long k = k_a + kap0 + kl;
+        if (kl < valid && k >= cap.k_begin && k < cap.k_begin + cap.n)
+          cap.snr[(size_t)row * cap.n + (k - cap.k_begin)] = acc[r][cc];
+      }
+    }
+  }
+}
+
+void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int n_bd, int max_rows_pad,
+                        const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
+                        int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
+{
+  const size_t smem = sizeof(float) * (RC_KC * RC_RS + RC_KC * RC_YS + RC_RT * RC_RHO_S + 16 * 32);
+  static bool configured = false;
+  if (!configured) {
+    cudaFuncSetAttribute(recon_f32_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configured = true;
+  }
+  const int n_tiles = (c + RC_CT - 1) / RC_CT;
+  dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
+  recon_f32_q_kernel<<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
+                                             c, (long long)k_a, cap);
   ++*launches;
 }
 

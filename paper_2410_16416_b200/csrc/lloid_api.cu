@@ -87,6 +87,8 @@ struct lloid_bank {
   bool prof = false;
   std::vector<cudaEvent_t> events; std::vector<int> event_tag; size_t events_used = 0;
   F16Plan* plan16 = nullptr;
+  std::vector<Q32Group> q32_host;          // fp32 path: [n_bd][kNLowRates]
+  Q32Group* q32_dev = nullptr;
 
   int slice_index(int bin, int det, int s) const { return bp_host[bin * cfg.n_detectors + det].first_slice + s; }
 };
@@ -212,8 +214,16 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
   if (!b->f16) {
     launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, o, c, st, &b->last_launches);
     mark(b, st, kTagFir);
-    launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
-                     b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
+    if (b->q32_dev) {
+      launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, st,
+                              &b->last_launches);
+      mark(b, st, kTagLowRecon);
+      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+                         b->max_templates, c, k_a, b->cap, st, &b->last_launches);
+    } else {
+      launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
+                       b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
+    }
   } else {
     if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, o, c, st, &b->last_launches))
       return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -514,6 +524,31 @@ int lloid_bank_finalize(lloid_bank_t* b)
   launch_reset_state(b->state, 2 * (int64_t)nstate, 0);
   CU(cudaDeviceSynchronize());
 
+  if (!b->f16) {
+    // fp32 path: one rho^(d) buffer per (bin, detector, low rate), filled by lowrate_gemm_f32_kernel every chunk
+    b->q32_host.assign((size_t)b->n_bd * kNLowRates, Q32Group());
+    bool any = false, fits = true;
+    for (int bd = 0; bd < b->n_bd; ++bd) {
+      const BinParams& BP = b->bp_host[bd];
+      for (int l2 = 1; l2 < kMaxRates; ++l2) {
+        Q32Group& G = b->q32_host[(size_t)bd * kNLowRates + (l2 - 1)];
+        memset(&G, 0, sizeof G);
+        G.log2d = l2; G.rows_pad = BP.rows_pad; G.q_cols = (int)round_up((C >> l2) + 2 * Ku, 128);
+        for (int s = 0; s < BP.n_slices; ++s)
+          if (b->sp_host[BP.first_slice + s].log2d == l2) {
+            if (G.n_slices == kMaxGroupSlices) { fits = false; break; }
+            G.slice[G.n_slices++] = BP.first_slice + s;
+          }
+        if (G.n_slices) any = true;
+      }
+    }
+    if (any && fits) {
+      for (Q32Group& G : b->q32_host)
+        if (G.n_slices) { rc = dev_alloc(b, (void**)&G.Q, (size_t)G.rows_pad * G.q_cols * 4, true); if (rc) return rc; }
+      rc = dev_alloc(b, (void**)&b->q32_dev, b->q32_host.size() * sizeof(Q32Group), false); if (rc) return rc;
+      CU(cudaMemcpy(b->q32_dev, b->q32_host.data(), b->q32_host.size() * sizeof(Q32Group), cudaMemcpyHostToDevice));
+    }
+  }
   if (b->f16) {
     char err[256] = {0};
     const double* up_w[kMaxRates];

@@ -66,6 +66,15 @@ struct Capture {                   // lloid_debug_capture
   float*  snr; int64_t k_begin, n; int32_t bd; int32_t rows;
 };
 
+// fp32 path: rho^(d) = sum over the slices of one (bin, detector) at rate d of R^s y^s, computed ONCE per chunk at the
+// low rate (the fused f0 kernel then only interpolates it), fp32 row-major [rows_pad][q_cols]
+struct Q32Group {
+  int32_t n_slices;                // 0: no slice at this rate
+  int32_t slice[kMaxGroupSlices];  // indices into the SliceParams table
+  int32_t log2d, q_cols, rows_pad;
+  float*  Q;
+};
+
 // ---- launchers (one translation unit per kernel family) ---------------------------------------
 void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
                      const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
@@ -83,6 +92,13 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
                       cudaStream_t st, int64_t* launches);
 
 // A5/A6: one thread per (bin, detector, template, peak window touched by the chunk); state double-buffered
+// fp32 path, two kernels: low-rate reconstruction GEMM, then d = 1 reconstruction + interpolation + peaks
+void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_dev, const Q32Group* groups_host, int n_groups,
+                             int max_rows_pad, int c, cudaStream_t st, int64_t* launches);
+void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int n_bd, int max_rows_pad,
+                        const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
+                        int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches);
+
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
                           int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
                           PeakState* state_out, int n_det, void* triggers, int64_t capacity,
