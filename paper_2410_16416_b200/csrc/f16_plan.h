@@ -7,6 +7,8 @@
 
 namespace lloid {
 
+struct LowGeom { int32_t r_bytes[kNLowRates], n_stages[kNLowRates]; };   // low-rate kernel, per rate class: bytes of the stationary R, ring stages
+
 struct F16Plan {
   // A2 basis FIR
   int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
@@ -21,6 +23,7 @@ struct F16Plan {
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
+  LowGeom low_geom{};
   int f0_smem = 0, f0_stages = 0, f0_r_bufs = 1;
   int p_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;
   UpRate up[kNLowRates];

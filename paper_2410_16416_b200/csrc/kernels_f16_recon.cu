@@ -159,10 +159,11 @@ constexpr int LOW_THREADS = 352;             // warps: 0 producer A (+R), 1 MMA 
 
 __global__ void __launch_bounds__(LOW_THREADS, 1)
 lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
-                     const LowUnit* __restrict__ units, const __grid_constant__ SchedArgs sched, int r_bytes, int n_stages)
+                     const LowUnit* __restrict__ units, const __grid_constant__ SchedArgs sched, const __grid_constant__ LowGeom geom)
 {
   extern __shared__ __align__(1024) uint8_t smem[];
   __shared__ __align__(8) RingBars bars;
+  __shared__ __align__(8) uint64_t cfull[kNLowRates][RC16_MAX_STAGES], cempty[kNLowRates][RC16_MAX_STAGES], class_go[kNLowRates];
   __shared__ uint32_t tmem_slot;
   __shared__ SegLow seg[3];                             // [0], [2] the producers', [1] MMA issuer's
   __shared__ int s_rng[4];
@@ -173,14 +174,19 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
   const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
   if (u_lo == u_hi && t_lo == t_hi) return;
 
-  ring_setup(bars, &tmem_slot, n_stages, warp, tid, 256);
+  ring_setup(bars, &tmem_slot, 0, warp, tid, 256);
+  if (tid == 64) {                                      // one ring barrier set per rate class: a CTA visits a class once, and the
+    for (int cidx = 0; cidx < kNLowRates; ++cidx) {     // ring geometry (R size, stage count) differs between classes
+      for (int st = 0; st < RC16_MAX_STAGES; ++st) { mbar_init(smem_u32(&cfull[cidx][st]), 1); mbar_init(smem_u32(&cempty[cidx][st]), 1); }
+      mbar_init(smem_u32(&class_go[cidx]), 1);
+    }
+    mbar_init_fence();
+  }
   fence_before();
   __syncthreads();
   fence_after();
   const uint32_t tmem = tmem_slot;
-  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]);
-  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16
-  const uint32_t ring_u = sR_u + (uint32_t)r_bytes;
+  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16, then the class's ring
 
   if (warp == 0 || warp == 6) {
     // ===== producers: two elected threads fill alternate stages of the ring (one thread sustains ~1 instruction per
@@ -188,9 +194,10 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     if (elect_one()) {
     const int pr = warp == 0 ? 0 : 1;
     SegLow& sg = seg[2 * pr];
-    Ring rg{0, 0u, n_stages};
+    Ring rg{0, 0u, 1};
     int own = pr == 0;
-    int seg_i = 0;                                      // segments done so far by this CTA
+    int seg_i = 0, cur_cls = -1;                        // segments done so far by this CTA
+    uint32_t bfull = 0, bempty = 0, ring_u = 0;
     for (int u = u_lo; u <= u_hi; ++u) {
       if (u == u_hi && t_hi == 0) break;
       const int cls = sched_class(sched, u);
@@ -201,12 +208,22 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       seg_low_fill(sg, sp, G, un.rb);
       const int ns_u = G->n_slices;
       const uint32_t rbytes_u = (uint32_t)G->l_sum * 512u;
-      int countdown = (seg_i == 0) ? 0 : n_stages;      // ring stages to push before R is replaced
+      const bool new_cls = cls != cur_cls;
+      if (new_cls) {                                    // other ring geometry: start its ring (and its barrier set) afresh
+        cur_cls = cls;
+        rg = Ring{0, 0u, geom.n_stages[cls]}; own = pr == 0;
+        bfull = smem_u32(&cfull[cls][0]); bempty = smem_u32(&cempty[cls][0]); ring_u = sR_u + (uint32_t)geom.r_bytes[cls];
+        // the new ring overlaps the old R / ring: nothing may be written before the previous unit is complete
+        if (pr != 0 && seg_i > 0) mbar_wait(smem_u32(&class_go[cls]), 0u);
+      }
+      const int n_stages = geom.n_stages[cls];
+      int countdown = (seg_i == 0 || new_cls) ? 0 : n_stages;      // ring stages to push before R is replaced
       bool r_done = pr != 0;
       auto load_R = [&]() {
         // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
         // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
         if (seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(seg_i - 1) & 1u);
+        if (new_cls && seg_i > 0) mbar_arrive(smem_u32(&class_go[cls]));      // producer B may start on the new ring
         {
           mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
           uint32_t off = 0;
@@ -236,9 +253,11 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
     // ===== MMA issuer: one elected thread =====
     if (elect_one()) {
     const uint32_t idesc = idesc_f16(128, 128);
-    const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
+    const uint32_t a_base = desc_lo(sR_u, 4096u);
     const uint32_t tm = tmem;
-    Ring rg{0, 0u, n_stages};
+    Ring rg{0, 0u, 1};
+    int cur_cls = -1;
+    uint32_t bfull = 0, bempty = 0, b_base = 0;
     uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
     int buf = 0, seg_i = 0;
     for (int u = u_lo; u <= u_hi; ++u) {
@@ -250,6 +269,12 @@ lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __rest
       const RateGroup* G = groups + un.group;
       seg_low_fill(seg[1], sp, G, un.rb);
       const int ns_u = G->n_slices;
+      if (cls != cur_cls) {
+        cur_cls = cls;
+        rg = Ring{0, 0u, geom.n_stages[cls]};
+        bfull = smem_u32(&cfull[cls][0]); bempty = smem_u32(&cempty[cls][0]);
+        b_base = desc_lo(sR_u + (uint32_t)geom.r_bytes[cls], 2048u);
+      }
       mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
       fence_after();
       for (int t = t0; t < t1; ++t, buf ^= 1) {
@@ -804,6 +829,13 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   if (f0_fixed > RC16_SMEM_BUDGET || low_fixed > RC16_SMEM_BUDGET || pl->f0_stages < 4 || (pl->n_lr > 0 && pl->low_stages < 4)) return true;
   pl->f0_smem = f0_fixed + pl->f0_stages * RC16_STAGE;
   pl->low_smem = low_fixed + pl->low_stages * RC16_STAGE;
+  for (int r = 0; r < pl->n_lr; ++r) {                     // per rate class: R as large as its largest group, the rest is ring
+    int lmax = 0;
+    for (int b = 0; b < n_bd; ++b) lmax = std::max(lmax, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
+    pl->low_geom.r_bytes[r] = lmax * 512;
+    pl->low_geom.n_stages[r] = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - lmax * 512) / RC16_STAGE);
+    pl->low_smem = std::max(pl->low_smem, lmax * 512 + pl->low_geom.n_stages[r] * RC16_STAGE);
+  }
 
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
@@ -876,7 +908,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     }
     const int grid = (int)std::min<long long>(pl->n_sm, tiles_total);
     lowrate_recon_kernel<<<grid, LOW_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
-                                                                  sc, pl->l_sum_low_max * 512, pl->low_stages);
+                                                                  sc, pl->low_geom);
     ++*launches;
   }
   if (after_lowrate) cudaEventRecord(after_lowrate, st);
