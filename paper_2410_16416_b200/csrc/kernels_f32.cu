@@ -128,13 +128,13 @@ constexpr int RC_RT = 64, RC_CT = kTimeTile, RC_KC = 32, RC_RS = RC_RT + 4, RC_Y
 constexpr int RC_KSMAX = RC_CT / 2 + 2 * kKUp;   // 80 low-rate samples at d = 2
 constexpr int RC_RHO_S = RC_KSMAX + 1;
 
-template <int D>
-__device__ __forceinline__ void upsample_acc(float (&acc)[4][8], const float* __restrict__ rho,
+template <int D, int NR>
+__device__ __forceinline__ void upsample_acc(float (&acc)[NR][8], const float* __restrict__ rho,
                                              const float* __restrict__ wsm, int ty, int tx)
 {
-  // columns kl = 8 tx + cc;  low-rate local index ml = kl / D, phase phi = kl % D
+  // thread tile: rows NR ty + r, columns kl = 8 tx + cc;  low-rate local index ml = kl / D, phase phi = kl % D
   // c[kl] += sum_{i=-8}^{7} wsm[(i+8)*32 + phi] * rho[row][ml + 8 - i]
-  if (D >= 8) {
+  if constexpr (D >= 8) {
     const int ml = (8 * tx) / D;
     const int phi0 = (8 * tx) % D;
 #pragma unroll
@@ -142,8 +142,8 @@ __device__ __forceinline__ void upsample_acc(float (&acc)[4][8], const float* __
       const float4 w0 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0);
       const float4 w1 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0 + 4);
 #pragma unroll
-      for (int r = 0; r < 4; ++r) {
-        const float v = rho[(4 * ty + r) * RC_RHO_S + ml + kKUp - i];
+      for (int r = 0; r < NR; ++r) {
+        const float v = rho[(NR * ty + r) * RC_RHO_S + ml + kKUp - i];
         acc[r][0] = fmaf(w0.x, v, acc[r][0]); acc[r][1] = fmaf(w0.y, v, acc[r][1]);
         acc[r][2] = fmaf(w0.z, v, acc[r][2]); acc[r][3] = fmaf(w0.w, v, acc[r][3]);
         acc[r][4] = fmaf(w1.x, v, acc[r][4]); acc[r][5] = fmaf(w1.y, v, acc[r][5]);
@@ -151,21 +151,32 @@ __device__ __forceinline__ void upsample_acc(float (&acc)[4][8], const float* __
       }
     }
   } else {
+    // d = 2, 4: groups of TG taps whose TG x D weights stay in registers; per row the NM + TG - 1 low-rate samples
+    // the group touches are read once (the straightforward loop reads one sample per D multiply-adds)
     constexpr int NM = 8 / D;                     // distinct low-rate indices under the 8 columns
+    constexpr int TG = 16 / D;
+    constexpr int NV = NM + TG - 1;
     const int ml0 = (8 * tx) / D;
 #pragma unroll
-    for (int i = -kKUp; i < kKUp; ++i) {
-      float w[D];
+    for (int g = 0; g < 2 * kKUp / TG; ++g) {     // taps i = -K_up + g TG + t
+      float w[TG][D];
 #pragma unroll
-      for (int p = 0; p < D; ++p) w[p] = wsm[(i + kKUp) * 32 + p];
+      for (int t = 0; t < TG; ++t)
 #pragma unroll
-      for (int r = 0; r < 4; ++r) {
+        for (int p = 0; p < D; ++p) w[t][p] = wsm[(g * TG + t) * 32 + p];
 #pragma unroll
-        for (int m = 0; m < NM; ++m) {
-          const float v = rho[(4 * ty + r) * RC_RHO_S + ml0 + m + kKUp - i];
+      for (int r = 0; r < NR; ++r) {
+        // sample index ml0 + m + K_up - i = (ml0 + 2 K_up - g TG - (TG - 1)) + m + (TG - 1 - t)
+        const float* __restrict__ vr = rho + (NR * ty + r) * RC_RHO_S + ml0 + 2 * kKUp - g * TG - (TG - 1);
+        float v[NV];
 #pragma unroll
-          for (int p = 0; p < D; ++p) acc[r][m * D + p] = fmaf(w[p], v, acc[r][m * D + p]);
-        }
+        for (int j = 0; j < NV; ++j) v[j] = vr[j];
+#pragma unroll
+        for (int t = 0; t < TG; ++t)
+#pragma unroll
+          for (int m = 0; m < NM; ++m)
+#pragma unroll
+            for (int p = 0; p < D; ++p) acc[r][m * D + p] = fmaf(w[t][p], v[m + TG - 1 - t], acc[r][m * D + p]);
       }
     }
   }
@@ -289,11 +300,11 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
       }
       __syncthreads();
       switch (d) {
-        case 2: upsample_acc<2>(acc, rho, wsm, ty, tx); break;
-        case 4: upsample_acc<4>(acc, rho, wsm, ty, tx); break;
-        case 8: upsample_acc<8>(acc, rho, wsm, ty, tx); break;
-        case 16: upsample_acc<16>(acc, rho, wsm, ty, tx); break;
-        default: upsample_acc<32>(acc, rho, wsm, ty, tx); break;
+        case 2: upsample_acc<2, 4>(acc, rho, wsm, ty, tx); break;
+        case 4: upsample_acc<4, 4>(acc, rho, wsm, ty, tx); break;
+        case 8: upsample_acc<8, 4>(acc, rho, wsm, ty, tx); break;
+        case 16: upsample_acc<16, 4>(acc, rho, wsm, ty, tx); break;
+        default: upsample_acc<32, 4>(acc, rho, wsm, ty, tx); break;
       }
     }
   }
@@ -385,7 +396,9 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
 
   __shared__ __align__(16) float As[LG_K][LG_S], Bs[LG_K][LG_S];
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  const int lr = tid >> 1, lk = (tid & 1) * 8;          // this thread stages row lr, k = lk .. lk + 7 of both tiles
+  // this thread stages row lr, k = lk .. lk + 7 of both tiles (a lane pair reads 64 contiguous bytes); the upper k half
+  // is stored with the row index XOR 16, so a warp's transposed stores fall into 32 different banks
+  const int lr = tid >> 1, lk = (tid & 1) * 8, lc = lr ^ ((tid & 1) * 16);
   float acc[8][8];
 #pragma unroll
   for (int i = 0; i < 8; ++i)
@@ -402,15 +415,17 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
       float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
       if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0); b1 = *reinterpret_cast<const float4*>(Y + l0 + 4); }
       __syncthreads();
-      As[lk + 0][lr] = a0.x; As[lk + 1][lr] = a0.y; As[lk + 2][lr] = a0.z; As[lk + 3][lr] = a0.w;
-      As[lk + 4][lr] = a1.x; As[lk + 5][lr] = a1.y; As[lk + 6][lr] = a1.z; As[lk + 7][lr] = a1.w;
-      Bs[lk + 0][lr] = b0.x; Bs[lk + 1][lr] = b0.y; Bs[lk + 2][lr] = b0.z; Bs[lk + 3][lr] = b0.w;
-      Bs[lk + 4][lr] = b1.x; Bs[lk + 5][lr] = b1.y; Bs[lk + 6][lr] = b1.z; Bs[lk + 7][lr] = b1.w;
+      As[lk + 0][lc] = a0.x; As[lk + 1][lc] = a0.y; As[lk + 2][lc] = a0.z; As[lk + 3][lc] = a0.w;
+      As[lk + 4][lc] = a1.x; As[lk + 5][lc] = a1.y; As[lk + 6][lc] = a1.z; As[lk + 7][lc] = a1.w;
+      Bs[lk + 0][lc] = b0.x; Bs[lk + 1][lc] = b0.y; Bs[lk + 2][lc] = b0.z; Bs[lk + 3][lc] = b0.w;
+      Bs[lk + 4][lc] = b1.x; Bs[lk + 5][lc] = b1.y; Bs[lk + 6][lc] = b1.z; Bs[lk + 7][lc] = b1.w;
       __syncthreads();
 #pragma unroll
       for (int k = 0; k < LG_K; ++k) {
-        const float4 av0 = *reinterpret_cast<const float4*>(&As[k][ty * 8]), av1 = *reinterpret_cast<const float4*>(&As[k][ty * 8 + 4]);
-        const float4 bv0 = *reinterpret_cast<const float4*>(&Bs[k][tx * 8]), bv1 = *reinterpret_cast<const float4*>(&Bs[k][tx * 8 + 4]);
+        // thread tile: rows 8 ty + i, columns 4 tx + j and 64 + 4 tx + j (16 B lane stride: no bank conflicts)
+        const int sw = (k >> 3) * 16;
+        const float4 av0 = *reinterpret_cast<const float4*>(&As[k][(ty * 8) ^ sw]), av1 = *reinterpret_cast<const float4*>(&As[k][(ty * 8 + 4) ^ sw]);
+        const float4 bv0 = *reinterpret_cast<const float4*>(&Bs[k][(tx * 4) ^ sw]), bv1 = *reinterpret_cast<const float4*>(&Bs[k][(64 + tx * 4) ^ sw]);
         const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
         const float b[8] = {bv0.x, bv0.y, bv0.z, bv0.w, bv1.x, bv1.y, bv1.z, bv1.w};
 #pragma unroll
@@ -422,9 +437,9 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
   }
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    float* q = G.Q + (size_t)(row0 + ty * 8 + i) * G.q_cols + j0 + tx * 8;
+    float* q = G.Q + (size_t)(row0 + ty * 8 + i) * G.q_cols + j0 + tx * 4;
     *reinterpret_cast<float4*>(q) = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
-    *reinterpret_cast<float4*>(q + 4) = make_float4(acc[i][4], acc[i][5], acc[i][6], acc[i][7]);
+    *reinterpret_cast<float4*>(q + 64) = make_float4(acc[i][4], acc[i][5], acc[i][6], acc[i][7]);
   }
 }
 
@@ -442,31 +457,70 @@ void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_d
 
 // ------------------------------------------------------------------------------------------------
 // fp32 path, second kernel: A3 of the d = 1 slices + A4 + A5 fused as in recon_f32_kernel, but the low-rate
-// rho^(d) come precomputed from lowrate_gemm_f32_kernel: per rate the CTA stages a [64 rows x (128/d + 2 K_up)]
+// rho^(d) come precomputed from lowrate_gemm_f32_kernel: per rate the CTA stages a [128 rows x (128/d + 2 K_up)]
 // window of Q and interpolates it into its register accumulators.
+// CTA tile: 128 real rows (64 templates) x 128 f0 samples, 256 threads as 16 (row groups of 8) x 16 (column groups of
+// 8), an 8 x 8 fp32 accumulator per thread.  K chunks of 16 are staged transposed (upper k half XOR-swizzled: no bank
+// conflicts on the stores); the next chunk's global loads are in flight while the current one is multiplied.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+constexpr int RQ_T = 128, RQ_K = 16, RQ_S = RQ_T + 4;
+
+// Window [RQ_T rows x (128/D + 2 K_up)] of rho^(d) -> shared memory.  The window starts on a multiple of 4 columns
+// (r0 = 128 g / D), so it moves as float4; every thread has up to 8 loads in flight before its first store (with one
+// load per loop trip the kernel spent 38 % of its stall samples on the store behind it).
+template <int D>
+__device__ __forceinline__ void stage_rho(float* __restrict__ rho, const float* __restrict__ Q, int qc, int q_left, int tid)
+{
+  constexpr int K4 = (RC_CT / D + 2 * kKUp) / 4;       // float4 per row
+  constexpr int N4 = RQ_T * K4;
+  constexpr int NIT = (N4 + 255) / 256;
+#pragma unroll
+  for (int i0 = 0; i0 < NIT; i0 += 8) {
+    float4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      if (i0 + u >= NIT) continue;
+      const int e = tid + 256 * (i0 + u);
+      const int row = e / K4, c4 = (e % K4) * 4;
+      v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (e < N4 && c4 < q_left) v[u] = __ldg(reinterpret_cast<const float4*>(Q + (size_t)row * qc + c4));
+    }
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      if (i0 + u >= NIT) continue;
+      const int e = tid + 256 * (i0 + u);
+      const int row = e / K4, c4 = (e % K4) * 4;
+      if (e < N4) {
+        float* o = rho + row * RC_RHO_S + c4;
+        o[0] = v[u].x; o[1] = v[u].y; o[2] = v[u].z; o[3] = v[u].w;
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256, 2)
 recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict__ bp,
                    const float* const* __restrict__ upw, const Q32Group* __restrict__ groups,
                    Peak* __restrict__ partials, int tiles_cap, int max_templates, int c, long long k_a, Capture cap)
 {
   const int bd = blockIdx.z;
   const BinParams B = bp[bd];
-  const int row0 = blockIdx.y * RC_RT;
+  const int row0 = blockIdx.y * RQ_T;
   if (row0 >= 2 * B.n_templates) return;
   const int g = blockIdx.x;
   const int kap0 = g * RC_CT;
 
   extern __shared__ __align__(16) float smem_r[];
-  float* Rs = smem_r;                               // [RC_KC][RC_RS]
-  float* Ys = Rs + RC_KC * RC_RS;                   // [RC_KC][RC_YS]
-  float* rho = Ys + RC_KC * RC_YS;                  // [RC_RT][RC_RHO_S]
-  float* wsm = rho + RC_RT * RC_RHO_S;              // [16][32]
+  float* As = smem_r;                               // [RQ_K][RQ_S]  R tile, transposed
+  float* Bs = As + RQ_K * RQ_S;                     // [RQ_K][RQ_S]  y tile, transposed
+  float* rho = Bs + RQ_K * RQ_S;                    // [RQ_T][RC_RHO_S]
+  float* wsm = rho + RQ_T * RC_RHO_S;               // [16][32]
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-  float acc[4][8];
+  const int lr = tid >> 1, lk = (tid & 1) * 8, lc = lr ^ ((tid & 1) * 16);   // staging: row lr, k = lk .. lk + 7 (upper half swizzled)
+  float acc[8][8];
 #pragma unroll
-  for (int r = 0; r < 4; ++r)
+  for (int r = 0; r < 8; ++r)
 #pragma unroll
     for (int cc = 0; cc < 8; ++cc) acc[r][cc] = 0.f;
 
@@ -474,34 +528,35 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
   for (int s = 0; s < B.n_slices; ++s) {
     const SliceParams P = sp[B.first_slice + s];
     if (P.d != 1) continue;
-    const float* __restrict__ R = P.R32;
-    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y);
     const int Lp = P.L_pad;
-    for (int l0 = 0; l0 < Lp; l0 += RC_KC) {
+    const float* __restrict__ R = P.R32 + (size_t)(row0 + lr) * Lp + lk;
+    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)(kap0 + lr) * Lp + lk;
+    const bool y_ok = kap0 + lr < P.y_rows_cap;
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 a0 = __ldg(reinterpret_cast<const float4*>(R)), a1 = __ldg(reinterpret_cast<const float4*>(R + 4));
+    float4 b0 = y_ok ? *reinterpret_cast<const float4*>(Y) : z4, b1 = y_ok ? *reinterpret_cast<const float4*>(Y + 4) : z4;
+    for (int l0 = 0; l0 < Lp; l0 += RQ_K) {
       __syncthreads();
-#pragma unroll
-      for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
-        const int e = tid + 256 * i;
-        const int ll = e % RC_KC, row = e / RC_KC;
-        Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
-      }
-      for (int e = tid; e < RC_CT * RC_KC; e += 256) {
-        const int ll = e % RC_KC, col = e / RC_KC;
-        const int r = kap0 + col;
-        Ys[ll * RC_YS + col] = (r < P.y_rows_cap) ? Y[(size_t)r * Lp + l0 + ll] : 0.f;
-      }
+      As[(lk + 0) * RQ_S + lc] = a0.x; As[(lk + 1) * RQ_S + lc] = a0.y; As[(lk + 2) * RQ_S + lc] = a0.z; As[(lk + 3) * RQ_S + lc] = a0.w;
+      As[(lk + 4) * RQ_S + lc] = a1.x; As[(lk + 5) * RQ_S + lc] = a1.y; As[(lk + 6) * RQ_S + lc] = a1.z; As[(lk + 7) * RQ_S + lc] = a1.w;
+      Bs[(lk + 0) * RQ_S + lc] = b0.x; Bs[(lk + 1) * RQ_S + lc] = b0.y; Bs[(lk + 2) * RQ_S + lc] = b0.z; Bs[(lk + 3) * RQ_S + lc] = b0.w;
+      Bs[(lk + 4) * RQ_S + lc] = b1.x; Bs[(lk + 5) * RQ_S + lc] = b1.y; Bs[(lk + 6) * RQ_S + lc] = b1.z; Bs[(lk + 7) * RQ_S + lc] = b1.w;
       __syncthreads();
-#pragma unroll 8
-      for (int ll = 0; ll < RC_KC; ++ll) {
-        const float4 a = *reinterpret_cast<const float4*>(Rs + ll * RC_RS + 4 * ty);
-        const float4 b0 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx);
-        const float4 b1 = *reinterpret_cast<const float4*>(Ys + ll * RC_YS + 8 * tx + 4);
-        const float av[4] = {a.x, a.y, a.z, a.w};
-        const float bv[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+      if (l0 + RQ_K < Lp) {                          // next chunk, in flight during the multiply
+        a0 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K)); a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K + 4));
+        if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0 + RQ_K); b1 = *reinterpret_cast<const float4*>(Y + l0 + RQ_K + 4); }
+      }
 #pragma unroll
-        for (int r = 0; r < 4; ++r)
+      for (int k = 0; k < RQ_K; ++k) {
+        const int sw = (k >> 3) * 16;
+        const float4 av0 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8) ^ sw)), av1 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8 + 4) ^ sw));
+        const float4 bv0 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8) ^ sw)), bv1 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8 + 4) ^ sw));
+        const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
+        const float b[8] = {bv0.x, bv0.y, bv0.z, bv0.w, bv1.x, bv1.y, bv1.z, bv1.w};
 #pragma unroll
-          for (int cc = 0; cc < 8; ++cc) acc[r][cc] = fmaf(av[r], bv[cc], acc[r][cc]);
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
       }
     }
   }
@@ -511,33 +566,27 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
     const Q32Group* G = groups + (size_t)bd * kNLowRates + (l2 - 1);
     if (G->n_slices == 0) continue;
     const int d = 1 << l2;
-    const int Ks = (RC_CT >> l2) + 2 * kKUp;
     const int r0 = kap0 >> l2;
-    const float* __restrict__ Q = G->Q;
-    const int qc = G->q_cols;
+    const float* __restrict__ Q = G->Q + (size_t)row0 * G->q_cols + r0;
+    const int qc = G->q_cols, q_left = G->q_cols - r0;
     __syncthreads();                                 // previous readers of rho / wsm are done
     {
       const float* __restrict__ w = upw[l2];         // [16][d]
       for (int e = tid; e < 16 * d; e += 256) wsm[(e / d) * 32 + (e % d)] = __ldg(w + e);
     }
-    for (int e = tid; e < RC_RT * Ks; e += 256) {
-      const int col = e % Ks, row = e / Ks;
-      rho[row * RC_RHO_S + col] = (r0 + col < qc) ? Q[(size_t)(row0 + row) * qc + r0 + col] : 0.f;
-    }
-    __syncthreads();
     switch (d) {
-      case 2: upsample_acc<2>(acc, rho, wsm, ty, tx); break;
-      case 4: upsample_acc<4>(acc, rho, wsm, ty, tx); break;
-      case 8: upsample_acc<8>(acc, rho, wsm, ty, tx); break;
-      case 16: upsample_acc<16>(acc, rho, wsm, ty, tx); break;
-      default: upsample_acc<32>(acc, rho, wsm, ty, tx); break;
+      case 2: stage_rho<2>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<2, 8>(acc, rho, wsm, ty, tx); break;
+      case 4: stage_rho<4>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<4, 8>(acc, rho, wsm, ty, tx); break;
+      case 8: stage_rho<8>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<8, 8>(acc, rho, wsm, ty, tx); break;
+      case 16: stage_rho<16>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<16, 8>(acc, rho, wsm, ty, tx); break;
+      default: stage_rho<32>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<32, 8>(acc, rho, wsm, ty, tx); break;
     }
   }
 
   // ---- epilogue: |rho|^2, first maximum over the tile's valid columns, one Peak per template
   const int valid = min(RC_CT, c - kap0);           // ragged last tile of a chunk
 #pragma unroll
-  for (int t = 0; t < 2; ++t) {
+  for (int t = 0; t < 4; ++t) {
     float bq = -1.f, bre = 0.f, bim = 0.f;
     int bk = 0x7fffffff;
 #pragma unroll
@@ -555,7 +604,7 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       const int ok = __shfl_xor_sync(0xffffffffu, bk, off);
       if (oq > bq || (oq == bq && ok < bk)) { bq = oq; bre = ore; bim = oim; bk = ok; }
     }
-    const int p = (row0 + 4 * ty) / 2 + t;
+    const int p = (row0 + 8 * ty) / 2 + t;
     if (tx == 0 && p < B.n_templates) {
       Peak pk; pk.q = bq; pk.kappa = bk; pk.re = bre; pk.im = bim;
       partials[((size_t)bd * tiles_cap + g) * max_templates + p] = pk;
@@ -564,8 +613,8 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
 
   if (cap.snr != nullptr && cap.bd == bd) {         // test-only dense dump from the same accumulators
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int row = row0 + 4 * ty + r;
+    for (int r = 0; r < 8; ++r) {
+      const int row = row0 + 8 * ty + r;
       if (row >= cap.rows) continue;
 #pragma unroll
       for (int cc = 0; cc < 8; ++cc) {
@@ -582,14 +631,14 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
                         const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
                         int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
 {
-  const size_t smem = sizeof(float) * (RC_KC * RC_RS + RC_KC * RC_YS + RC_RT * RC_RHO_S + 16 * 32);
+  const size_t smem = sizeof(float) * (2 * RQ_K * RQ_S + RQ_T * RC_RHO_S + 16 * 32);
   static bool configured = false;
   if (!configured) {
     cudaFuncSetAttribute(recon_f32_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
-  dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
+  dim3 grid(n_tiles, (max_rows_pad + RQ_T - 1) / RQ_T, n_bd);
   recon_f32_q_kernel<<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
                                              c, (long long)k_a, cap);
   ++*launches;
