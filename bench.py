@@ -140,6 +140,9 @@ def oracle_sample(w, seconds: float):
 
 def make_workload(args, rank=0):
     from paper_2410_16416_b200 import workloads as wl
+    if args.workload == "config3":                        # batching over bins (A7): the paper's throughput-vs-banks curve
+        secs = args.seconds if args.seconds != 4096 else 256
+        return wl.config3(n_bins=args.bins, seconds=secs, n_detectors=args.detectors)
     w = wl.config2(n_templates=args.templates, seconds=args.seconds, n_detectors=args.detectors)
     if rank:
         w.strain = wl.make_strain(wl.SEED0 + 2000 + 10 * rank, w.n_detectors, w.n_samples, w.bins, w.injections, 15.0, 1024.0)
@@ -147,6 +150,10 @@ def make_workload(args, rank=0):
 
 
 def workload_name(args):
+    if args.workload == "config3":
+        secs = args.seconds if args.seconds != 4096 else 256
+        return (f"BASELINE config 3 geometry, {args.bins} of 100 BBH-like bins x 500 templates batched "
+                f"(3 slices 2048/512/128 Hz, L=64), {args.detectors} det x {secs} s")
     full = (args.templates, args.seconds, args.detectors) == (1000, 4096, 2)
     return "BASELINE config 2 (1 BNS bin: 1000 templates, 8 slices 2048..64 Hz, L=150, 2 det x 4096 s)" if full else \
         f"config-2 geometry reduced: {args.templates} templates, {args.detectors} det x {args.seconds} s"
@@ -261,7 +268,8 @@ def run_ours(args):
         pk = peaks["bf16_sustained"]
         # DRAM bytes (read + write) of ONE launch at the 131072-sample chunk, from the committed ncu --set full capture
         ncu_traffic = {"f0_kernel": 1.166e9, "lowrate_recon_kernel": 1.116e9, "fir_f16_pers_kernel": 0.127e9}
-        full_chunk = int(lb.lloid_chunk_samples(bank.handle)) == 131072 and (args.templates, args.detectors) == (1000, 2)
+        full_chunk = (int(lb.lloid_chunk_samples(bank.handle)) == 131072 and (args.templates, args.detectors) == (1000, 2)
+                      and args.workload == "config2")
         roofline = {"bound": "tensor", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
                     "traffic": ncu_traffic.get(dom) if full_chunk else None,
                     "traffic_source": "profiles/r1_03_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)", "peak_source": peaks["source"] + " (cuBLAS bf16 sustained; fp16 runs at the same rate)",
@@ -391,8 +399,10 @@ def main():
     ap.add_argument("--templates", type=int, default=1000)
     ap.add_argument("--seconds", type=int, default=4096)
     ap.add_argument("--detectors", type=int, default=2)
-    ap.add_argument("--workload", default="config2", choices=["config2", "config5"],
-                    help="config2: the headline bench line; config5: 1 s streaming buffers on the config-3 bank (p50/p99 latency)")
+    ap.add_argument("--workload", default="config2", choices=["config2", "config3", "config5"],
+                    help="config2: the headline bench line; config3: --bins BBH-like bins batched offline (throughput vs number of "
+                         "bins, PAPER.md:96); config5: 1 s streaming buffers on the config-3 bank (p50/p99 latency)")
+    ap.add_argument("--bins", type=int, default=100, help="number of SVD bins batched (--workload config3)")
     ap.add_argument("--chunk", type=int, default=0, help="library time-chunk length in samples (0 = automatic)")
     ap.add_argument("--ref-seconds", type=float, default=2.0, help="seconds of output the oracle sample covers")
     args = ap.parse_args()

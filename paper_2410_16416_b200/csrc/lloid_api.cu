@@ -413,7 +413,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
       const int64_t need = (S.d == 1) ? S.end_delay + S.n_taps : S.end_delay + (int64_t)S.d * (S.n_taps + Ku + Kd);
       H = std::max(H, need);
       ybytes_per_sample += (double)D * S.L_pad * esize / S.d;
-      if (b->f16 && S.d > 1) ybytes_per_sample += (double)D * B.rows_pad * 2 / S.d;   // rho^(d) staging (upper bound)
+      if (S.d > 1) ybytes_per_sample += (double)D * B.rows_pad * esize / S.d;         // rho^(d) staging (upper bound)
     }
   H = round_up(H, 256);
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
@@ -421,13 +421,12 @@ int lloid_bank_finalize(lloid_bank_t* b)
   if (C == 0) {
     // Every chunk costs four kernel boundaries (launch gap, prologue with TMEM allocation and the stationary
     // operands, pipeline fill and drain: ~60 us in total, measured), so chunks are made LONG: up to 2^17 samples,
-    // bounded by 4 GiB of chunk-local intermediates (y^s, and on the fp16 path the low-rate rho^(d)).  Keeping the
-    // intermediates L2-resident with short chunks was measured slower on every config.
-    // The fp32 path is different: its reconstruction kernel re-reads every y tile once per 64-row block, so there the
-    // chunk is sized to keep y^s in L2 (96 MB), as measured best (2.3 s vs 3.0 s per config-2 step).
-    const double budget = b->f16 ? 4.0 * 1024 * 1024 * 1024 : 96.0 * 1024 * 1024;
+    // bounded by 12 GiB of chunk-local intermediates (y^s and the low-rate rho^(d)).  Keeping the intermediates
+    // L2-resident with short chunks was measured slower on every config: fp16 100 bins 3.50e8 at
+    // 24576 samples, 3.58e8 at 65536; fp32 config 2 243 ms per 1024 s at 34816 samples (y^s in L2), 235 ms at 131072.
+    const double budget = 12.0 * 1024 * 1024 * 1024;
     C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
-    C = std::min<int64_t>(std::max<int64_t>(C, 2048), b->f16 ? 131072 : 65536);
+    C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
   }
   b->H = (int)H; b->C = (int)C;
   // A1 runs once per super-chunk of S samples (not per chunk): the strain is tiny (8 KB/s per detector), so a
