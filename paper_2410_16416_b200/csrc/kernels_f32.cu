@@ -8,6 +8,16 @@
 
 namespace lloid {
 
+// Packed fp32 FMA (FFMA2 on sm_100a): two independent fma.rn.f32 per instruction, bit-identical to the scalar form.
+// The FMA pipe runs it at the same flop rate, but it needs half the issue slots -- the register-tiled kernels below
+// were issue-bound (71 % issue-active, FFMA only 78 % of the instructions).  ptxas folds pack2(a, a) into a scalar
+// broadcast operand (R4.F32), so the duplicated multiplicand costs nothing.
+typedef unsigned long long u64;
+__device__ __forceinline__ u64 pack2(float lo, float hi) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ void ffma2(u64& c, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
+
+
 // ------------------------------------------------------------------------------------------------
 // A2  y^s_l[j] = sum_t U^s[l,t] x^s[j - n_s + t]                     ("cross-correlates")
 //
@@ -42,9 +52,9 @@ fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
   }
 
   const int tl = tid & 7, tj = tid >> 3;
-  float acc[8][4];
+  u64 acc[8][2];                      // [time row][basis pair], packed fp32 x 2
 #pragma unroll
-  for (int j = 0; j < 8; ++j) { acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f; }
+  for (int j = 0; j < 8; ++j) { acc[j][0] = acc[j][1] = 0ull; }
 
   const float* __restrict__ U = P.U32;
   for (int t0 = 0; t0 < n_taps; t0 += FIR_KC) {
@@ -69,12 +79,12 @@ fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
 #pragma unroll
       for (int tt = 0; tt < 8; ++tt) {
         const float4 u = *reinterpret_cast<const float4*>(Us + (tt8 + tt) * FIR_US + tl * 4);
+        const u64 u01 = pack2(u.x, u.y), u23 = pack2(u.z, u.w);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-          acc[j][0] = fmaf(zw[j + tt], u.x, acc[j][0]);
-          acc[j][1] = fmaf(zw[j + tt], u.y, acc[j][1]);
-          acc[j][2] = fmaf(zw[j + tt], u.z, acc[j][2]);
-          acc[j][3] = fmaf(zw[j + tt], u.w, acc[j][3]);
+          const u64 zz = pack2(zw[j + tt], zw[j + tt]);
+          ffma2(acc[j][0], zz, u01);
+          ffma2(acc[j][1], zz, u23);
         }
       }
     }
@@ -83,9 +93,9 @@ fir_f32_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
     const int r = r0 + tj * 8 + j;
-    if (r < P.y_rows_cap)
-      *reinterpret_cast<float4*>(Y + (size_t)r * P.L_pad + l0 + tl * 4) =
-          make_float4(acc[j][0], acc[j][1], acc[j][2], acc[j][3]);
+    float4 v;
+    unpack2(acc[j][0], v.x, v.y); unpack2(acc[j][1], v.z, v.w);
+    if (r < P.y_rows_cap) *reinterpret_cast<float4*>(Y + (size_t)r * P.L_pad + l0 + tl * 4) = v;
   }
 }
 
@@ -177,6 +187,59 @@ __device__ __forceinline__ void upsample_acc(float (&acc)[NR][8], const float* _
           for (int m = 0; m < NM; ++m)
 #pragma unroll
             for (int p = 0; p < D; ++p) acc[r][m * D + p] = fmaf(w[t][p], v[m + TG - 1 - t], acc[r][m * D + p]);
+      }
+    }
+  }
+}
+
+// Same interpolation on the packed accumulators of the 8 x 8 tile: acc[r][j] = columns (8 tx + 2 j, 8 tx + 2 j + 1).
+template <int D>
+__device__ __forceinline__ void upsample_acc2(u64 (&acc)[8][4], const float* __restrict__ rho,
+                                              const float* __restrict__ wsm, int ty, int tx)
+{
+  if constexpr (D >= 8) {
+    const int ml = (8 * tx) / D;
+    const int phi0 = (8 * tx) % D;
+#pragma unroll
+    for (int i = -kKUp; i < kKUp; ++i) {
+      const float4 w0 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0);
+      const float4 w1 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0 + 4);
+      const u64 wp[4] = {pack2(w0.x, w0.y), pack2(w0.z, w0.w), pack2(w1.x, w1.y), pack2(w1.z, w1.w)};
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const float v = rho[(8 * ty + r) * RC_RHO_S + ml + kKUp - i];
+        const u64 vv = pack2(v, v);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) ffma2(acc[r][j], vv, wp[j]);
+      }
+    }
+  } else {
+    constexpr int NM = 8 / D, TG = 16 / D, NV = NM + TG - 1, DH = D / 2;
+    const int ml0 = (8 * tx) / D;
+#pragma unroll
+    for (int g = 0; g < 2 * kKUp / TG; ++g) {     // taps i = -K_up + g TG + t
+      u64 w[TG][DH];
+#pragma unroll
+      for (int t = 0; t < TG; ++t)
+#pragma unroll
+        for (int h = 0; h < DH; ++h) {
+          const float2 ww = *reinterpret_cast<const float2*>(wsm + (g * TG + t) * 32 + 2 * h);
+          w[t][h] = pack2(ww.x, ww.y);
+        }
+#pragma unroll
+      for (int r = 0; r < 8; ++r) {
+        const float* __restrict__ vr = rho + (8 * ty + r) * RC_RHO_S + ml0 + 2 * kKUp - g * TG - (TG - 1);
+        float v[NV];
+#pragma unroll
+        for (int j = 0; j < NV; ++j) v[j] = vr[j];
+#pragma unroll
+        for (int t = 0; t < TG; ++t)
+#pragma unroll
+          for (int m = 0; m < NM; ++m) {
+            const u64 vv = pack2(v[m + TG - 1 - t], v[m + TG - 1 - t]);
+#pragma unroll
+            for (int h = 0; h < DH; ++h) ffma2(acc[r][m * DH + h], vv, w[t][h]);
+          }
       }
     }
   }
@@ -399,11 +462,11 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
   // this thread stages row lr, k = lk .. lk + 7 of both tiles (a lane pair reads 64 contiguous bytes); the upper k half
   // is stored with the row index XOR 16, so a warp's transposed stores fall into 32 different banks
   const int lr = tid >> 1, lk = (tid & 1) * 8, lc = lr ^ ((tid & 1) * 16);
-  float acc[8][8];
+  u64 acc[8][4];                                        // [row][column pair], packed fp32 x 2
 #pragma unroll
   for (int i = 0; i < 8; ++i)
 #pragma unroll
-    for (int j = 0; j < 8; ++j) acc[i][j] = 0.f;
+    for (int j = 0; j < 4; ++j) acc[i][j] = 0ull;
 
   for (int s = 0; s < G.n_slices; ++s) {
     const SliceParams P = sp[G.slice[s]];
@@ -427,19 +490,24 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
         const float4 av0 = *reinterpret_cast<const float4*>(&As[k][(ty * 8) ^ sw]), av1 = *reinterpret_cast<const float4*>(&As[k][(ty * 8 + 4) ^ sw]);
         const float4 bv0 = *reinterpret_cast<const float4*>(&Bs[k][(tx * 4) ^ sw]), bv1 = *reinterpret_cast<const float4*>(&Bs[k][(64 + tx * 4) ^ sw]);
         const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
-        const float b[8] = {bv0.x, bv0.y, bv0.z, bv0.w, bv1.x, bv1.y, bv1.z, bv1.w};
+        const u64 b[4] = {pack2(bv0.x, bv0.y), pack2(bv0.z, bv0.w), pack2(bv1.x, bv1.y), pack2(bv1.z, bv1.w)};
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < 8; ++i) {
+          const u64 aa = pack2(a[i], a[i]);
 #pragma unroll
-          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+          for (int j = 0; j < 4; ++j) ffma2(acc[i][j], aa, b[j]);
+        }
       }
     }
   }
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     float* q = G.Q + (size_t)(row0 + ty * 8 + i) * G.q_cols + j0 + tx * 4;
-    *reinterpret_cast<float4*>(q) = make_float4(acc[i][0], acc[i][1], acc[i][2], acc[i][3]);
-    *reinterpret_cast<float4*>(q + 64) = make_float4(acc[i][4], acc[i][5], acc[i][6], acc[i][7]);
+    float4 o0, o1;
+    unpack2(acc[i][0], o0.x, o0.y); unpack2(acc[i][1], o0.z, o0.w);
+    unpack2(acc[i][2], o1.x, o1.y); unpack2(acc[i][3], o1.z, o1.w);
+    *reinterpret_cast<float4*>(q) = o0;
+    *reinterpret_cast<float4*>(q + 64) = o1;
   }
 }
 
@@ -518,11 +586,11 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int lr = tid >> 1, lk = (tid & 1) * 8, lc = lr ^ ((tid & 1) * 16);   // staging: row lr, k = lk .. lk + 7 (upper half swizzled)
-  float acc[8][8];
+  u64 acc2[8][4];                                   // [row][column pair], packed fp32 x 2
 #pragma unroll
   for (int r = 0; r < 8; ++r)
 #pragma unroll
-    for (int cc = 0; cc < 8; ++cc) acc[r][cc] = 0.f;
+    for (int j = 0; j < 4; ++j) acc2[r][j] = 0ull;
 
   // ---- d = 1 slices: K-chunked SGEMM straight into the accumulators
   for (int s = 0; s < B.n_slices; ++s) {
@@ -552,11 +620,13 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
         const float4 av0 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8) ^ sw)), av1 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8 + 4) ^ sw));
         const float4 bv0 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8) ^ sw)), bv1 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8 + 4) ^ sw));
         const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
-        const float b[8] = {bv0.x, bv0.y, bv0.z, bv0.w, bv1.x, bv1.y, bv1.z, bv1.w};
+        const u64 b[4] = {pack2(bv0.x, bv0.y), pack2(bv0.z, bv0.w), pack2(bv1.x, bv1.y), pack2(bv1.z, bv1.w)};
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int i = 0; i < 8; ++i) {
+          const u64 aa = pack2(a[i], a[i]);
 #pragma unroll
-          for (int j = 0; j < 8; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+          for (int j = 0; j < 4; ++j) ffma2(acc2[i][j], aa, b[j]);
+        }
       }
     }
   }
@@ -575,15 +645,20 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       for (int e = tid; e < 16 * d; e += 256) wsm[(e / d) * 32 + (e % d)] = __ldg(w + e);
     }
     switch (d) {
-      case 2: stage_rho<2>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<2, 8>(acc, rho, wsm, ty, tx); break;
-      case 4: stage_rho<4>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<4, 8>(acc, rho, wsm, ty, tx); break;
-      case 8: stage_rho<8>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<8, 8>(acc, rho, wsm, ty, tx); break;
-      case 16: stage_rho<16>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<16, 8>(acc, rho, wsm, ty, tx); break;
-      default: stage_rho<32>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc<32, 8>(acc, rho, wsm, ty, tx); break;
+      case 2: stage_rho<2>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc2<2>(acc2, rho, wsm, ty, tx); break;
+      case 4: stage_rho<4>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc2<4>(acc2, rho, wsm, ty, tx); break;
+      case 8: stage_rho<8>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc2<8>(acc2, rho, wsm, ty, tx); break;
+      case 16: stage_rho<16>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc2<16>(acc2, rho, wsm, ty, tx); break;
+      default: stage_rho<32>(rho, Q, qc, q_left, tid); __syncthreads(); upsample_acc2<32>(acc2, rho, wsm, ty, tx); break;
     }
   }
 
   // ---- epilogue: |rho|^2, first maximum over the tile's valid columns, one Peak per template
+  float acc[8][8];
+#pragma unroll
+  for (int r = 0; r < 8; ++r)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) unpack2(acc2[r][j], acc[r][2 * j], acc[r][2 * j + 1]);
   const int valid = min(RC_CT, c - kap0);           // ragged last tile of a chunk
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
