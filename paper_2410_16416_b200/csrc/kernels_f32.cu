@@ -193,6 +193,12 @@ __device__ __forceinline__ void upsample_acc(float (&acc)[NR][8], const float* _
 }
 
 // Same interpolation on the packed accumulators of the 8 x 8 tile: acc[r][j] = columns (8 tx + 2 j, 8 tx + 2 j + 1).
+// rho rows have stride RQ_RHO_S = 84 floats.  d >= 8: one sample per (tap, row); the two row groups a warp covers
+// (ty, ty + 1) read the same columns, so odd row groups are stored with the column XOR 16 (disjoint banks).
+// d = 2, 4: the NM + TG - 1 samples of a tap group start one past a 16-byte (d = 2) / 8-byte (d = 4) boundary; they
+// are read as 3 aligned LDS.128 / LDS.64 (lane stride 16 / 8 bytes: no bank conflicts) and the first value dropped.
+constexpr int RQ_RHO_S = 84;
+
 template <int D>
 __device__ __forceinline__ void upsample_acc2(u64 (&acc)[8][4], const float* __restrict__ rho,
                                               const float* __restrict__ wsm, int ty, int tx)
@@ -200,21 +206,25 @@ __device__ __forceinline__ void upsample_acc2(u64 (&acc)[8][4], const float* __r
   if constexpr (D >= 8) {
     const int ml = (8 * tx) / D;
     const int phi0 = (8 * tx) % D;
+    const int sw = (ty & 1) * 16;
+    const float* __restrict__ rrow = rho + (8 * ty) * RQ_RHO_S;
 #pragma unroll
     for (int i = -kKUp; i < kKUp; ++i) {
       const float4 w0 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0);
       const float4 w1 = *reinterpret_cast<const float4*>(wsm + (i + kKUp) * 32 + phi0 + 4);
       const u64 wp[4] = {pack2(w0.x, w0.y), pack2(w0.z, w0.w), pack2(w1.x, w1.y), pack2(w1.z, w1.w)};
+      const int col = (ml + kKUp - i) ^ sw;
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
-        const float v = rho[(8 * ty + r) * RC_RHO_S + ml + kKUp - i];
+        const float v = rrow[r * RQ_RHO_S + col];
         const u64 vv = pack2(v, v);
 #pragma unroll
         for (int j = 0; j < 4; ++j) ffma2(acc[r][j], vv, wp[j]);
       }
     }
   } else {
-    constexpr int NM = 8 / D, TG = 16 / D, NV = NM + TG - 1, DH = D / 2;
+    constexpr int NM = 8 / D, TG = 16 / D, DH = D / 2;
+    constexpr int VW = (D == 2) ? 4 : 2;            // floats per aligned load; 3 loads cover the window + 1
     const int ml0 = (8 * tx) / D;
 #pragma unroll
     for (int g = 0; g < 2 * kKUp / TG; ++g) {     // taps i = -K_up + g TG + t
@@ -228,15 +238,25 @@ __device__ __forceinline__ void upsample_acc2(u64 (&acc)[8][4], const float* __r
         }
 #pragma unroll
       for (int r = 0; r < 8; ++r) {
-        const float* __restrict__ vr = rho + (8 * ty + r) * RC_RHO_S + ml0 + 2 * kKUp - g * TG - (TG - 1);
-        float v[NV];
+        // sample index ml0 + m + K_up - i = start + m + (TG - 1 - t), start = ml0 + 2 K_up - g TG - (TG - 1); start - 1 is aligned
+        const float* __restrict__ vr = rho + (8 * ty + r) * RQ_RHO_S + ml0 + 2 * kKUp - g * TG - (TG - 1) - 1;
+        float v[3 * VW];
 #pragma unroll
-        for (int j = 0; j < NV; ++j) v[j] = vr[j];
+        for (int q = 0; q < 3; ++q) {
+          if constexpr (D == 2) {
+            const float4 x = *reinterpret_cast<const float4*>(vr + 4 * q);
+            v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
+          } else {
+            const float2 x = *reinterpret_cast<const float2*>(vr + 2 * q);
+            v[2 * q] = x.x; v[2 * q + 1] = x.y;
+          }
+        }
 #pragma unroll
         for (int t = 0; t < TG; ++t)
 #pragma unroll
           for (int m = 0; m < NM; ++m) {
-            const u64 vv = pack2(v[m + TG - 1 - t], v[m + TG - 1 - t]);
+            const float x = v[1 + m + TG - 1 - t];
+            const u64 vv = pack2(x, x);
 #pragma unroll
             for (int h = 0; h < DH; ++h) ffma2(acc[r][m * DH + h], vv, w[t][h]);
           }
@@ -473,16 +493,20 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
     const float* __restrict__ R = P.R32 + (size_t)(row0 + lr) * P.L_pad + lk;
     const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)(j0 + lr) * P.L_pad + lk;
     const bool y_ok = j0 + lr < P.y_rows_cap;
+    float4 a0 = __ldg(reinterpret_cast<const float4*>(R)), a1 = __ldg(reinterpret_cast<const float4*>(R + 4));
+    float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+    if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y); b1 = *reinterpret_cast<const float4*>(Y + 4); }
     for (int l0 = 0; l0 < P.L_pad; l0 += LG_K) {
-      const float4 a0 = __ldg(reinterpret_cast<const float4*>(R + l0)), a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + 4));
-      float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-      if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0); b1 = *reinterpret_cast<const float4*>(Y + l0 + 4); }
       __syncthreads();
       As[lk + 0][lc] = a0.x; As[lk + 1][lc] = a0.y; As[lk + 2][lc] = a0.z; As[lk + 3][lc] = a0.w;
       As[lk + 4][lc] = a1.x; As[lk + 5][lc] = a1.y; As[lk + 6][lc] = a1.z; As[lk + 7][lc] = a1.w;
       Bs[lk + 0][lc] = b0.x; Bs[lk + 1][lc] = b0.y; Bs[lk + 2][lc] = b0.z; Bs[lk + 3][lc] = b0.w;
       Bs[lk + 4][lc] = b1.x; Bs[lk + 5][lc] = b1.y; Bs[lk + 6][lc] = b1.z; Bs[lk + 7][lc] = b1.w;
       __syncthreads();
+      if (l0 + LG_K < P.L_pad) {                     // next chunk, in flight during the multiply
+        a0 = __ldg(reinterpret_cast<const float4*>(R + l0 + LG_K)); a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + LG_K + 4));
+        if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0 + LG_K); b1 = *reinterpret_cast<const float4*>(Y + l0 + LG_K + 4); }
+      }
 #pragma unroll
       for (int k = 0; k < LG_K; ++k) {
         // thread tile: rows 8 ty + i, columns 4 tx + j and 64 + 4 tx + j (16 B lane stride: no bank conflicts)
@@ -531,7 +555,7 @@ void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_d
 // 8), an 8 x 8 fp32 accumulator per thread.  K chunks of 16 are staged transposed (upper k half XOR-swizzled: no bank
 // conflicts on the stores); the next chunk's global loads are in flight while the current one is multiplied.
 // ------------------------------------------------------------------------------------------------
-constexpr int RQ_T = 128, RQ_K = 16, RQ_S = RQ_T + 4;
+constexpr int RQ_T = 128, RQ_K = 16, RQ_S = RQ_T + 4, RQ_SB = 136;
 
 // Window [RQ_T rows x (128/D + 2 K_up)] of rho^(d) -> shared memory.  The window starts on a multiple of 4 columns
 // (r0 = 128 g / D), so it moves as float4; every thread has up to 8 loads in flight before its first store (with one
@@ -559,8 +583,8 @@ __device__ __forceinline__ void stage_rho(float* __restrict__ rho, const float* 
       const int e = tid + 256 * (i0 + u);
       const int row = e / K4, c4 = (e % K4) * 4;
       if (e < N4) {
-        float* o = rho + row * RC_RHO_S + c4;
-        o[0] = v[u].x; o[1] = v[u].y; o[2] = v[u].z; o[3] = v[u].w;
+        const int col = (D >= 8) ? (c4 ^ (((row >> 3) & 1) * 16)) : c4;      // see upsample_acc2
+        *reinterpret_cast<float4*>(rho + row * RQ_RHO_S + col) = v[u];
       }
     }
   }
@@ -580,12 +604,15 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
 
   extern __shared__ __align__(16) float smem_r[];
   float* As = smem_r;                               // [RQ_K][RQ_S]  R tile, transposed
-  float* Bs = As + RQ_K * RQ_S;                     // [RQ_K][RQ_S]  y tile, transposed
-  float* rho = Bs + RQ_K * RQ_S;                    // [RQ_T][RC_RHO_S]
-  float* wsm = rho + RQ_T * RC_RHO_S;               // [16][32]
+  // y tile, transposed and column-permuted: column c sits at 4 (c / 8) + c % 4 (+ 72 if c % 8 >= 4), so the 8 columns
+  // of a thread are two float4 with a 16-byte lane stride (the plain layout's 32-byte stride is a 2-way conflict)
+  float* Bs = As + RQ_K * RQ_S;                     // [RQ_K][RQ_SB]
+  float* rho = Bs + RQ_K * RQ_SB;                   // [RQ_T][RQ_RHO_S]
+  float* wsm = rho + RQ_T * RQ_RHO_S;               // [16][32]
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int lr = tid >> 1, lk = (tid & 1) * 8, lc = lr ^ ((tid & 1) * 16);   // staging: row lr, k = lk .. lk + 7 (upper half swizzled)
+  const int lcb = ((((lr >> 3) << 2) | (lr & 3)) ^ ((tid & 1) * 16)) + ((lr & 4) ? 72 : 0);
   u64 acc2[8][4];                                   // [row][column pair], packed fp32 x 2
 #pragma unroll
   for (int r = 0; r < 8; ++r)
@@ -607,8 +634,8 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       __syncthreads();
       As[(lk + 0) * RQ_S + lc] = a0.x; As[(lk + 1) * RQ_S + lc] = a0.y; As[(lk + 2) * RQ_S + lc] = a0.z; As[(lk + 3) * RQ_S + lc] = a0.w;
       As[(lk + 4) * RQ_S + lc] = a1.x; As[(lk + 5) * RQ_S + lc] = a1.y; As[(lk + 6) * RQ_S + lc] = a1.z; As[(lk + 7) * RQ_S + lc] = a1.w;
-      Bs[(lk + 0) * RQ_S + lc] = b0.x; Bs[(lk + 1) * RQ_S + lc] = b0.y; Bs[(lk + 2) * RQ_S + lc] = b0.z; Bs[(lk + 3) * RQ_S + lc] = b0.w;
-      Bs[(lk + 4) * RQ_S + lc] = b1.x; Bs[(lk + 5) * RQ_S + lc] = b1.y; Bs[(lk + 6) * RQ_S + lc] = b1.z; Bs[(lk + 7) * RQ_S + lc] = b1.w;
+      Bs[(lk + 0) * RQ_SB + lcb] = b0.x; Bs[(lk + 1) * RQ_SB + lcb] = b0.y; Bs[(lk + 2) * RQ_SB + lcb] = b0.z; Bs[(lk + 3) * RQ_SB + lcb] = b0.w;
+      Bs[(lk + 4) * RQ_SB + lcb] = b1.x; Bs[(lk + 5) * RQ_SB + lcb] = b1.y; Bs[(lk + 6) * RQ_SB + lcb] = b1.z; Bs[(lk + 7) * RQ_SB + lcb] = b1.w;
       __syncthreads();
       if (l0 + RQ_K < Lp) {                          // next chunk, in flight during the multiply
         a0 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K)); a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K + 4));
@@ -618,7 +645,7 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       for (int k = 0; k < RQ_K; ++k) {
         const int sw = (k >> 3) * 16;
         const float4 av0 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8) ^ sw)), av1 = *reinterpret_cast<const float4*>(As + k * RQ_S + ((ty * 8 + 4) ^ sw));
-        const float4 bv0 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8) ^ sw)), bv1 = *reinterpret_cast<const float4*>(Bs + k * RQ_S + ((tx * 8 + 4) ^ sw));
+        const float4 bv0 = *reinterpret_cast<const float4*>(Bs + k * RQ_SB + ((tx * 4) ^ sw)), bv1 = *reinterpret_cast<const float4*>(Bs + k * RQ_SB + 72 + ((tx * 4) ^ sw));
         const float a[8] = {av0.x, av0.y, av0.z, av0.w, av1.x, av1.y, av1.z, av1.w};
         const u64 b[4] = {pack2(bv0.x, bv0.y), pack2(bv0.z, bv0.w), pack2(bv1.x, bv1.y), pack2(bv1.z, bv1.w)};
 #pragma unroll
@@ -706,7 +733,7 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
                         const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
                         int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
 {
-  const size_t smem = sizeof(float) * (2 * RQ_K * RQ_S + RQ_T * RC_RHO_S + 16 * 32);
+  const size_t smem = sizeof(float) * (RQ_K * RQ_S + RQ_K * RQ_SB + RQ_T * RQ_RHO_S + 16 * 32);
   static bool configured = false;
   if (!configured) {
     cudaFuncSetAttribute(recon_f32_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
