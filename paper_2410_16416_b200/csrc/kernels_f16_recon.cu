@@ -39,7 +39,7 @@ using namespace tc;
 
 constexpr int RC16_STAGE = 8192;            // bytes per ring stage: one K = 32 (y) or K = 16 (rho^(d)) operand chunk
 constexpr int RC16_MAX_STAGES = 16;
-constexpr int RC16_SMEM_BUDGET = 220 * 1024;
+constexpr int RC16_SMEM_BUDGET = 219 * 1024;     // + 7 KB static (barriers, tables, epilogue exchange) = 226 of 227 KB
 
 struct LowUnit { int32_t group, rb; };
 
@@ -398,9 +398,12 @@ constexpr int kMaxTileItems = kNLowRates * 8;
 //   warp 1  IY   MMAs of the d = 1 slices into accumulator buf = tile parity, then commit -> ybar[buf]
 //   warp 8  IQ   waits ybar[buf] (the y part is COMPLETE: orders its accumulating MMAs after IY's zeroing one),
 //                interpolation MMAs, commit -> acc_full[buf]
-//   warps 2-5    epilogue (one thread = one template)
+//   warps 2-5    epilogue, columns [0, 64) of the tile (one thread = one template)
+//   warps 9-12   epilogue, columns [64, 128); hands its partial maximum to the first group through shared memory.
+//                With L = 64 (config 3) the MMAs of a tile take ~1000 cycles and a single 128-column epilogue pass
+//                ~2900: the kernel ran at the epilogue's pace.
 // While IQ works on tile t, IY already fills the other accumulator with tile t + 1.
-constexpr int F0_THREADS = 288;
+constexpr int F0_THREADS = 416;
 
 struct F0Bars {
   uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES];      // y ring: slots [0, nsy); chunk ring: slots [nsy, nsy + nsq)
@@ -435,6 +438,7 @@ f0_kernel(const __grid_constant__ F0Args a)
   __shared__ __align__(16) ItTab s_it[2][kMaxTileItems];
   __shared__ PrTab s_pr[2][kNLowRates];
   __shared__ int s_rng[4];
+  __shared__ __align__(16) Peak s_half[2][kTplBlock];    // second column half's partial maximum, per accumulator buffer
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   if (tid == 0) sched_range(a.sched, s_rng);
@@ -447,7 +451,7 @@ f0_kernel(const __grid_constant__ F0Args a)
   if (tid == 32) {
     for (int s = 0; s < RC16_MAX_STAGES; ++s) { mbar_init(smem_u32(&bars.full[s]), 1); mbar_init(smem_u32(&bars.empty[s]), 1); }
     for (int b = 0; b < 2; ++b) {
-      mbar_init(smem_u32(&bars.acc_full[b]), 1); mbar_init(smem_u32(&bars.acc_empty[b]), 128);
+      mbar_init(smem_u32(&bars.acc_full[b]), 1); mbar_init(smem_u32(&bars.acc_empty[b]), 256);
       mbar_init(smem_u32(&bars.ybar[b]), 1); mbar_init(smem_u32(&bars.consts[b]), 1); mbar_init(smem_u32(&bars.unit_done[b]), 1);
     }
     mbar_init_fence();
@@ -630,9 +634,10 @@ f0_kernel(const __grid_constant__ F0Args a)
         ++seg_i;
       }
     }
-  } else if (warp >= 2 && warp <= 5) {
-    // ===== epilogue: one thread = one template; |rho|^2 and first maximum over the tile's columns =====
-    const int q = warp & 3;
+  } else if ((warp >= 2 && warp <= 5) || warp >= 9) {
+    // ===== epilogue: one thread = one template and one half of the tile's columns; |rho|^2 and first maximum =====
+    const int q = warp & 3;                           // TMEM lane quarter this warp may access
+    const int half = warp >= 9 ? 1 : 0;
     const int pl = q * 32 + lane;
     uint32_t fph = 0u;
     int buf = 0;
@@ -652,7 +657,7 @@ f0_kernel(const __grid_constant__ F0Args a)
         float bq[4] = {-1.f, -1.f, -1.f, -1.f}, bre4[4] = {0.f, 0.f, 0.f, 0.f}, bim4[4] = {0.f, 0.f, 0.f, 0.f};
         int bk4[4] = {0, 0, 0, 0};
   #pragma unroll 1
-        for (int c0 = 0; c0 < 128; c0 += 32) {
+        for (int c0 = 64 * half; c0 < 64 * half + 64; c0 += 32) {
           uint32_t re[32], im[32];
           tmem_ld32(taddr + (uint32_t)c0, re);
           tmem_ld32(taddr + (uint32_t)(128 + c0), im);
@@ -690,9 +695,17 @@ f0_kernel(const __grid_constant__ F0Args a)
           if (bq[m] > best || (bq[m] == best && bk4[m] < bk)) { best = bq[m]; bk = bk4[m]; bre = bre4[m]; bim = bim4[m]; }
         fence_before();
         mbar_arrive(smem_u32(&bars.acc_empty[buf]));
-        if (p < n_templates) {
-          Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
-          a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+        // s_half[buf] of tile t is rewritten at tile t + 2, i.e. after the barrier of tile t + 1, which the first group
+        // reaches only after it has read tile t's entry
+        if (half) { Peak pk; pk.q = best; pk.kappa = bk; pk.re = bre; pk.im = bim; s_half[buf][pl] = pk; }
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        if (!half) {
+          const Peak o = s_half[buf][pl];
+          if (o.q > best) { best = o.q; bk = o.kappa; bre = o.re; bim = o.im; }   // its columns are later: ties stay with the first half
+          if (p < n_templates) {
+            Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
+            a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+          }
         }
       }
     }
