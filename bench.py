@@ -267,12 +267,12 @@ def run_ours(args):
         path_ach = (fl["fir"] + fl["recon"]) * samples / ((stage[1] + stage[2]) * 1e-3) / 1e12
         pk = peaks["bf16_sustained"]
         # DRAM bytes (read + write) of ONE launch at the 131072-sample chunk, from the committed ncu --set full capture
-        ncu_traffic = {"f0_kernel": 1.166e9, "lowrate_recon_kernel": 1.116e9, "fir_f16_pers_kernel": 0.127e9}
+        ncu_traffic = {"f0_kernel": 1.167e9, "lowrate_recon_kernel": 1.115e9, "fir_f16_pers_kernel": 0.127e9}
         full_chunk = (int(lb.lloid_chunk_samples(bank.handle)) == 131072 and (args.templates, args.detectors) == (1000, 2)
                       and args.workload == "config2")
         roofline = {"bound": "tensor", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
                     "traffic": ncu_traffic.get(dom) if full_chunk else None,
-                    "traffic_source": "profiles/r1_03_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)", "peak_source": peaks["source"] + " (cuBLAS bf16 sustained; fp16 runs at the same rate)",
+                    "traffic_source": "profiles/r1_04_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)", "peak_source": peaks["source"] + " (cuBLAS bf16 sustained; fp16 runs at the same rate)",
                     "launch_ms": kernels[dom][1] / n_chunks, "launches": n_chunks,
                     "kernels": {k: {"algorithmic_tflop": v[0] / 1e12, "ms": v[1], "tflops": v[0] / (v[1] * 1e-3) / 1e12,
                                     "frac": v[0] / (v[1] * 1e-3) / 1e12 / pk} for k, v in kernels.items()},
