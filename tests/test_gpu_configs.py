@@ -82,6 +82,27 @@ def test_config3_hundred_bins_batched(precision):
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
+def test_config3_ten_bins_units_between_half_and_all_sms(precision):
+    """10 bins x 2 detectors x 4 template blocks = 80 reconstruction units: more than half of the 148 SMs, fewer than
+    all.  The f0 kernel then deals tiles over all SMs and most CTAs replace their stationary R mid-way (the
+    whole-CTAs-per-unit rule would idle 68 SMs); same checks as the 100-bin case."""
+    w = wl.config3(n_bins=10, n_templates=500, seconds=40, n_detectors=2, n_basis=64)
+    tol = pu.TOL[precision]
+    W = w.peak_window
+    k0 = 10 * W
+    for bin_, det in ((4, 1), (9, 0)):
+        trigs, snr, info = pu.run_gpu(w, precision, capture=(bin_, det, k0, 2 * W))
+        rho = pu.oracle_snr(w, bin_, det, k0, k0 + 2 * W)
+        assert np.abs(snr - rho).max() <= tol
+        pu.check_triggers(trigs, rho, k0, w, bin_, det, tol)
+    assert _unique_keys(trigs, W)
+    assert set(np.unique(trigs["bin"])) == set(range(10))
+    strip = lambda t: sorted((int(x["detector"]), int(x["template_idx"]), int(x["sample"]), float(x["snr_re"])) for x in t)
+    assert w.bins[0] is w.bins[1]                   # bins of one shape class share their arrays: identical triggers
+    assert strip(trigs[trigs["bin"] == 0]) == strip(trigs[trigs["bin"] == 1])
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
 def test_config4_geometry_heterogeneous_L(precision):
     """BASELINE config 4 shape: 6 slices 2048..64 Hz, M = 64 s, L(b, s) = 100 + ((37 b + 61 s) mod 201) in
     [100, 300], 3 detectors; reduced to 5 bins x 160 templates x 100 s."""
