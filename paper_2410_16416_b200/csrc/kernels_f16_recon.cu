@@ -438,6 +438,7 @@ f0_kernel(const __grid_constant__ F0Args a)
   __shared__ __align__(16) ItTab s_it[2][kMaxTileItems];
   __shared__ PrTab s_pr[2][kNLowRates];
   __shared__ int s_rng[4];
+  __shared__ __align__(16) uint4 s_qst[RC16_MAX_STAGES];   // IQ: per chunk-ring stage {operand descriptor, full barrier, empty barrier}
   __shared__ __align__(16) Peak s_half[2][kTplBlock];    // second column half's partial maximum, per accumulator buffer
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -594,6 +595,11 @@ f0_kernel(const __grid_constant__ F0Args a)
       uint32_t yph = 0u;
       int seg_i = 0, buf = 0;
       Ring rg{0, 0u, nsq};
+      // Everything a chunk needs is read from two small tables (one LDS.128 each) instead of being recomputed: every
+      // value the MMA takes has to cross from a vector to a uniform register (R2UR), and this loop is the kernel's
+      // critical path.
+      for (int st = 0; st < nsq; ++st)
+        s_qst[st] = make_uint4(qa_base + (uint32_t)st * (RC16_STAGE / 16), qfull + 8u * st, qempty + 8u * st, 0u);
       FOR_SEGMENTS(u, t0, t1) {
         const F0Combo cb = a.combos[u];
         const BdPlan* B = a.bd + cb.bd;
@@ -604,7 +610,9 @@ f0_kernel(const __grid_constant__ F0Args a)
             const int vv = a.up[r].n_var > 1 ? v : 0;
             for (int i = 0; i < a.n_items[r][vv]; ++i) {
               const QItem it = a.item[r][vv][i];
-              ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.d_off = it.d_off; e.pad = 0;
+              // tiles of parity v use accumulator buf ^ ((v ^ t0) & 1): the accumulator address goes into the table
+              ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.pad = 0;
+              e.d_off = tmem + (uint32_t)((buf ^ ((v ^ t0) & 1)) * 256) + it.d_off;
               s_it[v][nit[v]++] = e;
             }
           }
@@ -613,18 +621,17 @@ f0_kernel(const __grid_constant__ F0Args a)
         for (int t = t0; t < t1; ++t, buf ^= 1) {
           mbar_wait(smem_u32(&bars.ybar[buf]), (yph >> buf) & 1u); yph ^= 1u << buf;
           fence_after();
-          const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
           const ItTab* tab = s_it[t & 1];
           const int n_it = nit[t & 1];
           for (int k = 0; k < n_it; ++k) {
-            const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, d_off
-            mbar_wait(qfull + 8u * rg.s, rg.ph);
+            const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, accumulator address
+            const uint4 q = s_qst[rg.s];                                  // operand descriptor, full, empty barrier
+            mbar_wait(q.y, rg.ph);
             fence_after();
-            const uint32_t qa = qa_base + (uint32_t)rg.s * (RC16_STAGE / 16);
             const uint64_t bdesc = desc64(e.y);
-            mma_ss(d_tmem + e.z,        desc64(qa),        bdesc, e.x, 1u);
-            mma_ss(d_tmem + 128u + e.z, desc64(qa + 128u), bdesc, e.x, 1u);
-            commit(qempty + 8u * rg.s);
+            mma_ss(e.z,        desc64(q.x),        bdesc, e.x, 1u);
+            mma_ss(e.z + 128u, desc64(q.x + 128u), bdesc, e.x, 1u);
+            commit(q.z);
             rg.advance();
           }
           commit(smem_u32(&bars.acc_full[buf]));
