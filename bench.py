@@ -286,6 +286,13 @@ def run_ours(args):
                                  "frac": merge_bytes / (stage[3] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[3]}
         roofline["resample_hbm"] = {"achieved": res_bytes / (stage[0] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
                                     "frac": res_bytes / (stage[0] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[0]}
+        # the direct-form decimator does 2 (2 K_dn d + 1) / d flop per input sample and rate: 27 flop per byte moved,
+        # 2.4 times the machine balance (74.4 TFLOP/s / 6.5 TB/s = 11.5 flop/B) -- its bound is the FP32 ALUs
+        res_flops = samples * sum(2.0 * (2 * w.k_down * d + 1) / d for d in rates if d > 1)
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        roofline["resample_alu"] = {"achieved": res_flops / (stage[0] * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+                                    "frac": res_flops / (stage[0] * 1e-3) / 1e12 / alu_peak,
+                                    "flop_per_byte": res_flops / res_bytes}
     else:
         alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12       # FFMA lanes x 2 flop x max SM clock
         dom = ("recon+upsample", (fl["recon"] + fl["upsample"]) * samples, stage[2]) if stage[2] >= stage[1] else ("fir", fl["fir"] * samples, stage[1])
