@@ -79,7 +79,8 @@ __global__ void __launch_bounds__(kRes4Threads)
 resample4_kernel(const RateParams* __restrict__ rates, const float* __restrict__ xw, int xw_pitch,
                  int xw_valid, int k_dn, int c, int want_f16)
 {
-  const RateParams R = rates[blockIdx.z];
+  // rates are stored by ascending d and a CTA's work grows with d: the largest d is dispatched first (short tail)
+  const RateParams R = rates[gridDim.z - 1 - blockIdx.z];
   const int det = blockIdx.y;
   const int d = R.d;
   const int jj_lo = R.jj_lo_fixed;
@@ -105,14 +106,15 @@ resample4_kernel(const RateParams* __restrict__ rates, const float* __restrict__
   float* tp = xsm + (size_t)d * 4 * Q;            // [d][K2], then the last tap
   const int seg = d * (kRes4Out + K2) + 1;
   const int base = d * (jj0 - k_dn);              // xw index of segment element 0
+  const int l2d = 31 - __clz(d);
   for (int i = t; i < seg; i += kRes4Threads) {
     const int gi = base + i;
     const float v = (gi >= 0 && gi < xw_valid) ? x[gi] : 0.f;
-    const int m = i / d, phi = i - m * d;
+    const int m = i >> l2d, phi = i & (d - 1);     // d is a power of two: the division cost as much as the filter itself
     xs4[(phi * 4 + (m & 3)) * Q + (m >> 2)] = v;
   }
   for (int i = t; i < K2 * d + 1; i += kRes4Threads) {
-    const int a = i / d, phi = i - a * d;
+    const int a = i >> l2d, phi = i & (d - 1);
     tp[(a == K2) ? d * K2 : phi * K2 + a] = __ldg(R.taps + i);
   }
   __syncthreads();
