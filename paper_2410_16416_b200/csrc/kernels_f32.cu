@@ -17,6 +17,39 @@ __device__ __forceinline__ u64 pack2(float lo, float hi) { u64 r; asm("mov.b64 %
 __device__ __forceinline__ void unpack2(u64 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ void ffma2(u64& c, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(c) : "l"(a), "l"(b)); }
 
+// Eight consecutive l of one reconstruction row i / one y row r, from the fp32 row-major arrays or (PK: the fp16
+// path's CUDA-core fallback for banks the tensor reconstruction cannot hold) from the packed fp16 operands, where the
+// same eight values are one 16-byte core-matrix row:  R16[p / 128][l / 8][part][p % 128][l % 8] with i = 2 p + part,
+// Y16[r / 128][l / 8][r % 128][l % 8].  l is a multiple of 8.
+__device__ __forceinline__ void h8_to_f(const uint4 v, float4& lo, float4& hi)
+{
+  const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+  const float2 c = __half22float2(*reinterpret_cast<const __half2*>(&v.z)), d = __half22float2(*reinterpret_cast<const __half2*>(&v.w));
+  lo = make_float4(a.x, a.y, b.x, b.y); hi = make_float4(c.x, c.y, d.x, d.y);
+}
+template <bool PK>
+__device__ __forceinline__ void load8_R(const SliceParams& P, int i, int l, float4& lo, float4& hi)
+{
+  if constexpr (PK) {
+    const int p = i >> 1;
+    h8_to_f(__ldg(reinterpret_cast<const uint4*>(P.R16 + ((((size_t)(p >> 7) * (P.L_pad >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8)), lo, hi);
+  } else {
+    const float* __restrict__ R = P.R32 + (size_t)i * P.L_pad + l;
+    lo = __ldg(reinterpret_cast<const float4*>(R)); hi = __ldg(reinterpret_cast<const float4*>(R + 4));
+  }
+}
+template <bool PK>
+__device__ __forceinline__ void load8_Y(const SliceParams& P, int r, int l, float4& lo, float4& hi)
+{
+  if constexpr (PK) {
+    const __half* __restrict__ Yh = reinterpret_cast<const __half*>(P.Y);
+    h8_to_f(*reinterpret_cast<const uint4*>(Yh + (((size_t)(r >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (r & 127)) * 8), lo, hi);
+  } else {
+    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)r * P.L_pad + l;
+    lo = *reinterpret_cast<const float4*>(Y); hi = *reinterpret_cast<const float4*>(Y + 4);
+  }
+}
+
 
 // ------------------------------------------------------------------------------------------------
 // A2  y^s_l[j] = sum_t U^s[l,t] x^s[j - n_s + t]                     ("cross-correlates")
@@ -468,7 +501,8 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
 // ------------------------------------------------------------------------------------------------
 constexpr int LG_T = 128, LG_K = 16, LG_S = LG_T + 4;
 
-__global__ void __launch_bounds__(256)
+template <bool PK>
+__global__ void __launch_bounds__(256, 2)
 lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __restrict__ groups, int c)
 {
   const Q32Group G = groups[blockIdx.z];
@@ -490,12 +524,10 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
 
   for (int s = 0; s < G.n_slices; ++s) {
     const SliceParams P = sp[G.slice[s]];
-    const float* __restrict__ R = P.R32 + (size_t)(row0 + lr) * P.L_pad + lk;
-    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)(j0 + lr) * P.L_pad + lk;
     const bool y_ok = j0 + lr < P.y_rows_cap;
-    float4 a0 = __ldg(reinterpret_cast<const float4*>(R)), a1 = __ldg(reinterpret_cast<const float4*>(R + 4));
-    float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-    if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y); b1 = *reinterpret_cast<const float4*>(Y + 4); }
+    float4 a0, a1, b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+    load8_R<PK>(P, row0 + lr, lk, a0, a1);
+    if (y_ok) load8_Y<PK>(P, j0 + lr, lk, b0, b1);
     for (int l0 = 0; l0 < P.L_pad; l0 += LG_K) {
       __syncthreads();
       As[lk + 0][lc] = a0.x; As[lk + 1][lc] = a0.y; As[lk + 2][lc] = a0.z; As[lk + 3][lc] = a0.w;
@@ -504,8 +536,8 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
       Bs[lk + 4][lc] = b1.x; Bs[lk + 5][lc] = b1.y; Bs[lk + 6][lc] = b1.z; Bs[lk + 7][lc] = b1.w;
       __syncthreads();
       if (l0 + LG_K < P.L_pad) {                     // next chunk, in flight during the multiply
-        a0 = __ldg(reinterpret_cast<const float4*>(R + l0 + LG_K)); a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + LG_K + 4));
-        if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0 + LG_K); b1 = *reinterpret_cast<const float4*>(Y + l0 + LG_K + 4); }
+        load8_R<PK>(P, row0 + lr, l0 + LG_K + lk, a0, a1);
+        if (y_ok) load8_Y<PK>(P, j0 + lr, l0 + LG_K + lk, b0, b1);
       }
 #pragma unroll
       for (int k = 0; k < LG_K; ++k) {
@@ -536,14 +568,15 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
 }
 
 void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_dev, const Q32Group* groups_host, int n_groups,
-                             int max_rows_pad, int c, cudaStream_t st, int64_t* launches)
+                             int max_rows_pad, int c, bool packed16, cudaStream_t st, int64_t* launches)
 {
   int max_cols = 0;
   for (int g = 0; g < n_groups; ++g)
     if (groups_host[g].n_slices) max_cols = std::max(max_cols, (c >> groups_host[g].log2d) + 2 * kKUp);
   if (max_cols == 0) return;
   dim3 grid((max_cols + LG_T - 1) / LG_T, (max_rows_pad + LG_T - 1) / LG_T, n_groups);
-  lowrate_gemm_f32_kernel<<<grid, 256, 0, st>>>(sp_dev, groups_dev, c);
+  if (packed16) lowrate_gemm_f32_kernel<true><<<grid, 256, 0, st>>>(sp_dev, groups_dev, c);
+  else lowrate_gemm_f32_kernel<false><<<grid, 256, 0, st>>>(sp_dev, groups_dev, c);
   ++*launches;
 }
 
@@ -590,6 +623,7 @@ __device__ __forceinline__ void stage_rho(float* __restrict__ rho, const float* 
   }
 }
 
+template <bool PK>
 __global__ void __launch_bounds__(256, 2)
 recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict__ bp,
                    const float* const* __restrict__ upw, const Q32Group* __restrict__ groups,
@@ -624,12 +658,10 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
     const SliceParams P = sp[B.first_slice + s];
     if (P.d != 1) continue;
     const int Lp = P.L_pad;
-    const float* __restrict__ R = P.R32 + (size_t)(row0 + lr) * Lp + lk;
-    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)(kap0 + lr) * Lp + lk;
     const bool y_ok = kap0 + lr < P.y_rows_cap;
-    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 a0 = __ldg(reinterpret_cast<const float4*>(R)), a1 = __ldg(reinterpret_cast<const float4*>(R + 4));
-    float4 b0 = y_ok ? *reinterpret_cast<const float4*>(Y) : z4, b1 = y_ok ? *reinterpret_cast<const float4*>(Y + 4) : z4;
+    float4 a0, a1, b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+    load8_R<PK>(P, row0 + lr, lk, a0, a1);
+    if (y_ok) load8_Y<PK>(P, kap0 + lr, lk, b0, b1);
     for (int l0 = 0; l0 < Lp; l0 += RQ_K) {
       __syncthreads();
       As[(lk + 0) * RQ_S + lc] = a0.x; As[(lk + 1) * RQ_S + lc] = a0.y; As[(lk + 2) * RQ_S + lc] = a0.z; As[(lk + 3) * RQ_S + lc] = a0.w;
@@ -638,8 +670,8 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       Bs[(lk + 4) * RQ_SB + lcb] = b1.x; Bs[(lk + 5) * RQ_SB + lcb] = b1.y; Bs[(lk + 6) * RQ_SB + lcb] = b1.z; Bs[(lk + 7) * RQ_SB + lcb] = b1.w;
       __syncthreads();
       if (l0 + RQ_K < Lp) {                          // next chunk, in flight during the multiply
-        a0 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K)); a1 = __ldg(reinterpret_cast<const float4*>(R + l0 + RQ_K + 4));
-        if (y_ok) { b0 = *reinterpret_cast<const float4*>(Y + l0 + RQ_K); b1 = *reinterpret_cast<const float4*>(Y + l0 + RQ_K + 4); }
+        load8_R<PK>(P, row0 + lr, l0 + RQ_K + lk, a0, a1);
+        if (y_ok) load8_Y<PK>(P, kap0 + lr, l0 + RQ_K + lk, b0, b1);
       }
 #pragma unroll
       for (int k = 0; k < RQ_K; ++k) {
@@ -731,18 +763,23 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
 
 void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int n_bd, int max_rows_pad,
                         const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
-                        int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches)
+                        int max_templates, int c, int64_t k_a, Capture cap, bool packed16, cudaStream_t st, int64_t* launches)
 {
   const size_t smem = sizeof(float) * (RQ_K * RQ_S + RQ_K * RQ_SB + RQ_T * RQ_RHO_S + 16 * 32);
   static bool configured = false;
   if (!configured) {
-    cudaFuncSetAttribute(recon_f32_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(recon_f32_q_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(recon_f32_q_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     configured = true;
   }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
   dim3 grid(n_tiles, (max_rows_pad + RQ_T - 1) / RQ_T, n_bd);
-  recon_f32_q_kernel<<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
-                                             c, (long long)k_a, cap);
+  if (packed16)
+    recon_f32_q_kernel<true><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
+                                                     c, (long long)k_a, cap);
+  else
+    recon_f32_q_kernel<false><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
+                                                      c, (long long)k_a, cap);
   ++*launches;
 }
 

@@ -215,11 +215,11 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     launch_fir_f32(b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, D, o, c, st, &b->last_launches);
     mark(b, st, kTagFir);
     if (b->q32_dev) {
-      launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, st,
+      launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, false, st,
                               &b->last_launches);
       mark(b, st, kTagLowRecon);
       launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
-                         b->max_templates, c, k_a, b->cap, st, &b->last_launches);
+                         b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
     } else {
       launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
                        b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
@@ -233,6 +233,14 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
       if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
                            &b->last_launches, grab(b, kTagLowRecon)))
         return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    } else if (b->q32_dev) {
+      // geometry the tensor reconstruction cannot hold: FFMA kernels of the fp32 path reading the
+      // packed fp16 y and R (3.6x faster than the single fused CUDA-core kernel on the config-4 geometry)
+      launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, true, st,
+                              &b->last_launches);
+      mark(b, st, kTagLowRecon);
+      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+                         b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
     } else {
       launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
                        b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
@@ -523,8 +531,17 @@ int lloid_bank_finalize(lloid_bank_t* b)
   launch_reset_state(b->state, 2 * (int64_t)nstate, 0);
   CU(cudaDeviceSynchronize());
 
-  if (!b->f16) {
-    // fp32 path: one rho^(d) buffer per (bin, detector, low rate), filled by lowrate_gemm_f32_kernel every chunk
+  if (b->f16) {
+    char err[256] = {0};
+    const double* up_w[kMaxRates];
+    for (int l2 = 0; l2 < kMaxRates; ++l2) up_w[l2] = upw64[l2].empty() ? nullptr : upw64[l2].data();
+    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, up_w,
+                                &b->bytes, err, sizeof err);
+    if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
+  }
+  if (!b->f16 || !f16_plan_tensor_recon(b->plan16)) {
+    // fp32 path (and the fp16 path's CUDA-core fallback): one fp32 rho^(d) buffer per (bin, detector, low rate), filled
+    // by lowrate_gemm_f32_kernel every chunk
     b->q32_host.assign((size_t)b->n_bd * kNLowRates, Q32Group());
     bool any = false, fits = true;
     for (int bd = 0; bd < b->n_bd; ++bd) {
@@ -547,14 +564,6 @@ int lloid_bank_finalize(lloid_bank_t* b)
       rc = dev_alloc(b, (void**)&b->q32_dev, b->q32_host.size() * sizeof(Q32Group), false); if (rc) return rc;
       CU(cudaMemcpy(b->q32_dev, b->q32_host.data(), b->q32_host.size() * sizeof(Q32Group), cudaMemcpyHostToDevice));
     }
-  }
-  if (b->f16) {
-    char err[256] = {0};
-    const double* up_w[kMaxRates];
-    for (int l2 = 0; l2 < kMaxRates; ++l2) up_w[l2] = upw64[l2].empty() ? nullptr : upw64[l2].data();
-    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, up_w,
-                                &b->bytes, err, sizeof err);
-    if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
   }
   b->finalized = true;
   return LLOID_OK;

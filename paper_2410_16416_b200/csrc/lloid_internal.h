@@ -94,10 +94,10 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
 // A5/A6: one thread per (bin, detector, template, peak window touched by the chunk); state double-buffered
 // fp32 path, two kernels: low-rate reconstruction GEMM, then d = 1 reconstruction + interpolation + peaks
 void launch_lowrate_gemm_f32(const SliceParams* sp_dev, const Q32Group* groups_dev, const Q32Group* groups_host, int n_groups,
-                             int max_rows_pad, int c, cudaStream_t st, int64_t* launches);
+                             int max_rows_pad, int c, bool packed16, cudaStream_t st, int64_t* launches);
 void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int n_bd, int max_rows_pad,
                         const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
-                        int max_templates, int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches);
+                        int max_templates, int c, int64_t k_a, Capture cap, bool packed16, cudaStream_t st, int64_t* launches);
 
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
                           int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
