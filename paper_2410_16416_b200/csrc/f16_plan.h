@@ -21,6 +21,8 @@ struct F16Plan {
   int fir_list_c[2] = {-1, -1}, fir_list_n[2] = {0, 0};
   // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_recon_kernel) + f0-rate kernel (f0_kernel)
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
+  std::vector<uint8_t> excluded;        // per (bin, detector): 1 = outside the limits, reconstructed by the FFMA kernels
+  bool any_excluded = false;
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
   LowGeom low_geom{};

@@ -757,12 +757,15 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   pl->n_lr = 0;
   for (int l2 = 1; l2 < kMaxRates; ++l2) { lr_of[l2] = -1; if (have[l2]) { lr_of[l2] = pl->n_lr; pl->up[pl->n_lr].log2d = l2; ++pl->n_lr; } }
 
-  bool ok = true;
+  // A (bin, detector) the tensor kernels cannot hold is EXCLUDED from their work lists and reconstructed by the FFMA
+  // kernels (lloid_api.cu); the others stay on the tensor path.
+  pl->excluded.assign(n_bd, 0);
   pl->bd_host.assign(n_bd, BdPlan());
   pl->groups_host.assign((size_t)n_bd * std::max(pl->n_lr, 1), RateGroup());
   pl->combos_host.clear();
   pl->l_sum_f0_max = pl->l_sum_low_max = 0;
-  for (int b = 0; b < n_bd && ok; ++b) {
+  for (int b = 0; b < n_bd; ++b) {
+    bool ok = true;
     BdPlan& B = pl->bd_host[b];
     memset(&B, 0, sizeof B);
     B.n_templates = bp_host[b].n_templates;
@@ -787,11 +790,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
       }
     }
     if (B.n_f0 == 0) ok = false;
-    pl->l_sum_f0_max = std::max(pl->l_sum_f0_max, B.l_sum);
-    for (int r = 0; r < pl->n_lr; ++r) pl->l_sum_low_max = std::max(pl->l_sum_low_max, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
-    for (int rb = 0; rb < B.n_rb; ++rb) pl->combos_host.push_back(F0Combo{b, rb});
+    if (!ok) pl->excluded[b] = 1;
   }
-  if (!ok) return true;                                   // unsupported geometry: CUDA-core fallback
 
   // band matrices P_d (A4):  c[kl] = sum_r Q[ws + r] P[r, kl],  ws = (128 t / d) & ~7, mis = 128 t / d - ws,
   // P[r, kl] = w_phi[i], i = mis + floor(kl / d) + K_up - r in [-K_up, K_up), phi = kl mod d
@@ -838,6 +838,22 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
       if (cnt == 0 || last - first + 1 != cnt) return true;
     }
 
+  // per-bin shared-memory limits: stationary R (single-buffered) + P + 4 ring stages / stationary R + 4 ring stages
+  {
+    const int lim_f0 = (RC16_SMEM_BUDGET - pl->p_bytes - 4 * RC16_STAGE) / 512;
+    const int lim_low = (RC16_SMEM_BUDGET - 4 * RC16_STAGE) / 512;
+    for (int b = 0; b < n_bd; ++b) {
+      if (pl->bd_host[b].l_sum > lim_f0) pl->excluded[b] = 1;
+      for (int r = 0; r < pl->n_lr; ++r)
+        if (pl->groups_host[(size_t)b * pl->n_lr + r].l_sum > lim_low) pl->excluded[b] = 1;
+      if (pl->excluded[b]) { pl->any_excluded = true; continue; }
+      pl->l_sum_f0_max = std::max(pl->l_sum_f0_max, pl->bd_host[b].l_sum);
+      for (int r = 0; r < pl->n_lr; ++r) pl->l_sum_low_max = std::max(pl->l_sum_low_max, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
+      for (int rb = 0; rb < pl->bd_host[b].n_rb; ++rb) pl->combos_host.push_back(F0Combo{b, rb});
+    }
+    if (pl->combos_host.empty()) return true;             // nothing fits: the whole bank goes to the FFMA kernels
+  }
+
   // shared-memory budgets (operands stationary: R of the CTA's template block, and P)
   // R double-buffered (no bubble at a unit switch) when that still leaves >= 8 ring stages
   pl->f0_r_bufs = (RC16_SMEM_BUDGET - 2 * pl->l_sum_f0_max * 512 - pl->p_bytes) / RC16_STAGE >= 8 ? 2 : 1;
@@ -851,7 +867,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   pl->low_smem = low_fixed + pl->low_stages * RC16_STAGE;
   for (int r = 0; r < pl->n_lr; ++r) {                     // per rate class: R as large as its largest group, the rest is ring
     int lmax = 0;
-    for (int b = 0; b < n_bd; ++b) lmax = std::max(lmax, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
+    for (int b = 0; b < n_bd; ++b) if (!pl->excluded[b]) lmax = std::max(lmax, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
     pl->low_geom.r_bytes[r] = lmax * 512;
     pl->low_geom.n_stages[r] = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - lmax * 512) / RC16_STAGE);
     pl->low_smem = std::max(pl->low_smem, lmax * 512 + pl->low_geom.n_stages[r] * RC16_STAGE);
@@ -864,7 +880,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     pl->units_per_rate[r] = 0; pl->low_wsum[r] = 0;
     for (int b = 0; b < n_bd; ++b) {
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
-      if (G.n_slices == 0) continue;
+      if (G.n_slices == 0 || pl->excluded[b]) continue;
       void* q = nullptr;
       if (!plan_alloc(pl, &q, (size_t)G.n_rb * G.q_groups_cap * 4096, true, bytes, err, errlen)) return false;
       G.Q = (__half*)q;
@@ -911,6 +927,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 }
 
 bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
+void f16_plan_disable_tensor_recon(F16Plan* pl) { if (pl) pl->tensor_recon = false; }
+const uint8_t* f16_plan_excluded(const F16Plan* pl) { return (pl && pl->tensor_recon && pl->any_excluded) ? pl->excluded.data() : nullptr; }
 
 int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)

@@ -630,6 +630,7 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
                    Peak* __restrict__ partials, int tiles_cap, int max_templates, int c, long long k_a, Capture cap)
 {
   const int bd = blockIdx.z;
+  if (groups[(size_t)bd * kNLowRates].rows_pad == 0) return;     // mixed fp16 bank: this bin is on the tensor kernels
   const BinParams B = bp[bd];
   const int row0 = blockIdx.y * RQ_T;
   if (row0 >= 2 * B.n_templates) return;

@@ -233,6 +233,12 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
       if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
                            &b->last_launches, grab(b, kTagLowRecon)))
         return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+      if (b->q32_dev) {                              // mixed bank: the bins outside the tensor kernels' limits
+        launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, true, st,
+                                &b->last_launches);
+        launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+                           b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
+      }
     } else if (b->q32_dev) {
       // geometry the tensor reconstruction cannot hold: FFMA kernels of the fp32 path reading the
       // packed fp16 y and R (3.6x faster than the single fused CUDA-core kernel on the config-4 geometry)
@@ -539,7 +545,8 @@ int lloid_bank_finalize(lloid_bank_t* b)
                                 &b->bytes, err, sizeof err);
     if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
   }
-  if (!b->f16 || !f16_plan_tensor_recon(b->plan16)) {
+  const uint8_t* excl = b->f16 ? f16_plan_excluded(b->plan16) : nullptr;   // mixed bank: only these bins use the FFMA kernels
+  if (!b->f16 || !f16_plan_tensor_recon(b->plan16) || excl) {
     // fp32 path (and the fp16 path's CUDA-core fallback): one fp32 rho^(d) buffer per (bin, detector, low rate), filled
     // by lowrate_gemm_f32_kernel every chunk
     b->q32_host.assign((size_t)b->n_bd * kNLowRates, Q32Group());
@@ -550,6 +557,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
         Q32Group& G = b->q32_host[(size_t)bd * kNLowRates + (l2 - 1)];
         memset(&G, 0, sizeof G);
         G.log2d = l2; G.rows_pad = BP.rows_pad; G.q_cols = (int)round_up((C >> l2) + 2 * Ku, 128);
+        if (excl && !excl[bd]) { G.rows_pad = 0; continue; }     // reconstructed by the tensor kernels: both FFMA kernels skip it
         for (int s = 0; s < BP.n_slices; ++s)
           if (b->sp_host[BP.first_slice + s].log2d == l2) {
             if (G.n_slices == kMaxGroupSlices) { fits = false; break; }
@@ -558,11 +566,13 @@ int lloid_bank_finalize(lloid_bank_t* b)
         if (G.n_slices) any = true;
       }
     }
-    if (any && fits) {
+    if ((any || excl) && fits) {
       for (Q32Group& G : b->q32_host)
         if (G.n_slices) { rc = dev_alloc(b, (void**)&G.Q, (size_t)G.rows_pad * G.q_cols * 4, true); if (rc) return rc; }
       rc = dev_alloc(b, (void**)&b->q32_dev, b->q32_host.size() * sizeof(Q32Group), false); if (rc) return rc;
       CU(cudaMemcpy(b->q32_dev, b->q32_host.data(), b->q32_host.size() * sizeof(Q32Group), cudaMemcpyHostToDevice));
+    } else if (excl) {
+      f16_plan_disable_tensor_recon(b->plan16);      // > 8 same-rate slices in an excluded bin: single fused CUDA-core kernel for the bank
     }
   }
   b->finalized = true;

@@ -162,6 +162,8 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
                          int64_t* bytes, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
 bool f16_plan_tensor_recon(const F16Plan*);   // false: bank outside the tensor reconstruction kernels' limits
+void f16_plan_disable_tensor_recon(F16Plan*);
+const uint8_t* f16_plan_excluded(const F16Plan*);   // tensor_recon only: per (bin, detector) flags of the bins left to the FFMA kernels, or null
 int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches);
 int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
