@@ -27,26 +27,38 @@ __device__ __forceinline__ void h8_to_f(const uint4 v, float4& lo, float4& hi)
   const float2 c = __half22float2(*reinterpret_cast<const __half2*>(&v.z)), d = __half22float2(*reinterpret_cast<const __half2*>(&v.w));
   lo = make_float4(a.x, a.y, b.x, b.y); hi = make_float4(c.x, c.y, d.x, d.y);
 }
+// base address of (row i, l) / (y row r, l) and the byte step per 8 l: both layouts are linear in l / 8
 template <bool PK>
-__device__ __forceinline__ void load8_R(const SliceParams& P, int i, int l, float4& lo, float4& hi)
+__device__ __forceinline__ const char* base8_R(const SliceParams& P, int i, int l, int& step)
 {
   if constexpr (PK) {
     const int p = i >> 1;
-    h8_to_f(__ldg(reinterpret_cast<const uint4*>(P.R16 + ((((size_t)(p >> 7) * (P.L_pad >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8)), lo, hi);
+    step = 2 * 128 * 8 * 2;
+    return reinterpret_cast<const char*>(P.R16 + ((((size_t)(p >> 7) * (P.L_pad >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8);
   } else {
-    const float* __restrict__ R = P.R32 + (size_t)i * P.L_pad + l;
-    lo = __ldg(reinterpret_cast<const float4*>(R)); hi = __ldg(reinterpret_cast<const float4*>(R + 4));
+    step = 32;
+    return reinterpret_cast<const char*>(P.R32 + (size_t)i * P.L_pad + l);
   }
 }
 template <bool PK>
-__device__ __forceinline__ void load8_Y(const SliceParams& P, int r, int l, float4& lo, float4& hi)
+__device__ __forceinline__ const char* base8_Y(const SliceParams& P, int r, int l, int& step)
 {
   if constexpr (PK) {
-    const __half* __restrict__ Yh = reinterpret_cast<const __half*>(P.Y);
-    h8_to_f(*reinterpret_cast<const uint4*>(Yh + (((size_t)(r >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (r & 127)) * 8), lo, hi);
+    step = 128 * 8 * 2;
+    return reinterpret_cast<const char*>(reinterpret_cast<const __half*>(P.Y) + (((size_t)(r >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (r & 127)) * 8);
   } else {
-    const float* __restrict__ Y = reinterpret_cast<const float*>(P.Y) + (size_t)r * P.L_pad + l;
-    lo = *reinterpret_cast<const float4*>(Y); hi = *reinterpret_cast<const float4*>(Y + 4);
+    step = 32;
+    return reinterpret_cast<const char*>(reinterpret_cast<const float*>(P.Y) + (size_t)r * P.L_pad + l);
+  }
+}
+template <bool PK, bool NC>
+__device__ __forceinline__ void load8(const char* p, float4& lo, float4& hi)
+{
+  if constexpr (PK) {
+    h8_to_f(NC ? __ldg(reinterpret_cast<const uint4*>(p)) : *reinterpret_cast<const uint4*>(p), lo, hi);
+  } else {
+    const float4* q = reinterpret_cast<const float4*>(p);
+    lo = NC ? __ldg(q) : q[0]; hi = NC ? __ldg(q + 1) : q[1];
   }
 }
 
@@ -526,8 +538,11 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
     const SliceParams P = sp[G.slice[s]];
     const bool y_ok = j0 + lr < P.y_rows_cap;
     float4 a0, a1, b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-    load8_R<PK>(P, row0 + lr, lk, a0, a1);
-    if (y_ok) load8_Y<PK>(P, j0 + lr, lk, b0, b1);
+    int r_step, y_step;
+    const char* Rb = base8_R<PK>(P, row0 + lr, lk, r_step);
+    const char* Yb = base8_Y<PK>(P, j0 + lr, lk, y_step);
+    load8<PK, true>(Rb, a0, a1);
+    if (y_ok) load8<PK, false>(Yb, b0, b1);
     for (int l0 = 0; l0 < P.L_pad; l0 += LG_K) {
       __syncthreads();
       As[lk + 0][lc] = a0.x; As[lk + 1][lc] = a0.y; As[lk + 2][lc] = a0.z; As[lk + 3][lc] = a0.w;
@@ -536,8 +551,9 @@ lowrate_gemm_f32_kernel(const SliceParams* __restrict__ sp, const Q32Group* __re
       Bs[lk + 4][lc] = b1.x; Bs[lk + 5][lc] = b1.y; Bs[lk + 6][lc] = b1.z; Bs[lk + 7][lc] = b1.w;
       __syncthreads();
       if (l0 + LG_K < P.L_pad) {                     // next chunk, in flight during the multiply
-        load8_R<PK>(P, row0 + lr, l0 + LG_K + lk, a0, a1);
-        if (y_ok) load8_Y<PK>(P, j0 + lr, l0 + LG_K + lk, b0, b1);
+        Rb += (LG_K / 8) * r_step; Yb += (LG_K / 8) * y_step;
+        load8<PK, true>(Rb, a0, a1);
+        if (y_ok) load8<PK, false>(Yb, b0, b1);
       }
 #pragma unroll
       for (int k = 0; k < LG_K; ++k) {
@@ -661,8 +677,11 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
     const int Lp = P.L_pad;
     const bool y_ok = kap0 + lr < P.y_rows_cap;
     float4 a0, a1, b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
-    load8_R<PK>(P, row0 + lr, lk, a0, a1);
-    if (y_ok) load8_Y<PK>(P, kap0 + lr, lk, b0, b1);
+    int r_step, y_step;
+    const char* Rb = base8_R<PK>(P, row0 + lr, lk, r_step);
+    const char* Yb = base8_Y<PK>(P, kap0 + lr, lk, y_step);
+    load8<PK, true>(Rb, a0, a1);
+    if (y_ok) load8<PK, false>(Yb, b0, b1);
     for (int l0 = 0; l0 < Lp; l0 += RQ_K) {
       __syncthreads();
       As[(lk + 0) * RQ_S + lc] = a0.x; As[(lk + 1) * RQ_S + lc] = a0.y; As[(lk + 2) * RQ_S + lc] = a0.z; As[(lk + 3) * RQ_S + lc] = a0.w;
@@ -671,8 +690,9 @@ recon_f32_q_kernel(const SliceParams* __restrict__ sp, const BinParams* __restri
       Bs[(lk + 4) * RQ_SB + lcb] = b1.x; Bs[(lk + 5) * RQ_SB + lcb] = b1.y; Bs[(lk + 6) * RQ_SB + lcb] = b1.z; Bs[(lk + 7) * RQ_SB + lcb] = b1.w;
       __syncthreads();
       if (l0 + RQ_K < Lp) {                          // next chunk, in flight during the multiply
-        load8_R<PK>(P, row0 + lr, l0 + RQ_K + lk, a0, a1);
-        if (y_ok) load8_Y<PK>(P, kap0 + lr, l0 + RQ_K + lk, b0, b1);
+        Rb += (RQ_K / 8) * r_step; Yb += (RQ_K / 8) * y_step;
+        load8<PK, true>(Rb, a0, a1);
+        if (y_ok) load8<PK, false>(Yb, b0, b1);
       }
 #pragma unroll
       for (int k = 0; k < RQ_K; ++k) {
