@@ -143,6 +143,9 @@ def make_workload(args, rank=0):
     if args.workload == "config3":                        # batching over bins (A7): the paper's throughput-vs-banks curve
         secs = args.seconds if args.seconds != 4096 else 256
         return wl.config3(n_bins=args.bins, seconds=secs, n_detectors=args.detectors)
+    if args.workload == "config4":                        # heterogeneous L = 100 ... 300 (full-bank geometry, reduced bin count)
+        secs = args.seconds if args.seconds != 4096 else 192
+        return wl.config4(n_bins=args.bins, n_templates=args.templates, seconds=secs, n_detectors=3, n_distinct=2)
     w = wl.config2(n_templates=args.templates, seconds=args.seconds, n_detectors=args.detectors)
     if rank:
         w.strain = wl.make_strain(wl.SEED0 + 2000 + 10 * rank, w.n_detectors, w.n_samples, w.bins, w.injections, 15.0, 1024.0)
@@ -150,6 +153,10 @@ def make_workload(args, rank=0):
 
 
 def workload_name(args):
+    if args.workload == "config4":
+        secs = args.seconds if args.seconds != 4096 else 192
+        return (f"BASELINE config 4 geometry, {args.bins} of 1000 bins x {args.templates} templates (6 slices 2048..64 Hz, M = 64 s, "
+                f"L(b, s) = 100 + ((37 b + 61 s) mod 201)), 3 det x {secs} s")
     if args.workload == "config3":
         secs = args.seconds if args.seconds != 4096 else 256
         return (f"BASELINE config 3 geometry, {args.bins} of 100 BBH-like bins x 500 templates batched "
@@ -406,10 +413,10 @@ def main():
     ap.add_argument("--templates", type=int, default=1000)
     ap.add_argument("--seconds", type=int, default=4096)
     ap.add_argument("--detectors", type=int, default=2)
-    ap.add_argument("--workload", default="config2", choices=["config2", "config3", "config5"],
+    ap.add_argument("--workload", default="config2", choices=["config2", "config3", "config4", "config5"],
                     help="config2: the headline bench line; config3: --bins BBH-like bins batched offline (throughput vs number of "
                          "bins, PAPER.md:96); config5: 1 s streaming buffers on the config-3 bank (p50/p99 latency)")
-    ap.add_argument("--bins", type=int, default=100, help="number of SVD bins batched (--workload config3)")
+    ap.add_argument("--bins", type=int, default=100, help="number of SVD bins batched (--workload config3 / config4: full-bank geometry with heterogeneous L)")
     ap.add_argument("--chunk", type=int, default=0, help="library time-chunk length in samples (0 = automatic)")
     ap.add_argument("--ref-seconds", type=float, default=2.0, help="seconds of output the oracle sample covers")
     args = ap.parse_args()
