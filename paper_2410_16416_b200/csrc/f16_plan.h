@@ -7,8 +7,6 @@
 
 namespace lloid {
 
-struct LowGeom { int32_t r_bytes[kNLowRates], n_stages[kNLowRates]; };   // low-rate kernel, per rate class: bytes of the stationary R, ring stages
-
 struct F16Plan {
   // A2 basis FIR
   int fir_grid_x = 0, fir_smem = 0, fir_stages = 0;
@@ -19,16 +17,15 @@ struct F16Plan {
   std::vector<int2> fir_list_host[2];
   void* fir_list_dev[2] = {nullptr, nullptr};
   int fir_list_c[2] = {-1, -1}, fir_list_n[2] = {0, 0};
-  // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_recon_kernel) + f0-rate kernel (f0_kernel)
+  // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_pair_kernel) + f0-rate kernel (f0_pair_kernel)
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
   std::vector<uint8_t> excluded;        // per (bin, detector): 1 = outside the limits, reconstructed by the FFMA kernels
   bool any_excluded = false;
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
-  LowGeom low_geom{};
-  int f0_smem = 0, f0_stages = 0, f0_r_bufs = 1;
-  int p_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;
-  UpRate up[kNLowRates];
+  int f0_smem = 0, f0_stages = 0;
+  int p_bytes = 0, q_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;   // per CTA: band-matrix blob, rho^(d) window buffers
+  PairRate rate[kNLowRates];
   std::vector<RateGroup> groups_host;   // [n_bd][n_lr]
   std::vector<BdPlan> bd_host;          // [n_bd]
   std::vector<F0Combo> combos_host;     // every (bd, template block)

@@ -153,6 +153,13 @@ resample4_kernel(const RateParams* __restrict__ rates, const float* __restrict__
   }
 }
 
+int configure_common_kernels()              // per device, at finalize (see configure_f32_kernels)
+{
+  cudaError_t e = set_max_dyn_smem(resample_kernel);
+  if (e == cudaSuccess) e = set_max_dyn_smem(resample4_kernel);
+  return e == cudaSuccess ? 0 : 1;
+}
+
 void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
                      const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
                      bool want_f16, cudaStream_t st, int64_t* launches)
@@ -170,11 +177,7 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
   }
   if (!any || max_blocks <= 0) return;
   const size_t smem = sizeof(float) * (size_t)max_d * (kResBlock + 2 * k_dn + 1);
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
-    cudaFuncSetAttribute(resample_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
-  }
+
   if (k_dn % 2 == 0) {                              // register-tiled kernel: 512 outputs per CTA
     int blocks4 = 0;
     for (int r = 0; r < n_rates; ++r) {
@@ -185,11 +188,6 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
     }
     const int Q = (kRes4Out + 2 * k_dn) / 4 + 1;
     const size_t smem4 = sizeof(float) * ((size_t)max_d * 4 * Q + (size_t)max_d * 2 * k_dn + 4);
-    static size_t configured4 = 0;
-    if (smem4 > 48 * 1024 && smem4 > configured4) {
-      cudaFuncSetAttribute(resample4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem4);
-      configured4 = smem4;
-    }
     dim3 grid4(blocks4, n_det, n_rates);
     resample4_kernel<<<grid4, kRes4Threads, smem4, st>>>(rates_dev, xw, xw_pitch, xw_valid, k_dn, c, want_f16 ? 1 : 0);
     ++*launches;
@@ -212,7 +210,7 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
-                     int tiles_cap, int c, long long k_a, int W, float theta,
+                     int slots_cap, const int32_t* __restrict__ slot_tiles, int c, long long k_a, int W, float theta,
                      const PeakState* __restrict__ state_in, PeakState* __restrict__ state_out, int n_det,
                      lloid_trigger_t* __restrict__ trig, long long capacity, unsigned long long* __restrict__ count)
 {
@@ -228,8 +226,12 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
   PeakState s;
   if (w * W < k_a) s = state_in[(size_t)bd * max_templates + p];      // window began in an earlier chunk
   else { s.q = -1.f; s.re = 0.f; s.im = 0.f; s.pad = 0; s.k = -1; }
-  const int g0 = (int)((lo - k_a) / kTimeTile), g1 = (int)((hi - k_a + kTimeTile - 1) / kTimeTile);
-  const Peak* __restrict__ pp = partials + ((size_t)bd * tiles_cap + g0) * max_templates + p;
+  // partial slots: runs of gt tiles aligned to absolute multiples of gt tiles (gt = 1: one slot per tile)
+  const int gt = slot_tiles ? slot_tiles[bd] : 1;
+  const long long a0 = k_a / kTimeTile;
+  const int t_lo = (int)((lo - k_a) / kTimeTile), t_hi = (int)((hi - k_a + kTimeTile - 1) / kTimeTile);   // tiles [t_lo, t_hi)
+  const int g0 = (int)((a0 + t_lo) / gt - a0 / gt), g1 = (int)((a0 + t_hi - 1) / gt - a0 / gt) + 1;
+  const Peak* __restrict__ pp = partials + ((size_t)bd * slots_cap + g0) * max_templates + p;
   for (int g = g0; g < g1; g += 8) {               // 8 independent 16-byte loads in flight per thread, then the ordered compare
     float4 v[8];
 #pragma unroll
@@ -257,13 +259,13 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
 }
 
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                          int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
-                          PeakState* state_out, int n_det, void* triggers, int64_t capacity,
+                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, int W, float theta,
+                          const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
                           unsigned long long* count, cudaStream_t st, int64_t* launches)
 {
   const int n_w = (int)((k_a + c - 1) / W - k_a / W) + 1;
   dim3 grid((max_templates + 127) / 128, n_bd, n_w);
-  merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, tiles_cap, c, (long long)k_a, W,
+  merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, slots_cap, slot_tiles_dev, c, (long long)k_a, W,
                                             theta, state_in, state_out, n_det, (lloid_trigger_t*)triggers,
                                             (long long)capacity, count);
   ++*launches;

@@ -12,8 +12,8 @@
 // each, mbarrier pipeline); MT time tiles of 128 rows share every U stage (MT accumulators in TMEM).
 //
 // Warp roles (192 threads): warp 0 = bulk-copy producer, warp 1 = MMA issuer, warps 2-5 = epilogue
-// (TMEM -> registers -> fp16 -> Y, packed in the Y16 layout of lloid_internal.h that the reconstruction
-// kernels fetch with 1-D bulk copies as an MMA operand).
+// (TMEM -> registers -> fp16 -> Y, packed in the Y16 layout of lloid_internal.h (64-row tiles) that the
+// reconstruction kernels fetch with 1-D bulk copies as an MMA operand).
 #include "f16_plan.h"
 #include "tc05.cuh"
 
@@ -156,7 +156,7 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     const size_t lgs = (size_t)(L_pad >> 3);
     for (int mt = 0; mt < mt_used; ++mt) {
       const int row = r0 + mt * 128 + q * 32 + lane;
-      __half* __restrict__ Yt = Y + ((size_t)(row >> 7) * lgs * 128 + (row & 127)) * 8;   // Y16[tile][lc][row % 128][8]
+      __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
       for (int c0 = 0; c0 < L_pad; c0 += 16) {
         uint32_t v[16];
@@ -170,8 +170,8 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
             h[i] = *reinterpret_cast<const uint32_t*>(&p);
           }
           const size_t lc = (size_t)(c0 >> 3);
-          *reinterpret_cast<uint4*>(Yt + lc * 1024) = make_uint4(h[0], h[1], h[2], h[3]);
-          *reinterpret_cast<uint4*>(Yt + (lc + 1) * 1024) = make_uint4(h[4], h[5], h[6], h[7]);
+          *reinterpret_cast<uint4*>(Yt + lc * 512) = make_uint4(h[0], h[1], h[2], h[3]);
+          *reinterpret_cast<uint4*>(Yt + (lc + 1) * 512) = make_uint4(h[4], h[5], h[6], h[7]);
         }
       }
     }
@@ -354,7 +354,7 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
       fence_after();
       for (int mt = 0; mt < U.mt_used; ++mt) {
         const int row = U.r0 + mt * 128 + q * 32 + lane;
-        __half* __restrict__ Yt = Y + ((size_t)(row >> 7) * lgs * 128 + (row & 127)) * 8;   // Y16[tile][lc][row % 128][8]
+        __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
         for (int c0 = 0; c0 < L_pad; c0 += 32) {
           uint32_t v[32];
@@ -369,7 +369,7 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
                 const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * g + 2 * i]), __uint_as_float(v[8 * g + 2 * i + 1]));
                 h[i] = *reinterpret_cast<const uint32_t*>(&p2);
               }
-              *reinterpret_cast<uint4*>(Yt + ((size_t)(c0 >> 3) + g) * 1024) = make_uint4(h[0], h[1], h[2], h[3]);
+              *reinterpret_cast<uint4*>(Yt + ((size_t)(c0 >> 3) + g) * 512) = make_uint4(h[0], h[1], h[2], h[3]);
             }
           }
         }
@@ -431,7 +431,7 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
       const int rows = (P.d == 1) ? chunk_cap : (chunk_cap >> P.log2d) + 2 * kKUp;
       cap_units += (size_t)(rows + 128 * mt - 1) / (128 * mt);
     }
-    bool ok = cudaFuncSetAttribute(fir_f16_pers_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_pers_smem) == cudaSuccess;
+    bool ok = set_max_dyn_smem(fir_f16_pers_kernel) == cudaSuccess;
     for (int k = 0; k < 2 && ok; ++k) {
       void* d = nullptr;
       ok = cudaMalloc(&d, (cap_units + 1) * sizeof(int2)) == cudaSuccess;
@@ -439,7 +439,7 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
     }
     pl->fir_pers = ok;
   }
-  cudaError_t e = cudaFuncSetAttribute(fir_f16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->fir_smem);
+  cudaError_t e = set_max_dyn_smem(fir_f16_kernel);
   if (e != cudaSuccess) { snprintf(err, errlen, "cudaFuncSetAttribute(fir_f16_kernel, %d): %s", pl->fir_smem, cudaGetErrorString(e)); delete pl; return nullptr; }
   if (!f16_plan_build_recon(pl, sp_host, n_problems, bp_host, n_bd, chunk_cap, up_w, bytes, err, errlen)) {
     f16_plan_destroy(pl);

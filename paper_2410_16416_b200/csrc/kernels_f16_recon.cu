@@ -2,29 +2,32 @@
 // tcgen05 tensor cores (include/lloid.h A3-A5; "matrix multiplication of the orthogonal SNR time
 // series with SVD coefficients, and finally up-samples and sums the physical SNR segments").
 //
-// Two persistent kernels per chunk (one CTA per SM, static cost-balanced (unit, tile) ranges: SchedArgs), built from
-// the same pieces: single-thread producer / MMA-issuer roles inside `if (elect_one())`, rings of 8 KB operand stages
-// filled by 1-D bulk copies, two TMEM accumulator buffers of 2 x 128 columns so the epilogue of tile t overlaps the
-// MMAs of tile t + 1:
+// Round-2 design: CTA PAIRS.  Both kernels run as 2-CTA clusters (one cluster per SM pair, persistent, static
+// cost-balanced schedule) and issue cta_group::2 MMAs with M = 256: every CTA owns 128 reconstruction ROWS in their
+// natural order (row 2p = cosine, 2p + 1 = sine of template p: 64 templates per CTA, 128 per pair) and HALF of every
+// B operand (64 of the 128 time samples of a y tile, 64 of the 128 output columns of a band matrix).  Compared with
+// the round-1 kernels (one CTA = 128 templates x 2 accumulators) every per-CTA byte count halves: the stationary R
+// (40 KB for L = 160, so L up to 512 and several full-rate slices fit), the y stages, the rho^(d) chunks -- which is
+// what buys (a) rings deep enough to cover the memory latency and (b) room to KEEP the rho^(d) windows of consecutive
+// tiles in shared memory, so each low-rate sample is fetched once instead of once per overlapping window
+// (14 -> 7.75 sixteen-row chunks per tile on BASELINE config 2).
 //
-//  lowrate_recon_kernel   rho^(d)[i, j] = sum_{slices s at rate d} sum_l R^s[i, l] y^s_l[j]     (d > 1)
-//      A = R^s (stationary in shared memory for the CTA's 128 templates), B = y^s tiles streamed by two alternating
-//      producer threads, D[lane = template, column = low-rate time].  Slices that share a rate are summed BEFORE
-//      upsampling (A4 is linear and its kernel depends only on d).  Output Q16: fp16 at the LOW rate, already in
-//      the core-matrix layout in which the f0 kernel consumes it as an MMA operand.  The dense f0-rate SNR is
-//      never written anywhere.
+//  lowrate_pair_kernel   rho^(d)[i, j] = sum_{slices s at rate d} sum_l R^s[i, l] y^s_l[j]     (d > 1)
+//      A = R^s (stationary), B = y^s tiles (ring), D[lane = row, column = low-rate time], four TMEM accumulators of
+//      128 columns; epilogue -> fp16 -> Q16, already in the core-matrix layout the f0 kernel consumes as an A operand.
 //
-//  f0_kernel   rho[i, k] = sum_{d = 1 slices} R^s y^s  +  sum_{d > 1} rho^(d)[i, window(k)] P_d      then A5
-//      The interpolation A4 is itself a tensor-core contraction with the fixed band matrix
-//      P_d[r, kl] = d lp_{d,K_up}[...] (16 non-zeros per column), restricted per 16-row chunk to the output
-//      columns its band touches.  Cosine and sine rows of a template go to two accumulators (columns
-//      [0,128) and [128,256)) of the SAME TMEM lane, so one epilogue thread owns one template: |rho|^2 and
-//      the running maximum over time need no cross-lane traffic at all.  Five single-thread roles on two rings
-//      (see the comment above f0_kernel).
+//  f0_pair_kernel   rho[i, k] = sum_{d = 1 slices} R^s y^s  +  sum_{d > 1} rho^(d)[i, window(k)] P_d      then A5
+//      The interpolation A4 is a tensor-core contraction with the fixed band matrix P_d (16 non-zeros per column),
+//      restricted per 16-row chunk to the columns its band touches.  The rho^(d) windows live in per-rate circular
+//      buffers: per tile only the rows that entered the window are fetched (one barrier per tile for all rates).
+//      Epilogue: a thread owns one ROW (lane); the cosine and sine rows of a template sit in adjacent lanes of one warp
+//      and swap half of their columns with one shuffle per column pair; |rho|^2, the running first maximum over a
+//      peak-window GRANULE (up to W / 128 tiles) -> ONE 16-byte partial per (template, granule).  The dense f0-rate
+//      SNR never leaves TMEM.
 //
-// A single thread retires about one instruction per 7 cycles: per-stage instruction counts of the role loops are
-// what bounds the pipeline once the data is there, so the loops carry incrementing ring / pointer / descriptor
-// state (no division, no 64-bit descriptor rebuild) and read per-unit tables from shared memory.
+// Pair plumbing (measured on B200, see tc05.cuh): only the leader CTA issues MMAs; tcgen05.commit multicasts "stage
+// free" / "accumulator full" to both CTAs; the peer CTA's loads complete on the peer's own barriers and one relay thread
+// per stream forwards "my half has landed" to the leader with a remote arrive.
 #include "f16_plan.h"
 #include "tc05.cuh"
 
@@ -37,22 +40,22 @@ namespace lloid {
 
 using namespace tc;
 
-constexpr int RC16_STAGE = 8192;            // bytes per ring stage: one K = 32 (y) or K = 16 (rho^(d)) operand chunk
-constexpr int RC16_MAX_STAGES = 16;
-constexpr int RC16_SMEM_BUDGET = 219 * 1024;     // + 7 KB static (barriers, tables, epilogue exchange) = 226 of 227 KB
+constexpr int PK_THREADS = 512;             // 16 warps: 0 PY, 1 IY, 2 PQ, 3 IQ, 4 relay y, 5 relay q, 8-15 epilogue
+constexpr int PK_YSTAGE = 8192;             // bytes per y ring stage per CTA: K = 64 x 64 rows
+constexpr int PK_NSY_MAX = 16;
+constexpr int PK_NACC = 4;                  // accumulator buffers of 128 columns
+constexpr int PK_NQB = 4;                   // rho^(d) tile events in flight (barrier slots)
+constexpr int PK_QDIST = 2;                 // the rows of tile e are requested when tile e - PK_QDIST has been consumed
+constexpr int PK_SMEM_BUDGET = 220 * 1024;  // dynamic; + static (barriers, tables) stays below 227 KB
 
-struct LowUnit { int32_t group, rb; };
-
-struct RingBars {
-  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES], acc_full[2], acc_empty[2], consts, unit_done;
-};
+struct LowUnit { int32_t group, pb; };
 
 struct Ring {                               // stage index + phase parity, advanced without division
   int s; uint32_t ph; int n;
   __device__ __forceinline__ void advance() { if (++s == n) { s = 0; ph ^= 1u; } }
 };
 
-// ---- static persistent schedule (SchedArgs in lloid_internal.h) ------------------------------------
+// ---- static persistent schedule (SchedArgs in lloid_internal.h), per CLUSTER --------------------------
 struct SchedPos { int u, t; };              // unit index, first tile
 
 __device__ __forceinline__ SchedPos sched_locate(const SchedArgs& s, long long b)
@@ -73,15 +76,6 @@ __device__ __forceinline__ SchedPos sched_locate(const SchedArgs& s, long long b
   return r;
 }
 
-// this CTA's range -> rng[0..3] = first unit, first tile, last unit, end tile in the last unit
-__device__ __forceinline__ void sched_range(const SchedArgs& s, int* rng)
-{
-  const long long T = s.cls_base[s.n_cls];
-  const SchedPos a = sched_locate(s, T * (long long)blockIdx.x / (long long)gridDim.x);
-  const SchedPos b = sched_locate(s, T * (long long)(blockIdx.x + 1) / (long long)gridDim.x);
-  rng[0] = a.u; rng[1] = a.t; rng[2] = b.u; rng[3] = b.t;
-}
-
 __device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
 {
   int c = 0;
@@ -89,17 +83,32 @@ __device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
   return c;
 }
 
-__device__ __forceinline__ void ring_setup(RingBars& B, uint32_t* tmem_slot, int n_stages, int warp, int tid, int n_epilogue_threads)
+// A range boundary inside a unit is moved up to the next granule start (tiles whose absolute index is a multiple of
+// gt; gt = 1: no snapping): both ends of every range use the same rule, so the ranges still tile the work.
+__device__ __forceinline__ SchedPos sched_snap(const SchedArgs& s, SchedPos p, long long a0, int gt)
 {
-  if (warp == 0) tmem_alloc(tmem_slot, 512);
-  if (tid == 32) {
-    for (int s = 0; s < n_stages; ++s) { mbar_init(smem_u32(&B.full[s]), 1); mbar_init(smem_u32(&B.empty[s]), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), n_epilogue_threads); }
-    mbar_init(smem_u32(&B.consts), 1);
-    mbar_init(smem_u32(&B.unit_done), 1);
-    mbar_init_fence();
-  }
+  if (gt <= 1 || p.t == 0 || p.u >= s.cls_begin[s.n_cls]) return p;
+  const int nt = s.n_tiles[sched_class(s, p.u)];
+  const int rem = (int)((a0 + p.t) % gt);
+  if (rem) p.t += gt - rem;
+  if (p.t >= nt) { ++p.u; p.t = 0; }
+  return p;
 }
+
+// this cluster's range -> rng[0..3] = first unit, first tile, last unit, end tile in the last unit
+__device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl, long long a0, int gt, int* rng)
+{
+  const long long T = s.cls_base[s.n_cls];
+  const SchedPos a = sched_snap(s, sched_locate(s, T * (long long)cid / (long long)ncl), a0, gt);
+  const SchedPos b = sched_snap(s, sched_locate(s, T * (long long)(cid + 1) / (long long)ncl), a0, gt);
+  rng[0] = a.u; rng[1] = a.t; rng[2] = b.u; rng[3] = b.t;
+}
+
+#define FOR_SEGMENTS(u, t0, t1, NT)                                                               \
+  for (int u = u_lo; u <= u_hi; ++u)                                                              \
+    if (u == u_hi && t_hi == 0) break;                                                            \
+    else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : (NT); t0 >= t1) continue; \
+    else
 
 __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, uint32_t bytes, uint32_t bar)
 {
@@ -109,618 +118,543 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
   }
 }
 
-// The producer and the MMA issuer each run as ONE elected thread inside `if (elect_one())`: ptxas recognises the
-// elect.sync-guarded region as single-threaded and keeps the whole loop (ring state, descriptors, barrier
-// addresses) in uniform registers -- about 25 SASS instructions per 4-MMA stage, no R2UR at all.  (A per-lane
-// predicate on the issuing instruction instead costs an ELECT + R2UR.BROADCAST waterfall per MMA: measured
-// ~450 issue cycles per stage, which bounded both kernels.)
-// producer: wait for the slot to be free, then one 8 KB bulk copy
-__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src)
-{
-  mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
-  mbar_expect_tx(bars_full + 8u * rg.s, RC16_STAGE);
-  bulk_g2s(ring_base + (uint32_t)rg.s * RC16_STAGE, src, RC16_STAGE, bars_full + 8u * rg.s);
-  rg.advance();
-}
-
-// one K = 32 chunk of a reconstruction: D[part] (+)= R[l-groups g .. g + 3][part] * stage^T, N = 128.
-// a_lo: descriptor of (group g, part 0) with LBO 4096; b_lo: descriptor of the stage with LBO 2048 (16-byte units)
-__device__ __forceinline__ void mma_recon_chunk(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t first)
-{
-  mma_ss(d_tmem,        desc64(a_lo),        desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss(d_tmem,        desc64(a_lo + 512u), desc64(b_lo + 256u), idesc, 1u);
-  mma_ss(d_tmem + 128u, desc64(a_lo + 128u), desc64(b_lo),        idesc, first ? 0u : 1u);
-  mma_ss(d_tmem + 128u, desc64(a_lo + 640u), desc64(b_lo + 256u), idesc, 1u);
-}
-
-// ------------------------------------------------------------------------------------------------
-struct SegLow {                             // per-role copy of the current unit's operand sources
-  const uint8_t* Y[kMaxGroupSlices];
-  const uint8_t* Rsrc[kMaxGroupSlices];
-  int L[kMaxGroupSlices];
+struct PairBars {
+  uint64_t yfull[PK_NSY_MAX], yempty[PK_NSY_MAX];
+  uint64_t qfull[PK_NQB], qempty[PK_NQB];
+  uint64_t acc_full[PK_NACC], acc_empty[PK_NACC], ybar[PK_NACC];
+  uint64_t consts, unit_done;
 };
 
-__device__ __forceinline__ void seg_low_fill(SegLow& S, const SliceParams* __restrict__ sp, const RateGroup* __restrict__ G, int rb)
+// Barrier counts: a "full" barrier of the leader gets two arrivals (its own producer's arrive.expect_tx and the peer's
+// relay), the peer's own copy one.  acc_empty lives in the leader: one arrival per epilogue warp of both CTAs.
+__device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int nsy, uint32_t rank, int warp, int tid)
 {
-  for (int i = 0; i < G->n_slices; ++i) {               // one thread
-    const SliceParams* P = sp + G->slice[i];
-    const int L = P->L_pad;
-    S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
-    S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 512;
-    S.L[i] = L;
-  }
-}
-
-// Persistent: CTA i of gridDim.x runs cost range i of the (rate, unit, tile) sequence (SchedArgs).  At a unit
-// switch the producer first refills the ring with the next unit's y tiles, then waits for the previous unit's
-// last accumulator (all MMAs that read the old R are complete) and only then replaces R: the bubble is one R load.
-constexpr int LOW_THREADS = 352;             // warps: 0 producer A (+R), 1 MMA issuer, 2-5 epilogue (cos rows), 6 producer B,
-                                             // 7-10 epilogue (sin rows): the TMEM -> fp16 -> rho^(d) pass was the slowest stage
-
-__global__ void __launch_bounds__(LOW_THREADS, 1)
-lowrate_recon_kernel(const SliceParams* __restrict__ sp, const RateGroup* __restrict__ groups,
-                     const LowUnit* __restrict__ units, const __grid_constant__ SchedArgs sched, const __grid_constant__ LowGeom geom)
-{
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) RingBars bars;
-  __shared__ __align__(8) uint64_t cfull[kNLowRates][RC16_MAX_STAGES], cempty[kNLowRates][RC16_MAX_STAGES], class_go[kNLowRates];
-  __shared__ uint32_t tmem_slot;
-  __shared__ SegLow seg[3];                             // [0], [2] the producers', [1] MMA issuer's
-  __shared__ int s_rng[4];
-
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) sched_range(sched, s_rng);
-  __syncthreads();
-  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
-  if (u_lo == u_hi && t_lo == t_hi) return;
-
-  ring_setup(bars, &tmem_slot, 0, warp, tid, 256);
-  if (tid == 64) {                                      // one ring barrier set per rate class: a CTA visits a class once, and the
-    for (int cidx = 0; cidx < kNLowRates; ++cidx) {     // ring geometry (R size, stage count) differs between classes
-      for (int st = 0; st < RC16_MAX_STAGES; ++st) { mbar_init(smem_u32(&cfull[cidx][st]), 1); mbar_init(smem_u32(&cempty[cidx][st]), 1); }
-      mbar_init(smem_u32(&class_go[cidx]), 1);
+  if (warp == 0) tmem_alloc2(tmem_slot, 512);
+  if (tid == 32) {
+    const uint32_t nfull = rank == 0 ? 2u : 1u;
+    for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), nfull); mbar_init(smem_u32(&B.yempty[s]), 1); }
+    for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), nfull); mbar_init(smem_u32(&B.qempty[s]), 1); }
+    for (int b = 0; b < PK_NACC; ++b) {
+      mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 16); mbar_init(smem_u32(&B.ybar[b]), 1);
     }
+    mbar_init(smem_u32(&B.consts), nfull);
+    mbar_init(smem_u32(&B.unit_done), 1);
     mbar_init_fence();
   }
   fence_before();
   __syncthreads();
+  cluster_sync();
   fence_after();
-  const uint32_t tmem = tmem_slot;
-  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][2][128][8] fp16, then the class's ring
+}
 
-  if (warp == 0 || warp == 6) {
-    // ===== producers: two elected threads fill alternate stages of the ring (one thread sustains ~1 instruction per
-    // 7 cycles: a single producer is slower than the MMAs it feeds); warp 0 also owns R =====
-    if (elect_one()) {
-    const int pr = warp == 0 ? 0 : 1;
-    SegLow& sg = seg[2 * pr];
-    Ring rg{0, 0u, 1};
-    int own = pr == 0;
-    int seg_i = 0, cur_cls = -1;                        // segments done so far by this CTA
-    uint32_t bfull = 0, bempty = 0, ring_u = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int cls = sched_class(sched, u);
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
-      if (t0 >= t1) continue;
-      const LowUnit un = units[u];
-      const RateGroup* G = groups + un.group;
-      seg_low_fill(sg, sp, G, un.rb);
-      const int ns_u = G->n_slices;
-      const uint32_t rbytes_u = (uint32_t)G->l_sum * 512u;
-      const bool new_cls = cls != cur_cls;
-      if (new_cls) {                                    // other ring geometry: start its ring (and its barrier set) afresh
-        cur_cls = cls;
-        rg = Ring{0, 0u, geom.n_stages[cls]}; own = pr == 0;
-        bfull = smem_u32(&cfull[cls][0]); bempty = smem_u32(&cempty[cls][0]); ring_u = sR_u + (uint32_t)geom.r_bytes[cls];
-        // the new ring overlaps the old R / ring: nothing may be written before the previous unit is complete
-        if (pr != 0 && seg_i > 0) mbar_wait(smem_u32(&class_go[cls]), 0u);
-      }
-      const int n_stages = geom.n_stages[cls];
-      int countdown = (seg_i == 0 || new_cls) ? 0 : n_stages;      // ring stages to push before R is replaced
-      bool r_done = pr != 0;
-      auto load_R = [&]() {
-        // every MMA that reads the old R is complete.  (A parity wait on acc_full is not usable here: with short tiles the
-        // producer runs several accumulator phases ahead and the parity would alias; this barrier is at most one phase away.)
-        if (seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(seg_i - 1) & 1u);
-        if (new_cls && seg_i > 0) mbar_arrive(smem_u32(&class_go[cls]));      // producer B may start on the new ring
-        {
-          mbar_expect_tx(smem_u32(&bars.consts), rbytes_u);
-          uint32_t off = 0;
-          for (int i = 0; i < ns_u; ++i) {
-            copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.L[i] * 512u, smem_u32(&bars.consts));
-            off += (uint32_t)sg.L[i] * 512u;
-          }
-        }
-        r_done = true;
-      };
-      if (!r_done && countdown == 0) load_R();
-      for (int t = t0; t < t1; ++t)
-        for (int i = 0; i < ns_u; ++i) {
-          const int L = sg.L[i];
-          const uint8_t* src = sg.Y[i] + (size_t)t * L * 256;          // tiles are contiguous in Y16
-          for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-            if (own) produce(rg, bfull, bempty, ring_u, src); else rg.advance();
-            own ^= 1;
-            if (!r_done && --countdown == 0) load_R();
-          }
-        }
-      if (!r_done) load_R();
-      ++seg_i;
-    }
-    }
-  } else if (warp == 1) {
-    // ===== MMA issuer: one elected thread =====
-    if (elect_one()) {
-    const uint32_t idesc = idesc_f16(128, 128);
-    const uint32_t a_base = desc_lo(sR_u, 4096u);
-    const uint32_t tm = tmem;
-    Ring rg{0, 0u, 1};
-    int cur_cls = -1;
-    uint32_t bfull = 0, bempty = 0, b_base = 0;
-    uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
-    int buf = 0, seg_i = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int cls = sched_class(sched, u);
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
-      if (t0 >= t1) continue;
-      const LowUnit un = units[u];
-      const RateGroup* G = groups + un.group;
-      seg_low_fill(seg[1], sp, G, un.rb);
-      const int ns_u = G->n_slices;
-      if (cls != cur_cls) {
-        cur_cls = cls;
-        rg = Ring{0, 0u, geom.n_stages[cls]};
-        bfull = smem_u32(&cfull[cls][0]); bempty = smem_u32(&cempty[cls][0]);
-        b_base = desc_lo(sR_u + (uint32_t)geom.r_bytes[cls], 2048u);
-      }
-      mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
-      fence_after();
-      for (int t = t0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
-        fence_after();
-        const uint32_t d_tmem = tm + (uint32_t)(buf * 256);
-        uint32_t first = 1u, a_lo = a_base;
-        for (int i = 0; i < ns_u; ++i) {
-          const int n_kc = seg[1].L[i] >> 5;
-          for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-            mbar_wait(bfull + 8u * rg.s, rg.ph);
-            fence_after();
-            mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc, first);
-            commit(bempty + 8u * rg.s);
-            first = 0u;
-            rg.advance();
-          }
-        }
-        commit(smem_u32(&bars.acc_full[buf]));
-      }
-      commit(smem_u32(&bars.unit_done));
-      ++seg_i;
-    }
-    }
-  } else {
-    // ===== epilogue: warps 2-5 convert the cosine accumulator, warps 7-10 the sine one (lane quarter = warp % 4) =====
-    const int q = warp & 3;
-    const int pl = q * 32 + lane;
-    const int part = warp >= 7 ? 1 : 0;
-    uint32_t fph = 0u;
-    int buf = 0;
-    for (int u = u_lo; u <= u_hi; ++u) {
-      if (u == u_hi && t_hi == 0) break;
-      const int cls = sched_class(sched, u);
-      const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : sched.n_tiles[cls];
-      if (t0 >= t1) continue;
-      const LowUnit un = units[u];
-      const RateGroup* Gp = groups + un.group;
-      __half* __restrict__ Q = Gp->Q;
-      const int q_cap = Gp->q_groups_cap;
-      for (int t = t0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
-        fence_after();
-        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
-#pragma unroll 1
-          for (int c0 = 0; c0 < 128; c0 += 32) {
-            uint32_t v[32];
-            tmem_ld32(taddr + (uint32_t)(part * 128 + c0), v);
-            tmem_ld_wait();
-#pragma unroll
-            for (int gq = 0; gq < 4; ++gq) {
-              uint32_t h[4];
-#pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const __half2 p2 = __floats2half2_rn(__uint_as_float(v[8 * gq + 2 * e]), __uint_as_float(v[8 * gq + 2 * e + 1]));
-                h[e] = *reinterpret_cast<const uint32_t*>(&p2);
-              }
-              const int jg = t * 16 + (c0 >> 3) + gq;
-              if (jg < q_cap)
-                *reinterpret_cast<uint4*>(Q + ((((size_t)un.rb * q_cap + jg) * 2 + part) * 128 + pl) * 8) =
-                    make_uint4(h[0], h[1], h[2], h[3]);
-            }
-          }
-        fence_before();
-        mbar_arrive(smem_u32(&bars.acc_empty[buf]));
-      }
-    }
-  }
+__device__ __forceinline__ void pair_teardown(uint32_t tmem, int warp)
+{
   fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 512);
+  cluster_sync();                           // the peer may still be reading accumulators this CTA's commit announced
+  if (warp == 0) tmem_dealloc2(tmem, 512);
+}
+
+// producer: wait for the slot to be free, then one bulk copy of `bytes` (<= PK_YSTAGE)
+__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src, uint32_t bytes)
+{
+  mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
+  mbar_expect_tx(bars_full + 8u * rg.s, bytes);
+  bulk_g2s(ring_base + (uint32_t)rg.s * PK_YSTAGE, src, bytes, bars_full + 8u * rg.s);
+  rg.advance();
+}
+
+// One y stage (K = ks, a multiple of 16, <= 64) of a reconstruction: D (+)= R[l-groups from a_lo] * stage^T, N = 128.
+// a_lo: descriptor of R at this K offset (LBO 2048: 128 rows per l-group); b_lo: descriptor of the stage (LBO 1024: 64 rows)
+__device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, int ks, uint32_t& first)
+{
+  for (int k16 = 0; k16 < (ks >> 4); ++k16) {
+    mma2_ss(d_tmem, desc64(a_lo + (uint32_t)k16 * 256u), desc64(b_lo + (uint32_t)k16 * 128u), idesc, first ? 0u : 1u);
+    first = 0u;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
-struct F0Args {
-  const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups; const uint8_t* P;
-  Peak* partials; Capture cap; long long k_a;
-  int n_lr, c, r_bytes, r_bufs, tiles_cap, max_templates, nsy, nsq, p_bytes;
-  SchedArgs sched;                                      // units = combos, one class
-  UpRate up[kNLowRates];
-  QItem item[kNLowRates][2][8];                         // per rate and variant: the active 16-row chunks, in order (kernel
-  int32_t n_items[kNLowRates][2];                       // parameters: read with uniform loads); QItem.ch = chunk index
+struct SegSrc {                             // per-role copy of the current unit's operand sources (this CTA's halves)
+  const uint8_t* Y[kMaxGroupSlices];        // slice's Y16 base
+  const uint8_t* Rsrc[kMaxGroupSlices];     // this CTA's 128-row block of the slice's R16
+  int L[kMaxGroupSlices];
+  int n;
 };
 
-struct SegF0 {                                          // per-role copy of the current unit's operand sources
-  const uint8_t* Y[kMaxF0Slices];
-  const uint8_t* Rsrc[kMaxF0Slices];
-  int L[kMaxF0Slices];
-  const uint8_t* Q[kNLowRates];                         // this template block's rho^(d), or null
-};
-
-__device__ __forceinline__ void seg_f0_fill(SegF0& S, const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B)
+__device__ __forceinline__ void seg_fill(SegSrc& S, const SliceParams* __restrict__ sp, const int32_t* slice, int n, int rb)
 {
-  for (int i = 0; i < B->n_f0; ++i) {                   // one thread
-    const SliceParams* P = a.sp + B->f0_slice[i];
+  S.n = n;
+  for (int i = 0; i < n; ++i) {             // one thread
+    const SliceParams* P = sp + slice[i];
     const int L = P->L_pad;
     S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
-    S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)cb.rb * L * 512;
+    S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 256;
     S.L[i] = L;
   }
-  for (int r = 0; r < a.n_lr; ++r) {
-    const RateGroup* G = a.groups + cb.bd * a.n_lr + r;
-    S.Q[r] = (G->n_slices > 0) ? reinterpret_cast<const uint8_t*>(G->Q) + (size_t)cb.rb * G->q_groups_cap * 4096 : nullptr;
-  }
 }
 
-// Per-unit tables of the interpolation work of one tile, so that the per-chunk code of the single-thread loops
-// is a table read plus the issuing instructions.  v = t & 1 selects the band-matrix variant of the rates whose
-// window start alternates (d = 32); the chunks of a (rate, variant) are consecutive.
-struct ItTab { uint32_t idesc, b_lo, d_off, pad; };                                  // MMA issuer: one per chunk
-struct PrTab { const uint8_t* q; int32_t log2d, ch0[2], n[2]; int32_t pad; };           // producer: one per rate present
-constexpr int kMaxTileItems = kNLowRates * 8;
+// PY role of both kernels: y stages of the unit's slices for tiles [t0, t1) (this CTA's 64-row half of every 128-row
+// tile), and the stationary R of the unit.  R goes out after `pre` stages of the new unit are in flight: the ring refills
+// while the previous unit drains.  extra/extra_bytes: loaded once with the first R (the f0 kernel's band matrices).
+struct PYState { Ring rg; int seg_i; };
 
-// f0_kernel roles.  A single thread sustains one instruction every ~7 cycles, so one producer and one issuer
-// thread cannot feed 19 eight-KB stages per 2600-cycle tile; the work is split over five single-thread roles
-// over two rings (y tiles: PY -> IY; window chunks: PQ0 / PQ1 alternate -> IQ).  Each ring has ONE consumer, so its
-// slots are released in order and a producer can never run two laps ahead of a slot (which would alias the
-// barrier's phase parity):
-//   warp 0  PY   bulk copies of the y tiles of the d = 1 slices; owns R and P (stationary operands)
-//   warp 6,7 PQ  bulk copies of the rho^(d) window chunks, even / odd chunk of the tile
-//   warp 1  IY   MMAs of the d = 1 slices into accumulator buf = tile parity, then commit -> ybar[buf]
-//   warp 8  IQ   waits ybar[buf] (the y part is COMPLETE: orders its accumulating MMAs after IY's zeroing one),
-//                interpolation MMAs, commit -> acc_full[buf]
-//   warps 2-5    epilogue, columns [0, 64) of the tile (one thread = one template)
-//   warps 9-12   epilogue, columns [64, 128); hands its partial maximum to the first group through shared memory.
-//                With L = 64 (config 3) the MMAs of a tile take ~1000 cycles and a single 128-column epilogue pass
-//                ~2900: the kernel ran at the epilogue's pace.
-// While IQ works on tile t, IY already fills the other accumulator with tile t + 1.
-constexpr int F0_THREADS = 416;
+__device__ __forceinline__ void py_segment(PYState& st, const SegSrc& sg, PairBars& bars, uint32_t sR_u, uint32_t ring_u,
+                                           uint32_t rank, int t0, int t1, uint32_t extra_dst, const uint8_t* extra, uint32_t extra_bytes)
+{
+  const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
+  int stages_per_tile = 0;
+  uint32_t rbytes = 0;
+  for (int i = 0; i < sg.n; ++i) { stages_per_tile += (sg.L[i] + 63) >> 6; rbytes += (uint32_t)sg.L[i] * 256u; }
+  int pre = (st.seg_i == 0) ? 0 : min(st.rg.n, stages_per_tile);
+  bool need_R = true;
+  auto load_R = [&]() {
+    if (st.seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(st.seg_i - 1) & 1u);   // every MMA that reads the old R is complete
+    const uint32_t cb = smem_u32(&bars.consts);
+    mbar_expect_tx(cb, rbytes + (st.seg_i == 0 ? extra_bytes : 0u));
+    uint32_t off = 0;
+    for (int i = 0; i < sg.n; ++i) {
+      copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.L[i] * 256u, cb);
+      off += (uint32_t)sg.L[i] * 256u;
+    }
+    if (st.seg_i == 0 && extra_bytes) copy_pieces(extra_dst, extra, extra_bytes, cb);
+    need_R = false;
+  };
+  if (pre == 0) load_R();
+  for (int t = t0; t < t1; ++t)
+    for (int i = 0; i < sg.n; ++i) {
+      const int L = sg.L[i];
+      const uint8_t* src = sg.Y[i] + (size_t)(2 * t + (int)rank) * L * 128;        // 64-row tiles are contiguous in Y16: L / 8 KB each
+      for (int k0 = 0; k0 < L; k0 += 64, src += PK_YSTAGE) {
+        const int ks = min(64, L - k0);
+        produce(st.rg, bfull, bempty, ring_u, src, (uint32_t)ks * 128u);
+        if (need_R && --pre == 0) load_R();
+      }
+    }
+  if (need_R) load_R();
+  ++st.seg_i;
+}
 
-struct F0Bars {
-  uint64_t full[RC16_MAX_STAGES], empty[RC16_MAX_STAGES];      // y ring: slots [0, nsy); chunk ring: slots [nsy, nsy + nsq)
-  uint64_t acc_full[2], acc_empty[2], ybar[2], consts[2], unit_done[2];
+// relay role (peer CTA): forwards the completion of this CTA's y stages and R loads to the leader's barriers
+__device__ __forceinline__ void relay_y_segment(Ring& rg, int& seg_i, const SegSrc& sg, PairBars& bars, int t0, int t1)
+{
+  // consts first (it is requested before or among the first stages of the unit and the leader needs it first)
+  mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
+  mbar_arrive_cluster(smem_u32(&bars.consts) & kLeaderMask);
+  int stages_per_tile = 0;
+  for (int i = 0; i < sg.n; ++i) stages_per_tile += (sg.L[i] + 63) >> 6;
+  const uint32_t bfull = smem_u32(&bars.yfull[0]);
+  for (int n = (t1 - t0) * stages_per_tile; n > 0; --n) {
+    mbar_wait(bfull + 8u * rg.s, rg.ph);
+    mbar_arrive_cluster((bfull + 8u * rg.s) & kLeaderMask);
+    rg.advance();
+  }
+  ++seg_i;
+}
+
+// ------------------------------------------------------------------------------------------------
+struct LowPArgs {
+  const SliceParams* sp; const RateGroup* groups; const LowUnit* units;
+  int r_bytes, nsy;
+  SchedArgs sched;
 };
 
-#define FOR_SEGMENTS(u, t0, t1)                                                                   \
-  for (int u = u_lo; u <= u_hi; ++u)                                                              \
-    if (u == u_hi && t_hi == 0) break;                                                            \
-    else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : n_tiles; t0 >= t1) continue; \
-    else
-
-// stages of one tile of this unit: y chunks, interpolation chunks per variant
-__device__ __forceinline__ void f0_unit_counts(const F0Args& a, const F0Combo cb, const BdPlan* __restrict__ B, int& ny, int (&nit)[2])
-{
-  ny = B->l_sum >> 5;
-  nit[0] = nit[1] = 0;
-  for (int r = 0; r < a.n_lr; ++r) {
-    if (a.groups[cb.bd * a.n_lr + r].n_slices == 0) continue;
-    nit[0] += a.n_items[r][0];
-    nit[1] += a.n_items[r][a.up[r].n_var > 1 ? 1 : 0];
-  }
-}
-
-__global__ void __launch_bounds__(F0_THREADS, 1)
-f0_kernel(const __grid_constant__ F0Args a)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PK_THREADS, 1)
+lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
 {
   extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ __align__(8) F0Bars bars;
+  __shared__ __align__(8) PairBars bars;
   __shared__ uint32_t tmem_slot;
-  __shared__ SegF0 seg[2];                              // [0] PY's, [1] IY's
-  __shared__ __align__(16) ItTab s_it[2][kMaxTileItems];
-  __shared__ PrTab s_pr[2][kNLowRates];
+  __shared__ SegSrc seg[3];                             // [0] PY, [1] IY, [2] relay
   __shared__ int s_rng[4];
-  __shared__ __align__(16) uint4 s_qst[RC16_MAX_STAGES];   // IQ: per chunk-ring stage {operand descriptor, full barrier, empty barrier}
-  __shared__ __align__(16) Peak s_half[2][kTplBlock];    // second column half's partial maximum, per accumulator buffer
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) sched_range(a.sched, s_rng);
+  const uint32_t rank = cluster_ctarank();
+  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, 0, 1, s_rng);
+  __syncthreads();
+  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
+  if (u_lo == u_hi && t_lo == t_hi) return;             // both CTAs of the cluster take the same decision
+
+  const int nsy = a.nsy;
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid);
+  const uint32_t tmem = tmem_slot;
+  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
+  const uint32_t ring_u = sR_u + (uint32_t)a.r_bytes;
+
+  if (warp == 0) {
+    if (elect_one()) {
+      PYState st{Ring{0, 0u, nsy}, 0};
+      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+        const LowUnit un = a.units[u];
+        const RateGroup* G = a.groups + un.group;
+        seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
+        py_segment(st, seg[0], bars, sR_u, ring_u, rank, t0, t1, 0u, nullptr, 0u);
+      }
+    }
+  } else if (warp == 4 && rank == 1) {
+    if (elect_one()) {
+      Ring rg{0, 0u, nsy};
+      int seg_i = 0;
+      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+        const LowUnit un = a.units[u];
+        const RateGroup* G = a.groups + un.group;
+        seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
+        relay_y_segment(rg, seg_i, seg[2], bars, t0, t1);
+      }
+    }
+  } else if (warp == 1 && rank == 0) {
+    // ===== MMA issuer: one elected thread of the leader CTA =====
+    if (elect_one()) {
+      const uint32_t idesc = idesc_f16_pair(128);
+      const uint32_t a_base = desc_lo(sR_u, 2048u), b_base = desc_lo(ring_u, 1024u);
+      const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
+      Ring rg{0, 0u, nsy};
+      int seg_i = 0;
+      uint32_t e = 0;
+      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+        const LowUnit un = a.units[u];
+        const RateGroup* G = a.groups + un.group;
+        seg_fill(seg[1], a.sp, G->slice, G->n_slices, 2 * un.pb);
+        mbar_wait_cluster(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
+        fence_after();
+        for (int t = t0; t < t1; ++t, ++e) {
+          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+          mbar_wait_cluster(smem_u32(&bars.acc_empty[b]), ph ^ 1u);
+          fence_after();
+          const uint32_t d_tmem = tmem + b * 128u;
+          uint32_t first = 1u, a_lo = a_base;
+          for (int i = 0; i < seg[1].n; ++i) {
+            const int L = seg[1].L[i];
+            for (int k0 = 0; k0 < L; k0 += 64) {
+              const int ks = min(64, L - k0);
+              mbar_wait_cluster(bfull + 8u * rg.s, rg.ph);
+              fence_after();
+              mma_y_stage(d_tmem, a_lo, b_base + (uint32_t)rg.s * (PK_YSTAGE / 16), idesc, ks, first);
+              commit2(bempty + 8u * rg.s, 3);
+              a_lo += (uint32_t)(ks >> 4) * 256u;
+              rg.advance();
+            }
+          }
+          commit2(smem_u32(&bars.acc_full[b]), 3);
+        }
+        commit2(smem_u32(&bars.unit_done), 3);
+        ++seg_i;
+      }
+    }
+  } else if (warp >= 8) {
+    // ===== epilogue: thread = row; warps 8-11 columns [0, 64), warps 12-15 columns [64, 128); fp32 -> fp16 -> Q16 =====
+    const int q = warp & 3, wg = (warp - 8) >> 2;
+    const int row = q * 32 + lane;
+    const uint32_t acc_empty_leader = smem_u32(&bars.acc_empty[0]) & kLeaderMask;
+    uint32_t e = 0;
+    FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+      const LowUnit un = a.units[u];
+      const RateGroup* Gp = a.groups + un.group;
+      const int q_cap = Gp->q_groups_cap;
+      __half* __restrict__ Q = Gp->Q + ((size_t)(2 * un.pb + (int)rank) * q_cap * 128 + row) * 8;
+      for (int t = t0; t < t1; ++t, ++e) {
+        const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+        mbar_wait(smem_u32(&bars.acc_full[b]), ph);
+        fence_after();
+        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
+        uint32_t v0[32], v1[32];
+        tmem_ld32(taddr, v0);
+        tmem_ld32(taddr + 32u, v1);
+        tmem_ld_wait();
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);   // the accumulator is in registers: free it first
+        const int jg0 = t * 16 + 8 * wg;
+#pragma unroll
+        for (int gq = 0; gq < 8; ++gq) {
+          const uint32_t* v = gq < 4 ? v0 + 8 * gq : v1 + 8 * (gq - 4);
+          uint32_t h[4];
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const __half2 p2 = __floats2half2_rn(__uint_as_float(v[2 * x]), __uint_as_float(v[2 * x + 1]));
+            h[x] = *reinterpret_cast<const uint32_t*>(&p2);
+          }
+          if (jg0 + gq < q_cap) *reinterpret_cast<uint4*>(Q + (size_t)(jg0 + gq) * 1024) = make_uint4(h[0], h[1], h[2], h[3]);
+        }
+      }
+    }
+  }
+  pair_teardown(tmem, warp);
+}
+
+// ------------------------------------------------------------------------------------------------
+struct F0PArgs {
+  const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups;
+  const uint8_t* P;                                     // [2][p_bytes]: band-matrix blob of rank 0, of rank 1
+  Peak* partials; Capture cap; long long k_a;
+  int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, slots_cap, max_templates, gt;
+  SchedArgs sched;                                      // units = combos, one class
+  PairRate rate[kNLowRates];
+};
+
+// chunks (16 low-rate rows) that must be resident before tile t's interpolation: ceil((adv t + adv + 16) / 16)
+__device__ __forceinline__ int q_chunks_upto(int adv, int t) { return (adv * t + adv + 16 + 15) >> 4; }
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PK_THREADS, 1)
+f0_pair_kernel(const __grid_constant__ F0PArgs a)
+{
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ __align__(8) PairBars bars;
+  __shared__ uint32_t tmem_slot;
+  __shared__ SegSrc seg[3];                             // [0] PY, [1] IY, [2] relay
+  __shared__ int s_rng[4];
+  __shared__ __align__(16) Peak s_x[2][64];             // epilogue: second column half -> first, per flush parity
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t rank = cluster_ctarank();
+  const long long a0 = a.k_a / kTimeTile;               // absolute index of the chunk's tile 0
+  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, a0, a.gt, s_rng);
   __syncthreads();
   const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
   if (u_lo == u_hi && t_lo == t_hi) return;
   const int n_tiles = a.sched.n_tiles[0];
 
-  if (warp == 0) tmem_alloc(&tmem_slot, 512);
-  if (tid == 32) {
-    for (int s = 0; s < RC16_MAX_STAGES; ++s) { mbar_init(smem_u32(&bars.full[s]), 1); mbar_init(smem_u32(&bars.empty[s]), 1); }
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(smem_u32(&bars.acc_full[b]), 1); mbar_init(smem_u32(&bars.acc_empty[b]), 256);
-      mbar_init(smem_u32(&bars.ybar[b]), 1); mbar_init(smem_u32(&bars.consts[b]), 1); mbar_init(smem_u32(&bars.unit_done[b]), 1);
-    }
-    mbar_init_fence();
-  }
-  fence_before();
-  __syncthreads();
-  fence_after();
+  const int nsy = a.nsy, n_lr = a.n_lr;
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid);
   const uint32_t tmem = tmem_slot;
-  const int n_lr = a.n_lr;
-  const int nsy = a.nsy, nsq = a.nsq;
-  const int r_bufs = a.r_bufs;
-  const uint32_t bfull = smem_u32(&bars.full[0]), bempty = smem_u32(&bars.empty[0]);
-  const uint32_t qfull = bfull + 8u * nsy, qempty = bempty + 8u * nsy;
-  const uint32_t sR_u = smem_u32(smem);                 // r_bufs x [l_sum / 8][2][128][8] fp16
-  const uint32_t sP_u = sR_u + (uint32_t)(a.r_bytes * r_bufs);   // band matrices
-  const uint32_t ring_u = sP_u + (uint32_t)a.p_bytes;
-  const uint32_t qring_u = ring_u + (uint32_t)nsy * RC16_STAGE;
+  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
+  const uint32_t sP_u = sR_u + (uint32_t)a.r_bytes;     // this rank's band-matrix blocks
+  const uint32_t sQ_u = sP_u + (uint32_t)a.p_bytes;     // per-rate circular buffers of 16-row chunks (4 KB each)
+  const uint32_t ring_u = sQ_u + (uint32_t)a.q_bytes;   // y ring
 
   if (warp == 0) {
     // ===== PY: y tiles of the d = 1 slices, R and P =====
     if (elect_one()) {
-      int seg_i = 0;
-      Ring rg{0, 0u, nsy};
-      FOR_SEGMENTS(u, t0, t1) {
+      PYState st{Ring{0, 0u, nsy}, 0};
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
         const F0Combo cb = a.combos[u];
         const BdPlan* B = a.bd + cb.bd;
-        seg_f0_fill(seg[0], a, cb, B);
-        const int nf_u = B->n_f0;
-        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
-        // R (and P, once) go out after `pre` y stages of the unit's first tile are in flight: the ring refills while
-        // the previous unit drains, and the switch costs one R load.  pre <= ring size, or IY (which waits for R) could
-        // never free the slot PY is waiting for.
-        int pre = (seg_i == 0) ? 0 : min(nsy, B->l_sum >> 5);
-        bool need_R = true;
-        auto load_R = [&]() {
-          // this R buffer's previous unit is complete (per-buffer barrier: never more than one phase away)
-          if (use > 0) mbar_wait(smem_u32(&bars.unit_done[rb_i]), (uint32_t)(use - 1) & 1u);
-          const uint32_t cb_u = smem_u32(&bars.consts[rb_i]);
-          mbar_expect_tx(cb_u, (uint32_t)B->l_sum * 512u + (seg_i == 0 ? (uint32_t)a.p_bytes : 0u));
-          uint32_t off = (uint32_t)(rb_i * a.r_bytes);
-          for (int i = 0; i < nf_u; ++i) {
-            copy_pieces(sR_u + off, seg[0].Rsrc[i], (uint32_t)seg[0].L[i] * 512u, cb_u);
-            off += (uint32_t)seg[0].L[i] * 512u;
-          }
-          if (seg_i == 0) copy_pieces(sP_u, a.P, (uint32_t)a.p_bytes, cb_u);
-          need_R = false;
-        };
-        if (pre == 0) load_R();
-        for (int t = t0; t < t1; ++t)
-          for (int i = 0; i < nf_u; ++i) {
-            const int L = seg[0].L[i];
-            const uint8_t* src = seg[0].Y[i] + (size_t)t * L * 256;      // tiles are contiguous in Y16
-            for (int kc = 0; kc < (L >> 5); ++kc, src += RC16_STAGE) {
-              produce(rg, bfull, bempty, ring_u, src);
-              if (need_R && --pre == 0) load_R();
-            }
-          }
-        ++seg_i;
+        seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb + (int)rank);
+        py_segment(st, seg[0], bars, sR_u, ring_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes);
       }
     }
-  } else if (warp == 6 || warp == 7) {
-    // ===== PQ: rho^(d) window chunks, even (warp 6) / odd (warp 7) chunk of the tile =====
+  } else if (warp == 4 && rank == 1) {
     if (elect_one()) {
-      const int pq = warp - 6;
-      PrTab* tab = s_pr[pq];
-      Ring rg{0, 0u, nsq};
-      int own = pq == 0;                                 // the ring's stages alternate between the two PQ threads
-      FOR_SEGMENTS(u, t0, t1) {
+      Ring rg{0, 0u, nsy};
+      int seg_i = 0;
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
         const F0Combo cb = a.combos[u];
-        int npr = 0;
+        const BdPlan* B = a.bd + cb.bd;
+        seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb + (int)rank);
+        relay_y_segment(rg, seg_i, seg[2], bars, t0, t1);
+      }
+    }
+  } else if (warp == 2) {
+    // ===== PQ: the rows of every rate's rho^(d) window that tile e needs and tile e - 1 did not have =====
+    if (elect_one()) {
+      uint32_t e = 0;
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
+        const F0Combo cb = a.combos[u];
+        const uint8_t* qsrc[kNLowRates];
         for (int r = 0; r < n_lr; ++r) {
           const RateGroup* G = a.groups + cb.bd * n_lr + r;
-          if (G->n_slices == 0) continue;
-          PrTab e;
-          e.q = reinterpret_cast<const uint8_t*>(G->Q) + (size_t)cb.rb * G->q_groups_cap * 4096;
-          e.log2d = a.up[r].log2d; e.pad = 0;
-          for (int v = 0; v < 2; ++v) {
-            const int vv = a.up[r].n_var > 1 ? v : 0;
-            e.n[v] = a.n_items[r][vv];
-            e.ch0[v] = e.n[v] > 0 ? (int)a.item[r][vv][0].ch : 0;
-          }
-          tab[npr++] = e;
+          qsrc[r] = (G->n_slices > 0) ? reinterpret_cast<const uint8_t*>(G->Q) + (size_t)(2 * cb.rb + (int)rank) * G->q_groups_cap * 2048 : nullptr;
         }
-        for (int t = t0; t < t1; ++t) {
-          const int v = t & 1;
-          for (int j = 0; j < npr; ++j) {
-            const PrTab* e = &tab[j];
-            const int ws = ((t * 128) >> e->log2d) & ~7;
-            const uint8_t* src = e->q + (size_t)(ws >> 3) * 4096 + (size_t)e->ch0[v] * RC16_STAGE;
-            const int n_it = e->n[v];
-            for (int i = 0; i < n_it; ++i, src += RC16_STAGE, own ^= 1) {
-              if (own) produce(rg, qfull, qempty, qring_u, src); else rg.advance();
-            }
+        for (int t = t0; t < t1; ++t, ++e) {
+          // a unit's first tile fetches whole windows into slots other tiles may still be reading: drain first
+          if (t == t0) { if (e > 0) mbar_wait(smem_u32(&bars.qempty[(e - 1) & (PK_NQB - 1)]), ((e - 1) >> 2) & 1u); }
+          else if (e >= PK_QDIST) mbar_wait(smem_u32(&bars.qempty[(e - PK_QDIST) & (PK_NQB - 1)]), ((e - PK_QDIST) >> 2) & 1u);
+          const uint32_t fb = smem_u32(&bars.qfull[e & (PK_NQB - 1)]);
+          uint32_t total = 0;
+          for (int r = 0; r < n_lr; ++r) {
+            if (!qsrc[r]) continue;
+            const int adv = a.rate[r].adv;
+            const int c_lo = (t == t0) ? (adv * t) >> 4 : q_chunks_upto(adv, t - 1);
+            total += (uint32_t)(q_chunks_upto(adv, t) - c_lo) * 4096u;
+          }
+          mbar_expect_tx(fb, total);                    // total == 0: a plain arrival
+          for (int r = 0; r < n_lr; ++r) {
+            if (!qsrc[r]) continue;
+            const int adv = a.rate[r].adv, cap = a.rate[r].cap_chunks;
+            const int c_lo = (t == t0) ? (adv * t) >> 4 : q_chunks_upto(adv, t - 1);
+            const int c_hi = q_chunks_upto(adv, t);
+            if (c_hi <= c_lo) continue;
+            const uint32_t base = sQ_u + (uint32_t)a.rate[r].ring_off;
+            const int s0 = c_lo % cap;
+            const int n1 = min(c_hi - c_lo, cap - s0);
+            copy_pieces(base + (uint32_t)s0 * 4096u, qsrc[r] + (size_t)c_lo * 4096, (uint32_t)n1 * 4096u, fb);
+            if (c_hi - c_lo > n1) copy_pieces(base, qsrc[r] + (size_t)(c_lo + n1) * 4096, (uint32_t)(c_hi - c_lo - n1) * 4096u, fb);
           }
         }
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == 5 && rank == 1) {
+    // ===== relay of the rho^(d) tile events =====
+    if (elect_one()) {
+      uint32_t e = 0;
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
+        for (int t = t0; t < t1; ++t, ++e) {
+          const uint32_t fb = smem_u32(&bars.qfull[e & (PK_NQB - 1)]);
+          mbar_wait(fb, (e >> 2) & 1u);
+          mbar_arrive_cluster(fb & kLeaderMask);
+        }
+      }
+    }
+  } else if (warp == 1 && rank == 0) {
     // ===== IY: MMAs of the d = 1 slices =====
     if (elect_one()) {
-      const uint32_t idesc128 = idesc_f16(128, 128);
-      const uint32_t a_base = desc_lo(sR_u, 4096u), b_base = desc_lo(ring_u, 2048u);
-      uint32_t eph = 3u;                                  // bit buf: parity to wait for on acc_empty (first use: free)
-      int seg_i = 0, buf = 0;
+      const uint32_t idesc = idesc_f16_pair(128);
+      const uint32_t a_base = desc_lo(sR_u, 2048u), b_base = desc_lo(ring_u, 1024u);
+      const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
       Ring rg{0, 0u, nsy};
-      FOR_SEGMENTS(u, t0, t1) {
+      int seg_i = 0;
+      uint32_t e = 0;
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
         const F0Combo cb = a.combos[u];
         const BdPlan* B = a.bd + cb.bd;
-        seg_f0_fill(seg[1], a, cb, B);
-        const int nf_u = B->n_f0;
-        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
-        mbar_wait(smem_u32(&bars.consts[rb_i]), (uint32_t)use & 1u);
+        seg_fill(seg[1], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb);
+        mbar_wait_cluster(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
         fence_after();
-        const uint32_t a_seg = a_base + (uint32_t)((rb_i * a.r_bytes) >> 4);
-        for (int t = t0; t < t1; ++t, buf ^= 1) {
-          mbar_wait(smem_u32(&bars.acc_empty[buf]), (eph >> buf) & 1u); eph ^= 1u << buf;
+        for (int t = t0; t < t1; ++t, ++e) {
+          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+          mbar_wait_cluster(smem_u32(&bars.acc_empty[b]), ph ^ 1u);
           fence_after();
-          const uint32_t d_tmem = tmem + (uint32_t)(buf * 256);
-          uint32_t first = 1u, a_lo = a_seg;
-          for (int i = 0; i < nf_u; ++i) {
-            const int n_kc = seg[1].L[i] >> 5;
-            for (int kc = 0; kc < n_kc; ++kc, a_lo += 1024u) {
-              mbar_wait(bfull + 8u * rg.s, rg.ph);
+          const uint32_t d_tmem = tmem + b * 128u;
+          uint32_t first = 1u, a_lo = a_base;
+          for (int i = 0; i < seg[1].n; ++i) {
+            const int L = seg[1].L[i];
+            for (int k0 = 0; k0 < L; k0 += 64) {
+              const int ks = min(64, L - k0);
+              mbar_wait_cluster(bfull + 8u * rg.s, rg.ph);
               fence_after();
-              mma_recon_chunk(d_tmem, a_lo, b_base + (uint32_t)rg.s * (RC16_STAGE / 16), idesc128, first);
-              commit(bempty + 8u * rg.s);
-              first = 0u;
+              mma_y_stage(d_tmem, a_lo, b_base + (uint32_t)rg.s * (PK_YSTAGE / 16), idesc, ks, first);
+              commit2(bempty + 8u * rg.s, 3);
+              a_lo += (uint32_t)(ks >> 4) * 256u;
               rg.advance();
             }
           }
-          commit(smem_u32(&bars.ybar[buf]));
+          commit2(smem_u32(&bars.ybar[b]), 1);
         }
         ++seg_i;
       }
     }
-  } else if (warp == 8) {
+  } else if (warp == 3 && rank == 0) {
     // ===== IQ: interpolation MMAs (A4), after the tile's y part is complete =====
     if (elect_one()) {
-      const uint32_t qa_base = desc_lo(qring_u, 4096u), p_base = desc_lo(sP_u, 2048u);
-      uint32_t yph = 0u;
-      int seg_i = 0, buf = 0;
-      Ring rg{0, 0u, nsq};
-      // Everything a chunk needs is read from two small tables (one LDS.128 each) instead of being recomputed: every
-      // value the MMA takes has to cross from a vector to a uniform register (R2UR), and this loop is the kernel's
-      // critical path.
-      for (int st = 0; st < nsq; ++st)
-        s_qst[st] = make_uint4(qa_base + (uint32_t)st * (RC16_STAGE / 16), qfull + 8u * st, qempty + 8u * st, 0u);
-      FOR_SEGMENTS(u, t0, t1) {
+      const uint32_t p_base = sP_u >> 4;
+      uint32_t e = 0;
+      FOR_SEGMENTS(u, t0, t1, n_tiles) {
         const F0Combo cb = a.combos[u];
-        const BdPlan* B = a.bd + cb.bd;
-        int nit[2] = {0, 0};
-        for (int v = 0; v < 2; ++v)
+        uint32_t present = 0;
+        for (int r = 0; r < n_lr; ++r) if (a.groups[cb.bd * n_lr + r].n_slices > 0) present |= 1u << r;
+        for (int t = t0; t < t1; ++t, ++e) {
+          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+          mbar_wait(smem_u32(&bars.ybar[b]), ph);
+          mbar_wait_cluster(smem_u32(&bars.qfull[e & (PK_NQB - 1)]), ph);
+          fence_after();
+          const uint32_t d_tmem = tmem + b * 128u;
           for (int r = 0; r < n_lr; ++r) {
-            if (a.groups[cb.bd * n_lr + r].n_slices == 0) continue;
-            const int vv = a.up[r].n_var > 1 ? v : 0;
-            for (int i = 0; i < a.n_items[r][vv]; ++i) {
-              const QItem it = a.item[r][vv][i];
-              // tiles of parity v use accumulator buf ^ ((v ^ t0) & 1): the accumulator address goes into the table
-              ItTab e; e.idesc = it.idesc; e.b_lo = p_base + it.b_off; e.pad = 0;
-              e.d_off = tmem + (uint32_t)((buf ^ ((v ^ t0) & 1)) * 256) + it.d_off;
-              s_it[v][nit[v]++] = e;
+            if (!(present >> r & 1u)) continue;
+            const PairRate& R = a.rate[r];
+            const int v = (R.adv >= 16) ? 0 : ((R.adv * t) & 15) / R.adv;
+            const int s0 = ((R.adv * t) >> 4) % R.cap_chunks;
+            const uint32_t qa = desc_lo(sQ_u + (uint32_t)R.ring_off, 2048u);
+            const int n_it = R.n_items[v];
+            for (int k = 0; k < n_it; ++k) {
+              const PairItem it = R.item[v][k];
+              int s = s0 + (int)it.ch; if (s >= R.cap_chunks) s -= R.cap_chunks;
+              mma2_ss(d_tmem + it.d_col, desc64(qa + (uint32_t)s * 256u), desc64(p_base + it.p_lo), it.idesc, 1u);
             }
           }
-        const int rb_i = seg_i % r_bufs, use = seg_i / r_bufs;
-        if (seg_i == 0) { mbar_wait(smem_u32(&bars.consts[0]), 0u); fence_after(); }   // P has landed (loaded once, with the first R)
-        for (int t = t0; t < t1; ++t, buf ^= 1) {
-          mbar_wait(smem_u32(&bars.ybar[buf]), (yph >> buf) & 1u); yph ^= 1u << buf;
-          fence_after();
-          const ItTab* tab = s_it[t & 1];
-          const int n_it = nit[t & 1];
-          for (int k = 0; k < n_it; ++k) {
-            const uint4 e = *reinterpret_cast<const uint4*>(tab + k);     // idesc, b_lo, accumulator address
-            const uint4 q = s_qst[rg.s];                                  // operand descriptor, full, empty barrier
-            mbar_wait(q.y, rg.ph);
-            fence_after();
-            const uint64_t bdesc = desc64(e.y);
-            mma_ss(e.z,        desc64(q.x),        bdesc, e.x, 1u);
-            mma_ss(e.z + 128u, desc64(q.x + 128u), bdesc, e.x, 1u);
-            commit(q.z);
-            rg.advance();
-          }
-          commit(smem_u32(&bars.acc_full[buf]));
+          commit2(smem_u32(&bars.qempty[e & (PK_NQB - 1)]), 3);
+          commit2(smem_u32(&bars.acc_full[b]), 3);
         }
-        commit(smem_u32(&bars.unit_done[rb_i]));
-        (void)use;
-        ++seg_i;
+        commit2(smem_u32(&bars.unit_done), 3);
       }
     }
-  } else if ((warp >= 2 && warp <= 5) || warp >= 9) {
-    // ===== epilogue: one thread = one template and one half of the tile's columns; |rho|^2 and first maximum =====
-    const int q = warp & 3;                           // TMEM lane quarter this warp may access
-    const int half = warp >= 9 ? 1 : 0;
-    const int pl = q * 32 + lane;
-    uint32_t fph = 0u;
-    int buf = 0;
-    FOR_SEGMENTS(u, t0, t1) {
+  } else if (warp >= 8) {
+    // ===== epilogue: thread = row (lane); lanes 2i / 2i + 1 of a warp hold the cosine / sine row of one template =====
+    const int q = warp & 3, wg = (warp - 8) >> 2;
+    const int row = q * 32 + lane;
+    const int part = lane & 1;
+    const uint32_t acc_empty_leader = smem_u32(&bars.acc_empty[0]) & kLeaderMask;
+    uint32_t e = 0, flush_i = 0;
+    FOR_SEGMENTS(u, t0, t1, n_tiles) {
       const F0Combo cb = a.combos[u];
       const int n_templates = a.bd[cb.bd].n_templates;
-      const int p = cb.rb * kTplBlock + pl;
-      const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && 2 * p + 1 < a.cap.rows;
-      for (int t = t0; t < t1; ++t, buf ^= 1) {
-        mbar_wait(smem_u32(&bars.acc_full[buf]), (fph >> buf) & 1u); fph ^= 1u << buf;
+      const int grow = (2 * cb.rb + (int)rank) * 128 + row;             // reconstruction row i = 2 p + part
+      const int p = grow >> 1;
+      const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && grow < a.cap.rows;
+      // running first maximum of this thread's columns over the current granule
+      float bq = -1.f, bmine = 0.f, brecv = 0.f;
+      int bk = 0;
+      for (int t = t0; t < t1; ++t, ++e) {
+        const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+        mbar_wait(smem_u32(&bars.acc_full[b]), ph);
         fence_after();
-        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 256);
+        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
+        uint32_t lo[32], hi[32];                        // columns 64 wg + [0, 32) and + [32, 64) of this row
+        tmem_ld32(taddr, lo);
+        tmem_ld32(taddr + 32u, hi);
+        tmem_ld_wait();
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);   // the tile is in registers: free the accumulator
         const int kap0 = t * 128;
         const int valid = min(128, a.c - kap0);
-        // four interleaved running maxima (columns j = m mod 4) break the serial compare/select chain; merged below
-        // with "larger q, then lower k" so that the first maximum of the tile still wins (R8)
-        float bq[4] = {-1.f, -1.f, -1.f, -1.f}, bre4[4] = {0.f, 0.f, 0.f, 0.f}, bim4[4] = {0.f, 0.f, 0.f, 0.f};
-        int bk4[4] = {0, 0, 0, 0};
-  #pragma unroll 1
-        for (int c0 = 64 * half; c0 < 64 * half + 64; c0 += 32) {
-          uint32_t re[32], im[32];
-          tmem_ld32(taddr + (uint32_t)c0, re);
-          tmem_ld32(taddr + (uint32_t)(128 + c0), im);
-          tmem_ld_wait();
-          if (c0 + 32 <= valid) {
-  #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-              const float qq = fmaf(x, x, y * y);
-              if (qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
-            }
-          } else {
-  #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const float x = __uint_as_float(re[j]), y = __uint_as_float(im[j]);
-              const float qq = fmaf(x, x, y * y);
-              if (c0 + j < valid && qq > bq[j & 3]) { bq[j & 3] = qq; bk4[j & 3] = c0 + j; bre4[j & 3] = x; bim4[j & 3] = y; }
-            }
-          }
-          if (capture) {
-  #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const long long k = a.k_a + kap0 + c0 + j;
-              if (c0 + j < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
-                a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(re[j]);
-                a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(im[j]);
-              }
-            }
+        if (capture) {
+#pragma unroll
+          for (int j = 0; j < 64; ++j) {
+            const int col = 64 * wg + j;
+            const long long k = a.k_a + kap0 + col;
+            if (col < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n)
+              a.cap.snr[(size_t)grow * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(j < 32 ? lo[j] : hi[j - 32]);
           }
         }
-        float best = bq[0], bre = bre4[0], bim = bim4[0];
-        int bk = bk4[0];
-  #pragma unroll
+        // even lanes (cosine row) take columns [0, 32) of the 64, odd lanes (sine row) [32, 64): one shuffle per column
+        // brings the partner row's value of the SAME column
+        const int cbase = 64 * wg + 32 * part;
+        float q4[4] = {-1.f, -1.f, -1.f, -1.f}, m4[4] = {0.f, 0.f, 0.f, 0.f}, r4[4] = {0.f, 0.f, 0.f, 0.f};
+        int k4[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const float send = __uint_as_float(part ? lo[j] : hi[j]);
+          const float mine = __uint_as_float(part ? hi[j] : lo[j]);
+          const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
+          const float qq = fmaf(mine, mine, recv * recv);
+          if (cbase + j < valid && qq > q4[j & 3]) { q4[j & 3] = qq; k4[j & 3] = cbase + j; m4[j & 3] = mine; r4[j & 3] = recv; }
+        }
+        float tq = q4[0], tm = m4[0], tr = r4[0];
+        int tk = k4[0];
+#pragma unroll
         for (int m = 1; m < 4; ++m)
-          if (bq[m] > best || (bq[m] == best && bk4[m] < bk)) { best = bq[m]; bk = bk4[m]; bre = bre4[m]; bim = bim4[m]; }
-        fence_before();
-        mbar_arrive(smem_u32(&bars.acc_empty[buf]));
-        // s_half[buf] of tile t is rewritten at tile t + 2, i.e. after the barrier of tile t + 1, which the first group
-        // reaches only after it has read tile t's entry
-        if (half) { Peak pk; pk.q = best; pk.kappa = bk; pk.re = bre; pk.im = bim; s_half[buf][pl] = pk; }
-        asm volatile("bar.sync 2, 256;" ::: "memory");
-        if (!half) {
-          const Peak o = s_half[buf][pl];
-          if (o.q > best) { best = o.q; bk = o.kappa; bre = o.re; bim = o.im; }   // its columns are later: ties stay with the first half
-          if (p < n_templates) {
-            Peak pk; pk.q = best; pk.kappa = kap0 + bk; pk.re = bre; pk.im = bim;
-            a.partials[((size_t)cb.bd * a.tiles_cap + t) * a.max_templates + p] = pk;
+          if (q4[m] > tq || (q4[m] == tq && k4[m] < tk)) { tq = q4[m]; tk = k4[m]; tm = m4[m]; tr = r4[m]; }
+        if (tq > bq) { bq = tq; bk = kap0 + tk; bmine = tm; brecv = tr; }      // later tiles never win ties
+        // granule end: merge the four partial maxima of a template (two lanes x two column halves), write one record
+        const long long at = a0 + t;
+        if (t + 1 == t1 || (at + 1) % a.gt == 0) {
+          // partner lane: the odd lane's columns are later, so the even lane wins ties
+          const float oq = __shfl_xor_sync(0xffffffffu, bq, 1), om = __shfl_xor_sync(0xffffffffu, bmine, 1), orv = __shfl_xor_sync(0xffffffffu, brecv, 1);
+          const int ok = __shfl_xor_sync(0xffffffffu, bk, 1);
+          float re = part ? brecv : bmine, im = part ? bmine : brecv;          // this thread's best as (re, im)
+          const float ore = part ? om : orv, oim = part ? orv : om;            // partner's best (its part is the other one)
+          if (oq > bq || (oq == bq && ok < bk)) { bq = oq; bk = ok; re = ore; im = oim; }
+          const int fp = flush_i & 1;
+          if (wg == 1 && part == 0) { Peak pk; pk.q = bq; pk.kappa = bk; pk.re = re; pk.im = im; s_x[fp][row >> 1] = pk; }
+          asm volatile("bar.sync 2, 256;" ::: "memory");
+          if (wg == 0 && part == 0) {
+            const Peak o = s_x[fp][row >> 1];
+            if (o.q > bq) { bq = o.q; bk = o.kappa; re = o.re; im = o.im; }    // its columns are later: ties stay here
+            if (p < n_templates) {
+              const int gi = (int)(at / a.gt - a0 / a.gt);
+              Peak pk; pk.q = bq; pk.kappa = bk; pk.re = re; pk.im = im;
+              a.partials[((size_t)cb.bd * a.slots_cap + gi) * a.max_templates + p] = pk;
+            }
           }
+          ++flush_i;
+          bq = -1.f; bk = 0; bmine = 0.f; brecv = 0.f;
         }
       }
     }
   }
-  fence_before();
-  __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem, 512);
+  pair_teardown(tmem, warp);
 }
+
 // ------------------------------------------------------------------------------------------------
 // host side: plan
 // ------------------------------------------------------------------------------------------------
@@ -736,6 +670,8 @@ bool plan_alloc(F16Plan* pl, void** p, size_t n, bool zero, int64_t* bytes, char
   *bytes += (int64_t)n;
   return true;
 }
+
+inline int chunks_upto(int adv, int t) { return (adv * t + adv + 16 + 15) >> 4; }
 
 }  // namespace
 
@@ -755,7 +691,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     for (int s = 0; s < bp_host[b].n_slices; ++s) have[sp_host[bp_host[b].first_slice + s].log2d] = true;
   int lr_of[kMaxRates];
   pl->n_lr = 0;
-  for (int l2 = 1; l2 < kMaxRates; ++l2) { lr_of[l2] = -1; if (have[l2]) { lr_of[l2] = pl->n_lr; pl->up[pl->n_lr].log2d = l2; ++pl->n_lr; } }
+  for (int l2 = 1; l2 < kMaxRates; ++l2) { lr_of[l2] = -1; if (have[l2]) { lr_of[l2] = pl->n_lr; pl->rate[pl->n_lr].log2d = l2; ++pl->n_lr; } }
 
   // A (bin, detector) the tensor kernels cannot hold is EXCLUDED from their work lists and reconstructed by the FFMA
   // kernels (lloid_api.cu); the others stay on the tensor path.
@@ -769,17 +705,17 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     BdPlan& B = pl->bd_host[b];
     memset(&B, 0, sizeof B);
     B.n_templates = bp_host[b].n_templates;
-    B.n_rb = (B.n_templates + kTplBlock - 1) / kTplBlock;
+    B.n_rb = (B.n_templates + kTplBlock - 1) / kTplBlock;              // pair blocks of 128 templates
     for (int r = 0; r < pl->n_lr; ++r) {
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
       memset(&G, 0, sizeof G);
-      G.log2d = pl->up[r].log2d; G.n_rb = B.n_rb;
+      G.log2d = pl->rate[r].log2d; G.n_rb = B.n_rb;
       G.q_groups_cap = (((chunk_cap >> G.log2d) + 2 * kKUp + 127) / 128) * 16 + 16;
     }
     for (int s = 0; s < bp_host[b].n_slices; ++s) {
       const int idx = bp_host[b].first_slice + s;
       const SliceParams& P = sp_host[idx];
-      if (P.rows_pad != B.n_rb * 2 * kTplBlock || P.L_pad % 32) { ok = false; break; }
+      if (P.rows_pad != B.n_rb * 2 * kTplBlock || P.L_pad % 16) { ok = false; break; }
       if (P.d == 1) {
         if (B.n_f0 == kMaxF0Slices) { ok = false; break; }
         B.f0_slice[B.n_f0++] = idx; B.l_sum += P.L_pad;
@@ -793,55 +729,69 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     if (!ok) pl->excluded[b] = 1;
   }
 
-  // band matrices P_d (A4):  c[kl] = sum_r Q[ws + r] P[r, kl],  ws = (128 t / d) & ~7, mis = 128 t / d - ws,
-  // P[r, kl] = w_phi[i], i = mis + floor(kl / d) + K_up - r in [-K_up, K_up), phi = kl mod d
-  std::vector<__half> pblob;
+  // Band matrices P_d (A4), one block per (rate, variant, 16-row chunk of the window):
+  //   c[kl] = sum_rw Q[16 floor(adv t / 16) + rw] P[rw, kl],  mis = adv t mod 16 (variant = mis / adv),
+  //   P[rw, kl] = w_phi[i], i = mis + floor(kl / d) + K_up - rw in [-K_up, K_up), phi = kl mod d.
+  // A block keeps the nn columns [n0, n0 + nn) its band touches; rank 0 stores columns [n0, n0 + nn / 2), rank 1 the
+  // rest (B operand of a cta_group::2 MMA), each as [2 row groups][nn / 2 columns][8 rows] fp16.
+  std::vector<__half> pblob[2];
+  int q_bytes = 0;
   for (int r = 0; r < pl->n_lr; ++r) {
-    UpRate& U = pl->up[r];
-    const int d = 1 << U.log2d;
-    if (!up_w || !up_w[U.log2d]) return true;
-    const double* w = up_w[U.log2d];
-    U.n_var = (128 / d) % 8 ? 2 : 1;
-    const int mis_max = (U.n_var == 2) ? 128 / d : 0;
-    U.k_win = (128 / d + 2 * kKUp + mis_max + 15) / 16 * 16;
-    if (U.k_win / 16 > 8) return true;
-    memset(U.n0, 0, sizeof U.n0); memset(U.nn, 0, sizeof U.nn);
-    U.p_off[1] = 0;
+    PairRate& U = pl->rate[r];
+    const int l2 = U.log2d, d = 1 << l2;
+    if (!up_w || !up_w[l2]) return true;
+    const double* w = up_w[l2];
+    U.adv = 128 >> l2;
+    U.n_var = U.adv >= 16 ? 1 : 16 / U.adv;
+    if (U.n_var > 4) return true;
+    // circular buffer: every chunk that tile t - PK_QDIST + 1 .. t may still read, while tile t's rows arrive
+    int cap = 0;
+    for (int t = 0; t < 64; ++t) cap = std::max(cap, chunks_upto(U.adv, t) - ((U.adv * std::max(t - PK_QDIST + 1, 0)) >> 4));
+    U.cap_chunks = cap;
+    U.ring_off = q_bytes;
+    q_bytes += cap * 4096;
+    for (int v = 0; v < 4; ++v) U.n_items[v] = 0;
     for (int v = 0; v < U.n_var; ++v) {
-      const int mis = v * mis_max;
-      U.p_off[v] = (int)(pblob.size() * sizeof(__half));
-      const size_t base = pblob.size();
-      pblob.resize(base + (size_t)U.k_win * 128, __float2half(0.f));
-      std::vector<int> cmin(U.k_win / 16, 1 << 30), cmax(U.k_win / 16, -1);
-      for (int rw = 0; rw < U.k_win; ++rw)
-        for (int kl = 0; kl < 128; ++kl) {
-          const int i = mis + kl / d + kKUp - rw;
-          if (i < -kKUp || i >= kKUp) continue;
-          pblob[base + ((size_t)(rw >> 3) * 128 + kl) * 8 + (rw & 7)] = __float2half_rn((float)w[(size_t)(i + kKUp) * d + kl % d]);
-          cmin[rw >> 4] = std::min(cmin[rw >> 4], kl); cmax[rw >> 4] = std::max(cmax[rw >> 4], kl);
-        }
-      for (int ch = 0; ch < U.k_win / 16; ++ch) {
-        if (cmax[ch] < 0) continue;
-        int n0 = cmin[ch] / 8 * 8;
-        const int nn = (cmax[ch] + 1 - n0 + 15) / 16 * 16;
+      const int mis = v * U.adv;
+      const int nch = (mis + U.adv + 2 * kKUp + 15) / 16;
+      if (nch > 5) return true;
+      for (int ch = 0; ch < nch; ++ch) {
+        int cmin = 1 << 30, cmax = -1;
+        for (int rr = 0; rr < 16; ++rr)
+          for (int kl = 0; kl < 128; ++kl) {
+            const int i = mis + kl / d + kKUp - (16 * ch + rr);
+            if (i < -kKUp || i >= kKUp) continue;
+            cmin = std::min(cmin, kl); cmax = std::max(cmax, kl);
+          }
+        if (cmax < 0) continue;
+        int n0 = cmin / 8 * 8;
+        const int nn = (cmax + 1 - n0 + 15) / 16 * 16;
         if (n0 + nn > 128) n0 = 128 - nn;
-        U.n0[v][ch] = (uint8_t)(n0 / 8); U.nn[v][ch] = (uint8_t)(nn / 8);
+        const int half = nn / 2;
+        const size_t base = pblob[0].size();
+        for (int c = 0; c < 2; ++c) pblob[c].resize(base + (size_t)16 * half, __float2half(0.f));
+        for (int rr = 0; rr < 16; ++rr)
+          for (int j = 0; j < nn; ++j) {
+            const int kl = n0 + j;
+            const int i = mis + kl / d + kKUp - (16 * ch + rr);
+            if (i < -kKUp || i >= kKUp) continue;
+            pblob[j / half][base + ((size_t)(rr >> 3) * half + (j % half)) * 8 + (rr & 7)] = __float2half_rn((float)w[(size_t)(i + kKUp) * d + kl % d]);
+          }
+        PairItem& it = U.item[v][U.n_items[v]++];
+        it.idesc = (1u << 4) | ((uint32_t)(nn >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
+        it.p_lo = (uint32_t)((base * sizeof(__half)) >> 4) | ((uint32_t)half << 16);     // LBO = half * 16 bytes
+        it.d_col = (uint32_t)n0;
+        it.ch = (uint32_t)ch;
       }
     }
   }
-  pl->p_bytes = (int)(pblob.size() * sizeof(__half));
-  for (int r = 0; r < pl->n_lr; ++r)                       // the kernels rely on: active chunks of a variant are consecutive,
-    for (int v = 0; v < pl->up[r].n_var; ++v) {            // and only a window start that alternates with t has two variants
-      int first = -1, last = -1, cnt = 0;
-      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch)
-        if (pl->up[r].nn[v][ch]) { if (first < 0) first = ch; last = ch; ++cnt; }
-      if (cnt == 0 || last - first + 1 != cnt) return true;
-    }
+  pl->p_bytes = (int)((pblob[0].size() * sizeof(__half) + 127) / 128 * 128);
+  pl->q_bytes = q_bytes;
 
-  // per-bin shared-memory limits: stationary R (single-buffered) + P + 4 ring stages / stationary R + 4 ring stages
+  // per-(bin, detector) shared-memory limits: stationary R (this CTA's 128 rows) + P + windows + >= 3 y stages
   {
-    const int lim_f0 = (RC16_SMEM_BUDGET - pl->p_bytes - 4 * RC16_STAGE) / 512;
-    const int lim_low = (RC16_SMEM_BUDGET - 4 * RC16_STAGE) / 512;
+    const int lim_f0 = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * PK_YSTAGE) / 256;
+    const int lim_low = (PK_SMEM_BUDGET - 3 * PK_YSTAGE) / 256;
     for (int b = 0; b < n_bd; ++b) {
       if (pl->bd_host[b].l_sum > lim_f0) pl->excluded[b] = 1;
       for (int r = 0; r < pl->n_lr; ++r)
@@ -853,25 +803,12 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
     if (pl->combos_host.empty()) return true;             // nothing fits: the whole bank goes to the FFMA kernels
   }
-
-  // shared-memory budgets (operands stationary: R of the CTA's template block, and P)
-  // R double-buffered (no bubble at a unit switch) when that still leaves >= 8 ring stages
-  pl->f0_r_bufs = (RC16_SMEM_BUDGET - 2 * pl->l_sum_f0_max * 512 - pl->p_bytes) / RC16_STAGE >= 8 ? 2 : 1;
-  const int f0_fixed = pl->f0_r_bufs * pl->l_sum_f0_max * 512 + pl->p_bytes;
-  const int low_fixed = pl->l_sum_low_max * 512;
-  pl->f0_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - f0_fixed) / RC16_STAGE);
-
-  pl->low_stages = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - low_fixed) / RC16_STAGE);
-  if (f0_fixed > RC16_SMEM_BUDGET || low_fixed > RC16_SMEM_BUDGET || pl->f0_stages < 4 || (pl->n_lr > 0 && pl->low_stages < 4)) return true;
-  pl->f0_smem = f0_fixed + pl->f0_stages * RC16_STAGE;
-  pl->low_smem = low_fixed + pl->low_stages * RC16_STAGE;
-  for (int r = 0; r < pl->n_lr; ++r) {                     // per rate class: R as large as its largest group, the rest is ring
-    int lmax = 0;
-    for (int b = 0; b < n_bd; ++b) if (!pl->excluded[b]) lmax = std::max(lmax, pl->groups_host[(size_t)b * pl->n_lr + r].l_sum);
-    pl->low_geom.r_bytes[r] = lmax * 512;
-    pl->low_geom.n_stages[r] = std::min(RC16_MAX_STAGES, (RC16_SMEM_BUDGET - lmax * 512) / RC16_STAGE);
-    pl->low_smem = std::max(pl->low_smem, lmax * 512 + pl->low_geom.n_stages[r] * RC16_STAGE);
-  }
+  const int f0_fixed = pl->l_sum_f0_max * 256 + pl->p_bytes + pl->q_bytes;
+  const int low_fixed = pl->l_sum_low_max * 256;
+  pl->f0_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - f0_fixed) / PK_YSTAGE);
+  pl->low_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - low_fixed) / PK_YSTAGE);
+  pl->f0_smem = f0_fixed + pl->f0_stages * PK_YSTAGE;
+  pl->low_smem = low_fixed + pl->low_stages * PK_YSTAGE;
 
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
@@ -882,24 +819,24 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
       if (G.n_slices == 0 || pl->excluded[b]) continue;
       void* q = nullptr;
-      if (!plan_alloc(pl, &q, (size_t)G.n_rb * G.q_groups_cap * 4096, true, bytes, err, errlen)) return false;
+      if (!plan_alloc(pl, &q, (size_t)G.n_rb * 2 * G.q_groups_cap * 2048, true, bytes, err, errlen)) return false;
       G.Q = (__half*)q;
       for (int rb = 0; rb < G.n_rb; ++rb) {
         units.push_back(LowUnit{b * pl->n_lr + r, rb});
-        low_sched.push_back(SchedUnit{G.l_sum / 32, (int32_t)pl->low_wsum[r]});
-        pl->low_wsum[r] += G.l_sum / 32;
+        low_sched.push_back(SchedUnit{G.l_sum / 16, (int32_t)pl->low_wsum[r]});
+        pl->low_wsum[r] += G.l_sum / 16;
       }
       pl->units_per_rate[r] += G.n_rb;
     }
   }
-  // f0 units = combos; cost per tile = ring stages: y chunks of the d == 1 slices + interpolation chunks
+  // f0 units = combos; cost per tile = MMAs: K / 16 of the d == 1 slices + interpolation chunks
   std::vector<SchedUnit> f0_sched;
   pl->f0_wsum = 0;
   for (const F0Combo& cb : pl->combos_host) {
-    int w = pl->bd_host[cb.bd].l_sum / 32;
+    int w = pl->bd_host[cb.bd].l_sum / 16;
     for (int r = 0; r < pl->n_lr; ++r) {
       if (pl->groups_host[(size_t)cb.bd * pl->n_lr + r].n_slices == 0) continue;
-      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch) w += pl->up[r].nn[0][ch] ? 1 : 0;
+      w += pl->rate[r].n_items[0];
     }
     f0_sched.push_back(SchedUnit{w, (int32_t)pl->f0_wsum});
     pl->f0_wsum += w;
@@ -914,13 +851,18 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   if (!upload((void**)&pl->bd_dev, pl->bd_host.data(), pl->bd_host.size() * sizeof(BdPlan))) return false;
   if (!upload((void**)&pl->combos_dev, pl->combos_host.data(), pl->combos_host.size() * sizeof(F0Combo))) return false;
   if (!upload((void**)&pl->units_dev, units.data(), units.size() * sizeof(LowUnit))) return false;
-  if (!upload((void**)&pl->p_dev, pblob.data(), pblob.size() * sizeof(__half))) return false;
+  {
+    std::vector<uint8_t> both((size_t)2 * pl->p_bytes + 16, 0);
+    for (int c = 0; c < 2; ++c) memcpy(both.data() + (size_t)c * pl->p_bytes, pblob[c].data(), pblob[c].size() * sizeof(__half));
+    if (!upload((void**)&pl->p_dev, both.data(), both.size())) return false;
+  }
   if (!upload((void**)&pl->low_sched_dev, low_sched.data(), low_sched.size() * sizeof(SchedUnit))) return false;
   if (!upload((void**)&pl->f0_sched_dev, f0_sched.data(), f0_sched.size() * sizeof(SchedUnit))) return false;
 
-  cudaError_t e = cudaFuncSetAttribute(f0_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->f0_smem);
-  if (e == cudaSuccess && pl->n_lr > 0)
-    e = cudaFuncSetAttribute(lowrate_recon_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl->low_smem);
+  // opt-in shared memory: the architecture maximum, for every kernel of this file, on this device (never lowered
+  // by a later, smaller bank)
+  cudaError_t e = set_max_dyn_smem(f0_pair_kernel);
+  if (e == cudaSuccess) e = set_max_dyn_smem(lowrate_pair_kernel);
   if (e != cudaSuccess) { snprintf(err, errlen, "fp16 plan: cudaFuncSetAttribute failed: %s", cudaGetErrorString(e)); return false; }
   pl->tensor_recon = true;
   return true;
@@ -930,60 +872,55 @@ bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
 void f16_plan_disable_tensor_recon(F16Plan* pl) { if (pl) pl->tensor_recon = false; }
 const uint8_t* f16_plan_excluded(const F16Plan* pl) { return (pl && pl->tensor_recon && pl->any_excluded) ? pl->excluded.data() : nullptr; }
 
-int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
-                     int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
+int f16_granule_tiles(int peak_window)
 {
+  int gt = peak_window / kTimeTile;
+  while (gt > 32 && gt % 2 == 0) gt /= 2;
+  return gt < 1 ? 1 : gt;
+}
+
+int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int slots_cap, int max_templates,
+                     int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
+{
+  const int n_clusters = std::max(1, pl->n_sm / 2);
   if (pl->low_units > 0) {
-    SchedArgs sc;
-    memset(&sc, 0, sizeof sc);
+    LowPArgs la;
+    memset(&la, 0, sizeof la);
+    la.sp = sp_dev; la.groups = pl->groups_dev; la.units = (const LowUnit*)pl->units_dev;
+    la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages;
+    SchedArgs& sc = la.sched;
     sc.units = pl->low_sched_dev; sc.n_cls = pl->n_lr;
     long long tiles_total = 0;
     for (int r = 0; r < pl->n_lr; ++r) {
       sc.cls_begin[r + 1] = sc.cls_begin[r] + pl->units_per_rate[r];
-      sc.n_tiles[r] = (((c >> pl->up[r].log2d) + 2 * kKUp) + 127) / 128;
+      sc.n_tiles[r] = (((c >> pl->rate[r].log2d) + 2 * kKUp) + 127) / 128;
       sc.cls_base[r + 1] = sc.cls_base[r] + pl->low_wsum[r] * sc.n_tiles[r];
       tiles_total += (long long)sc.n_tiles[r] * pl->units_per_rate[r];
     }
-    const int grid = (int)std::min<long long>(pl->n_sm, tiles_total);
-    lowrate_recon_kernel<<<grid, LOW_THREADS, pl->low_smem, st>>>(sp_dev, pl->groups_dev, (const LowUnit*)pl->units_dev,
-                                                                  sc, pl->low_geom);
+    const int grid = 2 * (int)std::min<long long>(n_clusters, tiles_total);
+    lowrate_pair_kernel<<<grid, PK_THREADS, pl->low_smem, st>>>(la);
     ++*launches;
   }
   if (after_lowrate) cudaEventRecord(after_lowrate, st);
-  if (getenv("LLOID_DEBUG_SYNC") && cudaStreamSynchronize(st) != cudaSuccess) { fprintf(stderr, "lloid: lowrate_recon_kernel faulted\n"); return 1; }
-  F0Args a;
+  if (getenv("LLOID_DEBUG_SYNC") && cudaStreamSynchronize(st) != cudaSuccess) { fprintf(stderr, "lloid: lowrate_pair_kernel faulted\n"); return 1; }
+  F0PArgs a;
   memset(&a, 0, sizeof a);
   a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;
   a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
   a.partials = partials; a.cap = cap; a.k_a = k_a;
-  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 512;
+  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
+  a.nsy = pl->f0_stages; a.slots_cap = slots_cap; a.max_templates = max_templates; a.gt = gt;
   const int n_combos = (int)pl->combos_host.size();
   const int n_tiles = (c + 127) / 128;
   a.sched.units = pl->f0_sched_dev; a.sched.n_cls = 1;
   a.sched.cls_begin[1] = n_combos; a.sched.n_tiles[0] = n_tiles;
   a.sched.cls_base[1] = pl->f0_wsum * n_tiles;
-  // one CTA per SM; a whole number of CTAs per unit (no CTA has to swap R mid-way) only when that leaves at most 3 % of
-  // the SMs idle -- 80 units on 148 SMs ran on 80 CTAs before this rule (a 2x step in the time-versus-bins curve)
-  int grid = pl->n_sm;
-  if (n_combos <= pl->n_sm && n_combos * (pl->n_sm / n_combos) * 100 >= pl->n_sm * 97) grid = n_combos * (pl->n_sm / n_combos);
-  grid = (int)std::min<long long>(grid, (long long)n_combos * n_tiles);
-  a.tiles_cap = tiles_cap; a.max_templates = max_templates; a.nsy = std::max(2, pl->f0_stages / 3); a.nsq = pl->f0_stages - a.nsy; a.r_bufs = pl->f0_r_bufs; a.p_bytes = pl->p_bytes;
-  for (int r = 0; r < kNLowRates; ++r) a.up[r] = pl->up[r];
-  for (int r = 0; r < pl->n_lr; ++r)
-    for (int v = 0; v < pl->up[r].n_var; ++v)
-      for (int ch = 0; ch < (pl->up[r].k_win >> 4); ++ch) {
-        const UpRate& U = pl->up[r];
-        if (!U.nn[v][ch]) continue;
-        QItem& it = a.item[r][v][a.n_items[r][v]++];
-        it.idesc = (1u << 4) | ((uint32_t)(U.nn[v][ch] * 8 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);   // idesc_f16(128, N)
-        it.b_off = (uint32_t)((U.p_off[v] + 2 * ch * 2048 + U.n0[v][ch] * 128) >> 4);
-        it.d_off = (uint32_t)U.n0[v][ch] * 8u;
-        it.ch = (uint32_t)ch;
-      }
-  f0_kernel<<<grid, F0_THREADS, pl->f0_smem, st>>>(a);
+  for (int r = 0; r < kNLowRates; ++r) a.rate[r] = pl->rate[r];
+  const int grid = 2 * (int)std::min<long long>(n_clusters, (long long)n_combos * n_tiles);
+  f0_pair_kernel<<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
   ++*launches;
   const cudaError_t e = cudaPeekAtLastError();
-  if (e != cudaSuccess) fprintf(stderr, "lloid: f0_kernel launch (grid %d, %d threads, %d B shared, %zu B params): %s\n", grid, F0_THREADS, pl->f0_smem, sizeof a, cudaGetErrorString(e));
+  if (e != cudaSuccess) fprintf(stderr, "lloid: f0_pair_kernel launch (grid %d, %d threads, %d B shared, %zu B params): %s\n", grid, PK_THREADS, pl->f0_smem, sizeof a, cudaGetErrorString(e));
   return e == cudaSuccess ? 0 : 1;
 }
 

@@ -19,8 +19,8 @@ __device__ __forceinline__ void ffma2(u64& c, u64 a, u64 b) { asm("fma.rn.f32x2 
 
 // Eight consecutive l of one reconstruction row i / one y row r, from the fp32 row-major arrays or (PK: the fp16
 // path's CUDA-core fallback for banks the tensor reconstruction cannot hold) from the packed fp16 operands, where the
-// same eight values are one 16-byte core-matrix row:  R16[p / 128][l / 8][part][p % 128][l % 8] with i = 2 p + part,
-// Y16[r / 128][l / 8][r % 128][l % 8].  l is a multiple of 8.
+// same eight values are one 16-byte core-matrix row:  R16[i / 128][l / 8][i % 128][l % 8],
+// Y16[r / 64][l / 8][r % 64][l % 8].  l is a multiple of 8.
 __device__ __forceinline__ void h8_to_f(const uint4 v, float4& lo, float4& hi)
 {
   const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
@@ -32,9 +32,8 @@ template <bool PK>
 __device__ __forceinline__ const char* base8_R(const SliceParams& P, int i, int l, int& step)
 {
   if constexpr (PK) {
-    const int p = i >> 1;
-    step = 2 * 128 * 8 * 2;
-    return reinterpret_cast<const char*>(P.R16 + ((((size_t)(p >> 7) * (P.L_pad >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8);
+    step = 128 * 8 * 2;
+    return reinterpret_cast<const char*>(P.R16 + (((size_t)(i >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (i & 127)) * 8);
   } else {
     step = 32;
     return reinterpret_cast<const char*>(P.R32 + (size_t)i * P.L_pad + l);
@@ -44,8 +43,8 @@ template <bool PK>
 __device__ __forceinline__ const char* base8_Y(const SliceParams& P, int r, int l, int& step)
 {
   if constexpr (PK) {
-    step = 128 * 8 * 2;
-    return reinterpret_cast<const char*>(reinterpret_cast<const __half*>(P.Y) + (((size_t)(r >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (r & 127)) * 8);
+    step = 64 * 8 * 2;
+    return reinterpret_cast<const char*>(reinterpret_cast<const __half*>(P.Y) + (((size_t)(r >> 6) * (P.L_pad >> 3) + (l >> 3)) * 64 + (r & 63)) * 8);
   } else {
     step = 32;
     return reinterpret_cast<const char*>(reinterpret_cast<const float*>(P.Y) + (size_t)r * P.L_pad + l);
@@ -158,11 +157,6 @@ void launch_fir_f32(const SliceParams* sp_dev, const SliceParams* sp_host, int n
   }
   const int zs_len = FIR_TM + ((max_taps + FIR_KC - 1) / FIR_KC) * FIR_KC + 16;
   const size_t smem = sizeof(float) * ((size_t)zs_len + FIR_KC * FIR_US);
-  static size_t configured = 0;
-  if (smem > 48 * 1024 && smem > configured) {
-    cudaFuncSetAttribute(fir_f32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = smem;
-  }
   dim3 grid((max_rows + FIR_TM - 1) / FIR_TM, max_lt, n_problems);
   fir_f32_kernel<<<grid, 128, smem, st>>>(sp_dev, rates_dev, o, c, zs_len);
   ++*launches;
@@ -376,20 +370,20 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
       for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
         const int e = tid + 256 * i;
         const int ll = e % RC_KC, row = e / RC_KC;
-        if (Y16) {                                   // packed fp16: R16[p / 128][l / 8][part][p % 128][l % 8]
-          const int i = row0 + row, p = i >> 1, l = l0 + ll;
-          Rs[ll * RC_RS + row] = __half2float(P.R16[((((size_t)(p >> 7) * (Lp >> 3) + (l >> 3)) * 2 + (i & 1)) * 128 + (p & 127)) * 8 + (l & 7)]);
+        if (Y16) {                                   // packed fp16: R16[i / 128][l / 8][i % 128][l % 8]
+          const int i = row0 + row, l = l0 + ll;
+          Rs[ll * RC_RS + row] = __half2float(P.R16[(((size_t)(i >> 7) * (Lp >> 3) + (l >> 3)) * 128 + (i & 127)) * 8 + (l & 7)]);
         } else {
           Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
         }
       }
-      if (Y16) {                                     // packed fp16: Y16[row / 128][l / 8][row % 128][l % 8]
+      if (Y16) {                                     // packed fp16: Y16[row / 64][l / 8][row % 64][l % 8]
         const __half* __restrict__ Yh = reinterpret_cast<const __half*>(P.Y);
         for (int e = tid; e < Ks * RC_KC; e += 256) {
           const int le = e & 7, col = (e >> 3) % Ks, lg = (e >> 3) / Ks;
           const int r = r0 + col, l = l0 + lg * 8 + le;
           Ys[(lg * 8 + le) * RC_YS + col] =
-              (r < P.y_rows_cap) ? __half2float(Yh[(((size_t)(r >> 7) * (Lp >> 3) + (l >> 3)) * 128 + (r & 127)) * 8 + le]) : 0.f;
+              (r < P.y_rows_cap) ? __half2float(Yh[(((size_t)(r >> 6) * (Lp >> 3) + (l >> 3)) * 64 + (r & 63)) * 8 + le]) : 0.f;
         }
       } else {
         for (int e = tid; e < Ks * RC_KC; e += 256) {
@@ -488,12 +482,6 @@ void launch_recon_f32(const SliceParams* sp_dev, const BinParams* bp_dev, const 
 {
   (void)bp_host;
   const size_t smem = sizeof(float) * (RC_KC * RC_RS + RC_KC * RC_YS + RC_RT * RC_RHO_S + 16 * 32);
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(recon_f32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(recon_f32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
-  }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
   dim3 grid(n_tiles, (max_rows_pad + RC_RT - 1) / RC_RT, n_bd);
   if (packed16)
@@ -787,12 +775,6 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
                         int max_templates, int c, int64_t k_a, Capture cap, bool packed16, cudaStream_t st, int64_t* launches)
 {
   const size_t smem = sizeof(float) * (RQ_K * RQ_S + RQ_K * RQ_SB + RQ_T * RQ_RHO_S + 16 * 32);
-  static bool configured = false;
-  if (!configured) {
-    cudaFuncSetAttribute(recon_f32_q_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaFuncSetAttribute(recon_f32_q_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    configured = true;
-  }
   const int n_tiles = (c + RC_CT - 1) / RC_CT;
   dim3 grid(n_tiles, (max_rows_pad + RQ_T - 1) / RQ_T, n_bd);
   if (packed16)
@@ -802,6 +784,19 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
     recon_f32_q_kernel<false><<<grid, 256, smem, st>>>(sp_dev, bp_dev, upw_dev, groups_dev, partials, tiles_cap, max_templates,
                                                       c, (long long)k_a, cap);
   ++*launches;
+}
+
+// Opt-in shared memory is a per-device, per-function attribute: set once per bank at finalize (after cudaSetDevice),
+// always to the architecture maximum, so banks on several devices or of different sizes never interfere.
+int configure_f32_kernels()
+{
+  const int m = 227 * 1024;
+  cudaError_t e = set_max_dyn_smem(fir_f32_kernel);
+  if (e == cudaSuccess) e = set_max_dyn_smem(recon_f32_kernel<false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(recon_f32_kernel<true>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(recon_f32_q_kernel<false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(recon_f32_q_kernel<true>);
+  return e == cudaSuccess ? 0 : 1;
 }
 
 }  // namespace lloid

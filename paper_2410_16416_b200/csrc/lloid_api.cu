@@ -73,6 +73,8 @@ struct lloid_bank {
   float* xw = nullptr;
   float* hist = nullptr;
   int H = 0, C = 0, xw_pitch = 0, tiles_cap = 0;
+  int slots_cap = 0, gt = 1;             // partial peaks: slots per chunk and (tensor path) tiles per granule
+  int32_t* slot_tiles_dev = nullptr;     // [n_bd] tiles per partial slot (null: 1 everywhere)
   int S = 0;                             // super-chunk: samples resampled by one A1 launch (multiple of C)
   PeakState* state = nullptr;            // [2][n_bd][max_templates], double-buffered per chunk
   int state_cur = 0;
@@ -127,8 +129,8 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     *U32 = (const float*)du; *R32 = (const float*)dr;
   } else {
     // fp16 path: U packed for the tcgen05 FIR kernel as [tap block of 64][tap group of 8][l < L_pad][8 taps]
-    // (taps zero-padded to a multiple of 64); R packed as R16[p / 128][l / 8][part][p % 128][l % 8]
-    // (lloid_internal.h): the reconstruction kernels bulk-copy a template block straight into MMA layout.
+    // (taps zero-padded to a multiple of 64); R packed as R16[i / 128][l / 8][i % 128][l % 8], rows in their natural
+    // order (lloid_internal.h): a reconstruction CTA bulk-copies its 128-row block straight into MMA layout.
     const int n_kb = (S.n_taps + 63) / 64;
     const size_t nup = (size_t)n_kb * 64 * S.L_pad;
     std::vector<__half> u(nup, __float2half(0.f));
@@ -138,12 +140,10 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
             __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
     std::vector<__half> r(nr, __float2half(0.f));
     const size_t lgs = (size_t)(S.L_pad >> 3);
-    for (int i = 0; i < 2 * B.N; ++i) {
-      const int p = i >> 1, part = i & 1;
+    for (int i = 0; i < 2 * B.N; ++i)
       for (int l = 0; l < S.L; ++l)
-        r[((((size_t)(p >> 7) * lgs + (l >> 3)) * 2 + part) * 128 + (p & 127)) * 8 + (l & 7)] =
+        r[(((size_t)(i >> 7) * lgs + (l >> 3)) * 128 + (i & 127)) * 8 + (l & 7)] =
             __float2half_rn((float)recon[(size_t)i * S.L + l]);
-    }
     void *du, *dr;
     int rc = dev_alloc(b, &du, nup * 2, false); if (rc) return rc;
     rc = dev_alloc(b, &dr, nr * 2, false); if (rc) return rc;
@@ -218,11 +218,11 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
       launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, false, st,
                               &b->last_launches);
       mark(b, st, kTagLowRecon);
-      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->slots_cap,
                          b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
     } else {
       launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
-                       b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
+                       b->partials, b->slots_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
     }
   } else {
     if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, o, c, st, &b->last_launches))
@@ -230,13 +230,13 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     mark(b, st, kTagFir);
     if (int rc = debug_sync("fir_f16_kernel", k_a, st)) return rc;
     if (f16_plan_tensor_recon(b->plan16)) {
-      if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, st,
+      if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->slots_cap, b->max_templates, c, k_a, b->gt, b->cap, st,
                            &b->last_launches, grab(b, kTagLowRecon)))
         return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
       if (b->q32_dev) {                              // mixed bank: the bins outside the tensor kernels' limits
         launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, true, st,
                                 &b->last_launches);
-        launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+        launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->slots_cap,
                            b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
       }
     } else if (b->q32_dev) {
@@ -245,17 +245,17 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
       launch_lowrate_gemm_f32(b->sp_dev, b->q32_dev, b->q32_host.data(), (int)b->q32_host.size(), b->max_rows_pad, c, true, st,
                               &b->last_launches);
       mark(b, st, kTagLowRecon);
-      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->tiles_cap,
+      launch_recon_f32_q(b->sp_dev, b->bp_dev, b->n_bd, b->max_rows_pad, b->upw_dev, b->q32_dev, b->partials, b->slots_cap,
                          b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
     } else {
       launch_recon_f32(b->sp_dev, b->bp_dev, b->bp_host.data(), b->n_bd, b->max_rows_pad, b->upw_dev,
-                       b->partials, b->tiles_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
+                       b->partials, b->slots_cap, b->max_templates, c, k_a, b->cap, true, st, &b->last_launches);
     }
   }
   mark(b, st, kTagRecon);
   if (int rc = debug_sync("reconstruction kernels", k_a, st)) return rc;
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
-  launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->tiles_cap, c, k_a,
+  launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->slots_cap, b->slot_tiles_dev, c, k_a,
                        b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
                        b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
   b->state_cur ^= 1;
@@ -432,15 +432,40 @@ int lloid_bank_finalize(lloid_bank_t* b)
   H = round_up(H, 256);
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
   int64_t C = b->cfg.max_chunk;
+  size_t mem_free = 0, mem_total = 0;
+  CU(cudaMemGetInfo(&mem_free, &mem_total));
   if (C == 0) {
     // Every chunk costs four kernel boundaries (launch gap, prologue with TMEM allocation and the stationary
-    // operands, pipeline fill and drain: ~60 us in total, measured), so chunks are made LONG: up to 2^17 samples,
-    // bounded by 12 GiB of chunk-local intermediates (y^s and the low-rate rho^(d)).  Keeping the intermediates
-    // L2-resident with short chunks was measured slower on every config: fp16 100 bins 3.50e8 at
-    // 24576 samples, 3.58e8 at 65536; fp32 config 2 243 ms per 1024 s at 34816 samples (y^s in L2), 235 ms at 131072.
-    const double budget = 12.0 * 1024 * 1024 * 1024;
+    // operands, pipeline fill and drain), and every low-rate slice computes 2 K_up halo rows and rounds its rows up to
+    // 128-row MMA tiles per chunk, so chunks are made LONG: up to 2^17 samples, bounded by the chunk-local
+    // intermediates (y^s and the low-rate rho^(d)), which may take 40 % of the free device memory (4 ... 64 GiB).
+    // BASELINE config 2 (2 (bin, detector) pairs): 131072 samples = 1.2 GB; config 4 (3000 pairs): 4096 samples = 58 GB.
+    double budget = 0.4 * (double)mem_free;
+    budget = std::min(std::max(budget, 4.0 * 1024 * 1024 * 1024), 64.0 * 1024 * 1024 * 1024);
     C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
     C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
+  }
+  {
+    // the allocations below, estimated up front so that a bank that cannot fit fails with a message instead of a
+    // cudaMalloc error half-way through (intermediates dominate; 128-row paddings and the halo included)
+    double need = 0.0;
+    for (const BinHost& B : b->bins)
+      for (const SliceHost& S : B.slices) {
+        const double rows = (S.d == 1) ? (double)C : (double)C / S.d + 2 * Ku;
+        need += (double)D * (std::ceil(rows / 128.0) * 128.0) * S.L_pad * esize;
+      }
+    if (b->f16)
+      for (const BinHost& B : b->bins) {
+        bool seen[kMaxRates] = {false, false, false, false, false, false};
+        for (const SliceHost& S : B.slices) {
+          if (S.d == 1 || seen[S.log2d]) continue;
+          seen[S.log2d] = true;
+          need += (double)D * ((std::ceil(((double)C / S.d + 2 * Ku) / 128.0) * 16 + 16) * 8) * B.rows_pad * 2.0;
+        }
+      }
+    if (need > 0.95 * (double)mem_free)
+      return fail(LLOID_ENOMEM, "bank does not fit: chunk-local intermediates need %.1f GB at a chunk of %lld samples, %.1f GB of device memory are free "
+                                "(reduce max_chunk, the number of bins per bank, or shard the bins over more GPUs)", need * 1e-9, (long long)C, (double)mem_free * 1e-9);
   }
   b->H = (int)H; b->C = (int)C;
   // A1 runs once per super-chunk of S samples (not per chunk): the strain is tiny (8 KB/s per detector), so a
@@ -532,11 +557,11 @@ int lloid_bank_finalize(lloid_bank_t* b)
 
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
   rc = dev_alloc(b, (void**)&b->state, 2 * nstate * sizeof(PeakState), false); if (rc) return rc;
-  rc = dev_alloc(b, (void**)&b->partials, nstate * b->tiles_cap * sizeof(Peak), true); if (rc) return rc;
   rc = dev_alloc(b, (void**)&b->stage_count, 8, true); if (rc) return rc;
   launch_reset_state(b->state, 2 * (int64_t)nstate, 0);
   CU(cudaDeviceSynchronize());
 
+  if (configure_common_kernels() || configure_f32_kernels()) return fail(LLOID_ECUDA, "cudaFuncSetAttribute failed: %s", cudaGetErrorString(cudaGetLastError()));
   if (b->f16) {
     char err[256] = {0};
     const double* up_w[kMaxRates];
@@ -573,6 +598,21 @@ int lloid_bank_finalize(lloid_bank_t* b)
       CU(cudaMemcpy(b->q32_dev, b->q32_host.data(), b->q32_host.size() * sizeof(Q32Group), cudaMemcpyHostToDevice));
     } else if (excl) {
       f16_plan_disable_tensor_recon(b->plan16);      // > 8 same-rate slices in an excluded bin: single fused CUDA-core kernel for the bank
+    }
+  }
+  // partial peaks: the tensor kernels write one record per (template, granule of gt tiles), the CUDA-core kernels one
+  // per tile; a mixed bank keeps per-tile slots for everyone and tells the merge kernel which rule a (bin, detector) uses
+  {
+    const bool tensor = b->f16 && f16_plan_tensor_recon(b->plan16);
+    b->gt = tensor ? f16_granule_tiles(b->cfg.peak_window) : 1;
+    const bool per_tile = !tensor || excl != nullptr;
+    b->slots_cap = per_tile ? b->tiles_cap : (int)(C / kTimeTile) / b->gt + 2;
+    rc = dev_alloc(b, (void**)&b->partials, nstate * b->slots_cap * sizeof(Peak), true); if (rc) return rc;
+    if (tensor) {
+      std::vector<int32_t> stl(b->n_bd, b->gt);
+      if (excl) for (int bd = 0; bd < b->n_bd; ++bd) if (excl[bd]) stl[bd] = 1;
+      rc = dev_alloc(b, (void**)&b->slot_tiles_dev, stl.size() * sizeof(int32_t), false); if (rc) return rc;
+      CU(cudaMemcpy(b->slot_tiles_dev, stl.data(), stl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
     }
   }
   b->finalized = true;

@@ -22,7 +22,7 @@ constexpr int kKUp = 8;            // interpolation half-width supported by the 
 constexpr int kTimeTile = 128;     // f0 samples per epilogue tile; chunk starts are aligned to it
 constexpr int kMaxRates = 6;       // d in {1,2,4,8,16,32}
 constexpr int kRowPad = 128;       // reconstruction rows padded to a multiple of this (fp32 path)
-constexpr int kRowPad16 = 256;     // fp16 path: 2 x 128 templates per reconstruction CTA
+constexpr int kRowPad16 = 256;     // fp16 path: a CTA pair reconstructs 2 x 128 rows = 128 templates
 constexpr int kMaxGroupSlices = 8; // slices of one (bin, detector) that share a rate
 constexpr int kMaxF0Slices = 4;    // full-rate (d == 1) slices of one (bin, detector)
 constexpr int kLPad = 32;          // basis count padded to a multiple of this
@@ -75,7 +75,20 @@ struct Q32Group {
   float*  Q;
 };
 
+// Opt-in dynamic shared memory of a kernel: the architecture maximum (227 KB per CTA) minus the kernel's static part.
+// A per-device, per-function attribute: set at finalize on the bank's device, always to the maximum, so banks of
+// different sizes or on different devices never lower each other's limit.
+template <class F> inline cudaError_t set_max_dyn_smem(F f)
+{
+  cudaFuncAttributes at;
+  cudaError_t e = cudaFuncGetAttributes(&at, f);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - (int)at.sharedSizeBytes);
+}
+
 // ---- launchers (one translation unit per kernel family) ---------------------------------------
+int configure_common_kernels();    // opt-in shared memory of every kernel of the TU, on the current device (finalize)
+int configure_f32_kernels();
 void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, int n_rates,
                      const float* xw, int xw_pitch, int xw_valid, int n_det, int k_dn, int c,
                      bool want_f16, cudaStream_t st, int64_t* launches);
@@ -99,9 +112,10 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
                         const float* const* upw_dev, const Q32Group* groups_dev, Peak* partials, int tiles_cap,
                         int max_templates, int c, int64_t k_a, Capture cap, bool packed16, cudaStream_t st, int64_t* launches);
 
+// partials: [bd][slot][template]; slot_tiles_dev[bd] = tiles per slot of that (bin, detector) (null: 1 everywhere)
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                          int tiles_cap, int c, int64_t k_a, int W, float theta, const PeakState* state_in,
-                          PeakState* state_out, int n_det, void* triggers, int64_t capacity,
+                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, int W, float theta,
+                          const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
                           unsigned long long* count, cudaStream_t st, int64_t* launches);
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
@@ -110,18 +124,19 @@ void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
 //
 // Packed fp16 layouts (all are the tcgen05 no-swizzle K-major canonical layout: a core matrix is 8 rows x
 // 8 fp16 = 128 contiguous bytes, so every operand tile is fetched with plain 1-D bulk copies):
-//   Y16  [time tile of 128 rows][l / 8][row % 128][l % 8]           y^s, written by the FIR kernel
-//   R16  [rb = p / 128][l / 8][part][p % 128][l % 8]                R^s, part 0 = cos rows 2p, 1 = sin rows 2p+1
-//   Q16  [rb][j / 8][part][p % 128][j % 8]                          rho^(d) = sum over the slices at rate d of R^s y^s
-constexpr int kTplBlock = 128;     // complex templates per reconstruction CTA (two M = 128 accumulators: re, im)
+//   Y16  [time tile of 64 rows][l / 8][row % 64][l % 8]             y^s, written by the FIR kernel; a CTA of a pair
+//                                                                   supplies one 64-row tile of a 128-sample MMA tile
+//   R16  [rb = i / 128][l / 8][i % 128][l % 8]                      R^s, rows i = 2p (cos), 2p + 1 (sin) in natural order
+//   Q16  [rb][j / 8][i % 128][j % 8]                                rho^(d) = sum over the slices at rate d of R^s y^s
+constexpr int kTplBlock = 128;     // complex templates per CTA PAIR (M = 256 rows: 128 per CTA)
 constexpr int kNLowRates = kMaxRates - 1;
 
 struct RateGroup {                 // one per (bin, detector, distinct rate with d > 1)
   int32_t  n_slices;               // 0: this (bin, detector) has no slice at this rate
   int32_t  slice[kMaxGroupSlices]; // indices into the SliceParams table
   int32_t  log2d, q_groups_cap;    // q_groups_cap: allocated groups of 8 low-rate samples per template block
-  int32_t  l_sum, n_rb;            // sum of L_pad over the group's slices; template blocks of 128
-  __half*  Q;
+  int32_t  l_sum, n_rb;            // sum of L_pad over the group's slices; pair blocks of 128 templates
+  __half*  Q;                      // [2 n_rb row blocks][q_groups_cap][128][8]
 };
 
 struct BdPlan {                    // one per (bin, detector): what the f0-rate kernel needs
@@ -133,14 +148,23 @@ struct BdPlan {                    // one per (bin, detector): what the f0-rate 
 
 struct F0Combo { int32_t bd, rb; };   // (bin*detector, template block) handled back to back along time
 
-struct UpRate {                    // one per distinct rate with d > 1 (bank-wide): band matrices of A4
-  int32_t log2d, k_win;            // window length in low-rate samples (multiple of 16)
-  int32_t n_var;                   // 1, or 2 when the window start (multiple of 8 rows) alternates 0 / 4 rows off
-  int32_t p_off[2];                // byte offsets of the variants in the P blob, each [k_win / 8][128][8] fp16
-  uint8_t n0[2][8], nn[2][8];      // per variant and 16-row chunk: first output column / 8 and columns / 8 (0: skip)
+// A4 on the tensor cores (f0_pair_kernel): one interpolation MMA = one 16-row chunk of a rate's rho^(d) window times the
+// block of the band matrix P_d its rows touch
+struct PairItem {
+  uint32_t idesc;                  // cta_group::2 instruction descriptor, M = 256, N = columns of the block
+  uint32_t p_lo;                   // descriptor low word of the block relative to the P blob: offset >> 4 | (N / 2) << 16
+  uint32_t d_col;                  // first accumulator column
+  uint32_t ch;                     // chunk index inside the 16-row-aligned window
 };
-
-struct QItem { uint32_t idesc, b_off, d_off, ch; };
+struct PairRate {                  // one per distinct rate with d > 1 (bank-wide)
+  int32_t  log2d;
+  int32_t  adv;                    // low-rate rows per 128-sample tile: 128 / d
+  int32_t  cap_chunks;             // capacity of the rate's circular buffer, in chunks of 16 rows (4 KB per CTA)
+  int32_t  n_var;                  // window start is adv t: 16 / adv alignments of it inside a chunk (1 when adv >= 16)
+  int32_t  ring_off;               // byte offset of the circular buffer in the window area
+  int32_t  n_items[4];
+  PairItem item[4][5];             // per variant: the window's chunks, in order
+};
 
 // Static schedule of a persistent tensor kernel (A7).  Work = units x time tiles; a unit is one stationary
 // operand set (f0 kernel: one (bin, detector, template block); low-rate kernel: the same per rate).  Units are
@@ -166,8 +190,11 @@ void f16_plan_disable_tensor_recon(F16Plan*);
 const uint8_t* f16_plan_excluded(const F16Plan*);   // tensor_recon only: per (bin, detector) flags of the bins left to the FFMA kernels, or null
 int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                     const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches);
-int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int tiles_cap, int max_templates,
-                      int c, int64_t k_a, Capture cap, cudaStream_t st, int64_t* launches,
+// partials of the tensor path: ONE record per (bin, detector, template, granule); a granule is a run of gt tiles
+// aligned to absolute multiples of gt tiles, gt = f16_granule_tiles(W) dividing the peak window
+int  f16_granule_tiles(int peak_window);
+int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int slots_cap, int max_templates,
+                      int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches,
                       cudaEvent_t after_lowrate /* recorded between the two kernels when non-null */);
 
 }  // namespace lloid

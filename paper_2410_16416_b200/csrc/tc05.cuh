@@ -192,4 +192,53 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uin
                :: "r"(dst_smem), "l"(src), "r"(bytes), "r"(mbar) : "memory");
 }
 
+
+// ---- CTA pair (cta_group::2): two CTAs of a 2-CTA cluster issue ONE MMA with M = 256 -----------------
+// D rows [0,128) live in the TMEM of cluster rank 0, rows [128,256) in rank 1; each CTA supplies its own 128 rows of
+// A and HALF of B (rank 0: B rows [0, N/2), rank 1: [N/2, N)) from the same shared-memory offsets.  Only the leader
+// (rank 0) issues; tcgen05.commit with a CTA mask arrives on the barrier at the same offset in every masked CTA.
+// A 32-bit shared::cta address is also a valid shared::cluster address of the executing CTA; clearing bit 24 gives
+// the leader's copy of the same offset (measured on B200: a plain bulk copy cannot signal the peer's barrier -- it
+// hangs -- so the peer relays "my half has landed" with a remote arrive instead).
+constexpr uint32_t kLeaderMask = 0xFEFFFFFFu;
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync()
+{
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t idesc_f16_pair(int N) { return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(256 >> 4) << 24); }
+__device__ __forceinline__ void mma2_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+               :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrives (once every tcgen05 op issued so far by this thread has completed) on [mbar] of every CTA in cta_mask
+__device__ __forceinline__ void commit2(uint32_t mbar, uint16_t cta_mask)
+{
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               :: "r"(mbar), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void tmem_alloc2(uint32_t* slot_in_smem, uint32_t cols)     // one warp of EACH CTA of the pair
+{
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(slot_in_smem)), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc2(uint32_t taddr, uint32_t cols)
+{
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(taddr), "r"(cols) : "memory");
+}
+// arrive on a barrier given by its shared::cluster address (own or peer CTA), release at cluster scope
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t mbar_cluster)
+{
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(mbar_cluster) : "memory");
+}
+// wait with acquire at cluster scope (the arrivals may come from the peer CTA)
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t mbar, uint32_t parity)
+{
+  asm volatile("{\n\t.reg .pred p;\n\tWAITC_%=:\n\t"
+               "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+               "@p bra DONEC_%=;\n\tbra WAITC_%=;\n\tDONEC_%=:\n\t}\n" :: "r"(mbar), "r"(parity) : "memory");
+}
+
 }}  // namespace lloid::tc
