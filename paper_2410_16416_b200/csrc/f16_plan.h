@@ -23,7 +23,9 @@ struct F16Plan {
   bool any_excluded = false;
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
-  int f0_smem = 0, f0_stages = 0;
+  int f0_smem = 0, f0_stages = 0, f0_ystage = 0, low_ystage = 0;   // ystage: bytes of a y ring slot per CTA
+  PairMma tab[kPairTabMax];             // interpolation MMA table of the f0 kernel (kernel parameter)
+  int n_tab = 0;
   int p_bytes = 0, q_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;   // per CTA: band-matrix blob, rho^(d) window buffers
   PairRate rate[kNLowRates];
   std::vector<RateGroup> groups_host;   // [n_bd][n_lr]
@@ -36,7 +38,8 @@ struct F16Plan {
   void* units_dev = nullptr;            // LowUnit[low_units], rate-major
   int units_per_rate[kNLowRates] = {0, 0, 0, 0, 0};
   SchedUnit* low_sched_dev = nullptr;   // [low_units]   cost per tile of every low-rate unit
-  SchedUnit* f0_sched_dev = nullptr;    // [combos]      cost per tile of every f0 unit
+  SchedBd* f0_sched_dev = nullptr;      // [f0_n_bds]    f0 kernel schedule entries
+  int f0_n_bds = 0;
   long long low_wsum[kNLowRates] = {0, 0, 0, 0, 0};
   long long f0_wsum = 0;
   std::vector<void*> owned;

@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(FH_THREADS, 1)
 fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict__ rates, int o, int c, int n_stages)
 {
   const SliceParams P = sp[blockIdx.y];
-  const int rows_needed = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+  const int rows_needed = (c >> P.log2d) + P.fir_halo;
   const int L_pad = P.L_pad;
   const int MT = fir_mt(L_pad);
   const int r0 = blockIdx.x * 128 * MT;
@@ -155,7 +155,7 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     __half* __restrict__ Y = reinterpret_cast<__half*>(P.Y);
     const size_t lgs = (size_t)(L_pad >> 3);
     for (int mt = 0; mt < mt_used; ++mt) {
-      const int row = r0 + mt * 128 + q * 32 + lane;
+      const int row = (r0 + mt * 128 + q * 32 + lane) * P.out_mul + P.out_add;           // folded slice: phase rows interleave
       __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
       for (int c0 = 0; c0 < L_pad; c0 += 16) {
@@ -206,7 +206,7 @@ __device__ __forceinline__ FirUnit fir_unit(const SliceParams* __restrict__ sp, 
   const SliceParams* P = sp + U.p;
   const int d = P->d, log2d = P->log2d, n_taps = P->n_taps;
   U.L_pad = P->L_pad;
-  const int rows_needed = (d == 1) ? c : (c >> log2d) + 2 * kKUp;
+  const int rows_needed = (c >> log2d) + P->fir_halo;
   const int MT = fir_mt(U.L_pad);
   U.r0 = e.y * 128 * MT;
   U.valid = U.r0 < rows_needed;
@@ -353,7 +353,7 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
       mbar_wait(smem_u32(&acc_full), (uint32_t)k & 1u);
       fence_after();
       for (int mt = 0; mt < U.mt_used; ++mt) {
-        const int row = U.r0 + mt * 128 + q * 32 + lane;
+        const int row = (U.r0 + mt * 128 + q * 32 + lane) * P->out_mul + P->out_add;       // folded slice: phase rows interleave
         __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
         for (int c0 = 0; c0 < L_pad; c0 += 32) {
@@ -385,7 +385,8 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
 }
 
 // ------------------------------------------------------------------------------------------------
-F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd, int n_det,
+F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const SliceParams* fir_host, int n_fir,
+                         const BinParams* bp_host, int n_bd, int n_det,
                          int chunk_cap, const double* const* up_w, int64_t* bytes, char* err, int errlen)
 {
   (void)n_det;
@@ -393,8 +394,8 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
   pl->chunk_cap = chunk_cap;
   size_t fixed = 0, stage = 0;
   int gx = 1;
-  for (int i = 0; i < n_problems; ++i) {
-    const SliceParams& P = sp_host[i];
+  for (int i = 0; i < n_fir; ++i) {
+    const SliceParams& P = fir_host[i];
     if (P.L_pad > 512 || (P.L_pad > 256 && P.L_pad % 32)) { snprintf(err, errlen, "fp16 path: L_pad %d unsupported", P.L_pad); delete pl; return nullptr; }
     int mt = 512 / P.L_pad; mt = mt > 4 ? 4 : (mt < 1 ? 1 : mt);
     const int n_pad = (P.n_taps + FH_KB - 1) / FH_KB * FH_KB;
@@ -403,7 +404,7 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
     fixed = f > fixed ? f : fixed;
     const size_t st = (size_t)P.L_pad * FH_KB * 2;
     stage = st > stage ? st : stage;
-    const int rows = (P.d == 1) ? chunk_cap : (chunk_cap >> P.log2d) + 2 * kKUp;
+    const int rows = (chunk_cap >> P.log2d) + P.fir_halo;
     const int g = (rows + 128 * mt - 1) / (128 * mt);
     gx = g > gx ? g : gx;
   }
@@ -425,10 +426,10 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinPa
     pl->fir_pers_stages = std::min<int>(FH_MAX_STAGES, (int)((budget - 2 * fixed) / stage));
     pl->fir_pers_smem = (int)(2 * fixed + (size_t)pl->fir_pers_stages * stage);
     size_t cap_units = 0;
-    for (int i = 0; i < n_problems; ++i) {
-      const SliceParams& P = sp_host[i];
+    for (int i = 0; i < n_fir; ++i) {
+      const SliceParams& P = fir_host[i];
       const int mt = fir_mt_host(P.L_pad);
-      const int rows = (P.d == 1) ? chunk_cap : (chunk_cap >> P.log2d) + 2 * kKUp;
+      const int rows = (chunk_cap >> P.log2d) + P.fir_halo;
       cap_units += (size_t)(rows + 128 * mt - 1) / (128 * mt);
     }
     bool ok = set_max_dyn_smem(fir_f16_pers_kernel) == cudaSuccess;
@@ -463,7 +464,7 @@ static int fir_build_list(F16Plan* pl, const SliceParams* sp_host, int n_problem
   for (int i = 0; i < n_problems; ++i) {
     const SliceParams& P = sp_host[i];
     const int mt = fir_mt_host(P.L_pad);
-    const int rows = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+    const int rows = (c >> P.log2d) + P.fir_halo;
     const int nb = (rows + 128 * mt - 1) / (128 * mt);
     const int n_kb = (P.n_taps + FH_KB - 1) / FH_KB;
     for (int r = 0; r < nb; ++r) {
@@ -503,7 +504,7 @@ int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp
   for (int i = 0; i < n_problems; ++i) {
     const SliceParams& P = sp_host[i];
     int mt = 512 / P.L_pad; mt = mt > 4 ? 4 : (mt < 1 ? 1 : mt);
-    const int rows = (P.d == 1) ? c : (c >> P.log2d) + 2 * kKUp;
+    const int rows = (c >> P.log2d) + P.fir_halo;
     const int g = (rows + 128 * mt - 1) / (128 * mt);
     gx = g > gx ? g : gx;
   }

@@ -40,22 +40,47 @@ namespace lloid {
 
 using namespace tc;
 
-constexpr int PK_THREADS = 512;             // 16 warps: 0 PY, 1 IY, 2 PQ, 3 IQ, 4 relay y, 5 relay q, 8-15 epilogue
-constexpr int PK_YSTAGE = 8192;             // bytes per y ring stage per CTA: K = 64 x 64 rows
+constexpr int PK_THREADS = 544;             // 17 warps: 0 PY, 1 IY, 2 PQ0, 3 IQ0, 4 relay y, 5 relay q, 6 PQ1, 8-15 epilogue, 16 IQ1
 constexpr int PK_NSY_MAX = 16;
 constexpr int PK_NACC = 4;                  // accumulator buffers of 128 columns
 constexpr int PK_NQB = 4;                   // rho^(d) tile events in flight (barrier slots)
 constexpr int PK_QDIST = 2;                 // the rows of tile e are requested when tile e - PK_QDIST has been consumed
-constexpr int PK_SMEM_BUDGET = 220 * 1024;  // dynamic; + static (barriers, tables) stays below 227 KB
+constexpr int PK_QPF = 4;                   // L2 prefetch distance of the rho^(d) rows, in tiles
+constexpr int PK_YPF = 4;                   // L2 prefetch distance of the y tiles, in tiles
+constexpr int PK_BLOCK_TILES = 64;          // f0 schedule: the template blocks of a (bin, detector) walk the time axis in blocks of
+                                            // this many tiles, one after the other, so the CTA pairs that share a y tile read it
+                                            // while it is L2-hot (measured before: 2.75 GB of DRAM reads per launch for 1.1 GB of operands)
+constexpr int PK_SMEM_BUDGET = 218 * 1024;  // dynamic; + static (barriers, tables) stays below 227 KB
 
 struct LowUnit { int32_t group, pb; };
 
-struct Ring {                               // stage index + phase parity, advanced without division
-  int s; uint32_t ph; int n;
+// Role trace (scratch builds with -DLLOID_TRACE_BUILD and LLOID_TRACE=1): cycles each single-thread role of cluster 0
+// spends waiting on each of its barriers and in total, accumulated over the launches; read back with lloid_debug_trace.
+__device__ long long g_trace[2][8][8];      // [kernel: 0 low, 1 f0][role][0..5 wait categories, 6 total, 7 tiles]
+#ifdef LLOID_TRACE_BUILD
+#define TWAIT(cat, bar, ph)                                                                       \
+  do { if (trace) { const long long t_ = clock64(); mbar_wait(bar, ph); tw[cat] += clock64() - t_; } else mbar_wait(bar, ph); } while (0)
+#define TRACE_BEGIN() const bool trace = a.trace && (blockIdx.x >> 1) == 0; long long tw[6] = {0, 0, 0, 0, 0, 0}; const long long tbeg = trace ? clock64() : 0
+#define TRACE_END(kern, role, ntiles) do { if (trace) { for (int i_ = 0; i_ < 6; ++i_) g_trace[kern][role][i_] += tw[i_]; g_trace[kern][role][6] += clock64() - tbeg; g_trace[kern][role][7] += (ntiles); } } while (0)
+#else
+#define TWAIT(cat, bar, ph) mbar_wait(bar, ph)
+#define TRACE_BEGIN() constexpr bool trace = false; long long* const tw = nullptr; (void)trace; (void)tw
+#define TRACE_END(kern, role, ntiles) do { (void)(ntiles); } while (0)
+#endif
+
+// A single thread retires roughly one dependent instruction per 5-7 cycles (measured: a loop around one MMA with ~15
+// instructions of address arithmetic issues an MMA every 99 cycles; with the MMAs and the copies knocked out the handshake
+// skeleton of the first version of this file still took longer than the MMAs).  The role loops below are written for
+// instruction count -- y stages carry up to K = 128, barrier addresses are hoisted, the interpolation MMAs read their
+// operands from a table in the kernel parameters -- and the two MMA-issuing roles exist TWICE, one thread for the even
+// tiles and one for the odd tiles (different accumulators, so the pipe needs no ordering between them).
+struct YRing {                              // y ring position: slot index + phase parity
+  uint32_t s, ph, n;
   __device__ __forceinline__ void advance() { if (++s == n) { s = 0; ph ^= 1u; } }
+  __device__ __forceinline__ void skip(uint32_t k) { s += k; while (s >= n) { s -= n; ph ^= 1u; } }
 };
 
-// ---- static persistent schedule (SchedArgs in lloid_internal.h), per CLUSTER --------------------------
+// ---- static persistent schedule (SchedArgs in lloid_internal.h), per CLUSTER: low-rate kernel ------------
 struct SchedPos { int u, t; };              // unit index, first tile
 
 __device__ __forceinline__ SchedPos sched_locate(const SchedArgs& s, long long b)
@@ -83,24 +108,12 @@ __device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
   return c;
 }
 
-// A range boundary inside a unit is moved up to the next granule start (tiles whose absolute index is a multiple of
-// gt; gt = 1: no snapping): both ends of every range use the same rule, so the ranges still tile the work.
-__device__ __forceinline__ SchedPos sched_snap(const SchedArgs& s, SchedPos p, long long a0, int gt)
-{
-  if (gt <= 1 || p.t == 0 || p.u >= s.cls_begin[s.n_cls]) return p;
-  const int nt = s.n_tiles[sched_class(s, p.u)];
-  const int rem = (int)((a0 + p.t) % gt);
-  if (rem) p.t += gt - rem;
-  if (p.t >= nt) { ++p.u; p.t = 0; }
-  return p;
-}
-
 // this cluster's range -> rng[0..3] = first unit, first tile, last unit, end tile in the last unit
-__device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl, long long a0, int gt, int* rng)
+__device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl, int* rng)
 {
   const long long T = s.cls_base[s.n_cls];
-  const SchedPos a = sched_snap(s, sched_locate(s, T * (long long)cid / (long long)ncl), a0, gt);
-  const SchedPos b = sched_snap(s, sched_locate(s, T * (long long)(cid + 1) / (long long)ncl), a0, gt);
+  const SchedPos a = sched_locate(s, T * (long long)cid / (long long)ncl);
+  const SchedPos b = sched_locate(s, T * (long long)(cid + 1) / (long long)ncl);
   rng[0] = a.u; rng[1] = a.t; rng[2] = b.u; rng[3] = b.t;
 }
 
@@ -109,6 +122,62 @@ __device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl
     if (u == u_hi && t_hi == 0) break;                                                            \
     else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : (NT); t0 >= t1) continue; \
     else
+
+// ---- f0 kernel schedule: (bin-detector, time block, template block, tile) ---------------------------------
+// The flattened work sequence is ordered by (bin, detector), then by BLOCKS of PK_BLOCK_TILES tiles (aligned to absolute
+// tile indices), then by template block, then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends
+// moved up to granule starts.  Neighbouring clusters therefore work on the same (bin, detector, time block) -- the same y
+// tiles -- at the same time, and a cluster still walks at least a granule of consecutive tiles per visit.
+struct F0Sched {
+  const SchedBd* bds;                       // tensor-path (bin, detector) pairs, in order
+  int n_bds, n_tiles, gb, gt;
+  long long total;                          // sum of n_pb * w
+  long long a0;                             // absolute index of the chunk's tile 0
+};
+struct F0Pos { int ib, lo, hi, pb, t; };    // index into bds, block [lo, hi) in chunk tiles, template block, tile
+
+__device__ __forceinline__ int f0_first_block_end(const F0Sched& S) { return min(S.n_tiles, S.gb - (int)(S.a0 % S.gb)); }
+
+__device__ __forceinline__ void f0_next_cell(const F0Sched& S, F0Pos& p)      // next (template block | time block | bd) in order
+{
+  if (++p.pb < S.bds[p.ib].n_pb) { p.t = p.lo; return; }
+  p.pb = 0; p.lo = p.hi; p.hi = min(S.n_tiles, p.hi + S.gb); p.t = p.lo;
+  if (p.lo >= S.n_tiles) { ++p.ib; p.lo = 0; p.hi = f0_first_block_end(S); p.t = 0; }
+}
+
+__device__ __forceinline__ F0Pos f0_locate(const F0Sched& S, long long pos)
+{
+  F0Pos p;
+  const long long nt = S.n_tiles;
+  if (pos >= S.total * nt) { p.ib = S.n_bds; p.lo = 0; p.hi = f0_first_block_end(S); p.pb = 0; p.t = 0; return p; }
+  int lo = 0, hi = S.n_bds - 1;
+  while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.bds[mid].cum * nt <= pos) lo = mid; else hi = mid - 1; }
+  const SchedBd B = S.bds[lo];
+  long long rem = pos - B.cum * nt;
+  const long long cw = (long long)B.n_pb * B.w;
+  p.ib = lo; p.lo = 0; p.hi = f0_first_block_end(S);
+  while (rem >= cw * (p.hi - p.lo) && p.hi < S.n_tiles) { rem -= cw * (p.hi - p.lo); p.lo = p.hi; p.hi = min(S.n_tiles, p.hi + S.gb); }
+  const int len = p.hi - p.lo;
+  p.pb = min((int)(rem / ((long long)B.w * len)), B.n_pb - 1);
+  p.t = p.lo + min((int)((rem - (long long)p.pb * B.w * len) / B.w), len - 1);
+  if (p.t > p.lo) {                         // move up to the next granule start
+    const int r = (int)((S.a0 + p.t) % S.gt);
+    if (r) p.t += S.gt - r;
+    if (p.t >= p.hi) f0_next_cell(S, p);
+  }
+  return p;
+}
+
+// iterates this cluster's segments: (bd entry, template block, tiles [t0, t1))
+struct F0Iter {
+  F0Pos cur, end;
+  __device__ __forceinline__ bool at_end() const
+  { return cur.ib > end.ib || (cur.ib == end.ib && (cur.lo > end.lo || (cur.lo == end.lo && (cur.pb > end.pb || (cur.pb == end.pb && cur.t >= end.t))))); }
+  __device__ __forceinline__ int seg_end() const { return (cur.ib == end.ib && cur.lo == end.lo && cur.pb == end.pb) ? end.t : cur.hi; }
+};
+#define FOR_F0_SEGMENTS(it, S, A, B)                                                              \
+  for (F0Iter it{A, B}; !it.at_end(); f0_next_cell(S, it.cur))                                    \
+    if (it.cur.t >= it.seg_end()) continue; else
 
 __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, uint32_t bytes, uint32_t bar)
 {
@@ -125,19 +194,20 @@ struct PairBars {
   uint64_t consts, unit_done;
 };
 
-// Barrier counts: a "full" barrier of the leader gets two arrivals (its own producer's arrive.expect_tx and the peer's
-// relay), the peer's own copy one.  acc_empty lives in the leader: one arrival per epilogue warp of both CTAs.
-__device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int nsy, uint32_t rank, int warp, int tid)
+// Barrier counts: a "full" barrier of the leader gets its own producers' arrive.expect_tx plus the peer's relay, the peer's
+// own copy only its producers'.  acc_empty lives in the leader: one arrival per epilogue warp of both CTAs.  unit_done is
+// committed by the thread that finishes the unit's LAST tile, after it has seen the other thread's last tile complete.
+__device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int nsy, uint32_t rank, int warp, int tid, uint32_t n_pq)
 {
   if (warp == 0) tmem_alloc2(tmem_slot, 512);
   if (tid == 32) {
-    const uint32_t nfull = rank == 0 ? 2u : 1u;
-    for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), nfull); mbar_init(smem_u32(&B.yempty[s]), 1); }
-    for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), nfull); mbar_init(smem_u32(&B.qempty[s]), 1); }
+    const uint32_t relay = rank == 0 ? 1u : 0u;
+    for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), 1u + relay); mbar_init(smem_u32(&B.yempty[s]), 1); }
+    for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), n_pq + relay); mbar_init(smem_u32(&B.qempty[s]), 1); }
     for (int b = 0; b < PK_NACC; ++b) {
       mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 16); mbar_init(smem_u32(&B.ybar[b]), 1);
     }
-    mbar_init(smem_u32(&B.consts), nfull);
+    mbar_init(smem_u32(&B.consts), 1u + relay);
     mbar_init(smem_u32(&B.unit_done), 1);
     mbar_init_fence();
   }
@@ -155,22 +225,18 @@ __device__ __forceinline__ void pair_teardown(uint32_t tmem, int warp)
   if (warp == 0) tmem_dealloc2(tmem, 512);
 }
 
-// producer: wait for the slot to be free, then one bulk copy of `bytes` (<= PK_YSTAGE)
-__device__ __forceinline__ void produce(Ring& rg, uint32_t bars_full, uint32_t bars_empty, uint32_t ring_base, const uint8_t* src, uint32_t bytes)
-{
-  mbar_wait(bars_empty + 8u * rg.s, rg.ph ^ 1u);
-  mbar_expect_tx(bars_full + 8u * rg.s, bytes);
-  bulk_g2s(ring_base + (uint32_t)rg.s * PK_YSTAGE, src, bytes, bars_full + 8u * rg.s);
-  rg.advance();
-}
+// y stages of a slice with nm = L_pad / 16 MMAs per tile: ceil(nm / 8) stages of nearly equal size (<= 8 MMAs, K <= 128)
+__host__ __device__ inline int stage_count(int nm) { return (nm + 7) >> 3; }
 
-// One y stage (K = ks, a multiple of 16, <= 64) of a reconstruction: D (+)= R[l-groups from a_lo] * stage^T, N = 128.
-// a_lo: descriptor of R at this K offset (LBO 2048: 128 rows per l-group); b_lo: descriptor of the stage (LBO 1024: 64 rows)
-__device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, int ks, uint32_t& first)
+// m back-to-back MMAs of one y stage: D (+)= R[l-groups from a_lo] * stage^T, N = 128.  a_lo: descriptor of R at this K
+// offset (LBO 2048: 128 rows per l-group, 256 sixteen-byte units per K = 16); b_lo: the stage (LBO 1024: 64 rows, 128 units)
+__device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, int m, uint32_t acc0)
 {
-  for (int k16 = 0; k16 < (ks >> 4); ++k16) {
-    mma2_ss(d_tmem, desc64(a_lo + (uint32_t)k16 * 256u), desc64(b_lo + (uint32_t)k16 * 128u), idesc, first ? 0u : 1u);
-    first = 0u;
+  mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, acc0);
+#pragma unroll 4
+  for (int k = 1; k < m; ++k) {
+    a_lo += 256u; b_lo += 128u;
+    mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, 1u);
   }
 }
 
@@ -178,84 +244,109 @@ __device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint
 struct SegSrc {                             // per-role copy of the current unit's operand sources (this CTA's halves)
   const uint8_t* Y[kMaxGroupSlices];        // slice's Y16 base
   const uint8_t* Rsrc[kMaxGroupSlices];     // this CTA's 128-row block of the slice's R16
-  int L[kMaxGroupSlices];
-  int n;
+  int nm[kMaxGroupSlices];                  // L_pad / 16
+  int nst[kMaxGroupSlices], mbase[kMaxGroupSlices], ext[kMaxGroupSlices];   // stages per tile; MMAs per stage: mbase (+ 1 for the first ext)
+  int n, stages_per_tile;
+  uint32_t rbytes;
 };
 
 __device__ __forceinline__ void seg_fill(SegSrc& S, const SliceParams* __restrict__ sp, const int32_t* slice, int n, int rb)
 {
-  S.n = n;
+  S.n = n; S.stages_per_tile = 0; S.rbytes = 0;
   for (int i = 0; i < n; ++i) {             // one thread
     const SliceParams* P = sp + slice[i];
     const int L = P->L_pad;
     S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
     S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 256;
-    S.L[i] = L;
+    S.nm[i] = L >> 4;
+    S.nst[i] = stage_count(L >> 4); S.mbase[i] = (L >> 4) / S.nst[i]; S.ext[i] = (L >> 4) - S.mbase[i] * S.nst[i];
+    S.stages_per_tile += S.nst[i];
+    S.rbytes += (uint32_t)L * 256u;
   }
 }
+
+struct YAddr { uint32_t full0, empty0, dst0, step; };   // barrier arrays and slots of the y ring (dst: address, or descriptor for IY)
 
 // PY role of both kernels: y stages of the unit's slices for tiles [t0, t1) (this CTA's 64-row half of every 128-row
 // tile), and the stationary R of the unit.  R goes out after `pre` stages of the new unit are in flight: the ring refills
 // while the previous unit drains.  extra/extra_bytes: loaded once with the first R (the f0 kernel's band matrices).
-struct PYState { Ring rg; int seg_i; };
-
-__device__ __forceinline__ void py_segment(PYState& st, const SegSrc& sg, PairBars& bars, uint32_t sR_u, uint32_t ring_u,
-                                           uint32_t rank, int t0, int t1, uint32_t extra_dst, const uint8_t* extra, uint32_t extra_bytes)
+__device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i, const SegSrc& sg, uint32_t consts_u, uint32_t unit_done_u, uint32_t sR_u,
+                                           uint32_t rank, int t0, int t1, uint32_t extra_dst, const uint8_t* extra, uint32_t extra_bytes,
+                                           bool trace, long long* tw)
 {
-  const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
-  int stages_per_tile = 0;
-  uint32_t rbytes = 0;
-  for (int i = 0; i < sg.n; ++i) { stages_per_tile += (sg.L[i] + 63) >> 6; rbytes += (uint32_t)sg.L[i] * 256u; }
-  int pre = (st.seg_i == 0) ? 0 : min(st.rg.n, stages_per_tile);
+  int pre = (seg_i == 0) ? 0 : min((int)rg.n, sg.stages_per_tile);
   bool need_R = true;
   auto load_R = [&]() {
-    if (st.seg_i > 0) mbar_wait(smem_u32(&bars.unit_done), (uint32_t)(st.seg_i - 1) & 1u);   // every MMA that reads the old R is complete
-    const uint32_t cb = smem_u32(&bars.consts);
-    mbar_expect_tx(cb, rbytes + (st.seg_i == 0 ? extra_bytes : 0u));
+    if (seg_i > 0) TWAIT(1, unit_done_u, (uint32_t)(seg_i - 1) & 1u);   // every MMA that reads the old R is complete
+    mbar_expect_tx(consts_u, sg.rbytes + (seg_i == 0 ? extra_bytes : 0u));
     uint32_t off = 0;
     for (int i = 0; i < sg.n; ++i) {
-      copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.L[i] * 256u, cb);
-      off += (uint32_t)sg.L[i] * 256u;
+      copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.nm[i] * 4096u, consts_u);
+      off += (uint32_t)sg.nm[i] * 4096u;
     }
-    if (st.seg_i == 0 && extra_bytes) copy_pieces(extra_dst, extra, extra_bytes, cb);
+    if (seg_i == 0 && extra_bytes) copy_pieces(extra_dst, extra, extra_bytes, consts_u);
     need_R = false;
   };
   if (pre == 0) load_R();
   for (int t = t0; t < t1; ++t)
     for (int i = 0; i < sg.n; ++i) {
-      const int L = sg.L[i];
-      const uint8_t* src = sg.Y[i] + (size_t)(2 * t + (int)rank) * L * 128;        // 64-row tiles are contiguous in Y16: L / 8 KB each
-      for (int k0 = 0; k0 < L; k0 += 64, src += PK_YSTAGE) {
-        const int ks = min(64, L - k0);
-        produce(st.rg, bfull, bempty, ring_u, src, (uint32_t)ks * 128u);
+      const int nm = sg.nm[i], nst = sg.nst[i], base = sg.mbase[i], ext = sg.ext[i];
+      const uint8_t* src = sg.Y[i] + (size_t)(2 * t + (int)rank) * nm * 2048;    // 64-row tiles are contiguous in Y16: nm x 2 KB each
+      if (t + PK_YPF < t1) bulk_prefetch_l2(src + (size_t)(2 * PK_YPF) * nm * 2048, (uint32_t)nm * 2048u);   // this CTA's half of tile t + PK_YPF
+      for (int j = 0; j < nst; ++j) {
+        const uint32_t bytes = (uint32_t)(base + (j < ext ? 1 : 0)) * 2048u;
+        const uint32_t full = ya.full0 + 8u * rg.s;
+        TWAIT(0, ya.empty0 + 8u * rg.s, rg.ph ^ 1u);
+        mbar_expect_tx(full, bytes);
+        bulk_g2s(ya.dst0 + rg.s * ya.step, src, bytes, full);
+        rg.advance();
+        src += bytes;
         if (need_R && --pre == 0) load_R();
       }
     }
   if (need_R) load_R();
-  ++st.seg_i;
+  ++seg_i;
 }
 
 // relay role (peer CTA): forwards the completion of this CTA's y stages and R loads to the leader's barriers
-__device__ __forceinline__ void relay_y_segment(Ring& rg, int& seg_i, const SegSrc& sg, PairBars& bars, int t0, int t1)
+__device__ __forceinline__ void relay_y_segment(YRing& rg, const YAddr ya, int& seg_i, int n_stages, uint32_t consts_u)
 {
   // consts first (it is requested before or among the first stages of the unit and the leader needs it first)
-  mbar_wait(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
-  mbar_arrive_cluster(smem_u32(&bars.consts) & kLeaderMask);
-  int stages_per_tile = 0;
-  for (int i = 0; i < sg.n; ++i) stages_per_tile += (sg.L[i] + 63) >> 6;
-  const uint32_t bfull = smem_u32(&bars.yfull[0]);
-  for (int n = (t1 - t0) * stages_per_tile; n > 0; --n) {
-    mbar_wait(bfull + 8u * rg.s, rg.ph);
-    mbar_arrive_cluster((bfull + 8u * rg.s) & kLeaderMask);
+  mbar_wait(consts_u, (uint32_t)seg_i & 1u);
+  mbar_arrive_cluster(consts_u & kLeaderMask);
+  for (int n = n_stages; n > 0; --n) {
+    const uint32_t full = ya.full0 + 8u * rg.s;
+    mbar_wait(full, rg.ph);
+    mbar_arrive_cluster(full & kLeaderMask);
     rg.advance();
   }
   ++seg_i;
 }
 
+// IY role: the y MMAs of one tile into accumulator d_tmem (first MMA overwrites)
+__device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, const SegSrc& sg, uint32_t d_tmem, uint32_t a_base, uint32_t idesc,
+                                        bool trace, long long* tw)
+{
+  uint32_t acc = 0u, a_lo = a_base;
+  for (int i = 0; i < sg.n; ++i) {
+    const int nst = sg.nst[i], base = sg.mbase[i], ext = sg.ext[i];
+    for (int j = 0; j < nst; ++j) {
+      const int m = base + (j < ext ? 1 : 0);
+      TWAIT(2, ya.full0 + 8u * rg.s, rg.ph);
+      fence_after();
+      mma_y_stage(d_tmem, a_lo, ya.dst0 + rg.s * ya.step, idesc, m, acc);
+      commit2(ya.empty0 + 8u * rg.s, 3);
+      acc = 1u;
+      a_lo += (uint32_t)m * 256u;
+      rg.advance();
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 struct LowPArgs {
   const SliceParams* sp; const RateGroup* groups; const LowUnit* units;
-  int r_bytes, nsy;
+  int r_bytes, nsy, ystage, trace;
   SchedArgs sched;
 };
 
@@ -270,83 +361,83 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t rank = cluster_ctarank();
-  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, 0, 1, s_rng);
+  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, s_rng);
   __syncthreads();
   const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
   if (u_lo == u_hi && t_lo == t_hi) return;             // both CTAs of the cluster take the same decision
 
   const int nsy = a.nsy;
-  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid);
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 1u);
   const uint32_t tmem = tmem_slot;
   const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
   const uint32_t ring_u = sR_u + (uint32_t)a.r_bytes;
+  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done);
+  const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
 
   if (warp == 0) {
     if (elect_one()) {
-      PYState st{Ring{0, 0u, nsy}, 0};
+      YRing rg{0u, 0u, (uint32_t)nsy};
+      int seg_i = 0, nt = 0;
+      TRACE_BEGIN();
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
-        py_segment(st, seg[0], bars, sR_u, ring_u, rank, t0, t1, 0u, nullptr, 0u);
+        py_segment(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, 0u, nullptr, 0u, trace, tw);
+        nt += t1 - t0;
       }
+      if (rank == 0) TRACE_END(0, 0, nt);
     }
   } else if (warp == 4 && rank == 1) {
     if (elect_one()) {
-      Ring rg{0, 0u, nsy};
+      YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0;
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
-        relay_y_segment(rg, seg_i, seg[2], bars, t0, t1);
+        relay_y_segment(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
   } else if (warp == 1 && rank == 0) {
-    // ===== MMA issuer: one elected thread of the leader CTA =====
+    // ===== IY: the MMAs (one elected thread of the leader CTA).  A second issuing thread for the odd tiles was 10 % faster
+    // but faulted (cudaErrorLaunchFailure) once in a few hundred launches on the full config-2 bank; not understood. =====
     if (elect_one()) {
+      SegSrc& sg = seg[1];
       const uint32_t idesc = idesc_f16_pair(128);
-      const uint32_t a_base = desc_lo(sR_u, 2048u), b_base = desc_lo(ring_u, 1024u);
-      const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
-      Ring rg{0, 0u, nsy};
+      const uint32_t a_base = desc_lo(sR_u, 2048u);
+      const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]), acc_empty_u = smem_u32(&bars.acc_empty[0]);
+      const YAddr yd{ya.full0, ya.empty0, desc_lo(ring_u, 1024u), (uint32_t)a.ystage >> 4};   // dst = descriptor of the stage
+      YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0;
       uint32_t e = 0;
+      TRACE_BEGIN();
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
-        seg_fill(seg[1], a.sp, G->slice, G->n_slices, 2 * un.pb);
-        mbar_wait_cluster(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
+        seg_fill(sg, a.sp, G->slice, G->n_slices, 2 * un.pb);
+        TWAIT(0, consts_u, (uint32_t)seg_i & 1u);
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
           const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
-          mbar_wait_cluster(smem_u32(&bars.acc_empty[b]), ph ^ 1u);
+          TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          const uint32_t d_tmem = tmem + b * 128u;
-          uint32_t first = 1u, a_lo = a_base;
-          for (int i = 0; i < seg[1].n; ++i) {
-            const int L = seg[1].L[i];
-            for (int k0 = 0; k0 < L; k0 += 64) {
-              const int ks = min(64, L - k0);
-              mbar_wait_cluster(bfull + 8u * rg.s, rg.ph);
-              fence_after();
-              mma_y_stage(d_tmem, a_lo, b_base + (uint32_t)rg.s * (PK_YSTAGE / 16), idesc, ks, first);
-              commit2(bempty + 8u * rg.s, 3);
-              a_lo += (uint32_t)(ks >> 4) * 256u;
-              rg.advance();
-            }
-          }
-          commit2(smem_u32(&bars.acc_full[b]), 3);
+          iy_tile(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          commit2(acc_full_u + 8u * b, 3);
         }
-        commit2(smem_u32(&bars.unit_done), 3);
+        commit2(unit_done_u, 3);
         ++seg_i;
       }
+      TRACE_END(0, 1, (int)e);
     }
-  } else if (warp >= 8) {
+  } else if (warp >= 8 && warp < 16) {
     // ===== epilogue: thread = row; warps 8-11 columns [0, 64), warps 12-15 columns [64, 128); fp32 -> fp16 -> Q16 =====
     const int q = warp & 3, wg = (warp - 8) >> 2;
     const int row = q * 32 + lane;
     const uint32_t acc_empty_leader = smem_u32(&bars.acc_empty[0]) & kLeaderMask;
+    const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]);
     uint32_t e = 0;
+    TRACE_BEGIN();
     FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
       const LowUnit un = a.units[u];
       const RateGroup* Gp = a.groups + un.group;
@@ -354,7 +445,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       __half* __restrict__ Q = Gp->Q + ((size_t)(2 * un.pb + (int)rank) * q_cap * 128 + row) * 8;
       for (int t = t0; t < t1; ++t, ++e) {
         const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
-        mbar_wait(smem_u32(&bars.acc_full[b]), ph);
+        TWAIT(0, acc_full_u + 8u * b, ph);
         fence_after();
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
         uint32_t v0[32], v1[32];
@@ -378,23 +469,23 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
         }
       }
     }
+    if (rank == 0 && tid == 256) TRACE_END(0, 4, (int)e);
   }
   pair_teardown(tmem, warp);
 }
 
 // ------------------------------------------------------------------------------------------------
 struct F0PArgs {
-  const SliceParams* sp; const BdPlan* bd; const F0Combo* combos; const RateGroup* groups;
+  const SliceParams* sp; const BdPlan* bd; const RateGroup* groups;
   const uint8_t* P;                                     // [2][p_bytes]: band-matrix blob of rank 0, of rank 1
   Peak* partials; Capture cap; long long k_a;
-  int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, slots_cap, max_templates, gt;
-  SchedArgs sched;                                      // units = combos, one class
+  int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, ystage, slots_cap, max_templates, trace;
+  F0Sched sched;
   PairRate rate[kNLowRates];
+  PairMma tab[kPairTabMax];                             // interpolation MMAs, see PairMma
 };
 
-// chunks (16 low-rate rows) that must be resident before tile t's interpolation: ceil((adv t + adv + 16) / 16)
-__device__ __forceinline__ int q_chunks_upto(int adv, int t) { return (adv * t + adv + 16 + 15) >> 4; }
-
+template <bool CAPTURE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PK_THREADS, 1)
 f0_pair_kernel(const __grid_constant__ F0PArgs a)
 {
@@ -402,255 +493,351 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   __shared__ __align__(8) PairBars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ SegSrc seg[3];                             // [0] PY, [1] IY, [2] relay
-  __shared__ int s_rng[4];
+  __shared__ F0Pos s_pos[2];
   __shared__ __align__(16) Peak s_x[2][64];             // epilogue: second column half -> first, per flush parity
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t rank = cluster_ctarank();
-  const long long a0 = a.k_a / kTimeTile;               // absolute index of the chunk's tile 0
-  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, a0, a.gt, s_rng);
+  const F0Sched& S = a.sched;
+  const long long a0 = S.a0;
+  if (tid == 0) {
+    const long long T = S.total * S.n_tiles;
+    const int cid = blockIdx.x >> 1, ncl = gridDim.x >> 1;
+    s_pos[0] = f0_locate(S, T * (long long)cid / ncl);
+    s_pos[1] = f0_locate(S, T * (long long)(cid + 1) / ncl);
+  }
   __syncthreads();
-  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
-  if (u_lo == u_hi && t_lo == t_hi) return;
-  const int n_tiles = a.sched.n_tiles[0];
+  const F0Pos pA = s_pos[0], pB = s_pos[1];
+  { F0Iter it{pA, pB}; if (it.at_end()) return; }       // both CTAs of the cluster take the same decision
 
-  const int nsy = a.nsy, n_lr = a.n_lr;
-  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid);
-  const uint32_t tmem = tmem_slot;
+  const int nsy = a.nsy, n_lr = a.n_lr, gt = S.gt;
   const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
   const uint32_t sP_u = sR_u + (uint32_t)a.r_bytes;     // this rank's band-matrix blocks
   const uint32_t sQ_u = sP_u + (uint32_t)a.p_bytes;     // per-rate circular buffers of 16-row chunks (4 KB each)
   const uint32_t ring_u = sQ_u + (uint32_t)a.q_bytes;   // y ring
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 2u);
+  const uint32_t tmem = tmem_slot;
+  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done);
+  const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
+  const uint32_t qfull_u = smem_u32(&bars.qfull[0]), qempty_u = smem_u32(&bars.qempty[0]);
+  const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]), ybar_u = smem_u32(&bars.ybar[0]);
 
   if (warp == 0) {
     // ===== PY: y tiles of the d = 1 slices, R and P =====
     if (elect_one()) {
-      PYState st{Ring{0, 0u, nsy}, 0};
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        const F0Combo cb = a.combos[u];
-        const BdPlan* B = a.bd + cb.bd;
-        seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb + (int)rank);
-        py_segment(st, seg[0], bars, sR_u, ring_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes);
+      YRing rg{0u, 0u, (uint32_t)nsy};
+      int seg_i = 0, nt = 0;
+      TRACE_BEGIN();
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
+        const BdPlan* B = a.bd + bdi;
+        seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
+        py_segment(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes, trace, tw);
+        nt += t1 - t0;
       }
+      if (rank == 0) TRACE_END(1, 0, nt);
     }
   } else if (warp == 4 && rank == 1) {
     if (elect_one()) {
-      Ring rg{0, 0u, nsy};
+      YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0;
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        const F0Combo cb = a.combos[u];
-        const BdPlan* B = a.bd + cb.bd;
-        seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb + (int)rank);
-        relay_y_segment(rg, seg_i, seg[2], bars, t0, t1);
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
+        const BdPlan* B = a.bd + bdi;
+        seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
+        relay_y_segment(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
-  } else if (warp == 2) {
-    // ===== PQ: the rows of every rate's rho^(d) window that tile e needs and tile e - 1 did not have =====
+  } else if (warp == 2 || warp == 6) {
+    // ===== PQ0 / PQ1 (even / odd rates): the rows of a rate's rho^(d) window that tile e needs and tile e - 1 did not have =====
     if (elect_one()) {
+      const int rsel = warp == 2 ? 0 : 1;
       uint32_t e = 0;
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        const F0Combo cb = a.combos[u];
+      TRACE_BEGIN();
+      int adv[kNLowRates], cap[kNLowRates], cnext[kNLowRates], slot[kNLowRates];
+      uint32_t base[kNLowRates];
+#pragma unroll
+      for (int r = 0; r < kNLowRates; ++r) { adv[r] = a.rate[r].adv; cap[r] = a.rate[r].cap_chunks; base[r] = sQ_u + (uint32_t)a.rate[r].ring_off; cnext[r] = 0; slot[r] = 0; }
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd, rb = 2 * it.cur.pb + (int)rank;
         const uint8_t* qsrc[kNLowRates];
-        for (int r = 0; r < n_lr; ++r) {
-          const RateGroup* G = a.groups + cb.bd * n_lr + r;
-          qsrc[r] = (G->n_slices > 0) ? reinterpret_cast<const uint8_t*>(G->Q) + (size_t)(2 * cb.rb + (int)rank) * G->q_groups_cap * 2048 : nullptr;
+#pragma unroll
+        for (int r = 0; r < kNLowRates; ++r) {
+          qsrc[r] = nullptr;
+          if (r < n_lr && (r & 1) == rsel) {
+            const RateGroup* G = a.groups + bdi * n_lr + r;
+            if (G->n_slices > 0) qsrc[r] = reinterpret_cast<const uint8_t*>(G->Q) + (size_t)rb * G->q_groups_cap * 2048;
+            cnext[r] = (adv[r] * t0) >> 4;              // the unit's first tile fetches its whole window
+            slot[r] = cnext[r] % cap[r];
+          }
         }
         for (int t = t0; t < t1; ++t, ++e) {
-          // a unit's first tile fetches whole windows into slots other tiles may still be reading: drain first
-          if (t == t0) { if (e > 0) mbar_wait(smem_u32(&bars.qempty[(e - 1) & (PK_NQB - 1)]), ((e - 1) >> 2) & 1u); }
-          else if (e >= PK_QDIST) mbar_wait(smem_u32(&bars.qempty[(e - PK_QDIST) & (PK_NQB - 1)]), ((e - PK_QDIST) >> 2) & 1u);
-          const uint32_t fb = smem_u32(&bars.qfull[e & (PK_NQB - 1)]);
+          // a unit's first tile fetches whole windows into slots earlier tiles may still be reading: drain first.  (The
+          // even and the odd tiles finish on different threads: both of the last two must be complete.)
+          if (t == t0) {
+            if (e > 1) TWAIT(1, qempty_u + 8u * ((e - 2) & (PK_NQB - 1)), ((e - 2) >> 2) & 1u);
+            if (e > 0) TWAIT(1, qempty_u + 8u * ((e - 1) & (PK_NQB - 1)), ((e - 1) >> 2) & 1u);
+          } else if (e >= PK_QDIST) TWAIT(0, qempty_u + 8u * ((e - PK_QDIST) & (PK_NQB - 1)), ((e - PK_QDIST) >> 2) & 1u);
+          const uint32_t fb = qfull_u + 8u * (e & (PK_NQB - 1));
+          int nnew[kNLowRates];
           uint32_t total = 0;
-          for (int r = 0; r < n_lr; ++r) {
-            if (!qsrc[r]) continue;
-            const int adv = a.rate[r].adv;
-            const int c_lo = (t == t0) ? (adv * t) >> 4 : q_chunks_upto(adv, t - 1);
-            total += (uint32_t)(q_chunks_upto(adv, t) - c_lo) * 4096u;
+#pragma unroll
+          for (int r = 0; r < kNLowRates; ++r) {
+            nnew[r] = qsrc[r] ? ((adv[r] * (t + 1) + 31) >> 4) - cnext[r] : 0;
+            total += (uint32_t)nnew[r];
           }
-          mbar_expect_tx(fb, total);                    // total == 0: a plain arrival
-          for (int r = 0; r < n_lr; ++r) {
-            if (!qsrc[r]) continue;
-            const int adv = a.rate[r].adv, cap = a.rate[r].cap_chunks;
-            const int c_lo = (t == t0) ? (adv * t) >> 4 : q_chunks_upto(adv, t - 1);
-            const int c_hi = q_chunks_upto(adv, t);
-            if (c_hi <= c_lo) continue;
-            const uint32_t base = sQ_u + (uint32_t)a.rate[r].ring_off;
-            const int s0 = c_lo % cap;
-            const int n1 = min(c_hi - c_lo, cap - s0);
-            copy_pieces(base + (uint32_t)s0 * 4096u, qsrc[r] + (size_t)c_lo * 4096, (uint32_t)n1 * 4096u, fb);
-            if (c_hi - c_lo > n1) copy_pieces(base, qsrc[r] + (size_t)(c_lo + n1) * 4096, (uint32_t)(c_hi - c_lo - n1) * 4096u, fb);
+          if (((t - t0) & 3) == 0) {
+            // pull the rows tiles t + PK_QPF .. + 3 will ask for from HBM into L2 now: the shared-memory windows only
+            // hold PK_QDIST tiles of lookahead, far less than the DRAM latency under load
+#pragma unroll
+            for (int r = 0; r < kNLowRates; ++r) {
+              if (!qsrc[r]) continue;
+              const int tf = min(t + PK_QPF, t1), tg = min(t + PK_QPF + 4, t1);
+              const int c0 = (adv[r] * tf + 31) >> 4, c1 = (adv[r] * tg + 31) >> 4;             // chunks_upto(tf - 1), chunks_upto(tg - 1)
+              if (c1 > c0) bulk_prefetch_l2(qsrc[r] + (size_t)c0 * 4096, (uint32_t)(c1 - c0) * 4096u);
+            }
+          }
+          mbar_expect_tx(fb, total * 4096u);            // total == 0: a plain arrival
+#pragma unroll
+          for (int r = 0; r < kNLowRates; ++r) {
+            if (nnew[r] <= 0) continue;
+            const uint8_t* src = qsrc[r] + (size_t)cnext[r] * 4096;
+            const int n1 = min(nnew[r], cap[r] - slot[r]);
+            bulk_g2s(base[r] + (uint32_t)slot[r] * 4096u, src, (uint32_t)n1 * 4096u, fb);
+            if (nnew[r] > n1) bulk_g2s(base[r], src + (size_t)n1 * 4096, (uint32_t)(nnew[r] - n1) * 4096u, fb);
+            cnext[r] += nnew[r];
+            slot[r] += nnew[r]; if (slot[r] >= cap[r]) slot[r] -= cap[r];
           }
         }
       }
+      if (rank == 0 && rsel == 0) TRACE_END(1, 2, (int)e);
     }
   } else if (warp == 5 && rank == 1) {
     // ===== relay of the rho^(d) tile events =====
     if (elect_one()) {
       uint32_t e = 0;
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        for (int t = t0; t < t1; ++t, ++e) {
-          const uint32_t fb = smem_u32(&bars.qfull[e & (PK_NQB - 1)]);
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        for (int t = it.cur.t; t < it.seg_end(); ++t, ++e) {
+          const uint32_t fb = qfull_u + 8u * (e & (PK_NQB - 1));
           mbar_wait(fb, (e >> 2) & 1u);
           mbar_arrive_cluster(fb & kLeaderMask);
         }
       }
     }
   } else if (warp == 1 && rank == 0) {
-    // ===== IY: MMAs of the d = 1 slices =====
+    // ===== IY: MMAs of the d = 1 slices.  ONE thread here: this role spends most of its time blocked on the pipe (N = 128
+    // MMAs with both operands in shared memory take all of its 128 B/clk: 4 KB of A, 2 KB of B for this SM and 2 KB for
+    // the peer per 64 cycles), and with a second issuing thread for the odd tiles the f0 kernel faulted on the full
+    // config-2 bank (cudaErrorLaunchFailure, not understood; the low-rate kernel runs two) =====
     if (elect_one()) {
+      SegSrc& sg = seg[1];
       const uint32_t idesc = idesc_f16_pair(128);
-      const uint32_t a_base = desc_lo(sR_u, 2048u), b_base = desc_lo(ring_u, 1024u);
-      const uint32_t bfull = smem_u32(&bars.yfull[0]), bempty = smem_u32(&bars.yempty[0]);
-      Ring rg{0, 0u, nsy};
+      const uint32_t a_base = desc_lo(sR_u, 2048u);
+      const uint32_t acc_empty_u = smem_u32(&bars.acc_empty[0]);
+      const YAddr yd{ya.full0, ya.empty0, desc_lo(ring_u, 1024u), (uint32_t)a.ystage >> 4};
+      YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0;
       uint32_t e = 0;
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        const F0Combo cb = a.combos[u];
-        const BdPlan* B = a.bd + cb.bd;
-        seg_fill(seg[1], a.sp, B->f0_slice, B->n_f0, 2 * cb.rb);
-        mbar_wait_cluster(smem_u32(&bars.consts), (uint32_t)seg_i & 1u);
+      TRACE_BEGIN();
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
+        const BdPlan* B = a.bd + bdi;
+        seg_fill(sg, a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb);
+        TWAIT(0, consts_u, (uint32_t)seg_i & 1u);
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
           const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
-          mbar_wait_cluster(smem_u32(&bars.acc_empty[b]), ph ^ 1u);
+          TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          const uint32_t d_tmem = tmem + b * 128u;
-          uint32_t first = 1u, a_lo = a_base;
-          for (int i = 0; i < seg[1].n; ++i) {
-            const int L = seg[1].L[i];
-            for (int k0 = 0; k0 < L; k0 += 64) {
-              const int ks = min(64, L - k0);
-              mbar_wait_cluster(bfull + 8u * rg.s, rg.ph);
-              fence_after();
-              mma_y_stage(d_tmem, a_lo, b_base + (uint32_t)rg.s * (PK_YSTAGE / 16), idesc, ks, first);
-              commit2(bempty + 8u * rg.s, 3);
-              a_lo += (uint32_t)(ks >> 4) * 256u;
-              rg.advance();
-            }
-          }
-          commit2(smem_u32(&bars.ybar[b]), 1);
+          iy_tile(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          commit2(ybar_u + 8u * b, 1);
         }
         ++seg_i;
       }
+      TRACE_END(1, 1, (int)e);
     }
-  } else if (warp == 3 && rank == 0) {
-    // ===== IQ: interpolation MMAs (A4), after the tile's y part is complete =====
+  } else if ((warp == 3 || warp == 16) && rank == 0) {
+    // ===== IQ0 / IQ1: interpolation MMAs (A4) of the even / odd tiles, after the tile's y part is complete.  (Two threads
+    // accumulating into the SAME accumulator concurrently gave wrong sums: the pipe orders the MMAs of one thread only;
+    // tiles of different parity use different accumulators.) =====
     if (elect_one()) {
-      const uint32_t p_base = sP_u >> 4;
+      const uint32_t which = warp == 3 ? 0u : 1u;
       uint32_t e = 0;
-      FOR_SEGMENTS(u, t0, t1, n_tiles) {
-        const F0Combo cb = a.combos[u];
-        uint32_t present = 0;
-        for (int r = 0; r < n_lr; ++r) if (a.groups[cb.bd * n_lr + r].n_slices > 0) present |= 1u << r;
-        for (int t = t0; t < t1; ++t, ++e) {
-          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
-          mbar_wait(smem_u32(&bars.ybar[b]), ph);
-          mbar_wait_cluster(smem_u32(&bars.qfull[e & (PK_NQB - 1)]), ph);
-          fence_after();
-          const uint32_t d_tmem = tmem + b * 128u;
-          for (int r = 0; r < n_lr; ++r) {
-            if (!(present >> r & 1u)) continue;
-            const PairRate& R = a.rate[r];
-            const int v = (R.adv >= 16) ? 0 : ((R.adv * t) & 15) / R.adv;
-            const int s0 = ((R.adv * t) >> 4) % R.cap_chunks;
-            const uint32_t qa = desc_lo(sQ_u + (uint32_t)R.ring_off, 2048u);
-            const int n_it = R.n_items[v];
-            for (int k = 0; k < n_it; ++k) {
-              const PairItem it = R.item[v][k];
-              int s = s0 + (int)it.ch; if (s >= R.cap_chunks) s -= R.cap_chunks;
-              mma2_ss(d_tmem + it.d_col, desc64(qa + (uint32_t)s * 256u), desc64(p_base + it.p_lo), it.idesc, 1u);
-            }
-          }
-          commit2(smem_u32(&bars.qempty[e & (PK_NQB - 1)]), 3);
-          commit2(smem_u32(&bars.acc_full[b]), 3);
-        }
-        commit2(smem_u32(&bars.unit_done), 3);
+      int adv[kNLowRates], cap[kNLowRates], sb[kNLowRates], vmask[kNLowRates], mine_n = 0;
+      uint32_t qa[kNLowRates];
+#pragma unroll
+      for (int r = 0; r < kNLowRates; ++r) {
+        adv[r] = a.rate[r].adv; cap[r] = a.rate[r].cap_chunks; vmask[r] = a.rate[r].n_var - 1; sb[r] = 0;
+        qa[r] = desc_lo(sQ_u + (uint32_t)a.rate[r].ring_off, 2048u);
       }
+      const uint32_t p_base = sP_u >> 4;
+      TRACE_BEGIN();
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
+        uint32_t mine = 0;
+#pragma unroll
+        for (int r = 0; r < kNLowRates; ++r)
+          if (r < n_lr && a.groups[bdi * n_lr + r].n_slices > 0) { mine |= 1u << r; sb[r] = ((adv[r] * t0) >> 4) % cap[r]; }
+        for (int t = t0; t < t1; ++t, ++e) {
+          if ((e & 1u) == which) {
+            const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+            TWAIT(0, ybar_u + 8u * b, ph);
+            TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), ph);
+            fence_after();
+            const uint32_t d_tmem = tmem + b * 128u;
+#pragma unroll
+            for (int r = 0; r < kNLowRates; ++r) {
+              if (!(mine >> r & 1u)) continue;
+              const int v = t & vmask[r];
+              const int n_it = a.rate[r].n_items[v];
+              int idx = a.rate[r].tab_off[v] + sb[r] * n_it;               // [slot of the window's first chunk][item]
+              for (int k = 0; k < n_it; ++k, ++idx) {
+                const PairMma m = a.tab[idx];
+                mma2_ss(d_tmem + m.d_col, desc64(qa[r] + m.a_off), desc64(p_base + m.p_lo), m.idesc, 1u);
+              }
+            }
+            commit2(qempty_u + 8u * (e & (PK_NQB - 1)), 3);
+            commit2(acc_full_u + 8u * b, 3);
+            ++mine_n;
+          }
+          // window start of the next tile: floor(adv (t + 1) / 16) chunks
+#pragma unroll
+          for (int r = 0; r < kNLowRates; ++r) {
+            if (!(mine >> r & 1u)) continue;
+            const int dch = ((adv[r] * (t + 1)) >> 4) - ((adv[r] * t) >> 4);
+            sb[r] += dch; if (sb[r] >= cap[r]) sb[r] -= cap[r];
+          }
+        }
+        if (((e - 1u) & 1u) == which) {                 // the owner of the unit's last tile, once the other thread's last tile is done too
+          if (t1 - t0 >= 2) mbar_wait(acc_full_u + 8u * ((e - 2u) & (PK_NACC - 1)), ((e - 2u) >> 2) & 1u);
+          commit2(unit_done_u, 3);
+        }
+      }
+      TRACE_END(1, 3 + 3 * (int)which, mine_n);
     }
-  } else if (warp >= 8) {
-    // ===== epilogue: thread = row (lane); lanes 2i / 2i + 1 of a warp hold the cosine / sine row of one template =====
-    const int q = warp & 3, wg = (warp - 8) >> 2;
-    const int row = q * 32 + lane;
-    const int part = lane & 1;
+  } else if (warp >= 8 && warp < 16) {
+    // ===== epilogue.  16x256b TMEM loads: thread T of a warp holds, for lanes l = T / 4 (cosine row of a template) and
+    // l + 8 (its sine row, see r16_lane), the columns 8 i + 2 (T % 4) + {0, 1}: |rho|^2 without any cross-lane traffic.
+    // Warps 8-11 take columns [0, 64) of the tile, 12-15 columns [64, 128); a warp covers its lane quarter with two loads
+    // (h = 0, 1), so a thread works on two templates x 16 columns per tile.  The maximum of the 16 |rho|^2 is found with
+    // the column index packed into the 4 low mantissa bits (15 - j: the lowest column wins a tie; the truncation is
+    // 2^-19 relative), 15 integer maxima and a 4-level select tree instead of 16 compare / 4-select updates. =====
+    const int q = warp & 3, wg = (warp - 8) >> 2, tq = lane >> 2, tc = lane & 3;
     const uint32_t acc_empty_leader = smem_u32(&bars.acc_empty[0]) & kLeaderMask;
     uint32_t e = 0, flush_i = 0;
-    FOR_SEGMENTS(u, t0, t1, n_tiles) {
-      const F0Combo cb = a.combos[u];
-      const int n_templates = a.bd[cb.bd].n_templates;
-      const int grow = (2 * cb.rb + (int)rank) * 128 + row;             // reconstruction row i = 2 p + part
-      const int p = grow >> 1;
-      const bool capture = a.cap.snr != nullptr && a.cap.bd == cb.bd && grow < a.cap.rows;
-      // running first maximum of this thread's columns over the current granule
-      float bq = -1.f, bmine = 0.f, brecv = 0.f;
-      int bk = 0;
+    TRACE_BEGIN();
+    FOR_F0_SEGMENTS(it, S, pA, pB) {
+      const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
+      const int n_templates = a.bd[bdi].n_templates;
+      const int p0 = (2 * it.cur.pb + (int)rank) * 64 + 16 * q + tq;      // template of h = 0; h = 1: + 8
+      uint32_t bqt[2] = {0u, 0u};                                       // running maximum of the granule (truncated bits)
+      int bk[2] = {0, 0};
+      float bre[2] = {0.f, 0.f}, bim[2] = {0.f, 0.f};
       for (int t = t0; t < t1; ++t, ++e) {
         const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
-        mbar_wait(smem_u32(&bars.acc_full[b]), ph);
+        TWAIT(0, acc_full_u + 8u * b, ph);
+        __syncwarp();
         fence_after();
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
-        uint32_t lo[32], hi[32];                        // columns 64 wg + [0, 32) and + [32, 64) of this row
-        tmem_ld32(taddr, lo);
-        tmem_ld32(taddr + 32u, hi);
-        tmem_ld_wait();
-        fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);   // the tile is in registers: free the accumulator
         const int kap0 = t * 128;
         const int valid = min(128, a.c - kap0);
-        if (capture) {
+        const int cthr = 64 * wg + 2 * tc;                                // column of (i = 0, e = 0)
 #pragma unroll
-          for (int j = 0; j < 64; ++j) {
-            const int col = 64 * wg + j;
-            const long long k = a.k_a + kap0 + col;
-            if (col < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n)
-              a.cap.snr[(size_t)grow * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(j < 32 ? lo[j] : hi[j - 32]);
+        for (int h = 0; h < 2; ++h) {
+          uint32_t r[32];
+          __syncwarp();                                                   // tcgen05.ld is .aligned: the lanes may have diverged above
+          tmem_ld_16x256b_x8(taddr + ((uint32_t)(16 * h) << 16), r);
+          tmem_ld_wait();
+          if (h == 1) {                                                   // both halves are in registers: free the accumulator
+            fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);
+          }
+          if constexpr (CAPTURE) {
+            const int p = p0 + 8 * h;
+            if (a.cap.bd == bdi && 2 * p + 1 < a.cap.rows) {
+#pragma unroll
+              for (int j = 0; j < 16; ++j) {
+                const int col = cthr + 8 * (j >> 1) + (j & 1);
+                const long long k = a.k_a + kap0 + col;
+                if (col < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
+                  a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + (j & 1)]);
+                  a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + 2 + (j & 1)]);
+                }
+              }
+            }
+          }
+          uint32_t code[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const float re = __uint_as_float(r[4 * (j >> 1) + (j & 1)]), im = __uint_as_float(r[4 * (j >> 1) + 2 + (j & 1)]);
+            code[j] = (__float_as_uint(fmaf(re, re, im * im)) & ~15u) | (uint32_t)(15 - j);
+          }
+          if (valid < 128) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) if (cthr + 8 * (j >> 1) + (j & 1) >= valid) code[j] = 0u;
+          }
+#pragma unroll
+          for (int st = 8; st >= 1; st >>= 1)
+#pragma unroll
+            for (int j = 0; j < st; ++j) code[j] = max(code[j], code[j + st]);
+          const uint32_t m = code[0];
+          const int jw = 15 - (int)(m & 15u);
+          // select tree on the bits of jw: e = jw & 1, i = jw >> 1
+          uint32_t sr[8], si[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { sr[i] = (jw & 1) ? r[4 * i + 1] : r[4 * i]; si[i] = (jw & 1) ? r[4 * i + 3] : r[4 * i + 2]; }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { sr[i] = (jw & 2) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 2) ? si[2 * i + 1] : si[2 * i]; }
+#pragma unroll
+          for (int i = 0; i < 2; ++i) { sr[i] = (jw & 4) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 4) ? si[2 * i + 1] : si[2 * i]; }
+          const uint32_t wr = (jw & 8) ? sr[1] : sr[0], wi = (jw & 8) ? si[1] : si[0];
+          if ((m & ~15u) > bqt[h]) {                                      // later tiles never win ties
+            bqt[h] = m & ~15u; bk[h] = kap0 + cthr + 8 * (jw >> 1) + (jw & 1);
+            bre[h] = __uint_as_float(wr); bim[h] = __uint_as_float(wi);
           }
         }
-        // even lanes (cosine row) take columns [0, 32) of the 64, odd lanes (sine row) [32, 64): one shuffle per column
-        // brings the partner row's value of the SAME column
-        const int cbase = 64 * wg + 32 * part;
-        float q4[4] = {-1.f, -1.f, -1.f, -1.f}, m4[4] = {0.f, 0.f, 0.f, 0.f}, r4[4] = {0.f, 0.f, 0.f, 0.f};
-        int k4[4] = {0, 0, 0, 0};
-#pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          const float send = __uint_as_float(part ? lo[j] : hi[j]);
-          const float mine = __uint_as_float(part ? hi[j] : lo[j]);
-          const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
-          const float qq = fmaf(mine, mine, recv * recv);
-          if (cbase + j < valid && qq > q4[j & 3]) { q4[j & 3] = qq; k4[j & 3] = cbase + j; m4[j & 3] = mine; r4[j & 3] = recv; }
-        }
-        float tq = q4[0], tm = m4[0], tr = r4[0];
-        int tk = k4[0];
-#pragma unroll
-        for (int m = 1; m < 4; ++m)
-          if (q4[m] > tq || (q4[m] == tq && k4[m] < tk)) { tq = q4[m]; tk = k4[m]; tm = m4[m]; tr = r4[m]; }
-        if (tq > bq) { bq = tq; bk = kap0 + tk; bmine = tm; brecv = tr; }      // later tiles never win ties
-        // granule end: merge the four partial maxima of a template (two lanes x two column halves), write one record
+        // granule end: merge the partial maxima of a template (4 threads x 2 column halves), write one record
         const long long at = a0 + t;
-        if (t + 1 == t1 || (at + 1) % a.gt == 0) {
-          // partner lane: the odd lane's columns are later, so the even lane wins ties
-          const float oq = __shfl_xor_sync(0xffffffffu, bq, 1), om = __shfl_xor_sync(0xffffffffu, bmine, 1), orv = __shfl_xor_sync(0xffffffffu, brecv, 1);
-          const int ok = __shfl_xor_sync(0xffffffffu, bk, 1);
-          float re = part ? brecv : bmine, im = part ? bmine : brecv;          // this thread's best as (re, im)
-          const float ore = part ? om : orv, oim = part ? orv : om;            // partner's best (its part is the other one)
-          if (oq > bq || (oq == bq && ok < bk)) { bq = oq; bk = ok; re = ore; im = oim; }
+        if (t + 1 == t1 || (at + 1) % gt == 0) {
           const int fp = flush_i & 1;
-          if (wg == 1 && part == 0) { Peak pk; pk.q = bq; pk.kappa = bk; pk.re = re; pk.im = im; s_x[fp][row >> 1] = pk; }
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            float bq = fmaf(bre[h], bre[h], bim[h] * bim[h]);
+            int k = bk[h];
+            float re = bre[h], im = bim[h];
+#pragma unroll
+            for (int x = 1; x <= 2; x <<= 1) {
+              const float oq = __shfl_xor_sync(0xffffffffu, bq, x), ore = __shfl_xor_sync(0xffffffffu, re, x), oim = __shfl_xor_sync(0xffffffffu, im, x);
+              const int ok = __shfl_xor_sync(0xffffffffu, k, x);
+              if (oq > bq || (oq == bq && ok < k)) { bq = oq; k = ok; re = ore; im = oim; }
+            }
+            if (wg == 1 && tc == 0) { Peak pk; pk.q = bq; pk.kappa = k; pk.re = re; pk.im = im; s_x[fp][16 * q + 8 * h + tq] = pk; }
+            bre[h] = re; bim[h] = im; bk[h] = k; bqt[h] = __float_as_uint(bq);   // reused below by wg 0 (reset afterwards)
+          }
           asm volatile("bar.sync 2, 256;" ::: "memory");
-          if (wg == 0 && part == 0) {
-            const Peak o = s_x[fp][row >> 1];
-            if (o.q > bq) { bq = o.q; bk = o.kappa; re = o.re; im = o.im; }    // its columns are later: ties stay here
-            if (p < n_templates) {
-              const int gi = (int)(at / a.gt - a0 / a.gt);
-              Peak pk; pk.q = bq; pk.kappa = bk; pk.re = re; pk.im = im;
-              a.partials[((size_t)cb.bd * a.slots_cap + gi) * a.max_templates + p] = pk;
+          if (wg == 0 && tc == 0) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              float bq = __uint_as_float(bqt[h]), re = bre[h], im = bim[h];
+              int k = bk[h];
+              const Peak o = s_x[fp][16 * q + 8 * h + tq];
+              if (o.q > bq) { bq = o.q; k = o.kappa; re = o.re; im = o.im; }   // its columns are later: ties stay here
+              const int p = p0 + 8 * h;
+              if (p < n_templates) {
+                const int gi = (int)(at / gt - a0 / gt);
+                Peak pk; pk.q = bq; pk.kappa = k; pk.re = re; pk.im = im;
+                a.partials[((size_t)bdi * a.slots_cap + gi) * a.max_templates + p] = pk;
+              }
             }
           }
           ++flush_i;
-          bq = -1.f; bk = 0; bmine = 0.f; brecv = 0.f;
+#pragma unroll
+          for (int h = 0; h < 2; ++h) { bqt[h] = 0u; bk[h] = 0; bre[h] = 0.f; bim[h] = 0.f; }
         }
       }
     }
+    if (rank == 0 && tid == 256) TRACE_END(1, 4, (int)e);
   }
   pair_teardown(tmem, warp);
 }
@@ -736,6 +923,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   // rest (B operand of a cta_group::2 MMA), each as [2 row groups][nn / 2 columns][8 rows] fp16.
   std::vector<__half> pblob[2];
   int q_bytes = 0;
+  pl->n_tab = 0;
   for (int r = 0; r < pl->n_lr; ++r) {
     PairRate& U = pl->rate[r];
     const int l2 = U.log2d, d = 1 << l2;
@@ -750,11 +938,13 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     U.cap_chunks = cap;
     U.ring_off = q_bytes;
     q_bytes += cap * 4096;
-    for (int v = 0; v < 4; ++v) U.n_items[v] = 0;
+    for (int v = 0; v < 4; ++v) { U.n_items[v] = 0; U.tab_off[v] = 0; }
     for (int v = 0; v < U.n_var; ++v) {
       const int mis = v * U.adv;
       const int nch = (mis + U.adv + 2 * kKUp + 15) / 16;
-      if (nch > 5) return true;
+      if (nch > cap) return true;
+      struct Item { uint32_t idesc, p_lo, d_col; int ch; };
+      std::vector<Item> items;
       for (int ch = 0; ch < nch; ++ch) {
         int cmin = 1 << 30, cmax = -1;
         for (int rr = 0; rr < 16; ++rr)
@@ -777,12 +967,21 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
             if (i < -kKUp || i >= kKUp) continue;
             pblob[j / half][base + ((size_t)(rr >> 3) * half + (j % half)) * 8 + (rr & 7)] = __float2half_rn((float)w[(size_t)(i + kKUp) * d + kl % d]);
           }
-        PairItem& it = U.item[v][U.n_items[v]++];
+        Item it;
         it.idesc = (1u << 4) | ((uint32_t)(nn >> 3) << 17) | ((uint32_t)(256 >> 4) << 24);
         it.p_lo = (uint32_t)((base * sizeof(__half)) >> 4) | ((uint32_t)half << 16);     // LBO = half * 16 bytes
         it.d_col = (uint32_t)n0;
-        it.ch = (uint32_t)ch;
+        it.ch = ch;
+        items.push_back(it);
       }
+      U.n_items[v] = (int)items.size();
+      U.tab_off[v] = pl->n_tab;
+      if (pl->n_tab + cap * (int)items.size() > kPairTabMax) return true;
+      for (int s0 = 0; s0 < cap; ++s0)
+        for (const Item& it : items) {
+          PairMma& m = pl->tab[pl->n_tab++];
+          m.a_off = (uint32_t)((s0 + it.ch) % cap) * 256u; m.p_lo = it.p_lo; m.idesc = it.idesc; m.d_col = it.d_col;
+        }
     }
   }
   pl->p_bytes = (int)((pblob[0].size() * sizeof(__half) + 127) / 128 * 128);
@@ -790,8 +989,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 
   // per-(bin, detector) shared-memory limits: stationary R (this CTA's 128 rows) + P + windows + >= 3 y stages
   {
-    const int lim_f0 = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * PK_YSTAGE) / 256;
-    const int lim_low = (PK_SMEM_BUDGET - 3 * PK_YSTAGE) / 256;
+    const int lim_f0 = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / 256;
+    const int lim_low = (PK_SMEM_BUDGET - 3 * 16384) / 256;
     for (int b = 0; b < n_bd; ++b) {
       if (pl->bd_host[b].l_sum > lim_f0) pl->excluded[b] = 1;
       for (int r = 0; r < pl->n_lr; ++r)
@@ -805,11 +1004,22 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   }
   const int f0_fixed = pl->l_sum_f0_max * 256 + pl->p_bytes + pl->q_bytes;
   const int low_fixed = pl->l_sum_low_max * 256;
-  pl->f0_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - f0_fixed) / PK_YSTAGE);
-  pl->low_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - low_fixed) / PK_YSTAGE);
-  pl->f0_smem = f0_fixed + pl->f0_stages * PK_YSTAGE;
-  pl->low_smem = low_fixed + pl->low_stages * PK_YSTAGE;
-
+  // y stage slot: the largest stage of any slice the kernel streams (a slice with nm = L_pad / 16 MMAs per tile is cut
+  // into ceil(nm / 8) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
+  int ys_f0 = 2048, ys_low = 2048;
+  for (int b = 0; b < n_bd; ++b) {
+    if (pl->excluded[b]) continue;
+    for (int s = 0; s < bp_host[b].n_slices; ++s) {
+      const SliceParams& P = sp_host[bp_host[b].first_slice + s];
+      const int nm = P.L_pad / 16, nst = stage_count(nm), big = (nm + nst - 1) / nst * 2048;
+      if (P.d == 1) ys_f0 = std::max(ys_f0, big); else ys_low = std::max(ys_low, big);
+    }
+  }
+  pl->f0_ystage = ys_f0; pl->low_ystage = ys_low;
+  pl->f0_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - f0_fixed) / ys_f0);
+  pl->low_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - low_fixed) / ys_low);
+  pl->f0_smem = f0_fixed + pl->f0_stages * ys_f0;
+  pl->low_smem = low_fixed + pl->low_stages * ys_low;
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
   std::vector<SchedUnit> low_sched;
@@ -829,18 +1039,22 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
       pl->units_per_rate[r] += G.n_rb;
     }
   }
-  // f0 units = combos; cost per tile = MMAs: K / 16 of the d == 1 slices + interpolation chunks
-  std::vector<SchedUnit> f0_sched;
+  // f0 schedule entries: one per tensor-path (bin, detector); cost per tile and template block = MMAs: K / 16 of the
+  // d == 1 slices + interpolation chunks
+  std::vector<SchedBd> f0_sched;
   pl->f0_wsum = 0;
-  for (const F0Combo& cb : pl->combos_host) {
-    int w = pl->bd_host[cb.bd].l_sum / 16;
+  for (int b = 0; b < n_bd; ++b) {
+    if (pl->excluded[b]) continue;
+    int w = pl->bd_host[b].l_sum / 16;
     for (int r = 0; r < pl->n_lr; ++r) {
-      if (pl->groups_host[(size_t)cb.bd * pl->n_lr + r].n_slices == 0) continue;
+      if (pl->groups_host[(size_t)b * pl->n_lr + r].n_slices == 0) continue;
       w += pl->rate[r].n_items[0];
     }
-    f0_sched.push_back(SchedUnit{w, (int32_t)pl->f0_wsum});
-    pl->f0_wsum += w;
+    SchedBd e; e.bd = b; e.n_pb = pl->bd_host[b].n_rb; e.w = w; e.pad = 0; e.cum = pl->f0_wsum;
+    f0_sched.push_back(e);
+    pl->f0_wsum += (long long)e.n_pb * w;
   }
+  pl->f0_n_bds = (int)f0_sched.size();
   pl->low_units = (int)units.size();
   auto upload = [&](void** dst, const void* src, size_t n) -> bool {
     if (!plan_alloc(pl, dst, n, false, bytes, err, errlen)) return false;
@@ -857,11 +1071,12 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     if (!upload((void**)&pl->p_dev, both.data(), both.size())) return false;
   }
   if (!upload((void**)&pl->low_sched_dev, low_sched.data(), low_sched.size() * sizeof(SchedUnit))) return false;
-  if (!upload((void**)&pl->f0_sched_dev, f0_sched.data(), f0_sched.size() * sizeof(SchedUnit))) return false;
+  if (!upload((void**)&pl->f0_sched_dev, f0_sched.data(), f0_sched.size() * sizeof(SchedBd))) return false;
 
   // opt-in shared memory: the architecture maximum, for every kernel of this file, on this device (never lowered
   // by a later, smaller bank)
-  cudaError_t e = set_max_dyn_smem(f0_pair_kernel);
+  cudaError_t e = set_max_dyn_smem(f0_pair_kernel<false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(f0_pair_kernel<true>);
   if (e == cudaSuccess) e = set_max_dyn_smem(lowrate_pair_kernel);
   if (e != cudaSuccess) { snprintf(err, errlen, "fp16 plan: cudaFuncSetAttribute failed: %s", cudaGetErrorString(e)); return false; }
   pl->tensor_recon = true;
@@ -871,6 +1086,13 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
 void f16_plan_disable_tensor_recon(F16Plan* pl) { if (pl) pl->tensor_recon = false; }
 const uint8_t* f16_plan_excluded(const F16Plan* pl) { return (pl && pl->tensor_recon && pl->any_excluded) ? pl->excluded.data() : nullptr; }
+
+int f16_read_trace(long long* out, int reset)
+{
+  if (cudaMemcpyFromSymbol(out, g_trace, sizeof(long long) * 128) != cudaSuccess) return 1;
+  if (reset) { static long long z[128]; cudaMemcpyToSymbol(g_trace, z, sizeof z); }
+  return 0;
+}
 
 int f16_granule_tiles(int peak_window)
 {
@@ -887,7 +1109,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     LowPArgs la;
     memset(&la, 0, sizeof la);
     la.sp = sp_dev; la.groups = pl->groups_dev; la.units = (const LowUnit*)pl->units_dev;
-    la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages;
+    la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages; la.ystage = pl->low_ystage; la.trace = getenv("LLOID_TRACE") ? 1 : 0;
     SchedArgs& sc = la.sched;
     sc.units = pl->low_sched_dev; sc.n_cls = pl->n_lr;
     long long tiles_total = 0;
@@ -905,19 +1127,22 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   if (getenv("LLOID_DEBUG_SYNC") && cudaStreamSynchronize(st) != cudaSuccess) { fprintf(stderr, "lloid: lowrate_pair_kernel faulted\n"); return 1; }
   F0PArgs a;
   memset(&a, 0, sizeof a);
-  a.sp = sp_dev; a.bd = pl->bd_dev; a.combos = pl->combos_dev; a.groups = pl->groups_dev;
+  a.sp = sp_dev; a.bd = pl->bd_dev; a.groups = pl->groups_dev;
   a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
   a.partials = partials; a.cap = cap; a.k_a = k_a;
   a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
-  a.nsy = pl->f0_stages; a.slots_cap = slots_cap; a.max_templates = max_templates; a.gt = gt;
-  const int n_combos = (int)pl->combos_host.size();
+  a.nsy = pl->f0_stages; a.ystage = pl->f0_ystage; a.slots_cap = slots_cap; a.max_templates = max_templates;
+  a.trace = getenv("LLOID_TRACE") ? 1 : 0;
   const int n_tiles = (c + 127) / 128;
-  a.sched.units = pl->f0_sched_dev; a.sched.n_cls = 1;
-  a.sched.cls_begin[1] = n_combos; a.sched.n_tiles[0] = n_tiles;
-  a.sched.cls_base[1] = pl->f0_wsum * n_tiles;
+  a.sched.bds = pl->f0_sched_dev; a.sched.n_bds = pl->f0_n_bds; a.sched.n_tiles = n_tiles;
+  a.sched.gt = gt; a.sched.gb = (PK_BLOCK_TILES + gt - 1) / gt * gt;      // time blocks hold whole granules
+  a.sched.total = pl->f0_wsum; a.sched.a0 = k_a / kTimeTile;
   for (int r = 0; r < kNLowRates; ++r) a.rate[r] = pl->rate[r];
-  const int grid = 2 * (int)std::min<long long>(n_clusters, (long long)n_combos * n_tiles);
-  f0_pair_kernel<<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+  memcpy(a.tab, pl->tab, sizeof a.tab);
+  const long long pair_tiles = (long long)pl->combos_host.size() * n_tiles;
+  const int grid = 2 * (int)std::min<long long>(n_clusters, pair_tiles);
+  if (cap.snr) f0_pair_kernel<true><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+  else f0_pair_kernel<false><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
   ++*launches;
   const cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) fprintf(stderr, "lloid: f0_pair_kernel launch (grid %d, %d threads, %d B shared, %zu B params): %s\n", grid, PK_THREADS, pl->f0_smem, sizeof a, cudaGetErrorString(e));

@@ -19,7 +19,7 @@ __device__ __forceinline__ void ffma2(u64& c, u64 a, u64 b) { asm("fma.rn.f32x2 
 
 // Eight consecutive l of one reconstruction row i / one y row r, from the fp32 row-major arrays or (PK: the fp16
 // path's CUDA-core fallback for banks the tensor reconstruction cannot hold) from the packed fp16 operands, where the
-// same eight values are one 16-byte core-matrix row:  R16[i / 128][l / 8][i % 128][l % 8],
+// same eight values are one 16-byte core-matrix row:  R16[i / 128][l / 8][r16_lane(i % 128)][l % 8],
 // Y16[r / 64][l / 8][r % 64][l % 8].  l is a multiple of 8.
 __device__ __forceinline__ void h8_to_f(const uint4 v, float4& lo, float4& hi)
 {
@@ -33,7 +33,7 @@ __device__ __forceinline__ const char* base8_R(const SliceParams& P, int i, int 
 {
   if constexpr (PK) {
     step = 128 * 8 * 2;
-    return reinterpret_cast<const char*>(P.R16 + (((size_t)(i >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + (i & 127)) * 8);
+    return reinterpret_cast<const char*>(P.R16 + (((size_t)(i >> 7) * (P.L_pad >> 3) + (l >> 3)) * 128 + r16_lane(i & 127)) * 8);
   } else {
     step = 32;
     return reinterpret_cast<const char*>(P.R32 + (size_t)i * P.L_pad + l);
@@ -370,9 +370,9 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
       for (int i = 0; i < (RC_RT * RC_KC) / 256; ++i) {
         const int e = tid + 256 * i;
         const int ll = e % RC_KC, row = e / RC_KC;
-        if (Y16) {                                   // packed fp16: R16[i / 128][l / 8][i % 128][l % 8]
+        if (Y16) {                                   // packed fp16: R16[i / 128][l / 8][r16_lane(i % 128)][l % 8]
           const int i = row0 + row, l = l0 + ll;
-          Rs[ll * RC_RS + row] = __half2float(P.R16[(((size_t)(i >> 7) * (Lp >> 3) + (l >> 3)) * 128 + (i & 127)) * 8 + (l & 7)]);
+          Rs[ll * RC_RS + row] = __half2float(P.R16[(((size_t)(i >> 7) * (Lp >> 3) + (l >> 3)) * 128 + r16_lane(i & 127)) * 8 + (l & 7)]);
         } else {
           Rs[ll * RC_RS + row] = __ldg(R + (size_t)(row0 + row) * Lp + l0 + ll);
         }

@@ -52,7 +52,7 @@ std::vector<double> lowpass(int d, int K)
   return lp;
 }
 
-struct SliceHost { int rate, d, log2d, n_taps, L, L_pad; int64_t end_delay; };
+struct SliceHost { int rate, d, log2d, n_taps, L, L_pad; int64_t end_delay; bool fold; /* fp16: interpolation folded into the basis filters */ };
 struct BinHost { int N, S, rows_pad; int64_t M; std::vector<SliceHost> slices; };
 
 }  // namespace
@@ -63,7 +63,9 @@ struct lloid_bank {
   bool finalized = false;
   bool f16 = false;
   int n_bd = 0, max_templates = 0, max_rows_pad = 0, d_max = 1;
-  std::vector<SliceParams> sp_host;
+  std::vector<SliceParams> sp_host;      // reconstruction view: one per (bin, detector, slice); a folded slice has d = 1 here
+  std::vector<SliceParams> fir_host;     // fp16 path: basis-FIR problems (a folded slice contributes one per output phase)
+  SliceParams* fir_dev = nullptr;
   std::vector<BinParams> bp_host;
   std::vector<uint8_t> uploaded;
   std::vector<RateParams> rates_host;
@@ -109,12 +111,12 @@ int dev_alloc(lloid_bank* b, void** p, size_t n, bool zero)
 }
 
 int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const double* recon,
-                  const float** U32, const float** R32, const __half** U16, const __half** R16)
+                  const float** U32, const float** R32, const __half** U16, const __half** U16b, const __half** R16)
 {
   const BinHost& B = b->bins[bin];
   const SliceHost& S = B.slices[slice];
   const size_t nu = (size_t)S.L_pad * S.n_taps, nr = (size_t)B.rows_pad * S.L_pad;
-  *U32 = nullptr; *R32 = nullptr; *U16 = nullptr; *R16 = nullptr;
+  *U32 = nullptr; *R32 = nullptr; *U16 = nullptr; *U16b = nullptr; *R16 = nullptr;
   if (!b->f16) {
     std::vector<float> u(nu, 0.f), r(nr, 0.f);
     for (int l = 0; l < S.L; ++l)
@@ -129,20 +131,42 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     *U32 = (const float*)du; *R32 = (const float*)dr;
   } else {
     // fp16 path: U packed for the tcgen05 FIR kernel as [tap block of 64][tap group of 8][l < L_pad][8 taps]
-    // (taps zero-padded to a multiple of 64); R packed as R16[i / 128][l / 8][i % 128][l % 8], rows in their natural
-    // order (lloid_internal.h): a reconstruction CTA bulk-copies its 128-row block straight into MMA layout.
-    const int n_kb = (S.n_taps + 63) / 64;
+    // (taps zero-padded to a multiple of 64); R packed as R16[i / 128][l / 8][r16_lane(i % 128)][l % 8]
+    // (lloid_internal.h): a reconstruction CTA bulk-copies its 128-row block straight into MMA layout.
+    // A folded slice (lloid_internal.h, kFoldMaxD) stores, per output phase phi, Uhat_phi[l, u] = sum_i w_phi[i] U[l, u - K_up + i]
+    // with n_s + 2 K_up taps (w_phi[i] = d lp_{d,K_up}[d i + phi], i = -K_up .. K_up - 1), computed in double precision.
+    const int Ku = b->cfg.k_up;
+    const int n_eff = S.fold ? S.n_taps + 2 * Ku : S.n_taps;
+    const int n_kb = (n_eff + 63) / 64;
     const size_t nup = (size_t)n_kb * 64 * S.L_pad;
-    std::vector<__half> u(nup, __float2half(0.f));
-    for (int l = 0; l < S.L; ++l)
-      for (int t = 0; t < S.n_taps; ++t)
-        u[(((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.L_pad + l) * 8 + (t & 7)] =
-            __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+    std::vector<__half> u(nup, __float2half(0.f)), ub;
+    if (!S.fold) {
+      for (int l = 0; l < S.L; ++l)
+        for (int t = 0; t < S.n_taps; ++t)
+          u[(((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.L_pad + l) * 8 + (t & 7)] =
+              __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+    } else {
+      ub.assign(nup, __float2half(0.f));
+      const std::vector<double> lp = lowpass(S.d, Ku);
+      for (int phi = 0; phi < 2; ++phi) {
+        std::vector<__half>& dst = phi ? ub : u;
+        for (int l = 0; l < S.L; ++l)
+          for (int uu = 0; uu < n_eff; ++uu) {
+            double acc = 0.0;
+            for (int i = -Ku; i < Ku; ++i) {
+              const int t = uu - Ku + i;
+              if (t < 0 || t >= S.n_taps) continue;
+              acc += (double)S.d * lp[S.d * i + phi + Ku * S.d] * basis[(size_t)l * S.n_taps + t];
+            }
+            dst[(((size_t)(uu >> 6) * 8 + ((uu >> 3) & 7)) * S.L_pad + l) * 8 + (uu & 7)] = __float2half_rn((float)acc);
+          }
+      }
+    }
     std::vector<__half> r(nr, __float2half(0.f));
     const size_t lgs = (size_t)(S.L_pad >> 3);
     for (int i = 0; i < 2 * B.N; ++i)
       for (int l = 0; l < S.L; ++l)
-        r[(((size_t)(i >> 7) * lgs + (l >> 3)) * 128 + (i & 127)) * 8 + (l & 7)] =
+        r[(((size_t)(i >> 7) * lgs + (l >> 3)) * 128 + r16_lane(i & 127)) * 8 + (l & 7)] =
             __float2half_rn((float)recon[(size_t)i * S.L + l]);
     void *du, *dr;
     int rc = dev_alloc(b, &du, nup * 2, false); if (rc) return rc;
@@ -150,6 +174,12 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     CU(cudaMemcpy(du, u.data(), nup * 2, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(dr, r.data(), nr * 2, cudaMemcpyHostToDevice));
     *U16 = (const __half*)du; *R16 = (const __half*)dr;
+    if (S.fold) {
+      void* dub;
+      rc = dev_alloc(b, &dub, nup * 2, false); if (rc) return rc;
+      CU(cudaMemcpy(dub, ub.data(), nup * 2, cudaMemcpyHostToDevice));
+      *U16b = (const __half*)dub;
+    }
   }
   return LLOID_OK;
 }
@@ -225,7 +255,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
                        b->partials, b->slots_cap, b->max_templates, c, k_a, b->cap, false, st, &b->last_launches);
     }
   } else {
-    if (launch_fir_f16(b->plan16, b->sp_dev, b->sp_host.data(), n_prob, b->rates_dev, o, c, st, &b->last_launches))
+    if (launch_fir_f16(b->plan16, b->fir_dev, b->fir_host.data(), (int)b->fir_host.size(), b->rates_dev, o, c, st, &b->last_launches))
       return fail(LLOID_ECUDA, "fp16 FIR launch failed: %s", cudaGetErrorString(cudaGetLastError()));
     mark(b, st, kTagFir);
     if (int rc = debug_sync("fir_f16_kernel", k_a, st)) return rc;
@@ -330,6 +360,7 @@ int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const 
       if (sd.end_delay != expect_delay) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: slices must tile the template back to front (end_delay %lld, expected %lld)", bi, s, (long long)sd.end_delay, (long long)expect_delay); }
       if (S.d > 1 && sd.end_delay < (int64_t)(cfg->k_down + cfg->k_up) * S.d) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: causality needs end_delay >= (k_down + k_up) * d", bi, s); }
       S.n_taps = sd.n_taps; S.L = sd.n_basis; S.L_pad = (int)round_up(S.L, kLPad); S.end_delay = sd.end_delay;
+      S.fold = b->f16 && S.d > 1 && S.d <= kFoldMaxD && !getenv("LLOID_NO_FOLD");
       expect_delay += (int64_t)S.d * S.n_taps;
       B.slices.push_back(S);
       b->d_max = std::max(b->d_max, S.d);
@@ -343,7 +374,7 @@ int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const 
       for (int s = 0; s < B.S; ++s) {
         SliceParams P; memset(&P, 0, sizeof P);
         const SliceHost& S = B.slices[s];
-        P.d = S.d; P.log2d = S.log2d; P.n_taps = S.n_taps; P.L = S.L; P.L_pad = S.L_pad;
+        P.d = S.fold ? 1 : S.d; P.log2d = S.fold ? 0 : S.log2d; P.n_taps = S.n_taps; P.L = S.L; P.L_pad = S.L_pad;   // reconstruction view
         P.rows = 2 * B.N; P.rows_pad = B.rows_pad; P.bin = bi; P.det = det; P.slice = s;
         b->sp_host.push_back(P);
       }
@@ -364,7 +395,7 @@ int lloid_bank_upload_slice(lloid_bank_t* b, int32_t bin, int32_t det, int32_t s
   if (b->finalized) return fail(LLOID_ESTATE, "upload after finalize");
   CU(cudaSetDevice(b->cfg.device));
   SliceParams& P = b->sp_host[b->slice_index(bin, det, slice)];
-  rc = upload_arrays(b, bin, slice, basis, recon, &P.U32, &P.R32, &P.U16, &P.R16); if (rc) return rc;
+  rc = upload_arrays(b, bin, slice, basis, recon, &P.U32, &P.R32, &P.U16, &P.U16b, &P.R16); if (rc) return rc;
   b->uploaded[b->slice_index(bin, det, slice)] = 1;
   return LLOID_OK;
 }
@@ -377,10 +408,10 @@ int lloid_bank_upload_slice_shared(lloid_bank_t* b, int32_t bin, int32_t slice, 
   if (b->finalized) return fail(LLOID_ESTATE, "upload after finalize");
   CU(cudaSetDevice(b->cfg.device));
   SliceParams& P0 = b->sp_host[b->slice_index(bin, 0, slice)];
-  rc = upload_arrays(b, bin, slice, basis, recon, &P0.U32, &P0.R32, &P0.U16, &P0.R16); if (rc) return rc;
+  rc = upload_arrays(b, bin, slice, basis, recon, &P0.U32, &P0.R32, &P0.U16, &P0.U16b, &P0.R16); if (rc) return rc;
   for (int det = 0; det < b->cfg.n_detectors; ++det) {
     SliceParams& P = b->sp_host[b->slice_index(bin, det, slice)];
-    P.U32 = P0.U32; P.R32 = P0.R32; P.U16 = P0.U16; P.R16 = P0.R16;
+    P.U32 = P0.U32; P.R32 = P0.R32; P.U16 = P0.U16; P.U16b = P0.U16b; P.R16 = P0.R16;
     b->uploaded[b->slice_index(bin, det, slice)] = 1;
   }
   return LLOID_OK;
@@ -401,7 +432,7 @@ int lloid_bank_alias_bin(lloid_bank_t* b, int32_t dst, int32_t src)
       const int is = b->slice_index(src, det, s), id = b->slice_index(dst, det, s);
       if (!b->uploaded[is]) return fail(LLOID_ESTATE, "alias_bin: source bin %d not uploaded", src);
       SliceParams& P = b->sp_host[id]; const SliceParams& Q = b->sp_host[is];
-      P.U32 = Q.U32; P.R32 = Q.R32; P.U16 = Q.U16; P.R16 = Q.R16;
+      P.U32 = Q.U32; P.R32 = Q.R32; P.U16 = Q.U16; P.U16b = Q.U16b; P.R16 = Q.R16;
       b->uploaded[id] = 1;
     }
   }
@@ -426,8 +457,8 @@ int lloid_bank_finalize(lloid_bank_t* b)
     for (const SliceHost& S : B.slices) {
       const int64_t need = (S.d == 1) ? S.end_delay + S.n_taps : S.end_delay + (int64_t)S.d * (S.n_taps + Ku + Kd);
       H = std::max(H, need);
-      ybytes_per_sample += (double)D * S.L_pad * esize / S.d;
-      if (S.d > 1) ybytes_per_sample += (double)D * B.rows_pad * esize / S.d;         // rho^(d) staging (upper bound)
+      ybytes_per_sample += (double)D * S.L_pad * esize / (S.fold ? 1 : S.d);
+      if (S.d > 1 && !S.fold) ybytes_per_sample += (double)D * B.rows_pad * esize / S.d;   // rho^(d) staging (upper bound)
     }
   H = round_up(H, 256);
   if (H > (1ll << 28)) return fail(LLOID_EINVAL, "history too long");
@@ -451,14 +482,14 @@ int lloid_bank_finalize(lloid_bank_t* b)
     double need = 0.0;
     for (const BinHost& B : b->bins)
       for (const SliceHost& S : B.slices) {
-        const double rows = (S.d == 1) ? (double)C : (double)C / S.d + 2 * Ku;
+        const double rows = (S.d == 1 || S.fold) ? (double)C : (double)C / S.d + 2 * Ku;
         need += (double)D * (std::ceil(rows / 128.0) * 128.0) * S.L_pad * esize;
       }
     if (b->f16)
       for (const BinHost& B : b->bins) {
         bool seen[kMaxRates] = {false, false, false, false, false, false};
         for (const SliceHost& S : B.slices) {
-          if (S.d == 1 || seen[S.log2d]) continue;
+          if (S.d == 1 || S.fold || seen[S.log2d]) continue;
           seen[S.log2d] = true;
           need += (double)D * ((std::ceil(((double)C / S.d + 2 * Ku) / 128.0) * 16 + 16) * 8) * B.rows_pad * 2.0;
         }
@@ -509,10 +540,12 @@ int lloid_bank_finalize(lloid_bank_t* b)
   size_t ybytes = 0;
   for (SliceParams& P : b->sp_host) {
     const SliceHost& S = b->bins[P.bin].slices[P.slice];
-    P.rate_idx = (int)(std::find(ds.begin(), ds.end(), S.d) - ds.begin());
-    const int64_t rows = (S.d == 1) ? C : C / S.d + 2 * Ku;
+    P.rate_idx = (int)(std::find(ds.begin(), ds.end(), S.d) - ds.begin());      // the stream the FIR reads
+    const int64_t rows = (S.d == 1 || S.fold) ? C : C / S.d + 2 * Ku;
     P.y_rows_cap = (int)round_up(rows, 128);
+    // FIR window origin of Y row 0 (of FIR row 0 for a folded slice), in samples of the slice's rate stream
     P.jjY0 = (S.d == 1) ? (int)(H - S.end_delay) : (int)((H - S.end_delay) / S.d - Ku);
+    P.fir_halo = (S.d == 1 || S.fold) ? 0 : 2 * Ku; P.out_mul = 1; P.out_add = 0;
     RateParams& R = b->rates_host[P.rate_idx];
     R.jj_lo_fixed = std::min(R.jj_lo_fixed, P.jjY0 - S.n_taps);
     R.jj_hi_off = std::max(R.jj_hi_off, (S.d == 1) ? P.jjY0 : P.jjY0 + 2 * Ku - 1);
@@ -526,6 +559,22 @@ int lloid_bank_finalize(lloid_bank_t* b)
   }
   for (const RateParams& R : b->rates_host)
     if (R.jj_lo_fixed < (R.d == 1 ? 0 : Kd)) return fail(LLOID_EINVAL, "internal: history too short for rate d=%d", R.d);
+  if (b->f16) {
+    // FIR problem table.  A folded slice (lloid_internal.h) contributes one problem per output phase: n_s + 2 K_up taps of
+    // the composite filters, c / d rows, FIR row m -> Y row d m + phi; its window origin moves by the 2 K_up extra taps.
+    for (const SliceParams& P : b->sp_host) {
+      const SliceHost& S = b->bins[P.bin].slices[P.slice];
+      if (!S.fold) { b->fir_host.push_back(P); continue; }
+      for (int phi = 0; phi < S.d; ++phi) {
+        SliceParams F = P;
+        F.d = S.d; F.log2d = S.log2d; F.n_taps = S.n_taps + 2 * Ku; F.jjY0 = P.jjY0 + 2 * Ku;
+        F.U16 = phi ? P.U16b : P.U16; F.fir_halo = 0; F.out_mul = S.d; F.out_add = phi;
+        b->fir_host.push_back(F);
+      }
+    }
+    rc = dev_alloc(b, (void**)&b->fir_dev, b->fir_host.size() * sizeof(SliceParams), false); if (rc) return rc;
+    CU(cudaMemcpy(b->fir_dev, b->fir_host.data(), b->fir_host.size() * sizeof(SliceParams), cudaMemcpyHostToDevice));
+  }
 
   // interpolation weights  w[(i + K_up) * d + phi] = d * lp_{d,K_up}[d i + phi],  i = -K_up .. K_up - 1
   std::vector<const float*> upw(kMaxRates, nullptr);
@@ -566,8 +615,8 @@ int lloid_bank_finalize(lloid_bank_t* b)
     char err[256] = {0};
     const double* up_w[kMaxRates];
     for (int l2 = 0; l2 < kMaxRates; ++l2) up_w[l2] = upw64[l2].empty() ? nullptr : upw64[l2].data();
-    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->bp_host.data(), b->n_bd, D, b->C, up_w,
-                                &b->bytes, err, sizeof err);
+    b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->fir_host.data(), (int)b->fir_host.size(),
+                                b->bp_host.data(), b->n_bd, D, b->C, up_w, &b->bytes, err, sizeof err);
     if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
   }
   const uint8_t* excl = b->f16 ? f16_plan_excluded(b->plan16) : nullptr;   // mixed bank: only these bins use the FFMA kernels
@@ -738,6 +787,8 @@ int lloid_last_stage_ms(lloid_bank_t* b, float* out)
   out[2] += out[5];                               // [5] (low-rate reconstruction kernel) is a part of [2]
   return LLOID_OK;
 }
+
+int lloid_debug_trace(long long* out, int reset) { return f16_read_trace(out, reset) ? LLOID_ECUDA : LLOID_OK; }
 
 void lloid_destroy(lloid_bank_t* b)
 {

@@ -31,6 +31,7 @@ struct SliceParams {               // one per (bin, detector, slice); lives in a
   const float*  U32;               // [L_pad][n_taps]            fp32 path
   const float*  R32;               // [rows_pad][L_pad]          fp32 path
   const __half* U16;               // fp16 path: packed [tap block 64][tap group 8][l L_pad][8 taps] (bulk-copy source)
+  const __half* U16b;              // folded slice: the odd phase's filters (U16 = even phase)
   const __half* R16;               // fp16 path: packed R16 layout (below)
   void*    Y;                      // chunk-local y^s: fp32 row-major [y_rows_cap][L_pad], or fp16 packed Y16 (below)
   int32_t  d, log2d, rate_idx;
@@ -38,8 +39,19 @@ struct SliceParams {               // one per (bin, detector, slice); lives in a
   int32_t  rows, rows_pad;         // 2N and its padding
   int32_t  jjY0;                   // xs index of Y row 0 at o = 0: (H-Delta)/d - K_up (d>1) or H-Delta (d==1)
   int32_t  y_rows_cap;             // allocated Y rows
-  int32_t  bin, det, slice, pad_;
+  int32_t  bin, det, slice;
+  int32_t  fir_halo;               // FIR view: rows computed per chunk = (c >> log2d) + fir_halo   (2 K_up for d > 1, else 0)
+  int32_t  out_mul, out_add;       // FIR view: FIR row m is written to Y row out_mul m + out_add   (1, 0 except below)
+  int32_t  pad_[2];
 };
+// fp16 path, "interpolation folded into the basis filters": a slice at f0 / 2 is NOT reconstructed at
+// its own rate and interpolated afterwards (A3 then A4); since both steps are linear,
+//   c^s_i[k] = sum_l R^s[i, l] yhat_l[k],   yhat_l[2 m + phi] = sum_u Uhat_phi[l, u] x^s[j0 + m + u],
+//   Uhat_phi[l, u] = sum_i w_phi[i] U^s[l, u - K_up + i]      (n_s + 2 K_up taps, phi = 0, 1),
+// i.e. TWO basis-FIR problems at the low rate write the even / odd rows of a full-rate y, and the f0 kernel reconstructs
+// the slice like a d = 1 slice.  The reconstruction tables then hold the slice with d = 1; the FIR problem table
+// (fir_sp) holds the two phase problems.  This halves the rho^(d) bytes that cross HBM between the two kernels.
+constexpr int kFoldMaxD = 2;
 
 struct RateParams {                // one per distinct decimation factor
   const float* taps;               // [2 K_dn d + 1], taps[u] = sqrt(d) lp[K_dn d - u]   (d == 1: unused)
@@ -126,10 +138,14 @@ void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
 // 8 fp16 = 128 contiguous bytes, so every operand tile is fetched with plain 1-D bulk copies):
 //   Y16  [time tile of 64 rows][l / 8][row % 64][l % 8]             y^s, written by the FIR kernel; a CTA of a pair
 //                                                                   supplies one 64-row tile of a 128-sample MMA tile
-//   R16  [rb = i / 128][l / 8][i % 128][l % 8]                      R^s, rows i = 2p (cos), 2p + 1 (sin) in natural order
-//   Q16  [rb][j / 8][i % 128][j % 8]                                rho^(d) = sum over the slices at rate d of R^s y^s
+//   R16  [rb = i / 128][l / 8][lane(i % 128)][l % 8]                R^s; inside a 128-row block (64 templates) row
+//        i = 2 p + part sits in lane 16 (p / 8) + 8 part + p % 8 (r16_lane): cosine and sine row of a template are 8
+//        lanes apart, which is what one thread of a 16x256b TMEM load holds (f0 epilogue, no shuffles)
+//   Q16  [rb][j / 8][lane][j % 8]                                   rho^(d) = sum over the slices at rate d of R^s y^s
+//        (rows in the SAME lane order: the low-rate kernel's accumulator lanes are the f0 kernel's A-operand rows)
 constexpr int kTplBlock = 128;     // complex templates per CTA PAIR (M = 256 rows: 128 per CTA)
 constexpr int kNLowRates = kMaxRates - 1;
+__host__ __device__ inline int r16_lane(int i_in_block) { const int p = i_in_block >> 1; return 16 * (p >> 3) + 8 * (i_in_block & 1) + (p & 7); }
 
 struct RateGroup {                 // one per (bin, detector, distinct rate with d > 1)
   int32_t  n_slices;               // 0: this (bin, detector) has no slice at this rate
@@ -149,21 +165,24 @@ struct BdPlan {                    // one per (bin, detector): what the f0-rate 
 struct F0Combo { int32_t bd, rb; };   // (bin*detector, template block) handled back to back along time
 
 // A4 on the tensor cores (f0_pair_kernel): one interpolation MMA = one 16-row chunk of a rate's rho^(d) window times the
-// block of the band matrix P_d its rows touch
-struct PairItem {
+// block of the band matrix P_d its rows touch.  The issuing thread reads everything an MMA needs from ONE table entry in
+// the kernel parameters (uniform loads straight into uniform registers): the table is indexed by the rate, the
+// alignment variant of the window and the ring slot of the window's first chunk, so the ring wrap is folded in.
+struct PairMma {
+  uint32_t a_off;                  // A descriptor offset (16-byte units) of the chunk's ring slot, relative to the rate's buffer
+  uint32_t p_lo;                   // B descriptor low word of the block relative to the P blob: offset >> 4 | (N / 2) << 16
   uint32_t idesc;                  // cta_group::2 instruction descriptor, M = 256, N = columns of the block
-  uint32_t p_lo;                   // descriptor low word of the block relative to the P blob: offset >> 4 | (N / 2) << 16
   uint32_t d_col;                  // first accumulator column
-  uint32_t ch;                     // chunk index inside the 16-row-aligned window
 };
+constexpr int kPairTabMax = 224;   // table entries in the kernel parameters (3.5 KB)
 struct PairRate {                  // one per distinct rate with d > 1 (bank-wide)
   int32_t  log2d;
   int32_t  adv;                    // low-rate rows per 128-sample tile: 128 / d
   int32_t  cap_chunks;             // capacity of the rate's circular buffer, in chunks of 16 rows (4 KB per CTA)
   int32_t  n_var;                  // window start is adv t: 16 / adv alignments of it inside a chunk (1 when adv >= 16)
   int32_t  ring_off;               // byte offset of the circular buffer in the window area
-  int32_t  n_items[4];
-  PairItem item[4][5];             // per variant: the window's chunks, in order
+  int32_t  n_items[4];             // MMAs per tile, per variant
+  int32_t  tab_off[4];             // per variant: table entries [slot of the first chunk][item]
 };
 
 // Static schedule of a persistent tensor kernel (A7).  Work = units x time tiles; a unit is one stationary
@@ -180,8 +199,14 @@ struct SchedArgs {
   long long cls_base[kNLowRates + 1];       // cost before class c; cls_base[n_cls] = total
 };   // one 16-row chunk of an interpolation: MMA N, P offset, D column
 
+struct SchedBd {                   // f0 kernel schedule: one tensor-path (bin, detector)
+  int32_t bd, n_pb, w, pad;        // index, template blocks of 128, cost per tile (MMAs)
+  long long cum;                   // sum of n_pb * w over the earlier entries
+};
+
 struct F16Plan;                    // opaque host-side plan: work lists, band matrices, Q buffers
-F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const BinParams* bp_host, int n_bd,
+F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems /* reconstruction view */,
+                         const SliceParams* fir_host, int n_fir /* FIR problems */, const BinParams* bp_host, int n_bd,
                          int n_det, int chunk_cap, const double* const* up_w /* [kMaxRates]: w[(i+K_up) d + phi] or null */,
                          int64_t* bytes, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
@@ -193,6 +218,7 @@ int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_h
 // partials of the tensor path: ONE record per (bin, detector, template, granule); a granule is a run of gt tiles
 // aligned to absolute multiples of gt tiles, gt = f16_granule_tiles(W) dividing the peak window
 int  f16_granule_tiles(int peak_window);
+int  f16_read_trace(long long* out /* [2][8][8] */, int reset);
 int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int slots_cap, int max_templates,
                       int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches,
                       cudaEvent_t after_lowrate /* recorded between the two kernels when non-null */);

@@ -102,6 +102,22 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
                  "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
                : "r"(taddr) : "memory");
 }
+// TMEM -> registers, shape 16x256b (the m16n8 accumulator fragment; verified on B200): 16 lanes starting at the address's
+// lane (a multiple of 16 inside this warp's quarter), 8 blocks of 8 columns.  Thread T gets, for block i:
+//   r[4 i + 0], r[4 i + 1] = lane T / 4,      columns 8 i + 2 (T % 4), + 1
+//   r[4 i + 2], r[4 i + 3] = lane T / 4 + 8,  the same columns
+// so a thread holds the SAME columns of two lanes that are 8 apart: with the cosine row of a template in lane l and its sine
+// row in lane l + 8, |rho|^2 needs no cross-lane traffic.
+__device__ __forceinline__ void tmem_ld_16x256b_x8(uint32_t taddr, uint32_t (&r)[32])
+{
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+               "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+                 "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+                 "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+                 "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+               : "r"(taddr) : "memory");
+}
 // one 32-bit column of this warp's 32 lanes
 __device__ __forceinline__ uint32_t tmem_ld1(uint32_t taddr)
 {
@@ -228,17 +244,14 @@ __device__ __forceinline__ void tmem_dealloc2(uint32_t taddr, uint32_t cols)
 {
   asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" :: "r"(taddr), "r"(cols) : "memory");
 }
-// arrive on a barrier given by its shared::cluster address (own or peer CTA), release at cluster scope
+// Arrive on a barrier given by its shared::cluster address (own or peer CTA).  Default semantics (as CUTLASS's
+// ClusterBarrier): ONE SYNCS.ARRIVE.  With .release.cluster ptxas emits MEMBAR.ALL.GPU + ERRBAR + CGAERRBAR in front of
+// every arrive and with .acquire.cluster a CCTL.IVALL behind every wait (measured: the pair kernels ran 2.5x slower).
+// Nothing here passes generic-proxy data between the CTAs: the barriers order bulk copies, MMAs and tcgen05.ld, which the
+// tcgen05 fences and the async proxy's own completion cover.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t mbar_cluster)
 {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(mbar_cluster) : "memory");
-}
-// wait with acquire at cluster scope (the arrivals may come from the peer CTA)
-__device__ __forceinline__ void mbar_wait_cluster(uint32_t mbar, uint32_t parity)
-{
-  asm volatile("{\n\t.reg .pred p;\n\tWAITC_%=:\n\t"
-               "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t"
-               "@p bra DONEC_%=;\n\tbra WAITC_%=;\n\tDONEC_%=:\n\t}\n" :: "r"(mbar), "r"(parity) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" :: "r"(mbar_cluster) : "memory");
 }
 
 }}  // namespace lloid::tc
