@@ -19,6 +19,7 @@ struct F16Plan {
   int fir_list_c[2] = {-1, -1}, fir_list_n[2] = {0, 0};
   // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_pair_kernel) + f0-rate kernel (f0_pair_kernel)
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
+  bool r_tmem = false;                  // reconstruction kernels keep the unit's stationary R in TMEM (K <= 512) instead of shared memory
   std::vector<uint8_t> excluded;        // per (bin, detector): 1 = outside the limits, reconstructed by the FFMA kernels
   bool any_excluded = false;
   int n_bd = 0, n_lr = 0, n_sm = 148;

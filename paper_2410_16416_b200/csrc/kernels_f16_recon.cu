@@ -42,7 +42,16 @@ using namespace tc;
 
 constexpr int PK_THREADS = 544;             // 17 warps: 0 PY, 1 IY, 2 PQ0, 3 IQ0, 4 relay y, 5 relay q, 6 PQ1, 8-15 epilogue, 16 IQ1
 constexpr int PK_NSY_MAX = 16;
-constexpr int PK_NACC = 4;                  // accumulator buffers of 128 columns
+constexpr int PK_NACC_MAX = 4;              // accumulator buffers of 128 columns: 4 with R in shared memory, 2 with R in TMEM
+constexpr int PK_ACOL = 256;                // R in TMEM: columns [256, 256 + K / 2) beside two accumulators
+constexpr int PK_KMAX = 512;                // ... so a unit's summed L_pad is at most 512 there
+// Both kernels exist in two variants (template parameter RT).  RT = false: the unit's stationary R (128 rows x K per CTA) sits
+// in shared memory and every y MMA reads both operands from there -- the fastest variant on BASELINE config 2, but R, the band
+// matrices, the rho^(d) windows and the y ring must share 218 KB, which holds K <= ~320.  RT = true: the epilogue warps copy R
+// into TMEM once per unit and the y MMAs take A from TMEM (tcgen05.mma [d], [a], b-desc): K up to 512 (BASELINE config 4:
+// L up to 300 on the full-rate slice), half the shared-memory operand traffic, but only two accumulators.  The plan picks
+// RT = true only when some (bin, detector) needs it.
+template <bool RT> struct Acc { static constexpr uint32_t N = RT ? 2u : 4u; };
 constexpr int PK_NQB = 4;                   // rho^(d) tile events in flight (barrier slots)
 constexpr int PK_QDIST = 2;                 // the rows of tile e are requested when tile e - PK_QDIST has been consumed
 constexpr int PK_QPF = 4;                   // L2 prefetch distance of the rho^(d) rows, in tiles
@@ -190,8 +199,8 @@ __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, ui
 struct PairBars {
   uint64_t yfull[PK_NSY_MAX], yempty[PK_NSY_MAX];
   uint64_t qfull[PK_NQB], qempty[PK_NQB];
-  uint64_t acc_full[PK_NACC], acc_empty[PK_NACC], ybar[PK_NACC];
-  uint64_t consts, unit_done;
+  uint64_t acc_full[PK_NACC_MAX], acc_empty[PK_NACC_MAX], ybar[PK_NACC_MAX];
+  uint64_t consts, unit_done, r_ready;
 };
 
 // Barrier counts: a "full" barrier of the leader gets its own producers' arrive.expect_tx plus the peer's relay, the peer's
@@ -204,11 +213,12 @@ __device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int
     const uint32_t relay = rank == 0 ? 1u : 0u;
     for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), 1u + relay); mbar_init(smem_u32(&B.yempty[s]), 1); }
     for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), n_pq + relay); mbar_init(smem_u32(&B.qempty[s]), 1); }
-    for (int b = 0; b < PK_NACC; ++b) {
+    for (int b = 0; b < PK_NACC_MAX; ++b) {
       mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 16); mbar_init(smem_u32(&B.ybar[b]), 1);
     }
     mbar_init(smem_u32(&B.consts), 1u + relay);
     mbar_init(smem_u32(&B.unit_done), 1);
+    mbar_init(smem_u32(&B.r_ready), 16);          // RT: "the unit's R is in TMEM": one arrival per epilogue warp of both CTAs
     mbar_init_fence();
   }
   fence_before();
@@ -230,13 +240,15 @@ __host__ __device__ inline int stage_count(int nm) { return (nm + 7) >> 3; }
 
 // m back-to-back MMAs of one y stage: D (+)= R[l-groups from a_lo] * stage^T, N = 128.  a_lo: descriptor of R at this K
 // offset (LBO 2048: 128 rows per l-group, 256 sixteen-byte units per K = 16); b_lo: the stage (LBO 1024: 64 rows, 128 units)
+// RT: a_lo is the TMEM address of R's columns for this K offset (8 columns per K = 16).
+template <bool RT>
 __device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, int m, uint32_t acc0)
 {
-  mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, acc0);
+  if constexpr (RT) mma2_ts(d_tmem, a_lo, desc64(b_lo), idesc, acc0); else mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, acc0);
 #pragma unroll 4
   for (int k = 1; k < m; ++k) {
-    a_lo += 256u; b_lo += 128u;
-    mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, 1u);
+    a_lo += RT ? 8u : 256u; b_lo += 128u;
+    if constexpr (RT) mma2_ts(d_tmem, a_lo, desc64(b_lo), idesc, 1u); else mma2_ss(d_tmem, desc64(a_lo), desc64(b_lo), idesc, 1u);
   }
 }
 
@@ -270,12 +282,21 @@ struct YAddr { uint32_t full0, empty0, dst0, step; };   // barrier arrays and sl
 // PY role of both kernels: y stages of the unit's slices for tiles [t0, t1) (this CTA's 64-row half of every 128-row
 // tile), and the stationary R of the unit.  R goes out after `pre` stages of the new unit are in flight: the ring refills
 // while the previous unit drains.  extra/extra_bytes: loaded once with the first R (the f0 kernel's band matrices).
+// RT (R in TMEM, loaded by the epilogue warps): only the band matrices go out, with the first unit.
+template <bool RT>
 __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i, const SegSrc& sg, uint32_t consts_u, uint32_t unit_done_u, uint32_t sR_u,
                                            uint32_t rank, int t0, int t1, uint32_t extra_dst, const uint8_t* extra, uint32_t extra_bytes,
                                            bool trace, long long* tw)
 {
   int pre = (seg_i == 0) ? 0 : min((int)rg.n, sg.stages_per_tile);
   bool need_R = true;
+  if constexpr (RT) {
+    need_R = false;
+    if (seg_i == 0) {
+      if (extra_bytes) { mbar_expect_tx(consts_u, extra_bytes); copy_pieces(extra_dst, extra, extra_bytes, consts_u); }
+      else mbar_arrive(consts_u);
+    }
+  }
   auto load_R = [&]() {
     if (seg_i > 0) TWAIT(1, unit_done_u, (uint32_t)(seg_i - 1) & 1u);   // every MMA that reads the old R is complete
     mbar_expect_tx(consts_u, sg.rbytes + (seg_i == 0 ? extra_bytes : 0u));
@@ -287,7 +308,7 @@ __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i
     if (seg_i == 0 && extra_bytes) copy_pieces(extra_dst, extra, extra_bytes, consts_u);
     need_R = false;
   };
-  if (pre == 0) load_R();
+  if (need_R && pre == 0) load_R();
   for (int t = t0; t < t1; ++t)
     for (int i = 0; i < sg.n; ++i) {
       const int nm = sg.nm[i], nst = sg.nst[i], base = sg.mbase[i], ext = sg.ext[i];
@@ -309,11 +330,14 @@ __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i
 }
 
 // relay role (peer CTA): forwards the completion of this CTA's y stages and R loads to the leader's barriers
+template <bool RT>
 __device__ __forceinline__ void relay_y_segment(YRing& rg, const YAddr ya, int& seg_i, int n_stages, uint32_t consts_u)
 {
-  // consts first (it is requested before or among the first stages of the unit and the leader needs it first)
-  mbar_wait(consts_u, (uint32_t)seg_i & 1u);
-  mbar_arrive_cluster(consts_u & kLeaderMask);
+  // consts first (it is requested before or among the first stages of the unit and the leader needs it first); RT: once
+  if (!RT || seg_i == 0) {
+    mbar_wait(consts_u, (uint32_t)seg_i & 1u);
+    mbar_arrive_cluster(consts_u & kLeaderMask);
+  }
   for (int n = n_stages; n > 0; --n) {
     const uint32_t full = ya.full0 + 8u * rg.s;
     mbar_wait(full, rg.ph);
@@ -323,7 +347,38 @@ __device__ __forceinline__ void relay_y_segment(YRing& rg, const YAddr ya, int& 
   ++seg_i;
 }
 
+// RT, epilogue warps at the start of a unit: the unit's R block of this CTA (128 rows x K) -> TMEM columns [PK_ACOL, PK_ACOL + K / 2).
+// R16 is [l / 8][lane][8 fp16]: a thread (= lane) reads the 16 bytes of one l-group and stores them as four 32-bit columns;
+// the two warp groups (wg) take alternate l-groups.  Called when every MMA of the previous unit is complete (the caller has
+// just drained that unit's last accumulator); afterwards r_ready tells the issuing thread.
+__device__ __forceinline__ void load_R_tmem(const SliceParams* __restrict__ sp, const int32_t* slice, int n, int rb,
+                                            uint32_t tmem_lane_base, int lane_row, int wg)
+{
+  uint32_t col = tmem_lane_base + PK_ACOL;
+  for (int i = 0; i < n; ++i) {
+    const SliceParams* P = sp + slice[i];
+    const int ng = P->L_pad >> 3;
+    const uint4* __restrict__ src = reinterpret_cast<const uint4*>(reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * P->L_pad * 256) + lane_row;
+    int g = wg;
+    for (; g + 6 < ng; g += 8) {             // four loads in flight
+      const uint4 v0 = __ldg(src + (size_t)g * 128), v1 = __ldg(src + (size_t)(g + 2) * 128);
+      const uint4 v2 = __ldg(src + (size_t)(g + 4) * 128), v3 = __ldg(src + (size_t)(g + 6) * 128);
+      tmem_st4(col + 4u * g, v0.x, v0.y, v0.z, v0.w);
+      tmem_st4(col + 4u * (g + 2), v1.x, v1.y, v1.z, v1.w);
+      tmem_st4(col + 4u * (g + 4), v2.x, v2.y, v2.z, v2.w);
+      tmem_st4(col + 4u * (g + 6), v3.x, v3.y, v3.z, v3.w);
+    }
+    for (; g < ng; g += 2) {
+      const uint4 v = __ldg(src + (size_t)g * 128);
+      tmem_st4(col + 4u * g, v.x, v.y, v.z, v.w);
+    }
+    col += 4u * ng;
+  }
+  tmem_st_wait();
+}
+
 // IY role: the y MMAs of one tile into accumulator d_tmem (first MMA overwrites)
+template <bool RT>
 __device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, const SegSrc& sg, uint32_t d_tmem, uint32_t a_base, uint32_t idesc,
                                         bool trace, long long* tw)
 {
@@ -334,10 +389,10 @@ __device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, const SegSrc&
       const int m = base + (j < ext ? 1 : 0);
       TWAIT(2, ya.full0 + 8u * rg.s, rg.ph);
       fence_after();
-      mma_y_stage(d_tmem, a_lo, ya.dst0 + rg.s * ya.step, idesc, m, acc);
+      mma_y_stage<RT>(d_tmem, a_lo, ya.dst0 + rg.s * ya.step, idesc, m, acc);
       commit2(ya.empty0 + 8u * rg.s, 3);
       acc = 1u;
-      a_lo += (uint32_t)m * 256u;
+      a_lo += (uint32_t)m * (RT ? 8u : 256u);
       rg.advance();
     }
   }
@@ -350,6 +405,7 @@ struct LowPArgs {
   SchedArgs sched;
 };
 
+template <bool RT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PK_THREADS, 1)
 lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
 {
@@ -369,9 +425,10 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   const int nsy = a.nsy;
   pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 1u);
   const uint32_t tmem = tmem_slot;
-  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
-  const uint32_t ring_u = sR_u + (uint32_t)a.r_bytes;
-  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done);
+  constexpr uint32_t NACC = Acc<RT>::N;
+  const uint32_t sR_u = smem_u32(smem);                 // !RT: [l_sum / 8][128 rows][8] fp16
+  const uint32_t ring_u = sR_u + (RT ? 0u : (uint32_t)a.r_bytes);
+  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done), r_ready_u = smem_u32(&bars.r_ready);
   const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
 
   if (warp == 0) {
@@ -383,7 +440,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
-        py_segment(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, 0u, nullptr, 0u, trace, tw);
+        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, 0u, nullptr, 0u, trace, tw);
         nt += t1 - t0;
       }
       if (rank == 0) TRACE_END(0, 0, nt);
@@ -396,7 +453,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
-        relay_y_segment(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
+        relay_y_segment<RT>(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
   } else if (warp == 1 && rank == 0) {
@@ -405,7 +462,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
     if (elect_one()) {
       SegSrc& sg = seg[1];
       const uint32_t idesc = idesc_f16_pair(128);
-      const uint32_t a_base = desc_lo(sR_u, 2048u);
+      const uint32_t a_base = RT ? tmem + PK_ACOL : desc_lo(sR_u, 2048u);
       const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]), acc_empty_u = smem_u32(&bars.acc_empty[0]);
       const YAddr yd{ya.full0, ya.empty0, desc_lo(ring_u, 1024u), (uint32_t)a.ystage >> 4};   // dst = descriptor of the stage
       YRing rg{0u, 0u, (uint32_t)nsy};
@@ -416,16 +473,16 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(sg, a.sp, G->slice, G->n_slices, 2 * un.pb);
-        TWAIT(0, consts_u, (uint32_t)seg_i & 1u);
+        if constexpr (RT) TWAIT(0, r_ready_u, (uint32_t)seg_i & 1u); else TWAIT(0, consts_u, (uint32_t)seg_i & 1u);   // the unit's R is in place
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
-          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+          const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
           TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          iy_tile(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          iy_tile<RT>(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
           commit2(acc_full_u + 8u * b, 3);
         }
-        commit2(unit_done_u, 3);
+        if constexpr (!RT) commit2(unit_done_u, 3);
         ++seg_i;
       }
       TRACE_END(0, 1, (int)e);
@@ -442,9 +499,17 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       const LowUnit un = a.units[u];
       const RateGroup* Gp = a.groups + un.group;
       const int q_cap = Gp->q_groups_cap;
+      if constexpr (RT) {
+        // this warp has drained the previous unit's last accumulator, so every MMA that read the old R is complete
+        __syncwarp();
+        load_R_tmem(a.sp, Gp->slice, Gp->n_slices, 2 * un.pb + (int)rank, tmem + ((uint32_t)(q * 32) << 16), row, wg);
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(r_ready_u & kLeaderMask);
+      }
       __half* __restrict__ Q = Gp->Q + ((size_t)(2 * un.pb + (int)rank) * q_cap * 128 + row) * 8;
       for (int t = t0; t < t1; ++t, ++e) {
-        const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+        const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
         TWAIT(0, acc_full_u + 8u * b, ph);
         fence_after();
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
@@ -485,7 +550,7 @@ struct F0PArgs {
   PairMma tab[kPairTabMax];                             // interpolation MMAs, see PairMma
 };
 
-template <bool CAPTURE>
+template <bool CAPTURE, bool RT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(PK_THREADS, 1)
 f0_pair_kernel(const __grid_constant__ F0PArgs a)
 {
@@ -511,13 +576,14 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   { F0Iter it{pA, pB}; if (it.at_end()) return; }       // both CTAs of the cluster take the same decision
 
   const int nsy = a.nsy, n_lr = a.n_lr, gt = S.gt;
-  const uint32_t sR_u = smem_u32(smem);                 // [l_sum / 8][128 rows][8] fp16
-  const uint32_t sP_u = sR_u + (uint32_t)a.r_bytes;     // this rank's band-matrix blocks
+  constexpr uint32_t NACC = Acc<RT>::N;
+  const uint32_t sR_u = smem_u32(smem);                 // !RT: [l_sum / 8][128 rows][8] fp16
+  const uint32_t sP_u = sR_u + (RT ? 0u : (uint32_t)a.r_bytes);     // this rank's band-matrix blocks
   const uint32_t sQ_u = sP_u + (uint32_t)a.p_bytes;     // per-rate circular buffers of 16-row chunks (4 KB each)
   const uint32_t ring_u = sQ_u + (uint32_t)a.q_bytes;   // y ring
   pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 2u);
   const uint32_t tmem = tmem_slot;
-  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done);
+  const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done), r_ready_u = smem_u32(&bars.r_ready);
   const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
   const uint32_t qfull_u = smem_u32(&bars.qfull[0]), qempty_u = smem_u32(&bars.qempty[0]);
   const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]), ybar_u = smem_u32(&bars.ybar[0]);
@@ -532,7 +598,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
         seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
-        py_segment(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes, trace, tw);
+        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes, trace, tw);
         nt += t1 - t0;
       }
       if (rank == 0) TRACE_END(1, 0, nt);
@@ -545,7 +611,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
         seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
-        relay_y_segment(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
+        relay_y_segment<RT>(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
   } else if (warp == 2 || warp == 6) {
@@ -632,7 +698,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
     if (elect_one()) {
       SegSrc& sg = seg[1];
       const uint32_t idesc = idesc_f16_pair(128);
-      const uint32_t a_base = desc_lo(sR_u, 2048u);
+      const uint32_t a_base = RT ? tmem + PK_ACOL : desc_lo(sR_u, 2048u);
       const uint32_t acc_empty_u = smem_u32(&bars.acc_empty[0]);
       const YAddr yd{ya.full0, ya.empty0, desc_lo(ring_u, 1024u), (uint32_t)a.ystage >> 4};
       YRing rg{0u, 0u, (uint32_t)nsy};
@@ -643,13 +709,13 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
         seg_fill(sg, a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb);
-        TWAIT(0, consts_u, (uint32_t)seg_i & 1u);
+        if constexpr (RT) TWAIT(0, r_ready_u, (uint32_t)seg_i & 1u); else TWAIT(0, consts_u, (uint32_t)seg_i & 1u);   // the unit's R is in place
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
-          const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+          const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
           TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          iy_tile(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          iy_tile<RT>(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
           commit2(ybar_u + 8u * b, 1);
         }
         ++seg_i;
@@ -672,6 +738,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
       }
       const uint32_t p_base = sP_u >> 4;
       TRACE_BEGIN();
+      if constexpr (RT) { mbar_wait(consts_u, 0u); fence_after(); }   // the band matrices of both CTAs have landed (!RT: they come with the first R)
       FOR_F0_SEGMENTS(it, S, pA, pB) {
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         uint32_t mine = 0;
@@ -680,9 +747,9 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
           if (r < n_lr && a.groups[bdi * n_lr + r].n_slices > 0) { mine |= 1u << r; sb[r] = ((adv[r] * t0) >> 4) % cap[r]; }
         for (int t = t0; t < t1; ++t, ++e) {
           if ((e & 1u) == which) {
-            const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+            const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
             TWAIT(0, ybar_u + 8u * b, ph);
-            TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), ph);
+            TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), (e >> 2) & 1u);
             fence_after();
             const uint32_t d_tmem = tmem + b * 128u;
 #pragma unroll
@@ -708,8 +775,8 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
             sb[r] += dch; if (sb[r] >= cap[r]) sb[r] -= cap[r];
           }
         }
-        if (((e - 1u) & 1u) == which) {                 // the owner of the unit's last tile, once the other thread's last tile is done too
-          if (t1 - t0 >= 2) mbar_wait(acc_full_u + 8u * ((e - 2u) & (PK_NACC - 1)), ((e - 2u) >> 2) & 1u);
+        if (!RT && ((e - 1u) & 1u) == which) {          // the owner of the unit's last tile, once the other thread's last tile is done too
+          if (t1 - t0 >= 2) mbar_wait(acc_full_u + 8u * ((e - 2u) & (NACC - 1)), ((e - 2u) / NACC) & 1u);
           commit2(unit_done_u, 3);
         }
       }
@@ -730,11 +797,20 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
       const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
       const int n_templates = a.bd[bdi].n_templates;
       const int p0 = (2 * it.cur.pb + (int)rank) * 64 + 16 * q + tq;      // template of h = 0; h = 1: + 8
+      if constexpr (RT) {
+        // this warp has drained the previous unit's last accumulator, so every MMA that read the old R is complete
+        const BdPlan* B = a.bd + bdi;
+        __syncwarp();
+        load_R_tmem(a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank, tmem + ((uint32_t)(q * 32) << 16), q * 32 + lane, wg);
+        fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(r_ready_u & kLeaderMask);
+      }
       uint32_t bqt[2] = {0u, 0u};                                       // running maximum of the granule (truncated bits)
       int bk[2] = {0, 0};
       float bre[2] = {0.f, 0.f}, bim[2] = {0.f, 0.f};
       for (int t = t0; t < t1; ++t, ++e) {
-        const uint32_t b = e & (PK_NACC - 1), ph = (e >> 2) & 1u;
+        const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
         TWAIT(0, acc_full_u + 8u * b, ph);
         __syncwarp();
         fence_after();
@@ -987,10 +1063,22 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   pl->p_bytes = (int)((pblob[0].size() * sizeof(__half) + 127) / 128 * 128);
   pl->q_bytes = q_bytes;
 
-  // per-(bin, detector) shared-memory limits: stationary R (this CTA's 128 rows) + P + windows + >= 3 y stages
+  // Where the stationary R of a unit lives (template parameter RT of the kernels).  In shared memory it competes with P, the
+  // windows and >= 3 y stages: if EVERY (bin, detector) fits that way the bank runs the RT = false kernels; otherwise the
+  // whole bank runs the RT = true kernels (R in TMEM, K <= 512), and only what exceeds THAT is left to the FFMA kernels.
   {
-    const int lim_f0 = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / 256;
-    const int lim_low = (PK_SMEM_BUDGET - 3 * 16384) / 256;
+    const int lim_f0_smem = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / 256;
+    const int lim_low_smem = (PK_SMEM_BUDGET - 3 * 16384) / 256;
+    bool rt = false;
+    for (int b = 0; b < n_bd; ++b) {
+      if (pl->excluded[b]) continue;
+      if (pl->bd_host[b].l_sum > lim_f0_smem) rt = true;
+      for (int r = 0; r < pl->n_lr; ++r) if (pl->groups_host[(size_t)b * pl->n_lr + r].l_sum > lim_low_smem) rt = true;
+    }
+    if (getenv("LLOID_R_TMEM")) rt = atoi(getenv("LLOID_R_TMEM")) != 0;      // debugging / A-B measurements
+    pl->r_tmem = rt;
+    const int lim_f0 = rt ? PK_KMAX : lim_f0_smem, lim_low = rt ? PK_KMAX : lim_low_smem;
+    if (rt && PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes < 3 * 16384) return true;
     for (int b = 0; b < n_bd; ++b) {
       if (pl->bd_host[b].l_sum > lim_f0) pl->excluded[b] = 1;
       for (int r = 0; r < pl->n_lr; ++r)
@@ -1002,8 +1090,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
     if (pl->combos_host.empty()) return true;             // nothing fits: the whole bank goes to the FFMA kernels
   }
-  const int f0_fixed = pl->l_sum_f0_max * 256 + pl->p_bytes + pl->q_bytes;
-  const int low_fixed = pl->l_sum_low_max * 256;
+  const int f0_fixed = (pl->r_tmem ? 0 : pl->l_sum_f0_max * 256) + pl->p_bytes + pl->q_bytes;
+  const int low_fixed = pl->r_tmem ? 0 : pl->l_sum_low_max * 256;
   // y stage slot: the largest stage of any slice the kernel streams (a slice with nm = L_pad / 16 MMAs per tile is cut
   // into ceil(nm / 8) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
   int ys_f0 = 2048, ys_low = 2048;
@@ -1075,9 +1163,12 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 
   // opt-in shared memory: the architecture maximum, for every kernel of this file, on this device (never lowered
   // by a later, smaller bank)
-  cudaError_t e = set_max_dyn_smem(f0_pair_kernel<false>);
-  if (e == cudaSuccess) e = set_max_dyn_smem(f0_pair_kernel<true>);
-  if (e == cudaSuccess) e = set_max_dyn_smem(lowrate_pair_kernel);
+  cudaError_t e = set_max_dyn_smem(f0_pair_kernel<false, false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(f0_pair_kernel<true, false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(f0_pair_kernel<false, true>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(f0_pair_kernel<true, true>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(lowrate_pair_kernel<false>);
+  if (e == cudaSuccess) e = set_max_dyn_smem(lowrate_pair_kernel<true>);
   if (e != cudaSuccess) { snprintf(err, errlen, "fp16 plan: cudaFuncSetAttribute failed: %s", cudaGetErrorString(e)); return false; }
   pl->tensor_recon = true;
   return true;
@@ -1120,7 +1211,8 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
       tiles_total += (long long)sc.n_tiles[r] * pl->units_per_rate[r];
     }
     const int grid = 2 * (int)std::min<long long>(n_clusters, tiles_total);
-    lowrate_pair_kernel<<<grid, PK_THREADS, pl->low_smem, st>>>(la);
+    if (pl->r_tmem) lowrate_pair_kernel<true><<<grid, PK_THREADS, pl->low_smem, st>>>(la);
+    else lowrate_pair_kernel<false><<<grid, PK_THREADS, pl->low_smem, st>>>(la);
     ++*launches;
   }
   if (after_lowrate) cudaEventRecord(after_lowrate, st);
@@ -1141,8 +1233,13 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   memcpy(a.tab, pl->tab, sizeof a.tab);
   const long long pair_tiles = (long long)pl->combos_host.size() * n_tiles;
   const int grid = 2 * (int)std::min<long long>(n_clusters, pair_tiles);
-  if (cap.snr) f0_pair_kernel<true><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
-  else f0_pair_kernel<false><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+  if (pl->r_tmem) {
+    if (cap.snr) f0_pair_kernel<true, true><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+    else f0_pair_kernel<false, true><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+  } else {
+    if (cap.snr) f0_pair_kernel<true, false><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+    else f0_pair_kernel<false, false><<<grid, PK_THREADS, pl->f0_smem, st>>>(a);
+  }
   ++*launches;
   const cudaError_t e = cudaPeekAtLastError();
   if (e != cudaSuccess) fprintf(stderr, "lloid: f0_pair_kernel launch (grid %d, %d threads, %d B shared, %zu B params): %s\n", grid, PK_THREADS, pl->f0_smem, sizeof a, cudaGetErrorString(e));

@@ -366,6 +366,13 @@ int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const 
       b->d_max = std::max(b->d_max, S.d);
     }
     if (expect_delay != B.M) { delete b; return fail(LLOID_EINVAL, "bin %d: slices cover %lld samples, template_len is %lld", bi, (long long)expect_delay, (long long)B.M); }
+    {
+      // folded slices are reconstructed at f0 next to the d = 1 slices: their summed L_pad must fit the f0 kernel's
+      // stationary operand (512 basis filters); otherwise the bin keeps its low-rate slices on the low-rate path
+      int l_f0 = 0, n_f0 = 0;
+      for (const SliceHost& S : B.slices) if (S.d == 1 || S.fold) { l_f0 += S.L_pad; ++n_f0; }
+      if (l_f0 > 512 || n_f0 > kMaxF0Slices) for (SliceHost& S : B.slices) S.fold = false;
+    }
     b->max_templates = std::max(b->max_templates, B.N);
     b->max_rows_pad = std::max(b->max_rows_pad, B.rows_pad);
     for (int det = 0; det < cfg->n_detectors; ++det) {

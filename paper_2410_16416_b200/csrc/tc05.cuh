@@ -132,6 +132,11 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* r)
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                :: "r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
 }
+// registers -> TMEM, 4 consecutive columns of this warp's 32 lanes (one 16-byte group of 8 fp16 of an A operand row)
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3)
+{
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" :: "r"(taddr), "r"(r0), "r"(r1), "r"(r2), "r"(r3) : "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // ---- warp-uniform single-thread issue -----------------------------------------------------------
@@ -228,6 +233,14 @@ __device__ __forceinline__ void mma2_ss(uint32_t d_tmem, uint64_t adesc, uint64_
   asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
                "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
                :: "r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// the same with A in TMEM: each CTA's 128 rows in ITS lanes, columns [a_tmem, a_tmem + 8) per K = 16 (two fp16 per column).
+// Only B then comes out of shared memory (4 KB per N = 128 MMA: half of the 128 B/clk an SS MMA of this shape takes)
+__device__ __forceinline__ void mma2_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate)
+{
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+               "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n"
+               :: "r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
 // arrives (once every tcgen05 op issued so far by this thread has completed) on [mbar] of every CTA in cta_mask
 __device__ __forceinline__ void commit2(uint32_t mbar, uint16_t cta_mask)
