@@ -55,14 +55,14 @@ typedef struct {
   int32_t n_bins;            /* B                                                                  */
   int32_t n_detectors;       /* D                                                                  */
   int32_t full_rate_hz;      /* f0, e.g. 2048                                                      */
-  int32_t peak_window;       /* W in f0 samples (e.g. 2048); multiple of 256                       */
+  int32_t peak_window;       /* W in f0 samples (e.g. 2048); multiple of 128                       */
   float   snr_threshold;     /* theta; trigger iff |rho| > theta (strict)             */
   int32_t k_down;            /* K_dn: decimation kernel half-width in low-rate zero crossings (16) */
   int32_t k_up;              /* K_up: interpolation kernel half-width (8); must be 8 in this version */
   int32_t precision;         /* lloid_precision_t                                                  */
   int32_t device;            /* CUDA device ordinal                                                */
   int32_t max_chunk;         /* 0 = automatic; else internal time-chunk length in f0 samples
-                                (multiple of 256): lloid_filter walks the buffer in chunks of this
+                                (multiple of 128): lloid_filter walks the buffer in chunks of this
                                 size so that intermediates stay bounded / L2-resident              */
 } lloid_bank_config_t;
 
@@ -167,6 +167,13 @@ int64_t lloid_samples_consumed(const lloid_bank_t *bank);
 int64_t lloid_chunk_samples(const lloid_bank_t *bank);
 int64_t lloid_last_launch_count(const lloid_bank_t *bank);
 int64_t lloid_device_bytes(const lloid_bank_t *bank);
+
+/* Which kernels a finalized bank runs on (introspection for tests and benchmarks): out[0] = 1 if the fp16 bank's
+ * reconstruction runs on the tcgen05 kernels, out[1] = 1 if those keep the stationary reconstruction matrix in TMEM
+ * (banks whose full-rate slices have more basis filters than fit shared memory), out[2] = number of (bin, detector)
+ * pairs left to the CUDA-core reconstruction kernels, out[3] = number of (bin, slice) pairs whose interpolation is
+ * folded into the basis filters.  All zero for an fp32 bank.  out: host, int32[4]. */
+int lloid_path_info(const lloid_bank_t *bank, int32_t *out);
 
 /* Time (ms, CUDA events on the call's stream) spent by the last lloid_filter call in each stage:
  * out_ms[0..5] = resample, basis FIR, reconstruction+epilogue (both kernels of the fp16 path), peak

@@ -65,6 +65,7 @@ EXPORTS = {
     "lloid_chunk_samples": (C.c_int64, [C.c_void_p]),
     "lloid_last_launch_count": (C.c_int64, [C.c_void_p]),
     "lloid_device_bytes": (C.c_int64, [C.c_void_p]),
+    "lloid_path_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
     "lloid_set_profiling": (C.c_int, [C.c_void_p, C.c_int32]),
     "lloid_last_stage_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
     "lloid_destroy": (None, [C.c_void_p]),
@@ -184,6 +185,12 @@ def lloid_last_launch_count(bank) -> int:
 
 def lloid_device_bytes(bank) -> int:
     return lib().lloid_device_bytes(bank)
+
+
+def lloid_path_info(bank) -> dict:
+    out = (C.c_int32 * 4)()
+    _check(lib().lloid_path_info(bank, out))
+    return dict(tensor_recon=bool(out[0]), r_in_tmem=bool(out[1]), cuda_core_bds=int(out[2]), folded_slices=int(out[3]))
 
 
 def lloid_set_profiling(bank, enable: bool) -> None:

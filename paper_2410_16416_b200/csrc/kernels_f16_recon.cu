@@ -1175,6 +1175,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
 }
 
 bool f16_plan_tensor_recon(const F16Plan* pl) { return pl && pl->tensor_recon; }
+bool f16_plan_r_tmem(const F16Plan* pl) { return pl && pl->tensor_recon && pl->r_tmem; }
 void f16_plan_disable_tensor_recon(F16Plan* pl) { if (pl) pl->tensor_recon = false; }
 const uint8_t* f16_plan_excluded(const F16Plan* pl) { return (pl && pl->tensor_recon && pl->any_excluded) ? pl->excluded.data() : nullptr; }
 

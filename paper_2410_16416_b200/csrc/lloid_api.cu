@@ -795,7 +795,24 @@ int lloid_last_stage_ms(lloid_bank_t* b, float* out)
   return LLOID_OK;
 }
 
-int lloid_debug_trace(long long* out, int reset) { return f16_read_trace(out, reset) ? LLOID_ECUDA : LLOID_OK; }
+#ifdef LLOID_TRACE_BUILD
+int lloid_debug_trace(long long* out, int reset) { return f16_read_trace(out, reset) ? LLOID_ECUDA : LLOID_OK; }   // scratch builds only
+#endif
+
+int lloid_path_info(const lloid_bank_t* b, int32_t* out)
+{
+  if (!b || !out) return fail(LLOID_EINVAL, "null argument");
+  if (!b->finalized) return fail(LLOID_ESTATE, "path info before finalize");
+  out[0] = out[1] = out[2] = out[3] = 0;
+  if (b->f16 && b->plan16) {
+    out[0] = f16_plan_tensor_recon(b->plan16) ? 1 : 0;
+    out[1] = f16_plan_r_tmem(b->plan16) ? 1 : 0;
+    if (const uint8_t* ex = f16_plan_excluded(b->plan16)) for (int i = 0; i < b->n_bd; ++i) out[2] += ex[i];
+    else if (!out[0]) out[2] = b->n_bd;
+    for (const BinHost& B : b->bins) for (const SliceHost& S : B.slices) out[3] += S.fold ? 1 : 0;
+  }
+  return LLOID_OK;
+}
 
 void lloid_destroy(lloid_bank_t* b)
 {

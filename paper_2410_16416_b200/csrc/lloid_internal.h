@@ -210,6 +210,7 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems /* reconstru
                          int n_det, int chunk_cap, const double* const* up_w /* [kMaxRates]: w[(i+K_up) d + phi] or null */,
                          int64_t* bytes, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
+bool f16_plan_r_tmem(const F16Plan*);          // reconstruction kernels keep the stationary R in TMEM (K <= 512)
 bool f16_plan_tensor_recon(const F16Plan*);   // false: bank outside the tensor reconstruction kernels' limits
 void f16_plan_disable_tensor_recon(F16Plan*);
 const uint8_t* f16_plan_excluded(const F16Plan*);   // tensor_recon only: per (bin, detector) flags of the bins left to the FFMA kernels, or null

@@ -193,8 +193,8 @@ def retruncate(bin_: BinData, n_basis: Sequence[int]) -> BinData:
     for sl, U, R, L in zip(bin_.slices, bin_.basis, bin_.recon, n_basis):
         L = min(int(L), U.shape[0])
         slices.append(SliceSpec(sl.rate, sl.d, sl.a, sl.b, sl.n_taps, L, sl.end_delay))
-        basis.append(np.ascontiguousarray(U[:L]))
-        recon.append(np.ascontiguousarray(R[:, :L]))
+        basis.append(U[:L])                    # views: 1000 re-truncated bins share the base bins' memory
+        recon.append(R[:, :L])
     return BinData(bin_.n_templates, bin_.template_len, slices, basis, recon, bin_.sigma,
                    None, None, bin_.mchirp)
 
@@ -322,8 +322,18 @@ def config4(n_bins: int = 1000, n_templates: int = 1000, seconds: int = 3600, n_
     for b in range(n_bins):
         L = [100 + ((37 * b + 61 * s) % 201) for s in range(len(CONFIG4_SPANS))]
         bins.append(retruncate(base[b % n_distinct], L))
-    x = make_strain(SEED0 + 1000 * 4, n_detectors, seconds * F0, bins, [], 15.0, 1024.0)
-    return Workload("config4", bins, n_detectors, x, [])
+    # 100 injections (BASELINE config 4): injection i -> bin 10 i, template 37 i mod N, A = 8 ... 20, phase
+    # 2 pi i / 100, the same in every detector; those whose bin exists in a reduced bank are kept.  End times are spread
+    # over the strain past the start-up transient, off every decimation grid.
+    n = seconds * F0
+    inj = []
+    if n > 2 * M + 64:
+        n_inj = min(100, (n_bins + 9) // 10)
+        for i in range(n_inj):
+            e = M + (i + 1) * ((n - 2 * M) // (n_inj + 1)) + 13 * i + 777
+            inj.append(Injection(10 * i, (37 * i) % n_templates, 8.0 + 12.0 * i / 99.0, 2.0 * math.pi * i / 100.0, int(e)))
+    x = make_strain(SEED0 + 1000 * 4, n_detectors, n, bins, inj, 15.0, 1024.0)
+    return Workload("config4", bins, n_detectors, x, inj)
 
 
 def toy(n_templates: int = 4, M: int = 256, spans=((2048, 0.0, 0.0625), (1024, 0.0625, 0.125)),

@@ -52,7 +52,8 @@ def run_gpu(w, precision, pieces: Optional[Sequence[int]] = None, capture: Optio
             launches += lb.lloid_last_launch_count(bank.handle)
             a += c
         info = dict(counts=counts, launches=launches, chunk=lb.lloid_chunk_samples(bank.handle),
-                    consumed=lb.lloid_samples_consumed(bank.handle), bytes=lb.lloid_device_bytes(bank.handle))
+                    consumed=lb.lloid_samples_consumed(bank.handle), bytes=lb.lloid_device_bytes(bank.handle),
+                    path=lb.lloid_path_info(bank.handle))
         trigs = np.concatenate(out) if out else np.zeros(0, dtype=lb.TRIGGER_DTYPE)
         return trigs, (None if snr is None else snr.cpu().numpy()), info
     finally:

@@ -122,6 +122,45 @@ def test_config4_geometry_heterogeneous_L(precision):
     assert _unique_keys(trigs, W)
 
 
+@pytest.fixture(scope="module")
+def cfg4_64():
+    return wl.config4(n_bins=64, n_templates=1000, seconds=160, n_detectors=3, n_distinct=2)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_config4_64_bins_full_template_count_chunk_2048(cfg4_64, precision):
+    """BASELINE config 4 at its per-bin size: 64 bins x 1000 templates x 3 detectors, L(b, s) in [100, 300], with the chunk
+    length forced to 2048 samples -- the clamp the 1000-bin bank runs into (less than one 128-row tile per chunk at
+    d = 32) -- 1536 reconstruction units per detector set, injections in bins 0, 10, ..., 60.  Dense window + trigger rules
+    on bin 5 (L = 285 on the full-rate slice), bin 10 (injected) and bin 63."""
+    w = cfg4_64
+    assert len(w.injections) == 7 and w.bins[5].slices[0].n_basis == 285
+    tol = pu.TOL[precision]
+    W = w.peak_window
+    inj = w.injections[1]
+    assert inj.bin == 10
+    k0 = (inj.end // W) * W
+    for bin_, det in ((5, 2), (10, 1), (63, 0)):
+        trigs, snr, info = pu.run_gpu(w, precision, capture=(bin_, det, k0, W), max_chunk=2048)
+        assert info["chunk"] == 2048 and info["consumed"] == w.n_samples
+        rho = pu.oracle_snr(w, bin_, det, k0, k0 + W)
+        assert not np.isnan(snr).any()
+        assert np.abs(snr - rho).max() <= tol
+        pu.check_triggers(trigs, rho, k0, w, bin_, det, tol)
+        if precision == lb.LLOID_F16:
+            assert info["path"]["tensor_recon"] and info["path"]["cuda_core_bds"] == 0, info["path"]   # no bin leaves tcgen05
+            assert info["path"]["r_in_tmem"]                                                          # L = 285 + folded 1024 Hz slice
+    assert _unique_keys(trigs, W)
+    # every injection in every detector.  At SNR 8 in unit noise the peak of a 64 s chirp (most of its power below 100 Hz)
+    # moves by a few samples (measured: up to 5), so the time is checked to +-8 samples here; exact indices are checked
+    # against the oracle above.
+    for i in w.injections:
+        for d in range(w.n_detectors):
+            hit = trigs[(trigs["bin"] == i.bin) & (trigs["detector"] == d) & (trigs["template_idx"] == i.template) & (np.abs(trigs["sample"] - i.end) <= 8)]
+            assert len(hit) >= 1, f"injection bin={i.bin} p={i.template} e={i.end} det={d} not recovered"
+            assert abs(float(np.hypot(hit["snr_re"], hit["snr_im"]).max()) - i.amplitude) < 4.5   # unit noise on an SNR-8 peak
+
+
 def _as_set(trigs):
     return sorted((int(t["bin"]), int(t["detector"]), int(t["template_idx"]), int(t["sample"]),
                    float(t["snr_re"]), float(t["snr_im"])) for t in trigs)
