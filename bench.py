@@ -113,29 +113,41 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
-def oracle_sample(w, seconds: float):
-    """Time the float64 oracle on a bounded sample: bin 0, detector 0, `seconds` of output past the
-    start-up transient, all templates, O1..O6.  Returns (template*s per wall-second, wall, cores)."""
+def _oracle_stretch(args):
+    """One oracle call: bin 0, detector 0, output samples [k0, k1).  Module-level so that a process pool can run it."""
+    w, k0, k1 = args
     from oracle import lloid_oracle as oc
-    try:
-        from threadpoolctl import threadpool_limits
-        limiter = threadpool_limits(1)
-        cores = 1
-    except Exception:
-        limiter, cores = None, os.cpu_count()
+    b = w.bins[0]
+    rho = oc.snr_series(w.strain[0].astype(np.float64), b.slices, b.basis, b.recon, k0, k1, w.k_down, w.k_up)
+    return len(oc.triggers(rho, k0, w.peak_window, w.threshold))
+
+
+def oracle_sample(w, seconds: float, all_cores: bool = False):
+    """Time the float64 oracle AS IT STANDS (single-threaded numpy; BLAS pinned to one thread) on a bounded sample:
+    bin 0, detector 0, `seconds` of output past the start-up transient, all templates, O1..O6.  all_cores: the same call
+    in one process per host core, each on its own `seconds`-long stretch (the work is independent across time).
+    Returns (template*s per wall-second, wall, cores actually used, description)."""
+    from threadpoolctl import threadpool_limits          # in the image; the oracle leg must not silently use more threads
     b = w.bins[0]
     W = w.peak_window
     k0 = ((b.template_len + W - 1) // W + 1) * W
-    k1 = min(w.n_samples, k0 + max(1, int(round(seconds * w.f0)) // W) * W)
-    x = w.strain[0].astype(np.float64)
-    t0 = time.perf_counter()
-    rho = oc.snr_series(x, b.slices, b.basis, b.recon, k0, k1, w.k_down, w.k_up)
-    trig = oc.triggers(rho, k0, W, w.threshold)
-    wall = time.perf_counter() - t0
-    if limiter is not None:
-        limiter.restore_original_limits()
-    ts = b.n_templates * (k1 - k0) / w.f0
-    return ts / wall, wall, cores, f"bin 0, detector 0, {b.n_templates} templates x {(k1 - k0) / w.f0:.0f} s of output (k in [{k0},{k1})), {len(trig)} triggers"
+    span = max(1, int(round(seconds * w.f0)) // W) * W
+    n_proc = 1
+    if all_cores:
+        n_proc = max(1, min(os.cpu_count() or 1, (w.n_samples - k0) // span))
+    jobs = [(w, k0 + i * span, k0 + (i + 1) * span) for i in range(n_proc)]
+    with threadpool_limits(1):
+        t0 = time.perf_counter()
+        if n_proc == 1:
+            n_trig = _oracle_stretch(jobs[0])
+        else:
+            import multiprocessing as mp
+            with mp.get_context("fork").Pool(n_proc) as pool:
+                n_trig = sum(pool.map(_oracle_stretch, jobs))
+        wall = time.perf_counter() - t0
+    ts = b.n_templates * n_proc * span / w.f0
+    return ts / wall, wall, n_proc, (f"bin 0, detector 0, {b.n_templates} templates x {n_proc} x {span / w.f0:.0f} s of output "
+                                    f"(from k = {k0}), {n_trig} triggers")
 
 
 def make_workload(args, rank=0):
@@ -187,6 +199,151 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def time_bank(w, precision, steps, warmup, chunk, local=0, world=1, bins=None, want_e2e=True, flush=None):
+    """Build a bank over `w` and time `steps` passes of the whole hot path.  Device leg: strain resident in HBM, CUDA
+    events around lloid_filter on the launching stream, L2 flushed between steps, the library's per-stage events recorded
+    DURING these steps.  e2e leg: lloid_filter_host from pinned host strain to host triggers.  Returns a dict; times are
+    this rank's (the caller takes the max over ranks)."""
+    import torch
+    from paper_2410_16416_b200 import binding as lb
+    bank = lb.Bank(w, precision, device=local, max_chunk=chunk, bins=bins)
+    n, D = w.n_samples, w.n_detectors
+    ids = bank.bin_ids
+    n_templates = sum(w.bins[b].n_templates for b in ids)
+    cap = n_templates * D * (n // w.peak_window + 1)
+    strain_dev = torch.from_numpy(w.strain).cuda()
+    trig_dev = torch.empty(cap * 32, dtype=torch.uint8, device="cuda")
+    cnt_dev = torch.zeros(1, dtype=torch.int64, device="cuda")
+    if flush is None:
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step_device():
+        lb.lloid_reset(bank.handle, stream)
+        bank.filter(strain_dev, trig_dev, cnt_dev, stream)
+
+    out = {"launches": 0, "times": []}
+    stage_sum = np.zeros(6)
+    with ClockSampler(local) as clocks:          # started before the warm-up: nvidia-smi needs a moment to come up
+        for _ in range(warmup):
+            step_device()
+        torch.cuda.synchronize()
+        lb.lloid_set_profiling(bank.handle, True)   # stage events on the stream, inside the timed steps (5 records per chunk)
+        clocks.mark_begin()
+        for _ in range(steps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            step_device()
+            e1.record()
+            e1.synchronize()
+            out["times"].append(e0.elapsed_time(e1))
+            out["launches"] += lb.lloid_last_launch_count(bank.handle)
+            stage_sum += lb.lloid_last_stage_ms(bank.handle)
+        torch.cuda.synchronize()
+        clocks.mark_end()
+        lb.lloid_set_profiling(bank.handle, False)
+    out["clocks"] = clocks.summary()
+    out["stage_ms"] = stage_sum / steps              # resample, FIR, recon (both kernels), merge, whole call, low-rate kernel
+    out["n_trig"] = int(cnt_dev.item())
+    out["units"] = n_templates * D * (n / w.f0)      # template * detector * seconds of strain per step, this rank
+    out["chunk"] = int(lb.lloid_chunk_samples(bank.handle))
+    out["dev_bytes"] = int(lb.lloid_device_bytes(bank.handle))
+    out["path"] = lb.lloid_path_info(bank.handle)
+    out["n_templates"] = n_templates
+    if want_e2e:
+        strain_pin = torch.from_numpy(w.strain).pin_memory()
+        trig_np = torch.empty(cap * 32, dtype=torch.uint8).pin_memory().numpy().view(lb.TRIGGER_DTYPE)
+        strain_np = strain_pin.numpy()
+        e2e_times, d2h = [], 0
+        for i in range(1 + steps):
+            lb.lloid_reset(bank.handle, stream)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            got, rc = bank.filter_host(strain_np, trig_np, stream)
+            dt = time.perf_counter() - t0
+            if i > 0:
+                e2e_times.append(dt)
+                d2h = 8 + 32 * min(got, cap)
+        out["e2e_s"] = sum(e2e_times)
+        out["d2h"] = int(d2h)
+        out["h2d"] = int(w.strain.nbytes)
+        out["last_triggers"] = trig_np[:min(got, cap)].copy()
+    del strain_dev, trig_dev
+    bank.close()
+    return out
+
+
+def load_traffic():
+    """DRAM bytes per launch of the reconstruction / FIR kernels from the committed ncu capture (profiles/r2_traffic.json,
+    written from `ncu --set full` by hand: dram__bytes_read.sum + dram__bytes_write.sum of one launch at the 131072-sample
+    chunk of config 2).  None when the file is missing."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return None
+
+
+def roofline_f16(w, stage, n_chunks, chunk, args, peaks):
+    """Roofline of the dominant kernel from the stage times of the TIMED steps.  Tensor credit is algorithmic flops only:
+    the interpolation MMAs (A4) and the extra taps of the folded slices are work done on the tensor pipe that is not counted."""
+    fl = workload_flops(w)
+    samples = float(w.n_samples) * w.n_detectors
+    # a slice at f0 / 2 is reconstructed by the f0 kernel (its interpolation is folded into the basis filters, DESIGN.md section 6)
+    f0_flops = sum(2.0 * 2 * b.n_templates * s.n_basis / s.d for b in w.bins for s in b.slices if s.d <= 2) * samples
+    low_flops = fl["recon"] * samples - f0_flops
+    f0_ms, low_ms = stage[2] - stage[5], stage[5]
+    kernels = {"fir_f16_pers_kernel": (fl["fir"] * samples, stage[1]), "lowrate_pair_kernel": (low_flops, low_ms),
+               "f0_pair_kernel": (f0_flops, f0_ms)}
+    dom = max(kernels, key=lambda k: kernels[k][1])
+    ach = kernels[dom][0] / (kernels[dom][1] * 1e-3) / 1e12
+    path_ach = (fl["fir"] + fl["recon"]) * samples / ((stage[1] + stage[2]) * 1e-3) / 1e12
+    pk = peaks["bf16_sustained"]
+    tr = load_traffic()
+    full_chunk = chunk == 131072 and (args.templates, args.detectors) == (1000, 2) and args.workload == "config2"
+    traffic = tr["kernels"].get(dom) if (tr and full_chunk) else None
+    roofline = {"bound": "tensor", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
+                "traffic": traffic,
+                "traffic_source": (tr or {}).get("source") if traffic is not None else None,
+                "peak_source": peaks["source"] + " (cuBLAS bf16 sustained; fp16 runs at the same rate)",
+                "times_from": "CUDA events recorded by the library inside the timed steps (mean over the steps)",
+                "launch_ms": kernels[dom][1] / n_chunks, "launches": n_chunks,
+                "kernels": {k: {"algorithmic_tflop": v[0] / 1e12, "ms": v[1], "tflops": v[0] / (v[1] * 1e-3) / 1e12,
+                                "frac": v[0] / (v[1] * 1e-3) / 1e12 / pk} for k, v in kernels.items() if v[1] > 0},
+                "fused_tensor_path": {"achieved": path_ach, "frac": path_ach / pk, "frac_of_datasheet_2250": path_ach / 2250.0}}
+    rates = sorted({s.d for b in w.bins for s in b.slices})
+    res_bytes = samples * (4.0 + sum((6.0 / d) if d > 1 else 2.0 for d in rates))
+    n_templates = sum(b.n_templates for b in w.bins)
+    merge_bytes = (w.n_samples / w.peak_window) * n_templates * w.n_detectors * (16.0 + 32.0 * 0.1)   # one partial per template and window + triggers
+    roofline["merge_hbm"] = {"achieved": merge_bytes / (stage[3] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                             "frac": merge_bytes / (stage[3] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[3],
+                             "note": "one 16-byte partial per template and peak window since round 2: launch-latency bound, not bandwidth bound"}
+    roofline["resample_hbm"] = {"achieved": res_bytes / (stage[0] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                                "frac": res_bytes / (stage[0] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[0]}
+    res_flops = samples * sum(2.0 * (2 * w.k_down * d + 1) / d for d in rates if d > 1)
+    alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+    roofline["resample_alu"] = {"achieved": res_flops / (stage[0] * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+                                "frac": res_flops / (stage[0] * 1e-3) / 1e12 / alu_peak, "flop_per_byte": res_flops / res_bytes,
+                                "note": "the direct-form decimator is ALU-bound (27 flop/B, 2.4x the machine balance): this is the bound it is judged against"}
+    return roofline
+
+
+def roofline_f32(w, stage):
+    fl = workload_flops(w)
+    samples = float(w.n_samples) * w.n_detectors
+    alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12       # FFMA lanes x 2 flop x max SM clock (DESIGN.md section 6)
+    dom = ("recon+upsample", (fl["recon"] + fl["upsample"]) * samples, stage[2]) if stage[2] >= stage[1] else ("fir", fl["fir"] * samples, stage[1])
+    ach = dom[1] / (dom[2] * 1e-3) / 1e12
+    return {"bound": "alu", "kernel": dom[0], "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
+            "traffic": None, "peak_source": "derived: 148 SM x 128 FFMA/clk x 2 x 1.965 GHz"}
+
+
+def stage_dict(stage):
+    return {"resample": stage[0], "fir": stage[1], "recon_epilogue": stage[2], "merge_compact": stage[3], "total": stage[4],
+            "recon_lowrate_part": stage[5]}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -202,204 +359,172 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     precision = lb.LLOID_F16 if args.precision == "f16" else lb.LLOID_F32
 
-    w = make_workload(args, rank)                         # weak scaling: one config-2 replica per rank
-    bank = lb.Bank(w, precision, device=local, max_chunk=args.chunk)
-    n, D = w.n_samples, w.n_detectors
-    n_templates = sum(b.n_templates for b in w.bins)
-    cap = n_templates * D * (n // w.peak_window + 1)
-    strain_dev = torch.from_numpy(w.strain).cuda()
-    trig_dev = torch.empty(cap * 32, dtype=torch.uint8, device="cuda")
-    cnt_dev = torch.zeros(1, dtype=torch.int64, device="cuda")
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    stream = torch.cuda.current_stream().cuda_stream
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step_device():
-        lb.lloid_reset(bank.handle, stream)
-        bank.filter(strain_dev, trig_dev, cnt_dev, stream)
-
-    # ---- device-resident throughput -----------------------------------------------------------
-    launches = 0
-    times = []
-    with ClockSampler(local) as clocks:          # started before the warm-up: nvidia-smi needs a moment to come up
-        for _ in range(args.warmup):
-            step_device()
-        barrier()
-        clocks.mark_begin()
-        for _ in range(args.steps):
-            flush.zero_()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            step_device()
-            e1.record()
-            e1.synchronize()
-            times.append(e0.elapsed_time(e1))
-            launches += lb.lloid_last_launch_count(bank.handle)
-        barrier()
-        clocks.mark_end()
-    n_trig = int(cnt_dev.item())
-    t_dev = torch.tensor([sum(times)], dtype=torch.float64, device="cuda")
+    w = make_workload(args, rank)                         # weak scaling: one replica of the workload per rank, own noise
+    barrier()
+    r = time_bank(w, precision, args.steps, args.warmup, args.chunk, local, world)
+    barrier()
+    t_dev = torch.tensor([sum(r["times"]), r["e2e_s"]], dtype=torch.float64, device="cuda")
     if world > 1:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-    total_ms = float(t_dev.item())
-    units = n_templates * D * (n / w.f0)                  # template * seconds of strain, this rank
-    value = world * units * args.steps / (total_ms * 1e-3)
-
-    # ---- stage times -> roofline of the dominant kernel ------------------------------------------
-    lb.lloid_set_profiling(bank.handle, True)
-    step_device()
-    torch.cuda.synchronize()
-    stage = lb.lloid_last_stage_ms(bank.handle)          # resample, FIR, recon+epilogue, merge, total
-    lb.lloid_set_profiling(bank.handle, False)
-    fl = workload_flops(w)
+        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)      # the slowest rank sets the time
+    total_ms, e2e_s = float(t_dev[0].item()), float(t_dev[1].item())
+    value = world * r["units"] * args.steps / (total_ms * 1e-3)
+    e2e_value = world * r["units"] * args.steps / e2e_s
+    stage = r["stage_ms"]
+    n_chunks = max(1, -(-w.n_samples // r["chunk"]))
     peaks = load_peaks()
-    samples = float(n) * D
-    launches_per_step = max(1, int(lb.lloid_last_launch_count(bank.handle)))
-    n_chunks = max(1, -(-n // int(lb.lloid_chunk_samples(bank.handle))))
-    if precision == lb.LLOID_F16:
-        # dominant kernel = f0_kernel (A3 of the full-rate slices + A4 + A5); its tensor credit is ONLY the algorithmic
-        # reconstruction flops of the d = 1 slices -- the interpolation MMAs (A4) are ALU-equivalent work done on the
-        # tensor pipe and are not counted.  The whole fused tensor path (A2 + A3, three kernels) is reported beside it.
-        f0_flops = sum(2.0 * 2 * b.n_templates * s.n_basis for b in w.bins for s in b.slices if s.d == 1) * samples
-        low_flops = fl["recon"] * samples - f0_flops
-        f0_ms, low_ms = stage[2] - stage[5], stage[5]
-        kernels = {"fir_f16_pers_kernel": (fl["fir"] * samples, stage[1]), "lowrate_recon_kernel": (low_flops, low_ms),
-                   "f0_kernel": (f0_flops, f0_ms)}
-        dom = max(kernels, key=lambda k: kernels[k][1])
-        ach = kernels[dom][0] / (kernels[dom][1] * 1e-3) / 1e12
-        path_ach = (fl["fir"] + fl["recon"]) * samples / ((stage[1] + stage[2]) * 1e-3) / 1e12
-        pk = peaks["bf16_sustained"]
-        # DRAM bytes (read + write) of ONE launch at the 131072-sample chunk, from the committed ncu --set full capture
-        ncu_traffic = {"f0_kernel": 1.167e9, "lowrate_recon_kernel": 1.115e9, "fir_f16_pers_kernel": 0.127e9}
-        full_chunk = (int(lb.lloid_chunk_samples(bank.handle)) == 131072 and (args.templates, args.detectors) == (1000, 2)
-                      and args.workload == "config2")
-        roofline = {"bound": "tensor", "kernel": dom, "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
-                    "traffic": ncu_traffic.get(dom) if full_chunk else None,
-                    "traffic_source": "profiles/r1_04_ncu_full.md (dram__bytes_read.sum + dram__bytes_write.sum, one launch)", "peak_source": peaks["source"] + " (cuBLAS bf16 sustained; fp16 runs at the same rate)",
-                    "launch_ms": kernels[dom][1] / n_chunks, "launches": n_chunks,
-                    "kernels": {k: {"algorithmic_tflop": v[0] / 1e12, "ms": v[1], "tflops": v[0] / (v[1] * 1e-3) / 1e12,
-                                    "frac": v[0] / (v[1] * 1e-3) / 1e12 / pk} for k, v in kernels.items()},
-                    "fused_tensor_path": {"achieved": path_ach, "frac": path_ach / pk,
-                                          "frac_of_datasheet_2250": path_ach / 2250.0}}
-        # A1 resampler against HBM: bytes = read x (4 B) + write every rate stream (fp32 + fp16) per f0 sample
-        rates = sorted({s.d for b in w.bins for s in b.slices})
-        res_bytes = samples * (4.0 + sum((6.0 / d) if d > 1 else 2.0 for d in rates))
-        merge_bytes = (n / 128.0) * n_templates * D * 16.0          # one 16-byte partial peak per template and 128-sample tile
-        roofline["merge_hbm"] = {"achieved": merge_bytes / (stage[3] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
-                                 "frac": merge_bytes / (stage[3] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[3]}
-        roofline["resample_hbm"] = {"achieved": res_bytes / (stage[0] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
-                                    "frac": res_bytes / (stage[0] * 1e-3) / 1e9 / peaks["hbm"], "ms": stage[0]}
-        # the direct-form decimator does 2 (2 K_dn d + 1) / d flop per input sample and rate: 27 flop per byte moved,
-        # 2.4 times the machine balance (74.4 TFLOP/s / 6.5 TB/s = 11.5 flop/B) -- its bound is the FP32 ALUs
-        res_flops = samples * sum(2.0 * (2 * w.k_down * d + 1) / d for d in rates if d > 1)
-        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        roofline["resample_alu"] = {"achieved": res_flops / (stage[0] * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
-                                    "frac": res_flops / (stage[0] * 1e-3) / 1e12 / alu_peak,
-                                    "flop_per_byte": res_flops / res_bytes}
-    else:
-        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12       # FFMA lanes x 2 flop x max SM clock
-        dom = ("recon+upsample", (fl["recon"] + fl["upsample"]) * samples, stage[2]) if stage[2] >= stage[1] else ("fir", fl["fir"] * samples, stage[1])
-        ach = dom[1] / (dom[2] * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": dom[0], "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
-                    "traffic": None, "peak_source": "derived: 148 SM x 128 FFMA/clk x 2 x 1.965 GHz"}
-    roofline["stage_ms"] = {"resample": stage[0], "fir": stage[1], "recon_epilogue": stage[2], "merge_compact": stage[3], "total": stage[4],
-                            "recon_lowrate_part": stage[5]}
+    roofline = roofline_f16(w, stage, n_chunks, r["chunk"], args, peaks) if precision == lb.LLOID_F16 else roofline_f32(w, stage)
+    roofline["stage_ms"] = stage_dict(stage)
 
-    # ---- end to end: pinned host strain in, triggers out ---------------------------------------
-    strain_pin = torch.from_numpy(w.strain).pin_memory()
-    trig_pin = torch.empty(cap * 32, dtype=torch.uint8).pin_memory()
-    trig_np = trig_pin.numpy().view(lb.TRIGGER_DTYPE)
-    strain_np = strain_pin.numpy()
-    e2e_times, d2h = [], 0
-    for i in range(1 + args.steps):
-        lb.lloid_reset(bank.handle, stream)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        got, rc = bank.filter_host(strain_np, trig_np, stream)
-        dt = time.perf_counter() - t0
-        if i > 0:
-            e2e_times.append(dt)
-            d2h = 8 + 32 * min(got, cap)
-    t_e2e = torch.tensor([sum(e2e_times)], dtype=torch.float64, device="cuda")
+    extra = {}
     if world > 1:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    e2e_value = world * units * args.steps / float(t_e2e.item())
-
-    chunk = int(lb.lloid_chunk_samples(bank.handle))
-    dev_bytes = int(lb.lloid_device_bytes(bank.handle))
-    bank.close()
+        extra["config3_sharded"] = sharded_config3(args, rank, world, local)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     cpu_v, cpu_wall, cores, sample = oracle_sample(w, args.ref_seconds)
+    cpu_all = oracle_sample(w, args.ref_seconds, all_cores=True)
+    if world == 1 and args.extras and args.workload == "config2" and precision == lb.LLOID_F16:
+        extra.update(run_extras(args, w))
+    D = w.n_detectors
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": args.precision, "data": "synthetic",
             "config": {"workload": workload_name(args), "units": "templates x detectors x seconds of strain per detector",
                        "per_detector_template_s_per_s": value / D, "l2": "flushed between steps (512 MiB write)",
-                       "chunk_samples": chunk, "bank_device_bytes": dev_bytes, "triggers_per_step": n_trig,
-                       "parallelism": f"replica per rank x{world}"},
-            "clocks": clocks.summary(),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.strain.nbytes), "d2h_bytes_per_step": int(d2h)},
-            "gpu_launches": int(launches),
+                       "chunk_samples": r["chunk"], "bank_device_bytes": r["dev_bytes"], "triggers_per_step": r["n_trig"],
+                       "kernels": r["path"], "parallelism": f"replica per rank x{world}"},
+            "clocks": r["clocks"],
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"]},
+            "gpu_launches": int(r["launches"]),
             "roofline": roofline,
-            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "wall_s": cpu_wall},
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "wall_s": cpu_wall,
+                             "nproc": os.cpu_count(),
+                             "all_cores": {"value": cpu_all[0], "cores": cpu_all[2], "wall_s": cpu_all[1], "sample": cpu_all[3],
+                                           "per_core": cpu_all[0] / cpu_all[2]}},
+            "extra": extra,
             "context": "paper: up to 169x (A100, float16) over GstLAL on one EPYC 7313 core (PAPER.md:96)"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
+def sharded_config3(args, rank, world, local):
+    """N > 1: BASELINE config 3 (100 bins) with the bins sharded over the ranks (parallel.shard_bins, LPT), the same
+    strain on every rank, triggers gathered over NCCL (parallel.gather_triggers): strong scaling of one bank."""
+    import torch
+    import torch.distributed as dist
+    from paper_2410_16416_b200 import binding as lb, parallel as par, workloads as wl
+    w = wl.config3(seconds=256)
+    shards = par.shard_bins([par.bin_cost(b) for b in w.bins], world)
+    dist.barrier(); torch.cuda.synchronize()
+    r = time_bank(w, lb.LLOID_F16, 2, 1, 0, local, world, bins=shards[rank], want_e2e=True)
+    t = torch.tensor([sum(r["times"])], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    allt = par.gather_triggers(par.to_global_bins(r["last_triggers"], shards[rank]), device="cuda")
+    units = sum(b.n_templates for b in w.bins) * w.n_detectors * (w.n_samples / w.f0)
+    return {"workload": "BASELINE config 3, 100 bins sharded over the ranks, 2 det x 256 s", "scaling": "strong",
+            "value": units * 2 / (float(t.item()) * 1e-3), "unit": UNIT, "ms_per_step": float(t.item()) / 2,
+            "bins_per_rank": [len(s) for s in shards], "triggers_gathered": int(len(allt))}
+
+
+def run_extras(args, w2):
+    """Sub-results carried in the same JSON line (N = 1): the fp32 path on config 2, config 3 (100 bins batched), config 5
+    (1 s streaming buffers) and a reduced config 4 (full-bank geometry).  Each is a short run of the same library."""
+    import torch
+    from paper_2410_16416_b200 import binding as lb, workloads as wl
+    ex = {}
+    r = time_bank(w2, lb.LLOID_F32, 3, 1, 0, want_e2e=False)
+    ex["config2_fp32"] = {"value": r["units"] * 3 / (sum(r["times"]) * 1e-3), "unit": UNIT, "ms_per_step": sum(r["times"]) / 3, "steps": 3,
+                          "dtype": "f32", "stage_ms": stage_dict(r["stage_ms"]), "roofline": roofline_f32(w2, r["stage_ms"])}
+    w3 = wl.config3(seconds=2048)
+    r = time_bank(w3, lb.LLOID_F16, 3, 1, 0, want_e2e=False)
+    ex["config3_100bins"] = {"workload": "BASELINE config 3: 100 bins x 500 templates, 2 det x 2048 s", "value": r["units"] * 3 / (sum(r["times"]) * 1e-3),
+                             "unit": UNIT, "ms_per_step": sum(r["times"]) / 3, "steps": 3, "dtype": "f16", "stage_ms": stage_dict(r["stage_ms"]),
+                             "kernels": r["path"], "chunk_samples": r["chunk"]}
+    ex["config5_stream"] = stream_measure(wl.config3(seconds=600), lb.LLOID_F16, 0)
+    if args.extra_config4_bins > 0:
+        nb = args.extra_config4_bins
+        w4 = wl.config4(n_bins=nb, n_templates=1000, seconds=192, n_detectors=3, n_distinct=2)
+        r = time_bank(w4, lb.LLOID_F16, 2, 1, 0, want_e2e=False)
+        ex["config4_reduced"] = {"workload": f"BASELINE config 4 geometry: {nb} of 1000 bins x 1000 templates, L = 100 ... 300, 3 det x 192 s "
+                                             "(the full 1000-bin run is profiles/r2_bench_config4_1000bins.json)",
+                                 "value": r["units"] * 2 / (sum(r["times"]) * 1e-3), "unit": UNIT, "ms_per_step": sum(r["times"]) / 2, "steps": 2,
+                                 "dtype": "f16", "stage_ms": stage_dict(r["stage_ms"]), "kernels": r["path"], "chunk_samples": r["chunk"]}
+    return ex
+
+
+def stream_measure(w, precision, chunk):
+    """BASELINE config 5: 1 s buffers with history carried, back to back, stream-synchronised per call; per-buffer device
+    latency from CUDA events around each lloid_filter call.  The calls are replayed from ONE captured CUDA graph."""
+    import torch
+    from paper_2410_16416_b200 import binding as lb
+    secs = w.n_samples // w.f0
+    bank = lb.Bank(w, precision, max_chunk=chunk)
+    D, f0 = w.n_detectors, w.f0
+    n_templates = sum(b.n_templates for b in w.bins)
+    strain = torch.from_numpy(w.strain).cuda()
+    cap = n_templates * D * 2
+    trig = torch.empty(cap * 32, dtype=torch.uint8, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    buf = torch.empty((D, f0), dtype=torch.float32, device="cuda")           # the graph's fixed input buffer
+    side = torch.cuda.Stream()
+    graph = None
+    with torch.cuda.stream(side):
+        for i in range(min(8, secs)):                                        # warm-up calls (eager)
+            buf.copy_(strain[:, i * f0:(i + 1) * f0])
+            bank.filter(buf, trig, cnt, side.cuda_stream)
+        side.synchronize()
+        if lb.lloid_graph_safe(bank.handle, f0):
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                bank.filter(buf, trig, cnt, side.cuda_stream)
+        lb.lloid_reset(bank.handle, side.cuda_stream)
+        side.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(secs)]
+        n_trig = 0
+        with ClockSampler(0) as clocks:
+            t0 = time.perf_counter()
+            for i in range(secs):
+                buf.copy_(strain[:, i * f0:(i + 1) * f0])
+                ev[i][0].record(side)
+                if graph is not None:
+                    lb.lloid_graph_advance(bank.handle, f0)                  # host-side sample counter of the replayed call
+                    graph.replay()
+                else:
+                    bank.filter(buf, trig, cnt, side.cuda_stream)
+                ev[i][1].record(side)
+                ev[i][1].synchronize()                                       # a live search reads the count after every buffer
+                n_trig += int(cnt.item())
+            wall = time.perf_counter() - t0
+    lat = np.array([a.elapsed_time(b) for a, b in ev])
+    units = n_templates * D * secs
+    out = {"workload": f"BASELINE config 5 (config-3 bank: {len(w.bins)} bins x 500 templates, {D} det; {secs} x 1 s buffers, history carried)",
+           "value": units / (lat.sum() * 1e-3), "unit": UNIT, "ms_per_buffer": float(lat.mean()),
+           "latency_ms": {"p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)), "max": float(lat.max())},
+           "value_including_host_sync": units / wall, "triggers": n_trig, "cuda_graph": graph is not None,
+           "chunk_samples": int(lb.lloid_chunk_samples(bank.handle)), "launches_per_buffer": int(lb.lloid_last_launch_count(bank.handle)),
+           "clocks": clocks.summary()}
+    bank.close()
+    return out
+
+
 def run_stream(args):
-    """BASELINE config 5: the config-3 bank (100 BBH-like bins x 500 templates, 2 detectors) fed 1 s buffers with
-    history carried, back to back; per-buffer device latency (CUDA events around each lloid_filter call) and
-    throughput.  Not the default bench line (config 2 is); run with --workload config5."""
+    """--workload config5: the streaming line on its own."""
     import torch
     from paper_2410_16416_b200 import binding as lb, workloads as wl
     torch.cuda.set_device(0)
     secs = args.seconds if args.seconds != 4096 else 600
-    w = wl.config3(seconds=secs)
-    precision = lb.LLOID_F16 if args.precision == "f16" else lb.LLOID_F32
-    bank = lb.Bank(w, precision, max_chunk=args.chunk)
-    D, f0 = w.n_detectors, w.f0
-    n_templates = sum(b.n_templates for b in w.bins)
-    strain = torch.from_numpy(w.strain).cuda()
-    bufs = [strain[:, i * f0:(i + 1) * f0].contiguous() for i in range(secs)]
-    cap = n_templates * D * 2
-    trig = torch.empty(cap * 32, dtype=torch.uint8, device="cuda")
-    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
-    stream = torch.cuda.current_stream().cuda_stream
-    for i in range(min(8, secs)):                                  # warm-up calls
-        bank.filter(bufs[i], trig, cnt, stream)
-    lb.lloid_reset(bank.handle, stream)
-    torch.cuda.synchronize()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(secs)]
-    n_trig = 0
-    with ClockSampler(0) as clocks:
-        t0 = time.perf_counter()
-        for i in range(secs):
-            ev[i][0].record()
-            bank.filter(bufs[i], trig, cnt, stream)
-            ev[i][1].record()
-            ev[i][1].synchronize()                                 # stream-synchronised per call (a live search reads the count)
-            n_trig += int(cnt.item())
-        wall = time.perf_counter() - t0
-    lat = np.array([a.elapsed_time(b) for a, b in ev])
-    units = n_templates * D * secs
-    line = {"metric": METRIC, "value": units / (lat.sum() * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": secs, "warmup": 8,
-            "ms_per_step": float(lat.mean()), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": args.precision, "data": "synthetic",
-            "config": {"workload": f"BASELINE config 5 (config-3 bank: 100 bins x 500 templates, 2 det; {secs} x 1 s buffers, history carried)",
-                       "latency_ms": {"p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)), "max": float(lat.max())},
-                       "value_including_host_sync": units / wall, "triggers": n_trig,
-                       "chunk_samples": int(lb.lloid_chunk_samples(bank.handle)), "launches_per_buffer": int(lb.lloid_last_launch_count(bank.handle))},
-            "clocks": clocks.summary(), "gpu_launches": int(lb.lloid_last_launch_count(bank.handle)) * secs}
-    bank.close()
+    r = stream_measure(wl.config3(seconds=secs), lb.LLOID_F16 if args.precision == "f16" else lb.LLOID_F32, args.chunk)
+    line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": 1, "steps": secs, "warmup": 8, "ms_per_step": r["ms_per_buffer"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+            "config": {k: r[k] for k in ("workload", "latency_ms", "value_including_host_sync", "triggers", "cuda_graph", "chunk_samples", "launches_per_buffer")},
+            "clocks": r["clocks"], "gpu_launches": r["launches_per_buffer"] * secs}
     print(json.dumps(line), flush=True)
 
 
@@ -419,7 +544,18 @@ def main():
     ap.add_argument("--bins", type=int, default=100, help="number of SVD bins batched (--workload config3 / config4: full-bank geometry with heterogeneous L)")
     ap.add_argument("--chunk", type=int, default=0, help="library time-chunk length in samples (0 = automatic)")
     ap.add_argument("--ref-seconds", type=float, default=2.0, help="seconds of output the oracle sample covers")
+    ap.add_argument("--no-extras", dest="extras", action="store_false", help="skip the sub-results (fp32, config 3, 5, reduced 4) of the default line")
+    ap.add_argument("--extra-config4-bins", type=int, default=16, help="bins of the reduced config-4 sub-result (0: skip)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started as `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, NCCL), rank 0 prints the line
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = max(args.warmup, 1)
     if args.workload == "config5":

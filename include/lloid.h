@@ -21,8 +21,9 @@
  * gives a thread-local, library-owned, NUL-terminated message for the last failure on this thread.
  * "host" / "device" is stated for every pointer.  The library never takes ownership of caller
  * memory.  create / upload / finalize / destroy / reset are host-synchronous and not thread-safe
- * per handle.  lloid_filter only enqueues work on the given CUDA stream: it does not allocate, does
- * not synchronise the device and does not read device results on the host.
+ * per handle.  lloid_filter only enqueues work on the given CUDA stream: it does not allocate device memory,
+ * does not synchronise the device and does not read device results on the host (the first call with a new
+ * buffer length sorts one work list on the host and uploads it from pinned memory).
  * There is no CPU fallback: every entry point that needs the GPU fails with LLOID_ECUDA without one.
  */
 #ifndef LLOID_H
@@ -138,6 +139,17 @@ int lloid_bank_finalize(lloid_bank_t *bank);
 int lloid_filter(lloid_bank_t *bank, const float *strain_dev, int64_t n_samples,
                  lloid_trigger_t *triggers_dev, int64_t capacity, int64_t *n_triggers_dev,
                  void *cuda_stream);
+
+/* CUDA graphs (low-latency streaming, BASELINE config 5).  lloid_filter only enqueues work, so a call can be captured
+ * in a CUDA graph and replayed for every following buffer of the same length: the absolute sample index that triggers
+ * carry is read from device memory, which every call advances on the stream.  Conditions, checked by lloid_graph_safe
+ * (returns 1 / 0): n_samples and the number of samples consumed so far are multiples of peak_window (every call then
+ * makes the same host-side decisions).  Protocol: make at least one eager lloid_filter call with this n_samples (the
+ * first call with a new buffer length builds a work list on the host and is refused during capture); capture ONE call;
+ * before every replay call lloid_graph_advance(bank, n_samples), which keeps the host-side sample counter in step.
+ * The buffers captured (strain, triggers, count) are the ones every replay uses. */
+int lloid_graph_safe(const lloid_bank_t *bank, int64_t n_samples);
+int lloid_graph_advance(lloid_bank_t *bank, int64_t n_samples);
 
 /* Same call with HOST buffers (the end-to-end path): `strain_host` float32 [D][n_samples] is copied
  * to a library-owned device staging buffer, filtered, and the count plus min(count, capacity)

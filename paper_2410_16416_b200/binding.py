@@ -66,6 +66,8 @@ EXPORTS = {
     "lloid_last_launch_count": (C.c_int64, [C.c_void_p]),
     "lloid_device_bytes": (C.c_int64, [C.c_void_p]),
     "lloid_path_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_int32)]),
+    "lloid_graph_safe": (C.c_int, [C.c_void_p, C.c_int64]),
+    "lloid_graph_advance": (C.c_int, [C.c_void_p, C.c_int64]),
     "lloid_set_profiling": (C.c_int, [C.c_void_p, C.c_int32]),
     "lloid_last_stage_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
     "lloid_destroy": (None, [C.c_void_p]),
@@ -185,6 +187,14 @@ def lloid_last_launch_count(bank) -> int:
 
 def lloid_device_bytes(bank) -> int:
     return lib().lloid_device_bytes(bank)
+
+
+def lloid_graph_safe(bank, n_samples: int) -> bool:
+    return bool(lib().lloid_graph_safe(bank, n_samples))
+
+
+def lloid_graph_advance(bank, n_samples: int) -> None:
+    _check(lib().lloid_graph_advance(bank, n_samples))
 
 
 def lloid_path_info(bank) -> dict:

@@ -14,9 +14,15 @@ struct F16Plan {
   // persistent FIR (fir_f16_pers_kernel): unit lists per chunk length ([0]: the full chunk, [1]: the last one used)
   bool fir_pers = false;
   int fir_n_sm = 148, fir_hk_bytes = 0, fir_stage_cap = 0, fir_pers_stages = 0, fir_pers_smem = 0;
-  std::vector<int2> fir_list_host[2];
-  void* fir_list_dev[2] = {nullptr, nullptr};
-  int fir_list_c[2] = {-1, -1}, fir_list_n[2] = {0, 0};
+  // unit lists per chunk length: slot 0 = the full chunk (built at finalize), slots 1..3 = the last other lengths seen
+  // (tails, streaming buffers), least recently used replaced.  Host copies are PINNED, so the upload is a true async copy.
+  static constexpr int kFirSlots = 4;
+  int2* fir_list_pin[kFirSlots] = {nullptr, nullptr, nullptr, nullptr};
+  void* fir_list_dev[kFirSlots] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t fir_list_ev[kFirSlots] = {nullptr, nullptr, nullptr, nullptr};   // the slot's last upload
+  int fir_list_c[kFirSlots] = {-1, -1, -1, -1}, fir_list_n[kFirSlots] = {0, 0, 0, 0};
+  long long fir_list_use[kFirSlots] = {0, 0, 0, 0}, fir_tick = 0;
+  size_t fir_cap_units = 0;
   // A3-A5 on the tensor cores: low-rate reconstruction (lowrate_pair_kernel) + f0-rate kernel (f0_pair_kernel)
   bool tensor_recon = false;            // false: bank outside the kernels' limits -> CUDA-core fallback
   bool r_tmem = false;                  // reconstruction kernels keep the unit's stationary R in TMEM (K <= 512) instead of shared memory

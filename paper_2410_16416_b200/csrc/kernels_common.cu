@@ -210,7 +210,8 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128)
 merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
-                     int slots_cap, const int32_t* __restrict__ slot_tiles, int c, long long k_a, int W, float theta,
+                     int slots_cap, const int32_t* __restrict__ slot_tiles, int c, const long long* __restrict__ k_base, long long k_off,
+                     int W, float theta,
                      const PeakState* __restrict__ state_in, PeakState* __restrict__ state_out, int n_det,
                      lloid_trigger_t* __restrict__ trig, long long capacity, unsigned long long* __restrict__ count)
 {
@@ -218,6 +219,9 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
   const BinParams B = bp[bd];
   if (p >= B.n_templates) return;
+  // absolute index of the chunk's first sample: the call's first sample is read from DEVICE memory (advanced on the stream at
+  // the end of every lloid_filter call), so a call captured in a CUDA graph stamps the right times when it is replayed
+  const long long k_a = *k_base + k_off;
   const long long w_first = k_a / W, w_last = (k_a + c - 1) / W;
   const long long w = w_first + blockIdx.z;
   if (w > w_last) return;
@@ -259,17 +263,21 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
 }
 
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, int W, float theta,
+                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, const long long* k_base_dev, int64_t k_off,
+                          int W, float theta,
                           const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
                           unsigned long long* count, cudaStream_t st, int64_t* launches)
 {
-  const int n_w = (int)((k_a + c - 1) / W - k_a / W) + 1;
+  const int n_w = (int)((k_a + c - 1) / W - k_a / W) + 1;      // host copy of k_a: only the launch geometry depends on it
   dim3 grid((max_templates + 127) / 128, n_bd, n_w);
-  merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, slots_cap, slot_tiles_dev, c, (long long)k_a, W,
+  merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, slots_cap, slot_tiles_dev, c, k_base_dev, (long long)k_off, W,
                                             theta, state_in, state_out, n_det, (lloid_trigger_t*)triggers,
                                             (long long)capacity, count);
   ++*launches;
 }
+
+__global__ void advance_counter_kernel(long long* k_base, long long n) { *k_base += n; }
+void launch_advance_counter(long long* k_base_dev, int64_t n, cudaStream_t st) { advance_counter_kernel<<<1, 1, 0, st>>>(k_base_dev, (long long)n); }
 
 __global__ void reset_state_kernel(PeakState* s, long long n)
 {

@@ -433,10 +433,13 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const Slice
       cap_units += (size_t)(rows + 128 * mt - 1) / (128 * mt);
     }
     bool ok = set_max_dyn_smem(fir_f16_pers_kernel) == cudaSuccess;
-    for (int k = 0; k < 2 && ok; ++k) {
+    pl->fir_cap_units = cap_units;
+    for (int k = 0; k < F16Plan::kFirSlots && ok; ++k) {
       void* d = nullptr;
       ok = cudaMalloc(&d, (cap_units + 1) * sizeof(int2)) == cudaSuccess;
       if (ok) { pl->owned.push_back(d); pl->fir_list_dev[k] = d; pl->fir_list_c[k] = -1; *bytes += (int64_t)((cap_units + 1) * sizeof(int2)); }
+      if (ok) ok = cudaMallocHost((void**)&pl->fir_list_pin[k], (cap_units + 1) * sizeof(int2)) == cudaSuccess;
+      if (ok) ok = cudaEventCreateWithFlags(&pl->fir_list_ev[k], cudaEventDisableTiming) == cudaSuccess;
     }
     pl->fir_pers = ok;
   }
@@ -452,6 +455,10 @@ F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const Slice
 void f16_plan_destroy(F16Plan* p)
 {
   if (!p) return;
+  for (int k = 0; k < F16Plan::kFirSlots; ++k) {
+    if (p->fir_list_pin[k]) cudaFreeHost(p->fir_list_pin[k]);
+    if (p->fir_list_ev[k]) cudaEventDestroy(p->fir_list_ev[k]);
+  }
   for (void* q : p->owned) cudaFree(q);
   delete p;
 }
@@ -473,9 +480,10 @@ static int fir_build_list(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
   }
   std::stable_sort(ents.begin(), ents.end(), [](const Ent& a, const Ent& b) { return a.cost > b.cost; });
+  if (ents.size() > pl->fir_cap_units) return 1;
   const int G = std::min<int>(pl->fir_n_sm, (int)ents.size());
-  std::vector<int2>& L = pl->fir_list_host[slot];
-  L.resize(ents.size());
+  if (pl->fir_list_c[slot] >= 0) cudaEventSynchronize(pl->fir_list_ev[slot]);     // the slot's previous upload has left the pinned buffer
+  int2* L = pl->fir_list_pin[slot];
   const size_t full = ents.size() / G * G;                  // complete rounds are mirrored on odd rounds, the last partial one is not
   for (size_t i = 0; i < ents.size(); ++i) {
     const size_t round = i / G, j = i % G;
@@ -483,15 +491,28 @@ static int fir_build_list(F16Plan* pl, const SliceParams* sp_host, int n_problem
     L[pos] = make_int2(ents[i].p, ents[i].r);
   }
   pl->fir_list_c[slot] = c; pl->fir_list_n[slot] = (int)ents.size();
-  return cudaMemcpyAsync(pl->fir_list_dev[slot], L.data(), L.size() * sizeof(int2), cudaMemcpyHostToDevice, st) == cudaSuccess ? 0 : 1;
+  if (cudaMemcpyAsync(pl->fir_list_dev[slot], L, ents.size() * sizeof(int2), cudaMemcpyHostToDevice, st) != cudaSuccess) return 1;
+  cudaEventRecord(pl->fir_list_ev[slot], st);
+  return 0;
 }
 
 int launch_fir_f16(F16Plan* pl, const SliceParams* sp_dev, const SliceParams* sp_host, int n_problems,
                    const RateParams* rates_dev, int o, int c, cudaStream_t st, int64_t* launches)
 {
   if (pl->fir_pers) {
-    int slot = (c == pl->chunk_cap) ? 0 : 1;
-    if (pl->fir_list_c[slot] != c && fir_build_list(pl, sp_host, n_problems, c, slot, st)) return 1;
+    // the unit list of this chunk length: cached per length; building one (sort on the host + one async upload from pinned
+    // memory) happens the first time a length is seen and is refused while the stream is being captured into a CUDA graph
+    int slot = -1;
+    for (int k = 0; k < F16Plan::kFirSlots; ++k) if (pl->fir_list_c[k] == c) slot = k;
+    if (slot < 0) {
+      cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+      cudaStreamIsCapturing(st, &cs);
+      if (cs != cudaStreamCaptureStatusNone) { fprintf(stderr, "lloid: graph capture of a chunk length (%d) never filtered before: make one eager call first\n", c); return 1; }
+      slot = (c == pl->chunk_cap) ? 0 : 1;
+      if (slot) for (int k = 2; k < F16Plan::kFirSlots; ++k) if (pl->fir_list_use[k] < pl->fir_list_use[slot]) slot = k;
+      if (fir_build_list(pl, sp_host, n_problems, c, slot, st)) return 1;
+    }
+    pl->fir_list_use[slot] = ++pl->fir_tick;
     const int n_units = pl->fir_list_n[slot];
     const int grid = std::min(pl->fir_n_sm, n_units);
     fir_f16_pers_kernel<<<grid, FP_THREADS, pl->fir_pers_smem, st>>>(sp_dev, rates_dev, o, c, pl->fir_pers_stages,

@@ -84,6 +84,8 @@ struct lloid_bank {
   const float** upw_dev = nullptr;
   std::vector<void*> owned;
   int64_t consumed = 0, bytes = 0, last_launches = 0;
+  int64_t call_start = 0;                // absolute index of the current call's first sample (host copy)
+  long long* k_base_dev = nullptr;       // the same on the device: read by the merge kernel, advanced at the end of every call
   Capture cap{nullptr, 0, 0, -1, 0};
   float* stage_strain = nullptr; size_t stage_strain_elems = 0;
   lloid_trigger_t* stage_trig = nullptr; int64_t stage_trig_cap = 0;
@@ -285,7 +287,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
   mark(b, st, kTagRecon);
   if (int rc = debug_sync("reconstruction kernels", k_a, st)) return rc;
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
-  launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->slots_cap, b->slot_tiles_dev, c, k_a,
+  launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->slots_cap, b->slot_tiles_dev, c, k_a, b->k_base_dev, k_a - b->call_start,
                        b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
                        b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
   b->state_cur ^= 1;
@@ -614,6 +616,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
   rc = dev_alloc(b, (void**)&b->state, 2 * nstate * sizeof(PeakState), false); if (rc) return rc;
   rc = dev_alloc(b, (void**)&b->stage_count, 8, true); if (rc) return rc;
+  rc = dev_alloc(b, (void**)&b->k_base_dev, 8, true); if (rc) return rc;
   launch_reset_state(b->state, 2 * (int64_t)nstate, 0);
   CU(cudaDeviceSynchronize());
 
@@ -689,6 +692,7 @@ int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trig
   b->events_used = 0;
   CU(cudaMemsetAsync(count_dev, 0, 8, st));
   int64_t k = b->consumed, off = 0, rem = n;
+  b->call_start = k;
   while (rem > 0) {
     const int n_s = (int)std::min<int64_t>(rem, b->S);
     int rc = stage_superchunk(b, strain_dev + off, n, n_s, st);
@@ -704,7 +708,27 @@ int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trig
     }
     k += n_s; off += n_s; rem -= n_s;
   }
-  b->consumed = k;
+  launch_advance_counter(b->k_base_dev, n, st);
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(st, &cs);
+  if (cs == cudaStreamCaptureStatusNone) b->consumed = k;     // a captured call has not run: replays advance with lloid_graph_advance
+  return LLOID_OK;
+}
+
+int lloid_graph_safe(const lloid_bank_t* b, int64_t n)
+{
+  if (!b || !b->finalized || n <= 0) return 0;
+  const int64_t W = b->cfg.peak_window;
+  // every replay must make the same host-side decisions as the captured call: chunk boundaries, window counts and granule
+  // alignment depend on the running sample count modulo the peak window only
+  return (n % W == 0 && b->consumed % W == 0 && n % b->d_max == 0) ? 1 : 0;
+}
+
+int lloid_graph_advance(lloid_bank_t* b, int64_t n)
+{
+  if (!b || !b->finalized) return fail(LLOID_ESTATE, "graph_advance before finalize");
+  if (!lloid_graph_safe(b, n)) return fail(LLOID_EINVAL, "graph replay needs n_samples and the running sample count to be multiples of the peak window");
+  b->consumed += n;
   return LLOID_OK;
 }
 
@@ -750,6 +774,7 @@ int lloid_reset(lloid_bank_t* b, void* stream)
   cudaStream_t st = (cudaStream_t)stream;
   CU(cudaSetDevice(b->cfg.device));
   CU(cudaMemsetAsync(b->hist, 0, (size_t)b->cfg.n_detectors * b->H * 4, st));
+  CU(cudaMemsetAsync(b->k_base_dev, 0, 8, st));
   launch_reset_state(b->state, 2 * (int64_t)b->n_bd * b->max_templates, st);
   b->consumed = 0;
   return LLOID_OK;

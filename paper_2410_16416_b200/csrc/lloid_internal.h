@@ -126,9 +126,12 @@ void launch_recon_f32_q(const SliceParams* sp_dev, const BinParams* bp_dev, int 
 
 // partials: [bd][slot][template]; slot_tiles_dev[bd] = tiles per slot of that (bin, detector) (null: 1 everywhere)
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
-                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, int W, float theta,
+                          int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a /* host copy: launch geometry */,
+                          const long long* k_base_dev /* first sample of the call, device */, int64_t k_off /* chunk - call start */,
+                          int W, float theta,
                           const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
                           unsigned long long* count, cudaStream_t st, int64_t* launches);
+void launch_advance_counter(long long* k_base_dev, int64_t n, cudaStream_t st);
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
 

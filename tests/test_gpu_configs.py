@@ -174,3 +174,79 @@ def test_config5_one_second_buffers_equal_one_shot(precision):
     many, _, info = pu.run_gpu(w, precision, pieces=[w.f0] * 24)
     assert info["consumed"] == w.n_samples and len(info["counts"]) == 24
     assert _as_set(one) == _as_set(many) and len(one) > 0
+
+
+def test_config5_cuda_graph_replay_equals_one_shot():
+    """BASELINE config 5 through a CUDA graph: ONE captured 1 s-buffer lloid_filter call, replayed for every following
+    buffer (lloid_graph_safe / lloid_graph_advance), gives the triggers of the one-shot call."""
+    import torch
+    w = wl.config3(n_bins=12, n_templates=500, seconds=24, n_detectors=2, n_basis=64)
+    one, _, _ = pu.run_gpu(w, lb.LLOID_F16)
+    bank = lb.Bank(w, lb.LLOID_F16)
+    try:
+        f0, D = w.f0, w.n_detectors
+        cap = sum(b.n_templates for b in w.bins) * D * 2
+        strain = torch.from_numpy(w.strain).cuda()
+        buf = torch.empty((D, f0), dtype=torch.float32, device="cuda")
+        trig = torch.zeros(cap * 32, dtype=torch.uint8, device="cuda")
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        side = torch.cuda.Stream()
+        out = []
+        with torch.cuda.stream(side):
+            # buffer 0 eagerly (builds the work list of this buffer length), then capture a call and replay it 23 times
+            buf.copy_(strain[:, :f0])
+            bank.filter(buf, trig, cnt, side.cuda_stream)
+            side.synchronize()
+            out.append(trig.cpu().numpy().view(lb.TRIGGER_DTYPE)[:int(cnt.item())].copy())
+            assert lb.lloid_graph_safe(bank.handle, f0) and not lb.lloid_graph_safe(bank.handle, f0 // 2)
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                bank.filter(buf, trig, cnt, side.cuda_stream)
+            assert lb.lloid_samples_consumed(bank.handle) == f0          # the captured call has not run
+            for i in range(1, 24):
+                buf.copy_(strain[:, i * f0:(i + 1) * f0])
+                lb.lloid_graph_advance(bank.handle, f0)
+                g.replay()
+                side.synchronize()
+                out.append(trig.cpu().numpy().view(lb.TRIGGER_DTYPE)[:int(cnt.item())].copy())
+        assert lb.lloid_samples_consumed(bank.handle) == 24 * f0
+        many = np.concatenate(out)
+        assert _as_set(one) == _as_set(many) and len(one) > 0
+    finally:
+        bank.close()
+
+
+def test_two_banks_alive_and_interleaved_precisions():
+    """Opt-in shared memory is a per-device function attribute: a large fp16 bank must keep working while a small bank and
+    an fp32 bank are created and used next to it."""
+    import torch
+    big = wl.config2(n_templates=120, seconds=72, n_detectors=2, n_basis=150, n_injections=0)
+    small = wl.toy(n_templates=5, M=1024, spans=((2048, 0.0, 0.125), (512, 0.125, 0.5)), seconds=2.0, n_basis=[7, 9], f_low=40.0)
+    ref_big, _, _ = pu.run_gpu(big, lb.LLOID_F16)
+    ref_small16, _, _ = pu.run_gpu(small, lb.LLOID_F16)
+    ref_small32, _, _ = pu.run_gpu(small, lb.LLOID_F32)
+
+    def run(bank, w):
+        n = w.n_samples
+        cap = sum(b.n_templates for b in w.bins) * w.n_detectors * (n // w.peak_window + 1) + 16
+        strain = torch.from_numpy(w.strain).cuda()
+        trig = torch.zeros(cap * 32, dtype=torch.uint8, device="cuda")
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        lb.lloid_reset(bank.handle)
+        bank.filter(strain, trig, cnt)
+        torch.cuda.synchronize()
+        return trig.cpu().numpy().view(lb.TRIGGER_DTYPE)[:int(cnt.item())].copy()
+
+    b_big = lb.Bank(big, lb.LLOID_F16)
+    try:
+        b_s16 = lb.Bank(small, lb.LLOID_F16)        # created while the large bank is alive
+        b_s32 = lb.Bank(small, lb.LLOID_F32)
+        try:
+            for _ in range(2):                      # interleaved
+                assert _as_set(run(b_s16, small)) == _as_set(ref_small16)
+                assert _as_set(run(b_big, big)) == _as_set(ref_big)
+                assert _as_set(run(b_s32, small)) == _as_set(ref_small32)
+        finally:
+            b_s16.close(); b_s32.close()
+    finally:
+        b_big.close()

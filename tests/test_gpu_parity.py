@@ -56,6 +56,17 @@ def test_toy_banks_dense_and_triggers(name, precision):
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
+def test_one_tile_windows_and_chunks(precision):
+    """peak_window = 128 and max_chunk = 128: one tile per window, per chunk and per partial-peak granule (the smallest values
+    include/lloid.h allows)."""
+    w = wl.toy(**TOYS["two_rates"])
+    w.peak_window = 128
+    n = w.n_samples
+    _, _, _, info, stats = _dense_check(w, precision, 0, n, max_chunk=128)
+    assert info["chunk"] == 128 and stats["checked"] == w.bins[0].n_templates * (n // 128)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
 def test_config1_dense_snr_and_triggers(cfg1, precision):
     """BASELINE config 1 in full: 16 s, 64 templates, 2 slices, L = 32, injection at k = 19209."""
     w = cfg1
