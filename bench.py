@@ -37,6 +37,14 @@ METRIC = "template_seconds_of_strain_filtered_per_second"
 UNIT = "template*s/s"
 
 
+_T0 = time.time()
+
+
+def note(msg):
+    """Progress to stderr (stdout carries the one JSON line only)."""
+    print(f"[bench {time.time() - _T0:7.1f} s] {msg}", file=sys.stderr, flush=True)
+
+
 # ------------------------------------------------------------------------------------------------
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -113,9 +121,13 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------
+_ORACLE_W = None          # the workload of the oracle legs: forked workers inherit it (pickling 1000 bins per job would copy them)
+
+
 def _oracle_stretch(args):
     """One oracle call: bin 0, detector 0, output samples [k0, k1).  Module-level so that a process pool can run it."""
-    w, k0, k1 = args
+    k0, k1 = args
+    w = _ORACLE_W
     from oracle import lloid_oracle as oc
     b = w.bins[0]
     rho = oc.snr_series(w.strain[0].astype(np.float64), b.slices, b.basis, b.recon, k0, k1, w.k_down, w.k_up)
@@ -135,7 +147,9 @@ def oracle_sample(w, seconds: float, all_cores: bool = False):
     n_proc = 1
     if all_cores:
         n_proc = max(1, min(os.cpu_count() or 1, (w.n_samples - k0) // span))
-    jobs = [(w, k0 + i * span, k0 + (i + 1) * span) for i in range(n_proc)]
+    global _ORACLE_W
+    _ORACLE_W = w
+    jobs = [(k0 + i * span, k0 + (i + 1) * span) for i in range(n_proc)]
     with threadpool_limits(1):
         t0 = time.perf_counter()
         if n_proc == 1:
@@ -206,11 +220,15 @@ def time_bank(w, precision, steps, warmup, chunk, local=0, world=1, bins=None, w
     this rank's (the caller takes the max over ranks)."""
     import torch
     from paper_2410_16416_b200 import binding as lb
+    note(f"uploading {len(w.bins) if bins is None else len(bins)} bins")
     bank = lb.Bank(w, precision, device=local, max_chunk=chunk, bins=bins)
+    note(f"bank resident: {lb.lloid_device_bytes(bank.handle) / 2**30:.2f} GiB, chunk {lb.lloid_chunk_samples(bank.handle)} samples")
     n, D = w.n_samples, w.n_detectors
     ids = bank.bin_ids
     n_templates = sum(w.bins[b].n_templates for b in ids)
     cap = n_templates * D * (n // w.peak_window + 1)
+    if cap * 32 > (4 << 30):                         # full-bank runs: room for a 0.35 trigger rate (0.11 measured); overflow is reported
+        cap = int(0.35 * cap)
     strain_dev = torch.from_numpy(w.strain).cuda()
     trig_dev = torch.empty(cap * 32, dtype=torch.uint8, device="cuda")
     cnt_dev = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -246,6 +264,7 @@ def time_bank(w, precision, steps, warmup, chunk, local=0, world=1, bins=None, w
     out["clocks"] = clocks.summary()
     out["stage_ms"] = stage_sum / steps              # resample, FIR, recon (both kernels), merge, whole call, low-rate kernel
     out["n_trig"] = int(cnt_dev.item())
+    out["trigger_capacity"] = int(cap)
     out["units"] = n_templates * D * (n / w.f0)      # template * detector * seconds of strain per step, this rank
     out["chunk"] = int(lb.lloid_chunk_samples(bank.handle))
     out["dev_bytes"] = int(lb.lloid_device_bytes(bank.handle))
@@ -364,7 +383,9 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    w = make_workload(args, rank)                         # weak scaling: one replica of the workload per rank, own noise
+    note("generating the workload")
+    w = make_workload(args, rank)
+    note("workload ready")                         # weak scaling: one replica of the workload per rank, own noise
     barrier()
     r = time_bank(w, precision, args.steps, args.warmup, args.chunk, local, world)
     barrier()
@@ -387,8 +408,10 @@ def run_ours(args):
         if world > 1:
             dist.destroy_process_group()
         return
+    note("device and e2e legs done; oracle legs")
     cpu_v, cpu_wall, cores, sample = oracle_sample(w, args.ref_seconds)
     cpu_all = oracle_sample(w, args.ref_seconds, all_cores=True)
+    note("oracle legs done")
     if world == 1 and args.extras and args.workload == "config2" and precision == lb.LLOID_F16:
         extra.update(run_extras(args, w))
     D = w.n_detectors

@@ -135,7 +135,12 @@ int lloid_bank_finalize(lloid_bank_t *bank);
  * the running in-window peak of every template and the absolute sample counter are carried, so
  * feeding a stream in pieces gives the same triggers as feeding it at once (A8, BASELINE config 5).
  * Only windows completed by this call emit triggers.  Asynchronous; the strain buffer must stay
- * valid until the stream has finished the call.  Errors: LLOID_EINVAL, LLOID_ESTATE, LLOID_ECUDA. */
+ * valid until the stream has finished the call.  Errors: LLOID_EINVAL, LLOID_ESTATE, LLOID_ECUDA.
+ * The strain must be FINITE and is not checked: a NaN or Inf sample makes every SNR value whose filter
+ * span covers it non-finite, a non-finite |rho|^2 never wins the peak comparison, so the templates of
+ * that detector emit no trigger until the sample has left the carried history (H samples, about the
+ * template length).  Remove such samples first (the pipeline's gating step, "conditioned
+ * data": outside this path); the fp16 path additionally needs |x^s| < 65504 after the sqrt(d) gain. */
 int lloid_filter(lloid_bank_t *bank, const float *strain_dev, int64_t n_samples,
                  lloid_trigger_t *triggers_dev, int64_t capacity, int64_t *n_triggers_dev,
                  void *cuda_stream);

@@ -264,6 +264,66 @@ def test_injection_recovered_at_injected_snr_and_time(phase):
     assert abs(math.hypot(ex[0, 3], ex[1, 3]) - A) < 1e-5
 
 
+def _eight_slice_bin(mc_lo, mc_hi, n, L):
+    return wl.make_bin(np.linspace(mc_lo, mc_hi, n), 131072, 15.0, 1024.0, wl.CONFIG2_SPANS, L)
+
+
+@pytest.mark.parametrize("phase", [0.0, 1.0])
+def test_injection_recovered_on_eight_slice_bank(phase):
+    """P6 on config 2's geometry (8 slices, d = 1 ... 32, M = 131072) with chirp masses whose frequency stays
+    below 0.75 of every slice's Nyquist (Mc 2.0-2.1: 23 Hz at tau = 48 s against 32 Hz), so the resamplers are in
+    their pass band and the noise-free peak is A times the retained power, at exactly k = e."""
+    b = _eight_slice_bin(2.0, 2.1, 48, 16)
+    p, A, e = 29, 12.0, 131072 + 40019                     # e is off every decimation grid
+    x = wl.make_strain(0, 1, 2 * 131072 + 65536, [b], [wl.Injection(0, p, A, phase, e)], 15.0, 1024.0, noise=False)[0]
+    rho = oc.snr_series(x.astype(np.float64), b.slices, b.basis, b.recon, e - 200, e + 200, KD, KU)
+    q = rho[0::2] ** 2 + rho[1::2] ** 2
+    assert np.argmax(q[p]) + e - 200 == e
+    kc = sum(np.sum(R[2 * p] ** 2) for R in b.recon)
+    ks = sum(np.sum(R[2 * p + 1] ** 2) for R in b.recon)
+    kx = sum(np.sum(R[2 * p] * R[2 * p + 1]) for R in b.recon)      # cos/sin rows are not exactly orthogonal
+    assert 0.5 < kc < 0.97 and 0.5 < ks < 0.97                      # L = 16 truncates for real
+    assert abs(rho[2 * p, 200] - A * (math.cos(phase) * kc + math.sin(phase) * kx)) < 0.003 * A
+    assert abs(rho[2 * p + 1, 200] - A * (math.sin(phase) * ks + math.cos(phase) * kx)) < 0.003 * A
+    # a neighbouring template responds with the truncated overlap  sum_s R_p'. R_p  (U^s orthonormal)
+    p2 = p + 3
+    o = sum(np.sum(R[2 * p2] * (math.cos(phase) * R[2 * p] + math.sin(phase) * R[2 * p + 1])) for R in b.recon)
+    assert abs(rho[2 * p2, 200] - A * o) < 0.003 * A
+
+
+def _taps_gain(d, K, f):
+    lp = oc.lowpass_taps(d, K)
+    i = np.arange(len(lp)) - K * d
+    return np.sum(lp[None, :] * np.cos(2 * np.pi * f[:, None] * i[None, :]), axis=1)
+
+
+def test_config2_band_loses_power_in_its_64_hz_slice():
+    """Config 2's own chirp masses (1.1-1.3) sweep 28-33 Hz inside the 64 Hz slice: the noise-free
+    peak is A kappa times the resamplers' gain there.  Stationary phase predicts the gain: the power-weighted mean
+    (weight tau^-1/2) of H_down(f(tau)) H_up(f(tau)) over the support; good to a few per cent at the band edge."""
+    b = _eight_slice_bin(1.18, 1.22, 32, 64)
+    p, A, e = 17, 12.0, 131072 + 40019
+    x = wl.make_strain(0, 1, 2 * 131072 + 65536, [b], [wl.Injection(0, p, A, 0.0, e)], 15.0, 1024.0, noise=False)[0]
+    rho = oc.snr_series(x.astype(np.float64), b.slices, b.basis, b.recon, e - 8, e + 8, KD, KU)
+    q = rho[0::2] ** 2 + rho[1::2] ** 2
+    assert np.argmax(q[p]) == 8
+    kc = sum(np.sum(R[2 * p] ** 2) for R in b.recon)
+    assert abs(kc - 1.0) < 1e-3                                     # L = 64 keeps the whole narrow bank
+    a_c = wl.chirp_coefficient(np.array([b.mchirp[p]]))[0]
+    tau_end, tau_start = (a_c / 1024.0) ** (8 / 3), min(64.0, (a_c / 15.0) ** (8 / 3))
+    num = den = 0.0
+    for rate, tlo, thi in wl.CONFIG2_SPANS:
+        d = wl.F0 // rate
+        t = np.linspace(max(tlo, tau_end), min(thi, tau_start), 4001)
+        f = a_c * t ** (-3 / 8) / wl.F0
+        g = np.ones_like(t) if d == 1 else _taps_gain(d, KD, f) * _taps_gain(d, KU, f)
+        w = t ** -0.5
+        num += np.sum(0.5 * (w[1:] * g[1:] + w[:-1] * g[:-1]) * np.diff(t))
+        den += np.sum(0.5 * (w[1:] + w[:-1]) * np.diff(t))
+    got = rho[2 * p, 8] / A
+    assert 0.90 < got < 0.96 and abs(got - num / den) < 0.035, (got, num / den)
+
+
 # ---------------------------------------------------------------------------------- P7: white-noise normalisation
 def test_white_noise_snr_is_chi2_two_dof():
     b = wl.make_bin(np.linspace(1.20, 1.25, 64), 8192, 30.0, 1024.0, wl.CONFIG1_SPANS, 32)
