@@ -31,6 +31,7 @@ struct F16Plan {
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
   int f0_smem = 0, f0_stages = 0, f0_ystage = 0, low_ystage = 0;   // ystage: bytes of a y ring slot per CTA
+  int ycap = 8;                         // MMAs per y stage at most (K = 16 each)
   PairMma tab[kPairTabMax];             // interpolation MMA table of the f0 kernel (kernel parameter)
   int n_tab = 0;
   int p_bytes = 0, q_bytes = 0, l_sum_f0_max = 0, l_sum_low_max = 0;   // per CTA: band-matrix blob, rho^(d) window buffers

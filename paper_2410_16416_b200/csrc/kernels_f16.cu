@@ -153,10 +153,9 @@ fir_f16_kernel(const SliceParams* __restrict__ sp, const RateParams* __restrict_
     mbar_wait(smem_u32(&bar_acc), 0);
     fence_after();
     __half* __restrict__ Y = reinterpret_cast<__half*>(P.Y);
-    const size_t lgs = (size_t)(L_pad >> 3);
     for (int mt = 0; mt < mt_used; ++mt) {
       const int row = (r0 + mt * 128 + q * 32 + lane) * P.out_mul + P.out_add;           // folded slice: phase rows interleave
-      __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
+      __half* __restrict__ Yt = reinterpret_cast<__half*>(reinterpret_cast<char*>(Y) + (size_t)(row >> 6) * P.y_step64) + (row & 63) * 8;   // Y16[64-row tile][slice][lc][row % 64][8]
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
       for (int c0 = 0; c0 < L_pad; c0 += 16) {
         uint32_t v[16];
@@ -347,14 +346,13 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
       if (!U.valid) continue;
       const SliceParams* P = sp + U.p;
       __half* __restrict__ Y = reinterpret_cast<__half*>(P->Y);
-      const int y_rows_cap = P->y_rows_cap;
+      const int y_rows_cap = P->y_rows_cap, y_step64 = P->y_step64;
       const int L_pad = U.L_pad;
-      const size_t lgs = (size_t)(L_pad >> 3);
-      mbar_wait(smem_u32(&acc_full), (uint32_t)k & 1u);
+        mbar_wait(smem_u32(&acc_full), (uint32_t)k & 1u);
       fence_after();
       for (int mt = 0; mt < U.mt_used; ++mt) {
         const int row = (U.r0 + mt * 128 + q * 32 + lane) * P->out_mul + P->out_add;       // folded slice: phase rows interleave
-        __half* __restrict__ Yt = Y + ((size_t)(row >> 6) * lgs * 64 + (row & 63)) * 8;     // Y16[64-row tile][lc][row % 64][8]
+        __half* __restrict__ Yt = reinterpret_cast<__half*>(reinterpret_cast<char*>(Y) + (size_t)(row >> 6) * y_step64) + (row & 63) * 8;   // Y16[64-row tile][slice][lc][row % 64][8]
         const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(mt * L_pad);
         for (int c0 = 0; c0 < L_pad; c0 += 32) {
           uint32_t v[32];

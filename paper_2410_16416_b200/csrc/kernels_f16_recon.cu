@@ -40,7 +40,8 @@ namespace lloid {
 
 using namespace tc;
 
-constexpr int PK_THREADS = 544;             // 17 warps: 0 PY, 1 IY, 2 PQ0, 3 IQ0, 4 relay y, 5 relay q, 6 PQ1, 8-15 epilogue, 16 IQ1
+constexpr int PK_THREADS = 512;             // 16 warps (4 per scheduler: 128 registers per thread): 0 PY, 1 IY (leader), 2 PQ0, 3 IQ0 (leader),
+                                            // 4 relay y (peer), 5 IQ1 (leader) / relay q (peer), 6 PQ1, 7 L2 prefetcher, 8-15 epilogue
 constexpr int PK_NSY_MAX = 16;
 constexpr int PK_NACC_MAX = 4;              // accumulator buffers of 128 columns: 4 with R in shared memory, 2 with R in TMEM
 constexpr int PK_ACOL = 256;                // R in TMEM: columns [256, 256 + K / 2) beside two accumulators
@@ -56,24 +57,29 @@ constexpr int PK_NQB = 4;                   // rho^(d) tile events in flight (ba
 constexpr int PK_QDIST = 2;                 // the rows of tile e are requested when tile e - PK_QDIST has been consumed
 constexpr int PK_QPF = 4;                   // L2 prefetch distance of the rho^(d) rows, in tiles
 constexpr int PK_YPF = 4;                   // L2 prefetch distance of the y tiles, in tiles
-constexpr int PK_BLOCK_TILES = 64;          // f0 schedule: the template blocks of a (bin, detector) walk the time axis in blocks of
-                                            // this many tiles, one after the other, so the CTA pairs that share a y tile read it
-                                            // while it is L2-hot (measured before: 2.75 GB of DRAM reads per launch for 1.1 GB of operands)
 constexpr int PK_SMEM_BUDGET = 218 * 1024;  // dynamic; + static (barriers, tables) stays below 227 KB
 
 struct LowUnit { int32_t group, pb; };
 
 // Role trace (scratch builds with -DLLOID_TRACE_BUILD and LLOID_TRACE=1): cycles each single-thread role of cluster 0
 // spends waiting on each of its barriers and in total, accumulated over the launches; read back with lloid_debug_trace.
-__device__ long long g_trace[2][8][8];      // [kernel: 0 low, 1 f0][role][0..5 wait categories, 6 total, 7 tiles]
+__device__ long long g_trace[2][8][8];
+#ifdef LLOID_TRACE_BUILD
+__constant__ int g_exp;                      // scratch knock-outs: 1 no interpolation MMAs, 2 no y MMAs (f0), 4 no epilogue arithmetic (f0)
+__constant__ int g_fake_half_r;            // scratch experiment: f0 kernel keeps only the first slice's R in shared memory (wrong sums, same work)
+#endif      // [kernel: 0 low, 1 f0][role][0..5 wait categories, 6 total, 7 tiles]
 #ifdef LLOID_TRACE_BUILD
 #define TWAIT(cat, bar, ph)                                                                       \
   do { if (trace) { const long long t_ = clock64(); mbar_wait(bar, ph); tw[cat] += clock64() - t_; } else mbar_wait(bar, ph); } while (0)
 #define TRACE_BEGIN() const bool trace = a.trace && (blockIdx.x >> 1) == 0; long long tw[6] = {0, 0, 0, 0, 0, 0}; const long long tbeg = trace ? clock64() : 0
+#define TSPAN_BEGIN() const long long ts_ = trace ? clock64() : 0
+#define TSPAN_END(cat) do { if (trace) tw[cat] += clock64() - ts_; } while (0)
 #define TRACE_END(kern, role, ntiles) do { if (trace) { for (int i_ = 0; i_ < 6; ++i_) g_trace[kern][role][i_] += tw[i_]; g_trace[kern][role][6] += clock64() - tbeg; g_trace[kern][role][7] += (ntiles); } } while (0)
 #else
 #define TWAIT(cat, bar, ph) mbar_wait(bar, ph)
 #define TRACE_BEGIN() constexpr bool trace = false; long long* const tw = nullptr; (void)trace; (void)tw
+#define TSPAN_BEGIN() do { } while (0)
+#define TSPAN_END(cat) do { } while (0)
 #define TRACE_END(kern, role, ntiles) do { (void)(ntiles); } while (0)
 #endif
 
@@ -83,8 +89,8 @@ __device__ long long g_trace[2][8][8];      // [kernel: 0 low, 1 f0][role][0..5 
 // instruction count -- y stages carry up to K = 128, barrier addresses are hoisted, the interpolation MMAs read their
 // operands from a table in the kernel parameters -- and the two MMA-issuing roles exist TWICE, one thread for the even
 // tiles and one for the odd tiles (different accumulators, so the pipe needs no ordering between them).
-struct YRing {                              // y ring position: slot index + phase parity
-  uint32_t s, ph, n;
+struct YRing {                              // y ring position: slot index + phase parity (+ tiles started: PY only)
+  uint32_t s, ph, n, tiles = 0;
   __device__ __forceinline__ void advance() { if (++s == n) { s = 0; ph ^= 1u; } }
   __device__ __forceinline__ void skip(uint32_t k) { s += k; while (s >= n) { s -= n; ph ^= 1u; } }
 };
@@ -201,6 +207,7 @@ struct PairBars {
   uint64_t qfull[PK_NQB], qempty[PK_NQB];
   uint64_t acc_full[PK_NACC_MAX], acc_empty[PK_NACC_MAX], ybar[PK_NACC_MAX];
   uint64_t consts, unit_done, r_ready;
+  uint32_t py_tiles, pad_;                  // tiles the PY thread has started (read by the L2 prefetcher)
 };
 
 // Barrier counts: a "full" barrier of the leader gets its own producers' arrive.expect_tx plus the peer's relay, the peer's
@@ -210,6 +217,7 @@ __device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int
 {
   if (warp == 0) tmem_alloc2(tmem_slot, 512);
   if (tid == 32) {
+    B.py_tiles = 0u;
     const uint32_t relay = rank == 0 ? 1u : 0u;
     for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), 1u + relay); mbar_init(smem_u32(&B.yempty[s]), 1); }
     for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), n_pq + relay); mbar_init(smem_u32(&B.qempty[s]), 1); }
@@ -236,7 +244,7 @@ __device__ __forceinline__ void pair_teardown(uint32_t tmem, int warp)
 }
 
 // y stages of a slice with nm = L_pad / 16 MMAs per tile: ceil(nm / 8) stages of nearly equal size (<= 8 MMAs, K <= 128)
-__host__ __device__ inline int stage_count(int nm) { return (nm + 7) >> 3; }
+__host__ __device__ inline int stage_count(int nm, int cap) { return (nm + cap - 1) / cap; }
 
 // m back-to-back MMAs of one y stage: D (+)= R[l-groups from a_lo] * stage^T, N = 128.  a_lo: descriptor of R at this K
 // offset (LBO 2048: 128 rows per l-group, 256 sixteen-byte units per K = 16); b_lo: the stage (LBO 1024: 64 rows, 128 units)
@@ -254,27 +262,32 @@ __device__ __forceinline__ void mma_y_stage(uint32_t d_tmem, uint32_t a_lo, uint
 
 // ------------------------------------------------------------------------------------------------
 struct SegSrc {                             // per-role copy of the current unit's operand sources (this CTA's halves)
-  const uint8_t* Y[kMaxGroupSlices];        // slice's Y16 base
+  const uint8_t* Y0;                        // Y16 record of the unit's rate group: 64-row tile 0 (lloid_api.cu: the slices' y lie side by side)
   const uint8_t* Rsrc[kMaxGroupSlices];     // this CTA's 128-row block of the slice's R16
   int nm[kMaxGroupSlices];                  // L_pad / 16
-  int nst[kMaxGroupSlices], mbase[kMaxGroupSlices], ext[kMaxGroupSlices];   // stages per tile; MMAs per stage: mbase (+ 1 for the first ext)
   int n, stages_per_tile;
-  uint32_t rbytes;
+  uint32_t rbytes, ystep;                   // bytes of the unit's R block; bytes from one 64-row y tile to the next
+  uint64_t mlist;                           // MMAs per stage minus one, 4 bits per stage, in the order of the tile's stages (<= 16)
 };
 
-__device__ __forceinline__ void seg_fill(SegSrc& S, const SliceParams* __restrict__ sp, const int32_t* slice, int n, int rb)
+// The K = sum L_pad of a unit is one contiguous operand (y record in HBM, R in shared memory / TMEM), cut into
+// ceil(nm / ycap) stages of nearly equal size whatever the slice boundaries.
+__device__ __forceinline__ void seg_fill(SegSrc& S, const SliceParams* __restrict__ sp, const int32_t* slice, int n, int rb, int ycap)
 {
-  S.n = n; S.stages_per_tile = 0; S.rbytes = 0;
+  S.n = n; S.rbytes = 0; S.mlist = 0;
+  int nm_all = 0;
   for (int i = 0; i < n; ++i) {             // one thread
     const SliceParams* P = sp + slice[i];
     const int L = P->L_pad;
-    S.Y[i] = reinterpret_cast<const uint8_t*>(P->Y);
+    if (i == 0) { S.Y0 = reinterpret_cast<const uint8_t*>(P->Y); S.ystep = (uint32_t)P->y_step64; }
     S.Rsrc[i] = reinterpret_cast<const uint8_t*>(P->R16) + (size_t)rb * L * 256;
     S.nm[i] = L >> 4;
-    S.nst[i] = stage_count(L >> 4); S.mbase[i] = (L >> 4) / S.nst[i]; S.ext[i] = (L >> 4) - S.mbase[i] * S.nst[i];
-    S.stages_per_tile += S.nst[i];
+    nm_all += L >> 4;
     S.rbytes += (uint32_t)L * 256u;
   }
+  const int nst = stage_count(nm_all, ycap), base = nm_all / nst, ext = nm_all - base * nst;
+  for (int j = 0; j < nst; ++j) S.mlist |= (uint64_t)(base + (j < ext ? 1 : 0) - 1) << (4 * j);
+  S.stages_per_tile = nst;
 }
 
 struct YAddr { uint32_t full0, empty0, dst0, step; };   // barrier arrays and slots of the y ring (dst: address, or descriptor for IY)
@@ -284,7 +297,7 @@ struct YAddr { uint32_t full0, empty0, dst0, step; };   // barrier arrays and sl
 // while the previous unit drains.  extra/extra_bytes: loaded once with the first R (the f0 kernel's band matrices).
 // RT (R in TMEM, loaded by the epilogue warps): only the band matrices go out, with the first unit.
 template <bool RT>
-__device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i, const SegSrc& sg, uint32_t consts_u, uint32_t unit_done_u, uint32_t sR_u,
+__device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i, const SegSrc& sg, uint32_t consts_u, uint32_t unit_done_u, uint32_t sR_u, uint32_t progress_u,
                                            uint32_t rank, int t0, int t1, uint32_t extra_dst, const uint8_t* extra, uint32_t extra_bytes,
                                            bool trace, long long* tw)
 {
@@ -299,9 +312,16 @@ __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i
   }
   auto load_R = [&]() {
     if (seg_i > 0) TWAIT(1, unit_done_u, (uint32_t)(seg_i - 1) & 1u);   // every MMA that reads the old R is complete
+#ifdef LLOID_TRACE_BUILD
+    const bool fake = g_fake_half_r && extra_dst != 0u;
+    const int n_r = fake ? 1 : sg.n;
+    mbar_expect_tx(consts_u, (fake ? (uint32_t)sg.nm[0] * 4096u : sg.rbytes) + (seg_i == 0 ? extra_bytes : 0u));
+#else
+    const int n_r = sg.n;
     mbar_expect_tx(consts_u, sg.rbytes + (seg_i == 0 ? extra_bytes : 0u));
+#endif
     uint32_t off = 0;
-    for (int i = 0; i < sg.n; ++i) {
+    for (int i = 0; i < n_r; ++i) {
       copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.nm[i] * 4096u, consts_u);
       off += (uint32_t)sg.nm[i] * 4096u;
     }
@@ -309,22 +329,25 @@ __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i
     need_R = false;
   };
   if (need_R && pre == 0) load_R();
-  for (int t = t0; t < t1; ++t)
-    for (int i = 0; i < sg.n; ++i) {
-      const int nm = sg.nm[i], nst = sg.nst[i], base = sg.mbase[i], ext = sg.ext[i];
-      const uint8_t* src = sg.Y[i] + (size_t)(2 * t + (int)rank) * nm * 2048;    // 64-row tiles are contiguous in Y16: nm x 2 KB each
-      if (t + PK_YPF < t1) bulk_prefetch_l2(src + (size_t)(2 * PK_YPF) * nm * 2048, (uint32_t)nm * 2048u);   // this CTA's half of tile t + PK_YPF
-      for (int j = 0; j < nst; ++j) {
-        const uint32_t bytes = (uint32_t)(base + (j < ext ? 1 : 0)) * 2048u;
-        const uint32_t full = ya.full0 + 8u * rg.s;
-        TWAIT(0, ya.empty0 + 8u * rg.s, rg.ph ^ 1u);
-        mbar_expect_tx(full, bytes);
-        bulk_g2s(ya.dst0 + rg.s * ya.step, src, bytes, full);
-        rg.advance();
-        src += bytes;
-        if (need_R && --pre == 0) load_R();
-      }
+  const uint32_t step2 = 2u * sg.ystep;
+  const uint64_t mlist = sg.mlist;
+  const int nst = sg.stages_per_tile;
+  const uint8_t* src = sg.Y0 + (size_t)(2 * t0 + (int)rank) * sg.ystep;          // this CTA's 64-row half of tile t0
+  for (int t = t0; t < t1; ++t, src += step2) {
+    st_shared_u32(progress_u, ++rg.tiles);                 // paces the prefetcher (prefetch_segment)
+    const uint8_t* p = src;
+    uint64_t ml = mlist;
+    for (int j = 0; j < nst; ++j, ml >>= 4) {
+      const uint32_t bytes = ((uint32_t)(ml & 15u) + 1u) * 2048u;
+      const uint32_t full = ya.full0 + 8u * rg.s;
+      TWAIT(0, ya.empty0 + 8u * rg.s, rg.ph ^ 1u);
+      { TSPAN_BEGIN(); mbar_expect_tx(full, bytes); TSPAN_END(3); }
+      { TSPAN_BEGIN(); bulk_g2s(ya.dst0 + rg.s * ya.step, p, bytes, full); TSPAN_END(4); }
+      rg.advance();
+      p += bytes;
+      if (need_R && --pre == 0) load_R();
     }
+  }
   if (need_R) load_R();
   ++seg_i;
 }
@@ -345,6 +368,21 @@ __device__ __forceinline__ void relay_y_segment(YRing& rg, const YAddr ya, int& 
     rg.advance();
   }
   ++seg_i;
+}
+
+// L2 prefetcher (one thread of an otherwise idle warp, both CTAs): when PY starts tile t of a unit, the record of tile
+// t + PK_YPF is requested from HBM.  (Issued by PY itself the instruction cost it ~580 cycles per tile in the low-rate
+// kernel: cp.async.bulk.prefetch.L2 of a 20-40 KB record blocks the issuing thread.)  Paced by PY's progress word, which
+// only grows: no barrier phase can be missed.
+__device__ __forceinline__ void prefetch_segment(uint32_t& seen, uint32_t progress_u, const uint8_t* Y0, uint32_t ystep, uint32_t rank, int t0, int t1)
+{
+  const uint32_t step2 = 2u * ystep;
+  const uint8_t* src = Y0 + (size_t)(2 * (t0 + PK_YPF) + (int)rank) * ystep;
+  for (int t = t0; t < t1; ++t, src += step2) {
+    ++seen;
+    while (ld_shared_volatile_u32(progress_u) < seen) __nanosleep(64);
+    if (t + PK_YPF < t1) bulk_prefetch_l2(src, ystep);
+  }
 }
 
 // RT, epilogue warps at the start of a unit: the unit's R block of this CTA (128 rows x K) -> TMEM columns [PK_ACOL, PK_ACOL + K / 2).
@@ -377,31 +415,35 @@ __device__ __forceinline__ void load_R_tmem(const SliceParams* __restrict__ sp, 
   tmem_st_wait();
 }
 
-// IY role: the y MMAs of one tile into accumulator d_tmem (first MMA overwrites)
+// IY role: the y MMAs of one tile into accumulator d_tmem (first MMA overwrites).  mlist: the tile's stages in order, MMAs
+// per stage minus one in 4 bits each (SegSrc::mlist, read once per unit: the loop touches no shared memory but the barriers)
 template <bool RT>
-__device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, const SegSrc& sg, uint32_t d_tmem, uint32_t a_base, uint32_t idesc,
+__device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, uint64_t mlist, int n_stages, uint32_t d_tmem, uint32_t a_base, uint32_t idesc,
                                         bool trace, long long* tw)
 {
   uint32_t acc = 0u, a_lo = a_base;
-  for (int i = 0; i < sg.n; ++i) {
-    const int nst = sg.nst[i], base = sg.mbase[i], ext = sg.ext[i];
-    for (int j = 0; j < nst; ++j) {
-      const int m = base + (j < ext ? 1 : 0);
-      TWAIT(2, ya.full0 + 8u * rg.s, rg.ph);
-      fence_after();
-      mma_y_stage<RT>(d_tmem, a_lo, ya.dst0 + rg.s * ya.step, idesc, m, acc);
-      commit2(ya.empty0 + 8u * rg.s, 3);
-      acc = 1u;
-      a_lo += (uint32_t)m * (RT ? 8u : 256u);
-      rg.advance();
-    }
+  for (int j = 0; j < n_stages; ++j, mlist >>= 4) {
+    const int m = (int)(mlist & 15u) + 1;
+    TWAIT(2, ya.full0 + 8u * rg.s, rg.ph);
+    fence_after();
+#ifdef LLOID_TRACE_BUILD
+    if (!(g_exp & 2))
+#endif
+    { TSPAN_BEGIN(); mma_y_stage<RT>(d_tmem, a_lo, ya.dst0 + rg.s * ya.step, idesc, m, acc); TSPAN_END(3); }
+    { TSPAN_BEGIN(); commit2(ya.empty0 + 8u * rg.s, 3); TSPAN_END(4); }
+    acc = 1u;
+    a_lo += (uint32_t)m * (RT ? 8u : 256u);
+#ifdef LLOID_TRACE_BUILD
+    if (!RT && g_fake_half_r && a_lo >= a_base + 2560u) a_lo -= 2560u;      // experiment: config 2 only (10 MMAs = 40 KB)
+#endif
+    rg.advance();
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 struct LowPArgs {
   const SliceParams* sp; const RateGroup* groups; const LowUnit* units;
-  int r_bytes, nsy, ystage, trace;
+  int r_bytes, nsy, ystage, ycap, trace;
   SchedArgs sched;
 };
 
@@ -429,6 +471,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   const uint32_t sR_u = smem_u32(smem);                 // !RT: [l_sum / 8][128 rows][8] fp16
   const uint32_t ring_u = sR_u + (RT ? 0u : (uint32_t)a.r_bytes);
   const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done), r_ready_u = smem_u32(&bars.r_ready);
+  const uint32_t progress_u = smem_u32(&bars.py_tiles);
   const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
 
   if (warp == 0) {
@@ -439,11 +482,19 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
-        seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
-        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, 0u, nullptr, 0u, trace, tw);
+        seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank, a.ycap);
+        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, progress_u, rank, t0, t1, 0u, nullptr, 0u, trace, tw);
         nt += t1 - t0;
       }
       if (rank == 0) TRACE_END(0, 0, nt);
+    }
+  } else if (warp == 7) {
+    if (elect_one()) {
+      uint32_t seen = 0;
+      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+        const SliceParams* P = a.sp + a.groups[a.units[u].group].slice[0];
+        prefetch_segment(seen, progress_u, reinterpret_cast<const uint8_t*>(P->Y), (uint32_t)P->y_step64, rank, t0, t1);
+      }
     }
   } else if (warp == 4 && rank == 1) {
     if (elect_one()) {
@@ -452,7 +503,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
-        seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank);
+        seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank, a.ycap);
         relay_y_segment<RT>(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
@@ -472,14 +523,16 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
-        seg_fill(sg, a.sp, G->slice, G->n_slices, 2 * un.pb);
+        seg_fill(sg, a.sp, G->slice, G->n_slices, 2 * un.pb, a.ycap);
+        const uint64_t mlist = sg.mlist;
+        const int n_stages = sg.stages_per_tile;
         if constexpr (RT) TWAIT(0, r_ready_u, (uint32_t)seg_i & 1u); else TWAIT(0, consts_u, (uint32_t)seg_i & 1u);   // the unit's R is in place
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
           const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
           TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          iy_tile<RT>(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          iy_tile<RT>(rg, yd, mlist, n_stages, tmem + b * 128u, a_base, idesc, trace, tw);
           commit2(acc_full_u + 8u * b, 3);
         }
         if constexpr (!RT) commit2(unit_done_u, 3);
@@ -544,7 +597,7 @@ struct F0PArgs {
   const SliceParams* sp; const BdPlan* bd; const RateGroup* groups;
   const uint8_t* P;                                     // [2][p_bytes]: band-matrix blob of rank 0, of rank 1
   Peak* partials; Capture cap; long long k_a;
-  int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, ystage, slots_cap, max_templates, trace;
+  int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, ystage, ycap, slots_cap, max_templates, trace;
   F0Sched sched;
   PairRate rate[kNLowRates];
   PairMma tab[kPairTabMax];                             // interpolation MMAs, see PairMma
@@ -584,6 +637,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 2u);
   const uint32_t tmem = tmem_slot;
   const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done), r_ready_u = smem_u32(&bars.r_ready);
+  const uint32_t progress_u = smem_u32(&bars.py_tiles);
   const YAddr ya{smem_u32(&bars.yfull[0]), smem_u32(&bars.yempty[0]), ring_u, (uint32_t)a.ystage};
   const uint32_t qfull_u = smem_u32(&bars.qfull[0]), qempty_u = smem_u32(&bars.qempty[0]);
   const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]), ybar_u = smem_u32(&bars.ybar[0]);
@@ -597,11 +651,19 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
       FOR_F0_SEGMENTS(it, S, pA, pB) {
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
-        seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
-        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes, trace, tw);
+        seg_fill(seg[0], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank, a.ycap);
+        py_segment<RT>(rg, ya, seg_i, seg[0], consts_u, unit_done_u, sR_u, progress_u, rank, t0, t1, sP_u, a.P + (size_t)rank * a.p_bytes, (uint32_t)a.p_bytes, trace, tw);
         nt += t1 - t0;
       }
       if (rank == 0) TRACE_END(1, 0, nt);
+    }
+  } else if (warp == 7) {
+    if (elect_one()) {
+      uint32_t seen = 0;
+      FOR_F0_SEGMENTS(it, S, pA, pB) {
+        const SliceParams* P = a.sp + a.bd[S.bds[it.cur.ib].bd].f0_slice[0];
+        prefetch_segment(seen, progress_u, reinterpret_cast<const uint8_t*>(P->Y), (uint32_t)P->y_step64, rank, it.cur.t, it.seg_end());
+      }
     }
   } else if (warp == 4 && rank == 1) {
     if (elect_one()) {
@@ -610,7 +672,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
       FOR_F0_SEGMENTS(it, S, pA, pB) {
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
-        seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank);
+        seg_fill(seg[2], a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank, a.ycap);
         relay_y_segment<RT>(rg, ya, seg_i, (t1 - t0) * seg[2].stages_per_tile, consts_u);
       }
     }
@@ -708,21 +770,23 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
       FOR_F0_SEGMENTS(it, S, pA, pB) {
         const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
         const BdPlan* B = a.bd + bdi;
-        seg_fill(sg, a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb);
+        seg_fill(sg, a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb, a.ycap);
+        const uint64_t mlist = sg.mlist;
+        const int n_stages = sg.stages_per_tile;
         if constexpr (RT) TWAIT(0, r_ready_u, (uint32_t)seg_i & 1u); else TWAIT(0, consts_u, (uint32_t)seg_i & 1u);   // the unit's R is in place
         fence_after();
         for (int t = t0; t < t1; ++t, ++e) {
           const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
           TWAIT(1, acc_empty_u + 8u * b, ph ^ 1u);
           fence_after();
-          iy_tile<RT>(rg, yd, sg, tmem + b * 128u, a_base, idesc, trace, tw);
+          iy_tile<RT>(rg, yd, mlist, n_stages, tmem + b * 128u, a_base, idesc, trace, tw);
           commit2(ybar_u + 8u * b, 1);
         }
         ++seg_i;
       }
       TRACE_END(1, 1, (int)e);
     }
-  } else if ((warp == 3 || warp == 16) && rank == 0) {
+  } else if ((warp == 3 || warp == 5) && rank == 0) {
     // ===== IQ0 / IQ1: interpolation MMAs (A4) of the even / odd tiles, after the tile's y part is complete.  (Two threads
     // accumulating into the SAME accumulator concurrently gave wrong sums: the pipe orders the MMAs of one thread only;
     // tiles of different parity use different accumulators.) =====
@@ -752,19 +816,25 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
             TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), (e >> 2) & 1u);
             fence_after();
             const uint32_t d_tmem = tmem + b * 128u;
+            {
+              TSPAN_BEGIN();
 #pragma unroll
-            for (int r = 0; r < kNLowRates; ++r) {
-              if (!(mine >> r & 1u)) continue;
-              const int v = t & vmask[r];
-              const int n_it = a.rate[r].n_items[v];
-              int idx = a.rate[r].tab_off[v] + sb[r] * n_it;               // [slot of the window's first chunk][item]
-              for (int k = 0; k < n_it; ++k, ++idx) {
-                const PairMma m = a.tab[idx];
-                mma2_ss(d_tmem + m.d_col, desc64(qa[r] + m.a_off), desc64(p_base + m.p_lo), m.idesc, 1u);
+              for (int r = 0; r < kNLowRates; ++r) {
+                if (!(mine >> r & 1u)) continue;
+                const int v = t & vmask[r];
+                const int n_it = a.rate[r].n_items[v];
+                int idx = a.rate[r].tab_off[v] + sb[r] * n_it;               // [slot of the window's first chunk][item]
+                for (int k = 0; k < n_it; ++k, ++idx) {
+                  const PairMma m = a.tab[idx];
+#ifdef LLOID_TRACE_BUILD
+                  if (g_exp & 1) continue;
+#endif
+                  mma2_ss(d_tmem + m.d_col, desc64(qa[r] + m.a_off), desc64(p_base + m.p_lo), m.idesc, 1u);
+                }
               }
+              TSPAN_END(2);
             }
-            commit2(qempty_u + 8u * (e & (PK_NQB - 1)), 3);
-            commit2(acc_full_u + 8u * b, 3);
+            { TSPAN_BEGIN(); commit2(qempty_u + 8u * (e & (PK_NQB - 1)), 3); commit2(acc_full_u + 8u * b, 3); TSPAN_END(3); }
             ++mine_n;
           }
           // window start of the next tile: floor(adv (t + 1) / 16) chunks
@@ -818,17 +888,17 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         const int kap0 = t * 128;
         const int valid = min(128, a.c - kap0);
         const int cthr = 64 * wg + 2 * tc;                                // column of (i = 0, e = 0)
+        uint32_t rr[2][32];
+        __syncwarp();                                                     // tcgen05.ld is .aligned: the lanes may have diverged above
+        tmem_ld_16x256b_x8(taddr, rr[0]);
+        tmem_ld_16x256b_x8(taddr + (16u << 16), rr[1]);
+        tmem_ld_wait();
+        fence_before();                                                   // both halves are in registers: free the accumulator
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-          uint32_t r[32];
-          __syncwarp();                                                   // tcgen05.ld is .aligned: the lanes may have diverged above
-          tmem_ld_16x256b_x8(taddr + ((uint32_t)(16 * h) << 16), r);
-          tmem_ld_wait();
-          if (h == 1) {                                                   // both halves are in registers: free the accumulator
-            fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);
-          }
+          uint32_t (&r)[32] = rr[h];
           if constexpr (CAPTURE) {
             const int p = p0 + 8 * h;
             if (a.cap.bd == bdi && 2 * p + 1 < a.cap.rows) {
@@ -843,11 +913,21 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
               }
             }
           }
+#ifdef LLOID_TRACE_BUILD
+          if (g_exp & 4) continue;
+#endif
           uint32_t code[16];
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const float re = __uint_as_float(r[4 * (j >> 1) + (j & 1)]), im = __uint_as_float(r[4 * (j >> 1) + 2 + (j & 1)]);
-            code[j] = (__float_as_uint(fmaf(re, re, im * im)) & ~15u) | (uint32_t)(15 - j);
+          for (int i = 0; i < 8; ++i) {                                   // two columns per packed instruction: q = fma(re, re, im * im)
+            uint64_t re2, im2, q2;
+            asm("mov.b64 %0, {%1, %2};" : "=l"(re2) : "r"(r[4 * i]), "r"(r[4 * i + 1]));
+            asm("mov.b64 %0, {%1, %2};" : "=l"(im2) : "r"(r[4 * i + 2]), "r"(r[4 * i + 3]));
+            asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(q2) : "l"(im2));
+            asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(q2) : "l"(re2));
+            uint32_t q0, q1;
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(q0), "=r"(q1) : "l"(q2));
+            code[2 * i] = (q0 & ~15u) | (uint32_t)(15 - 2 * i);
+            code[2 * i + 1] = (q1 & ~15u) | (uint32_t)(14 - 2 * i);
           }
           if (valid < 128) {
 #pragma unroll
@@ -1067,7 +1147,11 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   // windows and >= 3 y stages: if EVERY (bin, detector) fits that way the bank runs the RT = false kernels; otherwise the
   // whole bank runs the RT = true kernels (R in TMEM, K <= 512), and only what exceeds THAT is left to the FFMA kernels.
   {
+#ifdef LLOID_TRACE_BUILD
+    const int lim_f0_smem = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / (getenv("LLOID_FAKE_HALF_R") ? 128 : 256);
+#else
     const int lim_f0_smem = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / 256;
+#endif
     const int lim_low_smem = (PK_SMEM_BUDGET - 3 * 16384) / 256;
     bool rt = false;
     for (int b = 0; b < n_bd; ++b) {
@@ -1090,17 +1174,25 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
     if (pl->combos_host.empty()) return true;             // nothing fits: the whole bank goes to the FFMA kernels
   }
+#ifdef LLOID_TRACE_BUILD
+  const int fake_half = getenv("LLOID_FAKE_HALF_R") ? 1 : 0;
+  cudaMemcpyToSymbol(g_fake_half_r, &fake_half, sizeof(int));
+  const int f0_fixed = (pl->r_tmem ? 0 : pl->l_sum_f0_max * (fake_half ? 128 : 256)) + pl->p_bytes + pl->q_bytes;
+#else
   const int f0_fixed = (pl->r_tmem ? 0 : pl->l_sum_f0_max * 256) + pl->p_bytes + pl->q_bytes;
+#endif
   const int low_fixed = pl->r_tmem ? 0 : pl->l_sum_low_max * 256;
-  // y stage slot: the largest stage of any slice the kernel streams (a slice with nm = L_pad / 16 MMAs per tile is cut
-  // into ceil(nm / 8) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
+  // y stage slot: the largest stage of any unit the kernel streams (a unit with nm = sum L_pad / 16 MMAs per tile is cut
+  // into ceil(nm / ycap) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
+  pl->ycap = getenv("LLOID_YCAP") ? std::max(2, std::min(16, atoi(getenv("LLOID_YCAP")))) : 8;
   int ys_f0 = 2048, ys_low = 2048;
+  auto stage_bytes = [&](int l_sum) { const int nm = l_sum / 16, nst = stage_count(nm, pl->ycap); return (nm + nst - 1) / nst * 2048; };
   for (int b = 0; b < n_bd; ++b) {
     if (pl->excluded[b]) continue;
-    for (int s = 0; s < bp_host[b].n_slices; ++s) {
-      const SliceParams& P = sp_host[bp_host[b].first_slice + s];
-      const int nm = P.L_pad / 16, nst = stage_count(nm), big = (nm + nst - 1) / nst * 2048;
-      if (P.d == 1) ys_f0 = std::max(ys_f0, big); else ys_low = std::max(ys_low, big);
+    ys_f0 = std::max(ys_f0, stage_bytes(pl->bd_host[b].l_sum));
+    for (int r = 0; r < pl->n_lr; ++r) {
+      const RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
+      if (G.n_slices) ys_low = std::max(ys_low, stage_bytes(G.l_sum));
     }
   }
   pl->f0_ystage = ys_f0; pl->low_ystage = ys_low;
@@ -1108,6 +1200,9 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   pl->low_stages = std::min(PK_NSY_MAX, (PK_SMEM_BUDGET - low_fixed) / ys_low);
   pl->f0_smem = f0_fixed + pl->f0_stages * ys_f0;
   pl->low_smem = low_fixed + pl->low_stages * ys_low;
+  if (getenv("LLOID_PLAN_PRINT"))
+    fprintf(stderr, "[lloid plan] r_tmem %d  f0: R %d B, P %d B, Q windows %d B, %d y slots of %d B   low: R %d B, %d y slots of %d B   ycap %d\n",
+            (int)pl->r_tmem, pl->l_sum_f0_max * 256, pl->p_bytes, pl->q_bytes, pl->f0_stages, ys_f0, pl->l_sum_low_max * 256, pl->low_stages, ys_low, pl->ycap);
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
   std::vector<SchedUnit> low_sched;
@@ -1197,11 +1292,14 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
                      int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
 {
   const int n_clusters = std::max(1, pl->n_sm / 2);
+#ifdef LLOID_TRACE_BUILD
+  { const int exp_bits = getenv("LLOID_EXP") ? atoi(getenv("LLOID_EXP")) : 0; cudaMemcpyToSymbol(g_exp, &exp_bits, sizeof(int)); }
+#endif
   if (pl->low_units > 0) {
     LowPArgs la;
     memset(&la, 0, sizeof la);
     la.sp = sp_dev; la.groups = pl->groups_dev; la.units = (const LowUnit*)pl->units_dev;
-    la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages; la.ystage = pl->low_ystage; la.trace = getenv("LLOID_TRACE") ? 1 : 0;
+    la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages; la.ystage = pl->low_ystage; la.ycap = pl->ycap; la.trace = getenv("LLOID_TRACE") ? 1 : 0;
     SchedArgs& sc = la.sched;
     sc.units = pl->low_sched_dev; sc.n_cls = pl->n_lr;
     long long tiles_total = 0;
@@ -1223,12 +1321,26 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   a.sp = sp_dev; a.bd = pl->bd_dev; a.groups = pl->groups_dev;
   a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
   a.partials = partials; a.cap = cap; a.k_a = k_a;
-  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
-  a.nsy = pl->f0_stages; a.ystage = pl->f0_ystage; a.slots_cap = slots_cap; a.max_templates = max_templates;
+  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; 
+#ifdef LLOID_TRACE_BUILD
+  if (getenv("LLOID_FAKE_HALF_R")) a.r_bytes /= 2;
+#endif
+  a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
+  a.nsy = pl->f0_stages; a.ystage = pl->f0_ystage; a.ycap = pl->ycap; a.slots_cap = slots_cap; a.max_templates = max_templates;
   a.trace = getenv("LLOID_TRACE") ? 1 : 0;
   const int n_tiles = (c + 127) / 128;
   a.sched.bds = pl->f0_sched_dev; a.sched.n_bds = pl->f0_n_bds; a.sched.n_tiles = n_tiles;
-  a.sched.gt = gt; a.sched.gb = (PK_BLOCK_TILES + gt - 1) / gt * gt;      // time blocks hold whole granules
+  // Time block = one cluster's share of the tiles, rounded up to whole granules: cluster i then works on (about) the i-th
+  // (time block, template block) cell, so the clusters that walk the template blocks of one time block start together
+  // and read the same y tiles within a few tiles of each other: 7 of the 8 reads of a y tile hit L2.  (With fixed blocks
+  // of 64 tiles a cluster walked 3.5 cells, a y tile was re-read 64 tiles = 0.1 ms later, long after L2 had turned over:
+  // 1.87 GB of DRAM reads per config-2 launch for 0.67 GB of operands.)
+  {
+    const long long all_tiles = (long long)pl->combos_host.size() * n_tiles;
+    long long gb = getenv("LLOID_F0_BLOCK") ? atoi(getenv("LLOID_F0_BLOCK")) : (all_tiles + n_clusters - 1) / n_clusters;
+    gb = std::max<long long>(gt, (gb + gt - 1) / gt * gt);
+    a.sched.gt = gt; a.sched.gb = (int)std::min<long long>(gb, (long long)(n_tiles + gt - 1) / gt * gt + gt);
+  }
   a.sched.total = pl->f0_wsum; a.sched.a0 = k_a / kTimeTile;
   for (int r = 0; r < kNLowRates; ++r) a.rate[r] = pl->rate[r];
   memcpy(a.tab, pl->tab, sizeof a.tab);

@@ -20,7 +20,7 @@ __device__ __forceinline__ void ffma2(u64& c, u64 a, u64 b) { asm("fma.rn.f32x2 
 // Eight consecutive l of one reconstruction row i / one y row r, from the fp32 row-major arrays or (PK: the fp16
 // path's CUDA-core fallback for banks the tensor reconstruction cannot hold) from the packed fp16 operands, where the
 // same eight values are one 16-byte core-matrix row:  R16[i / 128][l / 8][r16_lane(i % 128)][l % 8],
-// Y16[r / 64][l / 8][r % 64][l % 8].  l is a multiple of 8.
+// Y16[r / 64][slice of the rate group][l / 8][r % 64][l % 8] (y_step64 bytes per 64-row tile).  l is a multiple of 8.
 __device__ __forceinline__ void h8_to_f(const uint4 v, float4& lo, float4& hi)
 {
   const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
@@ -44,7 +44,7 @@ __device__ __forceinline__ const char* base8_Y(const SliceParams& P, int r, int 
 {
   if constexpr (PK) {
     step = 64 * 8 * 2;
-    return reinterpret_cast<const char*>(reinterpret_cast<const __half*>(P.Y) + (((size_t)(r >> 6) * (P.L_pad >> 3) + (l >> 3)) * 64 + (r & 63)) * 8);
+    return reinterpret_cast<const char*>(P.Y) + (size_t)(r >> 6) * P.y_step64 + (((size_t)(l >> 3)) * 64 + (r & 63)) * 16;
   } else {
     step = 32;
     return reinterpret_cast<const char*>(reinterpret_cast<const float*>(P.Y) + (size_t)r * P.L_pad + l);
@@ -383,7 +383,7 @@ recon_f32_kernel(const SliceParams* __restrict__ sp, const BinParams* __restrict
           const int le = e & 7, col = (e >> 3) % Ks, lg = (e >> 3) / Ks;
           const int r = r0 + col, l = l0 + lg * 8 + le;
           Ys[(lg * 8 + le) * RC_YS + col] =
-              (r < P.y_rows_cap) ? __half2float(Yh[(((size_t)(r >> 6) * (Lp >> 3) + (l >> 3)) * 64 + (r & 63)) * 8 + le]) : 0.f;
+              (r < P.y_rows_cap) ? __half2float(Yh[(size_t)(r >> 6) * (P.y_step64 >> 1) + ((size_t)(l >> 3) * 64 + (r & 63)) * 8 + le]) : 0.f;
         }
       } else {
         for (int e = tid; e < Ks * RC_KC; e += 256) {

@@ -478,12 +478,30 @@ int lloid_bank_finalize(lloid_bank_t* b)
     // Every chunk costs four kernel boundaries (launch gap, prologue with TMEM allocation and the stationary
     // operands, pipeline fill and drain), and every low-rate slice computes 2 K_up halo rows and rounds its rows up to
     // 128-row MMA tiles per chunk, so chunks are made LONG: up to 2^17 samples, bounded by the chunk-local
-    // intermediates (y^s and the low-rate rho^(d)), which may take 40 % of the free device memory (4 ... 64 GiB).
-    // BASELINE config 2 (2 (bin, detector) pairs): 131072 samples = 1.2 GB; config 4 (3000 pairs): 4096 samples = 58 GB.
-    double budget = 0.4 * (double)mem_free;
-    budget = std::min(std::max(budget, 4.0 * 1024 * 1024 * 1024), 64.0 * 1024 * 1024 * 1024);
+    // intermediates (y^s and the low-rate rho^(d)), which may take half of the free device memory (4 ... 96 GiB).
+    // BASELINE config 2 (2 (bin, detector) pairs): 131072 samples = 1.2 GB; config 4 (3000 pairs): 7680 samples = 60 GB.
+    double budget = 0.5 * (double)mem_free;
+    budget = std::min(std::max(budget, 4.0 * 1024 * 1024 * 1024), 96.0 * 1024 * 1024 * 1024);
     C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
     C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
+    if (b->f16 && C < 32768) {
+      // A memory-bound chunk is short, and then the 128-row MMA tiles of the low rates matter: a slice at f0 / d computes
+      // ceil((C / d + 2 K_up) / 128) tiles per chunk (C = 6144, d = 32: 208 rows in 2 tiles, 19 % padding; C = 7680: 256
+      // rows, none).  Take the multiple of 128 in (C_max / 2, C_max] with the least padded tensor work per sample.
+      const int64_t c_max = std::min<int64_t>((int64_t)(budget / ybytes_per_sample) / 128 * 128, 131072);
+      double best = 1e300;
+      for (int64_t c = std::max<int64_t>(2048, c_max / 2 / 128 * 128); c <= c_max; c += 128) {
+        double cost = 0.0;
+        for (const BinHost& B : b->bins)
+          for (const SliceHost& S : B.slices) {
+            const double w = (double)S.L_pad * (S.n_taps + B.rows_pad) / S.d;          // MACs per f0 sample
+            const double rows = (S.d == 1 || S.fold) ? (double)c : std::ceil(((double)c / S.d + 2 * Ku) / 128.0) * 128.0 * S.d;
+            cost += w * rows;
+          }
+        cost /= (double)c;
+        if (cost <= best * (1.0 + 1e-9)) { best = cost; C = c; }                       // ties: the longer chunk
+      }
+    }
   }
   {
     // the allocations below, estimated up front so that a bank that cannot fit fails with a message instead of a
@@ -562,9 +580,31 @@ int lloid_bank_finalize(lloid_bank_t* b)
   }
   char* ybase; rc = dev_alloc(b, (void**)&ybase, ybytes, true); if (rc) return rc;
   size_t yoff = 0;
-  for (SliceParams& P : b->sp_host) {
-    P.Y = ybase + yoff;
-    yoff += round_up((size_t)P.y_rows_cap * P.L_pad * esize, 256);
+  if (!b->f16) {
+    for (SliceParams& P : b->sp_host) {
+      P.Y = ybase + yoff; P.y_step64 = 0;
+      yoff += round_up((size_t)P.y_rows_cap * P.L_pad * esize, 256);
+    }
+  } else {
+    // Y16 is stored per RATE GROUP -- the slices of a (bin, detector) that are reconstructed at the same rate (a folded
+    // slice counts as d = 1), in slice order: [64-row tile][slice][l / 8][64][8].  One 64-row tile of the whole group is one
+    // contiguous record, so the reconstruction kernels stream a tile's K = sum L_pad operand with consecutive bulk copies.
+    for (size_t i = 0; i < b->sp_host.size(); ++i) {
+      SliceParams& P = b->sp_host[i];
+      if (P.Y) continue;                                   // already placed with its group
+      int rec = 0, rows_cap = 0;
+      for (size_t j = i; j < b->sp_host.size() && b->sp_host[j].bin == P.bin && b->sp_host[j].det == P.det; ++j)
+        if (b->sp_host[j].d == P.d) { rec += b->sp_host[j].L_pad * 128; rows_cap = std::max(rows_cap, b->sp_host[j].y_rows_cap); }
+      int off = 0;
+      for (size_t j = i; j < b->sp_host.size() && b->sp_host[j].bin == P.bin && b->sp_host[j].det == P.det; ++j) {
+        SliceParams& Q = b->sp_host[j];
+        if (Q.d != P.d) continue;
+        Q.Y = ybase + yoff + off; Q.y_step64 = rec; Q.y_rows_cap = rows_cap;
+        off += Q.L_pad * 128;
+      }
+      yoff += round_up((size_t)(rows_cap / 64) * rec, 256);
+    }
+    if (yoff > ybytes) return fail(LLOID_EINVAL, "internal: Y16 group layout exceeds its allocation");
   }
   for (const RateParams& R : b->rates_host)
     if (R.jj_lo_fixed < (R.d == 1 ? 0 : Kd)) return fail(LLOID_EINVAL, "internal: history too short for rate d=%d", R.d);

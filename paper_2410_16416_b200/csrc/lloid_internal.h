@@ -42,7 +42,8 @@ struct SliceParams {               // one per (bin, detector, slice); lives in a
   int32_t  bin, det, slice;
   int32_t  fir_halo;               // FIR view: rows computed per chunk = (c >> log2d) + fir_halo   (2 K_up for d > 1, else 0)
   int32_t  out_mul, out_add;       // FIR view: FIR row m is written to Y row out_mul m + out_add   (1, 0 except below)
-  int32_t  pad_[2];
+  int32_t  y_step64;               // fp16: bytes from one 64-row tile of this slice's Y16 to the next (the record of its rate group)
+  int32_t  pad_;
 };
 // fp16 path, "interpolation folded into the basis filters": a slice at f0 / 2 is NOT reconstructed at
 // its own rate and interpolated afterwards (A3 then A4); since both steps are linear,

@@ -267,4 +267,14 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t mbar_cluster)
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" :: "r"(mbar_cluster) : "memory");
 }
 
-}}  // namespace lloid::tc
+}
+// plain shared-memory word used as a monotone progress counter between two single-thread roles of a CTA
+__device__ __forceinline__ void st_shared_u32(uint32_t addr, uint32_t v) { asm volatile("st.volatile.shared::cta.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory"); }
+__device__ __forceinline__ uint32_t ld_shared_volatile_u32(uint32_t addr)
+{
+  uint32_t v;
+  asm volatile("ld.volatile.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+
+}  // namespace lloid::tc

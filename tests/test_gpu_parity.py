@@ -111,6 +111,8 @@ def test_streaming_pieces_equal_one_shot(cfg1, precision):
     small, _, info3 = pu.run_gpu(w, precision, max_chunk=512)           # library-internal chunking
     assert info3["chunk"] == 512 and _as_set(one) == _as_set(small)
     assert info2["consumed"] == n
+    odd, _, info4 = pu.run_gpu(w, precision, max_chunk=1920)            # 15 tiles: chunks cut the 16-tile peak windows anywhere
+    assert info4["chunk"] == 1920 and _as_set(one) == _as_set(odd)
 
 
 @pytest.mark.parametrize("precision", PRECISIONS)
