@@ -592,6 +592,8 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   pair_teardown(tmem, warp);
 }
 
+constexpr int kIqFast = 3;                  // interpolation MMAs per rate and tile held in registers (d >= 4: at most 3 chunks)
+
 // ------------------------------------------------------------------------------------------------
 struct F0PArgs {
   const SliceParams* sp; const BdPlan* bd; const RateGroup* groups;
@@ -812,23 +814,37 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         for (int t = t0; t < t1; ++t, ++e) {
           if ((e & 1u) == which) {
             const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
+            const uint32_t d_tmem = tmem + b * 128u;
+            // the tile's interpolation MMAs, read from the table BEFORE the waits: the indexed constant loads (a dependent
+            // chain of ~2000 cycles per tile when they sat between the wait and the MMAs) overlap the wait for the y part
+            PairMma im[kNLowRates][kIqFast];
+            int nit[kNLowRates], ix[kNLowRates];
+#pragma unroll
+            for (int r = 0; r < kNLowRates; ++r) {
+              nit[r] = 0; ix[r] = 0;
+              if (!(mine >> r & 1u)) continue;
+              const int v = t & vmask[r];
+              nit[r] = a.rate[r].n_items[v];
+              ix[r] = a.rate[r].tab_off[v] + sb[r] * nit[r];                 // [slot of the window's first chunk][item]
+#pragma unroll
+              for (int k = 0; k < kIqFast; ++k) if (k < nit[r]) im[r][k] = a.tab[ix[r] + k];
+            }
             TWAIT(0, ybar_u + 8u * b, ph);
+            fence_after();
             TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), (e >> 2) & 1u);
             fence_after();
-            const uint32_t d_tmem = tmem + b * 128u;
             {
               TSPAN_BEGIN();
+#ifdef LLOID_TRACE_BUILD
+              if (!(g_exp & 1))
+#endif
 #pragma unroll
               for (int r = 0; r < kNLowRates; ++r) {
-                if (!(mine >> r & 1u)) continue;
-                const int v = t & vmask[r];
-                const int n_it = a.rate[r].n_items[v];
-                int idx = a.rate[r].tab_off[v] + sb[r] * n_it;               // [slot of the window's first chunk][item]
-                for (int k = 0; k < n_it; ++k, ++idx) {
-                  const PairMma m = a.tab[idx];
-#ifdef LLOID_TRACE_BUILD
-                  if (g_exp & 1) continue;
-#endif
+#pragma unroll
+                for (int k = 0; k < kIqFast; ++k)
+                  if (k < nit[r]) mma2_ss(d_tmem + im[r][k].d_col, desc64(qa[r] + im[r][k].a_off), desc64(p_base + im[r][k].p_lo), im[r][k].idesc, 1u);
+                for (int k = kIqFast; k < nit[r]; ++k) {                     // d = 2 windows (5 chunks), when that rate is not folded
+                  const PairMma m = a.tab[ix[r] + k];
                   mma2_ss(d_tmem + m.d_col, desc64(qa[r] + m.a_off), desc64(p_base + m.p_lo), m.idesc, 1u);
                 }
               }
