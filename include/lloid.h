@@ -200,6 +200,35 @@ int lloid_path_info(const lloid_bank_t *bank, int32_t *out);
 int lloid_set_profiling(lloid_bank_t *bank, int32_t enable);
 int lloid_last_stage_ms(lloid_bank_t *bank, float *out_ms /* host, float[6] */);
 
+/* ---- allocation-free entry point -----------------------------------------------------------------------------------
+ * Steps A5 + A6 alone ("identifies peaks in the SNR time series with SNR > 4 ... 'triggers'") on a dense SNR
+ * series the caller already holds in device memory, for callers that may not allocate (CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc).  Needs no bank.  It calls no cudaMalloc / cudaFree / allocating routine: its scratch
+ * -- one 16-byte partial peak per template and 128-sample tile -- is a file-scope device array of
+ * lloid_noalloc_max_records() = 524288 records (8 MiB), which every GPU that loads the library holds until exit.
+ *   snr_dev          device, float32 [2 n_templates][row_stride], 16-byte aligned: row 2p = Re rho_p, row 2p+1 = Im rho_p;
+ *                    column j is absolute sample k_begin + j
+ *   n_templates      1 ... 65536;  n_templates * (n_samples / 128) <= lloid_noalloc_max_records(), else LLOID_EINVAL
+ *                    (the message says so: split the call in time at window boundaries, or over templates)
+ *   n_samples        positive multiple of 128;  row_stride >= n_samples, multiple of 4;  k_begin >= 0, multiple of 128
+ *   peak_window      W, multiple of 128: windows [wW, (w+1)W) of ABSOLUTE sample indices; only windows that lie completely
+ *                    inside [k_begin, k_begin + n_samples) emit
+ *   snr_threshold    theta: trigger iff |rho|(k*) > theta (strict), k* the first maximum of |rho|^2 in the window
+ *   bin, detector    copied into the records
+ *   triggers_dev     device, lloid_trigger_t[capacity], order unspecified;  n_triggers_dev: device int64, set to the number
+ *                    of triggers found (cleared on the stream first); beyond `capacity` records are counted, not stored
+ * Asynchronous on cuda_stream, uses the CURRENT device.  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress; lloid_noalloc_setup() does only that, e.g. before a capture begins).  All calls on a device share
+ * the array, which keeps the last call's contents (nothing in it needs clearing: every record read is written by the same
+ * call first).  Calls that OVERLAP on the GPU race on it: keep them on one stream or order them with events.
+ * Errors: LLOID_EINVAL, LLOID_ECUDA. */
+int64_t lloid_noalloc_max_records(void);
+int lloid_noalloc_setup(void);
+int lloid_window_peaks_noalloc(const float *snr_dev, int32_t n_templates, int64_t n_samples, int64_t row_stride,
+                               int64_t k_begin, int32_t peak_window, float snr_threshold, int32_t bin, int32_t detector,
+                               lloid_trigger_t *triggers_dev, int64_t capacity, int64_t *n_triggers_dev,
+                               void *cuda_stream);
+
 void lloid_destroy(lloid_bank_t *bank);
 const char *lloid_last_error(void);
 const char *lloid_version(void);

@@ -70,6 +70,10 @@ EXPORTS = {
     "lloid_graph_advance": (C.c_int, [C.c_void_p, C.c_int64]),
     "lloid_set_profiling": (C.c_int, [C.c_void_p, C.c_int32]),
     "lloid_last_stage_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
+    "lloid_noalloc_max_records": (C.c_int64, []),
+    "lloid_noalloc_setup": (C.c_int, []),
+    "lloid_window_peaks_noalloc": (C.c_int, [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_float, C.c_int32,
+                                             C.c_int32, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]),
     "lloid_destroy": (None, [C.c_void_p]),
     "lloid_last_error": (C.c_char_p, []),
     "lloid_version": (C.c_char_p, []),
@@ -201,6 +205,22 @@ def lloid_path_info(bank) -> dict:
     out = (C.c_int32 * 4)()
     _check(lib().lloid_path_info(bank, out))
     return dict(tensor_recon=bool(out[0]), r_in_tmem=bool(out[1]), cuda_core_bds=int(out[2]), folded_slices=int(out[3]))
+
+
+def lloid_noalloc_max_records() -> int:
+    return lib().lloid_noalloc_max_records()
+
+
+def lloid_noalloc_setup() -> None:
+    _check(lib().lloid_noalloc_setup())
+
+
+def lloid_window_peaks_noalloc(snr_dev_ptr: int, n_templates: int, n_samples: int, row_stride: int, k_begin: int,
+                               peak_window: int, snr_threshold: float, bin_: int, detector: int, triggers_dev_ptr: int,
+                               capacity: int, n_triggers_dev_ptr: int, cuda_stream: int = 0) -> None:
+    _check(lib().lloid_window_peaks_noalloc(snr_dev_ptr, n_templates, n_samples, row_stride, k_begin, peak_window,
+                                            snr_threshold, bin_, detector, triggers_dev_ptr, capacity,
+                                            n_triggers_dev_ptr, cuda_stream))
 
 
 def lloid_set_profiling(bank, enable: bool) -> None:

@@ -26,6 +26,13 @@ int fail(int code, const char* fmt, ...)
   return code;
 }
 
+}  // namespace
+
+// other translation units of the library (kernels_noalloc.cu) report through the same thread-local message
+namespace lloid { void set_last_error(const char* msg) { g_err = msg ? msg : ""; } }
+
+namespace {
+
 #define CU(call)                                                                              \
   do { cudaError_t e_ = (call);                                                               \
        if (e_ != cudaSuccess) return fail(LLOID_ECUDA, "%s failed: %s (%s:%d)", #call,        \
