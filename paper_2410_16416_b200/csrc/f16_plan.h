@@ -31,6 +31,9 @@ struct F16Plan {
   int n_bd = 0, n_lr = 0, n_sm = 148;
   int low_smem = 0, low_stages = 0, low_units = 0;
   int f0_smem = 0, f0_stages = 0, f0_ystage = 0, low_ystage = 0;   // ystage: bytes of a y ring slot per CTA
+  int f0_n_pb = 0;                      // f0 schedule: template blocks per (bin, detector) when all agree (else 0)
+  void* (*q_alloc)(void*, size_t) = nullptr;   // optional allocator of the rho^(d) buffers (zeroed memory or null)
+  void* q_ctx = nullptr;
   int ycap = 8;                         // MMAs per y stage at most (K = 16 each)
   PairMma tab[kPairTabMax];             // interpolation MMA table of the f0 kernel (kernel parameter)
   int n_tab = 0;

@@ -212,7 +212,7 @@ __global__ void __launch_bounds__(128)
 merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const Peak* __restrict__ partials,
                      int slots_cap, const int32_t* __restrict__ slot_tiles, int c, const long long* __restrict__ k_base, long long k_off,
                      int W, float theta,
-                     const PeakState* __restrict__ state_in, PeakState* __restrict__ state_out, int n_det,
+                     const PeakState* __restrict__ state_in, PeakState* __restrict__ state_out, int n_det, int bin_base,
                      lloid_trigger_t* __restrict__ trig, long long capacity, unsigned long long* __restrict__ count)
 {
   const int bd = blockIdx.y;
@@ -251,7 +251,7 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
     const unsigned long long idx = atomicAdd(count, 1ull);
     if ((long long)idx < capacity) {
       lloid_trigger_t t;
-      t.bin = bd / n_det; t.detector = bd % n_det; t.template_idx = p; t.reserved = 0;
+      t.bin = bin_base + bd / n_det; t.detector = bd % n_det; t.template_idx = p; t.reserved = 0;
       t.sample = s.k; t.snr_re = s.re; t.snr_im = s.im;
       trig[idx] = t;
     }
@@ -265,13 +265,13 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
 void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, const Peak* partials,
                           int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a, const long long* k_base_dev, int64_t k_off,
                           int W, float theta,
-                          const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
+                          const PeakState* state_in, PeakState* state_out, int n_det, int bin_base, void* triggers, int64_t capacity,
                           unsigned long long* count, cudaStream_t st, int64_t* launches)
 {
   const int n_w = (int)((k_a + c - 1) / W - k_a / W) + 1;      // host copy of k_a: only the launch geometry depends on it
   dim3 grid((max_templates + 127) / 128, n_bd, n_w);
   merge_windows_kernel<<<grid, 128, 0, st>>>(bp_dev, max_templates, partials, slots_cap, slot_tiles_dev, c, k_base_dev, (long long)k_off, W,
-                                            theta, state_in, state_out, n_det, (lloid_trigger_t*)triggers,
+                                            theta, state_in, state_out, n_det, bin_base, (lloid_trigger_t*)triggers,
                                             (long long)capacity, count);
   ++*launches;
 }

@@ -385,10 +385,12 @@ fir_f16_pers_kernel(const SliceParams* __restrict__ sp, const RateParams* __rest
 // ------------------------------------------------------------------------------------------------
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems, const SliceParams* fir_host, int n_fir,
                          const BinParams* bp_host, int n_bd, int n_det,
-                         int chunk_cap, const double* const* up_w, int64_t* bytes, char* err, int errlen)
+                         int chunk_cap, const double* const* up_w, void* (*q_alloc)(void*, size_t), void* q_ctx,
+                         int64_t* bytes, char* err, int errlen)
 {
   (void)n_det;
   F16Plan* pl = new F16Plan();
+  pl->q_alloc = q_alloc; pl->q_ctx = q_ctx;
   pl->chunk_cap = chunk_cap;
   size_t fixed = 0, stage = 0;
   int gx = 1;

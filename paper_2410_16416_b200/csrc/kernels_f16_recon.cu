@@ -138,14 +138,21 @@ __device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl
     else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : (NT); t0 >= t1) continue; \
     else
 
-// ---- f0 kernel schedule: (bin-detector, time block, template block, tile) ---------------------------------
-// The flattened work sequence is ordered by (bin, detector), then by BLOCKS of PK_BLOCK_TILES tiles (aligned to absolute
-// tile indices), then by template block, then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends
-// moved up to granule starts.  Neighbouring clusters therefore work on the same (bin, detector, time block) -- the same y
-// tiles -- at the same time, and a cluster still walks at least a granule of consecutive tiles per visit.
+// ---- f0 kernel schedule ------------------------------------------------------------------------------------------
+// The flattened work sequence is ordered by time BLOCKS of gb tiles (aligned to absolute tile indices), then by template
+// block, then by (bin, detector), then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends moved
+// up to granule starts.  The clusters that reconstruct the n_pb template blocks of one (bin, detector, time block) -- from
+// the same y tiles -- are then T / n_pb apart in the sequence, i.e. G / n_pb clusters apart, and reach the same tile at the
+// same time: one of them reads a y tile from DRAM, the others find it in L2.  That holds for few long cells (config 2: a
+// block is one cluster's share, cluster i works on cell i) and for many short ones (config 4: 3000 (bin, detector) pairs
+// per chunk of 55 tiles; ordered by (bin, detector) first, a cluster walked the 8 template blocks of a pair one after the
+// other and every y tile came from DRAM 8 times: 3.5 GB of reads per launch for 1 GB of operands).
+// Needs the same number of template blocks for every (bin, detector) (n_pb > 0); otherwise (n_pb == 0) the order is
+// (bin, detector), time block, template block, tile.
 struct F0Sched {
   const SchedBd* bds;                       // tensor-path (bin, detector) pairs, in order
   int n_bds, n_tiles, gb, gt;
+  int n_pb;                                 // template blocks of every entry if they all agree, else 0
   long long total;                          // sum of n_pb * w
   long long a0;                             // absolute index of the chunk's tile 0
 };
@@ -153,17 +160,50 @@ struct F0Pos { int ib, lo, hi, pb, t; };    // index into bds, block [lo, hi) in
 
 __device__ __forceinline__ int f0_first_block_end(const F0Sched& S) { return min(S.n_tiles, S.gb - (int)(S.a0 % S.gb)); }
 
-__device__ __forceinline__ void f0_next_cell(const F0Sched& S, F0Pos& p)      // next (template block | time block | bd) in order
+__device__ __forceinline__ void f0_next_cell(const F0Sched& S, F0Pos& p)      // next cell in order
 {
+  if (S.n_pb) {                             // (time block, template block, bd): past the end lo == n_tiles
+    if (++p.ib < S.n_bds) { p.t = p.lo; return; }
+    p.ib = 0;
+    if (++p.pb < S.n_pb) { p.t = p.lo; return; }
+    p.pb = 0; p.lo = p.hi; p.hi = min(S.n_tiles, p.hi + S.gb); p.t = p.lo;
+    return;
+  }
   if (++p.pb < S.bds[p.ib].n_pb) { p.t = p.lo; return; }
   p.pb = 0; p.lo = p.hi; p.hi = min(S.n_tiles, p.hi + S.gb); p.t = p.lo;
   if (p.lo >= S.n_tiles) { ++p.ib; p.lo = 0; p.hi = f0_first_block_end(S); p.t = 0; }
+}
+
+__device__ __forceinline__ void f0_granule_up(const F0Sched& S, F0Pos& p)      // move up to the next granule start
+{
+  if (p.t > p.lo) {
+    const int r = (int)((S.a0 + p.t) % S.gt);
+    if (r) p.t += S.gt - r;
+    if (p.t >= p.hi) f0_next_cell(S, p);
+  }
 }
 
 __device__ __forceinline__ F0Pos f0_locate(const F0Sched& S, long long pos)
 {
   F0Pos p;
   const long long nt = S.n_tiles;
+  if (S.n_pb) {
+    if (pos >= S.total * nt) { p.ib = 0; p.lo = p.hi = p.t = S.n_tiles; p.pb = 0; return p; }
+    long long rem = pos;
+    p.lo = 0; p.hi = f0_first_block_end(S);
+    while (rem >= S.total * (p.hi - p.lo) && p.hi < S.n_tiles) { rem -= S.total * (p.hi - p.lo); p.lo = p.hi; p.hi = min(S.n_tiles, p.hi + S.gb); }
+    const long long len = p.hi - p.lo;
+    const long long row = S.total / S.n_pb * len;                       // one template block of every bd
+    p.pb = (int)min(rem / row, (long long)S.n_pb - 1);
+    rem -= p.pb * row;
+    int lo = 0, hi = S.n_bds - 1;                                       // bds[i].cum / n_pb = sum of w over the earlier entries
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.bds[mid].cum / S.n_pb * len <= rem) lo = mid; else hi = mid - 1; }
+    rem -= S.bds[lo].cum / S.n_pb * len;
+    p.ib = lo;
+    p.t = p.lo + (int)min(rem / S.bds[lo].w, len - 1);
+    f0_granule_up(S, p);
+    return p;
+  }
   if (pos >= S.total * nt) { p.ib = S.n_bds; p.lo = 0; p.hi = f0_first_block_end(S); p.pb = 0; p.t = 0; return p; }
   int lo = 0, hi = S.n_bds - 1;
   while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (S.bds[mid].cum * nt <= pos) lo = mid; else hi = mid - 1; }
@@ -175,23 +215,24 @@ __device__ __forceinline__ F0Pos f0_locate(const F0Sched& S, long long pos)
   const int len = p.hi - p.lo;
   p.pb = min((int)(rem / ((long long)B.w * len)), B.n_pb - 1);
   p.t = p.lo + min((int)((rem - (long long)p.pb * B.w * len) / B.w), len - 1);
-  if (p.t > p.lo) {                         // move up to the next granule start
-    const int r = (int)((S.a0 + p.t) % S.gt);
-    if (r) p.t += S.gt - r;
-    if (p.t >= p.hi) f0_next_cell(S, p);
-  }
+  f0_granule_up(S, p);
   return p;
 }
 
 // iterates this cluster's segments: (bd entry, template block, tiles [t0, t1))
 struct F0Iter {
   F0Pos cur, end;
+  bool pb_major;                            // F0Sched::n_pb > 0: cells are ordered (lo, pb, ib), else (ib, lo, pb)
   __device__ __forceinline__ bool at_end() const
-  { return cur.ib > end.ib || (cur.ib == end.ib && (cur.lo > end.lo || (cur.lo == end.lo && (cur.pb > end.pb || (cur.pb == end.pb && cur.t >= end.t))))); }
+  {
+    if (pb_major)
+      return cur.lo > end.lo || (cur.lo == end.lo && (cur.pb > end.pb || (cur.pb == end.pb && (cur.ib > end.ib || (cur.ib == end.ib && cur.t >= end.t)))));
+    return cur.ib > end.ib || (cur.ib == end.ib && (cur.lo > end.lo || (cur.lo == end.lo && (cur.pb > end.pb || (cur.pb == end.pb && cur.t >= end.t)))));
+  }
   __device__ __forceinline__ int seg_end() const { return (cur.ib == end.ib && cur.lo == end.lo && cur.pb == end.pb) ? end.t : cur.hi; }
 };
 #define FOR_F0_SEGMENTS(it, S, A, B)                                                              \
-  for (F0Iter it{A, B}; !it.at_end(); f0_next_cell(S, it.cur))                                    \
+  for (F0Iter it{A, B, (S).n_pb > 0}; !it.at_end(); f0_next_cell(S, it.cur))                                    \
     if (it.cur.t >= it.seg_end()) continue; else
 
 __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, uint32_t bytes, uint32_t bar)
@@ -628,7 +669,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   }
   __syncthreads();
   const F0Pos pA = s_pos[0], pB = s_pos[1];
-  { F0Iter it{pA, pB}; if (it.at_end()) return; }       // both CTAs of the cluster take the same decision
+  { F0Iter it{pA, pB, S.n_pb > 0}; if (it.at_end()) return; }       // both CTAs of the cluster take the same decision
 
   const int nsy = a.nsy, n_lr = a.n_lr, gt = S.gt;
   constexpr uint32_t NACC = Acc<RT>::N;
@@ -707,7 +748,14 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
           if (t == t0) {
             if (e > 1) TWAIT(1, qempty_u + 8u * ((e - 2) & (PK_NQB - 1)), ((e - 2) >> 2) & 1u);
             if (e > 0) TWAIT(1, qempty_u + 8u * ((e - 1) & (PK_NQB - 1)), ((e - 1) >> 2) & 1u);
-          } else if (e >= PK_QDIST) TWAIT(0, qempty_u + 8u * ((e - PK_QDIST) & (PK_NQB - 1)), ((e - PK_QDIST) >> 2) & 1u);
+          } else {
+            // tile e's rows overwrite chunks that only tiles <= e - PK_QDIST read.  Even and odd tiles are finished by different
+            // threads, each in order: BOTH of e - PK_QDIST and e - PK_QDIST - 1 must be complete.  (Waiting for the first one
+            // only let a lagging thread's tile lose rows of its window while its MMAs were still to run: about one wrong SNR
+            // value in 10^8, seen as triggers that came and went between identical runs.)
+            if (e >= PK_QDIST + 1) TWAIT(0, qempty_u + 8u * ((e - PK_QDIST - 1) & (PK_NQB - 1)), ((e - PK_QDIST - 1) >> 2) & 1u);
+            if (e >= PK_QDIST) TWAIT(0, qempty_u + 8u * ((e - PK_QDIST) & (PK_NQB - 1)), ((e - PK_QDIST) >> 2) & 1u);
+          }
           const uint32_t fb = qfull_u + 8u * (e & (PK_NQB - 1));
           int nnew[kNLowRates];
           uint32_t total = 0;
@@ -831,6 +879,10 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
             }
             TWAIT(0, ybar_u + 8u * b, ph);
             fence_after();
+            // the tile's window holds rows that arrived with THIS tile's event and with the previous tile's, which the other
+            // IQ thread waited for, not this one -- and bulk copies complete in any order: wait for both.  (With the wait for
+            // the own event only, a window row could still be in flight when its MMA ran: see the note in the PQ role.)
+            if (e > 0) TWAIT(1, qfull_u + 8u * ((e - 1) & (PK_NQB - 1)), ((e - 1) >> 2) & 1u);
             TWAIT(1, qfull_u + 8u * (e & (PK_NQB - 1)), (e >> 2) & 1u);
             fence_after();
             {
@@ -1222,14 +1274,32 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
   std::vector<SchedUnit> low_sched;
+  // rho^(d) buffers: ONE allocation (chunk-local: a part of a split bank takes it from the parent's shared set)
+  size_t q_total = 0;
+  for (int r = 0; r < pl->n_lr; ++r)
+    for (int b = 0; b < n_bd; ++b) {
+      const RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
+      if (G.n_slices && !pl->excluded[b]) q_total += (size_t)G.n_rb * 2 * G.q_groups_cap * 2048;
+    }
+  uint8_t* q_base = nullptr;
+  if (q_total) {
+    if (pl->q_alloc) {
+      q_base = (uint8_t*)pl->q_alloc(pl->q_ctx, q_total);
+      if (!q_base) { snprintf(err, errlen, "fp16 plan: %zu bytes for the low-rate SNR buffers could not be allocated", q_total); return false; }
+    } else {
+      void* q = nullptr;
+      if (!plan_alloc(pl, &q, q_total, true, bytes, err, errlen)) return false;
+      q_base = (uint8_t*)q;
+    }
+  }
+  size_t q_off = 0;
   for (int r = 0; r < pl->n_lr; ++r) {
     pl->units_per_rate[r] = 0; pl->low_wsum[r] = 0;
     for (int b = 0; b < n_bd; ++b) {
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
       if (G.n_slices == 0 || pl->excluded[b]) continue;
-      void* q = nullptr;
-      if (!plan_alloc(pl, &q, (size_t)G.n_rb * 2 * G.q_groups_cap * 2048, true, bytes, err, errlen)) return false;
-      G.Q = (__half*)q;
+      G.Q = (__half*)(q_base + q_off);
+      q_off += (size_t)G.n_rb * 2 * G.q_groups_cap * 2048;
       for (int rb = 0; rb < G.n_rb; ++rb) {
         units.push_back(LowUnit{b * pl->n_lr + r, rb});
         low_sched.push_back(SchedUnit{G.l_sum / 16, (int32_t)pl->low_wsum[r]});
@@ -1254,6 +1324,8 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     pl->f0_wsum += (long long)e.n_pb * w;
   }
   pl->f0_n_bds = (int)f0_sched.size();
+  pl->f0_n_pb = f0_sched.empty() ? 0 : f0_sched[0].n_pb;                 // template blocks per (bin, detector) if uniform, else 0
+  for (const SchedBd& e : f0_sched) if (e.n_pb != pl->f0_n_pb) pl->f0_n_pb = 0;
   pl->low_units = (int)units.size();
   auto upload = [&](void** dst, const void* src, size_t n) -> bool {
     if (!plan_alloc(pl, dst, n, false, bytes, err, errlen)) return false;
@@ -1358,6 +1430,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     a.sched.gt = gt; a.sched.gb = (int)std::min<long long>(gb, (long long)(n_tiles + gt - 1) / gt * gt + gt);
   }
   a.sched.total = pl->f0_wsum; a.sched.a0 = k_a / kTimeTile;
+  a.sched.n_pb = getenv("LLOID_F0_ORDER_BD") ? 0 : pl->f0_n_pb;
   for (int r = 0; r < kNLowRates; ++r) a.rate[r] = pl->rate[r];
   memcpy(a.tab, pl->tab, sizeof a.tab);
   const long long pair_tiles = (long long)pl->combos_host.size() * n_tiles;

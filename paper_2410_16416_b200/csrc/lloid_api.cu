@@ -103,6 +103,17 @@ struct lloid_bank {
   std::vector<Q32Group> q32_host;          // fp32 path: [n_bd][kNLowRates]
   Q32Group* q32_dev = nullptr;
 
+  // A bank whose chunk-local intermediates (y^s, rho^(d)) would force chunks shorter than kSplitChunk is cut at finalize into
+  // PARTS: contiguous ranges of bins, each a bank of its own (plan, state, history) over the parent's uploaded arrays,
+  // run one after the other on the caller's stream.  The parts share one set of chunk-local buffers (scratch[]), so each
+  // can afford a chunk n_parts times longer.  A parent runs no kernels of its own.
+  std::vector<lloid_bank*> parts;
+  std::vector<int> part_of_bin;          // parent: part index of a bin
+  lloid_bank* parent = nullptr;
+  int bin_base = 0;                      // part: first bin of its range (added to the bin index of its triggers)
+  double budget = 0.0;                   // part: bytes its chunk-local intermediates may take (the parent decides)
+  struct Scratch { void* p = nullptr; size_t cap = 0; } scratch[3];   // parent: 0 y^s, 1 rho^(d) (fp16 plan), 2 partial peaks
+
   int slice_index(int bin, int det, int s) const { return bp_host[bin * cfg.n_detectors + det].first_slice + s; }
 };
 
@@ -117,6 +128,30 @@ int dev_alloc(lloid_bank* b, void** p, size_t n, bool zero)
   b->owned.push_back(*p);
   b->bytes += (int64_t)n;
   return LLOID_OK;
+}
+
+// Chunk-local buffers (kind: 0 y^s, 1 rho^(d), 2 partial peaks).  A whole bank allocates its own.  A part takes them from
+// its parent's shared set: every part's buffer of a kind starts at the same address -- fp16 data over fp16 data, records
+// over records, so whatever an earlier part left there is finite -- and the parts never run concurrently.
+int scratch_alloc(lloid_bank* b, int kind, void** p, size_t n, bool zero)
+{
+  if (!b->parent) return dev_alloc(b, p, n, zero);
+  lloid_bank::Scratch& S = b->parent->scratch[kind];
+  if (n > S.cap) {
+    const size_t want = n + n / 32;                  // the parts are finalized largest first; headroom for padding differences
+    void* q = nullptr;
+    int rc = dev_alloc(b->parent, &q, want, true);   // (an outgrown buffer stays with the parts that point into it)
+    if (rc) return rc;
+    S.p = q; S.cap = want;
+  }
+  *p = S.p;
+  return LLOID_OK;
+}
+
+void* plan_scratch_alloc(void* ctx, size_t n)
+{
+  void* p = nullptr;
+  return scratch_alloc((lloid_bank*)ctx, 1, &p, n, true) == LLOID_OK ? p : nullptr;
 }
 
 int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const double* recon,
@@ -296,7 +331,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
   const size_t nstate = (size_t)b->n_bd * b->max_templates;
   launch_merge_windows(b->bp_dev, b->n_bd, b->max_templates, b->partials, b->slots_cap, b->slot_tiles_dev, c, k_a, b->k_base_dev, k_a - b->call_start,
                        b->cfg.peak_window, b->cfg.snr_threshold, b->state + b->state_cur * nstate,
-                       b->state + (b->state_cur ^ 1) * nstate, D, trig, capacity, count, st, &b->last_launches);
+                       b->state + (b->state_cur ^ 1) * nstate, D, b->bin_base, trig, capacity, count, st, &b->last_launches);
   b->state_cur ^= 1;
   mark(b, st, kTagMerge);
   if (int rc = debug_sync("merge_windows_kernel", k_a, st)) return rc;
@@ -455,6 +490,68 @@ int lloid_bank_alias_bin(lloid_bank_t* b, int32_t dst, int32_t src)
   return LLOID_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+constexpr int64_t kSplitChunk = 32768;   // a bank whose automatic chunk would be shorter than this is cut into parts
+
+// bytes of chunk-local intermediates per f0 sample of bins [lo, hi): y^s of every slice, rho^(d) of the low-rate ones
+double intermediates_per_sample(const lloid_bank* b, int lo, int hi)
+{
+  const int D = b->cfg.n_detectors;
+  const size_t esize = b->f16 ? 2 : 4;
+  double v = 0.0;
+  for (int bi = lo; bi < hi; ++bi) {
+    const BinHost& B = b->bins[bi];
+    for (const SliceHost& S : B.slices) {
+      v += (double)D * S.L_pad * esize / (S.fold ? 1 : S.d);
+      if (S.d > 1 && !S.fold) v += (double)D * B.rows_pad * esize / S.d;
+    }
+  }
+  return v;
+}
+
+int finalize_impl(lloid_bank* b);
+int filter_one(lloid_bank* b, const float* strain_dev, int64_t n, lloid_trigger_t* trig, int64_t capacity, int64_t* count_dev, cudaStream_t st);
+
+// a part: bins [lo, hi) of the parent as a bank of its own over the parent's device arrays
+lloid_bank* make_part(lloid_bank* parent, int lo, int hi, double budget)
+{
+  lloid_bank* c = new (std::nothrow) lloid_bank();
+  if (!c) return nullptr;
+  c->cfg = parent->cfg; c->cfg.n_bins = hi - lo;
+  c->f16 = parent->f16; c->parent = parent; c->bin_base = lo; c->budget = budget;
+  c->bins.assign(parent->bins.begin() + lo, parent->bins.begin() + hi);
+  const int D = parent->cfg.n_detectors;
+  int first = 0;
+  for (int bi = lo; bi < hi; ++bi) {
+    const BinHost& B = parent->bins[bi];
+    c->max_templates = std::max(c->max_templates, B.N);
+    c->max_rows_pad = std::max(c->max_rows_pad, B.rows_pad);
+    for (const SliceHost& S : B.slices) c->d_max = std::max(c->d_max, S.d);
+    for (int det = 0; det < D; ++det) {
+      BinParams bp = parent->bp_host[(size_t)bi * D + det];
+      const int src = bp.first_slice;
+      bp.first_slice = first;
+      c->bp_host.push_back(bp);
+      for (int s = 0; s < B.S; ++s) {
+        SliceParams P = parent->sp_host[src + s];
+        P.bin = bi - lo;
+        c->sp_host.push_back(P);
+      }
+      first += B.S;
+    }
+  }
+  c->n_bd = (hi - lo) * D;
+  c->uploaded.assign(c->sp_host.size(), 1);
+  return c;
+}
+
+}  // namespace
+
+extern "C" {
+
 int lloid_bank_finalize(lloid_bank_t* b)
 {
   if (!b) return fail(LLOID_EINVAL, "null bank");
@@ -462,6 +559,62 @@ int lloid_bank_finalize(lloid_bank_t* b)
   for (size_t i = 0; i < b->uploaded.size(); ++i)
     if (!b->uploaded[i]) return fail(LLOID_ESTATE, "bin %d detector %d slice %d was never uploaded",
                                      b->sp_host[i].bin, b->sp_host[i].det, b->sp_host[i].slice);
+  CU(cudaSetDevice(b->cfg.device));
+  // Split?  fp16 path with automatic chunking only, when memory (not the 2^17 cap) would bound the chunk below kSplitChunk.
+  const int n_bins = b->cfg.n_bins;
+  if (b->f16 && b->cfg.max_chunk == 0 && n_bins >= 2 && !getenv("LLOID_NO_SPLIT")) {
+    size_t mem_free = 0, mem_total = 0;
+    CU(cudaMemGetInfo(&mem_free, &mem_total));
+    double budget = 0.5 * (double)mem_free;
+    budget = std::min(std::max(budget, 4.0 * 1024 * 1024 * 1024), 96.0 * 1024 * 1024 * 1024);
+    const double per_sample = intermediates_per_sample(b, 0, n_bins);
+    int n_parts = 1;
+    if (getenv("LLOID_PARTS")) n_parts = atoi(getenv("LLOID_PARTS"));                    // tests and A/B measurements
+    else if (budget / per_sample < (double)kSplitChunk) n_parts = (int)std::ceil(per_sample * (double)kSplitChunk / budget);
+    n_parts = std::max(1, std::min(n_parts, n_bins));
+    if (n_parts > 1) {
+      // contiguous ranges of bins with (nearly) equal shares of the intermediates, at least one bin each
+      std::vector<double> cum(n_bins + 1, 0.0);
+      for (int bi = 0; bi < n_bins; ++bi) cum[bi + 1] = cum[bi] + intermediates_per_sample(b, bi, bi + 1);
+      int lo = 0;
+      for (int part = 0; part < n_parts; ++part) {
+        int hi = lo + 1;
+        const int hi_max = n_bins - (n_parts - 1 - part);            // leave one bin for every part still to come
+        while (hi < hi_max && cum[hi + 1] <= cum[n_bins] * (part + 1) / n_parts * (1.0 + 1e-9)) ++hi;
+        if (part == n_parts - 1) hi = n_bins;
+        lloid_bank* c = make_part(b, lo, hi, budget);
+        if (!c) return fail(LLOID_ENOMEM, "out of host memory");
+        b->parts.push_back(c);
+        for (int bi = lo; bi < hi; ++bi) b->part_of_bin.push_back(part);
+        lo = hi;
+      }
+      // largest first: the shared chunk-local buffers are sized by the first part that asks
+      std::vector<int> order(n_parts);
+      for (int i = 0; i < n_parts; ++i) order[i] = i;
+      std::sort(order.begin(), order.end(), [&](int x, int y) {
+        const lloid_bank *X = b->parts[x], *Y = b->parts[y];
+        return cum[X->bin_base + X->cfg.n_bins] - cum[X->bin_base] > cum[Y->bin_base + Y->cfg.n_bins] - cum[Y->bin_base];
+      });
+      for (int i : order) {
+        const int rc = finalize_impl(b->parts[i]);
+        if (rc) return rc;
+      }
+      b->C = b->parts[0]->C; b->H = b->parts[0]->H; b->S = b->parts[0]->S;
+      for (const lloid_bank* c : b->parts) { b->C = std::min(b->C, c->C); b->H = std::max(b->H, c->H); }
+      int rc = dev_alloc(b, (void**)&b->stage_count, 8, true); if (rc) return rc;
+      b->finalized = true;
+      return LLOID_OK;
+    }
+  }
+  return finalize_impl(b);
+}
+
+}  // extern "C"
+
+namespace {
+
+int finalize_impl(lloid_bank* b)
+{
   CU(cudaSetDevice(b->cfg.device));
   const int D = b->cfg.n_detectors, Kd = b->cfg.k_down, Ku = b->cfg.k_up;
   const size_t esize = b->f16 ? 2 : 4;
@@ -489,6 +642,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
     // BASELINE config 2 (2 (bin, detector) pairs): 131072 samples = 1.2 GB; config 4 (3000 pairs): 7680 samples = 60 GB.
     double budget = 0.5 * (double)mem_free;
     budget = std::min(std::max(budget, 4.0 * 1024 * 1024 * 1024), 96.0 * 1024 * 1024 * 1024);
+    if (b->parent) budget = b->budget;                    // a part: the parent's figure (the parts share the buffers)
     C = (int64_t)(budget / ybytes_per_sample) / 2048 * 2048;
     C = std::min<int64_t>(std::max<int64_t>(C, 2048), 131072);
     if (b->f16 && C < 32768) {
@@ -528,7 +682,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
           need += (double)D * ((std::ceil(((double)C / S.d + 2 * Ku) / 128.0) * 16 + 16) * 8) * B.rows_pad * 2.0;
         }
       }
-    if (need > 0.95 * (double)mem_free)
+    if (need > 0.95 * (double)mem_free + (b->parent ? (double)(b->parent->scratch[0].cap + b->parent->scratch[1].cap) : 0.0))
       return fail(LLOID_ENOMEM, "bank does not fit: chunk-local intermediates need %.1f GB at a chunk of %lld samples, %.1f GB of device memory are free "
                                 "(reduce max_chunk, the number of bins per bank, or shard the bins over more GPUs)", need * 1e-9, (long long)C, (double)mem_free * 1e-9);
   }
@@ -585,7 +739,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
     R.jj_hi_off = std::max(R.jj_hi_off, (S.d == 1) ? P.jjY0 : P.jjY0 + 2 * Ku - 1);
     ybytes += round_up((size_t)P.y_rows_cap * S.L_pad * esize, 256);
   }
-  char* ybase; rc = dev_alloc(b, (void**)&ybase, ybytes, true); if (rc) return rc;
+  char* ybase; rc = scratch_alloc(b, 0, (void**)&ybase, ybytes, true); if (rc) return rc;
   size_t yoff = 0;
   if (!b->f16) {
     for (SliceParams& P : b->sp_host) {
@@ -673,7 +827,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
     const double* up_w[kMaxRates];
     for (int l2 = 0; l2 < kMaxRates; ++l2) up_w[l2] = upw64[l2].empty() ? nullptr : upw64[l2].data();
     b->plan16 = f16_plan_create(b->sp_host.data(), (int)b->sp_host.size(), b->fir_host.data(), (int)b->fir_host.size(),
-                                b->bp_host.data(), b->n_bd, D, b->C, up_w, &b->bytes, err, sizeof err);
+                                b->bp_host.data(), b->n_bd, D, b->C, up_w, b->parent ? plan_scratch_alloc : nullptr, b, &b->bytes, err, sizeof err);
     if (!b->plan16) return fail(LLOID_ECUDA, "fp16 plan: %s", err);
   }
   const uint8_t* excl = b->f16 ? f16_plan_excluded(b->plan16) : nullptr;   // mixed bank: only these bins use the FFMA kernels
@@ -713,7 +867,7 @@ int lloid_bank_finalize(lloid_bank_t* b)
     b->gt = tensor ? f16_granule_tiles(b->cfg.peak_window) : 1;
     const bool per_tile = !tensor || excl != nullptr;
     b->slots_cap = per_tile ? b->tiles_cap : (int)(C / kTimeTile) / b->gt + 2;
-    rc = dev_alloc(b, (void**)&b->partials, nstate * b->slots_cap * sizeof(Peak), true); if (rc) return rc;
+    rc = scratch_alloc(b, 2, (void**)&b->partials, nstate * b->slots_cap * sizeof(Peak), true); if (rc) return rc;
     if (tensor) {
       std::vector<int32_t> stl(b->n_bd, b->gt);
       if (excl) for (int bd = 0; bd < b->n_bd; ++bd) if (excl[bd]) stl[bd] = 1;
@@ -725,6 +879,10 @@ int lloid_bank_finalize(lloid_bank_t* b)
   return LLOID_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
 int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trigger_t* trig, int64_t capacity,
                  int64_t* count_dev, void* stream)
 {
@@ -735,9 +893,30 @@ int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trig
   if (capacity < 0) return fail(LLOID_EINVAL, "negative capacity");
   cudaStream_t st = (cudaStream_t)stream;
   CU(cudaSetDevice(b->cfg.device));
+  CU(cudaMemsetAsync(count_dev, 0, 8, st));
+  if (!b->parts.empty()) {
+    // split bank: the parts filter the same buffer one after the other and append to the same trigger list
+    b->last_launches = 0;
+    for (lloid_bank* c : b->parts) {
+      const int rc = filter_one(c, strain_dev, n, trig, capacity, count_dev, st);
+      if (rc) return rc;
+      b->last_launches += c->last_launches;
+    }
+    b->consumed = b->parts[0]->consumed;
+    return LLOID_OK;
+  }
+  return filter_one(b, strain_dev, n, trig, capacity, count_dev, st);
+}
+
+}  // extern "C"
+
+namespace {
+
+// one bank (or one part of a split bank): the caller has validated the arguments and cleared the count
+int filter_one(lloid_bank* b, const float* strain_dev, int64_t n, lloid_trigger_t* trig, int64_t capacity, int64_t* count_dev, cudaStream_t st)
+{
   b->last_launches = 0;
   b->events_used = 0;
-  CU(cudaMemsetAsync(count_dev, 0, 8, st));
   int64_t k = b->consumed, off = 0, rem = n;
   b->call_start = k;
   while (rem > 0) {
@@ -762,6 +941,10 @@ int lloid_filter(lloid_bank_t* b, const float* strain_dev, int64_t n, lloid_trig
   return LLOID_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
 int lloid_graph_safe(const lloid_bank_t* b, int64_t n)
 {
   if (!b || !b->finalized || n <= 0) return 0;
@@ -776,6 +959,7 @@ int lloid_graph_advance(lloid_bank_t* b, int64_t n)
   if (!b || !b->finalized) return fail(LLOID_ESTATE, "graph_advance before finalize");
   if (!lloid_graph_safe(b, n)) return fail(LLOID_EINVAL, "graph replay needs n_samples and the running sample count to be multiples of the peak window");
   b->consumed += n;
+  for (lloid_bank* c : b->parts) c->consumed += n;
   return LLOID_OK;
 }
 
@@ -820,6 +1004,11 @@ int lloid_reset(lloid_bank_t* b, void* stream)
   if (!b->finalized) return fail(LLOID_ESTATE, "reset before finalize");
   cudaStream_t st = (cudaStream_t)stream;
   CU(cudaSetDevice(b->cfg.device));
+  if (!b->parts.empty()) {
+    for (lloid_bank* c : b->parts) { const int rc = lloid_reset(c, stream); if (rc) return rc; }
+    b->consumed = 0;
+    return LLOID_OK;
+  }
   CU(cudaMemsetAsync(b->hist, 0, (size_t)b->cfg.n_detectors * b->H * 4, st));
   CU(cudaMemsetAsync(b->k_base_dev, 0, 8, st));
   launch_reset_state(b->state, 2 * (int64_t)b->n_bd * b->max_templates, st);
@@ -830,6 +1019,13 @@ int lloid_reset(lloid_bank_t* b, void* stream)
 int lloid_debug_capture(lloid_bank_t* b, int32_t bin, int32_t det, int64_t k_begin, int64_t n, float* snr_dev)
 {
   int rc = check_ids(b, bin, det, 0); if (rc) return rc;
+  if (!b->parts.empty()) {
+    if (!b->finalized) return fail(LLOID_ESTATE, "capture before finalize");
+    for (lloid_bank* c : b->parts) c->cap = Capture{nullptr, 0, 0, -1, 0};
+    if (!snr_dev) return LLOID_OK;
+    lloid_bank* c = b->parts[b->part_of_bin[bin]];
+    return lloid_debug_capture(c, bin - c->bin_base, det, k_begin, n, snr_dev);
+  }
   if (!snr_dev) { b->cap = Capture{nullptr, 0, 0, -1, 0}; return LLOID_OK; }
   if (n <= 0) return fail(LLOID_EINVAL, "capture length must be positive");
   b->cap.snr = snr_dev; b->cap.k_begin = k_begin; b->cap.n = n;
@@ -840,12 +1036,19 @@ int lloid_debug_capture(lloid_bank_t* b, int32_t bin, int32_t det, int64_t k_beg
 int64_t lloid_samples_consumed(const lloid_bank_t* b) { return b ? b->consumed : -1; }
 int64_t lloid_chunk_samples(const lloid_bank_t* b) { return b ? b->C : -1; }
 int64_t lloid_last_launch_count(const lloid_bank_t* b) { return b ? b->last_launches : -1; }
-int64_t lloid_device_bytes(const lloid_bank_t* b) { return b ? b->bytes : -1; }
+int64_t lloid_device_bytes(const lloid_bank_t* b)
+{
+  if (!b) return -1;
+  int64_t v = b->bytes;
+  for (const lloid_bank* c : b->parts) v += c->bytes;
+  return v;
+}
 
 int lloid_set_profiling(lloid_bank_t* b, int32_t enable)
 {
   if (!b) return fail(LLOID_EINVAL, "null bank");
   b->prof = enable != 0; b->events_used = 0;
+  for (lloid_bank* c : b->parts) { c->prof = b->prof; c->events_used = 0; }
   return LLOID_OK;
 }
 
@@ -853,6 +1056,14 @@ int lloid_last_stage_ms(lloid_bank_t* b, float* out)
 {
   if (!b || !out) return fail(LLOID_EINVAL, "null argument");
   for (int i = 0; i < 6; ++i) out[i] = 0.f;
+  if (!b->parts.empty()) {                         // split bank: the parts ran back to back; their stage times add up
+    for (lloid_bank* c : b->parts) {
+      float v[6];
+      const int rc = lloid_last_stage_ms(c, v); if (rc) return rc;
+      for (int i = 0; i < 6; ++i) out[i] += v[i];
+    }
+    return LLOID_OK;
+  }
   if (!b->prof || b->events_used < 2) return fail(LLOID_ESTATE, "profiling was not enabled for the last call");
   CU(cudaEventSynchronize(b->events[b->events_used - 1]));
   for (size_t i = 1; i < b->events_used; ++i) {
@@ -876,6 +1087,15 @@ int lloid_path_info(const lloid_bank_t* b, int32_t* out)
   if (!b || !out) return fail(LLOID_EINVAL, "null argument");
   if (!b->finalized) return fail(LLOID_ESTATE, "path info before finalize");
   out[0] = out[1] = out[2] = out[3] = 0;
+  if (!b->parts.empty()) {                         // split bank: all parts on the tensor kernels / any with R in TMEM / sums
+    out[0] = 1;
+    for (const lloid_bank* c : b->parts) {
+      int32_t v[4];
+      const int rc = lloid_path_info(c, v); if (rc) return rc;
+      out[0] &= v[0]; out[1] |= v[1]; out[2] += v[2]; out[3] += v[3];
+    }
+    return LLOID_OK;
+  }
   if (b->f16 && b->plan16) {
     out[0] = f16_plan_tensor_recon(b->plan16) ? 1 : 0;
     out[1] = f16_plan_r_tmem(b->plan16) ? 1 : 0;
@@ -891,6 +1111,7 @@ void lloid_destroy(lloid_bank_t* b)
   if (!b) return;
   cudaSetDevice(b->cfg.device);
   cudaDeviceSynchronize();
+  for (lloid_bank* c : b->parts) lloid_destroy(c);  // before the parent's arrays, which they point into
   if (b->plan16) f16_plan_destroy(b->plan16);
   for (void* p : b->owned) cudaFree(p);
   if (b->stage_strain) cudaFree(b->stage_strain);

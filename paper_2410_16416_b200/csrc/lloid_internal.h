@@ -130,8 +130,8 @@ void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, 
                           int slots_cap, const int32_t* slot_tiles_dev, int c, int64_t k_a /* host copy: launch geometry */,
                           const long long* k_base_dev /* first sample of the call, device */, int64_t k_off /* chunk - call start */,
                           int W, float theta,
-                          const PeakState* state_in, PeakState* state_out, int n_det, void* triggers, int64_t capacity,
-                          unsigned long long* count, cudaStream_t st, int64_t* launches);
+                          const PeakState* state_in, PeakState* state_out, int n_det, int bin_base /* added to the bin index of every trigger */,
+                          void* triggers, int64_t capacity, unsigned long long* count, cudaStream_t st, int64_t* launches);
 void launch_advance_counter(long long* k_base_dev, int64_t n, cudaStream_t st);
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
@@ -212,6 +212,7 @@ struct F16Plan;                    // opaque host-side plan: work lists, band ma
 F16Plan* f16_plan_create(const SliceParams* sp_host, int n_problems /* reconstruction view */,
                          const SliceParams* fir_host, int n_fir /* FIR problems */, const BinParams* bp_host, int n_bd,
                          int n_det, int chunk_cap, const double* const* up_w /* [kMaxRates]: w[(i+K_up) d + phi] or null */,
+                         void* (*q_alloc)(void*, size_t) /* rho^(d) buffers: zeroed device memory or null; nullptr = cudaMalloc */, void* q_ctx,
                          int64_t* bytes, char* err, int errlen);
 void f16_plan_destroy(F16Plan*);
 bool f16_plan_r_tmem(const F16Plan*);          // reconstruction kernels keep the stationary R in TMEM (K <= 512)

@@ -270,3 +270,54 @@ def test_two_banks_alive_and_interleaved_precisions():
             b_s16.close(); b_s32.close()
     finally:
         b_big.close()
+
+
+def _canon(t):
+    return t[np.lexsort((t["sample"], t["template_idx"], t["detector"], t["bin"]))]
+
+
+def test_split_bank_equals_whole_bank(monkeypatch):
+    """A bank whose chunk-local intermediates would not fit a long chunk is cut at finalize into parts (ranges of bins
+    that share one set of chunk buffers and run one after the other: lloid_api.cu).  Forced here with LLOID_PARTS on a
+    5-bin config-4 bank: same triggers, record for record, same captured SNR, in one call and in pieces."""
+    w = wl.config4(n_bins=5, n_templates=160, seconds=100, n_detectors=3, n_distinct=2)
+    W = w.peak_window
+    k0 = 66 * W
+    monkeypatch.setenv("LLOID_NO_SPLIT", "1")
+    whole, snr_w, info_w = pu.run_gpu(w, lb.LLOID_F16, capture=(3, 1, k0, W))
+    monkeypatch.delenv("LLOID_NO_SPLIT")
+    monkeypatch.setenv("LLOID_PARTS", "3")
+    parts, snr_p, info_p = pu.run_gpu(w, lb.LLOID_F16, capture=(3, 1, k0, W))
+    assert info_p["consumed"] == w.n_samples and info_p["counts"] == info_w["counts"], (info_p, info_w)
+    assert info_p["path"] == info_w["path"] and info_p["launches"] > info_w["launches"]
+    assert sorted(set(parts["bin"].tolist())) == [0, 1, 2, 3, 4]
+    assert _canon(parts).tobytes() == _canon(whole).tobytes()
+    assert np.array_equal(snr_p, snr_w)
+    host, _, _ = pu.run_gpu(w, lb.LLOID_F16, host_path=True)
+    assert _canon(host).tobytes() == _canon(whole).tobytes()
+    n = w.n_samples
+    pieces = [W * 30, 2048 * 7 + 64, n - W * 30 - 2048 * 7 - 64]        # history, window state and counters are per part
+    streamed, _, _ = pu.run_gpu(w, lb.LLOID_F16, pieces=pieces)
+    monkeypatch.delenv("LLOID_PARTS")
+    monkeypatch.setenv("LLOID_NO_SPLIT", "1")
+    streamed_whole, _, _ = pu.run_gpu(w, lb.LLOID_F16, pieces=pieces)
+    assert len(streamed) == len(whole)
+    assert _canon(streamed).tobytes() == _canon(streamed_whole).tobytes()
+
+
+def test_repeated_runs_are_bit_identical():
+    """The same bank on the same strain gives the same trigger records, bit for bit, run after run, in both reconstruction
+    modes (R in TMEM: the config-4 bank; R in shared memory: the config-2 bank).  Regression test for a race in the f0
+    kernel: an interpolation issuer waited for its own tile's window rows but not for the previous tile's (which the
+    other issuing thread had waited for), so about one SNR value in 10^8 was built from rows still in flight and a
+    handful of near-threshold triggers came and went between identical runs."""
+    banks = (wl.config4(n_bins=5, n_templates=160, seconds=100, n_detectors=3, n_distinct=2),
+             wl.config2(n_templates=256, seconds=200, n_detectors=2, n_basis=150, n_injections=2))
+    for w, rt in zip(banks, (True, False)):
+        first = None
+        for _ in range(5):
+            t, _, info = pu.run_gpu(w, lb.LLOID_F16)
+            assert info["path"]["r_in_tmem"] == rt
+            c = _canon(t).tobytes()
+            first = c if first is None else first
+            assert c == first

@@ -249,3 +249,16 @@ def test_minimal_buffers_and_count_only_calls(cfg1, precision):
     assert int(cnt.item()) == len(one)
     assert lb.lloid_check_count(int(cnt.item()), 0) == lb.LLOID_EOVERFLOW
     bank.close()
+
+
+def test_fp16_bank_outside_the_tensor_limits_runs_the_cuda_core_reconstruction():
+    """Three 512 Hz slices with L_pad = 320 each: K = 960 at one rate, more than the tensor reconstruction kernels hold.
+    The bin's FIR still runs on tcgen05; its reconstruction falls back, inside the library and on the GPU, to the FFMA
+    kernels reading the packed fp16 operands.  Same tolerance as every fp16 test."""
+    w = wl.toy(n_templates=150, M=5120, spans=((2048, 0.0, 0.25), (512, 0.25, 1.0), (512, 1.0, 1.75), (512, 1.75, 2.5)),
+               seconds=7.0, n_basis=[40, 290, 290, 290], f_low=20.0, mc=(1.0, 1.4))
+    w.peak_window = 512
+    n = w.n_samples
+    _, _, _, info, stats = _dense_check(w, lb.LLOID_F16, 6144, n)
+    assert info["path"]["cuda_core_bds"] == 1, info["path"]
+    assert stats["checked"] == 150 * ((n - 6144) // 512)
