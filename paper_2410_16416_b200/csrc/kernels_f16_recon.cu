@@ -66,7 +66,6 @@ struct LowUnit { int32_t group, pb; };
 __device__ long long g_trace[2][8][8];
 #ifdef LLOID_TRACE_BUILD
 __constant__ int g_exp;                      // scratch knock-outs: 1 no interpolation MMAs, 2 no y MMAs (f0), 4 no epilogue arithmetic (f0)
-__constant__ int g_fake_half_r;            // scratch experiment: f0 kernel keeps only the first slice's R in shared memory (wrong sums, same work)
 #endif      // [kernel: 0 low, 1 f0][role][0..5 wait categories, 6 total, 7 tiles]
 #ifdef LLOID_TRACE_BUILD
 #define TWAIT(cat, bar, ph)                                                                       \
@@ -139,16 +138,16 @@ __device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl
     else
 
 // ---- f0 kernel schedule ------------------------------------------------------------------------------------------
-// The flattened work sequence is ordered by time BLOCKS of gb tiles (aligned to absolute tile indices), then by template
-// block, then by (bin, detector), then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends moved
-// up to granule starts.  The clusters that reconstruct the n_pb template blocks of one (bin, detector, time block) -- from
-// the same y tiles -- are then T / n_pb apart in the sequence, i.e. G / n_pb clusters apart, and reach the same tile at the
-// same time: one of them reads a y tile from DRAM, the others find it in L2.  That holds for few long cells (config 2: a
-// block is one cluster's share, cluster i works on cell i) and for many short ones (config 4: 3000 (bin, detector) pairs
-// per chunk of 55 tiles; ordered by (bin, detector) first, a cluster walked the 8 template blocks of a pair one after the
-// other and every y tile came from DRAM 8 times: 3.5 GB of reads per launch for 1 GB of operands).
-// Needs the same number of template blocks for every (bin, detector) (n_pb > 0); otherwise (n_pb == 0) the order is
-// (bin, detector), time block, template block, tile.
+// The flattened work sequence is ordered by (bin, detector), then by time BLOCKS of gb tiles (aligned to absolute tile
+// indices), then by template block, then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends
+// moved up to granule starts.  With a block of one cluster's share (launch_recon_f16) cluster i works on about the i-th
+// (time block, template block) cell: the clusters that reconstruct the template blocks of one time block from the same y
+// tiles run side by side and all but one of them find a y tile in L2.
+// n_pb > 0 selects the order (time block, template block, (bin, detector), tile) instead -- meant for banks with many
+// (bin, detector) pairs per chunk, where a cluster walks the template blocks of a pair one after the other and y comes
+// from DRAM every time (config 4: 3 GB of reads per launch for 1 GB of operands).  It needs the same number of template
+// blocks for every pair.  Measured (LLOID_F0_ORDER_PB): clusters G / n_pb apart do not stay in step; DRAM reads 3.5 -> 3.0
+// GB on config 4, 0.88 -> 1.07 GB on config 2, no gain in time.  Kept, off.
 struct F0Sched {
   const SchedBd* bds;                       // tensor-path (bin, detector) pairs, in order
   int n_bds, n_tiles, gb, gt;
@@ -353,14 +352,8 @@ __device__ __forceinline__ void py_segment(YRing& rg, const YAddr ya, int& seg_i
   }
   auto load_R = [&]() {
     if (seg_i > 0) TWAIT(1, unit_done_u, (uint32_t)(seg_i - 1) & 1u);   // every MMA that reads the old R is complete
-#ifdef LLOID_TRACE_BUILD
-    const bool fake = g_fake_half_r && extra_dst != 0u;
-    const int n_r = fake ? 1 : sg.n;
-    mbar_expect_tx(consts_u, (fake ? (uint32_t)sg.nm[0] * 4096u : sg.rbytes) + (seg_i == 0 ? extra_bytes : 0u));
-#else
     const int n_r = sg.n;
     mbar_expect_tx(consts_u, sg.rbytes + (seg_i == 0 ? extra_bytes : 0u));
-#endif
     uint32_t off = 0;
     for (int i = 0; i < n_r; ++i) {
       copy_pieces(sR_u + off, sg.Rsrc[i], (uint32_t)sg.nm[i] * 4096u, consts_u);
@@ -474,9 +467,6 @@ __device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, uint64_t mlis
     { TSPAN_BEGIN(); commit2(ya.empty0 + 8u * rg.s, 3); TSPAN_END(4); }
     acc = 1u;
     a_lo += (uint32_t)m * (RT ? 8u : 256u);
-#ifdef LLOID_TRACE_BUILD
-    if (!RT && g_fake_half_r && a_lo >= a_base + 2560u) a_lo -= 2560u;      // experiment: config 2 only (10 MMAs = 40 KB)
-#endif
     rg.advance();
   }
 }
@@ -641,6 +631,7 @@ struct F0PArgs {
   const uint8_t* P;                                     // [2][p_bytes]: band-matrix blob of rank 0, of rank 1
   Peak* partials; Capture cap; long long k_a;
   int n_lr, c, r_bytes, p_bytes, q_bytes, nsy, ystage, ycap, slots_cap, max_templates, trace;
+  uint32_t q_gate;                                      // bits of theta^2 (1 - 2^-16): |rho|^2 at or below it cannot trigger
   F0Sched sched;
   PairRate rate[kNLowRates];
   PairMma tab[kPairTabMax];                             // interpolation MMAs, see PairMma
@@ -944,6 +935,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         __syncwarp();
         if (lane == 0) mbar_arrive_cluster(r_ready_u & kLeaderMask);
       }
+      int g_left = gt - (int)((a0 + t0) % gt);                           // tiles to the end of the current granule (absolute grid)
       uint32_t bqt[2] = {0u, 0u};                                       // running maximum of the granule (truncated bits)
       int bk[2] = {0, 0};
       float bre[2] = {0.f, 0.f}, bim[2] = {0.f, 0.f};
@@ -992,15 +984,26 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
             asm("mov.b64 %0, {%1, %2};" : "=l"(im2) : "r"(r[4 * i + 2]), "r"(r[4 * i + 3]));
             asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(q2) : "l"(im2));
             asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(q2) : "l"(re2));
-            uint32_t q0, q1;
-            asm("mov.b64 {%0, %1}, %2;" : "=r"(q0), "=r"(q1) : "l"(q2));
-            code[2 * i] = (q0 & ~15u) | (uint32_t)(15 - 2 * i);
-            code[2 * i + 1] = (q1 & ~15u) | (uint32_t)(14 - 2 * i);
+            asm("mov.b64 {%0, %1}, %2;" : "=r"(code[2 * i]), "=r"(code[2 * i + 1]) : "l"(q2));
           }
           if (valid < 128) {
 #pragma unroll
             for (int j = 0; j < 16; ++j) if (cthr + 8 * (j >> 1) + (j & 1) >= valid) code[j] = 0u;
           }
+          // Gate: only a value above the threshold can become a trigger, and only one above the granule's running maximum
+          // changes it.  The plain maximum of the 16 |rho|^2 (8 instructions) against max(theta^2 (1 - 2^-16), running
+          // maximum) decides for the whole warp whether the index bookkeeping below (pack, 15 maxima, select tree: 80 of the
+          // 150 instructions per half tile) runs at all; at theta = 4 in noise it does for one warp in six.  A granule without
+          // any value above the threshold leaves a record with q = 0, which the merge kernel never turns into a trigger.
+          {
+            uint32_t mx = max(max(code[0], code[1]), code[2]);
+#pragma unroll
+            for (int j = 3; j < 15; j += 2) mx = max(max(mx, code[j]), code[j + 1]);
+            mx = max(mx, code[15]);
+            if (!__any_sync(0xffffffffu, mx > max(a.q_gate, bqt[h]))) continue;
+          }
+#pragma unroll
+          for (int j = 0; j < 16; ++j) code[j] = (code[j] & ~15u) | (uint32_t)(15 - j);
 #pragma unroll
           for (int st = 8; st >= 1; st >>= 1)
 #pragma unroll
@@ -1022,8 +1025,9 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
           }
         }
         // granule end: merge the partial maxima of a template (4 threads x 2 column halves), write one record
-        const long long at = a0 + t;
-        if (t + 1 == t1 || (at + 1) % gt == 0) {
+        if (t + 1 == t1 || --g_left == 0) {                                  // (no 64-bit division per tile: a countdown)
+          g_left = gt;
+          const long long at = a0 + t;
           const int fp = flush_i & 1;
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
@@ -1215,11 +1219,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   // windows and >= 3 y stages: if EVERY (bin, detector) fits that way the bank runs the RT = false kernels; otherwise the
   // whole bank runs the RT = true kernels (R in TMEM, K <= 512), and only what exceeds THAT is left to the FFMA kernels.
   {
-#ifdef LLOID_TRACE_BUILD
-    const int lim_f0_smem = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / (getenv("LLOID_FAKE_HALF_R") ? 128 : 256);
-#else
     const int lim_f0_smem = (PK_SMEM_BUDGET - pl->p_bytes - pl->q_bytes - 3 * 16384) / 256;
-#endif
     const int lim_low_smem = (PK_SMEM_BUDGET - 3 * 16384) / 256;
     bool rt = false;
     for (int b = 0; b < n_bd; ++b) {
@@ -1242,13 +1242,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     }
     if (pl->combos_host.empty()) return true;             // nothing fits: the whole bank goes to the FFMA kernels
   }
-#ifdef LLOID_TRACE_BUILD
-  const int fake_half = getenv("LLOID_FAKE_HALF_R") ? 1 : 0;
-  cudaMemcpyToSymbol(g_fake_half_r, &fake_half, sizeof(int));
-  const int f0_fixed = (pl->r_tmem ? 0 : pl->l_sum_f0_max * (fake_half ? 128 : 256)) + pl->p_bytes + pl->q_bytes;
-#else
   const int f0_fixed = (pl->r_tmem ? 0 : pl->l_sum_f0_max * 256) + pl->p_bytes + pl->q_bytes;
-#endif
   const int low_fixed = pl->r_tmem ? 0 : pl->l_sum_low_max * 256;
   // y stage slot: the largest stage of any unit the kernel streams (a unit with nm = sum L_pad / 16 MMAs per tile is cut
   // into ceil(nm / ycap) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
@@ -1377,7 +1371,7 @@ int f16_granule_tiles(int peak_window)
 }
 
 int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int slots_cap, int max_templates,
-                     int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
+                     int c, int64_t k_a, int gt, float theta, Capture cap, cudaStream_t st, int64_t* launches, cudaEvent_t after_lowrate)
 {
   const int n_clusters = std::max(1, pl->n_sm / 2);
 #ifdef LLOID_TRACE_BUILD
@@ -1409,11 +1403,7 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
   a.sp = sp_dev; a.bd = pl->bd_dev; a.groups = pl->groups_dev;
   a.P = reinterpret_cast<const uint8_t*>(pl->p_dev);
   a.partials = partials; a.cap = cap; a.k_a = k_a;
-  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; 
-#ifdef LLOID_TRACE_BUILD
-  if (getenv("LLOID_FAKE_HALF_R")) a.r_bytes /= 2;
-#endif
-  a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
+  a.n_lr = pl->n_lr; a.c = c; a.r_bytes = pl->l_sum_f0_max * 256; a.p_bytes = pl->p_bytes; a.q_bytes = pl->q_bytes;
   a.nsy = pl->f0_stages; a.ystage = pl->f0_ystage; a.ycap = pl->ycap; a.slots_cap = slots_cap; a.max_templates = max_templates;
   a.trace = getenv("LLOID_TRACE") ? 1 : 0;
   const int n_tiles = (c + 127) / 128;
@@ -1430,7 +1420,11 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     a.sched.gt = gt; a.sched.gb = (int)std::min<long long>(gb, (long long)(n_tiles + gt - 1) / gt * gt + gt);
   }
   a.sched.total = pl->f0_wsum; a.sched.a0 = k_a / kTimeTile;
-  a.sched.n_pb = getenv("LLOID_F0_ORDER_BD") ? 0 : pl->f0_n_pb;
+  a.sched.n_pb = getenv("LLOID_F0_ORDER_PB") ? pl->f0_n_pb : 0;          // template-block-major order: measured, no gain (see F0Sched)
+  {
+    const float g = theta * theta * (1.0f - 1.0f / 65536.0f);
+    a.q_gate = getenv("LLOID_NO_GATE") ? 0u : *reinterpret_cast<const uint32_t*>(&g);
+  }
   for (int r = 0; r < kNLowRates; ++r) a.rate[r] = pl->rate[r];
   memcpy(a.tab, pl->tab, sizeof a.tab);
   const long long pair_tiles = (long long)pl->combos_host.size() * n_tiles;

@@ -304,7 +304,7 @@ int process_chunk(lloid_bank* b, int o, int c, int64_t k_a, lloid_trigger_t* tri
     mark(b, st, kTagFir);
     if (int rc = debug_sync("fir_f16_kernel", k_a, st)) return rc;
     if (f16_plan_tensor_recon(b->plan16)) {
-      if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->slots_cap, b->max_templates, c, k_a, b->gt, b->cap, st,
+      if (launch_recon_f16(b->plan16, b->sp_dev, b->partials, b->slots_cap, b->max_templates, c, k_a, b->gt, b->cfg.snr_threshold, b->cap, st,
                            &b->last_launches, grab(b, kTagLowRecon)))
         return fail(LLOID_ECUDA, "fp16 reconstruction launch failed: %s", cudaGetErrorString(cudaGetLastError()));
       if (b->q32_dev) {                              // mixed bank: the bins outside the tensor kernels' limits

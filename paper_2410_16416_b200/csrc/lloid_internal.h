@@ -226,7 +226,7 @@ int  launch_fir_f16(F16Plan*, const SliceParams* sp_dev, const SliceParams* sp_h
 int  f16_granule_tiles(int peak_window);
 int  f16_read_trace(long long* out /* [2][8][8] */, int reset);
 int  launch_recon_f16(F16Plan*, const SliceParams* sp_dev, Peak* partials, int slots_cap, int max_templates,
-                      int c, int64_t k_a, int gt, Capture cap, cudaStream_t st, int64_t* launches,
+                      int c, int64_t k_a, int gt, float theta /* snr threshold: the epilogue's gate */, Capture cap, cudaStream_t st, int64_t* launches,
                       cudaEvent_t after_lowrate /* recorded between the two kernels when non-null */);
 
 }  // namespace lloid
