@@ -230,11 +230,14 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
   PeakState s;
   if (w * W < k_a) s = state_in[(size_t)bd * max_templates + p];      // window began in an earlier chunk
   else { s.q = -1.f; s.re = 0.f; s.im = 0.f; s.pad = 0; s.k = -1; }
-  // partial slots: runs of gt tiles aligned to absolute multiples of gt tiles (gt = 1: one slot per tile)
-  const int gt = slot_tiles ? slot_tiles[bd] : 1;
+  // partial slots: runs of gt tiles aligned to absolute multiples of gt tiles (gt = 1: one slot per tile), n_rec records per
+  // run (the tensor f0 kernel's two epilogue groups write one each: slot_tiles = gt | 1 << 16).  Records of a run are not
+  // in time order: the larger |rho|^2 wins, the earlier sample on a tie (R8).
+  const int st = slot_tiles ? slot_tiles[bd] : 1;
+  const int gt = st & 0xffff, n_rec = (st >> 16) ? 2 : 1;
   const long long a0 = k_a / kTimeTile;
   const int t_lo = (int)((lo - k_a) / kTimeTile), t_hi = (int)((hi - k_a + kTimeTile - 1) / kTimeTile);   // tiles [t_lo, t_hi)
-  const int g0 = (int)((a0 + t_lo) / gt - a0 / gt), g1 = (int)((a0 + t_hi - 1) / gt - a0 / gt) + 1;
+  const int g0 = n_rec * (int)((a0 + t_lo) / gt - a0 / gt), g1 = n_rec * ((int)((a0 + t_hi - 1) / gt - a0 / gt) + 1);
   const Peak* __restrict__ pp = partials + ((size_t)bd * slots_cap + g0) * max_templates + p;
   for (int g = g0; g < g1; g += 8) {               // 8 independent 16-byte loads in flight per thread, then the ordered compare
     float4 v[8];
@@ -242,8 +245,10 @@ merge_windows_kernel(const BinParams* __restrict__ bp, int max_templates, const 
     for (int i = 0; i < 8; ++i)
       v[i] = (g + i < g1) ? __ldcs(reinterpret_cast<const float4*>(pp + (size_t)i * max_templates)) : make_float4(-2.f, 0.f, 0.f, 0.f);
 #pragma unroll
-    for (int i = 0; i < 8; ++i)                     // Peak = {q, kappa, re, im}
-      if (v[i].x > s.q) { s.q = v[i].x; s.re = v[i].z; s.im = v[i].w; s.k = k_a + __float_as_int(v[i].y); }
+    for (int i = 0; i < 8; ++i) {                   // Peak = {q, kappa, re, im}
+      const long long k = k_a + __float_as_int(v[i].y);
+      if (v[i].x > s.q || (v[i].x == s.q && k < s.k)) { s.q = v[i].x; s.re = v[i].z; s.im = v[i].w; s.k = k; }
+    }
     pp += (size_t)8 * max_templates;
   }
   const bool complete = (w + 1) * W <= k_a + c;

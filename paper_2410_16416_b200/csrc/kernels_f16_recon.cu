@@ -253,7 +253,7 @@ struct PairBars {
 // Barrier counts: a "full" barrier of the leader gets its own producers' arrive.expect_tx plus the peer's relay, the peer's
 // own copy only its producers'.  acc_empty lives in the leader: one arrival per epilogue warp of both CTAs.  unit_done is
 // committed by the thread that finishes the unit's LAST tile, after it has seen the other thread's last tile complete.
-__device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int nsy, uint32_t rank, int warp, int tid, uint32_t n_pq)
+__device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int nsy, uint32_t rank, int warp, int tid, uint32_t n_pq, uint32_t n_drain)
 {
   if (warp == 0) tmem_alloc2(tmem_slot, 512);
   if (tid == 32) {
@@ -262,7 +262,7 @@ __device__ __forceinline__ void pair_setup(PairBars& B, uint32_t* tmem_slot, int
     for (int s = 0; s < nsy; ++s) { mbar_init(smem_u32(&B.yfull[s]), 1u + relay); mbar_init(smem_u32(&B.yempty[s]), 1); }
     for (int s = 0; s < PK_NQB; ++s) { mbar_init(smem_u32(&B.qfull[s]), n_pq + relay); mbar_init(smem_u32(&B.qempty[s]), 1); }
     for (int b = 0; b < PK_NACC_MAX; ++b) {
-      mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), 16); mbar_init(smem_u32(&B.ybar[b]), 1);
+      mbar_init(smem_u32(&B.acc_full[b]), 1); mbar_init(smem_u32(&B.acc_empty[b]), n_drain); mbar_init(smem_u32(&B.ybar[b]), 1);
     }
     mbar_init(smem_u32(&B.consts), 1u + relay);
     mbar_init(smem_u32(&B.unit_done), 1);
@@ -496,7 +496,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   if (u_lo == u_hi && t_lo == t_hi) return;             // both CTAs of the cluster take the same decision
 
   const int nsy = a.nsy;
-  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 1u);
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 1u, 16u);          // all 8 epilogue warps of both CTAs drain every tile
   const uint32_t tmem = tmem_slot;
   constexpr uint32_t NACC = Acc<RT>::N;
   const uint32_t sR_u = smem_u32(smem);                 // !RT: [l_sum / 8][128 rows][8] fp16
@@ -646,7 +646,6 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   __shared__ uint32_t tmem_slot;
   __shared__ SegSrc seg[3];                             // [0] PY, [1] IY, [2] relay
   __shared__ F0Pos s_pos[2];
-  __shared__ __align__(16) Peak s_x[2][64];             // epilogue: second column half -> first, per flush parity
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t rank = cluster_ctarank();
@@ -668,7 +667,7 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   const uint32_t sP_u = sR_u + (RT ? 0u : (uint32_t)a.r_bytes);     // this rank's band-matrix blocks
   const uint32_t sQ_u = sP_u + (uint32_t)a.p_bytes;     // per-rate circular buffers of 16-row chunks (4 KB each)
   const uint32_t ring_u = sQ_u + (uint32_t)a.q_bytes;   // y ring
-  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 2u);
+  pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 2u, 8u);           // 4 epilogue warps of each CTA drain a tile (the two groups alternate)
   const uint32_t tmem = tmem_slot;
   const uint32_t consts_u = smem_u32(&bars.consts), unit_done_u = smem_u32(&bars.unit_done), r_ready_u = smem_u32(&bars.r_ready);
   const uint32_t progress_u = smem_u32(&bars.py_tiles);
@@ -914,20 +913,27 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
   } else if (warp >= 8 && warp < 16) {
     // ===== epilogue.  16x256b TMEM loads: thread T of a warp holds, for lanes l = T / 4 (cosine row of a template) and
     // l + 8 (its sine row, see r16_lane), the columns 8 i + 2 (T % 4) + {0, 1}: |rho|^2 without any cross-lane traffic.
-    // Warps 8-11 take columns [0, 64) of the tile, 12-15 columns [64, 128); a warp covers its lane quarter with two loads
-    // (h = 0, 1), so a thread works on two templates x 16 columns per tile.  The maximum of the 16 |rho|^2 is found with
-    // the column index packed into the 4 low mantissa bits (15 - j: the lowest column wins a tie; the truncation is
-    // 2^-19 relative), 15 integer maxima and a 4-level select tree instead of 16 compare / 4-select updates. =====
+    // Two GROUPS of four warps (one per TMEM lane quarter) take alternate tiles -- group = parity of the ABSOLUTE tile index,
+    // so that the result does not depend on how the stream was cut into chunks -- and a warp walks the tile's two column
+    // halves with two loads each (h = 0, 1: lanes 0-15 / 16-31 of its quarter).  With all eight warps on every tile they
+    // all sat through the same barrier and TMEM-load latencies together (issue slots 21 % used); now one group computes
+    // while the other waits.  The maximum of 16 |rho|^2 is found with the column index packed into the 4 low mantissa bits
+    // (15 - j: the lowest column wins a tie; the truncation is 2^-19 relative), 15 integer maxima and a 4-level select tree.
+    // Each group keeps a running maximum per template over its tiles of a granule and writes its own record
+    // (slot 2 granule + group); the merge kernel takes the larger one, the earlier sample on a tie. =====
     const int q = warp & 3, wg = (warp - 8) >> 2, tq = lane >> 2, tc = lane & 3;
     const uint32_t acc_empty_leader = smem_u32(&bars.acc_empty[0]) & kLeaderMask;
-    uint32_t e = 0, flush_i = 0;
+    uint32_t e = 0;
     TRACE_BEGIN();
     FOR_F0_SEGMENTS(it, S, pA, pB) {
       const int t0 = it.cur.t, t1 = it.seg_end(), bdi = S.bds[it.cur.ib].bd;
       const int n_templates = a.bd[bdi].n_templates;
       const int p0 = (2 * it.cur.pb + (int)rank) * 64 + 16 * q + tq;      // template of h = 0; h = 1: + 8
       if constexpr (RT) {
-        // this warp has drained the previous unit's last accumulator, so every MMA that read the old R is complete
+        // Every MMA that read the old R must be complete: the previous unit's last two tiles.  One of them was this group's
+        // (drained); the other group's is waited for here as an observer (its accumulator cannot be reused before r_ready).
+        if (e > 1) mbar_wait(acc_full_u + 8u * ((e - 2u) & (NACC - 1)), ((e - 2u) / NACC) & 1u);
+        if (e > 0) mbar_wait(acc_full_u + 8u * ((e - 1u) & (NACC - 1)), ((e - 1u) / NACC) & 1u);
         const BdPlan* B = a.bd + bdi;
         __syncwarp();
         load_R_tmem(a.sp, B->f0_slice, B->n_f0, 2 * it.cur.pb + (int)rank, tmem + ((uint32_t)(q * 32) << 16), q * 32 + lane, wg);
@@ -936,99 +942,108 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
         if (lane == 0) mbar_arrive_cluster(r_ready_u & kLeaderMask);
       }
       int g_left = gt - (int)((a0 + t0) % gt);                           // tiles to the end of the current granule (absolute grid)
+      uint32_t own = (uint32_t)((a0 + t0) & 1) ^ (uint32_t)wg;            // 0: tile t is this group's
       uint32_t bqt[2] = {0u, 0u};                                       // running maximum of the granule (truncated bits)
       int bk[2] = {0, 0};
       float bre[2] = {0.f, 0.f}, bim[2] = {0.f, 0.f};
-      for (int t = t0; t < t1; ++t, ++e) {
-        const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
-        TWAIT(0, acc_full_u + 8u * b, ph);
-        __syncwarp();
-        fence_after();
-        const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * wg);
-        const int kap0 = t * 128;
-        const int valid = min(128, a.c - kap0);
-        const int cthr = 64 * wg + 2 * tc;                                // column of (i = 0, e = 0)
-        uint32_t rr[2][32];
-        __syncwarp();                                                     // tcgen05.ld is .aligned: the lanes may have diverged above
-        tmem_ld_16x256b_x8(taddr, rr[0]);
-        tmem_ld_16x256b_x8(taddr + (16u << 16), rr[1]);
-        tmem_ld_wait();
-        fence_before();                                                   // both halves are in registers: free the accumulator
-        __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);
+      for (int t = t0; t < t1; ++t, ++e, own ^= 1u) {
+        if (own == 0u) {
+          const uint32_t b = e & (NACC - 1), ph = (e / NACC) & 1u;
+          TWAIT(0, acc_full_u + 8u * b, ph);
+          __syncwarp();
+          fence_after();
+          const int kap0 = t * 128;
+          const int valid = min(128, a.c - kap0);
+#pragma unroll 1
+          for (int ch = 0; ch < 2; ++ch) {                                  // column halves [0, 64), [64, 128)
+            const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + b * 128u + (uint32_t)(64 * ch);
+            const int cthr = 64 * ch + 2 * tc;                              // column of (i = 0, e = 0)
+            uint32_t rr[2][32];
+            __syncwarp();                                                   // tcgen05.ld is .aligned: the lanes may have diverged above
+            tmem_ld_16x256b_x8(taddr, rr[0]);
+            tmem_ld_16x256b_x8(taddr + (16u << 16), rr[1]);
+            tmem_ld_wait();
+            if (ch == 1) {                                                  // the whole tile is in registers or done: free the accumulator
+              fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive_cluster(acc_empty_leader + 8u * b);
+            }
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          uint32_t (&r)[32] = rr[h];
-          if constexpr (CAPTURE) {
-            const int p = p0 + 8 * h;
-            if (a.cap.bd == bdi && 2 * p + 1 < a.cap.rows) {
+            for (int h = 0; h < 2; ++h) {
+              uint32_t (&r)[32] = rr[h];
+              if constexpr (CAPTURE) {
+                const int p = p0 + 8 * h;
+                if (a.cap.bd == bdi && 2 * p + 1 < a.cap.rows) {
 #pragma unroll
-              for (int j = 0; j < 16; ++j) {
-                const int col = cthr + 8 * (j >> 1) + (j & 1);
-                const long long k = a.k_a + kap0 + col;
-                if (col < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
-                  a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + (j & 1)]);
-                  a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + 2 + (j & 1)]);
+                  for (int j = 0; j < 16; ++j) {
+                    const int col = cthr + 8 * (j >> 1) + (j & 1);
+                    const long long k = a.k_a + kap0 + col;
+                    if (col < valid && k >= a.cap.k_begin && k < a.cap.k_begin + a.cap.n) {
+                      a.cap.snr[(size_t)(2 * p) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + (j & 1)]);
+                      a.cap.snr[(size_t)(2 * p + 1) * a.cap.n + (k - a.cap.k_begin)] = __uint_as_float(r[4 * (j >> 1) + 2 + (j & 1)]);
+                    }
+                  }
                 }
+              }
+#ifdef LLOID_TRACE_BUILD
+              if (g_exp & 4) continue;
+#endif
+              uint32_t code[16];
+#pragma unroll
+              for (int i = 0; i < 8; ++i) {                                 // two columns per packed instruction: q = fma(re, re, im * im)
+                uint64_t re2, im2, q2;
+                asm("mov.b64 %0, {%1, %2};" : "=l"(re2) : "r"(r[4 * i]), "r"(r[4 * i + 1]));
+                asm("mov.b64 %0, {%1, %2};" : "=l"(im2) : "r"(r[4 * i + 2]), "r"(r[4 * i + 3]));
+                asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(q2) : "l"(im2));
+                asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(q2) : "l"(re2));
+                asm("mov.b64 {%0, %1}, %2;" : "=r"(code[2 * i]), "=r"(code[2 * i + 1]) : "l"(q2));
+              }
+              if (valid < 128) {
+#pragma unroll
+                for (int j = 0; j < 16; ++j) if (cthr + 8 * (j >> 1) + (j & 1) >= valid) code[j] = 0u;
+              }
+              // Gate: only a value above the threshold can become a trigger, and only one above the granule's running
+              // maximum changes it.  The plain maximum of the 16 |rho|^2 (8 instructions) against max(theta^2 (1 - 2^-16),
+              // running maximum) decides for the whole warp whether the index bookkeeping below (pack, 15 maxima, select
+              // tree: 80 of the 150 instructions per half tile) runs at all; at theta = 4 in noise it does for one warp in
+              // six.  A granule without any value above the threshold leaves a record with q = 0, which the merge kernel
+              // never turns into a trigger.
+              {
+                uint32_t mx = max(max(code[0], code[1]), code[2]);
+#pragma unroll
+                for (int j = 3; j < 15; j += 2) mx = max(max(mx, code[j]), code[j + 1]);
+                mx = max(mx, code[15]);
+                if (!__any_sync(0xffffffffu, mx > max(a.q_gate, bqt[h]))) continue;
+              }
+#pragma unroll
+              for (int j = 0; j < 16; ++j) code[j] = (code[j] & ~15u) | (uint32_t)(15 - j);
+#pragma unroll
+              for (int st = 8; st >= 1; st >>= 1)
+#pragma unroll
+                for (int j = 0; j < st; ++j) code[j] = max(code[j], code[j + st]);
+              const uint32_t m = code[0];
+              const int jw = 15 - (int)(m & 15u);
+              // select tree on the bits of jw: e = jw & 1, i = jw >> 1
+              uint32_t sr[8], si[8];
+#pragma unroll
+              for (int i = 0; i < 8; ++i) { sr[i] = (jw & 1) ? r[4 * i + 1] : r[4 * i]; si[i] = (jw & 1) ? r[4 * i + 3] : r[4 * i + 2]; }
+#pragma unroll
+              for (int i = 0; i < 4; ++i) { sr[i] = (jw & 2) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 2) ? si[2 * i + 1] : si[2 * i]; }
+#pragma unroll
+              for (int i = 0; i < 2; ++i) { sr[i] = (jw & 4) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 4) ? si[2 * i + 1] : si[2 * i]; }
+              const uint32_t wr = (jw & 8) ? sr[1] : sr[0], wi = (jw & 8) ? si[1] : si[0];
+              if ((m & ~15u) > bqt[h]) {                                    // later columns and later tiles never win ties
+                bqt[h] = m & ~15u; bk[h] = kap0 + cthr + 8 * (jw >> 1) + (jw & 1);
+                bre[h] = __uint_as_float(wr); bim[h] = __uint_as_float(wi);
               }
             }
           }
-#ifdef LLOID_TRACE_BUILD
-          if (g_exp & 4) continue;
-#endif
-          uint32_t code[16];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {                                   // two columns per packed instruction: q = fma(re, re, im * im)
-            uint64_t re2, im2, q2;
-            asm("mov.b64 %0, {%1, %2};" : "=l"(re2) : "r"(r[4 * i]), "r"(r[4 * i + 1]));
-            asm("mov.b64 %0, {%1, %2};" : "=l"(im2) : "r"(r[4 * i + 2]), "r"(r[4 * i + 3]));
-            asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(q2) : "l"(im2));
-            asm("fma.rn.f32x2 %0, %1, %1, %0;" : "+l"(q2) : "l"(re2));
-            asm("mov.b64 {%0, %1}, %2;" : "=r"(code[2 * i]), "=r"(code[2 * i + 1]) : "l"(q2));
-          }
-          if (valid < 128) {
-#pragma unroll
-            for (int j = 0; j < 16; ++j) if (cthr + 8 * (j >> 1) + (j & 1) >= valid) code[j] = 0u;
-          }
-          // Gate: only a value above the threshold can become a trigger, and only one above the granule's running maximum
-          // changes it.  The plain maximum of the 16 |rho|^2 (8 instructions) against max(theta^2 (1 - 2^-16), running
-          // maximum) decides for the whole warp whether the index bookkeeping below (pack, 15 maxima, select tree: 80 of the
-          // 150 instructions per half tile) runs at all; at theta = 4 in noise it does for one warp in six.  A granule without
-          // any value above the threshold leaves a record with q = 0, which the merge kernel never turns into a trigger.
-          {
-            uint32_t mx = max(max(code[0], code[1]), code[2]);
-#pragma unroll
-            for (int j = 3; j < 15; j += 2) mx = max(max(mx, code[j]), code[j + 1]);
-            mx = max(mx, code[15]);
-            if (!__any_sync(0xffffffffu, mx > max(a.q_gate, bqt[h]))) continue;
-          }
-#pragma unroll
-          for (int j = 0; j < 16; ++j) code[j] = (code[j] & ~15u) | (uint32_t)(15 - j);
-#pragma unroll
-          for (int st = 8; st >= 1; st >>= 1)
-#pragma unroll
-            for (int j = 0; j < st; ++j) code[j] = max(code[j], code[j + st]);
-          const uint32_t m = code[0];
-          const int jw = 15 - (int)(m & 15u);
-          // select tree on the bits of jw: e = jw & 1, i = jw >> 1
-          uint32_t sr[8], si[8];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) { sr[i] = (jw & 1) ? r[4 * i + 1] : r[4 * i]; si[i] = (jw & 1) ? r[4 * i + 3] : r[4 * i + 2]; }
-#pragma unroll
-          for (int i = 0; i < 4; ++i) { sr[i] = (jw & 2) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 2) ? si[2 * i + 1] : si[2 * i]; }
-#pragma unroll
-          for (int i = 0; i < 2; ++i) { sr[i] = (jw & 4) ? sr[2 * i + 1] : sr[2 * i]; si[i] = (jw & 4) ? si[2 * i + 1] : si[2 * i]; }
-          const uint32_t wr = (jw & 8) ? sr[1] : sr[0], wi = (jw & 8) ? si[1] : si[0];
-          if ((m & ~15u) > bqt[h]) {                                      // later tiles never win ties
-            bqt[h] = m & ~15u; bk[h] = kap0 + cthr + 8 * (jw >> 1) + (jw & 1);
-            bre[h] = __uint_as_float(wr); bim[h] = __uint_as_float(wi);
-          }
         }
-        // granule end: merge the partial maxima of a template (4 threads x 2 column halves), write one record
-        if (t + 1 == t1 || --g_left == 0) {                                  // (no 64-bit division per tile: a countdown)
+        // granule end (reached by both groups, whether or not the last tile was theirs): merge the 4 threads of a template,
+        // write this group's record -- also when it saw no tile or no value above the gate (q = 0)
+        if (t + 1 == t1 || --g_left == 0) {                                // (no 64-bit division per tile: a countdown)
           g_left = gt;
-          const long long at = a0 + t;
-          const int fp = flush_i & 1;
+          const int gi = (int)((a0 + t) / gt - a0 / gt);
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
             float bq = fmaf(bre[h], bre[h], bim[h] * bim[h]);
@@ -1040,28 +1055,13 @@ f0_pair_kernel(const __grid_constant__ F0PArgs a)
               const int ok = __shfl_xor_sync(0xffffffffu, k, x);
               if (oq > bq || (oq == bq && ok < k)) { bq = oq; k = ok; re = ore; im = oim; }
             }
-            if (wg == 1 && tc == 0) { Peak pk; pk.q = bq; pk.kappa = k; pk.re = re; pk.im = im; s_x[fp][16 * q + 8 * h + tq] = pk; }
-            bre[h] = re; bim[h] = im; bk[h] = k; bqt[h] = __float_as_uint(bq);   // reused below by wg 0 (reset afterwards)
-          }
-          asm volatile("bar.sync 2, 256;" ::: "memory");
-          if (wg == 0 && tc == 0) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              float bq = __uint_as_float(bqt[h]), re = bre[h], im = bim[h];
-              int k = bk[h];
-              const Peak o = s_x[fp][16 * q + 8 * h + tq];
-              if (o.q > bq) { bq = o.q; k = o.kappa; re = o.re; im = o.im; }   // its columns are later: ties stay here
-              const int p = p0 + 8 * h;
-              if (p < n_templates) {
-                const int gi = (int)(at / gt - a0 / gt);
-                Peak pk; pk.q = bq; pk.kappa = k; pk.re = re; pk.im = im;
-                a.partials[((size_t)bdi * a.slots_cap + gi) * a.max_templates + p] = pk;
-              }
+            const int p = p0 + 8 * h;
+            if (tc == 0 && p < n_templates) {
+              Peak pk; pk.q = bq; pk.kappa = k; pk.re = re; pk.im = im;
+              a.partials[((size_t)bdi * a.slots_cap + 2 * gi + wg) * a.max_templates + p] = pk;
             }
+            bqt[h] = 0u; bk[h] = 0; bre[h] = 0.f; bim[h] = 0.f;
           }
-          ++flush_i;
-#pragma unroll
-          for (int h = 0; h < 2; ++h) { bqt[h] = 0u; bk[h] = 0; bre[h] = 0.f; bim[h] = 0.f; }
         }
       }
     }

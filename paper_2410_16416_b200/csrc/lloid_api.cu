@@ -866,10 +866,11 @@ int finalize_impl(lloid_bank* b)
     const bool tensor = b->f16 && f16_plan_tensor_recon(b->plan16);
     b->gt = tensor ? f16_granule_tiles(b->cfg.peak_window) : 1;
     const bool per_tile = !tensor || excl != nullptr;
-    b->slots_cap = per_tile ? b->tiles_cap : (int)(C / kTimeTile) / b->gt + 2;
+    const int tensor_slots = 2 * ((int)(C / kTimeTile) / b->gt + 2);     // two records per granule (the f0 epilogue's two warp groups)
+    b->slots_cap = !tensor ? b->tiles_cap : (per_tile ? std::max(b->tiles_cap, tensor_slots) : tensor_slots);
     rc = scratch_alloc(b, 2, (void**)&b->partials, nstate * b->slots_cap * sizeof(Peak), true); if (rc) return rc;
     if (tensor) {
-      std::vector<int32_t> stl(b->n_bd, b->gt);
+      std::vector<int32_t> stl(b->n_bd, b->gt | (1 << 16));              // tiles per granule | two records per granule
       if (excl) for (int bd = 0; bd < b->n_bd; ++bd) if (excl[bd]) stl[bd] = 1;
       rc = dev_alloc(b, (void**)&b->slot_tiles_dev, stl.size() * sizeof(int32_t), false); if (rc) return rc;
       CU(cudaMemcpy(b->slot_tiles_dev, stl.data(), stl.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
