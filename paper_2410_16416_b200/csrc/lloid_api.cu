@@ -59,7 +59,23 @@ std::vector<double> lowpass(int d, int K)
   return lp;
 }
 
-struct SliceHost { int rate, d, log2d, n_taps, L, L_pad; int64_t end_delay; bool fold; /* fp16: interpolation folded into the basis filters */ };
+struct SliceHost {
+  int rate, d, log2d, n_taps, L, L_pad; int64_t end_delay;
+  bool fold;                       // fp16: interpolation folded into the basis filters
+  // fp16: the packed basis filters are stored in COLUMN BLOCKS of at most 160 filters, each a basis-FIR problem of its own.
+  // The FIR kernel keeps 512 / L_pad time tiles of accumulators in TMEM and streams all of U once per such group of tiles:
+  // at L_pad = 320 that is one tile per 2 MB of U (L2-bandwidth-bound on config 4); two blocks of 160 run three tiles each.
+  int n_ub = 1, ub_w[4] = {0, 0, 0, 0}, ub_l0[4] = {0, 0, 0, 0};
+  void set_blocks(bool f16)
+  {
+    n_ub = 1; ub_w[0] = L_pad; ub_l0[0] = 0;
+    if (!f16 || L_pad < 224 || getenv("LLOID_NO_USPLIT")) return;
+    n_ub = std::max(2, (L_pad + 159) / 160);
+    const int w = ((L_pad + n_ub - 1) / n_ub + 31) / 32 * 32;
+    for (int i = 0, l0 = 0; i < n_ub; ++i, l0 += w) { ub_l0[i] = l0; ub_w[i] = std::min(w, L_pad - l0); }
+  }
+  size_t ub_off(int i, int n_kb) const { return (size_t)n_kb * 64 * ub_l0[i]; }    // halves before block i in a packed array
+};
 struct BinHost { int N, S, rows_pad; int64_t M; std::vector<SliceHost> slices; };
 
 }  // namespace
@@ -184,11 +200,15 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
     const int n_kb = (n_eff + 63) / 64;
     const size_t nup = (size_t)n_kb * 64 * S.L_pad;
     std::vector<__half> u(nup, __float2half(0.f)), ub;
+    auto upos = [&](int l, int t) {            // column block of l, then [tap block][tap group][l in block][8 taps]
+      int bi = 0;
+      while (bi + 1 < S.n_ub && l >= S.ub_l0[bi + 1]) ++bi;
+      return S.ub_off(bi, n_kb) + (((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.ub_w[bi] + (l - S.ub_l0[bi])) * 8 + (t & 7);
+    };
     if (!S.fold) {
       for (int l = 0; l < S.L; ++l)
         for (int t = 0; t < S.n_taps; ++t)
-          u[(((size_t)(t >> 6) * 8 + ((t >> 3) & 7)) * S.L_pad + l) * 8 + (t & 7)] =
-              __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
+          u[upos(l, t)] = __float2half_rn((float)basis[(size_t)l * S.n_taps + t]);
     } else {
       ub.assign(nup, __float2half(0.f));
       const std::vector<double> lp = lowpass(S.d, Ku);
@@ -202,7 +222,7 @@ int upload_arrays(lloid_bank* b, int bin, int slice, const double* basis, const 
               if (t < 0 || t >= S.n_taps) continue;
               acc += (double)S.d * lp[S.d * i + phi + Ku * S.d] * basis[(size_t)l * S.n_taps + t];
             }
-            dst[(((size_t)(uu >> 6) * 8 + ((uu >> 3) & 7)) * S.L_pad + l) * 8 + (uu & 7)] = __float2half_rn((float)acc);
+            dst[upos(l, uu)] = __float2half_rn((float)acc);
           }
       }
     }
@@ -405,6 +425,7 @@ int lloid_bank_create(lloid_bank_t** out, const lloid_bank_config_t* cfg, const 
       if (S.d > 1 && sd.end_delay < (int64_t)(cfg->k_down + cfg->k_up) * S.d) { delete b; return fail(LLOID_EINVAL, "bin %d slice %d: causality needs end_delay >= (k_down + k_up) * d", bi, s); }
       S.n_taps = sd.n_taps; S.L = sd.n_basis; S.L_pad = (int)round_up(S.L, kLPad); S.end_delay = sd.end_delay;
       S.fold = b->f16 && S.d > 1 && S.d <= kFoldMaxD && !getenv("LLOID_NO_FOLD");
+      S.set_blocks(b->f16);
       expect_delay += (int64_t)S.d * S.n_taps;
       B.slices.push_back(S);
       b->d_max = std::max(b->d_max, S.d);
@@ -774,12 +795,21 @@ int finalize_impl(lloid_bank* b)
     // the composite filters, c / d rows, FIR row m -> Y row d m + phi; its window origin moves by the 2 K_up extra taps.
     for (const SliceParams& P : b->sp_host) {
       const SliceHost& S = b->bins[P.bin].slices[P.slice];
-      if (!S.fold) { b->fir_host.push_back(P); continue; }
-      for (int phi = 0; phi < S.d; ++phi) {
+      const int n_phase = S.fold ? S.d : 1;
+      const int n_kb = ((S.fold ? S.n_taps + 2 * Ku : S.n_taps) + 63) / 64;
+      for (int phi = 0; phi < n_phase; ++phi) {
         SliceParams F = P;
-        F.d = S.d; F.log2d = S.log2d; F.n_taps = S.n_taps + 2 * Ku; F.jjY0 = P.jjY0 + 2 * Ku;
-        F.U16 = phi ? P.U16b : P.U16; F.fir_halo = 0; F.out_mul = S.d; F.out_add = phi;
-        b->fir_host.push_back(F);
+        if (S.fold) {
+          F.d = S.d; F.log2d = S.log2d; F.n_taps = S.n_taps + 2 * Ku; F.jjY0 = P.jjY0 + 2 * Ku;
+          F.U16 = phi ? P.U16b : P.U16; F.fir_halo = 0; F.out_mul = S.d; F.out_add = phi;
+        }
+        for (int ub = 0; ub < S.n_ub; ++ub) {           // one problem per column block of the basis (SliceHost::set_blocks)
+          SliceParams G = F;
+          G.U16 = F.U16 + S.ub_off(ub, n_kb);
+          G.L_pad = S.ub_w[ub]; G.L = std::max(0, std::min(S.L - S.ub_l0[ub], S.ub_w[ub]));
+          G.Y = (char*)P.Y + (size_t)(S.ub_l0[ub] / 8) * 64 * 16;       // Y16 record: [slice][l / 8][64 rows][8]
+          b->fir_host.push_back(G);
+        }
       }
     }
     rc = dev_alloc(b, (void**)&b->fir_dev, b->fir_host.size() * sizeof(SliceParams), false); if (rc) return rc;
