@@ -1246,7 +1246,9 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   const int low_fixed = pl->r_tmem ? 0 : pl->l_sum_low_max * 256;
   // y stage slot: the largest stage of any unit the kernel streams (a unit with nm = sum L_pad / 16 MMAs per tile is cut
   // into ceil(nm / ycap) stages of ceil(nm / stages) MMAs at most, 2 KB per MMA and CTA)
-  pl->ycap = getenv("LLOID_YCAP") ? std::max(2, std::min(16, atoi(getenv("LLOID_YCAP")))) : 8;
+  // (with R in shared memory the ring is short -- 3 slots of 14 KB at config 2 -- and stages of <= 6 MMAs = 4 slots of 10 KB
+  // measured 4 % faster in the f0 kernel; with R in TMEM the ring is long and <= 8 is as good or better)
+  pl->ycap = getenv("LLOID_YCAP") ? std::max(2, std::min(16, atoi(getenv("LLOID_YCAP")))) : (pl->r_tmem ? 8 : 6);
   int ys_f0 = 2048, ys_low = 2048;
   auto stage_bytes = [&](int l_sum) { const int nm = l_sum / 16, nst = stage_count(nm, pl->ycap); return (nm + nst - 1) / nst * 2048; };
   for (int b = 0; b < n_bd; ++b) {
