@@ -186,8 +186,9 @@ void launch_resample(const RateParams* rates_dev, const RateParams* rates_host, 
     int r0 = 0;
     while (r0 < n_rates) {
       int r1 = r0, gmax_d = 1, blocks4 = 0;
-      const bool small = rates_host[r0].d <= 8;
-      while (r1 < n_rates && (rates_host[r1].d <= 8) == small) {
+      const bool one = c <= 16384;                 // short buffers (streaming): a second launch costs more than it saves
+      const bool small = one || rates_host[r0].d <= 8;
+      while (r1 < n_rates && (one || rates_host[r1].d <= 8) == small) {
         const RateParams& R = rates_host[r1];
         if (!(R.d == 1 && !want_f16)) {
           const int span = R.jj_hi_off + c / R.d - R.jj_lo_fixed;
