@@ -213,6 +213,41 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def time_coincidence(bank, w, trig_dev, n_trig, stream, reps=5):
+    """SURVEY.md section 8(f) NEXT-2 on the triggers of the last timed step: lloid_coincidence (same template, detectors a < b, within
+    max_dt samples: 10 ms baselines + 10 samples of timing resolution at 2048 Hz).  HBM-bound integer work; bytes = the
+    lookup table written once (memset) + the trigger list read by the scatter and by the match kernel + the partner
+    look-ups (3 windows x 4 B per other detector)."""
+    import torch
+    from paper_2410_16416_b200 import binding as lb
+    D, n = w.n_detectors, w.n_samples
+    max_dt = np.zeros((D, D), dtype=np.int32)
+    for a in range(D):
+        for b in range(a + 1, D):
+            max_dt[a, b] = 31
+    sb = lb.lloid_coincidence_scratch_bytes(bank.handle, 0, n)
+    scratch = torch.empty(sb, dtype=torch.uint8, device="cuda")
+    cap = max(1, n_trig)
+    pairs = torch.empty(cap * 16, dtype=torch.uint8, device="cuda")
+    pcnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    for i in range(reps + 1):
+        e0.record()
+        lb.lloid_coincidence(bank.handle, trig_dev.data_ptr(), n_trig, 0, n, max_dt, scratch.data_ptr(), sb, pairs.data_ptr(), cap, pcnt.data_ptr(), stream)
+        e1.record()
+        e1.synchronize()
+        if i:
+            times.append(e0.elapsed_time(e1))
+    ms = float(np.median(times))
+    nbytes = float(sb + n_trig * (32 + 32 + 12 * (D - 1)))
+    peak = load_peaks()["hbm"]
+    return {"what": "lloid_coincidence on the triggers of one step (PAPER.md:41 coincidence generator; max_dt = 31 samples)",
+            "n_triggers": int(n_trig), "n_pairs": int(pcnt.item()), "ms": ms, "launches": 2,
+            "roofline": {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": nbytes / (ms * 1e-3) / 1e9 / peak, "algorithmic_bytes": nbytes}}
+
+
 def time_bank(w, precision, steps, warmup, chunk, local=0, world=1, bins=None, want_e2e=True, flush=None):
     """Build a bank over `w` and time `steps` passes of the whole hot path.  Device leg: strain resident in HBM, CUDA
     events around lloid_filter on the launching stream, L2 flushed between steps, the library's per-stage events recorded
@@ -270,6 +305,8 @@ def time_bank(w, precision, steps, warmup, chunk, local=0, world=1, bins=None, w
     out["dev_bytes"] = int(lb.lloid_device_bytes(bank.handle))
     out["path"] = lb.lloid_path_info(bank.handle)
     out["n_templates"] = n_templates
+    if D >= 2 and bins is None and out["n_trig"] <= cap:
+        out["coincidence"] = time_coincidence(bank, w, trig_dev, out["n_trig"], stream)
     if want_e2e:
         strain_pin = torch.from_numpy(w.strain).pin_memory()
         trig_np = torch.empty(cap * 32, dtype=torch.uint8).pin_memory().numpy().view(lb.TRIGGER_DTYPE)
@@ -402,6 +439,8 @@ def run_ours(args):
     roofline["stage_ms"] = stage_dict(stage)
 
     extra = {}
+    if r.get("coincidence"):
+        extra["coincidence"] = r["coincidence"]
     if world > 1:
         extra["config3_sharded"] = sharded_config3(args, rank, world, local)
     if rank != 0:

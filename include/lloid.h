@@ -200,6 +200,29 @@ int lloid_path_info(const lloid_bank_t *bank, int32_t *out);
 int lloid_set_profiling(lloid_bank_t *bank, int32_t enable);
 int lloid_last_stage_ms(lloid_bank_t *bank, float *out_ms /* host, float[6] */);
 
+/* ---- coincidence (the step after the trigger generator) --------------------------------------
+ * "These triggers are passed to the coincidence generator, which identifies coincidences between triggers
+ * detected with the same template and within the light travel time between detectors."  Two triggers of ONE lloid_filter
+ * pass are coincident iff they have the same bin and template, different detectors a < b, and |sample_a - sample_b| <=
+ * max_dt[a * n_detectors + b] (the light travel time between a and b plus the timing resolution, in f0 samples; the caller
+ * chooses it: e.g. 21 + 10 samples at 2048 Hz for a 10 ms baseline).
+ *   triggers_dev   device, the records of one pass over absolute samples [k_begin, k_begin + n_samples): at most one per
+ *                  (bin, detector, template, peak window), which is what lloid_filter emits; records outside that range or
+ *                  with indices outside the bank are ignored; of two records with the same key one is ignored
+ *   n_triggers     host value, number of records (min(count, capacity) of the filter call)
+ *   max_dt         host, int32 [n_detectors][n_detectors], only a < b is read; 0 <= max_dt <= peak_window
+ *   scratch_dev    device, lloid_coincidence_scratch_bytes(bank, k_begin, n_samples) bytes, owned by the caller, overwritten
+ *   pairs_dev      device, lloid_coinc_t[capacity]: indices into triggers_dev, a = the lower-numbered detector's trigger;
+ *                  order unspecified.  n_pairs_dev: device int64, number of coincident pairs found; beyond capacity they
+ *                  are counted, not stored (lloid_check_count)
+ * A trigger can belong to several pairs (three detectors: ab, ac, bc are reported separately).  Asynchronous on cuda_stream;
+ * no device allocation.  Errors: LLOID_EINVAL, LLOID_ESTATE (bank not finalized), LLOID_ECUDA. */
+typedef struct { int64_t a, b; } lloid_coinc_t;
+int64_t lloid_coincidence_scratch_bytes(const lloid_bank_t *bank, int64_t k_begin, int64_t n_samples);
+int lloid_coincidence(const lloid_bank_t *bank, const lloid_trigger_t *triggers_dev, int64_t n_triggers, int64_t k_begin,
+                      int64_t n_samples, const int32_t *max_dt, void *scratch_dev, int64_t scratch_bytes,
+                      lloid_coinc_t *pairs_dev, int64_t capacity, int64_t *n_pairs_dev, void *cuda_stream);
+
 /* ---- allocation-free entry point -----------------------------------------------------------------------------------
  * Steps A5 + A6 alone ("identifies peaks in the SNR time series with SNR > 4 ... 'triggers'") on a dense SNR
  * series the caller already holds in device memory, for callers that may not allocate (CUDA graph capture, serving loops,

@@ -70,6 +70,9 @@ EXPORTS = {
     "lloid_graph_advance": (C.c_int, [C.c_void_p, C.c_int64]),
     "lloid_set_profiling": (C.c_int, [C.c_void_p, C.c_int32]),
     "lloid_last_stage_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float)]),
+    "lloid_coincidence_scratch_bytes": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int64]),
+    "lloid_coincidence": (C.c_int, [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_int64,
+                                    C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]),
     "lloid_noalloc_max_records": (C.c_int64, []),
     "lloid_noalloc_setup": (C.c_int, []),
     "lloid_window_peaks_noalloc": (C.c_int, [C.c_void_p, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int32, C.c_float, C.c_int32,
@@ -205,6 +208,21 @@ def lloid_path_info(bank) -> dict:
     out = (C.c_int32 * 4)()
     _check(lib().lloid_path_info(bank, out))
     return dict(tensor_recon=bool(out[0]), r_in_tmem=bool(out[1]), cuda_core_bds=int(out[2]), folded_slices=int(out[3]))
+
+
+COINC_DTYPE = np.dtype([("a", "<i8"), ("b", "<i8")])
+
+
+def lloid_coincidence_scratch_bytes(bank, k_begin: int, n_samples: int) -> int:
+    return lib().lloid_coincidence_scratch_bytes(bank, k_begin, n_samples)
+
+
+def lloid_coincidence(bank, triggers_dev_ptr: int, n_triggers: int, k_begin: int, n_samples: int, max_dt: np.ndarray,
+                      scratch_dev_ptr: int, scratch_bytes: int, pairs_dev_ptr: int, capacity: int, n_pairs_dev_ptr: int,
+                      cuda_stream: int = 0) -> None:
+    dt = np.ascontiguousarray(max_dt, dtype=np.int32)
+    _check(lib().lloid_coincidence(bank, triggers_dev_ptr, n_triggers, k_begin, n_samples, dt.ctypes.data, scratch_dev_ptr,
+                                   scratch_bytes, pairs_dev_ptr, capacity, n_pairs_dev_ptr, cuda_stream))
 
 
 def lloid_noalloc_max_records() -> int:

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblloid.so")
-SOURCES = ["lloid_api.cu", "kernels_common.cu", "kernels_f32.cu", "kernels_f16.cu", "kernels_f16_recon.cu", "kernels_noalloc.cu"]
+SOURCES = ["lloid_api.cu", "kernels_common.cu", "kernels_f32.cu", "kernels_f16.cu", "kernels_f16_recon.cu", "kernels_noalloc.cu", "kernels_coinc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

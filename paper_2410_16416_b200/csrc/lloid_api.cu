@@ -1137,6 +1137,61 @@ int lloid_path_info(const lloid_bank_t* b, int32_t* out)
   return LLOID_OK;
 }
 
+namespace {
+struct CoincGeom { long long k_w0; int n_w; long long total_t; size_t prefix_bytes, dt_bytes, table_bytes; };
+CoincGeom coinc_geom(const lloid_bank* b, int64_t k_begin, int64_t n_samples)
+{
+  CoincGeom g;
+  const long long W = b->cfg.peak_window;
+  g.k_w0 = k_begin / W * W;
+  g.n_w = (int)((k_begin + n_samples - g.k_w0 + W - 1) / W);
+  g.total_t = 0;
+  for (const BinHost& B : b->bins) g.total_t += B.N;
+  g.prefix_bytes = (size_t)round_up((int64_t)(b->bins.size() + 1) * 8, 256);
+  g.dt_bytes = (size_t)round_up((int64_t)b->cfg.n_detectors * b->cfg.n_detectors * 4, 256);
+  g.table_bytes = (size_t)g.total_t * b->cfg.n_detectors * g.n_w * sizeof(int);
+  return g;
+}
+}  // namespace
+
+int64_t lloid_coincidence_scratch_bytes(const lloid_bank_t* b, int64_t k_begin, int64_t n_samples)
+{
+  if (!b || k_begin < 0 || n_samples <= 0) return -1;
+  const CoincGeom g = coinc_geom(b, k_begin, n_samples);
+  return (int64_t)(g.prefix_bytes + g.dt_bytes + g.table_bytes);
+}
+
+int lloid_coincidence(const lloid_bank_t* b, const lloid_trigger_t* trig, int64_t n, int64_t k_begin, int64_t n_samples,
+                      const int32_t* max_dt, void* scratch, int64_t scratch_bytes, lloid_coinc_t* pairs, int64_t capacity,
+                      int64_t* n_pairs_dev, void* stream)
+{
+  if (!b) return fail(LLOID_EINVAL, "null bank");
+  if (!b->finalized) return fail(LLOID_ESTATE, "coincidence before finalize");
+  if (!max_dt || !scratch || !n_pairs_dev || (n > 0 && !trig) || (capacity > 0 && !pairs)) return fail(LLOID_EINVAL, "null buffer");
+  if (n < 0 || n > 0x7fffffffLL || capacity < 0 || k_begin < 0 || n_samples <= 0) return fail(LLOID_EINVAL, "bad size");
+  const int D = b->cfg.n_detectors;
+  for (int a = 0; a < D; ++a)
+    for (int c = a + 1; c < D; ++c)
+      if (max_dt[a * D + c] < 0 || max_dt[a * D + c] > b->cfg.peak_window)
+        return fail(LLOID_EINVAL, "max_dt[%d][%d] = %d outside [0, peak_window = %d]", a, c, max_dt[a * D + c], b->cfg.peak_window);
+  const CoincGeom g = coinc_geom(b, k_begin, n_samples);
+  if ((int64_t)(g.prefix_bytes + g.dt_bytes + g.table_bytes) > scratch_bytes)
+    return fail(LLOID_EINVAL, "scratch too small: %lld bytes needed (lloid_coincidence_scratch_bytes)", (long long)(g.prefix_bytes + g.dt_bytes + g.table_bytes));
+  cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaSetDevice(b->cfg.device));
+  std::vector<long long> prefix(b->bins.size() + 1, 0);
+  for (size_t i = 0; i < b->bins.size(); ++i) prefix[i + 1] = prefix[i] + b->bins[i].N;
+  char* base = (char*)scratch;
+  // small pageable copies: staged by the runtime before the call returns, ordered on the stream
+  CU(cudaMemcpyAsync(base, prefix.data(), prefix.size() * 8, cudaMemcpyHostToDevice, st));
+  CU(cudaMemcpyAsync(base + g.prefix_bytes, max_dt, (size_t)D * D * 4, cudaMemcpyHostToDevice, st));
+  launch_coincidence(trig, n, (const long long*)base, (int)b->bins.size(), D, g.k_w0, b->cfg.peak_window, g.n_w,
+                     (int*)(base + g.prefix_bytes + g.dt_bytes), g.table_bytes, (const int*)(base + g.prefix_bytes), pairs, capacity,
+                     (unsigned long long*)n_pairs_dev, st);
+  CU(cudaGetLastError());
+  return LLOID_OK;
+}
+
 void lloid_destroy(lloid_bank_t* b)
 {
   if (!b) return;

@@ -12,6 +12,7 @@
 // so that for every slice   c^s[kappa] = sum_{i=-K_up}^{K_up-1} w_phi[i] rho^s[row floor(kappa/d) + K_up - i],
 // phi = kappa mod d, w_phi[i] = d lp_{d,K_up}[d i + phi]   (A4 in include/lloid.h).
 #pragma once
+#include "../../include/lloid.h"
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
 #include <stdint.h>
@@ -133,6 +134,10 @@ void launch_merge_windows(const BinParams* bp_dev, int n_bd, int max_templates, 
                           const PeakState* state_in, PeakState* state_out, int n_det, int bin_base /* added to the bin index of every trigger */,
                           void* triggers, int64_t capacity, unsigned long long* count, cudaStream_t st, int64_t* launches);
 void launch_advance_counter(long long* k_base_dev, int64_t n, cudaStream_t st);
+// NEXT-2 coincidence (kernels_coinc.cu): table = int[total templates][n_det][n_w], filled with -1, then trigger indices
+void launch_coincidence(const lloid_trigger_t* trig, long long n, const long long* tmpl_off_dev, int n_bins, int n_det, long long k_w0, int W,
+                        int n_w, int* table, size_t table_bytes, const int* max_dt_dev, lloid_coinc_t* out, long long capacity,
+                        unsigned long long* count, cudaStream_t st);
 
 void launch_reset_state(PeakState* state, int64_t n, cudaStream_t st);
 

@@ -428,3 +428,48 @@ def test_golden_regression_values(cfg1):
     for i, k, val in rows:
         got = oc.snr_series(x, b.slices, b.basis, b.recon, int(k), int(k) + 1, KD, KU)[int(i), 0]
         assert abs(got - float(val)) < 1e-9
+
+
+# ---------------------------------------------------------------------------------- NEXT-2: coincidence oracle
+def _trigs(rows):
+    from paper_2410_16416_b200.binding import TRIGGER_DTYPE
+    t = np.zeros(len(rows), dtype=TRIGGER_DTYPE)
+    for i, (b, d, p, k) in enumerate(rows):
+        t[i]["bin"], t[i]["detector"], t[i]["template_idx"], t[i]["sample"] = b, d, p, k
+    return t
+
+
+def test_coincidence_oracle_hand_built_cases():
+    from oracle import coinc_oracle as co
+    dt = np.array([[0, 30, 50], [0, 0, 40], [0, 0, 0]])
+    rows = [(0, 0, 5, 10000),      # 0
+            (0, 1, 5, 10030),      # 1: exactly at the 0-1 tolerance         -> (0, 1)
+            (0, 1, 6, 10000),      # 2: other template                         -> nothing
+            (1, 1, 5, 10000),      # 3: other bin                              -> nothing
+            (0, 0, 7, 20000),      # 4
+            (0, 1, 7, 20031),      # 5: one sample outside                     -> nothing with 4
+            (0, 2, 7, 20049),      # 6: inside 0-2 (49 <= 50), inside 1-2 (18) -> (4, 6), (5, 6)
+            (0, 0, 9, 30000),      # 7
+            (0, 0, 9, 30005),      # 8: same detector twice                    -> nothing between 7 and 8
+            (0, 2, 9, 29960)]      # 9: 40 and 45 before                       -> (7, 9), (8, 9)
+    got = co.coincidences(_trigs(rows), dt)
+    assert got == {(0, 1), (4, 6), (5, 6), (7, 9), (8, 9)}
+    assert co.coincidences(_trigs([]), dt) == set()
+    assert co.coincidences(_trigs(rows), np.zeros((3, 3), dtype=int)) == set()          # nothing is simultaneous to the sample
+
+
+def test_coincidence_oracle_equals_double_loop_on_random_lists():
+    from oracle import coinc_oracle as co
+    rng = np.random.Generator(np.random.PCG64(5))
+    dt = [[0, 21, 35], [0, 0, 28], [0, 0, 0]]
+    for n in (1, 40, 300):
+        rows = [(int(rng.integers(0, 2)), int(rng.integers(0, 3)), int(rng.integers(0, 4)), int(rng.integers(0, 600))) for _ in range(n)]
+        t = _trigs(rows)
+        want = set()
+        for i, (bi, di, pi, ki) in enumerate(rows):            # the definition, pair by pair, no grouping
+            for j, (bj, dj, pj, kj) in enumerate(rows):
+                if bi == bj and pi == pj and di < dj and abs(ki - kj) <= dt[di][dj]:
+                    want.add((i, j))
+        assert co.coincidences(t, dt) == want
+        if n == 300:
+            assert len(want) > 20
