@@ -48,7 +48,8 @@ struct F16Plan {
   __half* p_dev = nullptr;
   void* units_dev = nullptr;            // LowUnit[low_units], rate-major
   int units_per_rate[kNLowRates] = {0, 0, 0, 0, 0};
-  SchedUnit* low_sched_dev = nullptr;   // [low_units]   cost per tile of every low-rate unit
+  SchedBd* low_cells_dev = nullptr;     // low-rate schedule: per rate class one entry per group (first unit, template blocks, cost per tile)
+  int low_cells_per_rate[kNLowRates] = {0, 0, 0, 0, 0};
   SchedBd* f0_sched_dev = nullptr;      // [f0_n_bds]    f0 kernel schedule entries
   int f0_n_bds = 0;
   long long low_wsum[kNLowRates] = {0, 0, 0, 0, 0};

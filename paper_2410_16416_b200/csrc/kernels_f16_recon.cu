@@ -94,49 +94,6 @@ struct YRing {                              // y ring position: slot index + pha
   __device__ __forceinline__ void skip(uint32_t k) { s += k; while (s >= n) { s -= n; ph ^= 1u; } }
 };
 
-// ---- static persistent schedule (SchedArgs in lloid_internal.h), per CLUSTER: low-rate kernel ------------
-struct SchedPos { int u, t; };              // unit index, first tile
-
-__device__ __forceinline__ SchedPos sched_locate(const SchedArgs& s, long long b)
-{
-  SchedPos r;
-  if (b >= s.cls_base[s.n_cls]) { r.u = s.cls_begin[s.n_cls]; r.t = 0; return r; }
-  int c = 0;
-  while (c + 1 < s.n_cls && b >= s.cls_base[c + 1]) ++c;
-  const long long rem = b - s.cls_base[c];
-  const long long nt = s.n_tiles[c];
-  int lo = s.cls_begin[c], hi = s.cls_begin[c + 1] - 1;   // largest u with wprefix[u] * nt <= rem
-  while (lo < hi) {
-    const int mid = (lo + hi + 1) >> 1;
-    if ((long long)s.units[mid].wprefix * nt <= rem) lo = mid; else hi = mid - 1;
-  }
-  const SchedUnit su = s.units[lo];
-  r.u = lo; r.t = (int)((rem - (long long)su.wprefix * nt) / su.w);
-  return r;
-}
-
-__device__ __forceinline__ int sched_class(const SchedArgs& s, int u)
-{
-  int c = 0;
-  while (c + 1 < s.n_cls && u >= s.cls_begin[c + 1]) ++c;
-  return c;
-}
-
-// this cluster's range -> rng[0..3] = first unit, first tile, last unit, end tile in the last unit
-__device__ __forceinline__ void sched_range(const SchedArgs& s, int cid, int ncl, int* rng)
-{
-  const long long T = s.cls_base[s.n_cls];
-  const SchedPos a = sched_locate(s, T * (long long)cid / (long long)ncl);
-  const SchedPos b = sched_locate(s, T * (long long)(cid + 1) / (long long)ncl);
-  rng[0] = a.u; rng[1] = a.t; rng[2] = b.u; rng[3] = b.t;
-}
-
-#define FOR_SEGMENTS(u, t0, t1, NT)                                                               \
-  for (int u = u_lo; u <= u_hi; ++u)                                                              \
-    if (u == u_hi && t_hi == 0) break;                                                            \
-    else if (const int t0 = (u == u_lo) ? t_lo : 0, t1 = (u == u_hi) ? t_hi : (NT); t0 >= t1) continue; \
-    else
-
 // ---- f0 kernel schedule ------------------------------------------------------------------------------------------
 // The flattened work sequence is ordered by (bin, detector), then by time BLOCKS of gb tiles (aligned to absolute tile
 // indices), then by template block, then by tile; cluster i takes the cost range [T i / G, T (i + 1) / G) of it, its ends
@@ -233,6 +190,58 @@ struct F0Iter {
 #define FOR_F0_SEGMENTS(it, S, A, B)                                                              \
   for (F0Iter it{A, B, (S).n_pb > 0}; !it.at_end(); f0_next_cell(S, it.cur))                                    \
     if (it.cur.t >= it.seg_end()) continue; else
+
+// ---- low-rate kernel schedule: per rate class the f0 kernel's order ((bin, detector), time block, template block, tile) ------
+// A class is a low rate: its cells are (group = the same-rate slices of a (bin, detector), template block), all with the
+// class's tile count.  The flattened sequence is class after class; cluster i takes the cost range [T i / G, T (i + 1) / G).
+// Inside a class the time block is one cluster's share of tiles, so the clusters that reconstruct the template blocks of a
+// group run side by side on the same y tiles (one reads a tile from DRAM, the others from L2) -- before, the units
+// (group, template block) followed one another whole, the 8 template blocks of a group were at different tiles at any
+// moment and y came from DRAM about 4.5 times (config 2: 267 MB of reads per launch for 75 MB of operands).
+struct LowSched {
+  const SchedBd* cells;                     // per class: one entry per group {first unit, template blocks, cost per tile, cum}
+  int n_cls;
+  int cell_begin[kNLowRates + 1];
+  int n_tiles[kNLowRates], gb[kNLowRates];
+  long long total[kNLowRates];              // sum of n_pb * w over the class's groups
+  long long base[kNLowRates + 1];           // cost before class c (total * n_tiles summed); base[n_cls] = T
+};
+
+struct LowIter {                            // yields this cluster's segments (unit, tiles [t0, t1)) in schedule order
+  const LowSched& L;
+  long long PA, PB;
+  int c;
+  F0Sched S;
+  F0Iter it;
+  bool open;
+  __device__ __forceinline__ LowIter(const LowSched& l, long long pa, long long pb) : L(l), PA(pa), PB(pb), c(-1), S{}, it{}, open(false) {}
+  __device__ __forceinline__ bool open_next_class()
+  {
+    while (++c < L.n_cls) {
+      const long long lo = max(PA, L.base[c]) - L.base[c], hi = min(PB, L.base[c + 1]) - L.base[c];
+      if (lo >= hi) continue;
+      S.bds = L.cells + L.cell_begin[c]; S.n_bds = L.cell_begin[c + 1] - L.cell_begin[c];
+      S.n_tiles = L.n_tiles[c]; S.gb = L.gb[c]; S.gt = 1; S.n_pb = 0; S.total = L.total[c]; S.a0 = 0;
+      it.cur = f0_locate(S, lo); it.end = f0_locate(S, hi); it.pb_major = false;
+      return true;
+    }
+    return false;
+  }
+  __device__ __forceinline__ bool next(int& u, int& t0, int& t1)
+  {
+    for (;;) {
+      if (!open) { if (!open_next_class()) return false; open = true; }
+      else f0_next_cell(S, it.cur);
+      while (!it.at_end() && it.cur.t >= it.seg_end()) f0_next_cell(S, it.cur);
+      if (it.at_end()) { open = false; continue; }
+      u = S.bds[it.cur.ib].bd + it.cur.pb; t0 = it.cur.t; t1 = it.seg_end();
+      return true;
+    }
+  }
+};
+#define FOR_LOW_SEGMENTS(u, t0, t1)                                                               \
+  for (LowIter li_(a.sched, PA, PB); ;)                                                           \
+    if (int u = 0, t0 = 0, t1 = 0; !li_.next(u, t0, t1)) break; else
 
 __device__ __forceinline__ void copy_pieces(uint32_t dst, const uint8_t* src, uint32_t bytes, uint32_t bar)
 {
@@ -475,7 +484,7 @@ __device__ __forceinline__ void iy_tile(YRing& rg, const YAddr ya, uint64_t mlis
 struct LowPArgs {
   const SliceParams* sp; const RateGroup* groups; const LowUnit* units;
   int r_bytes, nsy, ystage, ycap, trace;
-  SchedArgs sched;
+  LowSched sched;
 };
 
 template <bool RT>
@@ -486,14 +495,13 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   __shared__ __align__(8) PairBars bars;
   __shared__ uint32_t tmem_slot;
   __shared__ SegSrc seg[3];                             // [0] PY, [1] IY, [2] relay
-  __shared__ int s_rng[4];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const uint32_t rank = cluster_ctarank();
-  if (tid == 0) sched_range(a.sched, blockIdx.x >> 1, gridDim.x >> 1, s_rng);
-  __syncthreads();
-  const int u_lo = s_rng[0], t_lo = s_rng[1], u_hi = s_rng[2], t_hi = s_rng[3];
-  if (u_lo == u_hi && t_lo == t_hi) return;             // both CTAs of the cluster take the same decision
+  const long long T_all = a.sched.base[a.sched.n_cls];
+  const long long PA = T_all * (long long)(blockIdx.x >> 1) / (long long)(gridDim.x >> 1);
+  const long long PB = T_all * (long long)((blockIdx.x >> 1) + 1) / (long long)(gridDim.x >> 1);
+  if (PA >= PB) return;                                 // both CTAs of the cluster take the same decision
 
   const int nsy = a.nsy;
   pair_setup(bars, &tmem_slot, nsy, rank, warp, tid, 1u, 16u);          // all 8 epilogue warps of both CTAs drain every tile
@@ -510,7 +518,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0, nt = 0;
       TRACE_BEGIN();
-      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+      FOR_LOW_SEGMENTS(u, t0, t1) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[0], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank, a.ycap);
@@ -522,7 +530,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
   } else if (warp == 7) {
     if (elect_one()) {
       uint32_t seen = 0;
-      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+      FOR_LOW_SEGMENTS(u, t0, t1) {
         const SliceParams* P = a.sp + a.groups[a.units[u].group].slice[0];
         prefetch_segment(seen, progress_u, reinterpret_cast<const uint8_t*>(P->Y), (uint32_t)P->y_step64, rank, t0, t1);
       }
@@ -531,7 +539,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
     if (elect_one()) {
       YRing rg{0u, 0u, (uint32_t)nsy};
       int seg_i = 0;
-      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+      FOR_LOW_SEGMENTS(u, t0, t1) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(seg[2], a.sp, G->slice, G->n_slices, 2 * un.pb + (int)rank, a.ycap);
@@ -551,7 +559,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
       int seg_i = 0;
       uint32_t e = 0;
       TRACE_BEGIN();
-      FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+      FOR_LOW_SEGMENTS(u, t0, t1) {
         const LowUnit un = a.units[u];
         const RateGroup* G = a.groups + un.group;
         seg_fill(sg, a.sp, G->slice, G->n_slices, 2 * un.pb, a.ycap);
@@ -579,7 +587,7 @@ lowrate_pair_kernel(const __grid_constant__ LowPArgs a)
     const uint32_t acc_full_u = smem_u32(&bars.acc_full[0]);
     uint32_t e = 0;
     TRACE_BEGIN();
-    FOR_SEGMENTS(u, t0, t1, a.sched.n_tiles[sched_class(a.sched, u)]) {
+    FOR_LOW_SEGMENTS(u, t0, t1) {
       const LowUnit un = a.units[u];
       const RateGroup* Gp = a.groups + un.group;
       const int q_cap = Gp->q_groups_cap;
@@ -1269,7 +1277,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
             (int)pl->r_tmem, pl->l_sum_f0_max * 256, pl->p_bytes, pl->q_bytes, pl->f0_stages, ys_f0, pl->l_sum_low_max * 256, pl->low_stages, ys_low, pl->ycap);
   // device tables
   std::vector<LowUnit> units;                             // rate-major: all units of a rate have the same tile count
-  std::vector<SchedUnit> low_sched;
+  std::vector<SchedBd> low_cells;                         // low-rate schedule: per class one entry per group (LowSched)
   // rho^(d) buffers: ONE allocation (chunk-local: a part of a split bank takes it from the parent's shared set)
   size_t q_total = 0;
   for (int r = 0; r < pl->n_lr; ++r)
@@ -1290,17 +1298,19 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
   }
   size_t q_off = 0;
   for (int r = 0; r < pl->n_lr; ++r) {
-    pl->units_per_rate[r] = 0; pl->low_wsum[r] = 0;
+    pl->units_per_rate[r] = 0; pl->low_wsum[r] = 0; pl->low_cells_per_rate[r] = 0;
     for (int b = 0; b < n_bd; ++b) {
       RateGroup& G = pl->groups_host[(size_t)b * pl->n_lr + r];
       if (G.n_slices == 0 || pl->excluded[b]) continue;
       G.Q = (__half*)(q_base + q_off);
       q_off += (size_t)G.n_rb * 2 * G.q_groups_cap * 2048;
-      for (int rb = 0; rb < G.n_rb; ++rb) {
-        units.push_back(LowUnit{b * pl->n_lr + r, rb});
-        low_sched.push_back(SchedUnit{G.l_sum / 16, (int32_t)pl->low_wsum[r]});
-        pl->low_wsum[r] += G.l_sum / 16;
+      {
+        SchedBd e; e.bd = (int32_t)units.size(); e.n_pb = G.n_rb; e.w = G.l_sum / 16; e.pad = 0; e.cum = pl->low_wsum[r];
+        low_cells.push_back(e);
+        pl->low_wsum[r] += (long long)G.n_rb * e.w;
+        ++pl->low_cells_per_rate[r];
       }
+      for (int rb = 0; rb < G.n_rb; ++rb) units.push_back(LowUnit{b * pl->n_lr + r, rb});
       pl->units_per_rate[r] += G.n_rb;
     }
   }
@@ -1337,7 +1347,7 @@ bool f16_plan_build_recon(F16Plan* pl, const SliceParams* sp_host, int n_problem
     for (int c = 0; c < 2; ++c) memcpy(both.data() + (size_t)c * pl->p_bytes, pblob[c].data(), pblob[c].size() * sizeof(__half));
     if (!upload((void**)&pl->p_dev, both.data(), both.size())) return false;
   }
-  if (!upload((void**)&pl->low_sched_dev, low_sched.data(), low_sched.size() * sizeof(SchedUnit))) return false;
+  if (!upload((void**)&pl->low_cells_dev, low_cells.data(), low_cells.size() * sizeof(SchedBd))) return false;
   if (!upload((void**)&pl->f0_sched_dev, f0_sched.data(), f0_sched.size() * sizeof(SchedBd))) return false;
 
   // opt-in shared memory: the architecture maximum, for every kernel of this file, on this device (never lowered
@@ -1384,14 +1394,22 @@ int launch_recon_f16(F16Plan* pl, const SliceParams* sp_dev, Peak* partials, int
     memset(&la, 0, sizeof la);
     la.sp = sp_dev; la.groups = pl->groups_dev; la.units = (const LowUnit*)pl->units_dev;
     la.r_bytes = pl->l_sum_low_max * 256; la.nsy = pl->low_stages; la.ystage = pl->low_ystage; la.ycap = pl->ycap; la.trace = getenv("LLOID_TRACE") ? 1 : 0;
-    SchedArgs& sc = la.sched;
-    sc.units = pl->low_sched_dev; sc.n_cls = pl->n_lr;
+    LowSched& sc = la.sched;
+    sc.cells = pl->low_cells_dev; sc.n_cls = pl->n_lr;
     long long tiles_total = 0;
     for (int r = 0; r < pl->n_lr; ++r) {
-      sc.cls_begin[r + 1] = sc.cls_begin[r] + pl->units_per_rate[r];
+      sc.cell_begin[r + 1] = sc.cell_begin[r] + pl->low_cells_per_rate[r];
       sc.n_tiles[r] = (((c >> pl->rate[r].log2d) + 2 * kKUp) + 127) / 128;
-      sc.cls_base[r + 1] = sc.cls_base[r] + pl->low_wsum[r] * sc.n_tiles[r];
+      sc.total[r] = pl->low_wsum[r];
+      sc.base[r + 1] = sc.base[r] + pl->low_wsum[r] * sc.n_tiles[r];
       tiles_total += (long long)sc.n_tiles[r] * pl->units_per_rate[r];
+    }
+    for (int r = 0; r < pl->n_lr; ++r) {
+      // time block of class r = the tiles one cluster gets through in its share of the cost (mean cost per tile of the class)
+      const long long share = (sc.base[pl->n_lr] + n_clusters - 1) / n_clusters;
+      const long long w_mean = pl->units_per_rate[r] ? std::max<long long>(1, pl->low_wsum[r] / pl->units_per_rate[r]) : 1;
+      long long gb = getenv("LLOID_LOW_BLOCK") ? atoi(getenv("LLOID_LOW_BLOCK")) : share / w_mean;
+      sc.gb[r] = (int)std::max<long long>(1, std::min<long long>(gb, sc.n_tiles[r]));
     }
     const int grid = 2 * (int)std::min<long long>(n_clusters, tiles_total);
     if (pl->r_tmem) lowrate_pair_kernel<true><<<grid, PK_THREADS, pl->low_smem, st>>>(la);

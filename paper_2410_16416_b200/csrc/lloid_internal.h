@@ -194,22 +194,12 @@ struct PairRate {                  // one per distinct rate with d > 1 (bank-wid
   int32_t  tab_off[4];             // per variant: table entries [slot of the first chunk][item]
 };
 
-// Static schedule of a persistent tensor kernel (A7).  Work = units x time tiles; a unit is one stationary
-// operand set (f0 kernel: one (bin, detector, template block); low-rate kernel: the same per rate).  Units are
-// stored class-major (class = rate: every unit of a class has the same number of time tiles in a chunk) with a
-// cost w per tile (ring stages).  CTA i of G takes the cost range [T i / G, T (i + 1) / G) of the flattened
-// (class, unit, tile) sequence, so every SM gets the same tensor work whatever the bank geometry.
-struct SchedUnit { int32_t w, wprefix; };   // wprefix: sum of w over the earlier units of the same class
-struct SchedArgs {
-  const SchedUnit* units;
-  int32_t   n_cls;
-  int32_t   cls_begin[kNLowRates + 1];      // unit index range of class c: [cls_begin[c], cls_begin[c + 1])
-  int32_t   n_tiles[kNLowRates];            // time tiles per unit of class c for this chunk
-  long long cls_base[kNLowRates + 1];       // cost before class c; cls_base[n_cls] = total
-};   // one 16-row chunk of an interpolation: MMA N, P offset, D column
-
-struct SchedBd {                   // f0 kernel schedule: one tensor-path (bin, detector)
-  int32_t bd, n_pb, w, pad;        // index, template blocks of 128, cost per tile (MMAs)
+// Static schedules of the persistent reconstruction kernels (A7): F0Sched and LowSched in kernels_f16_recon.cu.  Work =
+// cells x time tiles; a cell is one stationary operand set ((bin, detector), template block -- per rate in the low-rate
+// kernel); cluster i of G takes the cost range [T i / G, T (i + 1) / G) of the flattened sequence, so every SM pair
+// gets the same tensor work whatever the bank geometry.
+struct SchedBd {                   // one tensor-path (bin, detector) (f0 kernel) / one of its rate groups (low-rate kernel)
+  int32_t bd, n_pb, w, pad;        // index (low-rate kernel: first unit), template blocks of 128, cost per tile (MMAs)
   long long cum;                   // sum of n_pb * w over the earlier entries
 };
 
