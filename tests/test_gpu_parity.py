@@ -262,3 +262,31 @@ def test_fp16_bank_outside_the_tensor_limits_runs_the_cuda_core_reconstruction()
     _, _, _, info, stats = _dense_check(w, lb.LLOID_F16, 6144, n)
     assert info["path"]["cuda_core_bds"] == 1, info["path"]
     assert stats["checked"] == 150 * ((n - 6144) // 512)
+
+
+@pytest.mark.parametrize("precision", PRECISIONS)
+def test_non_finite_strain_silences_one_detector_for_one_history_length(precision):
+    """include/lloid.h: the strain must be finite and is not checked.  What a NaN does is stated there and pinned here: every
+    SNR value whose filter span covers it is NaN, a NaN never wins the peak comparison, so that detector emits nothing
+    until the sample has left the carried history; the other detector is untouched and the first one recovers."""
+    import copy
+    w = wl.config3(n_bins=2, n_templates=24, seconds=40, n_detectors=2, n_basis=16)
+    w.threshold = 3.0
+    clean, _, _ = pu.run_gpu(w, precision)
+    bad = copy.copy(w)
+    bad.strain = w.strain.copy()
+    k_nan = 20 * 2048 + 77
+    bad.strain[0, k_nan] = np.nan
+    got, _, info = pu.run_gpu(bad, precision)
+    assert info["consumed"] == w.n_samples
+    assert np.isfinite(got["snr_re"]).all() and np.isfinite(got["snr_im"]).all()          # no NaN ever reaches a trigger
+    M = max(b.template_len for b in w.bins)
+    key = lambda t: sorted((int(x["bin"]), int(x["template_idx"]), int(x["sample"])) for x in t)   # noqa: E731
+    assert key(got[got["detector"] == 1]) == key(clean[clean["detector"] == 1])           # the other detector: identical
+    d0, c0 = got[got["detector"] == 0], clean[clean["detector"] == 0]
+    before = lambda t: t[t["sample"] < (k_nan // 2048) * 2048]                            # noqa: E731
+    after = lambda t: t[t["sample"] >= ((k_nan + M + 4096) // 2048 + 1) * 2048]           # noqa: E731
+    assert key(before(d0)) == key(before(c0)) and len(before(c0)) > 0
+    assert key(after(d0)) == key(after(c0)) and len(after(c0)) > 0                        # recovered
+    dead = d0[(d0["sample"] > k_nan + 64) & (d0["sample"] < k_nan + min(b.template_len for b in w.bins) - 64)]
+    assert len(dead) == 0                                                                # silent while every template covers the NaN
